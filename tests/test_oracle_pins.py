@@ -1,0 +1,255 @@
+"""Pins for the FP64 attention oracle (oracle/pkv_oracle.c): nothing here comes from the CUDA path.
+
+P1 brute-force dense numpy (Eq. 1)          P4 split-count invariance
+P2 page-pool permutation invariance  P5 dominant key at every boundary
+P3 K = 0  =>  O = mean(V), exact with integer V         P6 N = 1, N = 2, equal-keys closed forms
+"""
+import math
+
+import numpy as np
+import pytest
+
+from helpers import (Problem, default_scale, dense_attention_bruteforce, make_problem, permute_pool,
+                     token_location)
+from oracle import pkv_oracle, workqueue_oracle as wq
+from pkv_inputs import PAD_PAGE
+
+
+def oracle_attention(p: Problem, **kw):
+    return pkv_oracle.attention(p.q, p.k_cache, p.v_cache, p.block_table, p.seq_lens, Hkv=p.Hkv,
+                                page_size=p.page_size, scale=p.scale, **kw)
+
+
+def test_half_decoder_all_bit_patterns():
+    """The oracle's own FP16 decoder against numpy's float16 on all 65536 patterns."""
+    bits = np.arange(65536, dtype=np.uint16)
+    ref = bits.view(np.float16).astype(np.float64)
+    for b in range(65536):
+        got = pkv_oracle.half_to_double(b)
+        if math.isnan(ref[b]):
+            assert math.isnan(got)
+        else:
+            assert got == ref[b] and math.copysign(1.0, got) == math.copysign(1.0, ref[b]), b
+
+
+@pytest.mark.parametrize("Hkv", [8, 4])
+@pytest.mark.parametrize("lens", [[1], [2], [15, 16, 17], [31, 32, 33], [100, 1, 40]])
+def test_p1_bruteforce_dense(lens, Hkv):
+    p = make_problem(lens, seed=11 + len(lens) + Hkv, Hkv=Hkv)
+    out, lse = oracle_attention(p)
+    ref, ref_lse = dense_attention_bruteforce(p)
+    assert np.abs(out - ref).max() <= 1e-12
+    assert np.abs(lse - ref_lse).max() <= 1e-12
+
+
+def test_p1_bruteforce_other_shapes():
+    """A transposed operand or a wrong head map shows up when Hq, Hkv, d and P all differ."""
+    p = make_problem([37, 5], seed=5, Hq=6, Hkv=3, d=24, page_size=4)
+    out, lse = oracle_attention(p)
+    ref, ref_lse = dense_attention_bruteforce(p)
+    assert np.abs(out - ref).max() <= 1e-12
+    assert np.abs(lse - ref_lse).max() <= 1e-12
+
+
+def test_p2_page_pool_permutation_invariance_bit_identical():
+    p = make_problem([100, 33, 16], seed=21)
+    out, lse = oracle_attention(p)
+    p2 = permute_pool(p, seed=99)
+    assert not np.array_equal(p.block_table, p2.block_table)
+    out2, lse2 = oracle_attention(p2)
+    assert np.array_equal(out, out2) and np.array_equal(lse, lse2)
+
+
+def test_strided_layout_reading_a1():
+    """The paper's [page, Hkv, page_size, d] layout through explicit strides gives the
+    same bits as the BASELINE.json layout [page, page_size, Hkv, d]."""
+    p = make_problem([70, 19], seed=31)
+    out, lse = oracle_attention(p)
+    k_hnd = np.ascontiguousarray(p.k_cache.transpose(0, 2, 1, 3))
+    v_hnd = np.ascontiguousarray(p.v_cache.transpose(0, 2, 1, 3))
+    P, H, d = p.page_size, p.Hkv, p.d
+    out2, lse2 = pkv_oracle.attention(p.q, k_hnd, v_hnd, p.block_table, p.seq_lens, Hkv=H, page_size=P,
+                                      scale=p.scale, strides=(H * P * d, d, P * d))
+    assert np.array_equal(out, out2) and np.array_equal(lse, lse2)
+
+
+def test_p3_zero_keys_give_mean_of_values_exactly():
+    p = make_problem([100, 47], seed=41)
+    rng = np.random.Generator(np.random.PCG64(7))
+    p.k_cache[...] = 0
+    p.v_cache[...] = rng.integers(-8, 9, size=p.v_cache.shape).astype(np.float16)
+    out, lse = oracle_attention(p)
+    for i in range(p.B):
+        N = int(p.seq_lens[i])
+        for g in range(p.Hkv):
+            acc = np.zeros(p.d)
+            for j in range(N):
+                page, r = token_location(p, i, j)
+                acc += p.v_cache[page, r, g].astype(np.float64)
+            mean = acc / N                      # small integers: the sum is exact
+            for hh in range(p.G):
+                assert np.abs(out[i, g * p.G + hh] - mean).max() <= 1e-15
+                assert abs(lse[i, g * p.G + hh] - math.log(N)) <= 1e-14
+
+
+def test_a10_tail_and_unused_entries_never_read():
+    """Tokens >= N_i in the last page hold huge values and NaN, the unused block-table entries
+    hold PAD_PAGE; the result must not move (reading A10)."""
+    p = make_problem([37, 50], seed=51, reserve_extra=40)
+    out, lse = oracle_attention(p)
+    k2, v2 = p.k_cache.copy(), p.v_cache.copy()
+    owned = set()
+    for i in range(p.B):
+        for j in range(int(p.seq_lens[i])):
+            owned.add(token_location(p, i, j))
+    for page in range(k2.shape[0]):
+        for r in range(p.page_size):
+            if (page, r) not in owned:
+                k2[page, r] = np.float16(60000.0)
+                v2[page, r] = np.float16(np.nan)
+    t2 = p.block_table.copy()
+    for i in range(p.B):
+        t2[i, math.ceil(int(p.seq_lens[i]) / p.page_size):] = PAD_PAGE
+    out2, lse2 = pkv_oracle.attention(p.q, k2, v2, t2, p.seq_lens, Hkv=p.Hkv, page_size=p.page_size,
+                                      scale=p.scale)
+    assert np.array_equal(out, out2) and np.array_equal(lse, lse2)
+
+
+@pytest.mark.parametrize("S", [1, 2, 3, 4, 16, 64, 200])
+def test_p4_split_count_invariance(S):
+    """Split states merged by PAPER.md:60-61 equal Eq. (1) for any split count,
+    including S > T where trailing splits are empty."""
+    p = make_problem([1000, 95, 32, 1], seed=61)
+    ref, ref_lse = oracle_attention(p)
+    pol = wq.Policy(tile_tokens=32, num_splits=S)
+    q = wq.build_workqueue(p.seq_lens, p.Hkv, pol)
+    out, lse = pkv_oracle.attention_via_splits(p.q, p.k_cache, p.v_cache, p.block_table, p.seq_lens,
+                                               np.array(q.tasks, dtype=np.int32), q.split_offsets,
+                                               Hkv=p.Hkv, page_size=p.page_size, tile_tokens=32,
+                                               scale=p.scale)
+    assert np.abs(out - ref).max() <= 1e-12
+    assert np.abs(lse - ref_lse).max() <= 1e-12
+
+
+def test_p4_rect_route_neutral_states():
+    """Rectangular grid: empty splits carry (m, l, a) = (-inf, 0, 0) and drop out."""
+    p = make_problem([40, 700, 0], seed=62)
+    ref, ref_lse = oracle_attention(p)
+    pol = wq.Policy(tile_tokens=32, num_splits=8, route=wq.ROUTE_RECT)
+    q = wq.build_workqueue(p.seq_lens, p.Hkv, pol)
+    tasks = np.array(q.tasks, dtype=np.int32)
+    m, l, a = pkv_oracle.split_states(p.q, p.k_cache, p.v_cache, p.block_table, p.seq_lens, tasks,
+                                      Hkv=p.Hkv, page_size=p.page_size, tile_tokens=32, scale=p.scale)
+    empty = tasks[:, 3] >= tasks[:, 4]
+    assert empty.sum() == q.empty_ctas > 0
+    assert np.all(np.isneginf(m[empty])) and np.all(l[empty] == 0) and np.all(a[empty] == 0)
+    out, lse = pkv_oracle.attention_via_splits(p.q, p.k_cache, p.v_cache, p.block_table, p.seq_lens,
+                                               tasks, q.split_offsets, Hkv=p.Hkv,
+                                               page_size=p.page_size, tile_tokens=32, scale=p.scale)
+    assert np.abs(out - ref).max() <= 1e-12
+    assert np.all(out[2] == 0) and np.all(np.isneginf(lse[2]))          # reading A9
+
+
+def test_merge_associative_and_neutral():
+    rng = np.random.Generator(np.random.PCG64(3))
+    n, d = 7, 16
+    m = rng.standard_normal(n) * 5
+    l = rng.random(n) + 0.5
+    a = rng.standard_normal((n, d))
+    o_all, lse_all = pkv_oracle.merge(m, l, a)
+    # closed form of the definition: O = sum_s e^{m_s} a_s / sum_s e^{m_s} l_s
+    w = np.exp(m - m.max())
+    assert np.abs(o_all - (w[:, None] * a).sum(0) / (w * l).sum()).max() <= 1e-13
+    assert abs(lse_all - (m.max() + math.log((w * l).sum()))) <= 1e-13
+    # adding neutral states changes nothing
+    m2 = np.concatenate([m, [-np.inf, -np.inf]])
+    l2 = np.concatenate([l, [0.0, 0.0]])
+    a2 = np.concatenate([a, np.zeros((2, d))])
+    o2, lse2 = pkv_oracle.merge(m2, l2, a2)
+    assert np.array_equal(o2, o_all) and lse2 == lse_all
+    # all neutral -> O = 0, LSE = -inf (reading A9)
+    o3, lse3 = pkv_oracle.merge(np.full(3, -np.inf), np.zeros(3), np.zeros((3, d)))
+    assert np.all(o3 == 0) and lse3 == -np.inf
+
+
+def _dominant_positions(N, page_size, tile, splits):
+    pos = {0, N - 1}
+    for unit in (page_size, tile):
+        for b in range(unit, N, unit):
+            pos.update({b - 1, b, b + 1})
+    T = math.ceil(N / tile)
+    c = math.ceil(T / splits)
+    for s in range(1, splits):
+        b = s * c * tile
+        pos.update({b - 1, b, b + 1})
+    return sorted(x for x in pos if 0 <= x < N)
+
+
+def test_p5_dominant_key_selects_that_value():
+    """k_{j*} = 3 q for all G heads sharing one q  =>  x* >> the rest  =>  O = v_{j*}."""
+    N = 200
+    base = make_problem([N], seed=71)
+    for hh in range(1, base.G):                 # one q per KV group so a single key dominates all G heads
+        base.q[0, hh::base.G] = base.q[0, 0::base.G]
+    positions = _dominant_positions(N, base.page_size, 32, 4)
+    assert len(positions) > 30
+    for jstar in positions:
+        k2 = base.k_cache.copy()
+        page, r = token_location(base, 0, jstar)
+        for g in range(base.Hkv):
+            k2[page, r, g] = (3.0 * base.q[0, g * base.G].astype(np.float32)).astype(np.float16)
+        out, _ = pkv_oracle.attention(base.q, k2, base.v_cache, base.block_table, base.seq_lens,
+                                      Hkv=base.Hkv, page_size=base.page_size, scale=base.scale)
+        for h in range(base.Hq):
+            want = base.v_cache[page, r, h // base.G].astype(np.float64)
+            assert np.abs(out[0, h] - want).max() < 1e-6, (jstar, h)
+
+
+def test_p6_closed_forms_n1_n2_equal_keys():
+    # N = 1: O = v_0 exactly, LSE = x_0
+    p = make_problem([1], seed=81)
+    out, lse = oracle_attention(p)
+    page, r = token_location(p, 0, 0)
+    for h in range(p.Hq):
+        g = h // p.G
+        assert np.array_equal(out[0, h], p.v_cache[page, r, g].astype(np.float64))
+        x0 = p.scale * float(p.q[0, h].astype(np.float64) @ p.k_cache[page, r, g].astype(np.float64))
+        assert abs(lse[0, h] - x0) <= 1e-13
+    # N = 2: O = sigma(x0 - x1) v0 + sigma(x1 - x0) v1
+    p = make_problem([2], seed=82)
+    out, _ = oracle_attention(p)
+    (p0, r0), (p1, r1) = token_location(p, 0, 0), token_location(p, 0, 1)
+    for h in range(p.Hq):
+        g = h // p.G
+        qv = p.q[0, h].astype(np.float64)
+        x0 = p.scale * float(qv @ p.k_cache[p0, r0, g].astype(np.float64))
+        x1 = p.scale * float(qv @ p.k_cache[p1, r1, g].astype(np.float64))
+        s0 = 1.0 / (1.0 + math.exp(x1 - x0))
+        want = s0 * p.v_cache[p0, r0, g].astype(np.float64) + (1 - s0) * p.v_cache[p1, r1, g].astype(np.float64)
+        assert np.abs(out[0, h] - want).max() <= 1e-13
+    # all keys equal: uniform weights, O = mean(V) (V integer => exact sum)
+    p = make_problem([53], seed=83)
+    rng = np.random.Generator(np.random.PCG64(1))
+    p.k_cache[...] = p.k_cache[0, 0, 0][None, None, None, :]
+    p.v_cache[...] = rng.integers(-4, 5, size=p.v_cache.shape).astype(np.float16)
+    out, _ = oracle_attention(p)
+    for g in range(p.Hkv):
+        acc = np.zeros(p.d)
+        for j in range(53):
+            page, r = token_location(p, 0, j)
+            acc += p.v_cache[page, r, g].astype(np.float64)
+        for hh in range(p.G):
+            assert np.abs(out[0, g * p.G + hh] - acc / 53).max() <= 1e-13
+
+
+def test_scale_is_applied_to_scores():
+    """Doubling the scale is the same as doubling q (exact in FP16: power of two)."""
+    p = make_problem([60], seed=91)
+    p.q[...] = (p.q.astype(np.float32) * 0.25).astype(np.float16)
+    out_a, lse_a = pkv_oracle.attention(p.q, p.k_cache, p.v_cache, p.block_table, p.seq_lens, Hkv=p.Hkv,
+                                        page_size=p.page_size, scale=2.0 * p.scale)
+    q2 = (p.q.astype(np.float32) * 2).astype(np.float16)
+    out_b, lse_b = pkv_oracle.attention(q2, p.k_cache, p.v_cache, p.block_table, p.seq_lens, Hkv=p.Hkv,
+                                        page_size=p.page_size, scale=p.scale)
+    assert np.abs(out_a - out_b).max() <= 1e-13 and np.abs(lse_a - lse_b).max() <= 1e-12
+    assert default_scale(128) == float(np.float32(1 / math.sqrt(128)))
