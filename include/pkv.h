@@ -1,0 +1,213 @@
+/*
+ * pkv.h -- C ABI of libpkv: paged GQA decode attention for B200 (sm_100a).
+ *
+ * The hot path of arxiv/paper_2606_26666 ("PersistentKV"): single-query grouped-query decode
+ * attention that reads FP16 K/V through a native paged block table (sec. 3.2),
+ * splits each row's sequence into split-local online-softmax states (sec. 3.3),
+ * merges them exactly and launches only the non-empty (row, KV head, split)
+ * tasks of a ragged batch through a compact workqueue (sec. 3.4).
+ *
+ * Conventions
+ *   - plain C, no torch / C++ types.  "dev" pointers are CUDA device pointers, "host" pointers
+ *     are ordinary host memory.  `stream` is a cudaStream_t passed as void* (NULL = legacy
+ *     default stream).
+ *   - the CALLER OWNS EVERY BUFFER (q, caches, tables, out, workspace).  pkv_build_workqueue,
+ *     pkv_decode and pkv_merge never allocate, never synchronise and never read device data
+ *     on the host, so all three may be captured into a CUDA graph.
+ *   - every call returns a pkv_status; nothing throws or aborts.  pkv_last_error() gives a
+ *     thread-local description of the last non-OK status.
+ *   - host-checkable arguments are rejected before any launch.  Device-resident values
+ *     (seq_lens[i] > max_pages*page_size, a page id >= num_pages) cannot be checked without a
+ *     synchronisation: they are undefined behaviour.  seq_lens[i] == 0 is legal: the row
+ *     emits no task, out[i] = 0 and lse[i] = -inf (reading A9).
+ *   - compiled-in shapes: d = 128, page_size = 16, FP16, G = Hq/Hkv in {4, 8}.  Anything else
+ *     returns PKV_ERR_UNSUPPORTED.
+ */
+#ifndef PKV_H_
+#define PKV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(_WIN32)
+#define PKV_API
+#else
+#define PKV_API __attribute__((visibility("default")))
+#endif
+
+typedef enum {
+    PKV_OK = 0,
+    PKV_ERR_INVALID_ARG = 1,  /* null pointer, negative size, Hq % Hkv, misaligned pointer/stride */
+    PKV_ERR_UNSUPPORTED = 2,  /* shape / G / arch not compiled in                                */
+    PKV_ERR_WORKSPACE = 3,    /* caller workspace smaller than pkv_workspace_bytes()             */
+    PKV_ERR_CUDA = 4          /* CUDA runtime / driver error; see pkv_last_error()               */
+} pkv_status;
+
+typedef enum { PKV_ROUTE_RECT = 0, PKV_ROUTE_WORKQUEUE = 1 } pkv_route;
+typedef enum { PKV_MERGE_SEPARATE = 0, PKV_MERGE_FUSED = 1 } pkv_merge_mode;
+typedef enum { PKV_SPLIT_FIXED_COUNT = 0, PKV_SPLIT_FIXED_CHUNK = 1 } pkv_split_mode;
+/* which decode kernel runs the tile loop */
+typedef enum {
+    PKV_KERNEL_AUTO = 0, /* = PKV_KERNEL_TMA_MMA                                                 */
+    PKV_KERNEL_TMA_MMA = 1, /* TMA page loads -> mbarrier ring -> ldmatrix + HMMA, warp-specialised */
+    PKV_KERNEL_SIMT = 2  /* 16-byte vector loads straight from global, FP32 FFMA + warp shuffles */
+} pkv_kernel;
+
+/*
+ * Split policy (PAPER.md:63-67 row-local bounds; PAPER.md:89 split policy).  All bounds are in
+ * tiles of `tile_tokens` tokens, counted from the row's true length N_i = seq_lens[i]:
+ *   T_i = ceil(N_i / tile_tokens)
+ *   FIXED_COUNT: S_i = S                          (S = num_splits, or the auto rule when 0)
+ *   FIXED_CHUNK: S_i = min(S, ceil(T_i / chunk_tiles))   (S = num_splits, or 256 when 0)
+ *   c_i = ceil(T_i / S_i), n_i = ceil(T_i / c_i); split s of row i covers tiles
+ *   [s*c_i, min((s+1)*c_i, T_i)), s = 0 .. n_i-1                      (reading A6)
+ * Auto rule (A12): S = clamp(ceil(4*num_sms / (B*Hkv)), 1, 256).
+ */
+typedef struct {
+    int32_t tile_tokens; /* > 0, multiple of page_size; the paper uses 32          */
+    int32_t split_mode;  /* pkv_split_mode                                                       */
+    int32_t num_splits;  /* >= 0, <= 256; see above                                              */
+    int32_t chunk_tiles; /* FIXED_CHUNK: tiles per task (> 0)                                    */
+    int32_t route;       /* pkv_route                                                            */
+    int32_t merge_mode;  /* pkv_merge_mode                                                       */
+    int32_t num_sms;     /* SM count for the auto rule; 0 = the current device's (device calls
+                            only; the host builder needs it > 0 when num_splits == 0)            */
+    int32_t kernel;      /* pkv_kernel                                                           */
+} pkv_split_policy;
+
+/* One workqueue entry: tile interval [t_begin, t_end) of row `row`, KV head `kvh`;
+ * token range = [t_begin*tile_tokens, min(t_end*tile_tokens, N_row)). */
+typedef struct { int32_t row, kvh, split, t_begin, t_end; } pkv_task;
+
+/*
+ * Problem shape.  Caches are FP16 buffers addressed as
+ *   elem(page, token, head, c) = page*kv_stride_page + token*kv_stride_token + head*kv_stride_head + c
+ * (strides in elements, c is unit-stride).  All three strides 0 = the default layout
+ * [num_pages, page_size, Hkv, d] (BASELINE.json north_star; reading A1); the paper's
+ * [num_pages, Hkv, page_size, d] is kv_stride_head = page_size*d,
+ * kv_stride_token = d.  Strides must be multiples of 8 elements (16 bytes).
+ */
+typedef struct {
+    int32_t B, Hq, Hkv, d, page_size, max_pages; /* block_table is [B, max_pages] int32          */
+    int64_t num_pages;
+    int64_t kv_stride_page, kv_stride_token, kv_stride_head;
+} pkv_shape;
+
+/* Scheduler-derived counters with the definitions of Table 4 (A13,
+ * A14).  Filled by pkv_get_counters from the workqueue state of the last build / decode. */
+typedef struct {
+    int64_t tasks;           /* non-empty tasks (workqueue) or B*Hkv*S grid cells (rect)         */
+    int64_t empty_tasks;     /* rect route only: grid cells with an empty tile interval          */
+    int64_t decode_launches; /* 1, or 0 when there is no task                                    */
+    int64_t merge_launches;  /* 1 if a separate merge kernel is needed, else 0                   */
+    int64_t build_launches;  /* device builder kernel launches (the paper builds on the host)    */
+    int64_t useful_kv_bytes; /* sum_i N_i * 2*Hkv*d*2                                            */
+    int64_t merge_bytes;     /* partial slots * G * (d+2) * 4 (one pass)                         */
+    int64_t num_splits;      /* resolved S                                                       */
+    int64_t max_row_splits;  /* max_i n_i                                                        */
+    int64_t h2d_bytes;       /* pkv_decode_host only: bytes copied host->device this step        */
+    int64_t d2h_bytes;       /* pkv_decode_host only: bytes copied device->host this step        */
+} pkv_counters;
+
+/* Library/ABI version: (major << 16) | minor. */
+PKV_API int32_t pkv_version(void);
+/* Thread-local text of the last error on this thread ("" if none).  Never NULL. */
+PKV_API const char* pkv_last_error(void);
+
+/* Bytes of device workspace pkv_build_workqueue / pkv_decode need for this shape and policy.
+ * Pure function (no CUDA call).  Returns 0 on invalid arguments.  With num_splits == 0 and
+ * num_sms == 0 the bound for S = 256 is returned. */
+PKV_API size_t pkv_workspace_bytes(const pkv_shape* shape, const pkv_split_policy* policy);
+
+/* Split-bound policy + compact workqueue on the HOST.  Pure CPU, no CUDA.
+ * seq_lens_host [B].  Writes at most tasks_cap tasks in canonical order (row, kvh, split --
+ * DESIGN.md A7), split_offsets_out [B+1] = exclusive prefix sum of n_i (workqueue route) or of
+ * S (rect route), *num_tasks_out.  PKV_ERR_WORKSPACE if tasks_cap is too small (then
+ * *num_tasks_out holds the needed count).  tasks_out may be NULL with tasks_cap == 0 to count. */
+PKV_API pkv_status pkv_build_workqueue_host(const pkv_shape* shape, const pkv_split_policy* policy,
+                                            const int32_t* seq_lens_host, pkv_task* tasks_out,
+                                            int32_t tasks_cap, int32_t* split_offsets_out,
+                                            int32_t* num_tasks_out);
+
+/* The same, by one kernel on the DEVICE into the (private) workspace; seq_lens_dev [B] is read
+ * by the kernel only.  Marks the workspace's queue as built for the next pkv_decode. */
+PKV_API pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_policy* policy,
+                                       const int32_t* seq_lens_dev, void* workspace,
+                                       size_t workspace_bytes, void* stream);
+
+/*
+ * One decode step (Eq. 1 through the block table, split per `policy`).
+ *   q           dev [B, Hq, d] f16          k_cache, v_cache  dev, see pkv_shape
+ *   block_table dev [B, max_pages] i32      seq_lens          dev [B] i32
+ *   out         dev [B, Hq, d] f16          lse               dev [B, Hq] f32 or NULL
+ *   scale       <= 0 means 1/sqrt(d)        (natural-log LSE of the scaled scores)
+ * build_queue != 0: runs the device builder first (as pkv_build_workqueue); 0: uses the queue
+ * already in `workspace` (built for the same shape/policy and the same seq_lens values).
+ * Launches: [builder] + decode + [merge]; the merge launch is skipped when the policy cannot
+ * produce more than one split per row, or merge_mode is FUSED.
+ */
+PKV_API pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                              const void* k_cache, const void* v_cache, const int32_t* block_table,
+                              const int32_t* seq_lens, void* out, float* lse, float scale,
+                              int32_t build_queue, void* workspace, size_t workspace_bytes,
+                              void* stream);
+
+/*
+ * Exact merge of split states (segmented over each row's compact slot range,
+ * PAPER.md:75).  Public partial-state format, all FP32, natural-log domain:
+ *   part_m [slots, G], part_l [slots, G], part_acc [slots, G, d],
+ *   slot(i, g, s) = split_offsets[i]*Hkv + g*n_i + s,  n_i = split_offsets[i+1]-split_offsets[i]
+ * Neutral states (m = -inf, l = 0) drop out; a row with no state or only neutral states gives
+ * out = 0, lse = -inf.  split_offsets is dev [B+1].
+ */
+PKV_API pkv_status pkv_merge(const pkv_shape* shape, const float* part_m, const float* part_l,
+                             const float* part_acc, const int32_t* split_offsets, void* out,
+                             float* lse, void* stream);
+
+/* Host copies of the workspace's counters / queue.  These two SYNCHRONISE `stream`. */
+PKV_API pkv_status pkv_get_counters(const pkv_shape* shape, const pkv_split_policy* policy,
+                                    const void* workspace, size_t workspace_bytes,
+                                    pkv_counters* host_out, void* stream);
+PKV_API pkv_status pkv_read_workqueue(const pkv_shape* shape, const pkv_split_policy* policy,
+                                      const void* workspace, size_t workspace_bytes,
+                                      pkv_task* host_tasks, int32_t cap, int32_t* host_split_offsets,
+                                      int32_t* host_num_tasks, void* stream);
+/* Test hook: device pointers of the partial states inside the workspace (no sync). */
+PKV_API pkv_status pkv_workspace_partials(const pkv_shape* shape, const pkv_split_policy* policy,
+                                          void* workspace, size_t workspace_bytes, float** part_m,
+                                          float** part_l, float** part_acc, int64_t* slots_cap);
+
+/*
+ * One decode step with HOST buffers (the serving-facing path of PAPER.md:122-126: per-step
+ * metadata is planned on the host and uploaded; bench.py's e2e leg).  The K/V page pool is the
+ * model's resident state and stays on the device; q, block_table and seq_lens come from the
+ * host, out goes back to the host.  The call
+ *   1. plans the workqueue on the host from seq_lens_host (as pkv_build_workqueue_host),
+ *   2. packs header, split_offsets, seq_lens, q, block_table and the task list into
+ *      `host_staging` and copies that image to `dev_scratch` with ONE cudaMemcpyAsync,
+ *   3. launches decode (+ merge) -- skipping launches the plan shows to be empty, so
+ *      decode/merge launch counts equal the oracle's (A13) -- and
+ *   4. copies out to out_host and SYNCHRONISES the stream.
+ * host_staging: host memory of pkv_host_scratch_bytes() bytes (pinned recommended);
+ * dev_scratch: device memory of the same size, 256-byte aligned.  counters_out may be NULL.
+ */
+PKV_API size_t pkv_host_scratch_bytes(const pkv_shape* shape, const pkv_split_policy* policy);
+PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* policy,
+                                   const void* q_host, const void* k_cache_dev, const void* v_cache_dev,
+                                   const int32_t* block_table_host, const int32_t* seq_lens_host,
+                                   void* out_host, float scale, void* host_staging, void* dev_scratch,
+                                   size_t scratch_bytes, void* workspace, size_t workspace_bytes,
+                                   void* stream, pkv_counters* counters_out);
+
+/* Test hook: tensor-map form used by the TMA kernel for maps encoded after the call.
+ * -1 = automatic (rank-5 box, falling back to two rank-4 boxes), 0 = rank 5, 1 = rank 4. */
+PKV_API void pkv_debug_force_tma_mode(int mode);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PKV_H_ */

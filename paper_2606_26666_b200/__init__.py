@@ -1,0 +1,23 @@
+"""paper_2606_26666_b200 -- B200-native paged GQA decode attention (PersistentKV hot path).
+
+The product is ``libpkv.so`` (hand-written CUDA for sm_100a behind the C ABI of
+``include/pkv.h``); this package is its thin ctypes binding.  PyTorch is used by callers only
+for device memory, streams and CUDA graphs.  Importing the package loads (building if needed)
+the shared library and raises if that fails -- there is no CPU or PyTorch fallback.
+"""
+from .binding import (  # noqa: F401
+    PKV_OK, PKV_ERR_INVALID_ARG, PKV_ERR_UNSUPPORTED, PKV_ERR_WORKSPACE, PKV_ERR_CUDA,
+    ROUTE_RECT, ROUTE_WORKQUEUE, MERGE_SEPARATE, MERGE_FUSED, SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK,
+    KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT, EXPORTS,
+    PkvError, Shape, Policy,
+    pkv_version, pkv_last_error, pkv_workspace_bytes, pkv_host_scratch_bytes, pkv_build_workqueue_host,
+    pkv_build_workqueue, pkv_decode, pkv_merge, pkv_get_counters, pkv_read_workqueue, pkv_workspace_partials,
+    pkv_decode_host, pkv_debug_force_tma_mode,
+)
+
+
+def alloc_workspace(shape, policy, device="cuda"):
+    """A torch uint8 buffer of pkv_workspace_bytes(shape, policy) on ``device`` (plumbing only)."""
+    import torch
+
+    return torch.empty(pkv_workspace_bytes(shape, policy), dtype=torch.uint8, device=device)

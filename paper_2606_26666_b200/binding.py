@@ -1,0 +1,269 @@
+"""ctypes binding of libpkv.so -- argument marshalling only.
+
+Every function here has the name and the argument order of its C entry point in
+``include/pkv.h``; tensors are passed as raw device (or host) pointers taken from
+``torch.Tensor.data_ptr()`` / numpy arrays.  No step of the decode path runs in Python or in
+PyTorch ops: PyTorch only owns the memory and the stream.  There is no CPU fallback: if
+``libpkv.so`` cannot be loaded (or built), importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional, Tuple
+
+import numpy as np
+
+from . import build as _build
+
+PKV_OK, PKV_ERR_INVALID_ARG, PKV_ERR_UNSUPPORTED, PKV_ERR_WORKSPACE, PKV_ERR_CUDA = range(5)
+ROUTE_RECT, ROUTE_WORKQUEUE = 0, 1
+MERGE_SEPARATE, MERGE_FUSED = 0, 1
+SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK = 0, 1
+KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
+
+_i32, _i64 = ctypes.c_int32, ctypes.c_int64
+_vp = ctypes.c_void_p
+
+
+class pkv_split_policy(ctypes.Structure):
+    _fields_ = [("tile_tokens", _i32), ("split_mode", _i32), ("num_splits", _i32), ("chunk_tiles", _i32),
+                ("route", _i32), ("merge_mode", _i32), ("num_sms", _i32), ("kernel", _i32)]
+
+
+class pkv_task(ctypes.Structure):
+    _fields_ = [("row", _i32), ("kvh", _i32), ("split", _i32), ("t_begin", _i32), ("t_end", _i32)]
+
+
+class pkv_shape(ctypes.Structure):
+    _fields_ = [("B", _i32), ("Hq", _i32), ("Hkv", _i32), ("d", _i32), ("page_size", _i32), ("max_pages", _i32),
+                ("num_pages", _i64), ("kv_stride_page", _i64), ("kv_stride_token", _i64), ("kv_stride_head", _i64)]
+
+
+class pkv_counters(ctypes.Structure):
+    _fields_ = [(n, _i64) for n in ("tasks", "empty_tasks", "decode_launches", "merge_launches", "build_launches",
+                                    "useful_kv_bytes", "merge_bytes", "num_splits", "max_row_splits", "h2d_bytes",
+                                    "d2h_bytes")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+# every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
+EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_build_workqueue_host",
+           "pkv_build_workqueue", "pkv_decode", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
+           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_tma_mode")
+
+
+class PkvError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__("pkv status %d: %s" % (status, message))
+        self.status = status
+
+
+def _load() -> ctypes.CDLL:
+    path = _build.LIB
+    if not os.path.exists(path) or os.path.getmtime(path) < _build._deps_mtime():
+        _build.build()           # raises if nvcc is missing: no fallback
+    lib = ctypes.CDLL(path)
+    P = ctypes.POINTER
+    lib.pkv_version.restype = _i32
+    lib.pkv_last_error.restype = ctypes.c_char_p
+    lib.pkv_workspace_bytes.restype = ctypes.c_size_t
+    lib.pkv_workspace_bytes.argtypes = [P(pkv_shape), P(pkv_split_policy)]
+    lib.pkv_host_scratch_bytes.restype = ctypes.c_size_t
+    lib.pkv_host_scratch_bytes.argtypes = [P(pkv_shape), P(pkv_split_policy)]
+    lib.pkv_build_workqueue_host.restype = _i32
+    lib.pkv_build_workqueue_host.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _i32, _vp, P(_i32)]
+    lib.pkv_build_workqueue.restype = _i32
+    lib.pkv_build_workqueue.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, ctypes.c_size_t, _vp]
+    lib.pkv_decode.restype = _i32
+    lib.pkv_decode.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float,
+                               _i32, _vp, ctypes.c_size_t, _vp]
+    lib.pkv_merge.restype = _i32
+    lib.pkv_merge.argtypes = [P(pkv_shape), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.pkv_get_counters.restype = _i32
+    lib.pkv_get_counters.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, ctypes.c_size_t, P(pkv_counters), _vp]
+    lib.pkv_read_workqueue.restype = _i32
+    lib.pkv_read_workqueue.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, ctypes.c_size_t, _vp, _i32, _vp,
+                                       P(_i32), _vp]
+    lib.pkv_workspace_partials.restype = _i32
+    lib.pkv_workspace_partials.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, ctypes.c_size_t, P(_vp), P(_vp),
+                                           P(_vp), P(_i64)]
+    lib.pkv_decode_host.restype = _i32
+    lib.pkv_decode_host.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float,
+                                    _vp, _vp, ctypes.c_size_t, _vp, ctypes.c_size_t, _vp, P(pkv_counters)]
+    lib.pkv_debug_force_tma_mode.restype = None
+    lib.pkv_debug_force_tma_mode.argtypes = [ctypes.c_int]
+    return lib
+
+
+_lib = _load()
+
+
+def _check(status: int):
+    if status != PKV_OK:
+        raise PkvError(status, _lib.pkv_last_error().decode("utf-8", "replace"))
+
+
+# ------------------------------------------------------------------ argument helpers
+
+@dataclass
+class Shape:
+    B: int
+    Hq: int
+    Hkv: int
+    d: int = 128
+    page_size: int = 16
+    max_pages: int = 0
+    num_pages: int = 0
+    kv_strides: Tuple[int, int, int] = (0, 0, 0)   # (page, token, head) in elements; zeros = default layout
+
+    def c(self) -> pkv_shape:
+        return pkv_shape(self.B, self.Hq, self.Hkv, self.d, self.page_size, self.max_pages, self.num_pages,
+                         *self.kv_strides)
+
+
+@dataclass
+class Policy:
+    tile_tokens: int = 32
+    split_mode: int = SPLIT_FIXED_COUNT
+    num_splits: int = 1
+    chunk_tiles: int = 0
+    route: int = ROUTE_WORKQUEUE
+    merge_mode: int = MERGE_SEPARATE
+    num_sms: int = 0
+    kernel: int = KERNEL_AUTO
+
+    def c(self) -> pkv_split_policy:
+        return pkv_split_policy(self.tile_tokens, self.split_mode, self.num_splits, self.chunk_tiles, self.route,
+                                self.merge_mode, self.num_sms, self.kernel)
+
+
+def _ptr(x) -> Optional[int]:
+    """Raw address of a torch tensor, a numpy array, an int, or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        assert x.flags["C_CONTIGUOUS"]
+        return x.ctypes.data
+    assert x.is_contiguous(), "tensors must be contiguous"
+    return x.data_ptr()
+
+
+def _nbytes(x) -> int:
+    if isinstance(x, np.ndarray):
+        return x.nbytes
+    return x.numel() * x.element_size()
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+# ------------------------------------------------------------------ the ABI, name for name
+
+def pkv_version() -> int:
+    return int(_lib.pkv_version())
+
+
+def pkv_last_error() -> str:
+    return _lib.pkv_last_error().decode("utf-8", "replace")
+
+
+def pkv_workspace_bytes(shape: Shape, policy: Policy) -> int:
+    n = int(_lib.pkv_workspace_bytes(ctypes.byref(shape.c()), ctypes.byref(policy.c())))
+    if n == 0:
+        raise PkvError(PKV_ERR_INVALID_ARG, "pkv_workspace_bytes: invalid shape/policy")
+    return n
+
+
+def pkv_host_scratch_bytes(shape: Shape, policy: Policy) -> int:
+    n = int(_lib.pkv_host_scratch_bytes(ctypes.byref(shape.c()), ctypes.byref(policy.c())))
+    if n == 0:
+        raise PkvError(PKV_ERR_INVALID_ARG, "pkv_host_scratch_bytes: invalid shape/policy")
+    return n
+
+
+def pkv_build_workqueue_host(shape: Shape, policy: Policy, seq_lens_host: np.ndarray):
+    """Returns (tasks int32 [num_tasks, 5], split_offsets int32 [B+1])."""
+    seq = np.ascontiguousarray(seq_lens_host, dtype=np.int32)
+    offsets = np.zeros(shape.B + 1, dtype=np.int32)
+    n = _i32(0)
+    st = _lib.pkv_build_workqueue_host(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(seq), None, 0,
+                                       _ptr(offsets), ctypes.byref(n))
+    _check(st)
+    tasks = np.zeros((max(int(n.value), 1), 5), dtype=np.int32)
+    st = _lib.pkv_build_workqueue_host(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(seq), _ptr(tasks),
+                                       tasks.shape[0], _ptr(offsets), ctypes.byref(n))
+    _check(st)
+    return tasks[:int(n.value)], offsets
+
+
+def pkv_build_workqueue(shape: Shape, policy: Policy, seq_lens_dev, workspace, stream=None) -> None:
+    _check(_lib.pkv_build_workqueue(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(seq_lens_dev),
+                                    _ptr(workspace), _nbytes(workspace), _stream_ptr(stream)))
+
+
+def pkv_decode(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, seq_lens, out, lse=None,
+               scale: float = 0.0, build_queue: bool = True, workspace=None, stream=None) -> None:
+    _check(_lib.pkv_decode(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(q), _ptr(k_cache), _ptr(v_cache),
+                           _ptr(block_table), _ptr(seq_lens), _ptr(out), _ptr(lse), ctypes.c_float(scale),
+                           1 if build_queue else 0, _ptr(workspace), _nbytes(workspace), _stream_ptr(stream)))
+
+
+def pkv_merge(shape: Shape, part_m, part_l, part_acc, split_offsets, out, lse=None, stream=None) -> None:
+    _check(_lib.pkv_merge(ctypes.byref(shape.c()), _ptr(part_m), _ptr(part_l), _ptr(part_acc), _ptr(split_offsets),
+                          _ptr(out), _ptr(lse), _stream_ptr(stream)))
+
+
+def pkv_get_counters(shape: Shape, policy: Policy, workspace, stream=None) -> dict:
+    c = pkv_counters()
+    _check(_lib.pkv_get_counters(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(workspace),
+                                 _nbytes(workspace), ctypes.byref(c), _stream_ptr(stream)))
+    return c.as_dict()
+
+
+def pkv_read_workqueue(shape: Shape, policy: Policy, workspace, stream=None):
+    """Returns (tasks int32 [num_tasks, 5], split_offsets int32 [B+1]) copied from the device."""
+    offsets = np.zeros(shape.B + 1, dtype=np.int32)
+    n = _i32(0)
+    sp = _stream_ptr(stream)
+    _check(_lib.pkv_read_workqueue(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(workspace),
+                                   _nbytes(workspace), None, 0, _ptr(offsets), ctypes.byref(n), sp))
+    tasks = np.zeros((max(int(n.value), 1), 5), dtype=np.int32)
+    _check(_lib.pkv_read_workqueue(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(workspace),
+                                   _nbytes(workspace), _ptr(tasks), tasks.shape[0], _ptr(offsets), ctypes.byref(n), sp))
+    return tasks[:int(n.value)], offsets
+
+
+def pkv_workspace_partials(shape: Shape, policy: Policy, workspace):
+    """Returns (ptr_m, ptr_l, ptr_acc, slots_cap): device addresses inside the workspace."""
+    pm, pl, pa, cap = _vp(), _vp(), _vp(), _i64(0)
+    _check(_lib.pkv_workspace_partials(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(workspace),
+                                       _nbytes(workspace), ctypes.byref(pm), ctypes.byref(pl), ctypes.byref(pa),
+                                       ctypes.byref(cap)))
+    return int(pm.value), int(pl.value), int(pa.value), int(cap.value)
+
+
+def pkv_decode_host(shape: Shape, policy: Policy, q_host, k_cache_dev, v_cache_dev, block_table_host, seq_lens_host,
+                    out_host, scale: float, host_staging, dev_scratch, workspace, stream=None) -> dict:
+    c = pkv_counters()
+    _check(_lib.pkv_decode_host(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(q_host), _ptr(k_cache_dev),
+                                _ptr(v_cache_dev), _ptr(block_table_host), _ptr(seq_lens_host), _ptr(out_host),
+                                ctypes.c_float(scale), _ptr(host_staging), _ptr(dev_scratch),
+                                min(_nbytes(host_staging), _nbytes(dev_scratch)), _ptr(workspace), _nbytes(workspace),
+                                _stream_ptr(stream), ctypes.byref(c)))
+    return c.as_dict()
+
+
+def pkv_debug_force_tma_mode(mode: int) -> None:
+    _lib.pkv_debug_force_tma_mode(int(mode))

@@ -1,0 +1,546 @@
+// pkv_api.cu -- the CUDA-facing entry points of include/pkv.h: argument checks, tensor-map
+// encoding, workspace carving and the launch sequence [builder] -> decode -> [merge].
+// No allocation, no synchronisation and no host read of device data in pkv_build_workqueue,
+// pkv_decode and pkv_merge (they are CUDA-graph-capture-safe).
+#include <cuda.h>
+
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "pkv_device.cuh"
+
+namespace pkv {
+
+namespace {
+
+int g_force_tma_mode = -1;  // test hook: -1 auto, 0 = 5-D box, 1 = 4-D half boxes
+
+int device_sm_count() {
+    thread_local int cache[64];
+    thread_local bool have[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
+    if (!have[dev]) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+        cache[dev] = n;
+        have[dev] = true;
+    }
+    return cache[dev];
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        void* ptr = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(ptr);
+        tried = true;
+    }
+    return fn;
+}
+
+typedef CUresult (*MemsetD32Fn)(CUdeviceptr, unsigned int, size_t, CUstream);
+MemsetD32Fn memset_d32_fn() {
+    static MemsetD32Fn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        void* ptr = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuMemsetD32Async", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<MemsetD32Fn>(ptr);
+        tried = true;
+    }
+    return fn;
+}
+
+struct Strides { int64_t page, token, head; };
+Strides effective_strides(const pkv_shape& s) {
+    if (s.kv_stride_page == 0) return {(int64_t)s.page_size * s.Hkv * s.d, (int64_t)s.Hkv * s.d, (int64_t)s.d};
+    return {s.kv_stride_page, s.kv_stride_token, s.kv_stride_head};
+}
+
+// tma_mode: 0 = rank 5 (64 ch, 16 tok, 2 ch-halves, head, page), one 4 KiB box per (page, head);
+//           1 = rank 4 (128 ch, 16 tok, head, page), 2 = rank 4 (128 ch, head, 16 tok, page): two
+//           2 KiB boxes per (page, head), dimensions ordered by stride.
+bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int mode, CUtensorMap* out) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t pages = (cuuint64_t)(s.num_pages > 0 ? s.num_pages : 1);
+    cuuint64_t dims[5], strides[4];
+    cuuint32_t box[5], estr[5] = {1, 1, 1, 1, 1};
+    cuuint32_t rank;
+    if (mode == 0) {
+        rank = 5;
+        dims[0] = 64; dims[1] = 16; dims[2] = 2; dims[3] = (cuuint64_t)s.Hkv; dims[4] = pages;
+        strides[0] = (cuuint64_t)st.token * 2; strides[1] = 128; strides[2] = (cuuint64_t)st.head * 2;
+        strides[3] = (cuuint64_t)st.page * 2;
+        box[0] = 64; box[1] = 16; box[2] = 2; box[3] = 1; box[4] = 1;
+    } else if (mode == 1) {
+        rank = 4;
+        dims[0] = 128; dims[1] = 16; dims[2] = (cuuint64_t)s.Hkv; dims[3] = pages;
+        strides[0] = (cuuint64_t)st.token * 2; strides[1] = (cuuint64_t)st.head * 2; strides[2] = (cuuint64_t)st.page * 2;
+        box[0] = 64; box[1] = 16; box[2] = 1; box[3] = 1;
+    } else {
+        rank = 4;
+        dims[0] = 128; dims[1] = (cuuint64_t)s.Hkv; dims[2] = 16; dims[3] = pages;
+        strides[0] = (cuuint64_t)st.head * 2; strides[1] = (cuuint64_t)st.token * 2; strides[2] = (cuuint64_t)st.page * 2;
+        box[0] = 64; box[1] = 1; box[2] = 16; box[3] = 1;
+    }
+    const CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, rank, const_cast<void*>(base), dims, strides, box,
+                          estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+struct MapCacheEntry {
+    const void* base;
+    int64_t num_pages, sp, st, sh;
+    int32_t Hkv, mode;
+    CUtensorMap map;
+};
+
+// Returns the tensor map of `base` (encoding it on first use) and the mode it was encoded in.
+const CUtensorMap* get_map(const void* base, const pkv_shape& s, int* mode_out) {
+    thread_local std::vector<MapCacheEntry> cache;
+    thread_local size_t next = 0;
+    const Strides st = effective_strides(s);
+    for (const MapCacheEntry& e : cache)
+        if (e.base == base && e.num_pages == s.num_pages && e.sp == st.page && e.st == st.token && e.sh == st.head &&
+            e.Hkv == s.Hkv && (g_force_tma_mode < 0 || (g_force_tma_mode == 0) == (e.mode == 0))) {
+            *mode_out = e.mode;
+            return &e.map;
+        }
+    MapCacheEntry e;
+    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv;
+    bool ok = false;
+    if (g_force_tma_mode != 1) { e.mode = 0; ok = encode_map(base, s, st, 0, &e.map); }
+    if (!ok) { e.mode = st.head < st.token ? 2 : 1; ok = encode_map(base, s, st, e.mode, &e.map); }
+    if (!ok) return nullptr;
+    if (cache.size() < 16) {
+        cache.push_back(e);
+        *mode_out = e.mode;
+        return &cache.back().map;
+    }
+    cache[next] = e;
+    const CUtensorMap* r = &cache[next].map;
+    next = (next + 1) % cache.size();
+    *mode_out = e.mode;
+    return r;
+}
+
+pkv_status cuda_fail(cudaError_t e, const char* what) {
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    return PKV_ERR_CUDA;
+}
+
+struct QueuePtrs {
+    QueueHeader* hdr;
+    int32_t* split_offsets;
+    pkv_task* tasks;
+};
+
+struct WsPtrs {
+    QueuePtrs q;
+    int32_t* fuse_counters;
+    float *part_m, *part_l, *part_acc;
+};
+
+WsPtrs carve(void* workspace, const WorkspaceLayout& L) {
+    unsigned char* w = static_cast<unsigned char*>(workspace);
+    WsPtrs r;
+    r.q.hdr = reinterpret_cast<QueueHeader*>(w + L.header);
+    r.q.split_offsets = reinterpret_cast<int32_t*>(w + L.split_offsets);
+    r.q.tasks = reinterpret_cast<pkv_task*>(w + L.tasks);
+    r.fuse_counters = reinterpret_cast<int32_t*>(w + L.fuse_counters);
+    r.part_m = reinterpret_cast<float*>(w + L.part_m);
+    r.part_l = reinterpret_cast<float*>(w + L.part_l);
+    r.part_acc = reinterpret_cast<float*>(w + L.part_acc);
+    return r;
+}
+
+pkv_status check_workspace(const void* workspace, size_t bytes, const WorkspaceLayout& L) {
+    if (!workspace) { set_error("null workspace"); return PKV_ERR_INVALID_ARG; }
+    if (reinterpret_cast<uintptr_t>(workspace) % 256) { set_error("workspace must be 256-byte aligned"); return PKV_ERR_INVALID_ARG; }
+    if (bytes < L.total) { set_error("workspace has %zu bytes, %zu needed", bytes, L.total); return PKV_ERR_WORKSPACE; }
+    return PKV_OK;
+}
+
+// Launches decode (+ merge).  known_tasks / known_max_n >= 0: the queue was planned on the host,
+// so launches that have nothing to do are skipped (A13).
+pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, const void* k_cache, const void* v_cache,
+                      const int32_t* block_table, const int32_t* seq_lens, void* out, float* lse, float scale,
+                      const QueuePtrs& qp, const WsPtrs& ws, int64_t known_tasks, int known_max_n, int num_sms,
+                      cudaStream_t stream, int* decode_launches, int* merge_launches) {
+    DecodeParams p;
+    std::memset(&p, 0, sizeof(p));
+    const Strides st = effective_strides(s);
+    p.q = static_cast<const __half*>(q);
+    p.k_cache = static_cast<const __half*>(k_cache);
+    p.v_cache = static_cast<const __half*>(v_cache);
+    p.block_table = block_table;
+    p.seq_lens = seq_lens;
+    p.tasks = qp.tasks;
+    p.split_offsets = qp.split_offsets;
+    p.hdr = qp.hdr;
+    p.out = static_cast<__half*>(out);
+    p.lse = lse;
+    p.part_m = ws.part_m; p.part_l = ws.part_l; p.part_acc = ws.part_acc;
+    p.fuse_counters = ws.fuse_counters;
+    p.stride_page = st.page; p.stride_token = st.token; p.stride_head = st.head;
+    p.B = s.B; p.Hq = s.Hq; p.Hkv = s.Hkv; p.max_pages = s.max_pages;
+    p.tile_tokens = rp.tile_tokens; p.merge_mode = rp.merge_mode;
+    p.dynamic_sched = 1;
+    const float sc = scale > 0.f ? scale : 1.0f / std::sqrt((float)s.d);
+    p.scale = sc;
+    p.scale_log2 = sc * kLog2e;
+
+    if (decode_launches) *decode_launches = 0;
+    if (merge_launches) *merge_launches = 0;
+    if (s.B == 0) return PKV_OK;
+    const int64_t bound = known_tasks >= 0 ? known_tasks : (int64_t)s.B * s.Hkv * rp.S;
+    cudaError_t e;
+    if (known_tasks == 0) {
+        // every row is empty: out = 0, lse = -inf, no decode launch
+        e = cudaMemsetAsync(out, 0, (size_t)s.B * s.Hq * s.d * 2, stream);
+        if (e != cudaSuccess) return cuda_fail(e, "memset out");
+        if (lse) {
+            MemsetD32Fn ms = memset_d32_fn();
+            if (!ms || ms(reinterpret_cast<CUdeviceptr>(lse), 0xff800000u /* -inf */, (size_t)s.B * s.Hq, stream) !=
+                           CUDA_SUCCESS) {
+                set_error("cuMemsetD32Async failed");
+                return PKV_ERR_CUDA;
+            }
+        }
+    }
+    if (known_tasks != 0) {
+        if (rp.kernel == PKV_KERNEL_TMA_MMA) {
+            int mode_k = 0, mode_v = 0;
+            const CUtensorMap* mk = get_map(k_cache, s, &mode_k);
+            const CUtensorMap* mv = get_map(v_cache, s, &mode_v);
+            if (!mk || !mv || mode_k != mode_v) {
+                set_error("cuTensorMapEncodeTiled failed for the K/V cache (base %p/%p)", k_cache, v_cache);
+                return PKV_ERR_CUDA;
+            }
+            p.tma_rank = mode_k;  // 0: 5-D, 1/2: 4-D dimension orders
+            const int grid = (int)(bound < num_sms ? bound : num_sms);
+            e = launch_decode_tma(p, rp.G, grid, mk, mv, stream);
+        } else {
+            const int64_t cap = (int64_t)num_sms * 4;
+            const int grid = (int)(bound < cap ? bound : cap);
+            e = launch_decode_simt(p, rp.G, grid, stream);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "decode launch");
+        if (decode_launches) *decode_launches = 1;
+    }
+    const bool need_merge = rp.merge_mode == PKV_MERGE_SEPARATE &&
+                            (known_max_n >= 0 ? known_max_n > 1 : rp.S > 1) && known_tasks != 0;
+    if (need_merge) {
+        e = launch_merge(p, rp.G, stream);
+        if (e != cudaSuccess) return cuda_fail(e, "merge launch");
+        if (merge_launches) *merge_launches = 1;
+    }
+    return PKV_OK;
+}
+
+pkv_status check_decode_ptrs(const pkv_shape& s, const void* q, const void* k, const void* v, const int32_t* bt,
+                             const int32_t* sl, const void* out) {
+    if (s.B > 0 && (!q || !k || !v || !bt || !sl || !out)) { set_error("null pointer argument"); return PKV_ERR_INVALID_ARG; }
+    if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(k) | reinterpret_cast<uintptr_t>(v) |
+         reinterpret_cast<uintptr_t>(out)) % 16) {
+        set_error("q, k_cache, v_cache and out must be 16-byte aligned");
+        return PKV_ERR_INVALID_ARG;
+    }
+    return PKV_OK;
+}
+
+}  // namespace
+}  // namespace pkv
+
+using namespace pkv;
+
+extern "C" {
+
+// test hook (not in pkv.h): force the tensor-map mode of the next encodes
+PKV_API void pkv_debug_force_tma_mode(int mode) { g_force_tma_mode = mode; }
+
+pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_policy* policy, const int32_t* seq_lens_dev,
+                               void* workspace, size_t workspace_bytes, void* stream) {
+    clear_error();
+    Resolved rp;
+    pkv_status st = validate_and_resolve(shape, policy, device_sm_count(), false, &rp);
+    if (st != PKV_OK) return st;
+    if (!seq_lens_dev && shape->B > 0) { set_error("null seq_lens"); return PKV_ERR_INVALID_ARG; }
+    const WorkspaceLayout L = workspace_layout(*shape, rp.S);
+    st = check_workspace(workspace, workspace_bytes, L);
+    if (st != PKV_OK) return st;
+    const WsPtrs ws = carve(workspace, L);
+    const cudaError_t e = launch_builder(*shape, rp, seq_lens_dev, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
+                                         ws.q.tasks, L.slots_cap, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e, "builder launch");
+    return PKV_OK;
+}
+
+pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q, const void* k_cache,
+                      const void* v_cache, const int32_t* block_table, const int32_t* seq_lens, void* out, float* lse,
+                      float scale, int32_t build_queue, void* workspace, size_t workspace_bytes, void* stream) {
+    clear_error();
+    Resolved rp;
+    const int sms = device_sm_count();
+    pkv_status st = validate_and_resolve(shape, policy, sms, false, &rp);
+    if (st != PKV_OK) return st;
+    if (sms <= 0) { set_error("no CUDA device"); return PKV_ERR_CUDA; }
+    st = check_decode_ptrs(*shape, q, k_cache, v_cache, block_table, seq_lens, out);
+    if (st != PKV_OK) return st;
+    const WorkspaceLayout L = workspace_layout(*shape, rp.S);
+    st = check_workspace(workspace, workspace_bytes, L);
+    if (st != PKV_OK) return st;
+    const WsPtrs ws = carve(workspace, L);
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    if (build_queue) {
+        const cudaError_t e = launch_builder(*shape, rp, seq_lens, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
+                                             ws.q.tasks, L.slots_cap, cs);
+        if (e != cudaSuccess) return cuda_fail(e, "builder launch");
+    }
+    return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, out, lse, scale, ws.q, ws, -1, -1, sms,
+                      cs, nullptr, nullptr);
+}
+
+pkv_status pkv_merge(const pkv_shape* shape, const float* part_m, const float* part_l, const float* part_acc,
+                     const int32_t* split_offsets, void* out, float* lse, void* stream) {
+    clear_error();
+    pkv_split_policy pol;
+    std::memset(&pol, 0, sizeof(pol));
+    pol.tile_tokens = shape ? shape->page_size : 16;
+    pol.num_splits = 1;
+    Resolved rp;
+    pkv_status st = validate_and_resolve(shape, &pol, 0, true, &rp);
+    if (st != PKV_OK) return st;
+    if (shape->B > 0 && (!part_m || !part_l || !part_acc || !split_offsets || !out)) {
+        set_error("null pointer argument");
+        return PKV_ERR_INVALID_ARG;
+    }
+    DecodeParams p;
+    std::memset(&p, 0, sizeof(p));
+    p.part_m = const_cast<float*>(part_m);
+    p.part_l = const_cast<float*>(part_l);
+    p.part_acc = const_cast<float*>(part_acc);
+    p.split_offsets = split_offsets;
+    p.hdr = nullptr;
+    p.out = static_cast<__half*>(out);
+    p.lse = lse;
+    p.B = shape->B; p.Hq = shape->Hq; p.Hkv = shape->Hkv;
+    const cudaError_t e = launch_merge(p, rp.G, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e, "merge launch");
+    return PKV_OK;
+}
+
+pkv_status pkv_get_counters(const pkv_shape* shape, const pkv_split_policy* policy, const void* workspace,
+                            size_t workspace_bytes, pkv_counters* host_out, void* stream) {
+    clear_error();
+    Resolved rp;
+    pkv_status st = validate_and_resolve(shape, policy, device_sm_count(), false, &rp);
+    if (st != PKV_OK) return st;
+    if (!host_out) { set_error("null host_out"); return PKV_ERR_INVALID_ARG; }
+    const WorkspaceLayout L = workspace_layout(*shape, rp.S);
+    st = check_workspace(workspace, workspace_bytes, L);
+    if (st != PKV_OK) return st;
+    QueueHeader h;
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaMemcpyAsync(&h, static_cast<const unsigned char*>(workspace) + L.header, sizeof(h),
+                                    cudaMemcpyDeviceToHost, cs);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
+    if (e != cudaSuccess) return cuda_fail(e, "read header");
+    std::memset(host_out, 0, sizeof(*host_out));
+    host_out->tasks = h.num_tasks;
+    host_out->empty_tasks = h.empty_tasks;
+    host_out->decode_launches = h.num_tasks > 0 ? 1 : 0;
+    host_out->merge_launches =
+        (h.num_tasks > 0 && h.max_row_splits > 1 && rp.merge_mode == PKV_MERGE_SEPARATE) ? 1 : 0;
+    host_out->build_launches = 1;
+    host_out->useful_kv_bytes = h.sum_seq_lens * 2 * shape->Hkv * shape->d * 2;
+    host_out->merge_bytes = (int64_t)h.num_tasks * rp.G * (shape->d + 2) * 4;
+    host_out->num_splits = h.resolved_splits;
+    host_out->max_row_splits = h.max_row_splits;
+    return PKV_OK;
+}
+
+pkv_status pkv_read_workqueue(const pkv_shape* shape, const pkv_split_policy* policy, const void* workspace,
+                              size_t workspace_bytes, pkv_task* host_tasks, int32_t cap, int32_t* host_split_offsets,
+                              int32_t* host_num_tasks, void* stream) {
+    clear_error();
+    Resolved rp;
+    pkv_status st = validate_and_resolve(shape, policy, device_sm_count(), false, &rp);
+    if (st != PKV_OK) return st;
+    if (!host_num_tasks) { set_error("null host_num_tasks"); return PKV_ERR_INVALID_ARG; }
+    const WorkspaceLayout L = workspace_layout(*shape, rp.S);
+    st = check_workspace(workspace, workspace_bytes, L);
+    if (st != PKV_OK) return st;
+    const unsigned char* w = static_cast<const unsigned char*>(workspace);
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    QueueHeader h;
+    cudaError_t e = cudaMemcpyAsync(&h, w + L.header, sizeof(h), cudaMemcpyDeviceToHost, cs);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
+    if (e != cudaSuccess) return cuda_fail(e, "read header");
+    *host_num_tasks = h.num_tasks;
+    if (host_split_offsets) {
+        e = cudaMemcpyAsync(host_split_offsets, w + L.split_offsets, sizeof(int32_t) * ((size_t)shape->B + 1),
+                            cudaMemcpyDeviceToHost, cs);
+        if (e != cudaSuccess) return cuda_fail(e, "read split_offsets");
+    }
+    if (host_tasks && cap > 0) {
+        const int32_t n = h.num_tasks < cap ? h.num_tasks : cap;
+        e = cudaMemcpyAsync(host_tasks, w + L.tasks, sizeof(pkv_task) * (size_t)n, cudaMemcpyDeviceToHost, cs);
+        if (e != cudaSuccess) return cuda_fail(e, "read tasks");
+    }
+    e = cudaStreamSynchronize(cs);
+    if (e != cudaSuccess) return cuda_fail(e, "sync");
+    if (host_tasks && h.num_tasks > cap) { set_error("cap=%d < %d tasks", cap, h.num_tasks); return PKV_ERR_WORKSPACE; }
+    return PKV_OK;
+}
+
+pkv_status pkv_workspace_partials(const pkv_shape* shape, const pkv_split_policy* policy, void* workspace,
+                                  size_t workspace_bytes, float** part_m, float** part_l, float** part_acc,
+                                  int64_t* slots_cap) {
+    clear_error();
+    Resolved rp;
+    pkv_status st = validate_and_resolve(shape, policy, device_sm_count(), false, &rp);
+    if (st != PKV_OK) return st;
+    const WorkspaceLayout L = workspace_layout(*shape, rp.S);
+    st = check_workspace(workspace, workspace_bytes, L);
+    if (st != PKV_OK) return st;
+    const WsPtrs ws = carve(workspace, L);
+    if (part_m) *part_m = ws.part_m;
+    if (part_l) *part_l = ws.part_l;
+    if (part_acc) *part_acc = ws.part_acc;
+    if (slots_cap) *slots_cap = L.slots_cap;
+    return PKV_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ host-buffer path
+
+namespace pkv {
+namespace {
+
+// Image of one step's host inputs, identical in the pinned staging buffer and in dev_scratch:
+//   [QueueHeader][split_offsets B+1][seq_lens B][q B*Hq*d f16][block_table B*max_pages][tasks ...]
+// followed (device only) by the FP16 output.  Tasks are last so that one H2D copy of
+// (tasks_off + num_tasks * 20) bytes moves exactly what the step needs.
+struct HostImage {
+    size_t hdr, split_offsets, seq_lens, q, block_table, tasks, tasks_end, out, total;
+};
+HostImage host_image(const pkv_shape& s, int32_t S) {
+    HostImage h;
+    size_t off = 0;
+    h.hdr = off;           off = align_up(off + sizeof(QueueHeader), 256);
+    h.split_offsets = off; off = align_up(off + 4 * ((size_t)s.B + 1), 256);
+    h.seq_lens = off;      off = align_up(off + 4 * (size_t)s.B, 256);
+    h.q = off;             off = align_up(off + 2 * (size_t)s.B * s.Hq * s.d, 256);
+    h.block_table = off;   off = align_up(off + 4 * (size_t)s.B * s.max_pages, 256);
+    h.tasks = off;         off = align_up(off + sizeof(pkv_task) * (size_t)s.B * s.Hkv * S, 256);
+    h.tasks_end = off;
+    h.out = off;           off = align_up(off + 2 * (size_t)s.B * s.Hq * s.d, 256);
+    h.total = off;
+    return h;
+}
+
+}  // namespace
+}  // namespace pkv
+
+extern "C" {
+
+size_t pkv_host_scratch_bytes(const pkv_shape* shape, const pkv_split_policy* policy) {
+    Resolved rp;
+    if (validate_and_resolve(shape, policy, 0, /*bound_ok=*/true, &rp) != PKV_OK) return 0;
+    return host_image(*shape, rp.S).total;
+}
+
+pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* policy, const void* q_host,
+                           const void* k_cache_dev, const void* v_cache_dev, const int32_t* block_table_host,
+                           const int32_t* seq_lens_host, void* out_host, float scale, void* host_staging,
+                           void* dev_scratch, size_t scratch_bytes, void* workspace, size_t workspace_bytes,
+                           void* stream, pkv_counters* counters_out) {
+    clear_error();
+    Resolved rp;
+    const int sms = device_sm_count();
+    pkv_status st = validate_and_resolve(shape, policy, sms, false, &rp);
+    if (st != PKV_OK) return st;
+    if (sms <= 0) { set_error("no CUDA device"); return PKV_ERR_CUDA; }
+    const pkv_shape& s = *shape;
+    if (s.B > 0 && (!q_host || !k_cache_dev || !v_cache_dev || !block_table_host || !seq_lens_host || !out_host)) {
+        set_error("null pointer argument");
+        return PKV_ERR_INVALID_ARG;
+    }
+    if (!host_staging || !dev_scratch || reinterpret_cast<uintptr_t>(dev_scratch) % 256) {
+        set_error("host_staging / dev_scratch null or dev_scratch not 256-byte aligned");
+        return PKV_ERR_INVALID_ARG;
+    }
+    const HostImage im = host_image(s, rp.S);
+    if (scratch_bytes < im.total) { set_error("scratch has %zu bytes, %zu needed", scratch_bytes, im.total); return PKV_ERR_WORKSPACE; }
+    const WorkspaceLayout L = workspace_layout(s, rp.S);
+    st = check_workspace(workspace, workspace_bytes, L);
+    if (st != PKV_OK) return st;
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+
+    // host planning ("Python planning" is part of the serving-facing time)
+    unsigned char* hs = static_cast<unsigned char*>(host_staging);
+    unsigned char* ds = static_cast<unsigned char*>(dev_scratch);
+    QueueHeader* hdr = reinterpret_cast<QueueHeader*>(hs + im.hdr);
+    st = plan_host(s, rp, seq_lens_host, reinterpret_cast<pkv_task*>(hs + im.tasks),
+                   (int32_t)((im.tasks_end - im.tasks) / sizeof(pkv_task)),
+                   reinterpret_cast<int32_t*>(hs + im.split_offsets), hdr);
+    if (st != PKV_OK) { set_error("host plan overflow"); return st; }
+    std::memcpy(hs + im.seq_lens, seq_lens_host, 4 * (size_t)s.B);
+    std::memcpy(hs + im.q, q_host, 2 * (size_t)s.B * s.Hq * s.d);
+    std::memcpy(hs + im.block_table, block_table_host, 4 * (size_t)s.B * s.max_pages);
+    const size_t h2d = im.tasks + sizeof(pkv_task) * (size_t)hdr->num_tasks;
+    cudaError_t e = cudaMemcpyAsync(ds, hs, h2d, cudaMemcpyHostToDevice, cs);
+    if (e != cudaSuccess) return cuda_fail(e, "H2D step image");
+
+    WsPtrs ws = carve(workspace, L);
+    if (rp.merge_mode == PKV_MERGE_FUSED && hdr->max_row_splits > 1) {
+        e = cudaMemsetAsync(ws.fuse_counters, 0, 4 * (size_t)s.B * s.Hkv, cs);
+        if (e != cudaSuccess) return cuda_fail(e, "memset fuse counters");
+    }
+    QueuePtrs qp;
+    qp.hdr = reinterpret_cast<QueueHeader*>(ds + im.hdr);
+    qp.split_offsets = reinterpret_cast<int32_t*>(ds + im.split_offsets);
+    qp.tasks = reinterpret_cast<pkv_task*>(ds + im.tasks);
+    int dl = 0, ml = 0;
+    st = run_decode(s, rp, ds + im.q, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
+                    reinterpret_cast<const int32_t*>(ds + im.seq_lens), ds + im.out, nullptr, scale, qp, ws,
+                    hdr->num_tasks, hdr->max_row_splits, sms, cs, &dl, &ml);
+    if (st != PKV_OK) return st;
+    const size_t out_bytes = 2 * (size_t)s.B * s.Hq * s.d;
+    e = cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
+    if (e != cudaSuccess) return cuda_fail(e, "D2H out / sync");
+    if (counters_out) {
+        std::memset(counters_out, 0, sizeof(*counters_out));
+        counters_out->tasks = hdr->num_tasks;
+        counters_out->empty_tasks = hdr->empty_tasks;
+        counters_out->decode_launches = dl;
+        counters_out->merge_launches = ml;
+        counters_out->build_launches = 0;
+        counters_out->useful_kv_bytes = hdr->sum_seq_lens * 2 * s.Hkv * s.d * 2;
+        counters_out->merge_bytes = (int64_t)hdr->num_tasks * rp.G * (s.d + 2) * 4;
+        counters_out->num_splits = hdr->resolved_splits;
+        counters_out->max_row_splits = hdr->max_row_splits;
+        counters_out->h2d_bytes = (int64_t)h2d;
+        counters_out->d2h_bytes = (int64_t)out_bytes;
+    }
+    return PKV_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,173 @@
+// pkv_aux.cu -- the two small kernels around the decode kernel:
+//   * device workqueue builder: split-bound policy from the true row lengths
+//     and the compact task list in canonical order (A6-A8);
+//   * segmented merge of split states.
+#include "pkv_device.cuh"
+
+namespace pkv {
+
+namespace {
+
+constexpr int kBuildThreads = 1024;
+
+struct BuildArgs {
+    const int32_t* seq_lens;
+    QueueHeader* hdr;
+    int32_t* split_offsets;
+    int32_t* fuse_counters;
+    pkv_task* tasks;
+    int64_t tasks_cap;
+    int32_t B, Hkv, S, tile_tokens, split_mode, chunk_tiles, route;
+};
+
+// One CTA.  Phase 1: per-row slot counts and their exclusive prefix sum (split_offsets).
+// Phase 2: every thread fills task entries idx = tid, tid + 1024, ...; the row of an entry is
+// found by binary search in split_offsets, so the list comes out in (row, kvh, split) order.
+__global__ void __launch_bounds__(kBuildThreads) pkv_build_workqueue_kernel(const BuildArgs a) {
+    __shared__ int32_t warp_sums[32];
+    __shared__ int32_t carry_s;
+    __shared__ int32_t max_n_s, empties_s;
+    __shared__ unsigned long long sum_seq_s;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        carry_s = 0;
+        max_n_s = 0;
+        empties_s = 0;
+        sum_seq_s = 0ull;
+        a.split_offsets[0] = 0;
+    }
+    __syncthreads();
+    for (int base = 0; base < a.B; base += kBuildThreads) {
+        const int i = base + tid;
+        int32_t slots = 0, N = 0;
+        if (i < a.B) {
+            N = max(a.seq_lens[i], 0);
+            const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
+            slots = a.route == PKV_ROUTE_WORKQUEUE ? r.n : a.S;
+        }
+        // inclusive warp scan, then scan of warp totals
+        int32_t v = slots;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const int32_t u = __shfl_up_sync(0xffffffffu, v, off);
+            if (lane >= off) v += u;
+        }
+        if (lane == 31) warp_sums[warp] = v;
+        __syncthreads();
+        if (warp == 0) {
+            int32_t w = warp_sums[lane];
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                const int32_t u = __shfl_up_sync(0xffffffffu, w, off);
+                if (lane >= off) w += u;
+            }
+            warp_sums[lane] = w;  // inclusive
+        }
+        __syncthreads();
+        const int32_t incl = carry_s + (warp > 0 ? warp_sums[warp - 1] : 0) + v;
+        if (i < a.B) {
+            a.split_offsets[i + 1] = incl;
+            atomicMax(&max_n_s, slots);
+            atomicAdd(&sum_seq_s, (unsigned long long)N);
+        }
+        __syncthreads();
+        if (tid == kBuildThreads - 1) carry_s = incl;
+        __syncthreads();
+    }
+    for (int i = tid; i < a.B * a.Hkv; i += kBuildThreads) a.fuse_counters[i] = 0;
+    __threadfence_block();
+    __syncthreads();
+
+    const int64_t total = (int64_t)carry_s * a.Hkv;
+    const int64_t lim = total < a.tasks_cap ? total : a.tasks_cap;
+    int32_t my_empties = 0;
+    for (int64_t idx = tid; idx < lim; idx += kBuildThreads) {
+        // largest row with split_offsets[row] * Hkv <= idx
+        int lo = 0, hi = a.B - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if ((int64_t)a.split_offsets[mid] * a.Hkv <= idx) lo = mid; else hi = mid - 1;
+        }
+        const int row = lo;
+        const int32_t so = a.split_offsets[row];
+        const int32_t slots = a.split_offsets[row + 1] - so;
+        const int32_t local = (int32_t)(idx - (int64_t)so * a.Hkv);
+        const int32_t g = local / slots, s = local % slots;
+        const int32_t N = max(a.seq_lens[row], 0);
+        const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
+        int32_t tb = 0, te = 0;
+        if (r.T > 0) {
+            const int64_t b = (int64_t)s * r.c, e = (int64_t)(s + 1) * r.c;
+            tb = (int32_t)(b < r.T ? b : r.T);
+            te = (int32_t)(e < r.T ? e : r.T);
+        }
+        if (tb >= te) ++my_empties;
+        pkv_task t;
+        t.row = row; t.kvh = g; t.split = s; t.t_begin = tb; t.t_end = te;
+        a.tasks[idx] = t;
+    }
+    if (my_empties) atomicAdd(&empties_s, my_empties);
+    __syncthreads();
+    if (tid == 0) {
+        QueueHeader h;
+        h.num_tasks = (int32_t)lim;
+        h.max_row_splits = max_n_s;
+        h.total_row_slots = carry_s;
+        h.resolved_splits = a.S;
+        h.empty_tasks = empties_s;
+        h.work_counter = 0;
+        h.done_counter = 0;
+        h.error_word = total > a.tasks_cap ? 1 : 0;
+        h.sum_seq_lens = (int64_t)sum_seq_s;
+        h.pad_[0] = h.pad_[1] = h.pad_[2] = 0;
+        *a.hdr = h;
+    }
+}
+
+// One CTA per (row, kvh), one thread per (head in group, channel).  Rows with at most one slot
+// were written directly by the decode kernel.
+template <int G>
+__global__ void __launch_bounds__(G * kD) pkv_merge_kernel(const DecodeParams p) {
+    const int row = blockIdx.x / p.Hkv, kvh = blockIdx.x % p.Hkv;
+    const int so = p.split_offsets[row];
+    const int n = p.split_offsets[row + 1] - so;
+    if (n <= 1 && p.hdr != nullptr) return;   // library path: decode already produced out/lse
+    if (n <= 0) {                             // public pkv_merge: a row without states -> 0, -inf
+        const int64_t o = (int64_t)row * p.Hq + kvh * G + threadIdx.x / kD;
+        p.out[o * kD + threadIdx.x % kD] = __float2half_rn(0.f);
+        if (p.lse && threadIdx.x % kD == 0) p.lse[o] = -INFINITY;
+        return;
+    }
+    const int64_t base = (int64_t)so * p.Hkv + (int64_t)kvh * n;
+    merge_one<G>(p, base, n, row, kvh, threadIdx.x / kD, threadIdx.x % kD);
+}
+
+}  // namespace
+
+cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
+                           QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, pkv_task* tasks,
+                           int64_t tasks_cap, cudaStream_t stream) {
+    BuildArgs a;
+    a.seq_lens = seq_lens_dev;
+    a.hdr = hdr;
+    a.split_offsets = split_offsets;
+    a.fuse_counters = fuse_counters;
+    a.tasks = tasks;
+    a.tasks_cap = tasks_cap;
+    a.B = shape.B; a.Hkv = shape.Hkv; a.S = rp.S; a.tile_tokens = rp.tile_tokens;
+    a.split_mode = rp.split_mode; a.chunk_tiles = rp.chunk_tiles; a.route = rp.route;
+    pkv_build_workqueue_kernel<<<1, kBuildThreads, 0, stream>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
+    const int grid = p.B * p.Hkv;
+    if (grid <= 0) return cudaSuccess;
+    if (G == 4)
+        pkv_merge_kernel<4><<<grid, 4 * kD, 0, stream>>>(p);
+    else
+        pkv_merge_kernel<8><<<grid, 8 * kD, 0, stream>>>(p);
+    return cudaGetLastError();
+}
+
+}  // namespace pkv

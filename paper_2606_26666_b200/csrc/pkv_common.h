@@ -1,0 +1,89 @@
+// pkv_common.h -- internal declarations shared by the host planner and the CUDA translation
+// units of libpkv.  Not part of the ABI (include/pkv.h is).
+#pragma once
+
+#include <cstddef>
+#include <cstdint>
+
+#include "pkv.h"
+
+namespace pkv {
+
+constexpr int kD = 128;         // head dimension compiled in
+constexpr int kPage = 16;       // page size compiled in
+constexpr int kAutoCMin = 4;    // PAPER.md:85 "C_min = 4 CTAs/SM" (auto split rule, A12)
+constexpr int kMaxSplits = 256; // cap on S (and on n_i in FIXED_CHUNK mode)
+
+void set_error(const char* fmt, ...);
+void clear_error();
+
+inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Device-resident header at the front of the workspace (and of the host-planned queue image).
+// Written by the builder kernel (or by the host planner), read by decode / merge / counters.
+struct QueueHeader {
+    int32_t num_tasks;       // entries in the task list (rect route: includes empty intervals)
+    int32_t max_row_splits;  // max_i n_i (rect: S)
+    int32_t total_row_slots; // split_offsets[B]
+    int32_t resolved_splits; // S
+    int32_t empty_tasks;     // rect route: entries with t_begin >= t_end
+    int32_t work_counter;    // dynamic task scheduler; self-resetting
+    int32_t done_counter;    // CTAs that finished; self-resetting
+    int32_t error_word;      // reserved
+    int64_t sum_seq_lens;    // sum_i N_i
+    int64_t pad_[3];
+};
+static_assert(sizeof(QueueHeader) == 64, "QueueHeader layout");
+
+// Policy with every "0 = auto" field resolved.
+struct Resolved {
+    int32_t S;          // split count (FIXED_COUNT) or cap on n_i (FIXED_CHUNK)
+    int32_t tile_tokens;
+    int32_t split_mode;
+    int32_t chunk_tiles;
+    int32_t route;
+    int32_t merge_mode;
+    int32_t kernel;
+    int32_t G;
+};
+
+// Byte offsets inside the caller's workspace.  Pure function of (shape, S bound).
+struct WorkspaceLayout {
+    size_t header, split_offsets, fuse_counters, tasks, part_m, part_l, part_acc, total;
+    int64_t slots_cap; // B * Hkv * S
+};
+
+// Validates shape/policy (host-checkable part).  num_sms_or_0: SM count to use when the policy
+// says num_sms == 0 and num_splits == 0; if that is 0 too, S resolves to kMaxSplits when
+// `bound_ok`, else an error is returned.
+pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* policy,
+                                int num_sms_or_0, bool bound_ok, Resolved* out);
+WorkspaceLayout workspace_layout(const pkv_shape& shape, int32_t S);
+
+// Row-local split bounds (A6): T tiles, c tiles per split, n non-empty
+// splits.  Same integer formulas on host and device.
+struct RowSplits { int32_t T, c, n; };
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+inline RowSplits row_splits(int32_t N, int32_t tile_tokens, int32_t split_mode, int32_t S,
+                            int32_t chunk_tiles) {
+    RowSplits r;
+    r.T = N > 0 ? (N + tile_tokens - 1) / tile_tokens : 0;
+    if (r.T == 0) { r.c = 0; r.n = 0; return r; }
+    int32_t Si = S;
+    if (split_mode == PKV_SPLIT_FIXED_CHUNK) {
+        int32_t want = (r.T + chunk_tiles - 1) / chunk_tiles;
+        Si = want < S ? want : S;
+    }
+    r.c = (r.T + Si - 1) / Si;
+    r.n = (r.T + r.c - 1) / r.c;
+    return r;
+}
+
+// Host planner shared by pkv_build_workqueue_host and pkv_decode_host.
+pkv_status plan_host(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens,
+                     pkv_task* tasks, int32_t tasks_cap, int32_t* split_offsets, QueueHeader* hdr);
+
+}  // namespace pkv

@@ -1,0 +1,192 @@
+// pkv_host.cpp -- the pure-CPU part of libpkv: argument validation, policy resolution,
+// workspace layout and the host workqueue planner.  No CUDA here.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "pkv_common.h"
+
+namespace pkv {
+
+static thread_local char g_error[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_error, sizeof(g_error), fmt, ap);
+    va_end(ap);
+}
+void clear_error() { g_error[0] = 0; }
+
+pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* policy,
+                                int num_sms_or_0, bool bound_ok, Resolved* out) {
+    if (!shape || !policy || !out) { set_error("null shape/policy"); return PKV_ERR_INVALID_ARG; }
+    const pkv_shape& s = *shape;
+    const pkv_split_policy& p = *policy;
+    if (s.B < 0 || s.Hq <= 0 || s.Hkv <= 0 || s.d <= 0 || s.page_size <= 0 || s.max_pages < 0 ||
+        s.num_pages < 0) {
+        set_error("negative or zero dimension in pkv_shape");
+        return PKV_ERR_INVALID_ARG;
+    }
+    if (s.Hq % s.Hkv != 0) { set_error("Hq=%d is not a multiple of Hkv=%d", s.Hq, s.Hkv); return PKV_ERR_INVALID_ARG; }
+    if (s.d != kD) { set_error("d=%d not compiled in (d=128 only)", s.d); return PKV_ERR_UNSUPPORTED; }
+    if (s.page_size != kPage) { set_error("page_size=%d not compiled in (16 only)", s.page_size); return PKV_ERR_UNSUPPORTED; }
+    const int G = s.Hq / s.Hkv;
+    if (G != 4 && G != 8) { set_error("G=Hq/Hkv=%d not compiled in (4 and 8 only)", G); return PKV_ERR_UNSUPPORTED; }
+    const bool default_strides = s.kv_stride_page == 0 && s.kv_stride_token == 0 && s.kv_stride_head == 0;
+    if (!default_strides) {
+        if (s.kv_stride_page <= 0 || s.kv_stride_token <= 0 || s.kv_stride_head <= 0) {
+            set_error("kv strides must be all zero (default layout) or all positive");
+            return PKV_ERR_INVALID_ARG;
+        }
+        if (s.kv_stride_page % 8 || s.kv_stride_token % 8 || s.kv_stride_head % 8) {
+            set_error("kv strides must be multiples of 8 elements (16 bytes)");
+            return PKV_ERR_INVALID_ARG;
+        }
+    }
+    if (p.tile_tokens <= 0 || p.tile_tokens % s.page_size != 0) {
+        set_error("tile_tokens=%d must be a positive multiple of page_size=%d", p.tile_tokens, s.page_size);
+        return PKV_ERR_INVALID_ARG;
+    }
+    if (p.split_mode != PKV_SPLIT_FIXED_COUNT && p.split_mode != PKV_SPLIT_FIXED_CHUNK) {
+        set_error("bad split_mode %d", p.split_mode);
+        return PKV_ERR_INVALID_ARG;
+    }
+    if (p.num_splits < 0 || p.num_splits > kMaxSplits) {
+        set_error("num_splits=%d outside [0, %d]", p.num_splits, kMaxSplits);
+        return PKV_ERR_INVALID_ARG;
+    }
+    if (p.split_mode == PKV_SPLIT_FIXED_CHUNK && p.chunk_tiles <= 0) {
+        set_error("FIXED_CHUNK needs chunk_tiles > 0");
+        return PKV_ERR_INVALID_ARG;
+    }
+    if (p.route != PKV_ROUTE_RECT && p.route != PKV_ROUTE_WORKQUEUE) { set_error("bad route %d", p.route); return PKV_ERR_INVALID_ARG; }
+    if (p.merge_mode != PKV_MERGE_SEPARATE && p.merge_mode != PKV_MERGE_FUSED) { set_error("bad merge_mode %d", p.merge_mode); return PKV_ERR_INVALID_ARG; }
+    if (p.kernel < PKV_KERNEL_AUTO || p.kernel > PKV_KERNEL_SIMT) { set_error("bad kernel %d", p.kernel); return PKV_ERR_INVALID_ARG; }
+    if (p.num_sms < 0) { set_error("num_sms < 0"); return PKV_ERR_INVALID_ARG; }
+
+    int32_t S = p.num_splits;
+    if (S == 0) {
+        if (p.split_mode == PKV_SPLIT_FIXED_CHUNK) {
+            S = kMaxSplits;
+        } else {
+            int sms = p.num_sms > 0 ? p.num_sms : num_sms_or_0;
+            if (sms > 0) {
+                int64_t units = (int64_t)(s.B > 0 ? s.B : 1) * s.Hkv;
+                int64_t want = ceil_div64((int64_t)kAutoCMin * sms, units);
+                S = (int32_t)(want < 1 ? 1 : (want > kMaxSplits ? kMaxSplits : want));
+            } else if (bound_ok) {
+                S = kMaxSplits;
+            } else {
+                set_error("num_splits == 0 (auto) needs policy.num_sms > 0 in a host-only call");
+                return PKV_ERR_INVALID_ARG;
+            }
+        }
+    }
+    out->S = S;
+    out->tile_tokens = p.tile_tokens;
+    out->split_mode = p.split_mode;
+    out->chunk_tiles = p.chunk_tiles > 0 ? p.chunk_tiles : 1;
+    out->route = p.route;
+    out->merge_mode = p.merge_mode;
+    out->kernel = p.kernel == PKV_KERNEL_AUTO ? PKV_KERNEL_TMA_MMA : p.kernel;
+    out->G = G;
+    return PKV_OK;
+}
+
+WorkspaceLayout workspace_layout(const pkv_shape& s, int32_t S) {
+    WorkspaceLayout L;
+    const int G = s.Hq / s.Hkv;
+    L.slots_cap = (int64_t)s.B * s.Hkv * S;
+    size_t off = 0;
+    L.header = off;         off = align_up(off + sizeof(QueueHeader), 256);
+    L.split_offsets = off;  off = align_up(off + sizeof(int32_t) * ((size_t)s.B + 1), 256);
+    L.fuse_counters = off;  off = align_up(off + sizeof(int32_t) * ((size_t)s.B * s.Hkv + 1), 256);
+    L.tasks = off;          off = align_up(off + sizeof(pkv_task) * (size_t)L.slots_cap, 256);
+    L.part_m = off;         off = align_up(off + sizeof(float) * (size_t)L.slots_cap * G, 256);
+    L.part_l = off;         off = align_up(off + sizeof(float) * (size_t)L.slots_cap * G, 256);
+    L.part_acc = off;       off = align_up(off + sizeof(float) * (size_t)L.slots_cap * G * s.d, 256);
+    L.total = off;
+    return L;
+}
+
+pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_lens, pkv_task* tasks,
+                     int32_t tasks_cap, int32_t* split_offsets, QueueHeader* hdr) {
+    int64_t count = 0, sum_seq = 0;
+    int32_t max_n = 0, empties = 0, off = 0;
+    bool overflow = false;
+    if (split_offsets) split_offsets[0] = 0;
+    for (int32_t i = 0; i < s.B; ++i) {
+        const int32_t N = seq_lens[i] > 0 ? seq_lens[i] : 0;
+        sum_seq += N;
+        const RowSplits r = row_splits(N, rp.tile_tokens, rp.split_mode, rp.S, rp.chunk_tiles);
+        const int32_t slots = rp.route == PKV_ROUTE_WORKQUEUE ? r.n : rp.S;
+        if (slots > max_n) max_n = slots;
+        for (int32_t g = 0; g < s.Hkv; ++g) {
+            for (int32_t sp = 0; sp < slots; ++sp) {
+                int32_t tb = 0, te = 0;
+                if (r.T > 0) {
+                    int64_t b = (int64_t)sp * r.c, e = (int64_t)(sp + 1) * r.c;
+                    tb = (int32_t)(b < r.T ? b : r.T);
+                    te = (int32_t)(e < r.T ? e : r.T);
+                }
+                if (tb >= te) ++empties;
+                if (count < tasks_cap && tasks) {
+                    pkv_task t = {i, g, sp, tb, te};
+                    tasks[count] = t;
+                } else {
+                    overflow = true;
+                }
+                ++count;
+            }
+        }
+        off += slots;
+        if (split_offsets) split_offsets[i + 1] = off;
+    }
+    if (hdr) {
+        std::memset(hdr, 0, sizeof(*hdr));
+        hdr->num_tasks = (int32_t)count;
+        hdr->max_row_splits = max_n;
+        hdr->total_row_slots = off;
+        hdr->resolved_splits = rp.S;
+        hdr->empty_tasks = empties;
+        hdr->sum_seq_lens = sum_seq;
+    }
+    if (overflow && tasks) return PKV_ERR_WORKSPACE;
+    return PKV_OK;
+}
+
+}  // namespace pkv
+
+using namespace pkv;
+
+extern "C" {
+
+int32_t pkv_version(void) { return (1 << 16) | 0; }
+const char* pkv_last_error(void) { return g_error; }
+
+size_t pkv_workspace_bytes(const pkv_shape* shape, const pkv_split_policy* policy) {
+    Resolved rp;
+    if (validate_and_resolve(shape, policy, 0, /*bound_ok=*/true, &rp) != PKV_OK) return 0;
+    return workspace_layout(*shape, rp.S).total;
+}
+
+pkv_status pkv_build_workqueue_host(const pkv_shape* shape, const pkv_split_policy* policy,
+                                    const int32_t* seq_lens_host, pkv_task* tasks_out, int32_t tasks_cap,
+                                    int32_t* split_offsets_out, int32_t* num_tasks_out) {
+    clear_error();
+    Resolved rp;
+    pkv_status st = validate_and_resolve(shape, policy, 0, /*bound_ok=*/false, &rp);
+    if (st != PKV_OK) return st;
+    if ((!seq_lens_host && shape->B > 0) || !num_tasks_out || tasks_cap < 0 || (tasks_cap > 0 && !tasks_out)) {
+        set_error("null pointer in pkv_build_workqueue_host");
+        return PKV_ERR_INVALID_ARG;
+    }
+    QueueHeader hdr;
+    st = plan_host(*shape, rp, seq_lens_host, tasks_out, tasks_cap, split_offsets_out, &hdr);
+    *num_tasks_out = hdr.num_tasks;
+    if (st == PKV_ERR_WORKSPACE) set_error("tasks_cap=%d < %d tasks", tasks_cap, hdr.num_tasks);
+    return st;
+}
+
+}  // extern "C"
