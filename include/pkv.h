@@ -203,9 +203,10 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
                                    size_t scratch_bytes, void* workspace, size_t workspace_bytes,
                                    void* stream, pkv_counters* counters_out);
 
-/* Test hook: tensor-map form used by the TMA kernel for maps encoded after the call.
- * -1 = automatic (rank-5 box, falling back to two rank-4 boxes), 0 = rank 5, 1 = rank 4. */
-PKV_API void pkv_debug_force_tma_mode(int mode);
+/* Test hook: KV heads one CTA of the TMA kernel streams together.
+ * 0 = automatic (largest of 8/4/2/1 dividing Hkv that leaves >= one work unit per SM), else
+ * 1, 2, 4 or 8 (ignored when it does not divide Hkv).  Process-wide. */
+PKV_API void pkv_debug_force_heads_per_cta(int heads);
 
 #ifdef __cplusplus
 }

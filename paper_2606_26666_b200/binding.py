@@ -53,7 +53,7 @@ class pkv_counters(ctypes.Structure):
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_build_workqueue_host",
            "pkv_build_workqueue", "pkv_decode", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
-           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_tma_mode")
+           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_heads_per_cta")
 
 
 class PkvError(RuntimeError):
@@ -94,8 +94,8 @@ def _load() -> ctypes.CDLL:
     lib.pkv_decode_host.restype = _i32
     lib.pkv_decode_host.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float,
                                     _vp, _vp, ctypes.c_size_t, _vp, ctypes.c_size_t, _vp, P(pkv_counters)]
-    lib.pkv_debug_force_tma_mode.restype = None
-    lib.pkv_debug_force_tma_mode.argtypes = [ctypes.c_int]
+    lib.pkv_debug_force_heads_per_cta.restype = None
+    lib.pkv_debug_force_heads_per_cta.argtypes = [ctypes.c_int]
     return lib
 
 
@@ -265,5 +265,5 @@ def pkv_decode_host(shape: Shape, policy: Policy, q_host, k_cache_dev, v_cache_d
     return c.as_dict()
 
 
-def pkv_debug_force_tma_mode(mode: int) -> None:
-    _lib.pkv_debug_force_tma_mode(int(mode))
+def pkv_debug_force_heads_per_cta(heads: int) -> None:
+    _lib.pkv_debug_force_heads_per_cta(int(heads))

@@ -14,7 +14,7 @@ namespace pkv {
 
 namespace {
 
-int g_force_tma_mode = -1;  // test hook: -1 auto, 0 = 5-D box, 1 = 4-D half boxes
+int g_force_hg = 0;  // test hook: 0 = automatic heads-per-CTA, else 1/2/4/8
 
 int device_sm_count() {
     thread_local int cache[64];
@@ -69,35 +69,19 @@ Strides effective_strides(const pkv_shape& s) {
     return {s.kv_stride_page, s.kv_stride_token, s.kv_stride_head};
 }
 
-// tma_mode: 0 = rank 5 (64 ch, 16 tok, 2 ch-halves, head, page), one 4 KiB box per (page, head);
-//           1 = rank 4 (128 ch, 16 tok, head, page), 2 = rank 4 (128 ch, head, 16 tok, page): two
-//           2 KiB boxes per (page, head), dimensions ordered by stride.
-bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int mode, CUtensorMap* out) {
+// Rank-5 tensor map over one cache: dims (64 ch, 16 tok, 2 ch-halves, Hkv heads, pages), strides
+// from the caller's layout, box (64, 16, 2, HG, 1): the HG-head slice of one page, landing in
+// shared memory as [head][ch-half][tok][64 ch] with the 128-byte swizzle (conflict-free ldmatrix).
+bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int HG, CUtensorMap* out) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t pages = (cuuint64_t)(s.num_pages > 0 ? s.num_pages : 1);
-    cuuint64_t dims[5], strides[4];
-    cuuint32_t box[5], estr[5] = {1, 1, 1, 1, 1};
-    cuuint32_t rank;
-    if (mode == 0) {
-        rank = 5;
-        dims[0] = 64; dims[1] = 16; dims[2] = 2; dims[3] = (cuuint64_t)s.Hkv; dims[4] = pages;
-        strides[0] = (cuuint64_t)st.token * 2; strides[1] = 128; strides[2] = (cuuint64_t)st.head * 2;
-        strides[3] = (cuuint64_t)st.page * 2;
-        box[0] = 64; box[1] = 16; box[2] = 2; box[3] = 1; box[4] = 1;
-    } else if (mode == 1) {
-        rank = 4;
-        dims[0] = 128; dims[1] = 16; dims[2] = (cuuint64_t)s.Hkv; dims[3] = pages;
-        strides[0] = (cuuint64_t)st.token * 2; strides[1] = (cuuint64_t)st.head * 2; strides[2] = (cuuint64_t)st.page * 2;
-        box[0] = 64; box[1] = 16; box[2] = 1; box[3] = 1;
-    } else {
-        rank = 4;
-        dims[0] = 128; dims[1] = (cuuint64_t)s.Hkv; dims[2] = 16; dims[3] = pages;
-        strides[0] = (cuuint64_t)st.head * 2; strides[1] = (cuuint64_t)st.token * 2; strides[2] = (cuuint64_t)st.page * 2;
-        box[0] = 64; box[1] = 1; box[2] = 16; box[3] = 1;
-    }
-    const CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, rank, const_cast<void*>(base), dims, strides, box,
-                          estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+    cuuint64_t dims[5] = {64, 16, 2, (cuuint64_t)s.Hkv, pages};
+    cuuint64_t strides[4] = {(cuuint64_t)st.token * 2, 128, (cuuint64_t)st.head * 2, (cuuint64_t)st.page * 2};
+    cuuint32_t box[5] = {64, 16, 2, (cuuint32_t)HG, 1};
+    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 5, const_cast<void*>(base), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
 }
@@ -105,37 +89,41 @@ bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int mod
 struct MapCacheEntry {
     const void* base;
     int64_t num_pages, sp, st, sh;
-    int32_t Hkv, mode;
+    int32_t Hkv, HG;
     CUtensorMap map;
 };
 
-// Returns the tensor map of `base` (encoding it on first use) and the mode it was encoded in.
-const CUtensorMap* get_map(const void* base, const pkv_shape& s, int* mode_out) {
-    thread_local std::vector<MapCacheEntry> cache;
-    thread_local size_t next = 0;
+// Returns the tensor map of `base` for HG heads per box, encoding it on first use (per thread).
+const CUtensorMap* get_map(const void* base, const pkv_shape& s, int HG) {
+    constexpr int kCap = 32;
+    thread_local MapCacheEntry cache[kCap];   // fixed storage: returned pointers stay valid
+    thread_local int count = 0, next = 0;
     const Strides st = effective_strides(s);
-    for (const MapCacheEntry& e : cache)
+    for (int i = 0; i < count; ++i) {
+        const MapCacheEntry& e = cache[i];
         if (e.base == base && e.num_pages == s.num_pages && e.sp == st.page && e.st == st.token && e.sh == st.head &&
-            e.Hkv == s.Hkv && (g_force_tma_mode < 0 || (g_force_tma_mode == 0) == (e.mode == 0))) {
-            *mode_out = e.mode;
+            e.Hkv == s.Hkv && e.HG == HG)
             return &e.map;
-        }
-    MapCacheEntry e;
-    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv;
-    bool ok = false;
-    if (g_force_tma_mode != 1) { e.mode = 0; ok = encode_map(base, s, st, 0, &e.map); }
-    if (!ok) { e.mode = st.head < st.token ? 2 : 1; ok = encode_map(base, s, st, e.mode, &e.map); }
-    if (!ok) return nullptr;
-    if (cache.size() < 16) {
-        cache.push_back(e);
-        *mode_out = e.mode;
-        return &cache.back().map;
     }
-    cache[next] = e;
-    const CUtensorMap* r = &cache[next].map;
-    next = (next + 1) % cache.size();
-    *mode_out = e.mode;
-    return r;
+    MapCacheEntry e;
+    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv; e.HG = HG;
+    if (!encode_map(base, s, st, HG, &e.map)) return nullptr;
+    const int slot = count < kCap ? count++ : (next = (next + 1) % kCap);
+    cache[slot] = e;
+    return &cache[slot].map;
+}
+
+// KV heads one CTA streams together: the largest divisor of Hkv in {8, 4, 2, 1} that still
+// leaves at least one work unit per SM (units = row slots x Hkv / HG).
+int choose_heads_per_cta(int Hkv, int64_t row_slots, int num_sms) {
+    if (g_force_hg > 0 && Hkv % g_force_hg == 0) return g_force_hg;
+    int best = 1;
+    for (int hg = 8; hg >= 1; hg >>= 1) {
+        if (hg > Hkv || Hkv % hg) continue;
+        best = hg;
+        if (row_slots * (Hkv / hg) >= num_sms) return hg;
+    }
+    return best;   // nothing fills the machine: smallest valid group = most units
 }
 
 pkv_status cuda_fail(cudaError_t e, const char* what) {
@@ -179,7 +167,8 @@ pkv_status check_workspace(const void* workspace, size_t bytes, const WorkspaceL
 // so launches that have nothing to do are skipped (A13).
 pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, const void* k_cache, const void* v_cache,
                       const int32_t* block_table, const int32_t* seq_lens, void* out, float* lse, float scale,
-                      const QueuePtrs& qp, const WsPtrs& ws, int64_t known_tasks, int known_max_n, int num_sms,
+                      const QueuePtrs& qp, const WsPtrs& ws, int64_t known_tasks, int known_max_n, int64_t known_slots,
+                      int num_sms,
                       cudaStream_t stream, int* decode_launches, int* merge_launches) {
     DecodeParams p;
     std::memset(&p, 0, sizeof(p));
@@ -224,16 +213,18 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     }
     if (known_tasks != 0) {
         if (rp.kernel == PKV_KERNEL_TMA_MMA) {
-            int mode_k = 0, mode_v = 0;
-            const CUtensorMap* mk = get_map(k_cache, s, &mode_k);
-            const CUtensorMap* mv = get_map(v_cache, s, &mode_v);
-            if (!mk || !mv || mode_k != mode_v) {
+            const int64_t row_slots = known_slots >= 0 ? known_slots : (int64_t)s.B * rp.S;
+            const int HG = choose_heads_per_cta(s.Hkv, row_slots, num_sms);
+            const CUtensorMap* mk = get_map(k_cache, s, HG);
+            const CUtensorMap* mv = get_map(v_cache, s, HG);
+            if (!mk || !mv) {
                 set_error("cuTensorMapEncodeTiled failed for the K/V cache (base %p/%p)", k_cache, v_cache);
                 return PKV_ERR_CUDA;
             }
-            p.tma_rank = mode_k;  // 0: 5-D, 1/2: 4-D dimension orders
-            const int grid = (int)(bound < num_sms ? bound : num_sms);
-            e = launch_decode_tma(p, rp.G, grid, mk, mv, stream);
+            p.heads_per_cta = HG;
+            const int64_t units = row_slots * (s.Hkv / HG);
+            const int grid = (int)(units < num_sms ? units : num_sms);
+            e = launch_decode_tma(p, rp.G, HG, grid, mk, mv, stream);
         } else {
             const int64_t cap = (int64_t)num_sms * 4;
             const int grid = (int)(bound < cap ? bound : cap);
@@ -270,8 +261,7 @@ using namespace pkv;
 
 extern "C" {
 
-// test hook (not in pkv.h): force the tensor-map mode of the next encodes
-PKV_API void pkv_debug_force_tma_mode(int mode) { g_force_tma_mode = mode; }
+void pkv_debug_force_heads_per_cta(int hg) { g_force_hg = hg; }
 
 pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_policy* policy, const int32_t* seq_lens_dev,
                                void* workspace, size_t workspace_bytes, void* stream) {
@@ -311,7 +301,7 @@ pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, co
                                              ws.q.tasks, L.slots_cap, cs);
         if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     }
-    return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, out, lse, scale, ws.q, ws, -1, -1, sms,
+    return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, out, lse, scale, ws.q, ws, -1, -1, -1, sms,
                       cs, nullptr, nullptr);
 }
 
@@ -520,7 +510,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     int dl = 0, ml = 0;
     st = run_decode(s, rp, ds + im.q, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
                     reinterpret_cast<const int32_t*>(ds + im.seq_lens), ds + im.out, nullptr, scale, qp, ws,
-                    hdr->num_tasks, hdr->max_row_splits, sms, cs, &dl, &ml);
+                    hdr->num_tasks, hdr->max_row_splits, hdr->total_row_slots, sms, cs, &dl, &ml);
     if (st != PKV_OK) return st;
     const size_t out_bytes = 2 * (size_t)s.B * s.Hq * s.d;
     e = cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);

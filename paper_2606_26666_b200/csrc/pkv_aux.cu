@@ -124,22 +124,36 @@ __global__ void __launch_bounds__(kBuildThreads) pkv_build_workqueue_kernel(cons
     }
 }
 
-// One CTA per (row, kvh), one thread per (head in group, channel).  Rows with at most one slot
-// were written directly by the decode kernel.
+// One CTA of 4 warps per (row, query head): warp k computes the interleaved partial P_k of
+// pkv_device.cuh's merge arithmetic, warp 0 combines the four in order.  Rows with at most one
+// slot were written directly by the decode kernel.
 template <int G>
-__global__ void __launch_bounds__(G * kD) pkv_merge_kernel(const DecodeParams p) {
-    const int row = blockIdx.x / p.Hkv, kvh = blockIdx.x % p.Hkv;
+__global__ void __launch_bounds__(128) pkv_merge_kernel(const DecodeParams p) {
+    __shared__ float4 sA[4][32];
+    __shared__ float sL[4];
+    const int row = blockIdx.x / p.Hq, h = blockIdx.x % p.Hq;
+    const int kvh = h / G, hh = h % G;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int so = p.split_offsets[row];
     const int n = p.split_offsets[row + 1] - so;
     if (n <= 1 && p.hdr != nullptr) return;   // library path: decode already produced out/lse
-    if (n <= 0) {                             // public pkv_merge: a row without states -> 0, -inf
-        const int64_t o = (int64_t)row * p.Hq + kvh * G + threadIdx.x / kD;
-        p.out[o * kD + threadIdx.x % kD] = __float2half_rn(0.f);
-        if (p.lse && threadIdx.x % kD == 0) p.lse[o] = -INFINITY;
-        return;
-    }
     const int64_t base = (int64_t)so * p.Hkv + (int64_t)kvh * n;
-    merge_one<G>(p, base, n, row, kvh, threadIdx.x / kD, threadIdx.x % kD);
+    const float M = merge_row_max<G>(p, base, n, hh, lane);
+    float L;
+    float4 A;
+    merge_partial<G>(p, base, n, hh, M, warp, lane, L, A);
+    sA[warp][lane] = A;
+    if (lane == 0) sL[warp] = L;
+    __syncthreads();
+    if (warp == 0) {
+        const float Ls = ((sL[0] + sL[1]) + sL[2]) + sL[3];
+        float4 As;
+        As.x = ((sA[0][lane].x + sA[1][lane].x) + sA[2][lane].x) + sA[3][lane].x;
+        As.y = ((sA[0][lane].y + sA[1][lane].y) + sA[2][lane].y) + sA[3][lane].y;
+        As.z = ((sA[0][lane].z + sA[1][lane].z) + sA[2][lane].z) + sA[3][lane].z;
+        As.w = ((sA[0][lane].w + sA[1][lane].w) + sA[2][lane].w) + sA[3][lane].w;
+        merge_store(p, (int64_t)row * p.Hq + h, lane, M, Ls, As);
+    }
 }
 
 }  // namespace
@@ -161,12 +175,12 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
 }
 
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
-    const int grid = p.B * p.Hkv;
+    const int grid = p.B * p.Hq;
     if (grid <= 0) return cudaSuccess;
     if (G == 4)
-        pkv_merge_kernel<4><<<grid, 4 * kD, 0, stream>>>(p);
+        pkv_merge_kernel<4><<<grid, 128, 0, stream>>>(p);
     else
-        pkv_merge_kernel<8><<<grid, 8 * kD, 0, stream>>>(p);
+        pkv_merge_kernel<8><<<grid, 128, 0, stream>>>(p);
     return cudaGetLastError();
 }
 

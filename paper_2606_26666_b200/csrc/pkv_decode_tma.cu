@@ -1,26 +1,31 @@
 // pkv_decode_tma.cu -- PKV_KERNEL_TMA_MMA: the B200 decode kernel.
 //
-// Persistent, warp-specialised CTA, one per SM (PAPER.md:42 maps one CTA to one (request, KV
-// head, split) work item; here a resident CTA walks many such tasks -- DESIGN.md A20):
+// Persistent, warp-specialised CTA, one per SM.  The paper maps one CTA to one (request, KV head,
+// split) work item; here a resident CTA walks many work UNITS, a unit being the HG
+// tasks (row, kvh = hg*HG .. hg*HG+HG-1, split) of the workqueue that share a tile interval
+// (DESIGN.md "CTA mapping").  With HG = Hkv = 8 a unit streams whole pages: one page of K (or V)
+// is ONE contiguous 32 KiB TMA box in the default [page, token, head, d] layout.
 //
-//   warp 0 (producer)    takes tasks (static stride or an atomic counter), walks the task's
-//                        slice of the block table (PAPER.md:50 page accessor) 32 entries at a
-//                        time, and for every page issues ONE TMA box for K and one for V: the
-//                        page's 16 tokens x 128 channels of the task's KV head, 4 KiB each,
-//                        128-byte swizzled, into a ring of kStages 8 KiB stages guarded by
-//                        full/empty mbarriers.  It runs ahead across task boundaries, so the
-//                        ring never drains between tasks.
-//   warps 1..8 (compute) page j of a task belongs to warp j % 8.  Per page:
-//                        S^T[16 tok x 8 heads] = K[16 x 128] . Q^T      8 HMMA m16n8k16
-//                        exact online softmax in FP32, P -> FP16
-//                        O^T[128 x 8 heads]  += V^T[128 x 16] . P^T     8 HMMA m16n8k16
+//   producer warps (NP)  producer 0 takes units (first by block index, then from an atomic
+//                        counter), resolves (row, split) and publishes the unit on a small
+//                        ring.  Every producer walks its share of the unit's slice of the
+//                        block table (PAPER.md:50 page accessor), 32 entries per load, and per
+//                        page issues one TMA box for K and one for V -- 16 tokens x HG heads x
+//                        128 channels, 128-byte swizzled -- into a ring of stages guarded by
+//                        full(K)/full(V)/empty mbarriers.  Producers run ahead across unit
+//                        boundaries, so the ring never drains between units.
+//   compute warps (8)    warp cw serves head cw % HG; the 8/HG warps of a head take pages
+//                        round-robin.  Per page and head:
+//                          S^T[16 tok x 8 heads] = K[16 x 128] . Q^T      8 HMMA m16n8k16
+//                          exact online softmax in FP32, P -> FP16
+//                          O^T[128 x 8 heads]  += V^T[128 x 16] . P^T     8 HMMA m16n8k16
 //                        Tokens sit on the MMA M axis and the G <= 8 grouped query heads
 //                         on the N = 8 axis, so G = 8 fills the tile and G = 4
 //                        half of it; K is read with ldmatrix, V with ldmatrix.trans, P^T is
-//                        produced from the S^T accumulator layout with movmatrix.
-//   task end             the 8 warp states are combined through shared memory and stored as
-//                        the split's partial state, or directly as FP16 output when the row
-//                        has a single split (pkv_device.cuh finalize_task).
+//                        made from the S^T accumulator layout with movmatrix.
+//   unit end             the warps of a head combine their states through shared memory and
+//                        store the task's partial state, or the FP16 output directly when the
+//                        row has a single split (pkv_device.cuh finalize_task).
 #include <cuda.h>
 
 #include "pkv_device.cuh"
@@ -30,35 +35,47 @@ namespace pkv {
 namespace {
 
 constexpr int kComputeWarps = 8;
-constexpr int kThreadsTma = (1 + kComputeWarps) * 32;
-constexpr int kComputeThreads = kComputeWarps * 32;
-constexpr int kStageBytes = 8192;   // K 4096 | V 4096
-constexpr int kRing = 4;            // task-id ring between producer and compute warps
-constexpr int kBarCompute = 1;      // named barrier of the compute warps
+constexpr int kRing = 4;            // unit ring between producer 0 and everybody else
+constexpr int kMaxStages = 24;
+
+__host__ __device__ constexpr int producers_for(int HG) { return HG >= 4 ? 1 : (HG == 2 ? 2 : 4); }
+
+struct UnitInfo {
+    int unit;   // -1: no more work
+    int row;
+};
 
 template <int G>
 struct SmemTail {
     CombineBuf<G, kComputeWarps> cb;
-    unsigned long long full_bar[32];   // kStages <= 32
-    unsigned long long empty_bar[32];
+    unsigned long long full_k[kMaxStages];
+    unsigned long long full_v[kMaxStages];
+    unsigned long long empty_bar[kMaxStages];
     unsigned long long ring_full[kRing];
     unsigned long long ring_empty[kRing];
-    int task_ring[kRing];
+    UnitInfo ring[kRing];
 };
 
-template <int G>
+template <int G, int HG>
 __host__ __device__ constexpr int stages_for() {
     // 227 KiB per CTA, minus the tail, minus 1 KiB alignment slack
-    return (int)((232448 - 1024 - (int)sizeof(SmemTail<G>)) / kStageBytes) > 32
-               ? 32
-               : (int)((232448 - 1024 - (int)sizeof(SmemTail<G>)) / kStageBytes);
+    constexpr int avail = 232448 - 1024 - (int)sizeof(SmemTail<G>);
+    constexpr int n = avail / (HG * 8192);
+    constexpr int capped = n > kMaxStages ? kMaxStages : n;
+    // a multiple of the producer count, so that a stage always belongs to the same producer:
+    // two producers sharing a stage could pass each other on its parity-only empty barrier
+    return capped / producers_for(HG) * producers_for(HG);
 }
 
-template <int G>
-__global__ void __launch_bounds__(kThreadsTma, 1)
+template <int G, int HG>
+__global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
     pkv_decode_tma_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap_k,
                           const __grid_constant__ CUtensorMap tmap_v) {
-    constexpr int kStages = stages_for<G>();
+    constexpr int kStages = stages_for<G, HG>();
+    constexpr int kStageBytes = HG * 8192;   // K: HG x 4096 | V: HG x 4096
+    constexpr int NP = producers_for(HG);
+    constexpr int WPH = kComputeWarps / HG;  // warps per head
+    static_assert(kStages >= 2, "ring too small");
     extern __shared__ unsigned char smem_raw[];
     // 128-byte swizzle: every 2 KiB half-box must start on a 1024-byte boundary
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -66,19 +83,21 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t stage_base = smem_u32(smem);
-    const uint32_t full0 = smem_u32(&tail.full_bar[0]);
+    const uint32_t fullk0 = smem_u32(&tail.full_k[0]);
+    const uint32_t fullv0 = smem_u32(&tail.full_v[0]);
     const uint32_t empty0 = smem_u32(&tail.empty_bar[0]);
     const uint32_t rfull0 = smem_u32(&tail.ring_full[0]);
     const uint32_t rempty0 = smem_u32(&tail.ring_empty[0]);
 
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) {
-            mbar_init(full0 + 8 * s, 1);
-            mbar_init(empty0 + 8 * s, 1);
+            mbar_init(fullk0 + 8 * s, 1);
+            mbar_init(fullv0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, HG);    // one arrival per head of the page
         }
         for (int r = 0; r < kRing; ++r) {
             mbar_init(rfull0 + 8 * r, 1);
-            mbar_init(rempty0 + 8 * r, kComputeWarps);
+            mbar_init(rempty0 + 8 * r, kComputeWarps + NP - 1);
         }
         mbar_fence_init();
         tma_prefetch_desc(&tmap_k);
@@ -87,12 +106,15 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
     zero_empty_rows(p);
     __syncthreads();
 
-    const int num_tasks = p.hdr->num_tasks;
+    const int HGn = p.Hkv / HG;                               // head groups per (row, split)
+    const int num_units = p.hdr->total_row_slots * HGn;
 
-    if (warp == 0) {
-        // ================================================================ producer warp
-        uint32_t seq = 0;  // pages issued by this CTA so far
-        for (int k = 0;; ++k) {
+    // ---- unit hand-out (producer 0) / pick-up (everybody else) -------------------------------
+    int cur_row = 0;   // producer 0: units arrive in increasing order, so the row only moves forward
+    auto next_unit = [&](int k) -> UnitInfo {
+        const int r = k % kRing;
+        UnitInfo u;
+        if (warp == 0) {
             int t;
             if (k == 0 || !p.dynamic_sched) {
                 t = blockIdx.x + k * gridDim.x;
@@ -101,57 +123,70 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
                 if (lane == 0) t = atomicAdd(&p.hdr->work_counter, 1) + gridDim.x;
                 t = __shfl_sync(0xffffffffu, t, 0);
             }
-            if (t >= num_tasks) t = -1;
-            const int r = k % kRing;
+            if (t >= num_units) t = -1;
+            if (t >= 0) {
+                const int rs = t / HGn;
+                while (p.split_offsets[cur_row + 1] <= rs) ++cur_row;
+            }
+            u.unit = t;
+            u.row = cur_row;
             if (lane == 0) {
                 mbar_wait(rempty0 + 8 * r, ((k / kRing) & 1) ^ 1);
-                tail.task_ring[r] = t;
+                tail.ring[r] = u;
                 mbar_arrive(rfull0 + 8 * r);
             }
-            if (t < 0) break;
-            const pkv_task task = p.tasks[t];
-            const int N = p.seq_lens[task.row];
+        } else {
+            mbar_wait(rfull0 + 8 * r, (k / kRing) & 1);
+            u = tail.ring[r];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(rempty0 + 8 * r);
+        }
+        return u;
+    };
+
+    if (warp < NP) {
+        // ================================================================ producer warps
+        uint32_t seq_base = 0;  // pages of earlier units of this CTA
+        for (int k = 0;; ++k) {
+            const UnitInfo u = next_unit(k);
+            if (u.unit < 0) break;
+            const int row = u.row, hg = u.unit % HGn;
+            const int so = p.split_offsets[row];
+            const int split = u.unit / HGn - so;
+            const pkv_task task = p.tasks[(int64_t)so * p.Hkv + split];   // the kvh = 0 task of (row, split)
+            const int N = p.seq_lens[row];
             const int tok0 = task.t_begin * p.tile_tokens;
             const int tok1 = min(task.t_end * p.tile_tokens, N);
             if (tok0 >= tok1) continue;  // empty split: nothing is staged
             const int p0 = tok0 >> 4;
             const int np = ((tok1 + 15) >> 4) - p0;
-            const int32_t* bt = p.block_table + (int64_t)task.row * p.max_pages + p0;
-            int mine = (lane < np) ? bt[lane] : 0;
-            for (int c = 0; c < np; c += 32) {
-                // next 32 table entries are fetched while this batch of boxes is issued
-                const int nxt = (c + 32 + lane < np) ? bt[c + 32 + lane] : 0;
-                const int cnt = min(32, np - c);
-                for (int j = 0; j < cnt; ++j) {
-                    const int page = __shfl_sync(0xffffffffu, mine, j);
+            const int32_t* bt = p.block_table + (int64_t)row * p.max_pages + p0;
+            const int head0 = hg * HG;
+            // this producer's pages: j = warp, warp + NP, ...; table entries 32 at a time
+            int mine = (warp + lane * NP < np) ? bt[warp + lane * NP] : 0;
+            for (int c = warp; c < np; c += 32 * NP) {
+                const int nxt = (c + (32 + lane) * NP < np) ? bt[c + (32 + lane) * NP] : 0;
+                const int cnt = min(32, (np - c + NP - 1) / NP);
+                for (int i = 0; i < cnt; ++i) {
+                    const int page = __shfl_sync(0xffffffffu, mine, i);
                     if (lane == 0) {
-                        const uint32_t s = seq % kStages;
-                        const uint32_t use = seq / kStages;
-                        mbar_wait(empty0 + 8 * s, (use & 1) ^ 1);
-                        const uint32_t fb = full0 + 8 * s;
+                        const uint32_t sq = seq_base + c + i * NP;
+                        const uint32_t s = sq % kStages;
+                        mbar_wait(empty0 + 8 * s, ((sq / kStages) & 1) ^ 1);
                         const uint32_t dst = stage_base + s * kStageBytes;
-                        mbar_arrive_expect_tx(fb, kStageBytes);
-                        if (p.tma_rank == 0) {
-                            // dims: (64 ch, 16 tok, 2 ch-halves, head, page)
-                            tma_load_5d(dst, &tmap_k, fb, 0, 0, 0, task.kvh, page);
-                            tma_load_5d(dst + 4096, &tmap_v, fb, 0, 0, 0, task.kvh, page);
-                        } else {
-                            // dims: (128 ch, 16 tok, head, page) or (128 ch, head, 16 tok, page); box 64 ch wide
-                            const int c1 = p.tma_rank == 1 ? 0 : task.kvh;
-                            const int c2 = p.tma_rank == 1 ? task.kvh : 0;
-                            tma_load_4d(dst, &tmap_k, fb, 0, c1, c2, page);
-                            tma_load_4d(dst + 2048, &tmap_k, fb, 64, c1, c2, page);
-                            tma_load_4d(dst + 4096, &tmap_v, fb, 0, c1, c2, page);
-                            tma_load_4d(dst + 6144, &tmap_v, fb, 64, c1, c2, page);
-                        }
+                        // box dims: (64 ch, 16 tok, 2 ch-halves, HG heads, 1 page)
+                        mbar_arrive_expect_tx(fullk0 + 8 * s, HG * 4096);
+                        tma_load_5d(dst, &tmap_k, fullk0 + 8 * s, 0, 0, 0, head0, page);
+                        mbar_arrive_expect_tx(fullv0 + 8 * s, HG * 4096);
+                        tma_load_5d(dst + HG * 4096, &tmap_v, fullv0 + 8 * s, 0, 0, 0, head0, page);
                     }
-                    ++seq;
                 }
                 mine = nxt;
             }
+            seq_base += np;
         }
-        // the last CTA to run out of tasks re-arms the counters for the next launch / replay
-        if (lane == 0) {
+        // the last CTA to run out of units re-arms the counters for the next launch / replay
+        if (warp == 0 && lane == 0) {
             const int old = atomicAdd(&p.hdr->done_counter, 1);
             if (old == (int)gridDim.x - 1) {
                 p.hdr->work_counter = 0;
@@ -160,12 +195,14 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
         }
     } else {
         // ================================================================ compute warps
-        const int cw = warp - 1;             // 0..7
-        const int ctid = tid - 32;           // 0..255
+        const int cw = warp - NP;            // 0..7
+        const int hl = cw % HG;              // head within the unit's head group
+        const int sub = cw / HG;             // which of the head's WPH warps
+        const int gtid = sub * 32 + lane;    // thread index within the head's warp group
         const int g4 = lane >> 2;            // fragment "groupID"
         const int t4 = lane & 3;             // fragment "threadID_in_group"
-        const int hA = 2 * t4, hB = 2 * t4 + 1;   // the two heads (MMA N columns) this lane tracks
-        // ldmatrix lane addressing inside a stage (see header comment)
+        const int hA = 2 * t4, hB = 2 * t4 + 1;   // the two query heads (MMA N columns) this lane tracks
+        // ldmatrix lane addressing inside a head's 4 KiB [2 halves][16 tok][64 ch] block
         const uint32_t k_tok = (lane & 7) + ((lane >> 3) & 1) * 8;
         const uint32_t k_sel = lane >> 4;
         const uint32_t v_tok = ((lane >> 4) << 3) + (lane & 7);
@@ -174,22 +211,20 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
 
         uint32_t seq_base = 0;
         for (int k = 0;; ++k) {
-            const int r = k % kRing;
-            mbar_wait(rfull0 + 8 * r, (k / kRing) & 1);
-            const int t = tail.task_ring[r];
-            __syncwarp();
-            if (lane == 0) mbar_arrive(rempty0 + 8 * r);
-            if (t < 0) break;
-            const pkv_task task = p.tasks[t];
-            const int row = task.row, kvh = task.kvh;
-            const int N = p.seq_lens[row];
+            const UnitInfo u = next_unit(k);
+            if (u.unit < 0) break;
+            const int row = u.row, hg = u.unit % HGn;
             const int so = p.split_offsets[row];
             const int n_i = p.split_offsets[row + 1] - so;
-            const int64_t slot = (int64_t)so * p.Hkv + (int64_t)kvh * n_i + task.split;
+            const int split = u.unit / HGn - so;
+            const pkv_task task = p.tasks[(int64_t)so * p.Hkv + split];
+            const int kvh = hg * HG + hl;
+            const int64_t slot = (int64_t)so * p.Hkv + (int64_t)kvh * n_i + split;
+            const int N = p.seq_lens[row];
             const int tok0 = task.t_begin * p.tile_tokens;
             const int tok1 = min(task.t_end * p.tile_tokens, N);
             if (tok0 >= tok1) {
-                store_empty_task<G>(p, row, kvh, n_i, slot, ctid, kComputeThreads);
+                store_empty_task<G>(p, row, kvh, n_i, slot, gtid, WPH * 32);
                 continue;
             }
             const int p0 = tok0 >> 4;
@@ -212,15 +247,16 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
 #pragma unroll
             for (int mt = 0; mt < 8; ++mt) o[mt][0] = o[mt][1] = o[mt][2] = o[mt][3] = 0.f;
 
-            for (int j = cw; j < np; j += kComputeWarps) {
+            for (int j = sub; j < np; j += WPH) {
                 const uint32_t sq = seq_base + j;
                 const uint32_t s = sq % kStages;
-                mbar_wait(full0 + 8 * s, (sq / kStages) & 1);
-                const uint32_t kb = stage_base + s * kStageBytes;
-                const uint32_t vb = kb + 4096;
+                const uint32_t par = (sq / kStages) & 1;
+                const uint32_t kb = stage_base + s * kStageBytes + hl * 4096;
+                const uint32_t vb = kb + HG * 4096;
                 const int nvalid = tok1 - ((p0 + j) << 4);  // >= 1; >= 16 for all but the last page
 
                 // ---- S^T = K . Q^T, two accumulation chains (channel halves)
+                mbar_wait(fullk0 + 8 * s, par);
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk) {
@@ -263,13 +299,14 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
                 const float p1f = ex2_approx(fmaf(s1, p.scale_log2, -offB));
                 const float p2f = ex2_approx(fmaf(s2, p.scale_log2, -offA));
                 const float p3f = ex2_approx(fmaf(s3, p.scale_log2, -offB));
-                lA += p0f + p2f;   // lane-partial sums; reduced across lanes at task end
+                lA += p0f + p2f;   // lane-partial sums; reduced across lanes at unit end
                 lB += p1f + p3f;
                 // P^T as the MMA B operand: transpose the two 8x8 (token x head) blocks
                 const uint32_t pb0 = movmatrix_trans(pack_half2(p0f, p1f));
                 const uint32_t pb1 = movmatrix_trans(pack_half2(p2f, p3f));
 
                 // ---- O^T += V^T . P^T
+                mbar_wait(fullv0 + 8 * s, par);
 #pragma unroll
                 for (int mt = 0; mt < 8; ++mt) {
                     uint32_t a0, a1, a2, a3;
@@ -278,11 +315,11 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
                     mma_16816(o[mt], a0, a1, a2, a3, pb0, pb1);
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(empty0 + 8 * s);   // stage may be refilled
+                if (lane == 0) mbar_arrive(empty0 + 8 * s);   // this head's part of the stage is consumed
             }
             seq_base += np;
 
-            // ---- warp state -> combine buffer
+            // ---- warp state -> combine buffer row cw
 #pragma unroll
             for (int off = 4; off <= 16; off <<= 1) {
                 lA += __shfl_xor_sync(0xffffffffu, lA, off);
@@ -301,37 +338,48 @@ __global__ void __launch_bounds__(kThreadsTma, 1)
                     tail.cb.l[cw][hA] = lA; tail.cb.l[cw][hB] = lB;
                 }
             }
-            named_bar_sync(kBarCompute, kComputeThreads);
-            finalize_task<G, kComputeWarps>(p, tail.cb, row, kvh, task.split, n_i, slot, ctid, kComputeThreads,
-                                            kBarCompute);
+            group_sync<WPH>(1 + hl);
+            finalize_task<G, WPH, kComputeWarps>(p, tail.cb, hl, HG, row, kvh, split, n_i, slot, gtid, 1 + hl);
         }
     }
 }
 
-}  // namespace
-
-int decode_tma_smem_bytes(int G) {
-    return G == 4 ? stages_for<4>() * kStageBytes + (int)sizeof(SmemTail<4>) + 1024
-                  : stages_for<8>() * kStageBytes + (int)sizeof(SmemTail<8>) + 1024;
+template <int G, int HG>
+cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, const CUtensorMap& mv,
+                       cudaStream_t stream) {
+    constexpr int smem = stages_for<G, HG>() * HG * 8192 + (int)sizeof(SmemTail<G>) + 1024;
+    constexpr int threads = (producers_for(HG) + kComputeWarps) * 32;
+    static bool attr_set = false;
+    if (!attr_set) {
+        const cudaError_t e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    pkv_decode_tma_kernel<G, HG><<<grid, threads, smem, stream>>>(p, mk, mv);
+    return cudaGetLastError();
 }
 
-cudaError_t launch_decode_tma(const DecodeParams& p, int G, int grid, const void* tmap_k, const void* tmap_v,
-                              cudaStream_t stream) {
+}  // namespace
+
+int decode_tma_smem_bytes(int G, int HG) {
+    const int tail = G == 4 ? (int)sizeof(SmemTail<4>) : (int)sizeof(SmemTail<8>);
+    int st = (232448 - 1024 - tail) / (HG * 8192);
+    if (st > kMaxStages) st = kMaxStages;
+    st = st / producers_for(HG) * producers_for(HG);
+    return st * HG * 8192 + tail + 1024;
+}
+
+cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int grid, const void* tmap_k,
+                              const void* tmap_v, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
-    const int smem = decode_tma_smem_bytes(G);
     const CUtensorMap& mk = *reinterpret_cast<const CUtensorMap*>(tmap_k);
     const CUtensorMap& mv = *reinterpret_cast<const CUtensorMap*>(tmap_v);
-    cudaError_t e;
-    if (G == 4) {
-        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        pkv_decode_tma_kernel<4><<<grid, kThreadsTma, smem, stream>>>(p, mk, mv);
-    } else {
-        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        pkv_decode_tma_kernel<8><<<grid, kThreadsTma, smem, stream>>>(p, mk, mv);
-    }
-    return cudaGetLastError();
+#define PKV_CASE(GG, HH) \
+    if (G == GG && HG == HH) return launch_one<GG, HH>(p, grid, mk, mv, stream);
+    PKV_CASE(4, 8) PKV_CASE(4, 4) PKV_CASE(4, 2) PKV_CASE(4, 1)
+    PKV_CASE(8, 8) PKV_CASE(8, 4) PKV_CASE(8, 2) PKV_CASE(8, 1)
+#undef PKV_CASE
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace pkv

@@ -30,7 +30,7 @@ struct DecodeParams {
     int32_t* fuse_counters;     // [B*Hkv]
     int64_t stride_page, stride_token, stride_head; // elements
     int32_t B, Hq, Hkv, max_pages, tile_tokens, merge_mode;
-    int32_t tma_rank;           // tensor-map mode: 0 = rank 5, one box per (page, head); 1, 2 = rank 4, two boxes
+    int32_t heads_per_cta;       // TMA kernel: KV heads one CTA streams together (1, 2, 4 or 8)
     int32_t dynamic_sched;      // 1: tasks handed out by an atomic counter
     float scale;                // x = scale * <q, k>
     float scale_log2;           // scale * log2(e)
@@ -132,45 +132,89 @@ __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
 
 // ------------------------------------------------------------------ merge of split states
 
-// Exact merge of the n states of (row, kvh) for head-in-group `hh`, channel
-// `dd`.  States live at slots slot_base .. slot_base+n-1.  One thread per (hh, dd); the
-// summation order (s ascending) is the same in the separate and the fused merge.
+// Exact merge of the n states of one (row, kvh, head-in-group hh), stored at
+// slots slot_base .. slot_base+n-1.  The arithmetic is fixed so that the separate merge kernel
+// and the fused in-kernel merge give bit-identical results:
+//   M   = max_s m_s
+//   P_k = sum over s = k, k+4, k+8, ... (ascending) of exp(m_s - M) * (l_s, a_s),   k = 0..3
+//   (L, A) = ((P_0 + P_1) + P_2) + P_3,   O = A / L,   LSE = M + log L
+// A warp works on one head at a time; lane owns channels 4*lane .. 4*lane+3 (one 16-byte load
+// per state row).  Neutral states (m = -inf, l = 0) drop out; all-neutral gives O = 0, LSE = -inf.
+
 template <int G>
-__device__ __forceinline__ void merge_one(const DecodeParams& p, int64_t slot_base, int n, int row, int kvh,
-                                          int hh, int dd) {
+__device__ __forceinline__ float merge_row_max(const DecodeParams& p, int64_t slot_base, int n, int hh, int lane) {
     float M = -INFINITY;
-#pragma unroll 8
-    for (int s = 0; s < n; ++s) M = fmaxf(M, p.part_m[(slot_base + s) * G + hh]);
-    const int64_t o = ((int64_t)row * p.Hq + kvh * G + hh);
+    for (int s = lane; s < n; s += 32) M = fmaxf(M, p.part_m[(slot_base + s) * G + hh]);
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, off));
+    return M;
+}
+
+// P_k for one lane: interleaved partial sum k of (L, A[4 channels])
+template <int G>
+__device__ __forceinline__ void merge_partial(const DecodeParams& p, int64_t slot_base, int n, int hh, float M, int k,
+                                              int lane, float& L, float4& A) {
+    L = 0.f;
+    A = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 4
+    for (int s = k; s < n; s += 4) {
+        const int64_t r = (slot_base + s) * G + hh;
+        const float w = ex2_approx((p.part_m[r] - M) * kLog2e);  // exp2(-inf) = 0
+        const float4 a = *reinterpret_cast<const float4*>(p.part_acc + r * kD + lane * 4);
+        L = fmaf(w, p.part_l[r], L);
+        A.x = fmaf(w, a.x, A.x); A.y = fmaf(w, a.y, A.y); A.z = fmaf(w, a.z, A.z); A.w = fmaf(w, a.w, A.w);
+    }
+}
+
+__device__ __forceinline__ void merge_store(const DecodeParams& p, int64_t o, int lane, float M, float L, float4 A) {
+    __half2* dst = reinterpret_cast<__half2*>(p.out + o * kD + lane * 4);
     if (M == -INFINITY) {  // no state or only neutral states (A9)
-        p.out[o * kD + dd] = __float2half_rn(0.f);
-        if (p.lse && dd == 0) p.lse[o] = -INFINITY;
+        dst[0] = __floats2half2_rn(0.f, 0.f);
+        dst[1] = __floats2half2_rn(0.f, 0.f);
+        if (p.lse && lane == 0) p.lse[o] = -INFINITY;
         return;
     }
-    float L = 0.f, A = 0.f;
-#pragma unroll 8
-    for (int s = 0; s < n; ++s) {
-        const float ms = p.part_m[(slot_base + s) * G + hh];
-        const float w = ex2_approx((ms - M) * kLog2e);  // exp2(-inf) = 0: neutral states drop out
-        L += w * p.part_l[(slot_base + s) * G + hh];
-        A += w * p.part_acc[((slot_base + s) * G + hh) * kD + dd];
-    }
-    p.out[o * kD + dd] = __float2half_rn(A / L);
-    if (p.lse && dd == 0) p.lse[o] = M + logf(L);
+    const float inv = 1.0f / L;
+    dst[0] = __floats2half2_rn(A.x * inv, A.y * inv);
+    dst[1] = __floats2half2_rn(A.z * inv, A.w * inv);
+    if (p.lse && lane == 0) p.lse[o] = M + logf(L);
+}
+
+// One warp merges head hh completely (fused path; also any caller without helpers).
+template <int G>
+__device__ __forceinline__ void merge_head_warp(const DecodeParams& p, int64_t slot_base, int n, int row, int kvh,
+                                                int hh, int lane) {
+    const float M = merge_row_max<G>(p, slot_base, n, hh, lane);
+    float L[4];
+    float4 A[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) merge_partial<G>(p, slot_base, n, hh, M, k, lane, L[k], A[k]);
+    const float Ls = ((L[0] + L[1]) + L[2]) + L[3];
+    float4 As;
+    As.x = ((A[0].x + A[1].x) + A[2].x) + A[3].x;
+    As.y = ((A[0].y + A[1].y) + A[2].y) + A[3].y;
+    As.z = ((A[0].z + A[1].z) + A[2].z) + A[3].z;
+    As.w = ((A[0].w + A[1].w) + A[2].w) + A[3].w;
+    merge_store(p, (int64_t)row * p.Hq + kvh * G + hh, lane, M, Ls, As);
 }
 
 // ------------------------------------------------------------------ task epilogue
 
-// Shared-memory combine buffer of one CTA: the NW compute warps each leave the state of their
-// share of the task's tokens here; m in raw-dot units (x = scale * raw).
-constexpr int kAccStride = 132;  // floats per (warp, head) row of comb_acc; 132 % 32 = 4 spreads banks
-template <int G, int NW>
+// Shared-memory combine buffer of one CTA: every compute warp leaves the state of its share of
+// a task's tokens in its own row; m in raw-dot units (x = scale * raw).
+constexpr int kAccStride = 132;  // floats per (warp, head) row of acc; 132 % 32 = 4 spreads banks
+template <int G, int NWTOT>
 struct CombineBuf {
-    float acc[NW][G][kAccStride];
-    float m[NW][8];
-    float l[NW][8];
-    int flag;
+    float acc[NWTOT][G][kAccStride];
+    float m[NWTOT][8];
+    float l[NWTOT][8];
+    int flag[NWTOT];
 };
+
+template <int NW>
+__device__ __forceinline__ void group_sync(int bar_id) {
+    if (NW == 1) __syncwarp(); else named_bar_sync(bar_id, NW * 32);
+}
 
 // Writes an empty task's result (rect route): neutral partial state, or zeros when
 // the row has a single slot (direct output).
@@ -193,23 +237,25 @@ __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int row,
     }
 }
 
-// Combines the NW warp states in `cb` and stores the task's result: direct FP16 output when the
-// row has one split, else the FP32 partial state in its compact slot;
-// in FUSED mode the CTA that completes the last split of (row, kvh) merges in place
-// (PAPER.md:77).  Called by `nthreads` threads (tid 0..nthreads-1) that synchronise on named
-// barrier `bar_id`; the caller has already synchronised after filling `cb`.
-template <int G, int NW>
-__device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<G, NW>& cb, int row, int kvh,
-                                              int split, int n_i, int64_t slot, int tid, int nthreads,
+// A group of NW warps (rows w0, w0+wstride, ... of `cb`) has processed one task.  Combines the
+// NW warp states and stores the task's result: direct FP16 output when the row has one split,
+// else the FP32 partial state in its compact slot; in FUSED mode
+// the group that completes the last split of (row, kvh) merges in place.
+// gtid = 0..NW*32-1 within the group; the group synchronises with group_sync<NW>(bar_id); the
+// caller has synchronised after filling `cb`.
+template <int G, int NW, int NWTOT>
+__device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<G, NWTOT>& cb, int w0, int wstride,
+                                              int row, int kvh, int split, int n_i, int64_t slot, int gtid,
                                               int bar_id) {
-    for (int idx = tid; idx < G * kD; idx += nthreads) {
+    for (int idx = gtid; idx < G * kD; idx += NW * 32) {
         const int hh = idx / kD, dd = idx % kD;
         float M = -INFINITY;
 #pragma unroll
-        for (int w = 0; w < NW; ++w) M = fmaxf(M, cb.m[w][hh]);
+        for (int i = 0; i < NW; ++i) M = fmaxf(M, cb.m[w0 + i * wstride][hh]);
         float L = 0.f, A = 0.f;
 #pragma unroll
-        for (int w = 0; w < NW; ++w) {
+        for (int i = 0; i < NW; ++i) {
+            const int w = w0 + i * wstride;
             const float wgt = ex2_approx((cb.m[w][hh] - M) * p.scale_log2);  // m = -inf -> 0
             L += wgt * cb.l[w][hh];
             A += wgt * cb.acc[w][hh][dd];
@@ -228,21 +274,21 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
     }
     if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED) {
         __threadfence();  // partial state visible device-wide before the completion count
-        named_bar_sync(bar_id, nthreads);
-        if (tid == 0) {
+        group_sync<NW>(bar_id);
+        if (gtid == 0) {
             const int old = atomicAdd(&p.fuse_counters[row * p.Hkv + kvh], 1);
             const int last = (old == n_i - 1);
             if (last) p.fuse_counters[row * p.Hkv + kvh] = 0;  // self-reset for the next replay
-            cb.flag = last;
+            cb.flag[w0] = last;
         }
-        named_bar_sync(bar_id, nthreads);
-        if (cb.flag) {
+        group_sync<NW>(bar_id);
+        if (cb.flag[w0]) {
             __threadfence();
             const int64_t base = slot - split;  // first slot of (row, kvh): DESIGN.md A8
-            for (int idx = tid; idx < G * kD; idx += nthreads) merge_one<G>(p, base, n_i, row, kvh, idx / kD, idx % kD);
+            for (int hh = gtid >> 5; hh < G; hh += NW) merge_head_warp<G>(p, base, n_i, row, kvh, hh, gtid & 31);
         }
     }
-    named_bar_sync(bar_id, nthreads);  // cb may be refilled after this
+    group_sync<NW>(bar_id);  // cb rows may be refilled after this
 }
 
 // Rows with N_i = 0 emit no task in the workqueue route: out = 0, lse = -inf (A9).
@@ -259,12 +305,12 @@ __device__ __forceinline__ void zero_empty_rows(const DecodeParams& p) {
 
 // launchers implemented in the .cu files
 cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStream_t stream);
-cudaError_t launch_decode_tma(const DecodeParams& p, int G, int grid, const void* tmap_k, const void* tmap_v,
-                              cudaStream_t stream);
+cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int grid, const void* tmap_k,
+                              const void* tmap_v, cudaStream_t stream);
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
                            QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, pkv_task* tasks,
                            int64_t tasks_cap, cudaStream_t stream);
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream);
-int decode_tma_smem_bytes(int G);
+int decode_tma_smem_bytes(int G, int HG);
 
 }  // namespace pkv
