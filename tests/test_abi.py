@@ -1,0 +1,138 @@
+"""CPU-only checks of the C ABI: libpkv.so loads without a GPU, exports every symbol that
+include/pkv.h declares, validates host-checkable arguments, and its HOST workqueue builder is
+bit-exact against the pure-Python oracle.  No compute call is made here."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2606_26666_b200 as pkv
+from paper_2606_26666_b200 import binding
+from oracle import workqueue_oracle as wq
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def header_symbols():
+    text = open(os.path.join(ROOT, "include", "pkv.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"PKV_API\s+[\w\s\*]+?\b(pkv_\w+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    syms = header_symbols()
+    assert len(syms) >= 12
+    lib = ctypes.CDLL(pkv.binding._build.LIB)
+    for s in syms:
+        assert hasattr(lib, s), s
+    assert sorted(binding.EXPORTS) == syms
+
+
+def test_version_and_struct_sizes():
+    assert pkv.pkv_version() == (1 << 16)
+    assert ctypes.sizeof(binding.pkv_task) == 20            # 5 x int32
+    assert ctypes.sizeof(binding.pkv_split_policy) == 32
+    assert ctypes.sizeof(binding.pkv_shape) == 56
+    assert ctypes.sizeof(binding.pkv_counters) == 88
+
+
+def shape(B, Hkv=8, Hq=32, max_pages=4096):
+    return pkv.Shape(B=B, Hq=Hq, Hkv=Hkv, max_pages=max_pages, num_pages=1 << 20)
+
+
+@pytest.mark.parametrize("bad,status", [
+    (dict(d=64), pkv.PKV_ERR_UNSUPPORTED),
+    (dict(page_size=32), pkv.PKV_ERR_UNSUPPORTED),
+    (dict(Hq=8, Hkv=8), pkv.PKV_ERR_UNSUPPORTED),          # G = 1 not compiled in
+    (dict(Hq=30, Hkv=8), pkv.PKV_ERR_INVALID_ARG),
+    (dict(kv_strides=(4096, 4, 128)), pkv.PKV_ERR_INVALID_ARG),   # token stride not 16-byte multiple
+])
+def test_shape_validation(bad, status):
+    kw = dict(B=2, Hq=32, Hkv=8, max_pages=8, num_pages=64)
+    kw.update(bad)
+    with pytest.raises(pkv.PkvError) as e:
+        pkv.pkv_build_workqueue_host(pkv.Shape(**kw), pkv.Policy(num_splits=2), np.array([5, 6], np.int32))
+    assert e.value.status == status
+    assert pkv.pkv_last_error() != ""
+
+
+@pytest.mark.parametrize("bad", [dict(tile_tokens=24), dict(tile_tokens=0), dict(num_splits=257),
+                                 dict(split_mode=2), dict(route=3), dict(merge_mode=2), dict(kernel=9),
+                                 dict(split_mode=1, chunk_tiles=0), dict(num_splits=0, num_sms=0)])
+def test_policy_validation(bad):
+    with pytest.raises(pkv.PkvError) as e:
+        pkv.pkv_build_workqueue_host(shape(1), pkv.Policy(**bad), np.array([100], np.int32))
+    assert e.value.status == pkv.PKV_ERR_INVALID_ARG
+
+
+def test_workspace_bytes_is_monotone_and_pure():
+    a = pkv.pkv_workspace_bytes(shape(8), pkv.Policy(num_splits=4))
+    b = pkv.pkv_workspace_bytes(shape(8), pkv.Policy(num_splits=16))
+    assert 0 < a < b
+    assert a == pkv.pkv_workspace_bytes(shape(8), pkv.Policy(num_splits=4))
+    # partial states alone: slots * G * (d + 2) * 4 bytes (A11)
+    assert b >= 8 * 8 * 16 * 4 * 130 * 4
+    with pytest.raises(pkv.PkvError):
+        pkv.pkv_workspace_bytes(shape(8), pkv.Policy(tile_tokens=17))
+
+
+def oracle_tasks(seq_lens, Hkv, pol: pkv.Policy):
+    opol = wq.Policy(tile_tokens=pol.tile_tokens, split_mode=pol.split_mode, num_splits=pol.num_splits,
+                     chunk_tiles=pol.chunk_tiles, route=pol.route, merge_mode=pol.merge_mode, num_sms=pol.num_sms)
+    q = wq.build_workqueue(list(map(int, seq_lens)), Hkv, opol)
+    return np.array(q.tasks, dtype=np.int32).reshape(-1, 5), np.array(q.split_offsets, dtype=np.int32), q
+
+
+POLICIES = [
+    pkv.Policy(tile_tokens=32, num_splits=1),
+    pkv.Policy(tile_tokens=32, num_splits=20),
+    pkv.Policy(tile_tokens=64, num_splits=7),
+    pkv.Policy(tile_tokens=16, num_splits=256),
+    pkv.Policy(tile_tokens=32, num_splits=0, num_sms=28),
+    pkv.Policy(tile_tokens=32, num_splits=0, num_sms=148),
+    pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=16),
+    pkv.Policy(tile_tokens=128, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=12, chunk_tiles=3),
+    pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_RECT),
+    pkv.Policy(tile_tokens=64, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=9, chunk_tiles=4, route=pkv.ROUTE_RECT),
+]
+
+
+@pytest.mark.parametrize("pol", POLICIES, ids=lambda p: "T%d_m%d_S%d_c%d_r%d_sm%d" % (
+    p.tile_tokens, p.split_mode, p.num_splits, p.chunk_tiles, p.route, p.num_sms))
+def test_host_builder_bit_exact_vs_python_oracle(pol):
+    rng = np.random.Generator(np.random.PCG64(1234))
+    cases = [[0], [1], [0, 0, 0], [31, 32, 33, 0, 1], [65536], list(rng.integers(0, 70000, size=8)),
+             list(rng.integers(0, 3000, size=37)), [16384 + i for i in range(8)], []]
+    for Hkv in (8, 4):
+        for lens in cases:
+            lens = np.array(lens, dtype=np.int32)
+            ref_t, ref_o, _ = oracle_tasks(lens, Hkv, pol)
+            got_t, got_o = pkv.pkv_build_workqueue_host(shape(len(lens), Hkv=Hkv), pol, lens)
+            assert got_t.shape == ref_t.shape, (lens, Hkv)
+            assert np.array_equal(got_t, ref_t), (lens, Hkv)
+            assert np.array_equal(got_o, ref_o), (lens, Hkv)
+
+
+def test_host_builder_on_the_trace_configs():
+    import pkv_inputs
+    for w in (pkv_inputs.config3(), pkv_inputs.config4(), pkv_inputs.config4_b4(), pkv_inputs.config5()):
+        for step in (0, w.steps):
+            lens = w.seq_lens_at(step)
+            for pol in (pkv.Policy(tile_tokens=32, num_splits=20),
+                        pkv.Policy(tile_tokens=64, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=8)):
+                ref_t, ref_o, _ = oracle_tasks(lens, w.Hkv, pol)
+                got_t, got_o = pkv.pkv_build_workqueue_host(shape(w.B, Hkv=w.Hkv), pol, lens)
+                assert np.array_equal(got_t, ref_t) and np.array_equal(got_o, ref_o), (w.name, step)
+
+
+def test_tasks_cap_too_small_reports_needed_count():
+    s, pol = shape(1), pkv.Policy(num_splits=4)
+    lens = np.array([1000], np.int32)
+    tasks = np.zeros((3, 5), np.int32)
+    off = np.zeros(2, np.int32)
+    n = ctypes.c_int32(0)
+    st = binding._lib.pkv_build_workqueue_host(ctypes.byref(s.c()), ctypes.byref(pol.c()), lens.ctypes.data,
+                                               tasks.ctypes.data, 3, off.ctypes.data, ctypes.byref(n))
+    assert st == pkv.PKV_ERR_WORKSPACE and n.value == 32

@@ -1,0 +1,343 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle, element by element,
+on the same seeded inputs.  Tolerance = BASELINE.json north_star with DESIGN.md reading A15:
+max abs <= 2e-3, floored max rel <= 1e-2, mean abs <= 3e-4.  Integer work
+(tasks, split_offsets, counters, token counts) is compared bit-exactly."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_26666_b200 as pkv
+import pkv_inputs
+from gpu_helpers import DevProblem, oracle_attention, oracle_policy, read_partials, sm_count, to_dev
+from helpers import (assert_within_tolerance, default_scale, make_problem, permute_pool, token_location, Problem)
+from oracle import pkv_oracle, workqueue_oracle as wq
+from pkv_inputs import PAD_PAGE
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [pkv.KERNEL_TMA_MMA, pkv.KERNEL_SIMT]
+RAGGED = [1, 2, 15, 16, 17, 31, 32, 33, 100, 0, 257, 700]
+
+
+def check(dp, pol, ref=None, what=""):
+    out, lse, ws = dp.decode(pol)
+    if ref is None:
+        ref = oracle_attention(dp.p)
+    assert not np.isnan(out).any(), what
+    m = assert_within_tolerance(out, ref[0], what)
+    fin = np.isfinite(ref[1])
+    assert np.array_equal(np.isneginf(lse), np.isneginf(ref[1])), what
+    assert np.abs(lse[fin] - ref[1][fin]).max(initial=0.0) <= 2e-3, what
+    return out, lse, ws, m
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config1(kernel):
+    """BASELINE.json configs[0]: B=1, N=256, 16 pages of a 64-page pool, no splitting."""
+    w = pkv_inputs.config1()
+    p = Problem(q=pkv_inputs.fill_normal_f16((1, 32, 128), 1), k_cache=pkv_inputs.fill_normal_f16(w.pool_shape(), 2),
+                v_cache=pkv_inputs.fill_normal_f16(w.pool_shape(), 3), block_table=w.block_table,
+                seq_lens=w.seq_lens, Hkv=8, page_size=16, scale=default_scale(128))
+    dp = DevProblem(p)
+    for hg in (0, 1, 2, 4, 8):
+        pkv.pkv_debug_force_heads_per_cta(hg)
+        try:
+            check(dp, pkv.Policy(tile_tokens=32, num_splits=1, route=pkv.ROUTE_RECT, kernel=kernel), what="hg%d" % hg)
+        finally:
+            pkv.pkv_debug_force_heads_per_cta(0)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("Hkv", [8, 4])
+@pytest.mark.parametrize("route", [pkv.ROUTE_WORKQUEUE, pkv.ROUTE_RECT])
+def test_ragged_split_sweep(kernel, Hkv, route):
+    """Ragged rows spanning several tiles and a ragged tail, every split count incl. S > T
+    (neutral states), separate and fused merge."""
+    p = make_problem(RAGGED, seed=100 + Hkv, Hkv=Hkv)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    for S in (1, 2, 3, 4, 16, 64):
+        for mm in (pkv.MERGE_SEPARATE, pkv.MERGE_FUSED):
+            pol = pkv.Policy(tile_tokens=32, num_splits=S, route=route, merge_mode=mm, kernel=kernel)
+            check(dp, pol, ref, what="S%d mm%d" % (S, mm))
+    pol = pkv.Policy(tile_tokens=64, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=2, route=route,
+                     kernel=kernel)
+    check(dp, pol, ref, what="chunk")
+
+
+@pytest.mark.parametrize("hg", [1, 2, 4, 8])
+@pytest.mark.parametrize("Hkv", [8, 4])
+def test_tma_heads_per_cta_variants(hg, Hkv):
+    if hg > Hkv:
+        pytest.skip("hg > Hkv")
+    p = make_problem(RAGGED, seed=300 + Hkv, Hkv=Hkv)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    pkv.pkv_debug_force_heads_per_cta(hg)
+    try:
+        for S, mm in ((1, 0), (5, 0), (5, 1)):
+            check(dp, pkv.Policy(tile_tokens=32, num_splits=S, merge_mode=mm), ref, what="hg%d S%d" % (hg, S))
+    finally:
+        pkv.pkv_debug_force_heads_per_cta(0)
+
+
+@pytest.mark.parametrize("route", [pkv.ROUTE_WORKQUEUE, pkv.ROUTE_RECT])
+def test_device_builder_bit_exact(route):
+    """pkv_build_workqueue (device) == workqueue oracle: count, order, every field, split_offsets,
+    launches and Table-4 counters."""
+    rng = np.random.Generator(np.random.PCG64(77))
+    cases = [[0], [1], [0, 0], RAGGED, list(rng.integers(0, 70000, size=8)), list(rng.integers(0, 9000, size=128)),
+             list(rng.integers(1, 400, size=1500))]
+    pols = [pkv.Policy(tile_tokens=32, num_splits=20), pkv.Policy(tile_tokens=64, num_splits=0),
+            pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=16),
+            pkv.Policy(tile_tokens=16, num_splits=256)]
+    for lens in cases:
+        lens = np.array(lens, dtype=np.int32)
+        for base in pols:
+            for Hkv in (8, 4):
+                pol = pkv.Policy(**{**base.__dict__, "route": route})
+                shape = pkv.Shape(B=len(lens), Hq=32, Hkv=Hkv, max_pages=1, num_pages=1)
+                opol = oracle_policy(pol)
+                if pol.num_splits == 0 and pol.split_mode == pkv.SPLIT_FIXED_COUNT:
+                    opol = wq.Policy(**{**opol.__dict__, "num_sms": sm_count()})
+                ref = wq.build_workqueue(list(map(int, lens)), Hkv, opol)
+                ws = pkv.alloc_workspace(shape, pol)
+                pkv.pkv_build_workqueue(shape, pol, to_dev(lens), ws)
+                tasks, offs = pkv.pkv_read_workqueue(shape, pol, ws)
+                assert tasks.shape[0] == ref.num_tasks
+                assert np.array_equal(tasks, np.array(ref.tasks, dtype=np.int32).reshape(-1, 5))
+                assert np.array_equal(offs, np.array(ref.split_offsets, dtype=np.int32))
+                c = pkv.pkv_get_counters(shape, pol, ws)
+                assert c["tasks"] == ref.num_tasks and c["empty_tasks"] == ref.empty_ctas
+                assert c["decode_launches"] == ref.decode_launches and c["merge_launches"] == ref.merge_launches
+                assert c["num_splits"] == ref.num_splits
+                assert c["useful_kv_bytes"] == wq.useful_kv_bytes(lens, Hkv, 128)
+                assert c["merge_bytes"] == wq.merge_bytes(ref.num_tasks, 32 // Hkv, 128)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_p3_zero_keys_token_counts_exact(kernel):
+    """K = 0 => every score is 0, O = mean(V) (closed form) and each partial's l_s is EXACTLY the
+    token count of its range (integers < 2^24 are exact in FP32): catches a dropped or duplicated
+    token at any N (pin P3)."""
+    lens = [4097, 33, 1, 1000]
+    p = make_problem(lens, seed=41)
+    rng = np.random.Generator(np.random.PCG64(7))
+    p.k_cache[...] = 0
+    p.v_cache[...] = rng.integers(-8, 9, size=p.v_cache.shape).astype(np.float16)
+    dp = DevProblem(p)
+    pol = pkv.Policy(tile_tokens=32, num_splits=7, kernel=kernel)
+    out, lse, ws = dp.decode(pol)
+    ref = oracle_attention(p)
+    assert_within_tolerance(out, ref[0])
+    q = wq.build_workqueue(lens, 8, oracle_policy(pol))
+    m, l, a = read_partials(dp, pol, ws, q.num_tasks)
+    for t, (row, kvh, split, tb, te) in enumerate(q.tasks):
+        n_i = q.split_offsets[row + 1] - q.split_offsets[row]
+        if n_i <= 1:
+            continue        # direct output, no partial state
+        slot = q.split_offsets[row] * 8 + kvh * n_i + split
+        cnt = min(te * 32, lens[row]) - tb * 32
+        assert np.all(l[slot] == cnt), (t, l[slot], cnt)
+        assert np.all(m[slot] == 0.0)
+    assert np.allclose(lse, np.log(np.array(lens, dtype=np.float64))[:, None], atol=1e-5)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_p5_dominant_key_at_boundaries(kernel):
+    """k_j* = 3 q for the 4 heads sharing... one query head's q: that head's output must be v_j*
+    (pin P5).  j* at 0, N-1 and around page / tile / split boundaries."""
+    N = 1000
+    S = 4
+    base = make_problem([N], seed=51)
+    c = -(-(-(-N // 32)) // S) * 32      # tokens per split
+    spots = sorted({0, 1, 15, 16, 17, 31, 32, 33, c - 1, c, c + 1, 2 * c - 1, 2 * c, N - 2, N - 1})
+    for j in spots:
+        p = Problem(q=base.q, k_cache=base.k_cache.copy(), v_cache=base.v_cache, block_table=base.block_table,
+                    seq_lens=base.seq_lens, Hkv=8, page_size=16, scale=base.scale)
+        page, r = token_location(p, 0, j)
+        for g in range(8):
+            p.k_cache[page, r, g] = (3.0 * p.q[0, g * 4].astype(np.float32)).astype(np.float16)
+        dp = DevProblem(p)
+        out, _, _ = dp.decode(pkv.Policy(tile_tokens=32, num_splits=S, kernel=kernel))
+        for g in range(8):
+            want = p.v_cache[page, r, g].astype(np.float64)
+            assert np.abs(out[0, g * 4] - want).max() <= 2e-3, (j, g)
+        assert_within_tolerance(out, oracle_attention(p)[0], "j=%d" % j)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_p2_pool_permutation_bit_identical(kernel):
+    p = make_problem([700, 33, 16, 257], seed=21)
+    pol = pkv.Policy(tile_tokens=32, num_splits=3, kernel=kernel)
+    o1, l1, _ = DevProblem(p).decode(pol)
+    o2, l2, _ = DevProblem(permute_pool(p, seed=99)).decode(pol)
+    assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
+    o3, l3, _ = DevProblem(p).decode(pol)
+    assert np.array_equal(o1, o3) and np.array_equal(l1, l3)      # run-to-run determinism
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_a10_tail_and_unused_entries_never_contribute(kernel):
+    """Tokens past N_i in the last page hold huge values; block-table entries past ceil(N_i/P)
+    hold PAD_PAGE: neither may change the result (reading A10)."""
+    lens = [45, 100, 17]
+    p = make_problem(lens, seed=61, max_pages=40)
+    ref = oracle_attention(p)
+    for i, N in enumerate(lens):
+        page, r = token_location(p, i, N - 1)
+        p.k_cache[page, r + 1:] = 60000.0
+        p.v_cache[page, r + 1:] = 60000.0
+        assert np.all(p.block_table[i, -(-N // 16):] == PAD_PAGE)
+    dp = DevProblem(p)
+    for S in (1, 3):
+        out, _, _ = dp.decode(pkv.Policy(tile_tokens=32, num_splits=S, kernel=kernel))
+        assert_within_tolerance(out, ref[0])
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_paper_layout_strides_reading_a1(kernel):
+    """The paper's [page, Hkv, page_size, d] layout through explicit strides."""
+    p = make_problem([300, 19], seed=31)
+    ref = oracle_attention(p)
+    k_hnd = to_dev(np.ascontiguousarray(p.k_cache.transpose(0, 2, 1, 3)))
+    v_hnd = to_dev(np.ascontiguousarray(p.v_cache.transpose(0, 2, 1, 3)))
+    dp = DevProblem(p, kv_strides=(8 * 16 * 128, 128, 16 * 128), k_dev=k_hnd, v_dev=v_hnd)
+    for S in (1, 4):
+        out, _, _ = dp.decode(pkv.Policy(tile_tokens=32, num_splits=S, kernel=kernel))
+        assert_within_tolerance(out, ref[0])
+
+
+def test_n1_bit_exact_and_scale_argument():
+    """N = 1 => O = v_0 bit-exactly in FP16 (pin P6); an explicit scale is honoured."""
+    p = make_problem([1, 1, 1], seed=71)
+    dp = DevProblem(p)
+    for kernel in KERNELS:
+        out, lse, _ = dp.decode(pkv.Policy(num_splits=1, kernel=kernel))
+        for i in range(3):
+            page, r = token_location(p, i, 0)
+            want = np.repeat(p.v_cache[page, r].astype(np.float64), 4, axis=0)
+            assert np.array_equal(out[i], want)
+    p2 = make_problem([90], seed=72)
+    p2.scale = 0.25
+    dp2 = DevProblem(p2)
+    out, lse, _ = dp2.decode(pkv.Policy(num_splits=2))
+    ref = oracle_attention(p2)
+    assert_within_tolerance(out, ref[0])
+    out0, _, _ = dp2.decode(pkv.Policy(num_splits=2), scale=0.0)     # <= 0 means 1/sqrt(d)
+    p2.scale = default_scale(128)
+    assert_within_tolerance(out0, oracle_attention(p2)[0])
+
+
+def test_pkv_merge_standalone_vs_oracle():
+    """pkv_merge on caller-provided states (public partial format) == oracle merge,
+    including neutral states and a row without any state."""
+    rng = np.random.Generator(np.random.PCG64(5))
+    Hkv, G, d = 8, 4, 128
+    n = [3, 0, 1, 17]
+    offs = np.concatenate([[0], np.cumsum(n)]).astype(np.int32)
+    slots = int(offs[-1]) * Hkv
+    m = rng.normal(0, 3, size=(slots, G)).astype(np.float32)
+    l = rng.uniform(0.5, 50, size=(slots, G)).astype(np.float32)
+    a = rng.normal(0, 4, size=(slots, G, d)).astype(np.float32)
+    m[1], l[1], a[1] = -np.inf, 0.0, 0.0                 # a neutral state inside row 0
+    shape = pkv.Shape(B=len(n), Hq=32, Hkv=Hkv)
+    out = torch.full((len(n), 32, d), float("nan"), dtype=torch.float16, device="cuda")
+    lse = torch.full((len(n), 32), float("nan"), dtype=torch.float32, device="cuda")
+    pkv.pkv_merge(shape, to_dev(m), to_dev(l), to_dev(a), to_dev(offs), out, lse)
+    torch.cuda.synchronize()
+    out, lse = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
+    for i, n_i in enumerate(n):
+        for g in range(Hkv):
+            b = int(offs[i]) * Hkv + g * n_i
+            for hh in range(G):
+                o_ref, lse_ref = pkv_oracle.merge(m[b:b + n_i, hh], l[b:b + n_i, hh], a[b:b + n_i, hh])
+                h = g * G + hh
+                if n_i == 0:
+                    assert np.all(out[i, h] == 0) and np.isneginf(lse[i, h])
+                else:
+                    assert np.abs(out[i, h] - o_ref).max() <= 2e-3 * max(1.0, np.abs(o_ref).max())
+                    assert abs(lse[i, h] - lse_ref) <= 1e-4
+
+
+def test_partial_states_match_oracle_split_states():
+    """GPU partial states vs the oracle's split form through the invariant pair
+    LSE_s = m_s + log l_s, O_s = a_s / l_s (reading A11)."""
+    lens = [1500, 64, 333]
+    p = make_problem(lens, seed=81)
+    dp = DevProblem(p)
+    for kernel in KERNELS:
+        pol = pkv.Policy(tile_tokens=32, num_splits=5, kernel=kernel)
+        _, _, ws = dp.decode(pol)
+        q = wq.build_workqueue(lens, 8, oracle_policy(pol))
+        tasks = np.array(q.tasks, dtype=np.int32)
+        rm, rl, ra = pkv_oracle.split_states(p.q, p.k_cache, p.v_cache, p.block_table, p.seq_lens, tasks, Hkv=8,
+                                             page_size=16, tile_tokens=32, scale=p.scale)
+        m, l, a = read_partials(dp, pol, ws, q.num_tasks)
+        # canonical order == slot order (reading A8)
+        assert np.abs((m + np.log(l)) - (rm + np.log(rl))).max() <= 1e-4
+        assert np.abs(a / l[..., None] - ra / rl[..., None]).max() <= 2e-3
+
+
+def test_decode_host_entry_point():
+    """pkv_decode_host: host planning + one H2D image + decode + merge + D2H;
+    launch counts equal the oracle's (reading A13)."""
+    lens = [1500, 64, 0, 333]
+    p = make_problem(lens, seed=91)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    for pol in (pkv.Policy(num_splits=6), pkv.Policy(num_splits=1), pkv.Policy(num_splits=6, merge_mode=pkv.MERGE_FUSED),
+                pkv.Policy(num_splits=6, route=pkv.ROUTE_RECT, kernel=pkv.KERNEL_SIMT)):
+        nb = pkv.pkv_host_scratch_bytes(dp.shape, pol)
+        staging = torch.empty(nb, dtype=torch.uint8).pin_memory()
+        scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
+        ws = pkv.alloc_workspace(dp.shape, pol)
+        out = np.full((p.B, p.Hq, p.d), np.nan, dtype=np.float16)
+        c = pkv.pkv_decode_host(dp.shape, pol, p.q, dp.k, dp.v, p.block_table, p.seq_lens, out, p.scale, staging,
+                                scratch, ws)
+        assert_within_tolerance(out.astype(np.float64), ref[0])
+        q = wq.build_workqueue(lens, 8, oracle_policy(pol))
+        assert c["tasks"] == q.num_tasks
+        assert c["decode_launches"] == q.decode_launches and c["merge_launches"] == q.merge_launches
+        assert c["d2h_bytes"] == out.nbytes and c["h2d_bytes"] > p.q.nbytes
+    # every row empty: no launch at all, out = 0
+    p0 = make_problem([0, 0], seed=92)
+    dp0 = DevProblem(p0)
+    pol = pkv.Policy(num_splits=2)
+    nb = pkv.pkv_host_scratch_bytes(dp0.shape, pol)
+    out = np.full((2, 32, 128), np.nan, dtype=np.float16)
+    c = pkv.pkv_decode_host(dp0.shape, pol, p0.q, dp0.k, dp0.v, p0.block_table, p0.seq_lens, out, p0.scale,
+                            torch.empty(nb, dtype=torch.uint8).pin_memory(),
+                            torch.empty(nb, dtype=torch.uint8, device="cuda"), pkv.alloc_workspace(dp0.shape, pol))
+    assert np.all(out == 0) and c["decode_launches"] == 0 and c["merge_launches"] == 0
+
+
+@pytest.mark.parametrize("mm", [pkv.MERGE_SEPARATE, pkv.MERGE_FUSED])
+def test_cuda_graph_replay_with_growing_lengths(mm):
+    """{device builder, decode, merge} captured once and replayed while seq_lens grows in place
+    (north_star (e)): the task count changes between replays, the graph does not."""
+    lens = np.array([60, 1000, 31, 257], dtype=np.int32)
+    steps = 40
+    p = make_problem(lens, seed=95, reserve_extra=steps)
+    dp = DevProblem(p)
+    pol = pkv.Policy(tile_tokens=32, num_splits=4, merge_mode=mm)
+    ws = pkv.alloc_workspace(dp.shape, pol)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        pkv.pkv_decode(dp.shape, pol, dp.q, dp.k, dp.v, dp.bt, dp.sl, dp.out, dp.lse, scale=p.scale, workspace=ws,
+                       stream=s)       # warm-up outside capture (sets function attributes)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            pkv.pkv_decode(dp.shape, pol, dp.q, dp.k, dp.v, dp.bt, dp.sl, dp.out, dp.lse, scale=p.scale,
+                           workspace=ws, stream=torch.cuda.current_stream())
+    for step in range(steps):
+        dp.sl.copy_(torch.from_numpy(lens + step))
+        dp.out.fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        if step % 13 == 0 or step == steps - 1:
+            p.seq_lens = (lens + step).astype(np.int32)
+            assert_within_tolerance(dp.out.cpu().numpy().astype(np.float64), oracle_attention(p)[0], "step %d" % step)
+            tasks, _ = pkv.pkv_read_workqueue(dp.shape, pol, ws)
+            assert tasks.shape[0] == wq.build_workqueue(list(lens + step), 8, oracle_policy(pol)).num_tasks
