@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
         const int tok0 = task.t_begin * p.tile_tokens;
         const int tok1 = min(task.t_end * p.tile_tokens, N);
         if (tok0 >= tok1) {  // empty split: neutral state, before loading Q
-            store_empty_task<G>(p, row, kvh, n_i, slot, tid, kThreads);
+            store_empty_task<G, kWarps>(p, &cb.flag[0], row, kvh, task.split, n_i, slot, tid, 0);
             continue;
         }
 

@@ -224,7 +224,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
             const int tok0 = task.t_begin * p.tile_tokens;
             const int tok1 = min(task.t_end * p.tile_tokens, N);
             if (tok0 >= tok1) {
-                store_empty_task<G>(p, row, kvh, n_i, slot, gtid, WPH * 32);
+                store_empty_task<G, WPH>(p, &tail.cb.flag[hl], row, kvh, split, n_i, slot, gtid, 1 + hl);
                 continue;
             }
             const int p0 = tok0 >> 4;

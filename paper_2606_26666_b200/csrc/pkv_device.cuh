@@ -216,12 +216,35 @@ __device__ __forceinline__ void group_sync(int bar_id) {
     if (NW == 1) __syncwarp(); else named_bar_sync(bar_id, NW * 32);
 }
 
+// FUSED merge tail: a group of NW warps has stored split `split` of (row, kvh); the
+// group that completes the last of the n_i splits (atomic completion counter, self-resetting for
+// graph replay) merges the row's slot range in place.  flag = a shared-memory word of the group.
+template <int G, int NW>
+__device__ __forceinline__ void fused_complete(const DecodeParams& p, int* flag, int row, int kvh, int split, int n_i,
+                                               int64_t slot, int gtid, int bar_id) {
+    __threadfence();  // partial state visible device-wide before the completion count
+    group_sync<NW>(bar_id);
+    if (gtid == 0) {
+        const int old = atomicAdd(&p.fuse_counters[row * p.Hkv + kvh], 1);
+        const int last = (old == n_i - 1);
+        if (last) p.fuse_counters[row * p.Hkv + kvh] = 0;
+        *flag = last;
+    }
+    group_sync<NW>(bar_id);
+    if (*flag) {
+        __threadfence();
+        const int64_t base = slot - split;  // first slot of (row, kvh): DESIGN.md A8
+        for (int hh = gtid >> 5; hh < G; hh += NW) merge_head_warp<G>(p, base, n_i, row, kvh, hh, gtid & 31);
+    }
+    group_sync<NW>(bar_id);  // flag may be rewritten after this
+}
+
 // Writes an empty task's result (rect route): neutral partial state, or zeros when
-// the row has a single slot (direct output).
-template <int G>
-__device__ __forceinline__ void store_empty_task(const DecodeParams& p, int row, int kvh, int n_i, int64_t slot,
-                                                 int tid, int nthreads) {
-    for (int idx = tid; idx < G * kD; idx += nthreads) {
+// the row has a single slot (direct output).  Called by the NW warps that own the task.
+template <int G, int NW>
+__device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* flag, int row, int kvh, int split,
+                                                 int n_i, int64_t slot, int gtid, int bar_id) {
+    for (int idx = gtid; idx < G * kD; idx += NW * 32) {
         const int hh = idx / kD, dd = idx % kD;
         if (n_i <= 1) {
             const int64_t o = (int64_t)row * p.Hq + kvh * G + hh;
@@ -235,6 +258,7 @@ __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int row,
             }
         }
     }
+    if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED) fused_complete<G, NW>(p, flag, row, kvh, split, n_i, slot, gtid, bar_id);
 }
 
 // A group of NW warps (rows w0, w0+wstride, ... of `cb`) has processed one task.  Combines the
@@ -272,22 +296,8 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
             }
         }
     }
-    if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED) {
-        __threadfence();  // partial state visible device-wide before the completion count
-        group_sync<NW>(bar_id);
-        if (gtid == 0) {
-            const int old = atomicAdd(&p.fuse_counters[row * p.Hkv + kvh], 1);
-            const int last = (old == n_i - 1);
-            if (last) p.fuse_counters[row * p.Hkv + kvh] = 0;  // self-reset for the next replay
-            cb.flag[w0] = last;
-        }
-        group_sync<NW>(bar_id);
-        if (cb.flag[w0]) {
-            __threadfence();
-            const int64_t base = slot - split;  // first slot of (row, kvh): DESIGN.md A8
-            for (int hh = gtid >> 5; hh < G; hh += NW) merge_head_warp<G>(p, base, n_i, row, kvh, hh, gtid & 31);
-        }
-    }
+    if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED)
+        fused_complete<G, NW>(p, &cb.flag[w0], row, kvh, split, n_i, slot, gtid, bar_id);
     group_sync<NW>(bar_id);  // cb rows may be refilled after this
 }
 
