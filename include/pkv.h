@@ -157,6 +157,20 @@ PKV_API pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* po
                               void* stream);
 
 /*
+ * The same step with an explicit choice of launches: `stages` is a bit set of pkv_stage.
+ * pkv_decode(build_queue) == pkv_decode_stages(DECODE | MERGE | (build_queue ? BUILD : 0)).
+ * A stage left out is simply not launched (the queue / the partial states of an earlier call in
+ * `workspace` are used as they are): this is how bench.py times the decode kernel alone with CUDA
+ * events and how a caller overlaps the builder of step t+1 with other work.  With MERGE left out
+ * and more than one split per row, `out` is not written for those rows.
+ */
+typedef enum { PKV_STAGE_BUILD = 1, PKV_STAGE_DECODE = 2, PKV_STAGE_MERGE = 4, PKV_STAGE_ALL = 7 } pkv_stage;
+PKV_API pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                                     const void* k_cache, const void* v_cache, const int32_t* block_table,
+                                     const int32_t* seq_lens, void* out, float* lse, float scale,
+                                     uint32_t stages, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Exact merge of split states (segmented over each row's compact slot range,
  * PAPER.md:75).  Public partial-state format, all FP32, natural-log domain:
  *   part_m [slots, G], part_l [slots, G], part_acc [slots, G, d],
@@ -207,6 +221,8 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
  * 0 = automatic (largest of 8/4/2/1 dividing Hkv that leaves >= one work unit per SM), else
  * 1, 2, 4 or 8 (ignored when it does not divide Hkv).  Process-wide. */
 PKV_API void pkv_debug_force_heads_per_cta(int heads);
+/* Test hook: 0 launches the kernels without programmatic dependent launch. Process-wide. */
+PKV_API void pkv_debug_set_pdl(int on);
 
 #ifdef __cplusplus
 }

@@ -22,6 +22,7 @@ ROUTE_RECT, ROUTE_WORKQUEUE = 0, 1
 MERGE_SEPARATE, MERGE_FUSED = 0, 1
 SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK = 0, 1
 KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
+STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL = 1, 2, 4, 7
 
 _i32, _i64 = ctypes.c_int32, ctypes.c_int64
 _vp = ctypes.c_void_p
@@ -52,8 +53,8 @@ class pkv_counters(ctypes.Structure):
 
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_build_workqueue_host",
-           "pkv_build_workqueue", "pkv_decode", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
-           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_heads_per_cta")
+           "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
+           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_heads_per_cta", "pkv_debug_set_pdl")
 
 
 class PkvError(RuntimeError):
@@ -81,6 +82,9 @@ def _load() -> ctypes.CDLL:
     lib.pkv_decode.restype = _i32
     lib.pkv_decode.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float,
                                _i32, _vp, ctypes.c_size_t, _vp]
+    lib.pkv_decode_stages.restype = _i32
+    lib.pkv_decode_stages.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp,
+                                      ctypes.c_float, ctypes.c_uint32, _vp, ctypes.c_size_t, _vp]
     lib.pkv_merge.restype = _i32
     lib.pkv_merge.argtypes = [P(pkv_shape), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.pkv_get_counters.restype = _i32
@@ -96,6 +100,8 @@ def _load() -> ctypes.CDLL:
                                     _vp, _vp, ctypes.c_size_t, _vp, ctypes.c_size_t, _vp, P(pkv_counters)]
     lib.pkv_debug_force_heads_per_cta.restype = None
     lib.pkv_debug_force_heads_per_cta.argtypes = [ctypes.c_int]
+    lib.pkv_debug_set_pdl.restype = None
+    lib.pkv_debug_set_pdl.argtypes = [ctypes.c_int]
     return lib
 
 
@@ -220,6 +226,14 @@ def pkv_decode(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, s
                            1 if build_queue else 0, _ptr(workspace), _nbytes(workspace), _stream_ptr(stream)))
 
 
+def pkv_decode_stages(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, seq_lens, out, lse=None,
+                      scale: float = 0.0, stages: int = STAGE_ALL, workspace=None, stream=None) -> None:
+    _check(_lib.pkv_decode_stages(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(q), _ptr(k_cache),
+                                  _ptr(v_cache), _ptr(block_table), _ptr(seq_lens), _ptr(out), _ptr(lse),
+                                  ctypes.c_float(scale), int(stages), _ptr(workspace), _nbytes(workspace),
+                                  _stream_ptr(stream)))
+
+
 def pkv_merge(shape: Shape, part_m, part_l, part_acc, split_offsets, out, lse=None, stream=None) -> None:
     _check(_lib.pkv_merge(ctypes.byref(shape.c()), _ptr(part_m), _ptr(part_l), _ptr(part_acc), _ptr(split_offsets),
                           _ptr(out), _ptr(lse), _stream_ptr(stream)))
@@ -267,3 +281,7 @@ def pkv_decode_host(shape: Shape, policy: Policy, q_host, k_cache_dev, v_cache_d
 
 def pkv_debug_force_heads_per_cta(heads: int) -> None:
     _lib.pkv_debug_force_heads_per_cta(int(heads))
+
+
+def pkv_debug_set_pdl(on: bool) -> None:
+    _lib.pkv_debug_set_pdl(1 if on else 0)

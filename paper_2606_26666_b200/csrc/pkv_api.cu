@@ -12,6 +12,8 @@
 
 namespace pkv {
 
+bool g_use_pdl = true;  // test hook (pkv_debug_set_pdl)
+
 namespace {
 
 int g_force_hg = 0;  // test hook: 0 = automatic heads-per-CTA, else 1/2/4/8
@@ -134,6 +136,7 @@ pkv_status cuda_fail(cudaError_t e, const char* what) {
 struct QueuePtrs {
     QueueHeader* hdr;
     int32_t* split_offsets;
+    RowSlot* rowslots;
     pkv_task* tasks;
 };
 
@@ -148,6 +151,7 @@ WsPtrs carve(void* workspace, const WorkspaceLayout& L) {
     WsPtrs r;
     r.q.hdr = reinterpret_cast<QueueHeader*>(w + L.header);
     r.q.split_offsets = reinterpret_cast<int32_t*>(w + L.split_offsets);
+    r.q.rowslots = reinterpret_cast<RowSlot*>(w + L.rowslots);
     r.q.tasks = reinterpret_cast<pkv_task*>(w + L.tasks);
     r.fuse_counters = reinterpret_cast<int32_t*>(w + L.fuse_counters);
     r.part_m = reinterpret_cast<float*>(w + L.part_m);
@@ -168,7 +172,7 @@ pkv_status check_workspace(const void* workspace, size_t bytes, const WorkspaceL
 pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, const void* k_cache, const void* v_cache,
                       const int32_t* block_table, const int32_t* seq_lens, void* out, float* lse, float scale,
                       const QueuePtrs& qp, const WsPtrs& ws, int64_t known_tasks, int known_max_n, int64_t known_slots,
-                      int num_sms,
+                      int num_sms, uint32_t stages,
                       cudaStream_t stream, int* decode_launches, int* merge_launches) {
     DecodeParams p;
     std::memset(&p, 0, sizeof(p));
@@ -179,6 +183,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.block_table = block_table;
     p.seq_lens = seq_lens;
     p.tasks = qp.tasks;
+    p.rowslots = qp.rowslots;
     p.split_offsets = qp.split_offsets;
     p.hdr = qp.hdr;
     p.out = static_cast<__half*>(out);
@@ -198,7 +203,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     if (s.B == 0) return PKV_OK;
     const int64_t bound = known_tasks >= 0 ? known_tasks : (int64_t)s.B * s.Hkv * rp.S;
     cudaError_t e;
-    if (known_tasks == 0) {
+    if (known_tasks == 0 && (stages & PKV_STAGE_DECODE)) {
         // every row is empty: out = 0, lse = -inf, no decode launch
         e = cudaMemsetAsync(out, 0, (size_t)s.B * s.Hq * s.d * 2, stream);
         if (e != cudaSuccess) return cuda_fail(e, "memset out");
@@ -211,7 +216,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             }
         }
     }
-    if (known_tasks != 0) {
+    if (known_tasks != 0 && (stages & PKV_STAGE_DECODE)) {
         if (rp.kernel == PKV_KERNEL_TMA_MMA) {
             const int64_t row_slots = known_slots >= 0 ? known_slots : (int64_t)s.B * rp.S;
             const int HG = choose_heads_per_cta(s.Hkv, row_slots, num_sms);
@@ -233,7 +238,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
         if (e != cudaSuccess) return cuda_fail(e, "decode launch");
         if (decode_launches) *decode_launches = 1;
     }
-    const bool need_merge = rp.merge_mode == PKV_MERGE_SEPARATE &&
+    const bool need_merge = (stages & PKV_STAGE_MERGE) && rp.merge_mode == PKV_MERGE_SEPARATE &&
                             (known_max_n >= 0 ? known_max_n > 1 : rp.S > 1) && known_tasks != 0;
     if (need_merge) {
         e = launch_merge(p, rp.G, stream);
@@ -262,6 +267,7 @@ using namespace pkv;
 extern "C" {
 
 void pkv_debug_force_heads_per_cta(int hg) { g_force_hg = hg; }
+void pkv_debug_set_pdl(int on) { g_use_pdl = on != 0; }
 
 pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_policy* policy, const int32_t* seq_lens_dev,
                                void* workspace, size_t workspace_bytes, void* stream) {
@@ -275,20 +281,22 @@ pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_policy* p
     if (st != PKV_OK) return st;
     const WsPtrs ws = carve(workspace, L);
     const cudaError_t e = launch_builder(*shape, rp, seq_lens_dev, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
-                                         ws.q.tasks, L.slots_cap, static_cast<cudaStream_t>(stream));
+                                         ws.q.rowslots, ws.q.tasks, L.slots_cap, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     return PKV_OK;
 }
 
-pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q, const void* k_cache,
-                      const void* v_cache, const int32_t* block_table, const int32_t* seq_lens, void* out, float* lse,
-                      float scale, int32_t build_queue, void* workspace, size_t workspace_bytes, void* stream) {
+pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                             const void* k_cache, const void* v_cache, const int32_t* block_table,
+                             const int32_t* seq_lens, void* out, float* lse, float scale, uint32_t stages,
+                             void* workspace, size_t workspace_bytes, void* stream) {
     clear_error();
     Resolved rp;
     const int sms = device_sm_count();
     pkv_status st = validate_and_resolve(shape, policy, sms, false, &rp);
     if (st != PKV_OK) return st;
     if (sms <= 0) { set_error("no CUDA device"); return PKV_ERR_CUDA; }
+    if (stages & ~(uint32_t)PKV_STAGE_ALL) { set_error("unknown stage bits 0x%x", stages); return PKV_ERR_INVALID_ARG; }
     st = check_decode_ptrs(*shape, q, k_cache, v_cache, block_table, seq_lens, out);
     if (st != PKV_OK) return st;
     const WorkspaceLayout L = workspace_layout(*shape, rp.S);
@@ -296,13 +304,21 @@ pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, co
     if (st != PKV_OK) return st;
     const WsPtrs ws = carve(workspace, L);
     cudaStream_t cs = static_cast<cudaStream_t>(stream);
-    if (build_queue) {
+    if (stages & PKV_STAGE_BUILD) {
         const cudaError_t e = launch_builder(*shape, rp, seq_lens, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
-                                             ws.q.tasks, L.slots_cap, cs);
+                                             ws.q.rowslots, ws.q.tasks, L.slots_cap, cs);
         if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     }
     return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, out, lse, scale, ws.q, ws, -1, -1, -1, sms,
-                      cs, nullptr, nullptr);
+                      stages, cs, nullptr, nullptr);
+}
+
+pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q, const void* k_cache,
+                      const void* v_cache, const int32_t* block_table, const int32_t* seq_lens, void* out, float* lse,
+                      float scale, int32_t build_queue, void* workspace, size_t workspace_bytes, void* stream) {
+    return pkv_decode_stages(shape, policy, q, k_cache, v_cache, block_table, seq_lens, out, lse, scale,
+                             PKV_STAGE_DECODE | PKV_STAGE_MERGE | (build_queue ? PKV_STAGE_BUILD : 0), workspace,
+                             workspace_bytes, stream);
 }
 
 pkv_status pkv_merge(const pkv_shape* shape, const float* part_m, const float* part_l, const float* part_acc,
@@ -424,11 +440,11 @@ namespace pkv {
 namespace {
 
 // Image of one step's host inputs, identical in the pinned staging buffer and in dev_scratch:
-//   [QueueHeader][split_offsets B+1][seq_lens B][q B*Hq*d f16][block_table B*max_pages][tasks ...]
+//   [QueueHeader][split_offsets B+1][seq_lens B][q B*Hq*d f16][block_table B*max_pages][rowslots B*S][tasks ...]
 // followed (device only) by the FP16 output.  Tasks are last so that one H2D copy of
 // (tasks_off + num_tasks * 20) bytes moves exactly what the step needs.
 struct HostImage {
-    size_t hdr, split_offsets, seq_lens, q, block_table, tasks, tasks_end, out, total;
+    size_t hdr, split_offsets, seq_lens, q, block_table, rowslots, tasks, tasks_end, out, total;
 };
 HostImage host_image(const pkv_shape& s, int32_t S) {
     HostImage h;
@@ -438,6 +454,7 @@ HostImage host_image(const pkv_shape& s, int32_t S) {
     h.seq_lens = off;      off = align_up(off + 4 * (size_t)s.B, 256);
     h.q = off;             off = align_up(off + 2 * (size_t)s.B * s.Hq * s.d, 256);
     h.block_table = off;   off = align_up(off + 4 * (size_t)s.B * s.max_pages, 256);
+    h.rowslots = off;      off = align_up(off + sizeof(RowSlot) * (size_t)s.B * S, 256);
     h.tasks = off;         off = align_up(off + sizeof(pkv_task) * (size_t)s.B * s.Hkv * S, 256);
     h.tasks_end = off;
     h.out = off;           off = align_up(off + 2 * (size_t)s.B * s.Hq * s.d, 256);
@@ -489,7 +506,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     QueueHeader* hdr = reinterpret_cast<QueueHeader*>(hs + im.hdr);
     st = plan_host(s, rp, seq_lens_host, reinterpret_cast<pkv_task*>(hs + im.tasks),
                    (int32_t)((im.tasks_end - im.tasks) / sizeof(pkv_task)),
-                   reinterpret_cast<int32_t*>(hs + im.split_offsets), hdr);
+                   reinterpret_cast<int32_t*>(hs + im.split_offsets), reinterpret_cast<RowSlot*>(hs + im.rowslots), hdr);
     if (st != PKV_OK) { set_error("host plan overflow"); return st; }
     std::memcpy(hs + im.seq_lens, seq_lens_host, 4 * (size_t)s.B);
     std::memcpy(hs + im.q, q_host, 2 * (size_t)s.B * s.Hq * s.d);
@@ -506,11 +523,12 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     QueuePtrs qp;
     qp.hdr = reinterpret_cast<QueueHeader*>(ds + im.hdr);
     qp.split_offsets = reinterpret_cast<int32_t*>(ds + im.split_offsets);
+    qp.rowslots = reinterpret_cast<RowSlot*>(ds + im.rowslots);
     qp.tasks = reinterpret_cast<pkv_task*>(ds + im.tasks);
     int dl = 0, ml = 0;
     st = run_decode(s, rp, ds + im.q, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
                     reinterpret_cast<const int32_t*>(ds + im.seq_lens), ds + im.out, nullptr, scale, qp, ws,
-                    hdr->num_tasks, hdr->max_row_splits, hdr->total_row_slots, sms, cs, &dl, &ml);
+                    hdr->num_tasks, hdr->max_row_splits, hdr->total_row_slots, sms, PKV_STAGE_ALL, cs, &dl, &ml);
     if (st != PKV_OK) return st;
     const size_t out_bytes = 2 * (size_t)s.B * s.Hq * s.d;
     e = cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);

@@ -8,36 +8,42 @@ namespace pkv {
 
 namespace {
 
-constexpr int kBuildThreads = 1024;
+constexpr int kBuildThreadsMax = 1024;
 
 struct BuildArgs {
     const int32_t* seq_lens;
     QueueHeader* hdr;
     int32_t* split_offsets;
     int32_t* fuse_counters;
+    RowSlot* rowslots;
     pkv_task* tasks;
     int64_t tasks_cap;
     int32_t B, Hkv, S, tile_tokens, split_mode, chunk_tiles, route;
 };
 
-// One CTA.  Phase 1: per-row slot counts and their exclusive prefix sum (split_offsets).
-// Phase 2: every thread fills task entries idx = tid, tid + 1024, ...; the row of an entry is
-// found by binary search in split_offsets, so the list comes out in (row, kvh, split) order.
-__global__ void __launch_bounds__(kBuildThreads) pkv_build_workqueue_kernel(const BuildArgs a) {
+// One CTA (blockDim.x = 128 .. 1024, a multiple of 32).
+// Phase 1: per-row slot counts and their exclusive prefix sum (split_offsets).
+// Phase 2: one thread per (row, split) pair rs = tid, tid + blockDim.x, ...: the row is found by
+// binary search in split_offsets; the thread writes the pair's RowSlot and its Hkv task entries
+// at so*Hkv + g*n + s, so the list comes out in (row, kvh, split) order.
+__global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(const BuildArgs a) {
     __shared__ int32_t warp_sums[32];
     __shared__ int32_t carry_s;
     __shared__ int32_t max_n_s, empties_s;
     __shared__ unsigned long long sum_seq_s;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthreads = blockDim.x, nwarps = nthreads >> 5;
+    pdl_launch_dependents();
     if (tid == 0) {
         carry_s = 0;
         max_n_s = 0;
         empties_s = 0;
         sum_seq_s = 0ull;
-        a.split_offsets[0] = 0;
     }
+    pdl_wait();   // the queue may still be read by the previous step's kernels
+    if (tid == 0) a.split_offsets[0] = 0;
     __syncthreads();
-    for (int base = 0; base < a.B; base += kBuildThreads) {
+    for (int base = 0; base < a.B; base += nthreads) {
         const int i = base + tid;
         int32_t slots = 0, N = 0;
         if (i < a.B) {
@@ -55,7 +61,7 @@ __global__ void __launch_bounds__(kBuildThreads) pkv_build_workqueue_kernel(cons
         if (lane == 31) warp_sums[warp] = v;
         __syncthreads();
         if (warp == 0) {
-            int32_t w = warp_sums[lane];
+            int32_t w = lane < nwarps ? warp_sums[lane] : 0;
 #pragma unroll
             for (int off = 1; off < 32; off <<= 1) {
                 const int32_t u = __shfl_up_sync(0xffffffffu, w, off);
@@ -71,28 +77,27 @@ __global__ void __launch_bounds__(kBuildThreads) pkv_build_workqueue_kernel(cons
             atomicAdd(&sum_seq_s, (unsigned long long)N);
         }
         __syncthreads();
-        if (tid == kBuildThreads - 1) carry_s = incl;
+        if (tid == nthreads - 1) carry_s = incl;
         __syncthreads();
     }
-    for (int i = tid; i < a.B * a.Hkv; i += kBuildThreads) a.fuse_counters[i] = 0;
+    for (int i = tid; i < a.B * a.Hkv; i += nthreads) a.fuse_counters[i] = 0;
     __threadfence_block();
     __syncthreads();
 
-    const int64_t total = (int64_t)carry_s * a.Hkv;
-    const int64_t lim = total < a.tasks_cap ? total : a.tasks_cap;
+    const int32_t row_slots = carry_s;
+    const int64_t total = (int64_t)row_slots * a.Hkv;
     int32_t my_empties = 0;
-    for (int64_t idx = tid; idx < lim; idx += kBuildThreads) {
-        // largest row with split_offsets[row] * Hkv <= idx
+    for (int32_t rs = tid; rs < row_slots; rs += nthreads) {
+        // largest row with split_offsets[row] <= rs
         int lo = 0, hi = a.B - 1;
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;
-            if ((int64_t)a.split_offsets[mid] * a.Hkv <= idx) lo = mid; else hi = mid - 1;
+            if (a.split_offsets[mid] <= rs) lo = mid; else hi = mid - 1;
         }
         const int row = lo;
         const int32_t so = a.split_offsets[row];
         const int32_t slots = a.split_offsets[row + 1] - so;
-        const int32_t local = (int32_t)(idx - (int64_t)so * a.Hkv);
-        const int32_t g = local / slots, s = local % slots;
+        const int32_t s = rs - so;
         const int32_t N = max(a.seq_lens[row], 0);
         const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
         int32_t tb = 0, te = 0;
@@ -101,18 +106,29 @@ __global__ void __launch_bounds__(kBuildThreads) pkv_build_workqueue_kernel(cons
             tb = (int32_t)(b < r.T ? b : r.T);
             te = (int32_t)(e < r.T ? e : r.T);
         }
-        if (tb >= te) ++my_empties;
-        pkv_task t;
-        t.row = row; t.kvh = g; t.split = s; t.t_begin = tb; t.t_end = te;
-        a.tasks[idx] = t;
+        if (tb >= te) my_empties += a.Hkv;
+        RowSlot d;
+        d.row = row; d.so = so; d.n = slots; d.split = s;
+        d.tok0 = tb * a.tile_tokens;
+        d.tok1 = min(te * a.tile_tokens, N);
+        d.pad_[0] = d.pad_[1] = 0;
+        a.rowslots[rs] = d;
+        for (int g = 0; g < a.Hkv; ++g) {
+            const int64_t idx = (int64_t)so * a.Hkv + (int64_t)g * slots + s;
+            if (idx < a.tasks_cap) {
+                pkv_task t;
+                t.row = row; t.kvh = g; t.split = s; t.t_begin = tb; t.t_end = te;
+                a.tasks[idx] = t;
+            }
+        }
     }
     if (my_empties) atomicAdd(&empties_s, my_empties);
     __syncthreads();
     if (tid == 0) {
         QueueHeader h;
-        h.num_tasks = (int32_t)lim;
+        h.num_tasks = (int32_t)(total < a.tasks_cap ? total : a.tasks_cap);
         h.max_row_splits = max_n_s;
-        h.total_row_slots = carry_s;
+        h.total_row_slots = row_slots;
         h.resolved_splits = a.S;
         h.empty_tasks = empties_s;
         h.work_counter = 0;
@@ -134,16 +150,18 @@ __global__ void __launch_bounds__(128) pkv_merge_kernel(const DecodeParams p) {
     const int row = blockIdx.x / p.Hq, h = blockIdx.x % p.Hq;
     const int kvh = h / G, hh = h % G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    pdl_launch_dependents();
+    pdl_wait();
     const int so = p.split_offsets[row];
     const int n = p.split_offsets[row + 1] - so;
     if (n <= 1 && p.hdr != nullptr) return;   // library path: decode already produced out/lse
     const int64_t base = (int64_t)so * p.Hkv + (int64_t)kvh * n;
     const float M = merge_row_max<G>(p, base, n, hh, lane);
-    float L;
-    float4 A;
-    merge_partial<G>(p, base, n, hh, M, warp, lane, L, A);
-    sA[warp][lane] = A;
-    if (lane == 0) sL[warp] = L;
+    float L[1];
+    float4 A[1];
+    merge_accumulate<G, 1>(p, base, n, hh, M, warp, 4, lane, L, A);
+    sA[warp][lane] = A[0];
+    if (lane == 0) sL[warp] = L[0];
     __syncthreads();
     if (warp == 0) {
         const float Ls = ((sL[0] + sL[1]) + sL[2]) + sL[3];
@@ -159,29 +177,30 @@ __global__ void __launch_bounds__(128) pkv_merge_kernel(const DecodeParams p) {
 }  // namespace
 
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
-                           QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, pkv_task* tasks,
-                           int64_t tasks_cap, cudaStream_t stream) {
+                           QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
+                           pkv_task* tasks, int64_t tasks_cap, cudaStream_t stream) {
     BuildArgs a;
     a.seq_lens = seq_lens_dev;
     a.hdr = hdr;
     a.split_offsets = split_offsets;
     a.fuse_counters = fuse_counters;
+    a.rowslots = rowslots;
     a.tasks = tasks;
     a.tasks_cap = tasks_cap;
     a.B = shape.B; a.Hkv = shape.Hkv; a.S = rp.S; a.tile_tokens = rp.tile_tokens;
     a.split_mode = rp.split_mode; a.chunk_tiles = rp.chunk_tiles; a.route = rp.route;
-    pkv_build_workqueue_kernel<<<1, kBuildThreads, 0, stream>>>(a);
-    return cudaGetLastError();
+    // one thread per (row, split) pair if that fits in a CTA, 128..1024 threads
+    const int64_t want = (int64_t)shape.B * rp.S;
+    int threads = 128;
+    while (threads < kBuildThreadsMax && threads < want) threads <<= 1;
+    return launch_pdl(pkv_build_workqueue_kernel, dim3(1), dim3(threads), 0, stream, a);
 }
 
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     const int grid = p.B * p.Hq;
     if (grid <= 0) return cudaSuccess;
-    if (G == 4)
-        pkv_merge_kernel<4><<<grid, 128, 0, stream>>>(p);
-    else
-        pkv_merge_kernel<8><<<grid, 128, 0, stream>>>(p);
-    return cudaGetLastError();
+    if (G == 4) return launch_pdl(pkv_merge_kernel<4>, dim3(grid), dim3(128), 0, stream, p);
+    return launch_pdl(pkv_merge_kernel<8>, dim3(grid), dim3(128), 0, stream, p);
 }
 
 }  // namespace pkv

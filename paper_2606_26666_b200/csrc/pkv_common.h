@@ -36,6 +36,19 @@ struct QueueHeader {
 };
 static_assert(sizeof(QueueHeader) == 64, "QueueHeader layout");
 
+// One (row, split) pair of the queue: what a work unit of the TMA kernel needs, in one 32-byte
+// load (the Hkv tasks of the pair share it; task(i, g, s) sits at so*Hkv + g*n + s).  Private.
+struct RowSlot {
+    int32_t row;
+    int32_t so;     // split_offsets[row]
+    int32_t n;      // slots of the row (n_i, or S on the rect route)
+    int32_t split;
+    int32_t tok0;   // token range [tok0, tok1) -- empty when tok0 >= tok1
+    int32_t tok1;
+    int32_t pad_[2];
+};
+static_assert(sizeof(RowSlot) == 32, "RowSlot layout");
+
 // Policy with every "0 = auto" field resolved.
 struct Resolved {
     int32_t S;          // split count (FIXED_COUNT) or cap on n_i (FIXED_CHUNK)
@@ -50,7 +63,7 @@ struct Resolved {
 
 // Byte offsets inside the caller's workspace.  Pure function of (shape, S bound).
 struct WorkspaceLayout {
-    size_t header, split_offsets, fuse_counters, tasks, part_m, part_l, part_acc, total;
+    size_t header, split_offsets, fuse_counters, rowslots, tasks, part_m, part_l, part_acc, total;
     int64_t slots_cap; // B * Hkv * S
 };
 
@@ -84,6 +97,7 @@ inline RowSplits row_splits(int32_t N, int32_t tile_tokens, int32_t split_mode, 
 
 // Host planner shared by pkv_build_workqueue_host and pkv_decode_host.
 pkv_status plan_host(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens,
-                     pkv_task* tasks, int32_t tasks_cap, int32_t* split_offsets, QueueHeader* hdr);
+                     pkv_task* tasks, int32_t tasks_cap, int32_t* split_offsets, RowSlot* rowslots,
+                     QueueHeader* hdr);
 
 }  // namespace pkv

@@ -43,6 +43,8 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
     const int hw = lane >> 4;   // half-warp: which of the warp's two tokens
     const int ch = lane & 15;   // 16-byte chunk of the 256-byte row: channels ch*8 .. ch*8+7
 
+    pdl_launch_dependents();
+    pdl_wait();
     zero_empty_rows(p);
     const int num_tasks = p.hdr->num_tasks;
     for (int t = blockIdx.x; t < num_tasks; t += gridDim.x) {
@@ -163,11 +165,8 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
 
 cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
-    if (G == 4)
-        pkv_decode_simt_kernel<4><<<grid, kThreads, 0, stream>>>(p);
-    else
-        pkv_decode_simt_kernel<8><<<grid, kThreads, 0, stream>>>(p);
-    return cudaGetLastError();
+    if (G == 4) return launch_pdl(pkv_decode_simt_kernel<4>, dim3(grid), dim3(kThreads), 0, stream, p);
+    return launch_pdl(pkv_decode_simt_kernel<8>, dim3(grid), dim3(kThreads), 0, stream, p);
 }
 
 }  // namespace pkv

@@ -42,7 +42,8 @@ __host__ __device__ constexpr int producers_for(int HG) { return HG >= 4 ? 1 : (
 
 struct UnitInfo {
     int unit;   // -1: no more work
-    int row;
+    int row, so, n, split, tok0, tok1;   // the unit's RowSlot
+    int pad_;
 };
 
 template <int G>
@@ -89,6 +90,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
     const uint32_t rfull0 = smem_u32(&tail.ring_full[0]);
     const uint32_t rempty0 = smem_u32(&tail.ring_empty[0]);
 
+    pdl_launch_dependents();
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) {
             mbar_init(fullk0 + 8 * s, 1);
@@ -103,14 +105,16 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
         tma_prefetch_desc(&tmap_k);
         tma_prefetch_desc(&tmap_v);
     }
-    zero_empty_rows(p);
     __syncthreads();
+    pdl_wait();   // queue (builder), q / seq_lens (upstream), out / partials (previous step's readers)
+    zero_empty_rows(p);
 
     const int HGn = p.Hkv / HG;                               // head groups per (row, split)
-    const int num_units = p.hdr->total_row_slots * HGn;
 
     // ---- unit hand-out (producer 0) / pick-up (everybody else) -------------------------------
-    int cur_row = 0;   // producer 0: units arrive in increasing order, so the row only moves forward
+    // producer 0 reads the unit's RowSlot (one 32-byte load; the first one is issued together with
+    // the header load) and publishes it on the ring; everybody else picks it up from shared memory
+    int num_units = 0;
     auto next_unit = [&](int k) -> UnitInfo {
         const int r = k % kRing;
         UnitInfo u;
@@ -123,13 +127,13 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 if (lane == 0) t = atomicAdd(&p.hdr->work_counter, 1) + gridDim.x;
                 t = __shfl_sync(0xffffffffu, t, 0);
             }
+            const int4* rsp = reinterpret_cast<const int4*>(p.rowslots + (k == 0 ? t / HGn : min(t, max(num_units - 1, 0)) / HGn));
+            const int4 a = __ldcg(rsp);
+            const int4 b = __ldcg(rsp + 1);
+            if (k == 0) num_units = __ldcg(&p.hdr->total_row_slots) * HGn;
             if (t >= num_units) t = -1;
-            if (t >= 0) {
-                const int rs = t / HGn;
-                while (p.split_offsets[cur_row + 1] <= rs) ++cur_row;
-            }
             u.unit = t;
-            u.row = cur_row;
+            u.row = a.x; u.so = a.y; u.n = a.z; u.split = a.w; u.tok0 = b.x; u.tok1 = b.y; u.pad_ = 0;
             if (lane == 0) {
                 mbar_wait(rempty0 + 8 * r, ((k / kRing) & 1) ^ 1);
                 tail.ring[r] = u;
@@ -151,26 +155,27 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
             const int row = u.row, hg = u.unit % HGn;
-            const int so = p.split_offsets[row];
-            const int split = u.unit / HGn - so;
-            const pkv_task task = p.tasks[(int64_t)so * p.Hkv + split];   // the kvh = 0 task of (row, split)
-            const int N = p.seq_lens[row];
-            const int tok0 = task.t_begin * p.tile_tokens;
-            const int tok1 = min(task.t_end * p.tile_tokens, N);
+            const int tok0 = u.tok0, tok1 = u.tok1;
             if (tok0 >= tok1) continue;  // empty split: nothing is staged
             const int p0 = tok0 >> 4;
             const int np = ((tok1 + 15) >> 4) - p0;
-            const int32_t* bt = p.block_table + (int64_t)row * p.max_pages + p0;
             const int head0 = hg * HG;
-            // this producer's pages: j = warp, warp + NP, ...; table entries 32 at a time
-            int mine = (warp + lane * NP < np) ? bt[warp + lane * NP] : 0;
-            for (int c = warp; c < np; c += 32 * NP) {
-                const int nxt = (c + (32 + lane) * NP < np) ? bt[c + (32 + lane) * NP] : 0;
-                const int cnt = min(32, (np - c + NP - 1) / NP);
+            // Page j of the unit has sequence number seq_base + j in this CTA's stream of pages and
+            // lands in stage (seq_base + j) % kStages.  A stage must always be filled by the same
+            // producer (its empty barrier carries one parity bit), so producer w takes the pages
+            // with (seq_base + j) % NP == w: the first is j0, then every NP-th.
+            const int j0 = (warp + NP - (int)(seq_base % NP)) % NP;
+            const int32_t* bt = p.block_table + (int64_t)row * p.max_pages + p0 + j0;
+            const int npw = np > j0 ? (np - j0 + NP - 1) / NP : 0;    // pages of this producer
+            // table entries 32 at a time (lane i holds this producer's i-th page of the batch)
+            int mine = lane < npw ? bt[lane * NP] : 0;
+            for (int c = 0; c < npw; c += 32) {
+                const int nxt = (c + 32 + lane < npw) ? bt[(c + 32 + lane) * NP] : 0;
+                const int cnt = min(32, npw - c);
                 for (int i = 0; i < cnt; ++i) {
                     const int page = __shfl_sync(0xffffffffu, mine, i);
                     if (lane == 0) {
-                        const uint32_t sq = seq_base + c + i * NP;
+                        const uint32_t sq = seq_base + j0 + (c + i) * NP;
                         const uint32_t s = sq % kStages;
                         mbar_wait(empty0 + 8 * s, ((sq / kStages) & 1) ^ 1);
                         const uint32_t dst = stage_base + s * kStageBytes;
@@ -214,15 +219,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
             const int row = u.row, hg = u.unit % HGn;
-            const int so = p.split_offsets[row];
-            const int n_i = p.split_offsets[row + 1] - so;
-            const int split = u.unit / HGn - so;
-            const pkv_task task = p.tasks[(int64_t)so * p.Hkv + split];
+            const int so = u.so, n_i = u.n, split = u.split;
             const int kvh = hg * HG + hl;
             const int64_t slot = (int64_t)so * p.Hkv + (int64_t)kvh * n_i + split;
-            const int N = p.seq_lens[row];
-            const int tok0 = task.t_begin * p.tile_tokens;
-            const int tok1 = min(task.t_end * p.tile_tokens, N);
+            const int tok0 = u.tok0, tok1 = u.tok1;
             if (tok0 >= tok1) {
                 store_empty_task<G, WPH>(p, &tail.cb.flag[hl], row, kvh, split, n_i, slot, gtid, 1 + hl);
                 continue;
@@ -355,8 +355,7 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    pkv_decode_tma_kernel<G, HG><<<grid, threads, smem, stream>>>(p, mk, mv);
-    return cudaGetLastError();
+    return launch_pdl(pkv_decode_tma_kernel<G, HG>, dim3(grid), dim3(threads), (size_t)smem, stream, p, mk, mv);
 }
 
 }  // namespace

@@ -6,6 +6,8 @@
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
+#include <utility>
+
 #include "pkv_common.h"
 
 namespace pkv {
@@ -20,6 +22,7 @@ struct DecodeParams {
     const int32_t* block_table; // [B, max_pages]
     const int32_t* seq_lens;    // [B]
     const pkv_task* tasks;
+    const RowSlot* rowslots;      // [split_offsets[B]] (row, split) pairs
     const int32_t* split_offsets; // [B+1]
     QueueHeader* hdr;
     __half* out;                // [B, Hq, d]
@@ -49,6 +52,11 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+
+// Programmatic dependent launch (PDL): every kernel of the step lets its successor's CTAs be
+// scheduled early and waits for its predecessor's results before touching global memory.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
@@ -144,25 +152,47 @@ __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
 template <int G>
 __device__ __forceinline__ float merge_row_max(const DecodeParams& p, int64_t slot_base, int n, int hh, int lane) {
     float M = -INFINITY;
-    for (int s = lane; s < n; s += 32) M = fmaxf(M, p.part_m[(slot_base + s) * G + hh]);
+    for (int s = lane; s < n; s += 32) M = fmaxf(M, __ldcg(p.part_m + (slot_base + s) * G + hh));
 #pragma unroll
     for (int off = 16; off >= 1; off >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, off));
     return M;
 }
 
-// P_k for one lane: interleaved partial sum k of (L, A[4 channels])
-template <int G>
-__device__ __forceinline__ void merge_partial(const DecodeParams& p, int64_t slot_base, int n, int hh, float M, int k,
-                                              int lane, float& L, float4& A) {
-    L = 0.f;
-    A = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 4
-    for (int s = k; s < n; s += 4) {
-        const int64_t r = (slot_base + s) * G + hh;
-        const float w = ex2_approx((p.part_m[r] - M) * kLog2e);  // exp2(-inf) = 0
-        const float4 a = *reinterpret_cast<const float4*>(p.part_acc + r * kD + lane * 4);
-        L = fmaf(w, p.part_l[r], L);
-        A.x = fmaf(w, a.x, A.x); A.y = fmaf(w, a.y, A.y); A.z = fmaf(w, a.z, A.z); A.w = fmaf(w, a.w, A.w);
+// NK interleaved partial sums of one lane's 4 channels over the states first, first+stride, ...:
+// NK = 4 (first 0, stride 1): state s goes to P_{s mod 4}; NK = 1 (first k, stride 4): P_k only.
+// Either way P_k is the same ascending fma chain, so one warp doing all four and four warps doing
+// one each give bit-identical sums.  kMergeBatch independent state loads are in flight per lane;
+// they bypass L1 (states are written by other SMs, in the fused path during this very launch).
+constexpr int kMergeBatch = 8;
+template <int G, int NK>
+__device__ __forceinline__ void merge_accumulate(const DecodeParams& p, int64_t slot_base, int n, int hh, float M,
+                                                 int first, int stride, int lane, float (&L)[NK], float4 (&A)[NK]) {
+#pragma unroll
+    for (int k = 0; k < NK; ++k) {
+        L[k] = 0.f;
+        A[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    const int cnt = n > first ? (n - first + stride - 1) / stride : 0;
+    for (int i0 = 0; i0 < cnt; i0 += kMergeBatch) {
+        float mv[kMergeBatch], lv[kMergeBatch];
+        float4 av[kMergeBatch];
+#pragma unroll
+        for (int j = 0; j < kMergeBatch; ++j) {
+            const bool ok = i0 + j < cnt;
+            const int64_t r = (slot_base + first + (int64_t)(ok ? i0 + j : 0) * stride) * G + hh;
+            mv[j] = ok ? __ldcg(p.part_m + r) : -INFINITY;
+            lv[j] = ok ? __ldcg(p.part_l + r) : 0.f;
+            av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * kD + lane * 4))
+                       : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int j = 0; j < kMergeBatch; ++j) {
+            const float w = ex2_approx((mv[j] - M) * kLog2e);  // exp2(-inf) = 0
+            const int k = NK == 4 ? (j & 3) : 0;
+            L[k] = fmaf(w, lv[j], L[k]);
+            A[k].x = fmaf(w, av[j].x, A[k].x); A[k].y = fmaf(w, av[j].y, A[k].y);
+            A[k].z = fmaf(w, av[j].z, A[k].z); A[k].w = fmaf(w, av[j].w, A[k].w);
+        }
     }
 }
 
@@ -187,8 +217,7 @@ __device__ __forceinline__ void merge_head_warp(const DecodeParams& p, int64_t s
     const float M = merge_row_max<G>(p, slot_base, n, hh, lane);
     float L[4];
     float4 A[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) merge_partial<G>(p, slot_base, n, hh, M, k, lane, L[k], A[k]);
+    merge_accumulate<G, 4>(p, slot_base, n, hh, M, 0, 1, lane, L, A);
     const float Ls = ((L[0] + L[1]) + L[2]) + L[3];
     float4 As;
     As.x = ((A[0].x + A[1].x) + A[2].x) + A[3].x;
@@ -313,13 +342,33 @@ __device__ __forceinline__ void zero_empty_rows(const DecodeParams& p) {
     }
 }
 
+// Launch with the programmatic-stream-serialization attribute: in a stream (and in a captured
+// graph) the kernel may start while its predecessor is still running; it orders itself with
+// pdl_wait().  g_use_pdl = false falls back to plain launches (test hook).
+extern bool g_use_pdl;
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                       Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = g_use_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 // launchers implemented in the .cu files
 cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStream_t stream);
 cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int grid, const void* tmap_k,
                               const void* tmap_v, cudaStream_t stream);
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
-                           QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, pkv_task* tasks,
-                           int64_t tasks_cap, cudaStream_t stream);
+                           QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
+                           pkv_task* tasks, int64_t tasks_cap, cudaStream_t stream);
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream);
 int decode_tma_smem_bytes(int G, int HG);
 

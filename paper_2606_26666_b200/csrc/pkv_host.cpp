@@ -102,6 +102,7 @@ WorkspaceLayout workspace_layout(const pkv_shape& s, int32_t S) {
     L.header = off;         off = align_up(off + sizeof(QueueHeader), 256);
     L.split_offsets = off;  off = align_up(off + sizeof(int32_t) * ((size_t)s.B + 1), 256);
     L.fuse_counters = off;  off = align_up(off + sizeof(int32_t) * ((size_t)s.B * s.Hkv + 1), 256);
+    L.rowslots = off;       off = align_up(off + sizeof(RowSlot) * (size_t)s.B * S, 256);
     L.tasks = off;          off = align_up(off + sizeof(pkv_task) * (size_t)L.slots_cap, 256);
     L.part_m = off;         off = align_up(off + sizeof(float) * (size_t)L.slots_cap * G, 256);
     L.part_l = off;         off = align_up(off + sizeof(float) * (size_t)L.slots_cap * G, 256);
@@ -111,7 +112,7 @@ WorkspaceLayout workspace_layout(const pkv_shape& s, int32_t S) {
 }
 
 pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_lens, pkv_task* tasks,
-                     int32_t tasks_cap, int32_t* split_offsets, QueueHeader* hdr) {
+                     int32_t tasks_cap, int32_t* split_offsets, RowSlot* rowslots, QueueHeader* hdr) {
     int64_t count = 0, sum_seq = 0;
     int32_t max_n = 0, empties = 0, off = 0;
     bool overflow = false;
@@ -138,6 +139,20 @@ pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_
                     overflow = true;
                 }
                 ++count;
+            }
+        }
+        if (rowslots) {
+            for (int32_t sp = 0; sp < slots; ++sp) {
+                RowSlot rs;
+                std::memset(&rs, 0, sizeof(rs));
+                rs.row = i; rs.so = off; rs.n = slots; rs.split = sp;
+                if (r.T > 0) {
+                    const int64_t b = (int64_t)sp * r.c, e = (int64_t)(sp + 1) * r.c;
+                    const int64_t t0 = (b < r.T ? b : r.T) * rp.tile_tokens, t1 = (e < r.T ? e : r.T) * rp.tile_tokens;
+                    rs.tok0 = (int32_t)t0;
+                    rs.tok1 = (int32_t)(t1 < N ? t1 : N);
+                }
+                rowslots[off + sp] = rs;
             }
         }
         off += slots;
@@ -183,7 +198,7 @@ pkv_status pkv_build_workqueue_host(const pkv_shape* shape, const pkv_split_poli
         return PKV_ERR_INVALID_ARG;
     }
     QueueHeader hdr;
-    st = plan_host(*shape, rp, seq_lens_host, tasks_out, tasks_cap, split_offsets_out, &hdr);
+    st = plan_host(*shape, rp, seq_lens_host, tasks_out, tasks_cap, split_offsets_out, nullptr, &hdr);
     *num_tasks_out = hdr.num_tasks;
     if (st == PKV_ERR_WORKSPACE) set_error("tasks_cap=%d < %d tasks", tasks_cap, hdr.num_tasks);
     return st;

@@ -341,3 +341,40 @@ def test_cuda_graph_replay_with_growing_lengths(mm):
             assert_within_tolerance(dp.out.cpu().numpy().astype(np.float64), oracle_attention(p)[0], "step %d" % step)
             tasks, _ = pkv.pkv_read_workqueue(dp.shape, pol, ws)
             assert tasks.shape[0] == wq.build_workqueue(list(lens + step), 8, oracle_policy(pol)).num_tasks
+
+
+@pytest.mark.parametrize("hg", [1, 2, 4, 8])
+def test_many_units_per_cta_odd_page_counts(hg):
+    """More work units than SMs, rows with odd page counts: every persistent CTA walks several
+    units, so its page ring wraps across unit boundaries with every residue of the page sequence
+    number (the stage-ownership rule of the multi-producer ring)."""
+    rng = np.random.Generator(np.random.PCG64(1234 + hg))
+    lens = rng.integers(1, 1500, size=96).astype(np.int32)
+    lens[::7] = rng.integers(1, 40, size=len(lens[::7]))          # some one- and two-page rows
+    p = make_problem(list(lens), seed=400 + hg)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    pkv.pkv_debug_force_heads_per_cta(hg)
+    try:
+        for pol in (pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=16, num_splits=3),
+                    pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=5,
+                               merge_mode=pkv.MERGE_FUSED)):
+            for _ in range(2):          # twice: the dynamic unit counter must have re-armed itself
+                check(dp, pol, ref, what="hg%d %s" % (hg, pol))
+    finally:
+        pkv.pkv_debug_force_heads_per_cta(0)
+
+
+def test_pdl_off_matches_pdl_on_bitwise():
+    """Programmatic dependent launch only changes when kernels start, never what they compute."""
+    p = make_problem([700, 33, 16, 257, 0, 2000], seed=23)
+    pol = pkv.Policy(tile_tokens=32, num_splits=5)
+    dp = DevProblem(p)
+    o1, l1, _ = dp.decode(pol)
+    pkv.pkv_debug_set_pdl(False)
+    try:
+        o2, l2, _ = dp.decode(pol)
+    finally:
+        pkv.pkv_debug_set_pdl(True)
+    assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
+    assert_within_tolerance(o1, oracle_attention(p)[0])
