@@ -14,6 +14,9 @@
  *   - the CALLER OWNS EVERY BUFFER (q, caches, tables, out, workspace).  pkv_build_workqueue,
  *     pkv_decode and pkv_merge never allocate, never synchronise and never read device data
  *     on the host, so all three may be captured into a CUDA graph.
+ *   - the first pkv_workspace_init_bytes() bytes of a workspace (the queue header and the
+ *     completion counters, all self-resetting) must be ZERO when the workspace is first used; the
+ *     library keeps them consistent from then on.
  *   - every call returns a pkv_status; nothing throws or aborts.  pkv_last_error() gives a
  *     thread-local description of the last non-OK status.
  *   - host-checkable arguments are rejected before any launch.  Device-resident values
@@ -122,6 +125,9 @@ PKV_API const char* pkv_last_error(void);
  * Pure function (no CUDA call).  Returns 0 on invalid arguments.  With num_splits == 0 and
  * num_sms == 0 the bound for S = 256 is returned. */
 PKV_API size_t pkv_workspace_bytes(const pkv_shape* shape, const pkv_split_policy* policy);
+/* Leading bytes of the workspace the caller must zero once before first use (a few hundred bytes +
+ * 4*B*Hkv).  Pure function; 0 on invalid arguments. */
+PKV_API size_t pkv_workspace_init_bytes(const pkv_shape* shape, const pkv_split_policy* policy);
 
 /* Split-bound policy + compact workqueue on the HOST.  Pure CPU, no CUDA.
  * seq_lens_host [B].  Writes at most tasks_cap tasks in canonical order (row, kvh, split --
@@ -147,8 +153,10 @@ PKV_API pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_p
  *   scale       <= 0 means 1/sqrt(d)        (natural-log LSE of the scaled scores)
  * build_queue != 0: runs the device builder first (as pkv_build_workqueue); 0: uses the queue
  * already in `workspace` (built for the same shape/policy and the same seq_lens values).
- * Launches: [builder] + decode + [merge]; the merge launch is skipped when the policy cannot
- * produce more than one split per row, or merge_mode is FUSED.
+ * Launches: [builder] + decode + [merge].  With the TMA kernel and B <= 512 the decode kernel
+ * derives the queue from seq_lens itself ("fused build": no builder launch; the queue is still
+ * written to the workspace, bit-identical to pkv_build_workqueue's).  The merge launch is skipped
+ * when the policy cannot produce more than one split per row, or merge_mode is FUSED.
  */
 PKV_API pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
                               const void* k_cache, const void* v_cache, const int32_t* block_table,
@@ -223,6 +231,12 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
 PKV_API void pkv_debug_force_heads_per_cta(int heads);
 /* Test hook: 0 launches the kernels without programmatic dependent launch. Process-wide. */
 PKV_API void pkv_debug_set_pdl(int on);
+/* Test hook: 0 makes pkv_decode run the builder as its own kernel even where the TMA decode kernel
+ * could derive the queue itself.  Process-wide. */
+PKV_API void pkv_debug_set_fused_build(int on);
+/* Debug hook: device buffer of grid*16 uint64 that the TMA decode kernel fills with %globaltimer
+ * stamps of its phases, or NULL to switch tracing off.  Process-wide. */
+PKV_API void pkv_debug_set_trace(void* dev_u64);
 
 #ifdef __cplusplus
 }

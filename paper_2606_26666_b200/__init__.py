@@ -10,14 +10,17 @@ from .binding import (  # noqa: F401
     ROUTE_RECT, ROUTE_WORKQUEUE, MERGE_SEPARATE, MERGE_FUSED, SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK,
     KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT, STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL, EXPORTS,
     PkvError, Shape, Policy,
-    pkv_version, pkv_last_error, pkv_workspace_bytes, pkv_host_scratch_bytes, pkv_build_workqueue_host,
+    pkv_version, pkv_last_error, pkv_workspace_bytes, pkv_workspace_init_bytes, pkv_host_scratch_bytes, pkv_build_workqueue_host,
     pkv_build_workqueue, pkv_decode, pkv_decode_stages, pkv_merge, pkv_get_counters, pkv_read_workqueue, pkv_workspace_partials,
-    pkv_decode_host, pkv_debug_force_heads_per_cta, pkv_debug_set_pdl,
+    pkv_decode_host, pkv_debug_force_heads_per_cta, pkv_debug_set_pdl, pkv_debug_set_fused_build, pkv_debug_set_trace,
 )
 
 
 def alloc_workspace(shape, policy, device="cuda"):
-    """A torch uint8 buffer of pkv_workspace_bytes(shape, policy) on ``device`` (plumbing only)."""
+    """A torch uint8 buffer of pkv_workspace_bytes(shape, policy) on ``device`` (plumbing only).
+    Its first pkv_workspace_init_bytes() bytes (queue header, completion counters) are zeroed, as include/pkv.h asks for a fresh workspace."""
     import torch
 
-    return torch.empty(pkv_workspace_bytes(shape, policy), dtype=torch.uint8, device=device)
+    ws = torch.empty(pkv_workspace_bytes(shape, policy), dtype=torch.uint8, device=device)
+    ws[:pkv_workspace_init_bytes(shape, policy)].zero_()
+    return ws

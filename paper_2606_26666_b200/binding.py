@@ -52,9 +52,9 @@ class pkv_counters(ctypes.Structure):
 
 
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_build_workqueue_host",
+EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspace_init_bytes", "pkv_build_workqueue_host",
            "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
-           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_heads_per_cta", "pkv_debug_set_pdl")
+           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_heads_per_cta", "pkv_debug_set_pdl", "pkv_debug_set_fused_build", "pkv_debug_set_trace")
 
 
 class PkvError(RuntimeError):
@@ -73,6 +73,8 @@ def _load() -> ctypes.CDLL:
     lib.pkv_last_error.restype = ctypes.c_char_p
     lib.pkv_workspace_bytes.restype = ctypes.c_size_t
     lib.pkv_workspace_bytes.argtypes = [P(pkv_shape), P(pkv_split_policy)]
+    lib.pkv_workspace_init_bytes.restype = ctypes.c_size_t
+    lib.pkv_workspace_init_bytes.argtypes = [P(pkv_shape), P(pkv_split_policy)]
     lib.pkv_host_scratch_bytes.restype = ctypes.c_size_t
     lib.pkv_host_scratch_bytes.argtypes = [P(pkv_shape), P(pkv_split_policy)]
     lib.pkv_build_workqueue_host.restype = _i32
@@ -102,6 +104,10 @@ def _load() -> ctypes.CDLL:
     lib.pkv_debug_force_heads_per_cta.argtypes = [ctypes.c_int]
     lib.pkv_debug_set_pdl.restype = None
     lib.pkv_debug_set_pdl.argtypes = [ctypes.c_int]
+    lib.pkv_debug_set_fused_build.restype = None
+    lib.pkv_debug_set_fused_build.argtypes = [ctypes.c_int]
+    lib.pkv_debug_set_trace.restype = None
+    lib.pkv_debug_set_trace.argtypes = [_vp]
     return lib
 
 
@@ -189,6 +195,13 @@ def pkv_workspace_bytes(shape: Shape, policy: Policy) -> int:
     n = int(_lib.pkv_workspace_bytes(ctypes.byref(shape.c()), ctypes.byref(policy.c())))
     if n == 0:
         raise PkvError(PKV_ERR_INVALID_ARG, "pkv_workspace_bytes: invalid shape/policy")
+    return n
+
+
+def pkv_workspace_init_bytes(shape: Shape, policy: Policy) -> int:
+    n = int(_lib.pkv_workspace_init_bytes(ctypes.byref(shape.c()), ctypes.byref(policy.c())))
+    if n == 0:
+        raise PkvError(PKV_ERR_INVALID_ARG, "pkv_workspace_init_bytes: invalid shape/policy")
     return n
 
 
@@ -285,3 +298,11 @@ def pkv_debug_force_heads_per_cta(heads: int) -> None:
 
 def pkv_debug_set_pdl(on: bool) -> None:
     _lib.pkv_debug_set_pdl(1 if on else 0)
+
+
+def pkv_debug_set_trace(dev_u64) -> None:
+    _lib.pkv_debug_set_trace(_ptr(dev_u64))
+
+
+def pkv_debug_set_fused_build(on: bool) -> None:
+    _lib.pkv_debug_set_fused_build(1 if on else 0)

@@ -16,6 +16,9 @@ bool g_use_pdl = true;  // test hook (pkv_debug_set_pdl)
 
 namespace {
 
+unsigned long long* g_trace = nullptr;  // debug hook
+bool g_fused_build = true;              // test hook (pkv_debug_set_fused_build)
+constexpr int kMaxFusedRows = 512;      // = pkv_decode_tma.cu
 int g_force_hg = 0;  // test hook: 0 = automatic heads-per-CTA, else 1/2/4/8
 
 int device_sm_count() {
@@ -172,7 +175,7 @@ pkv_status check_workspace(const void* workspace, size_t bytes, const WorkspaceL
 pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, const void* k_cache, const void* v_cache,
                       const int32_t* block_table, const int32_t* seq_lens, void* out, float* lse, float scale,
                       const QueuePtrs& qp, const WsPtrs& ws, int64_t known_tasks, int known_max_n, int64_t known_slots,
-                      int num_sms, uint32_t stages,
+                      int num_sms, uint32_t stages, bool fused_build, int64_t tasks_cap,
                       cudaStream_t stream, int* decode_launches, int* merge_launches) {
     DecodeParams p;
     std::memset(&p, 0, sizeof(p));
@@ -194,6 +197,10 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.B = s.B; p.Hq = s.Hq; p.Hkv = s.Hkv; p.max_pages = s.max_pages;
     p.tile_tokens = rp.tile_tokens; p.merge_mode = rp.merge_mode;
     p.dynamic_sched = 1;
+    p.plan = make_plan_args(s, rp);
+    p.tasks_cap = tasks_cap;
+    p.fused_build = fused_build ? 1 : 0;
+    p.trace = g_trace;
     const float sc = scale > 0.f ? scale : 1.0f / std::sqrt((float)s.d);
     p.scale = sc;
     p.scale_log2 = sc * kLog2e;
@@ -268,6 +275,8 @@ extern "C" {
 
 void pkv_debug_force_heads_per_cta(int hg) { g_force_hg = hg; }
 void pkv_debug_set_pdl(int on) { g_use_pdl = on != 0; }
+void pkv_debug_set_fused_build(int on) { g_fused_build = on != 0; }
+void pkv_debug_set_trace(void* dev) { g_trace = static_cast<unsigned long long*>(dev); }
 
 pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_policy* policy, const int32_t* seq_lens_dev,
                                void* workspace, size_t workspace_bytes, void* stream) {
@@ -304,13 +313,17 @@ pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_policy* pol
     if (st != PKV_OK) return st;
     const WsPtrs ws = carve(workspace, L);
     cudaStream_t cs = static_cast<cudaStream_t>(stream);
-    if (stages & PKV_STAGE_BUILD) {
+    // The TMA kernel derives the queue itself (fused build) when it runs in the same call;
+    // otherwise (builder alone, SIMT kernel, very large batches) the builder kernel runs first.
+    const bool fused = (stages & PKV_STAGE_BUILD) && (stages & PKV_STAGE_DECODE) && g_fused_build &&
+                       rp.kernel == PKV_KERNEL_TMA_MMA && shape->B <= kMaxFusedRows;
+    if ((stages & PKV_STAGE_BUILD) && !fused) {
         const cudaError_t e = launch_builder(*shape, rp, seq_lens, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
                                              ws.q.rowslots, ws.q.tasks, L.slots_cap, cs);
         if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     }
     return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, out, lse, scale, ws.q, ws, -1, -1, -1, sms,
-                      stages, cs, nullptr, nullptr);
+                      stages, fused, L.slots_cap, cs, nullptr, nullptr);
 }
 
 pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q, const void* k_cache,
@@ -340,7 +353,7 @@ pkv_status pkv_merge(const pkv_shape* shape, const float* part_m, const float* p
     p.part_m = const_cast<float*>(part_m);
     p.part_l = const_cast<float*>(part_l);
     p.part_acc = const_cast<float*>(part_acc);
-    p.split_offsets = split_offsets;
+    p.split_offsets = const_cast<int32_t*>(split_offsets);
     p.hdr = nullptr;
     p.out = static_cast<__half*>(out);
     p.lse = lse;
@@ -372,7 +385,7 @@ pkv_status pkv_get_counters(const pkv_shape* shape, const pkv_split_policy* poli
     host_out->decode_launches = h.num_tasks > 0 ? 1 : 0;
     host_out->merge_launches =
         (h.num_tasks > 0 && h.max_row_splits > 1 && rp.merge_mode == PKV_MERGE_SEPARATE) ? 1 : 0;
-    host_out->build_launches = 1;
+    host_out->build_launches = h.build_launches;
     host_out->useful_kv_bytes = h.sum_seq_lens * 2 * shape->Hkv * shape->d * 2;
     host_out->merge_bytes = (int64_t)h.num_tasks * rp.G * (shape->d + 2) * 4;
     host_out->num_splits = h.resolved_splits;
@@ -528,7 +541,8 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     int dl = 0, ml = 0;
     st = run_decode(s, rp, ds + im.q, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
                     reinterpret_cast<const int32_t*>(ds + im.seq_lens), ds + im.out, nullptr, scale, qp, ws,
-                    hdr->num_tasks, hdr->max_row_splits, hdr->total_row_slots, sms, PKV_STAGE_ALL, cs, &dl, &ml);
+                    hdr->num_tasks, hdr->max_row_splits, hdr->total_row_slots, sms, PKV_STAGE_ALL, false, L.slots_cap, cs, &dl,
+                    &ml);
     if (st != PKV_OK) return st;
     const size_t out_bytes = 2 * (size_t)s.B * s.Hq * s.d;
     e = cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);

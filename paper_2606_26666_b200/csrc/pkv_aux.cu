@@ -18,124 +18,40 @@ struct BuildArgs {
     RowSlot* rowslots;
     pkv_task* tasks;
     int64_t tasks_cap;
-    int32_t B, Hkv, S, tile_tokens, split_mode, chunk_tiles, route;
+    PlanArgs plan;
 };
 
-// One CTA (blockDim.x = 128 .. 1024, a multiple of 32).
-// Phase 1: per-row slot counts and their exclusive prefix sum (split_offsets).
-// Phase 2: one thread per (row, split) pair rs = tid, tid + blockDim.x, ...: the row is found by
-// binary search in split_offsets; the thread writes the pair's RowSlot and its Hkv task entries
-// at so*Hkv + g*n + s, so the list comes out in (row, kvh, split) order.
+// One CTA (blockDim.x = 128 .. 1024).  Phase 1: plan_scan -> split_offsets.  Phase 2: one thread
+// per (row, split) pair writes the pair's RowSlot and its Hkv task entries (pkv_device.cuh).
 __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(const BuildArgs a) {
-    __shared__ int32_t warp_sums[32];
-    __shared__ int32_t carry_s;
-    __shared__ int32_t max_n_s, empties_s;
-    __shared__ unsigned long long sum_seq_s;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nthreads = blockDim.x, nwarps = nthreads >> 5;
+    __shared__ PlanScratch sc;
+    const int tid = threadIdx.x, nthreads = blockDim.x;
     pdl_launch_dependents();
-    if (tid == 0) {
-        carry_s = 0;
-        max_n_s = 0;
-        empties_s = 0;
-        sum_seq_s = 0ull;
-    }
     pdl_wait();   // the queue may still be read by the previous step's kernels
-    if (tid == 0) a.split_offsets[0] = 0;
-    __syncthreads();
-    for (int base = 0; base < a.B; base += nthreads) {
-        const int i = base + tid;
-        int32_t slots = 0, N = 0;
-        if (i < a.B) {
-            N = max(a.seq_lens[i], 0);
-            const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
-            slots = a.route == PKV_ROUTE_WORKQUEUE ? r.n : a.S;
-        }
-        // inclusive warp scan, then scan of warp totals
-        int32_t v = slots;
-#pragma unroll
-        for (int off = 1; off < 32; off <<= 1) {
-            const int32_t u = __shfl_up_sync(0xffffffffu, v, off);
-            if (lane >= off) v += u;
-        }
-        if (lane == 31) warp_sums[warp] = v;
-        __syncthreads();
-        if (warp == 0) {
-            int32_t w = lane < nwarps ? warp_sums[lane] : 0;
-#pragma unroll
-            for (int off = 1; off < 32; off <<= 1) {
-                const int32_t u = __shfl_up_sync(0xffffffffu, w, off);
-                if (lane >= off) w += u;
-            }
-            warp_sums[lane] = w;  // inclusive
-        }
-        __syncthreads();
-        const int32_t incl = carry_s + (warp > 0 ? warp_sums[warp - 1] : 0) + v;
-        if (i < a.B) {
-            a.split_offsets[i + 1] = incl;
-            atomicMax(&max_n_s, slots);
-            atomicAdd(&sum_seq_s, (unsigned long long)N);
-        }
-        __syncthreads();
-        if (tid == nthreads - 1) carry_s = incl;
-        __syncthreads();
-    }
-    for (int i = tid; i < a.B * a.Hkv; i += nthreads) a.fuse_counters[i] = 0;
+    const PlanTotals tot = plan_scan(a.plan, a.seq_lens, a.split_offsets, nullptr, sc);
+    for (int i = tid; i < a.plan.B * a.plan.Hkv; i += nthreads) a.fuse_counters[i] = 0;
     __threadfence_block();
     __syncthreads();
-
-    const int32_t row_slots = carry_s;
-    const int64_t total = (int64_t)row_slots * a.Hkv;
-    int32_t my_empties = 0;
-    for (int32_t rs = tid; rs < row_slots; rs += nthreads) {
-        // largest row with split_offsets[row] <= rs
-        int lo = 0, hi = a.B - 1;
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (a.split_offsets[mid] <= rs) lo = mid; else hi = mid - 1;
-        }
-        const int row = lo;
-        const int32_t so = a.split_offsets[row];
-        const int32_t slots = a.split_offsets[row + 1] - so;
-        const int32_t s = rs - so;
-        const int32_t N = max(a.seq_lens[row], 0);
-        const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
-        int32_t tb = 0, te = 0;
-        if (r.T > 0) {
-            const int64_t b = (int64_t)s * r.c, e = (int64_t)(s + 1) * r.c;
-            tb = (int32_t)(b < r.T ? b : r.T);
-            te = (int32_t)(e < r.T ? e : r.T);
-        }
-        if (tb >= te) my_empties += a.Hkv;
-        RowSlot d;
-        d.row = row; d.so = so; d.n = slots; d.split = s;
-        d.tok0 = tb * a.tile_tokens;
-        d.tok1 = min(te * a.tile_tokens, N);
-        d.pad_[0] = d.pad_[1] = 0;
-        a.rowslots[rs] = d;
-        for (int g = 0; g < a.Hkv; ++g) {
-            const int64_t idx = (int64_t)so * a.Hkv + (int64_t)g * slots + s;
-            if (idx < a.tasks_cap) {
-                pkv_task t;
-                t.row = row; t.kvh = g; t.split = s; t.t_begin = tb; t.t_end = te;
-                a.tasks[idx] = t;
-            }
-        }
+    const int64_t total = (int64_t)tot.row_slots * a.plan.Hkv;
+    for (int32_t rs = tid; rs < tot.row_slots; rs += nthreads) {
+        int32_t tb, te;
+        const RowSlot d = make_rowslot(a.plan, a.split_offsets, a.seq_lens, rs, &tb, &te);
+        write_pair(a.plan, d, tb, te, rs, a.rowslots, a.tasks, a.tasks_cap);
     }
-    if (my_empties) atomicAdd(&empties_s, my_empties);
-    __syncthreads();
     if (tid == 0) {
         QueueHeader h;
         h.num_tasks = (int32_t)(total < a.tasks_cap ? total : a.tasks_cap);
-        h.max_row_splits = max_n_s;
-        h.total_row_slots = row_slots;
-        h.resolved_splits = a.S;
-        h.empty_tasks = empties_s;
+        h.max_row_splits = tot.max_n;
+        h.total_row_slots = tot.row_slots;
+        h.resolved_splits = a.plan.S;
+        h.empty_tasks = (tot.row_slots - tot.sum_n) * a.plan.Hkv;   // rect route; 0 on the workqueue route
         h.work_counter = 0;
         h.done_counter = 0;
         h.error_word = total > a.tasks_cap ? 1 : 0;
-        h.sum_seq_lens = (int64_t)sum_seq_s;
-        h.pad_[0] = h.pad_[1] = h.pad_[2] = 0;
+        h.sum_seq_lens = tot.sum_seq;
+        h.build_launches = 1;
+        h.pad32_ = 0;
+        h.pad_[0] = h.pad_[1] = 0;
         *a.hdr = h;
     }
 }
@@ -187,8 +103,7 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
     a.rowslots = rowslots;
     a.tasks = tasks;
     a.tasks_cap = tasks_cap;
-    a.B = shape.B; a.Hkv = shape.Hkv; a.S = rp.S; a.tile_tokens = rp.tile_tokens;
-    a.split_mode = rp.split_mode; a.chunk_tiles = rp.chunk_tiles; a.route = rp.route;
+    a.plan = make_plan_args(shape, rp);
     // one thread per (row, split) pair if that fits in a CTA, 128..1024 threads
     const int64_t want = (int64_t)shape.B * rp.S;
     int threads = 128;

@@ -32,7 +32,9 @@ struct QueueHeader {
     int32_t done_counter;    // CTAs that finished; self-resetting
     int32_t error_word;      // reserved
     int64_t sum_seq_lens;    // sum_i N_i
-    int64_t pad_[3];
+    int32_t build_launches;  // 1: written by the builder kernel, 0: by the decode kernel's fused build / the host
+    int32_t pad32_;
+    int64_t pad_[2];
 };
 static_assert(sizeof(QueueHeader) == 64, "QueueHeader layout");
 
@@ -63,7 +65,7 @@ struct Resolved {
 
 // Byte offsets inside the caller's workspace.  Pure function of (shape, S bound).
 struct WorkspaceLayout {
-    size_t header, split_offsets, fuse_counters, rowslots, tasks, part_m, part_l, part_acc, total;
+    size_t header, fuse_counters, init_bytes, split_offsets, rowslots, tasks, part_m, part_l, part_acc, total;
     int64_t slots_cap; // B * Hkv * S
 };
 

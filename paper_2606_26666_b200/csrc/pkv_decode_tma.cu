@@ -37,6 +37,7 @@ namespace {
 constexpr int kComputeWarps = 8;
 constexpr int kRing = 4;            // unit ring between producer 0 and everybody else
 constexpr int kMaxStages = 24;
+constexpr int kMaxFusedRows = 512;  // fused build: the batch's offsets and lengths sit in shared memory
 
 __host__ __device__ constexpr int producers_for(int HG) { return HG >= 4 ? 1 : (HG == 2 ? 2 : 4); }
 
@@ -55,6 +56,9 @@ struct SmemTail {
     unsigned long long ring_full[kRing];
     unsigned long long ring_empty[kRing];
     UnitInfo ring[kRing];
+    PlanScratch plan_scratch;
+    int32_t so_s[kMaxFusedRows + 1];   // fused build: split_offsets
+    int32_t len_s[kMaxFusedRows];      //              max(N_i, 0)
 };
 
 template <int G, int HG>
@@ -90,6 +94,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
     const uint32_t rfull0 = smem_u32(&tail.ring_full[0]);
     const uint32_t rempty0 = smem_u32(&tail.ring_empty[0]);
 
+    if (tid == 0) trace_stamp(p, 0);
     pdl_launch_dependents();
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) {
@@ -107,14 +112,50 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
     }
     __syncthreads();
     pdl_wait();   // queue (builder), q / seq_lens (upstream), out / partials (previous step's readers)
-    zero_empty_rows(p);
+    if (tid == 0) trace_stamp(p, 1);
 
     const int HGn = p.Hkv / HG;                               // head groups per (row, split)
+    int num_units = 0;
+    if (p.fused_build) {
+        // Fused build: every CTA derives split_offsets from seq_lens
+        // itself (one load round trip + a block scan) and computes the RowSlot of its units from
+        // shared memory; the CTAs share the writing of the queue (RowSlots, task list,
+        // split_offsets, header) that the merge kernel and pkv_read_workqueue read.
+        const PlanTotals tot = plan_scan(p.plan, p.seq_lens, tail.so_s, tail.len_s, tail.plan_scratch);
+        num_units = tot.row_slots * HGn;
+        for (int rs = blockIdx.x * blockDim.x + tid; rs < tot.row_slots; rs += gridDim.x * blockDim.x) {
+            int32_t tb, te;
+            const RowSlot d = make_rowslot(p.plan, tail.so_s, tail.len_s, rs, &tb, &te);
+            write_pair(p.plan, d, tb, te, rs, p.rowslots, p.tasks, p.tasks_cap);
+        }
+        if (blockIdx.x == 0) {
+            for (int i = tid; i <= p.B; i += blockDim.x) p.split_offsets[i] = tail.so_s[i];
+            if (tid == 0) {
+                const int64_t total = (int64_t)tot.row_slots * p.Hkv;
+                p.hdr->num_tasks = (int32_t)(total < p.tasks_cap ? total : p.tasks_cap);
+                p.hdr->max_row_splits = tot.max_n;
+                p.hdr->total_row_slots = tot.row_slots;
+                p.hdr->resolved_splits = p.plan.S;
+                p.hdr->empty_tasks = (tot.row_slots - tot.sum_n) * p.Hkv;
+                p.hdr->error_word = total > p.tasks_cap ? 1 : 0;
+                p.hdr->sum_seq_lens = tot.sum_seq;
+                p.hdr->build_launches = 0;
+            }
+        }
+        for (int i = blockIdx.x; i < p.B; i += gridDim.x) {   // rows without a task (A9)
+            if (tail.len_s[i] > 0) continue;
+            for (int e = tid; e < p.Hq * kD; e += blockDim.x) {
+                p.out[(int64_t)i * p.Hq * kD + e] = __float2half_rn(0.f);
+                if (p.lse && e < p.Hq) p.lse[(int64_t)i * p.Hq + e] = -INFINITY;
+            }
+        }
+    } else {
+        zero_empty_rows(p);
+    }
 
     // ---- unit hand-out (producer 0) / pick-up (everybody else) -------------------------------
     // producer 0 reads the unit's RowSlot (one 32-byte load; the first one is issued together with
     // the header load) and publishes it on the ring; everybody else picks it up from shared memory
-    int num_units = 0;
     auto next_unit = [&](int k) -> UnitInfo {
         const int r = k % kRing;
         UnitInfo u;
@@ -127,13 +168,22 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 if (lane == 0) t = atomicAdd(&p.hdr->work_counter, 1) + gridDim.x;
                 t = __shfl_sync(0xffffffffu, t, 0);
             }
-            const int4* rsp = reinterpret_cast<const int4*>(p.rowslots + (k == 0 ? t / HGn : min(t, max(num_units - 1, 0)) / HGn));
-            const int4 a = __ldcg(rsp);
-            const int4 b = __ldcg(rsp + 1);
-            if (k == 0) num_units = __ldcg(&p.hdr->total_row_slots) * HGn;
-            if (t >= num_units) t = -1;
+            if (p.fused_build) {
+                if (t >= num_units) t = -1;
+                RowSlot d = {};
+                int32_t tb, te;
+                if (t >= 0) d = make_rowslot(p.plan, tail.so_s, tail.len_s, t / HGn, &tb, &te);
+                u.row = d.row; u.so = d.so; u.n = d.n; u.split = d.split; u.tok0 = d.tok0; u.tok1 = d.tok1;
+            } else {
+                const int4* rsp = reinterpret_cast<const int4*>(p.rowslots + (k == 0 ? t / HGn : min(t, max(num_units - 1, 0)) / HGn));
+                const int4 a = __ldcg(rsp);
+                const int4 b = __ldcg(rsp + 1);
+                if (k == 0) num_units = __ldcg(&p.hdr->total_row_slots) * HGn;
+                if (t >= num_units) t = -1;
+                u.row = a.x; u.so = a.y; u.n = a.z; u.split = a.w; u.tok0 = b.x; u.tok1 = b.y;
+            }
             u.unit = t;
-            u.row = a.x; u.so = a.y; u.n = a.z; u.split = a.w; u.tok0 = b.x; u.tok1 = b.y; u.pad_ = 0;
+            u.pad_ = 0;
             if (lane == 0) {
                 mbar_wait(rempty0 + 8 * r, ((k / kRing) & 1) ^ 1);
                 tail.ring[r] = u;
@@ -154,6 +204,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
         for (int k = 0;; ++k) {
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
+            if (k == 0 && tid == 0) trace_stamp(p, 2);
             const int row = u.row, hg = u.unit % HGn;
             const int tok0 = u.tok0, tok1 = u.tok1;
             if (tok0 >= tok1) continue;  // empty split: nothing is staged
@@ -175,6 +226,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 for (int i = 0; i < cnt; ++i) {
                     const int page = __shfl_sync(0xffffffffu, mine, i);
                     if (lane == 0) {
+                        if (k == 0 && c == 0 && i == 0 && warp == 0) trace_stamp(p, 3 + (page & 0));
                         const uint32_t sq = seq_base + j0 + (c + i) * NP;
                         const uint32_t s = sq % kStages;
                         mbar_wait(empty0 + 8 * s, ((sq / kStages) & 1) ^ 1);
@@ -192,6 +244,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
         }
         // the last CTA to run out of units re-arms the counters for the next launch / replay
         if (warp == 0 && lane == 0) {
+            trace_stamp(p, 7);
             const int old = atomicAdd(&p.hdr->done_counter, 1);
             if (old == (int)gridDim.x - 1) {
                 p.hdr->work_counter = 0;
@@ -257,6 +310,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
 
                 // ---- S^T = K . Q^T, two accumulation chains (channel halves)
                 mbar_wait(fullk0 + 8 * s, par);
+                if (k == 0 && j == sub && cw == 0 && lane == 0) trace_stamp(p, 4);
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk) {
@@ -318,6 +372,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 if (lane == 0) mbar_arrive(empty0 + 8 * s);   // this head's part of the stage is consumed
             }
             seq_base += np;
+            if (k == 0 && cw == 0 && lane == 0) trace_stamp(p, 5);
 
             // ---- warp state -> combine buffer row cw
 #pragma unroll
@@ -340,6 +395,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
             }
             group_sync<WPH>(1 + hl);
             finalize_task<G, WPH, kComputeWarps>(p, tail.cb, hl, HG, row, kvh, split, n_i, slot, gtid, 1 + hl);
+            if (k == 0 && cw == 0 && lane == 0) trace_stamp(p, 6);
         }
     }
 }

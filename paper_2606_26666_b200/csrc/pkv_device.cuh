@@ -15,15 +15,19 @@ namespace pkv {
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 
+struct PlanArgs {   // split policy as the device-side planner needs it
+    int32_t B, Hkv, S, tile_tokens, split_mode, chunk_tiles, route;
+};
+
 struct DecodeParams {
     const __half* q;            // [B, Hq, d]
     const __half* k_cache;      // raw pointers (SIMT kernel; the TMA kernel uses tensor maps)
     const __half* v_cache;
     const int32_t* block_table; // [B, max_pages]
     const int32_t* seq_lens;    // [B]
-    const pkv_task* tasks;
-    const RowSlot* rowslots;      // [split_offsets[B]] (row, split) pairs
-    const int32_t* split_offsets; // [B+1]
+    pkv_task* tasks;              // written by the builder / the fused build, read by the SIMT kernel
+    RowSlot* rowslots;            // [split_offsets[B]] (row, split) pairs
+    int32_t* split_offsets;       // [B+1]
     QueueHeader* hdr;
     __half* out;                // [B, Hq, d]
     float* lse;                 // [B, Hq] or nullptr
@@ -33,10 +37,14 @@ struct DecodeParams {
     int32_t* fuse_counters;     // [B*Hkv]
     int64_t stride_page, stride_token, stride_head; // elements
     int32_t B, Hq, Hkv, max_pages, tile_tokens, merge_mode;
+    PlanArgs plan;               // split policy (fused build)
+    int64_t tasks_cap;
+    int32_t fused_build;         // TMA kernel: 1 = every CTA derives the queue from seq_lens itself
     int32_t heads_per_cta;       // TMA kernel: KV heads one CTA streams together (1, 2, 4 or 8)
     int32_t dynamic_sched;      // 1: tasks handed out by an atomic counter
     float scale;                // x = scale * <q, k>
     float scale_log2;           // scale * log2(e)
+    unsigned long long* trace;  // debug: [grid][16] %globaltimer stamps, or nullptr (pkv_debug_set_trace)
 };
 
 // ------------------------------------------------------------------ small PTX wrappers
@@ -57,6 +65,14 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 // scheduled early and waits for its predecessor's results before touching global memory.
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+__device__ __forceinline__ void trace_stamp(const DecodeParams& p, int slot) {
+    if (p.trace) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        p.trace[(size_t)blockIdx.x * 16 + slot] = t;
+    }
+}
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
@@ -136,6 +152,126 @@ __device__ __forceinline__ void mma_16816(float (&c)[4], uint32_t a0, uint32_t a
 __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
     __half2 h = __floats2half2_rn(lo, hi);
     return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// ------------------------------------------------------------------ split-bound policy on the device
+// (PAPER.md:63-75).  Shared by the builder kernel (pkv_aux.cu) and by the decode kernel's fused
+// build (pkv_decode_tma.cu): same integer formulas as the host planner (pkv_common.h row_splits).
+
+struct PlanScratch {   // shared memory of the calling CTA
+    int32_t warp_sums[32];
+    int32_t carry, max_n, sum_n;
+    unsigned long long sum_seq;
+};
+struct PlanTotals {
+    int32_t row_slots, max_n, sum_n;   // sum_n = sum_i n_i (non-empty splits)
+    long long sum_seq;
+};
+
+// Block-wide (every thread of the CTA calls it; blockDim.x a multiple of 32, <= 1024):
+// so_out[0..B] = exclusive prefix sum of the rows' slot counts (n_i, or S on the rect route),
+// len_out[i] = max(N_i, 0) if len_out != nullptr.  so_out / len_out may be global or shared.
+__device__ __forceinline__ PlanTotals plan_scan(const PlanArgs& a, const int32_t* seq_lens, int32_t* so_out,
+                                                int32_t* len_out, PlanScratch& sc) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthreads = blockDim.x, nwarps = nthreads >> 5;
+    if (tid == 0) {
+        sc.carry = 0;
+        sc.max_n = 0;
+        sc.sum_n = 0;
+        sc.sum_seq = 0ull;
+        so_out[0] = 0;
+    }
+    __syncthreads();
+    for (int base = 0; base < a.B; base += nthreads) {
+        const int i = base + tid;
+        int32_t slots = 0, N = 0, nonempty = 0;
+        if (i < a.B) {
+            N = max(__ldcg(seq_lens + i), 0);
+            const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
+            nonempty = r.n;
+            slots = a.route == PKV_ROUTE_WORKQUEUE ? r.n : a.S;
+        }
+        int32_t v = slots;   // inclusive warp scan, then scan of the warp totals
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const int32_t u = __shfl_up_sync(0xffffffffu, v, off);
+            if (lane >= off) v += u;
+        }
+        if (lane == 31) sc.warp_sums[warp] = v;
+        __syncthreads();
+        if (warp == 0) {
+            int32_t w = lane < nwarps ? sc.warp_sums[lane] : 0;
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                const int32_t u = __shfl_up_sync(0xffffffffu, w, off);
+                if (lane >= off) w += u;
+            }
+            sc.warp_sums[lane] = w;  // inclusive
+        }
+        __syncthreads();
+        const int32_t incl = sc.carry + (warp > 0 ? sc.warp_sums[warp - 1] : 0) + v;
+        if (i < a.B) {
+            so_out[i + 1] = incl;
+            if (len_out) len_out[i] = N;
+            atomicMax(&sc.max_n, slots);
+            atomicAdd(&sc.sum_n, nonempty);
+            atomicAdd(&sc.sum_seq, (unsigned long long)N);
+        }
+        __syncthreads();
+        if (tid == nthreads - 1) sc.carry = incl;
+        __syncthreads();
+    }
+    PlanTotals t;
+    t.row_slots = sc.carry;
+    t.max_n = sc.max_n;
+    t.sum_n = sc.sum_n;
+    t.sum_seq = (long long)sc.sum_seq;
+    return t;
+}
+
+// The (row, split) pair rs: the row by binary search in so[0..B], bounds from the row's length.
+// `lens` is indexed by row (seq_lens itself, or the clamped copy plan_scan made).
+__device__ __forceinline__ RowSlot make_rowslot(const PlanArgs& a, const int32_t* so, const int32_t* lens, int rs,
+                                                int32_t* t_begin, int32_t* t_end) {
+    int lo = 0, hi = a.B - 1;
+    while (lo < hi) {   // largest row with so[row] <= rs
+        const int mid = (lo + hi + 1) >> 1;
+        if (so[mid] <= rs) lo = mid; else hi = mid - 1;
+    }
+    RowSlot d;
+    d.row = lo;
+    d.so = so[lo];
+    d.n = so[lo + 1] - d.so;
+    d.split = rs - d.so;
+    const int32_t N = max(lens[lo], 0);
+    const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
+    int32_t tb = 0, te = 0;
+    if (r.T > 0) {
+        const long long b = (long long)d.split * r.c, e = (long long)(d.split + 1) * r.c;
+        tb = (int32_t)(b < r.T ? b : r.T);
+        te = (int32_t)(e < r.T ? e : r.T);
+    }
+    d.tok0 = tb * a.tile_tokens;
+    d.tok1 = min(te * a.tile_tokens, N);
+    d.pad_[0] = d.pad_[1] = 0;
+    *t_begin = tb;
+    *t_end = te;
+    return d;
+}
+
+// Writes pair rs's RowSlot and its Hkv task entries (canonical order: so*Hkv + g*n + s).
+__device__ __forceinline__ void write_pair(const PlanArgs& a, const RowSlot& d, int32_t tb, int32_t te, int rs,
+                                          RowSlot* rowslots, pkv_task* tasks, int64_t tasks_cap) {
+    rowslots[rs] = d;
+    for (int g = 0; g < a.Hkv; ++g) {
+        const int64_t idx = (int64_t)d.so * a.Hkv + (int64_t)g * d.n + d.split;
+        if (idx < tasks_cap) {
+            pkv_task t;
+            t.row = d.row; t.kvh = g; t.split = d.split; t.t_begin = tb; t.t_end = te;
+            tasks[idx] = t;
+        }
+    }
 }
 
 // ------------------------------------------------------------------ merge of split states
@@ -360,6 +496,13 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     cfg.attrs = attr;
     cfg.numAttrs = g_use_pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
+inline PlanArgs make_plan_args(const pkv_shape& shape, const Resolved& rp) {
+    PlanArgs a;
+    a.B = shape.B; a.Hkv = shape.Hkv; a.S = rp.S; a.tile_tokens = rp.tile_tokens;
+    a.split_mode = rp.split_mode; a.chunk_tiles = rp.chunk_tiles; a.route = rp.route;
+    return a;
 }
 
 // launchers implemented in the .cu files

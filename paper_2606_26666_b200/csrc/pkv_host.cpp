@@ -100,8 +100,9 @@ WorkspaceLayout workspace_layout(const pkv_shape& s, int32_t S) {
     L.slots_cap = (int64_t)s.B * s.Hkv * S;
     size_t off = 0;
     L.header = off;         off = align_up(off + sizeof(QueueHeader), 256);
-    L.split_offsets = off;  off = align_up(off + sizeof(int32_t) * ((size_t)s.B + 1), 256);
     L.fuse_counters = off;  off = align_up(off + sizeof(int32_t) * ((size_t)s.B * s.Hkv + 1), 256);
+    L.init_bytes = off;     // header + completion counters: zero on first use (include/pkv.h)
+    L.split_offsets = off;  off = align_up(off + sizeof(int32_t) * ((size_t)s.B + 1), 256);
     L.rowslots = off;       off = align_up(off + sizeof(RowSlot) * (size_t)s.B * S, 256);
     L.tasks = off;          off = align_up(off + sizeof(pkv_task) * (size_t)L.slots_cap, 256);
     L.part_m = off;         off = align_up(off + sizeof(float) * (size_t)L.slots_cap * G, 256);
@@ -184,6 +185,12 @@ size_t pkv_workspace_bytes(const pkv_shape* shape, const pkv_split_policy* polic
     Resolved rp;
     if (validate_and_resolve(shape, policy, 0, /*bound_ok=*/true, &rp) != PKV_OK) return 0;
     return workspace_layout(*shape, rp.S).total;
+}
+
+size_t pkv_workspace_init_bytes(const pkv_shape* shape, const pkv_split_policy* policy) {
+    Resolved rp;
+    if (validate_and_resolve(shape, policy, 0, /*bound_ok=*/true, &rp) != PKV_OK) return 0;
+    return workspace_layout(*shape, rp.S).init_bytes;
 }
 
 pkv_status pkv_build_workqueue_host(const pkv_shape* shape, const pkv_split_policy* policy,

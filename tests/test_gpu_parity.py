@@ -378,3 +378,39 @@ def test_pdl_off_matches_pdl_on_bitwise():
         pkv.pkv_debug_set_pdl(True)
     assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
     assert_within_tolerance(o1, oracle_attention(p)[0])
+
+
+@pytest.mark.parametrize("route", [pkv.ROUTE_WORKQUEUE, pkv.ROUTE_RECT])
+def test_fused_build_queue_bit_exact_and_same_output(route):
+    """pkv_decode's fused build (the TMA kernel derives the queue from seq_lens itself) leaves the
+    same queue in the workspace as the builder kernel and the oracle: count, order,
+    every field, split_offsets, counters; outputs are bitwise equal with the builder kernel's."""
+    lens = [700, 0, 33, 16, 257, 1, 2000, 31, 64, 65]
+    p = make_problem(lens, seed=29)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    pols = [pkv.Policy(tile_tokens=32, num_splits=5, route=route),
+            pkv.Policy(tile_tokens=16, num_splits=0, route=route),
+            pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=3, route=route),
+            pkv.Policy(tile_tokens=32, num_splits=7, route=route, merge_mode=pkv.MERGE_FUSED)]
+    for pol in pols:
+        opol = oracle_policy(pol)
+        if pol.num_splits == 0 and pol.split_mode == pkv.SPLIT_FIXED_COUNT:
+            opol = wq.Policy(**{**opol.__dict__, "num_sms": sm_count()})
+        want = wq.build_workqueue(lens, 8, opol)
+        outs = []
+        for fused in (True, False):
+            pkv.pkv_debug_set_fused_build(fused)
+            try:
+                out, lse, ws, _ = check(dp, pol, ref, what="fused=%s %s" % (fused, pol))
+            finally:
+                pkv.pkv_debug_set_fused_build(True)
+            outs.append((out, lse))
+            tasks, offs = pkv.pkv_read_workqueue(dp.shape, pol, ws)
+            assert np.array_equal(tasks, np.array(want.tasks, dtype=np.int32).reshape(-1, 5)), (fused, pol)
+            assert np.array_equal(offs, np.array(want.split_offsets, dtype=np.int32))
+            c = pkv.pkv_get_counters(dp.shape, pol, ws)
+            assert c["tasks"] == want.num_tasks and c["empty_tasks"] == want.empty_ctas
+            assert c["decode_launches"] == want.decode_launches and c["merge_launches"] == want.merge_launches
+            assert c["build_launches"] == (0 if fused else 1)
+        assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
