@@ -66,10 +66,9 @@ __host__ __device__ constexpr int stages_for() {
     // 227 KiB per CTA, minus the tail, minus 1 KiB alignment slack
     constexpr int avail = 232448 - 1024 - (int)sizeof(SmemTail<G>);
     constexpr int n = avail / (HG * 8192);
-    constexpr int capped = n > kMaxStages ? kMaxStages : n;
-    // a multiple of the producer count, so that a stage always belongs to the same producer:
-    // two producers sharing a stage could pass each other on its parity-only empty barrier
-    return capped / producers_for(HG) * producers_for(HG);
+    // Stage s always belongs to producer s % NP and, per head, to compute warp s % WPH (see the
+    // kernel): any stage count works, the shares differ by at most one stage.
+    return n > kMaxStages ? kMaxStages : n;
 }
 
 template <int G, int HG>
@@ -200,7 +199,13 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
 
     if (warp < NP) {
         // ================================================================ producer warps
-        uint32_t seq_base = 0;  // pages of earlier units of this CTA
+        // Page j of a unit is the next page of this CTA's stream of pages: it lands in stage ps,
+        // in that stage's fill number whose parity is pphase.  STAGE OWNERSHIP: stage s is always
+        // filled by producer s % NP and, per head, always consumed by compute warp s % WPH, so the
+        // owner of a stage sees every one of its phases in order.  (A parity wait can only tell
+        // adjacent phases apart: a warp that skipped a phase of a stage could pass the wait for
+        // the next one while the skipped fill is still in flight.)
+        uint32_t ps = 0, pphase = 0;
         for (int k = 0;; ++k) {
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
@@ -211,25 +216,20 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
             const int p0 = tok0 >> 4;
             const int np = ((tok1 + 15) >> 4) - p0;
             const int head0 = hg * HG;
-            // Page j of the unit has sequence number seq_base + j in this CTA's stream of pages and
-            // lands in stage (seq_base + j) % kStages.  A stage must always be filled by the same
-            // producer (its empty barrier carries one parity bit), so producer w takes the pages
-            // with (seq_base + j) % NP == w: the first is j0, then every NP-th.
-            const int j0 = (warp + NP - (int)(seq_base % NP)) % NP;
-            const int32_t* bt = p.block_table + (int64_t)row * p.max_pages + p0 + j0;
-            const int npw = np > j0 ? (np - j0 + NP - 1) / NP : 0;    // pages of this producer
-            // table entries 32 at a time (lane i holds this producer's i-th page of the batch)
-            int mine = lane < npw ? bt[lane * NP] : 0;
-            for (int c = 0; c < npw; c += 32) {
-                const int nxt = (c + 32 + lane < npw) ? bt[(c + 32 + lane) * NP] : 0;
-                const int cnt = min(32, npw - c);
+            const int32_t* bt = p.block_table + (int64_t)row * p.max_pages + p0;
+            // table entries 32 at a time (lane i holds page c + i of the unit)
+            int mine = lane < np ? bt[lane] : 0;
+            for (int c = 0; c < np; c += 32) {
+                const int nxt = (c + 32 + lane < np) ? bt[c + 32 + lane] : 0;
+                const int cnt = min(32, np - c);
                 for (int i = 0; i < cnt; ++i) {
                     const int page = __shfl_sync(0xffffffffu, mine, i);
+                    const uint32_t s = ps, par = pphase;
+                    if (++ps == (uint32_t)kStages) { ps = 0; pphase ^= 1; }
+                    if ((s % NP) != (uint32_t)warp) continue;
                     if (lane == 0) {
                         if (k == 0 && c == 0 && i == 0 && warp == 0) trace_stamp(p, 3 + (page & 0));
-                        const uint32_t sq = seq_base + j0 + (c + i) * NP;
-                        const uint32_t s = sq % kStages;
-                        mbar_wait(empty0 + 8 * s, ((sq / kStages) & 1) ^ 1);
+                        mbar_wait(empty0 + 8 * s, par ^ 1);
                         const uint32_t dst = stage_base + s * kStageBytes;
                         // box dims: (64 ch, 16 tok, 2 ch-halves, HG heads, 1 page)
                         mbar_arrive_expect_tx(fullk0 + 8 * s, HG * 4096);
@@ -240,7 +240,6 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 }
                 mine = nxt;
             }
-            seq_base += np;
         }
         // the last CTA to run out of units re-arms the counters for the next launch / replay
         if (warp == 0 && lane == 0) {
@@ -267,7 +266,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
         const uint32_t v_sel = (lane >> 3) & 1;
         const uint32_t xr = lane & 7;        // swizzle: 16-byte chunk index ^= token % 8
 
-        uint32_t seq_base = 0;
+        uint32_t cs = 0, cphase = 0;   // stage / phase parity of the unit's next page (= the producers' ps, pphase)
         for (int k = 0;; ++k) {
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
@@ -300,17 +299,19 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
 #pragma unroll
             for (int mt = 0; mt < 8; ++mt) o[mt][0] = o[mt][1] = o[mt][2] = o[mt][3] = 0.f;
 
-            for (int j = sub; j < np; j += WPH) {
-                const uint32_t sq = seq_base + j;
-                const uint32_t s = sq % kStages;
-                const uint32_t par = (sq / kStages) & 1;
+            bool first_page = true;
+            for (int j = 0; j < np; ++j) {
+                const uint32_t s = cs, par = cphase;
+                if (++cs == (uint32_t)kStages) { cs = 0; cphase ^= 1; }
+                if ((s % WPH) != (uint32_t)sub) continue;   // stage ownership (see the producers)
                 const uint32_t kb = stage_base + s * kStageBytes + hl * 4096;
                 const uint32_t vb = kb + HG * 4096;
                 const int nvalid = tok1 - ((p0 + j) << 4);  // >= 1; >= 16 for all but the last page
 
                 // ---- S^T = K . Q^T, two accumulation chains (channel halves)
                 mbar_wait(fullk0 + 8 * s, par);
-                if (k == 0 && j == sub && cw == 0 && lane == 0) trace_stamp(p, 4);
+                if (k == 0 && first_page && cw == 0 && lane == 0) trace_stamp(p, 4);
+                first_page = false;
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk) {
@@ -371,7 +372,6 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty0 + 8 * s);   // this head's part of the stage is consumed
             }
-            seq_base += np;
             if (k == 0 && cw == 0 && lane == 0) trace_stamp(p, 5);
 
             // ---- warp state -> combine buffer row cw
@@ -420,7 +420,6 @@ int decode_tma_smem_bytes(int G, int HG) {
     const int tail = G == 4 ? (int)sizeof(SmemTail<4>) : (int)sizeof(SmemTail<8>);
     int st = (232448 - 1024 - tail) / (HG * 8192);
     if (st > kMaxStages) st = kMaxStages;
-    st = st / producers_for(HG) * producers_for(HG);
     return st * HG * 8192 + tail + 1024;
 }
 

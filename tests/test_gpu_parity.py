@@ -343,15 +343,18 @@ def test_cuda_graph_replay_with_growing_lengths(mm):
             assert tasks.shape[0] == wq.build_workqueue(list(lens + step), 8, oracle_policy(pol)).num_tasks
 
 
+@pytest.mark.parametrize("Hkv", [8, 4])
 @pytest.mark.parametrize("hg", [1, 2, 4, 8])
-def test_many_units_per_cta_odd_page_counts(hg):
+def test_many_units_per_cta_odd_page_counts(hg, Hkv):
     """More work units than SMs, rows with odd page counts: every persistent CTA walks several
     units, so its page ring wraps across unit boundaries with every residue of the page sequence
     number (the stage-ownership rule of the multi-producer ring)."""
+    if hg > Hkv:
+        pytest.skip("hg > Hkv")
     rng = np.random.Generator(np.random.PCG64(1234 + hg))
     lens = rng.integers(1, 1500, size=96).astype(np.int32)
     lens[::7] = rng.integers(1, 40, size=len(lens[::7]))          # some one- and two-page rows
-    p = make_problem(list(lens), seed=400 + hg)
+    p = make_problem(list(lens), seed=400 + hg, Hkv=Hkv)
     dp = DevProblem(p)
     ref = oracle_attention(p)
     pkv.pkv_debug_force_heads_per_cta(hg)
@@ -360,6 +363,30 @@ def test_many_units_per_cta_odd_page_counts(hg):
                     pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=5,
                                merge_mode=pkv.MERGE_FUSED)):
             for _ in range(2):          # twice: the dynamic unit counter must have re-armed itself
+                check(dp, pol, ref, what="hg%d %s" % (hg, pol))
+    finally:
+        pkv.pkv_debug_force_heads_per_cta(0)
+
+
+@pytest.mark.parametrize("Hkv", [8, 4])
+@pytest.mark.parametrize("hg", [1, 2, 4, 8])
+def test_long_units_ring_wraps_many_times(hg, Hkv):
+    """Units of 16 pages and more on rings of 3..24 stages, several units per CTA, with several
+    compute warps per head (8 / hg) and several producers: a stage must be filled and consumed by
+    the same warps in every one of its phases; a warp that skips a
+    phase of a stage can pass the parity wait of the next phase early and read a stale page."""
+    if hg > Hkv:
+        pytest.skip("hg > Hkv")
+    rng = np.random.Generator(np.random.PCG64(77 + hg))
+    lens = rng.integers(1, 3000, size=128).astype(np.int32)
+    p = make_problem(list(lens), seed=500 + hg, Hkv=Hkv)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    pkv.pkv_debug_force_heads_per_cta(hg)
+    try:
+        for pol in (pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=8),
+                    pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=32, num_splits=4)):
+            for _ in range(3):
                 check(dp, pol, ref, what="hg%d %s" % (hg, pol))
     finally:
         pkv.pkv_debug_force_heads_per_cta(0)
