@@ -300,10 +300,20 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
             for (int mt = 0; mt < 8; ++mt) o[mt][0] = o[mt][1] = o[mt][2] = o[mt][3] = 0.f;
 
             bool first_page = true;
-            for (int j = 0; j < np; ++j) {
-                const uint32_t s = cs, par = cphase;
-                if (++cs == (uint32_t)kStages) { cs = 0; cphase ^= 1; }
-                if ((s % WPH) != (uint32_t)sub) continue;   // stage ownership (see the producers)
+            // This warp's pages of the unit: those landing in the stages it owns (s % WPH == sub).
+            // From an owned stage s the next owned one is s + WPH, or -- past the end of the ring --
+            // stage `sub` of the next phase.  (A per-page skip loop costs > 1 us per launch.)
+            int j;
+            uint32_t s, par;
+            {
+                const uint32_t d0 = (uint32_t)(sub + WPH - (int)(cs % WPH)) % WPH;
+                if (cs + d0 < (uint32_t)kStages) { j = (int)d0; s = cs + d0; par = cphase; }
+                else { j = (int)((uint32_t)kStages - cs) + sub; s = (uint32_t)sub; par = cphase ^ 1; }
+                const uint32_t adv = cs + (uint32_t)np;   // stream position after the unit
+                cs = adv % kStages;
+                cphase ^= (adv / kStages) & 1;
+            }
+            while (j < np) {
                 const uint32_t kb = stage_base + s * kStageBytes + hl * 4096;
                 const uint32_t vb = kb + HG * 4096;
                 const int nvalid = tok1 - ((p0 + j) << 4);  // >= 1; >= 16 for all but the last page
@@ -371,6 +381,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty0 + 8 * s);   // this head's part of the stage is consumed
+                if (s + WPH < (uint32_t)kStages) { s += WPH; j += WPH; }
+                else { j += (int)((uint32_t)kStages - s) + sub; s = (uint32_t)sub; par ^= 1; }
             }
             if (k == 0 && cw == 0 && lane == 0) trace_stamp(p, 5);
 
