@@ -102,11 +102,9 @@ def default_policy(pkv, name: str, args):
     """Per-workload default split policy (tuned on seed 20260622)."""
     if name in ("config1",):
         pol = pkv.Policy(tile_tokens=32, num_splits=1, route=pkv.ROUTE_RECT)
-    elif name == "config2":
-        pol = pkv.Policy(tile_tokens=32, num_splits=0, route=pkv.ROUTE_WORKQUEUE)
     else:
-        pol = pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=8,
-                         route=pkv.ROUTE_WORKQUEUE)
+        # BALANCED (DESIGN.md A21): chunk from the batch's true lengths, page-granular tiles
+        pol = pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, route=pkv.ROUTE_WORKQUEUE)
     if args.tile_tokens > 0:
         pol.tile_tokens = args.tile_tokens
     if args.split_mode >= 0:
@@ -504,21 +502,22 @@ def run_ours(args):
 
     sweep = {}
     if args.workload == "config2" and not args.no_sweep and args.splits < 0:
-        # BASELINE.json configs[1]: split counts {1, 4, 16, 64}; plus the auto rule (0)
-        for S in (1, 4, 16, 64, 0):
-            p2 = pkv.Policy(**{**pol.__dict__, "num_splits": S})
+        # BASELINE.json configs[1]: split counts {1, 4, 16, 64} (FIXED_COUNT, 32-token tiles), the
+        # paper's auto rule (A12) and the BALANCED policy (A21); the timed run uses the fastest
+        cands = [(str(S), pkv.Policy(tile_tokens=32, num_splits=S, route=pol.route, merge_mode=pol.merge_mode,
+                                     kernel=pol.kernel)) for S in (1, 4, 16, 64, 0)] + [("balanced", pol)]
+        pols = {}
+        for key, p2 in cands:
             r = time_workload(pkv, torch, w, p2, args, device, min(K, 4 * args.graph_steps), W, want_decode_only=False)
             us = 1e3 * r["ms_total"] / min(K, 4 * args.graph_steps)
-            sweep["auto(%d)" % r["counters"]["num_splits"] if S == 0 else str(S)] = {
-                "us_per_step": round(us, 3), "tasks": r["counters"]["tasks"],
-                "alg_GBps": round(algorithmic_bytes(w, w.seq_lens) / us / 1e3, 1)}
-            if S == 0:
-                best_auto = us
+            if key == "0":
+                key = "auto(%d)" % r["counters"]["num_splits"]
+            sweep[key] = {"us_per_step": round(us, 3), "tasks": r["counters"]["tasks"],
+                          "alg_GBps": round(algorithmic_bytes(w, w.seq_lens) / us / 1e3, 1)}
+            pols[key] = p2
             del r
             torch.cuda.empty_cache()
-        best_key = min(sweep, key=lambda k_: sweep[k_]["us_per_step"])
-        if not best_key.startswith("auto"):
-            pol = pkv.Policy(**{**pol.__dict__, "num_splits": int(best_key)})
+        pol = pols[min(sweep, key=lambda k_: sweep[k_]["us_per_step"])]
 
     if world > 1:
         dist.barrier()
@@ -573,7 +572,8 @@ def run_ours(args):
         "hbm_frac_whole_step": alg / us_step / 1e3 / peak,
         "launches_per_step": {"build": counters["build_launches"], "decode": counters["decode_launches"],
                               "merge": counters["merge_launches"], "tasks": counters["tasks"],
-                              "num_splits": counters["num_splits"]},
+                              "num_splits": counters["num_splits"], "chunk_tiles": counters["chunk_tiles"],
+                              "max_row_splits": counters["max_row_splits"]},
         "gpu_launches": int(launches_per_step * K),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": "pkv_decode_tma_kernel" if pol.kernel != pkv.KERNEL_SIMT else "pkv_decode_simt_kernel",
@@ -600,12 +600,17 @@ def run_ours(args):
         line["cpu_baseline"] = {"value": tps, "unit": "tokens/s", "cores": cores, "kind": "oracle", "sample": desc}
         line["parity"] = {"rows_checked": len(sel), "max_abs_err": float(err.max()), "mean_abs_err": float(err.mean()),
                           "tolerance_max_abs": 2e-3, "ok": bool(err.max() <= 2e-3)}
-    traffic_path = os.path.join(ROOT, "profiles", "traffic.json")
+    # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel from the
+    # committed `ncu --set full` capture of this workload (profiles/traffic.csv names the capture)
+    traffic_path = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(traffic_path):
         try:
             with open(traffic_path) as f:
-                tr = json.load(f)
-            line["roofline"]["traffic"] = tr.get(args.workload, {}).get("dram_bytes_per_launch")
+                for ln in f:
+                    cols = [c.strip() for c in ln.split(",")]
+                    if len(cols) >= 3 and cols[0] == args.workload:
+                        line["roofline"]["traffic"] = float(cols[2])
+                        line["roofline"]["traffic_source"] = cols[3] if len(cols) > 3 else "profiles/traffic.csv"
         except Exception:
             pass
     print(json.dumps(line))

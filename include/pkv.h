@@ -52,7 +52,7 @@ typedef enum {
 
 typedef enum { PKV_ROUTE_RECT = 0, PKV_ROUTE_WORKQUEUE = 1 } pkv_route;
 typedef enum { PKV_MERGE_SEPARATE = 0, PKV_MERGE_FUSED = 1 } pkv_merge_mode;
-typedef enum { PKV_SPLIT_FIXED_COUNT = 0, PKV_SPLIT_FIXED_CHUNK = 1 } pkv_split_mode;
+typedef enum { PKV_SPLIT_FIXED_COUNT = 0, PKV_SPLIT_FIXED_CHUNK = 1, PKV_SPLIT_BALANCED = 2 } pkv_split_mode;
 /* which decode kernel runs the tile loop */
 typedef enum {
     PKV_KERNEL_AUTO = 0, /* = PKV_KERNEL_TMA_MMA                                                 */
@@ -69,6 +69,16 @@ typedef enum {
  *   c_i = ceil(T_i / S_i), n_i = ceil(T_i / c_i); split s of row i covers tiles
  *   [s*c_i, min((s+1)*c_i, T_i)), s = 0 .. n_i-1                      (reading A6)
  * Auto rule (A12): S = clamp(ceil(4*num_sms / (B*Hkv)), 1, 256).
+ *   BALANCED: FIXED_CHUNK whose chunk_tiles is derived from the whole batch's true lengths
+ *   ("CTA-work and length-based tile bounds"; per-row split counts, PAPER.md:271;
+ *   DESIGN.md reading A21).  With U = num_sms, W = sum_i T_i, m = ceil(256 / tile_tokens):
+ *     c2 = max(m, ceil(W / (32*U)))                   (many waves: about 32 pairs per SM,
+ *                                                       handed out dynamically)
+ *     single wave: the smallest c in [ceil(W/U), ceil(W/U) + c2] with
+ *                  sum_i ceil(T_i / c) <= U   (every SM gets at most one (row, split) pair and
+ *                  the busiest SM's share exceeds the mean W/U by at most one many-wave chunk);
+ *     chunk = that c if it exists, else c2.
+ *   chunk_tiles of the policy is ignored; S = num_splits (256 when 0) still caps n_i.
  */
 typedef struct {
     int32_t tile_tokens; /* > 0, multiple of page_size; the paper uses 32          */
@@ -77,8 +87,8 @@ typedef struct {
     int32_t chunk_tiles; /* FIXED_CHUNK: tiles per task (> 0)                                    */
     int32_t route;       /* pkv_route                                                            */
     int32_t merge_mode;  /* pkv_merge_mode                                                       */
-    int32_t num_sms;     /* SM count for the auto rule; 0 = the current device's (device calls
-                            only; the host builder needs it > 0 when num_splits == 0)            */
+    int32_t num_sms;     /* SM count for the auto rule and for BALANCED; 0 = the current device's
+                            (device calls only; the host builder needs it > 0 then)             */
     int32_t kernel;      /* pkv_kernel                                                           */
 } pkv_split_policy;
 
@@ -112,6 +122,7 @@ typedef struct {
     int64_t merge_bytes;     /* partial slots * G * (d+2) * 4 (one pass)                         */
     int64_t num_splits;      /* resolved S                                                       */
     int64_t max_row_splits;  /* max_i n_i                                                        */
+    int64_t chunk_tiles;     /* FIXED_CHUNK / BALANCED: resolved tiles per task; else 0          */
     int64_t h2d_bytes;       /* pkv_decode_host only: bytes copied host->device this step        */
     int64_t d2h_bytes;       /* pkv_decode_host only: bytes copied device->host this step        */
 } pkv_counters;

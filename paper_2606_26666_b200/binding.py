@@ -20,7 +20,7 @@ from . import build as _build
 PKV_OK, PKV_ERR_INVALID_ARG, PKV_ERR_UNSUPPORTED, PKV_ERR_WORKSPACE, PKV_ERR_CUDA = range(5)
 ROUTE_RECT, ROUTE_WORKQUEUE = 0, 1
 MERGE_SEPARATE, MERGE_FUSED = 0, 1
-SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK = 0, 1
+SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK, SPLIT_BALANCED = 0, 1, 2
 KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
 STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL = 1, 2, 4, 7
 
@@ -44,7 +44,7 @@ class pkv_shape(ctypes.Structure):
 
 class pkv_counters(ctypes.Structure):
     _fields_ = [(n, _i64) for n in ("tasks", "empty_tasks", "decode_launches", "merge_launches", "build_launches",
-                                    "useful_kv_bytes", "merge_bytes", "num_splits", "max_row_splits", "h2d_bytes",
+                                    "useful_kv_bytes", "merge_bytes", "num_splits", "max_row_splits", "chunk_tiles", "h2d_bytes",
                                     "d2h_bytes")]
 
     def as_dict(self):

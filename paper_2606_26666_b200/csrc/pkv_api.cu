@@ -390,6 +390,7 @@ pkv_status pkv_get_counters(const pkv_shape* shape, const pkv_split_policy* poli
     host_out->merge_bytes = (int64_t)h.num_tasks * rp.G * (shape->d + 2) * 4;
     host_out->num_splits = h.resolved_splits;
     host_out->max_row_splits = h.max_row_splits;
+    host_out->chunk_tiles = h.chunk_tiles;
     return PKV_OK;
 }
 
@@ -559,6 +560,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         counters_out->merge_bytes = (int64_t)hdr->num_tasks * rp.G * (s.d + 2) * 4;
         counters_out->num_splits = hdr->resolved_splits;
         counters_out->max_row_splits = hdr->max_row_splits;
+        counters_out->chunk_tiles = hdr->chunk_tiles;
         counters_out->h2d_bytes = (int64_t)h2d;
         counters_out->d2h_bytes = (int64_t)out_bytes;
     }

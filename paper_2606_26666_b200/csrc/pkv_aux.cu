@@ -28,15 +28,16 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
     const int tid = threadIdx.x, nthreads = blockDim.x;
     pdl_launch_dependents();
     pdl_wait();   // the queue may still be read by the previous step's kernels
-    const PlanTotals tot = plan_scan(a.plan, a.seq_lens, a.split_offsets, nullptr, sc);
+    PlanArgs plan = a.plan;   // BALANCED: plan_scan resolves the batch-wide chunk into this copy
+    const PlanTotals tot = plan_scan(plan, a.seq_lens, a.split_offsets, nullptr, sc);
     for (int i = tid; i < a.plan.B * a.plan.Hkv; i += nthreads) a.fuse_counters[i] = 0;
     __threadfence_block();
     __syncthreads();
     const int64_t total = (int64_t)tot.row_slots * a.plan.Hkv;
     for (int32_t rs = tid; rs < tot.row_slots; rs += nthreads) {
         int32_t tb, te;
-        const RowSlot d = make_rowslot(a.plan, a.split_offsets, a.seq_lens, rs, &tb, &te);
-        write_pair(a.plan, d, tb, te, rs, a.rowslots, a.tasks, a.tasks_cap);
+        const RowSlot d = make_rowslot(plan, a.split_offsets, a.seq_lens, rs, &tb, &te);
+        write_pair(plan, d, tb, te, rs, a.rowslots, a.tasks, a.tasks_cap);
     }
     if (tid == 0) {
         QueueHeader h;
@@ -50,43 +51,86 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
         h.error_word = total > a.tasks_cap ? 1 : 0;
         h.sum_seq_lens = tot.sum_seq;
         h.build_launches = 1;
-        h.pad32_ = 0;
+        h.chunk_tiles = plan.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : plan.chunk_tiles;
         h.pad_[0] = h.pad_[1] = 0;
         *a.hdr = h;
     }
 }
 
-// One CTA of 4 warps per (row, query head): warp k computes the interleaved partial P_k of
-// pkv_device.cuh's merge arithmetic, warp 0 combines the four in order.  Rows with at most one
-// slot were written directly by the decode kernel.
+// One CTA of kMergeWarps warps per (row, query head).  Warp w owns the states w, w + NW, ...
+// of the (row, kvh) slot range; it issues the loads of kMergeBatch of them (m, l and one 16-byte
+// piece of acc per lane) before any arithmetic, so a row of up to NW * kMergeBatch = 128 splits
+// is ONE round trip to L2/HBM, and folds them into an online state (M_w, L_w, A_w) -- the merge
+// of PAPER.md:60-61 is associative, so the per-warp states combine exactly the same way.  Warp 0
+// combines the NW warp states in fixed order (deterministic).  Rows with at most one slot were
+// written directly by the decode kernel.
+constexpr int kMergeWarps = 16;
 template <int G>
-__global__ void __launch_bounds__(128) pkv_merge_kernel(const DecodeParams p) {
-    __shared__ float4 sA[4][32];
-    __shared__ float sL[4];
+__global__ void __launch_bounds__(kMergeWarps * 32) pkv_merge_kernel(const DecodeParams p) {
+    constexpr int NW = kMergeWarps, NB = kMergeBatch;
+    __shared__ float4 sA[NW][32];
+    __shared__ float sM[NW], sL[NW];
     const int row = blockIdx.x / p.Hq, h = blockIdx.x % p.Hq;
     const int kvh = h / G, hh = h % G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     pdl_launch_dependents();
     pdl_wait();
-    const int so = p.split_offsets[row];
-    const int n = p.split_offsets[row + 1] - so;
+    const int so = __ldcg(p.split_offsets + row);
+    const int n = __ldcg(p.split_offsets + row + 1) - so;
     if (n <= 1 && p.hdr != nullptr) return;   // library path: decode already produced out/lse
     const int64_t base = (int64_t)so * p.Hkv + (int64_t)kvh * n;
-    const float M = merge_row_max<G>(p, base, n, hh, lane);
-    float L[1];
-    float4 A[1];
-    merge_accumulate<G, 1>(p, base, n, hh, M, warp, 4, lane, L, A);
-    sA[warp][lane] = A[0];
-    if (lane == 0) sL[warp] = L[0];
+    float M = -INFINITY, L = 0.f;
+    float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int s0 = warp; s0 < n; s0 += NW * NB) {
+        float mv[NB], lv[NB];
+        float4 av[NB];
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+            const int s = s0 + j * NW;
+            const bool ok = s < n;
+            const int64_t r = (base + (ok ? s : 0)) * G + hh;
+            mv[j] = ok ? __ldcg(p.part_m + r) : -INFINITY;
+            lv[j] = ok ? __ldcg(p.part_l + r) : 0.f;
+            av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * kD + lane * 4))
+                       : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        float mb = mv[0];
+#pragma unroll
+        for (int j = 1; j < NB; ++j) mb = fmaxf(mb, mv[j]);
+        const float nM = fmaxf(M, mb);
+        if (nM == -INFINITY) continue;        // only neutral states so far (warp-uniform)
+        const float al = ex2_approx((M - nM) * kLog2e);   // M = -inf -> 0
+        L *= al;
+        A.x *= al; A.y *= al; A.z *= al; A.w *= al;
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+            const float w = ex2_approx((mv[j] - nM) * kLog2e);   // exp2(-inf) = 0
+            L = fmaf(w, lv[j], L);
+            A.x = fmaf(w, av[j].x, A.x); A.y = fmaf(w, av[j].y, A.y);
+            A.z = fmaf(w, av[j].z, A.z); A.w = fmaf(w, av[j].w, A.w);
+        }
+        M = nM;
+    }
+    sA[warp][lane] = A;
+    if (lane == 0) { sM[warp] = M; sL[warp] = L; }
     __syncthreads();
     if (warp == 0) {
-        const float Ls = ((sL[0] + sL[1]) + sL[2]) + sL[3];
-        float4 As;
-        As.x = ((sA[0][lane].x + sA[1][lane].x) + sA[2][lane].x) + sA[3][lane].x;
-        As.y = ((sA[0][lane].y + sA[1][lane].y) + sA[2][lane].y) + sA[3][lane].y;
-        As.z = ((sA[0][lane].z + sA[1][lane].z) + sA[2][lane].z) + sA[3][lane].z;
-        As.w = ((sA[0][lane].w + sA[1][lane].w) + sA[2][lane].w) + sA[3][lane].w;
-        merge_store(p, (int64_t)row * p.Hq + h, lane, M, Ls, As);
+        float Mf = sM[0];
+#pragma unroll
+        for (int w = 1; w < NW; ++w) Mf = fmaxf(Mf, sM[w]);
+        float Ls = 0.f;
+        float4 As = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (Mf != -INFINITY) {
+#pragma unroll
+            for (int w = 0; w < NW; ++w) {
+                const float wt = ex2_approx((sM[w] - Mf) * kLog2e);
+                const float4 a = sA[w][lane];
+                Ls = fmaf(wt, sL[w], Ls);
+                As.x = fmaf(wt, a.x, As.x); As.y = fmaf(wt, a.y, As.y);
+                As.z = fmaf(wt, a.z, As.z); As.w = fmaf(wt, a.w, As.w);
+            }
+        }
+        merge_store(p, (int64_t)row * p.Hq + h, lane, Mf, Ls, As);
     }
 }
 
@@ -114,8 +158,8 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     const int grid = p.B * p.Hq;
     if (grid <= 0) return cudaSuccess;
-    if (G == 4) return launch_pdl(pkv_merge_kernel<4>, dim3(grid), dim3(128), 0, stream, p);
-    return launch_pdl(pkv_merge_kernel<8>, dim3(grid), dim3(128), 0, stream, p);
+    if (G == 4) return launch_pdl(pkv_merge_kernel<4>, dim3(grid), dim3(kMergeWarps * 32), 0, stream, p);
+    return launch_pdl(pkv_merge_kernel<8>, dim3(grid), dim3(kMergeWarps * 32), 0, stream, p);
 }
 
 }  // namespace pkv

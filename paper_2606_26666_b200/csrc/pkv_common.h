@@ -33,7 +33,7 @@ struct QueueHeader {
     int32_t error_word;      // reserved
     int64_t sum_seq_lens;    // sum_i N_i
     int32_t build_launches;  // 1: written by the builder kernel, 0: by the decode kernel's fused build / the host
-    int32_t pad32_;
+    int32_t chunk_tiles;     // FIXED_CHUNK / BALANCED: resolved tiles per task, else 0
     int64_t pad_[2];
 };
 static_assert(sizeof(QueueHeader) == 64, "QueueHeader layout");
@@ -61,6 +61,7 @@ struct Resolved {
     int32_t merge_mode;
     int32_t kernel;
     int32_t G;
+    int32_t num_sms;    // BALANCED: U (policy.num_sms, else the device's)
 };
 
 // Byte offsets inside the caller's workspace.  Pure function of (shape, S bound).
@@ -88,13 +89,38 @@ inline RowSplits row_splits(int32_t N, int32_t tile_tokens, int32_t split_mode, 
     r.T = N > 0 ? (N + tile_tokens - 1) / tile_tokens : 0;
     if (r.T == 0) { r.c = 0; r.n = 0; return r; }
     int32_t Si = S;
-    if (split_mode == PKV_SPLIT_FIXED_CHUNK) {
+    if (split_mode != PKV_SPLIT_FIXED_COUNT) {   // FIXED_CHUNK, or BALANCED with its chunk resolved
         int32_t want = (r.T + chunk_tiles - 1) / chunk_tiles;
         Si = want < S ? want : S;
     }
     r.c = (r.T + Si - 1) / Si;
     r.n = (r.T + r.c - 1) / r.c;
     return r;
+}
+
+// BALANCED split mode (include/pkv.h; A21): the batch-wide chunk, from W = sum_i T_i,
+// U = num_sms and `fits(c)` = [sum_i ceil(T_i / c) <= U] (monotone in c).  The caller supplies
+// fits; host and device search the same interval the same way.
+constexpr int kBalWaves = 32;        // many-wave regime: about 32 pairs per SM
+constexpr int kBalMinTokens = 256;   // ... of at least 256 tokens each
+template <typename Fits>
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+inline int32_t balanced_chunk(int64_t W, int32_t U, int32_t tile_tokens, Fits fits) {
+    if (W <= 0 || U <= 0) return 1;
+    const int64_t m = (kBalMinTokens + tile_tokens - 1) / tile_tokens;
+    const int64_t w = (W + (int64_t)kBalWaves * U - 1) / ((int64_t)kBalWaves * U);
+    const int64_t c2 = w > m ? w : m;            // many-wave chunk
+    int64_t lo = (W + U - 1) / U, hi = lo + c2;  // single wave: c in [ceil(W/U), ceil(W/U) + c2]
+    if (fits((int32_t)hi)) {
+        while (lo < hi) {   // smallest c in [lo, hi] that fits
+            const int64_t mid = (lo + hi) >> 1;
+            if (fits((int32_t)mid)) hi = mid; else lo = mid + 1;
+        }
+        return (int32_t)lo;
+    }
+    return (int32_t)c2;
 }
 
 // Host planner shared by pkv_build_workqueue_host and pkv_decode_host.

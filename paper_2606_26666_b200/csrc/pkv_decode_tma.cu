@@ -115,17 +115,18 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
 
     const int HGn = p.Hkv / HG;                               // head groups per (row, split)
     int num_units = 0;
+    PlanArgs plan = p.plan;   // BALANCED: plan_scan resolves the batch-wide chunk into this copy
     if (p.fused_build) {
         // Fused build: every CTA derives split_offsets from seq_lens
         // itself (one load round trip + a block scan) and computes the RowSlot of its units from
         // shared memory; the CTAs share the writing of the queue (RowSlots, task list,
         // split_offsets, header) that the merge kernel and pkv_read_workqueue read.
-        const PlanTotals tot = plan_scan(p.plan, p.seq_lens, tail.so_s, tail.len_s, tail.plan_scratch);
+        const PlanTotals tot = plan_scan(plan, p.seq_lens, tail.so_s, tail.len_s, tail.plan_scratch);
         num_units = tot.row_slots * HGn;
         for (int rs = blockIdx.x * blockDim.x + tid; rs < tot.row_slots; rs += gridDim.x * blockDim.x) {
             int32_t tb, te;
-            const RowSlot d = make_rowslot(p.plan, tail.so_s, tail.len_s, rs, &tb, &te);
-            write_pair(p.plan, d, tb, te, rs, p.rowslots, p.tasks, p.tasks_cap);
+            const RowSlot d = make_rowslot(plan, tail.so_s, tail.len_s, rs, &tb, &te);
+            write_pair(plan, d, tb, te, rs, p.rowslots, p.tasks, p.tasks_cap);
         }
         if (blockIdx.x == 0) {
             for (int i = tid; i <= p.B; i += blockDim.x) p.split_offsets[i] = tail.so_s[i];
@@ -134,7 +135,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 p.hdr->num_tasks = (int32_t)(total < p.tasks_cap ? total : p.tasks_cap);
                 p.hdr->max_row_splits = tot.max_n;
                 p.hdr->total_row_slots = tot.row_slots;
-                p.hdr->resolved_splits = p.plan.S;
+                p.hdr->resolved_splits = plan.S;
+                p.hdr->chunk_tiles = plan.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : plan.chunk_tiles;
                 p.hdr->empty_tasks = (tot.row_slots - tot.sum_n) * p.Hkv;
                 p.hdr->error_word = total > p.tasks_cap ? 1 : 0;
                 p.hdr->sum_seq_lens = tot.sum_seq;
@@ -171,7 +173,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 if (t >= num_units) t = -1;
                 RowSlot d = {};
                 int32_t tb, te;
-                if (t >= 0) d = make_rowslot(p.plan, tail.so_s, tail.len_s, t / HGn, &tb, &te);
+                if (t >= 0) d = make_rowslot(plan, tail.so_s, tail.len_s, t / HGn, &tb, &te);
                 u.row = d.row; u.so = d.so; u.n = d.n; u.split = d.split; u.tok0 = d.tok0; u.tok1 = d.tok1;
             } else {
                 const int4* rsp = reinterpret_cast<const int4*>(p.rowslots + (k == 0 ? t / HGn : min(t, max(num_units - 1, 0)) / HGn));

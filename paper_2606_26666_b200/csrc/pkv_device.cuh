@@ -16,7 +16,7 @@ constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 
 struct PlanArgs {   // split policy as the device-side planner needs it
-    int32_t B, Hkv, S, tile_tokens, split_mode, chunk_tiles, route;
+    int32_t B, Hkv, S, tile_tokens, split_mode, chunk_tiles, route, num_sms;
 };
 
 struct DecodeParams {
@@ -168,13 +168,45 @@ struct PlanTotals {
     long long sum_seq;
 };
 
+// BALANCED (include/pkv.h): the batch-wide chunk, computed by one warp (every lane returns it).
+// lens[i] is row i's length (global or shared memory; values <= 0 count as empty rows).
+__device__ __forceinline__ int32_t balanced_chunk_warp(const PlanArgs& a, const int32_t* lens, int lane) {
+    long long W = 0;
+    for (int i = lane; i < a.B; i += 32) {
+        const int N = lens[i];
+        if (N > 0) W += (N + a.tile_tokens - 1) / a.tile_tokens;
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) W += __shfl_xor_sync(0xffffffffu, W, off);
+    return balanced_chunk((int64_t)W, a.num_sms, a.tile_tokens, [&](int32_t c) {
+        // ceil(T_i / c) = ceil(N_i / (tile_tokens * c)); 32-bit unsigned division
+        const long long span64 = (long long)a.tile_tokens * c;
+        const unsigned span = span64 >= 0x7fffffffLL ? 0x7fffffffu : (unsigned)span64;
+        int units = 0;
+        for (int i = lane; i < a.B; i += 32) {
+            const int N = lens[i];
+            if (N > 0) units += (int)(((unsigned)N + span - 1u) / span);
+        }
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) units += __shfl_xor_sync(0xffffffffu, units, off);
+        return units <= a.num_sms;
+    });
+}
+
 // Block-wide (every thread of the CTA calls it; blockDim.x a multiple of 32, <= 1024):
 // so_out[0..B] = exclusive prefix sum of the rows' slot counts (n_i, or S on the rect route),
 // len_out[i] = max(N_i, 0) if len_out != nullptr.  so_out / len_out may be global or shared.
-__device__ __forceinline__ PlanTotals plan_scan(const PlanArgs& a, const int32_t* seq_lens, int32_t* so_out,
+// BALANCED: resolves the batch-wide chunk first and rewrites `a` to the FIXED_CHUNK policy it
+// stands for (a.chunk_tiles = the chunk), which make_rowslot then uses.
+__device__ __forceinline__ PlanTotals plan_scan(PlanArgs& a, const int32_t* seq_lens, int32_t* so_out,
                                                 int32_t* len_out, PlanScratch& sc) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nthreads = blockDim.x, nwarps = nthreads >> 5;
+    const int32_t* lens = seq_lens;
+    if (len_out) {   // one global round trip: stage the lengths, plan from the staged copy
+        for (int i = tid; i < a.B; i += nthreads) len_out[i] = max(__ldcg(seq_lens + i), 0);
+        lens = len_out;
+    }
     if (tid == 0) {
         sc.carry = 0;
         sc.max_n = 0;
@@ -183,11 +215,15 @@ __device__ __forceinline__ PlanTotals plan_scan(const PlanArgs& a, const int32_t
         so_out[0] = 0;
     }
     __syncthreads();
+    if (a.split_mode == PKV_SPLIT_BALANCED) {
+        a.chunk_tiles = balanced_chunk_warp(a, lens, lane);   // every warp computes the same value
+        a.split_mode = PKV_SPLIT_FIXED_CHUNK;
+    }
     for (int base = 0; base < a.B; base += nthreads) {
         const int i = base + tid;
         int32_t slots = 0, N = 0, nonempty = 0;
         if (i < a.B) {
-            N = max(__ldcg(seq_lens + i), 0);
+            N = max(lens[i], 0);
             const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
             nonempty = r.n;
             slots = a.route == PKV_ROUTE_WORKQUEUE ? r.n : a.S;
@@ -213,7 +249,6 @@ __device__ __forceinline__ PlanTotals plan_scan(const PlanArgs& a, const int32_t
         const int32_t incl = sc.carry + (warp > 0 ? sc.warp_sums[warp - 1] : 0) + v;
         if (i < a.B) {
             so_out[i + 1] = incl;
-            if (len_out) len_out[i] = N;
             atomicMax(&sc.max_n, slots);
             atomicAdd(&sc.sum_n, nonempty);
             atomicAdd(&sc.sum_seq, (unsigned long long)N);
@@ -277,13 +312,13 @@ __device__ __forceinline__ void write_pair(const PlanArgs& a, const RowSlot& d, 
 // ------------------------------------------------------------------ merge of split states
 
 // Exact merge of the n states of one (row, kvh, head-in-group hh), stored at
-// slots slot_base .. slot_base+n-1.  The arithmetic is fixed so that the separate merge kernel
-// and the fused in-kernel merge give bit-identical results:
+// slots slot_base .. slot_base+n-1, by ONE warp -- the fused in-kernel merge of PAPER.md:77 (the
+// separate merge kernel, pkv_aux.cu, spreads a row over a whole CTA instead):
 //   M   = max_s m_s
 //   P_k = sum over s = k, k+4, k+8, ... (ascending) of exp(m_s - M) * (l_s, a_s),   k = 0..3
 //   (L, A) = ((P_0 + P_1) + P_2) + P_3,   O = A / L,   LSE = M + log L
-// A warp works on one head at a time; lane owns channels 4*lane .. 4*lane+3 (one 16-byte load
-// per state row).  Neutral states (m = -inf, l = 0) drop out; all-neutral gives O = 0, LSE = -inf.
+// Lane owns channels 4*lane .. 4*lane+3 (one 16-byte load per state row).  Neutral states
+// (m = -inf, l = 0) drop out; all-neutral gives O = 0, LSE = -inf.
 
 template <int G>
 __device__ __forceinline__ float merge_row_max(const DecodeParams& p, int64_t slot_base, int n, int hh, int lane) {
@@ -294,11 +329,9 @@ __device__ __forceinline__ float merge_row_max(const DecodeParams& p, int64_t sl
     return M;
 }
 
-// NK interleaved partial sums of one lane's 4 channels over the states first, first+stride, ...:
-// NK = 4 (first 0, stride 1): state s goes to P_{s mod 4}; NK = 1 (first k, stride 4): P_k only.
-// Either way P_k is the same ascending fma chain, so one warp doing all four and four warps doing
-// one each give bit-identical sums.  kMergeBatch independent state loads are in flight per lane;
-// they bypass L1 (states are written by other SMs, in the fused path during this very launch).
+// NK interleaved partial sums of one lane's 4 channels over the states first, first+stride, ...
+// kMergeBatch independent state loads are in flight per lane; they bypass L1 (states are written
+// by other SMs, in the fused path during this very launch).
 constexpr int kMergeBatch = 8;
 template <int G, int NK>
 __device__ __forceinline__ void merge_accumulate(const DecodeParams& p, int64_t slot_base, int n, int hh, float M,
@@ -501,7 +534,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 inline PlanArgs make_plan_args(const pkv_shape& shape, const Resolved& rp) {
     PlanArgs a;
     a.B = shape.B; a.Hkv = shape.Hkv; a.S = rp.S; a.tile_tokens = rp.tile_tokens;
-    a.split_mode = rp.split_mode; a.chunk_tiles = rp.chunk_tiles; a.route = rp.route;
+    a.split_mode = rp.split_mode; a.chunk_tiles = rp.chunk_tiles; a.route = rp.route; a.num_sms = rp.num_sms;
     return a;
 }
 

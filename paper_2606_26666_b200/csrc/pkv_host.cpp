@@ -48,7 +48,8 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
         set_error("tile_tokens=%d must be a positive multiple of page_size=%d", p.tile_tokens, s.page_size);
         return PKV_ERR_INVALID_ARG;
     }
-    if (p.split_mode != PKV_SPLIT_FIXED_COUNT && p.split_mode != PKV_SPLIT_FIXED_CHUNK) {
+    if (p.split_mode != PKV_SPLIT_FIXED_COUNT && p.split_mode != PKV_SPLIT_FIXED_CHUNK &&
+        p.split_mode != PKV_SPLIT_BALANCED) {
         set_error("bad split_mode %d", p.split_mode);
         return PKV_ERR_INVALID_ARG;
     }
@@ -66,8 +67,13 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     if (p.num_sms < 0) { set_error("num_sms < 0"); return PKV_ERR_INVALID_ARG; }
 
     int32_t S = p.num_splits;
+    out->num_sms = p.num_sms > 0 ? p.num_sms : num_sms_or_0;
+    if (p.split_mode == PKV_SPLIT_BALANCED && out->num_sms <= 0 && !bound_ok) {
+        set_error("BALANCED needs policy.num_sms > 0 in a host-only call");
+        return PKV_ERR_INVALID_ARG;
+    }
     if (S == 0) {
-        if (p.split_mode == PKV_SPLIT_FIXED_CHUNK) {
+        if (p.split_mode != PKV_SPLIT_FIXED_COUNT) {
             S = kMaxSplits;
         } else {
             int sms = p.num_sms > 0 ? p.num_sms : num_sms_or_0;
@@ -117,11 +123,23 @@ pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_
     int64_t count = 0, sum_seq = 0;
     int32_t max_n = 0, empties = 0, off = 0;
     bool overflow = false;
+    int32_t chunk = rp.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : rp.chunk_tiles;
+    if (rp.split_mode == PKV_SPLIT_BALANCED) {
+        int64_t W = 0;
+        for (int32_t i = 0; i < s.B; ++i)
+            if (seq_lens[i] > 0) W += ((int64_t)seq_lens[i] + rp.tile_tokens - 1) / rp.tile_tokens;
+        chunk = balanced_chunk(W, rp.num_sms, rp.tile_tokens, [&](int32_t c) {
+            int64_t units = 0;
+            for (int32_t i = 0; i < s.B; ++i)
+                if (seq_lens[i] > 0) units += ((int64_t)seq_lens[i] + (int64_t)rp.tile_tokens * c - 1) / ((int64_t)rp.tile_tokens * c);
+            return units <= rp.num_sms;
+        });
+    }
     if (split_offsets) split_offsets[0] = 0;
     for (int32_t i = 0; i < s.B; ++i) {
         const int32_t N = seq_lens[i] > 0 ? seq_lens[i] : 0;
         sum_seq += N;
-        const RowSplits r = row_splits(N, rp.tile_tokens, rp.split_mode, rp.S, rp.chunk_tiles);
+        const RowSplits r = row_splits(N, rp.tile_tokens, rp.split_mode, rp.S, chunk);
         const int32_t slots = rp.route == PKV_ROUTE_WORKQUEUE ? r.n : rp.S;
         if (slots > max_n) max_n = slots;
         for (int32_t g = 0; g < s.Hkv; ++g) {
@@ -167,6 +185,7 @@ pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_
         hdr->resolved_splits = rp.S;
         hdr->empty_tasks = empties;
         hdr->sum_seq_lens = sum_seq;
+        hdr->chunk_tiles = chunk;
     }
     if (overflow && tasks) return PKV_ERR_WORKSPACE;
     return PKV_OK;

@@ -43,9 +43,10 @@ class DevProblem:
 
 
 def oracle_policy(pol: pkv.Policy) -> wq.Policy:
+    """The same policy for the workqueue oracle; num_sms = 0 means the device's SM count."""
     return wq.Policy(tile_tokens=pol.tile_tokens, split_mode=pol.split_mode, num_splits=pol.num_splits,
                      chunk_tiles=pol.chunk_tiles, route=pol.route, merge_mode=pol.merge_mode,
-                     num_sms=pol.num_sms)
+                     num_sms=pol.num_sms if pol.num_sms > 0 else sm_count())
 
 
 def oracle_attention(p: Problem, **kw):

@@ -35,7 +35,7 @@ def test_version_and_struct_sizes():
     assert ctypes.sizeof(binding.pkv_task) == 20            # 5 x int32
     assert ctypes.sizeof(binding.pkv_split_policy) == 32
     assert ctypes.sizeof(binding.pkv_shape) == 56
-    assert ctypes.sizeof(binding.pkv_counters) == 88
+    assert ctypes.sizeof(binding.pkv_counters) == 96
 
 
 def shape(B, Hkv=8, Hq=32, max_pages=4096):
@@ -59,7 +59,7 @@ def test_shape_validation(bad, status):
 
 
 @pytest.mark.parametrize("bad", [dict(tile_tokens=24), dict(tile_tokens=0), dict(num_splits=257),
-                                 dict(split_mode=2), dict(route=3), dict(merge_mode=2), dict(kernel=9),
+                                 dict(split_mode=3), dict(split_mode=2, num_sms=0), dict(route=3), dict(merge_mode=2), dict(kernel=9),
                                  dict(split_mode=1, chunk_tiles=0), dict(num_splits=0, num_sms=0)])
 def test_policy_validation(bad):
     with pytest.raises(pkv.PkvError) as e:
@@ -94,6 +94,10 @@ POLICIES = [
     pkv.Policy(tile_tokens=32, num_splits=0, num_sms=148),
     pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=16),
     pkv.Policy(tile_tokens=128, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=12, chunk_tiles=3),
+    pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=148),
+    pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=148),
+    pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=28),
+    pkv.Policy(tile_tokens=64, split_mode=pkv.SPLIT_BALANCED, num_splits=5, num_sms=7),
     pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_RECT),
     pkv.Policy(tile_tokens=64, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=9, chunk_tiles=4, route=pkv.ROUTE_RECT),
 ]
@@ -121,7 +125,9 @@ def test_host_builder_on_the_trace_configs():
         for step in (0, w.steps):
             lens = w.seq_lens_at(step)
             for pol in (pkv.Policy(tile_tokens=32, num_splits=20),
-                        pkv.Policy(tile_tokens=64, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=8)):
+                        pkv.Policy(tile_tokens=64, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=8),
+                        pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=148),
+                        pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=148)):
                 ref_t, ref_o, _ = oracle_tasks(lens, w.Hkv, pol)
                 got_t, got_o = pkv.pkv_build_workqueue_host(shape(w.B, Hkv=w.Hkv), pol, lens)
                 assert np.array_equal(got_t, ref_t) and np.array_equal(got_o, ref_o), (w.name, step)

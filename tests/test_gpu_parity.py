@@ -90,7 +90,10 @@ def test_device_builder_bit_exact(route):
              list(rng.integers(1, 400, size=1500))]
     pols = [pkv.Policy(tile_tokens=32, num_splits=20), pkv.Policy(tile_tokens=64, num_splits=0),
             pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=16),
-            pkv.Policy(tile_tokens=16, num_splits=256)]
+            pkv.Policy(tile_tokens=16, num_splits=256),
+            pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0),
+            pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=7),
+            pkv.Policy(tile_tokens=64, split_mode=pkv.SPLIT_BALANCED, num_splits=12, num_sms=28)]
     for lens in cases:
         lens = np.array(lens, dtype=np.int32)
         for base in pols:
@@ -110,7 +113,7 @@ def test_device_builder_bit_exact(route):
                 c = pkv.pkv_get_counters(shape, pol, ws)
                 assert c["tasks"] == ref.num_tasks and c["empty_tasks"] == ref.empty_ctas
                 assert c["decode_launches"] == ref.decode_launches and c["merge_launches"] == ref.merge_launches
-                assert c["num_splits"] == ref.num_splits
+                assert c["num_splits"] == ref.num_splits and c["chunk_tiles"] == ref.chunk_tiles
                 assert c["useful_kv_bytes"] == wq.useful_kv_bytes(lens, Hkv, 128)
                 assert c["merge_bytes"] == wq.merge_bytes(ref.num_tasks, 32 // Hkv, 128)
 
@@ -419,7 +422,9 @@ def test_fused_build_queue_bit_exact_and_same_output(route):
     pols = [pkv.Policy(tile_tokens=32, num_splits=5, route=route),
             pkv.Policy(tile_tokens=16, num_splits=0, route=route),
             pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=3, route=route),
-            pkv.Policy(tile_tokens=32, num_splits=7, route=route, merge_mode=pkv.MERGE_FUSED)]
+            pkv.Policy(tile_tokens=32, num_splits=7, route=route, merge_mode=pkv.MERGE_FUSED),
+            pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, route=route),
+            pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=5, route=route)]
     for pol in pols:
         opol = oracle_policy(pol)
         if pol.num_splits == 0 and pol.split_mode == pkv.SPLIT_FIXED_COUNT:
@@ -439,5 +444,27 @@ def test_fused_build_queue_bit_exact_and_same_output(route):
             c = pkv.pkv_get_counters(dp.shape, pol, ws)
             assert c["tasks"] == want.num_tasks and c["empty_tasks"] == want.empty_ctas
             assert c["decode_launches"] == want.decode_launches and c["merge_launches"] == want.merge_launches
-            assert c["build_launches"] == (0 if fused else 1)
+            assert c["build_launches"] == (0 if fused else 1) and c["chunk_tiles"] == want.chunk_tiles
         assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+@pytest.mark.parametrize("Hkv", [8, 4])
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_balanced_policy_parity_single_wave_and_many_waves(kernel, Hkv):
+    """BALANCED split policy (A21) end to end: a ragged batch whose chunk comes from
+    the single-wave search (device SM count) and one forced into the many-wave regime
+    (num_sms = 3); tasks bit-exact vs the oracle, outputs within tolerance."""
+    lens = [9000, 40, 1300, 0, 517, 4097, 16, 2222]
+    p = make_problem(lens, seed=41, Hkv=Hkv)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    for pol in (pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, kernel=kernel),
+                pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=3, kernel=kernel),
+                pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=3, kernel=kernel,
+                           merge_mode=pkv.MERGE_FUSED)):
+        out, lse, ws, _ = check(dp, pol, ref, what=str(pol))
+        want = wq.build_workqueue(lens, Hkv, oracle_policy(pol))
+        tasks, offs = pkv.pkv_read_workqueue(dp.shape, pol, ws)
+        assert np.array_equal(tasks, np.array(want.tasks, dtype=np.int32).reshape(-1, 5)), pol
+        assert np.array_equal(offs, np.array(want.split_offsets, dtype=np.int32))
+        assert pkv.pkv_get_counters(dp.shape, pol, ws)["chunk_tiles"] == want.chunk_tiles

@@ -101,6 +101,51 @@ def test_p9_bruteforce_and_invariants_fuzz(mode):
         _check_invariants(seq, Hkv, polr, r)
 
 
+def test_balanced_policy_bruteforce_invariants_and_closed_forms():
+    """Reading A21 (BALANCED): the chunk search against an exhaustive scan over every c (the
+    brute force tests the single-wave conditions in rationals), the coverage invariants, the
+    single-wave guarantee (at most U (row, split) pairs, none longer than the chunk) and a few
+    cases worked by hand."""
+    rng = np.random.Generator(np.random.PCG64(77))
+    for trial in range(400):
+        B = int(rng.integers(1, 40))
+        Hkv = int(rng.choice([4, 8]))
+        tile = int(rng.choice([16, 32, 64]))
+        U = int(rng.choice([4, 28, 148]))
+        seq = [int(x) for x in rng.choice([0, 1, 16, 17, 100, 500, 1000, 5000, 40000, 65536], size=B)]
+        seq = [max(0, n + int(rng.integers(-3, 4))) for n in seq]
+        pol = wq.Policy(tile_tokens=tile, split_mode=wq.SPLIT_BALANCED, num_splits=int(rng.choice([0, 0, 7, 64])),
+                        num_sms=U)
+        q = wq.build_workqueue(seq, Hkv, pol)
+        assert q.tasks == wq.brute_force_tasks(seq, Hkv, pol)
+        _check_invariants(seq, Hkv, pol, q)
+        T = [-(-n // tile) for n in seq if n > 0]
+        W = sum(T)
+        if W == 0:
+            continue
+        c2 = max(-(-256 // tile), -(-W // (32 * U)))
+        assert all(te - tb <= max(q.chunk_tiles, -(-max(T) // q.num_splits)) for (_, _, _, tb, te) in q.tasks)
+        if q.chunk_tiles != c2 or sum(-(-t // c2) for t in T) <= U:
+            if pol.num_splits == 0:       # single wave (no cap on n_i in the way)
+                assert q.split_offsets[-1] <= U
+                assert -(-W // U) <= q.chunk_tiles <= -(-W // U) + c2
+                # minimality: one tile less per pair would need more than U pairs (or undercut the mean)
+                c = q.chunk_tiles - 1
+                assert c < -(-W // U) or sum(-(-t // c) for t in T) > U
+    # by hand, U = 148: one row of 32768 tokens, 32-token tiles: W = 1024, ceil(W/U) = 7,
+    # ceil(1024/7) = 147 <= 148 -> chunk 7, 147 splits (146 of 7 tiles, one of 2)
+    q = wq.build_workqueue([32768], 8, wq.Policy(tile_tokens=32, split_mode=wq.SPLIT_BALANCED, num_splits=0, num_sms=148))
+    assert q.chunk_tiles == 7 and q.split_offsets == [0, 147] and q.tasks[146] == (0, 0, 146, 1022, 1024)
+    # W <= U: every tile is its own task
+    q = wq.build_workqueue([256], 8, wq.Policy(tile_tokens=32, split_mode=wq.SPLIT_BALANCED, num_splits=0, num_sms=148))
+    assert q.chunk_tiles == 1 and q.split_offsets == [0, 8]
+    # more rows than SMs: no single wave exists -> many-wave chunk max(8, ceil(W / (32 U)))
+    q = wq.build_workqueue([3200] * 10, 8, wq.Policy(tile_tokens=32, split_mode=wq.SPLIT_BALANCED, num_splits=0, num_sms=4))
+    assert q.chunk_tiles == 8 and q.split_offsets[-1] == 10 * 13          # T = 100 -> S_i = 13, c = 8, n = 13
+    q = wq.build_workqueue([32000] * 10, 8, wq.Policy(tile_tokens=32, split_mode=wq.SPLIT_BALANCED, num_splits=0, num_sms=4))
+    assert q.chunk_tiles == -(-10000 // 128)                              # W = 10000, 32 U = 128 -> 79
+
+
 def test_known_small_case_by_hand():
     """N=100, tile 32 -> T=4; S=3 -> c=2, n=2: splits [0,2) and [2,4); N=10 -> T=1, n=1."""
     q = wq.build_workqueue([100, 10, 0], 2, wq.Policy(tile_tokens=32, num_splits=3))
