@@ -14,8 +14,8 @@ What is printed (ONE JSON line, rank 0):
              CUDA-event time of those K steps), inputs resident in HBM
   e2e        the same through pkv_decode_host with HOST buffers for q / block_table / seq_lens
              / out (host planning + one H2D image + launches + D2H + sync per step), wall clock
-  roofline   the decode kernel alone (PKV_STAGE_DECODE launches back to back between two CUDA
-             events): algorithmic bytes / average launch time / measured HBM peak
+  roofline   the decode kernel alone (PKV_STAGE_BUILD|PKV_STAGE_DECODE launches -- one kernel,
+             the queue is derived inside it -- back to back between two CUDA events): algorithmic bytes / average launch time / measured HBM peak
   cpu_baseline  oracle/ (FP64, test infrastructure) timed on this box's host cores, rank 0, N = 1
 L2: step t uses KV pool t % R of R rotating pools (R * KV bytes per step >> 126 MB L2), so no
 step finds its K/V in L2 ("inputs larger than L2").
@@ -161,12 +161,11 @@ class Runner:
         return self.lens_all_host[t % self.nlens]
 
     def launch_step(self, t, stages, stream):
-        """Step t: lengths of trace step t % (steps+1) copied into seq_lens (a D2D memcpy node),
-        then the chosen stages on pool t % R."""
+        """Step t: the chosen stages on pool t % R with the lengths of trace step t % (steps+1)
+        (row t of the device-resident [steps+1, B] length table: N_i += 1 per step)."""
         r = t % self.R
-        if self.nlens > 1 and (stages & self.pkv.STAGE_BUILD):
-            self.sl.copy_(self.lens_all[t % self.nlens], non_blocking=True)
-        self.pkv.pkv_decode_stages(self.shape, self.pol, self.q[r], self.k[r], self.v[r], self.bt[r], self.sl,
+        sl = self.lens_all[t % self.nlens] if (stages & self.pkv.STAGE_BUILD) else self.lens_all[0]
+        self.pkv.pkv_decode_stages(self.shape, self.pol, self.q[r], self.k[r], self.v[r], self.bt[r], sl,
                                    self.out, None, scale=self.scale, stages=stages, workspace=self.ws,
                                    stream=stream)
 
@@ -432,9 +431,9 @@ def time_workload(pkv, torch, w, pol, args, device, K, W, want_decode_only=True)
     ms = runner.run(K, chunk, pkv.STAGE_ALL)
     res = {"runner": runner, "R": R, "ms_total": ms, "counters": counters, "chunk": chunk}
     if want_decode_only:
-        runner.eager_step(0)                        # queue of step 0 in the workspace
-        runner.run(chunk, chunk, pkv.STAGE_DECODE)
-        res["ms_decode_only"] = runner.run(K, chunk, pkv.STAGE_DECODE)
+        dec = pkv.STAGE_BUILD | pkv.STAGE_DECODE     # the decode kernel as the step launches it (fused build)
+        runner.run(chunk, chunk, dec)
+        res["ms_decode_only"] = runner.run(K, chunk, dec)
     return res
 
 
@@ -481,6 +480,7 @@ def run_ours(args):
     import torch.distributed as dist
 
     import paper_2606_26666_b200 as pkv   # raises if libpkv.so is missing: there is no fallback
+    from paper_2606_26666_b200 import multirank
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -495,7 +495,7 @@ def run_ours(args):
     K, W = args.steps, max(args.warmup, 3)
 
     # every rank is a replica with its own seeded trace (data-parallel by row; DESIGN.md multi-GPU)
-    seed = args.seed + rank
+    seed = multirank.rank_seed(args.seed, rank)
     w = make_workload(args.workload, seed)
     pol = default_policy(pkv, args.workload, args)
     peak, peak_src = measured_hbm_peak()
@@ -536,9 +536,9 @@ def run_ours(args):
     torch.cuda.synchronize(device)
     if world > 1:
         dist.barrier()
-    runner.eager_step(0)
-    runner.run(chunk, chunk, pkv.STAGE_DECODE)
-    ms_dec = runner.run(K, chunk, pkv.STAGE_DECODE)
+    dec = pkv.STAGE_BUILD | pkv.STAGE_DECODE         # the decode kernel as the step launches it (fused build)
+    runner.run(chunk, chunk, dec)
+    ms_dec = runner.run(K, chunk, dec)
     clocks = sampler.result()
     counters = res["counters"]
 
@@ -548,10 +548,8 @@ def run_ours(args):
         e2e = (dt, c_e2e)
 
     # max over ranks
-    t_all = torch.tensor([ms_total, ms_dec, e2e[0] if e2e else 0.0], dtype=torch.float64, device=device)
-    if world > 1:
-        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
-    ms_total, ms_dec, e2e_s = [float(x) for x in t_all.cpu()]
+    ms_total, ms_dec, e2e_s = multirank.max_over_ranks([ms_total, ms_dec, e2e[0] if e2e else 0.0], device)
+    rows_all, = multirank.sum_over_ranks([w.B], device)
 
     if rank != 0:
         if world > 1:
@@ -563,7 +561,7 @@ def run_ours(args):
     us_dec = 1e3 * ms_dec / K
     launches_per_step = counters["build_launches"] + counters["decode_launches"] + counters["merge_launches"]
     line = {
-        "metric": "decode tokens/s", "value": w.B * world * K / (ms_total * 1e-3), "unit": "tokens/s",
+        "metric": "decode tokens/s", "value": multirank.whole_job_tokens_per_s(rows_all, K, ms_total), "unit": "tokens/s",
         "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_total / K, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f16 in / f32 accumulate", "data": "synthetic",
         "config": workload_config(w, pol, res["R"], args, world),
@@ -585,7 +583,7 @@ def run_ours(args):
         line["config"]["split_sweep"] = sweep
     if e2e:
         c = e2e[1]
-        line["e2e"] = {"value": w.B * world * K / e2e_s, "unit": "tokens/s", "us_per_step": 1e6 * e2e_s / K,
+        line["e2e"] = {"value": rows_all * K / e2e_s, "unit": "tokens/s", "us_per_step": 1e6 * e2e_s / K,
                        "h2d_bytes_per_step": c["h2d_bytes"], "d2h_bytes_per_step": c["d2h_bytes"],
                        "api": "pkv_decode_host (host planning + 1 H2D + launches + D2H + sync per step)"}
 

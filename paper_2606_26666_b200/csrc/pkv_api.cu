@@ -227,12 +227,17 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
         if (rp.kernel == PKV_KERNEL_TMA_MMA) {
             const int64_t row_slots = known_slots >= 0 ? known_slots : (int64_t)s.B * rp.S;
             const int HG = choose_heads_per_cta(s.Hkv, row_slots, num_sms);
-            const CUtensorMap* mk = get_map(k_cache, s, HG);
-            const CUtensorMap* mv = get_map(v_cache, s, HG);
-            if (!mk || !mv) {
+            // by value: inserting the V map may evict the cache entry the K pointer refers to
+            const CUtensorMap* pk = get_map(k_cache, s, HG);
+            CUtensorMap mk_copy, mv_copy;
+            if (pk) mk_copy = *pk;
+            const CUtensorMap* pv = get_map(v_cache, s, HG);
+            if (pv) mv_copy = *pv;
+            if (!pk || !pv) {
                 set_error("cuTensorMapEncodeTiled failed for the K/V cache (base %p/%p)", k_cache, v_cache);
                 return PKV_ERR_CUDA;
             }
+            const CUtensorMap *mk = &mk_copy, *mv = &mv_copy;
             p.heads_per_cta = HG;
             const int64_t units = row_slots * (s.Hkv / HG);
             const int grid = (int)(units < num_sms ? units : num_sms);

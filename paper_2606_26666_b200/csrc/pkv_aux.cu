@@ -65,6 +65,14 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
 // combines the NW warp states in fixed order (deterministic).  Rows with at most one slot were
 // written directly by the decode kernel.
 constexpr int kMergeWarps = 16;
+// debug trace (pkv_debug_set_trace): merge CTAs stamp behind the decode kernel's [148][16] block
+__device__ __forceinline__ void merge_trace_stamp(const DecodeParams& p, int slot) {
+    if (p.trace && blockIdx.x < 4096) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        p.trace[148 * 16 + (size_t)blockIdx.x * 4 + slot] = t;
+    }
+}
 template <int G>
 __global__ void __launch_bounds__(kMergeWarps * 32) pkv_merge_kernel(const DecodeParams p) {
     constexpr int NW = kMergeWarps, NB = kMergeBatch;
@@ -73,8 +81,10 @@ __global__ void __launch_bounds__(kMergeWarps * 32) pkv_merge_kernel(const Decod
     const int row = blockIdx.x / p.Hq, h = blockIdx.x % p.Hq;
     const int kvh = h / G, hh = h % G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) merge_trace_stamp(p, 0);
     pdl_launch_dependents();
     pdl_wait();
+    if (threadIdx.x == 0) merge_trace_stamp(p, 1);
     const int so = __ldcg(p.split_offsets + row);
     const int n = __ldcg(p.split_offsets + row + 1) - so;
     if (n <= 1 && p.hdr != nullptr) return;   // library path: decode already produced out/lse
@@ -114,6 +124,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32) pkv_merge_kernel(const Decod
     sA[warp][lane] = A;
     if (lane == 0) { sM[warp] = M; sL[warp] = L; }
     __syncthreads();
+    if (threadIdx.x == 0) merge_trace_stamp(p, 2);
     if (warp == 0) {
         float Mf = sM[0];
 #pragma unroll
@@ -131,6 +142,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32) pkv_merge_kernel(const Decod
             }
         }
         merge_store(p, (int64_t)row * p.Hq + h, lane, Mf, Ls, As);
+        if (lane == 0) merge_trace_stamp(p, 3);
     }
 }
 

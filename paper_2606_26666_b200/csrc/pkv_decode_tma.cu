@@ -35,6 +35,7 @@ namespace pkv {
 namespace {
 
 constexpr int kComputeWarps = 8;
+constexpr int kPlanBar = 9;         // named barrier: planner warp -> producer 0 (1..8 belong to the head groups)
 constexpr int kRing = 4;            // unit ring between producer 0 and everybody else
 constexpr int kMaxStages = 24;
 constexpr int kMaxFusedRows = 512;  // fused build: the batch's offsets and lengths sit in shared memory
@@ -56,7 +57,11 @@ struct SmemTail {
     unsigned long long ring_full[kRing];
     unsigned long long ring_empty[kRing];
     UnitInfo ring[kRing];
-    PlanScratch plan_scratch;
+    int32_t plan_row_slots;            // fused build: totals handed from the planner warp to producer 0
+    int32_t plan_chunk;
+    RowSlot first_slot;                // the RowSlot of this CTA's first unit (planner -> producer 0)
+    uint32_t sink_f[kComputeWarps];    // dependency sinks (see "stage release" in the kernel)
+    int sink_i[16];
     int32_t so_s[kMaxFusedRows + 1];   // fused build: split_offsets
     int32_t len_s[kMaxFusedRows];      //              max(N_i, 0)
 };
@@ -72,13 +77,14 @@ __host__ __device__ constexpr int stages_for() {
 }
 
 template <int G, int HG>
-__global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
+__global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 1)
     pkv_decode_tma_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap_k,
                           const __grid_constant__ CUtensorMap tmap_v) {
     constexpr int kStages = stages_for<G, HG>();
     constexpr int kStageBytes = HG * 8192;   // K: HG x 4096 | V: HG x 4096
     constexpr int NP = producers_for(HG);
     constexpr int WPH = kComputeWarps / HG;  // warps per head
+    constexpr int kPlanWarp = NP + kComputeWarps;   // the last warp plans and writes the queue
     static_assert(kStages >= 2, "ring too small");
     extern __shared__ unsigned char smem_raw[];
     // 128-byte swizzle: every 2 KiB half-box must start on a 1024-byte boundary
@@ -115,43 +121,61 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
 
     const int HGn = p.Hkv / HG;                               // head groups per (row, split)
     int num_units = 0;
-    PlanArgs plan = p.plan;   // BALANCED: plan_scan resolves the batch-wide chunk into this copy
-    if (p.fused_build) {
-        // Fused build: every CTA derives split_offsets from seq_lens
-        // itself (one load round trip + a block scan) and computes the RowSlot of its units from
-        // shared memory; the CTAs share the writing of the queue (RowSlots, task list,
-        // split_offsets, header) that the merge kernel and pkv_read_workqueue read.
-        const PlanTotals tot = plan_scan(plan, p.seq_lens, tail.so_s, tail.len_s, tail.plan_scratch);
-        num_units = tot.row_slots * HGn;
-        for (int rs = blockIdx.x * blockDim.x + tid; rs < tot.row_slots; rs += gridDim.x * blockDim.x) {
-            int32_t tb, te;
-            const RowSlot d = make_rowslot(plan, tail.so_s, tail.len_s, rs, &tb, &te);
-            write_pair(plan, d, tb, te, rs, p.rowslots, p.tasks, p.tasks_cap);
-        }
-        if (blockIdx.x == 0) {
-            for (int i = tid; i <= p.B; i += blockDim.x) p.split_offsets[i] = tail.so_s[i];
-            if (tid == 0) {
-                const int64_t total = (int64_t)tot.row_slots * p.Hkv;
-                p.hdr->num_tasks = (int32_t)(total < p.tasks_cap ? total : p.tasks_cap);
-                p.hdr->max_row_splits = tot.max_n;
-                p.hdr->total_row_slots = tot.row_slots;
-                p.hdr->resolved_splits = plan.S;
-                p.hdr->chunk_tiles = plan.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : plan.chunk_tiles;
-                p.hdr->empty_tasks = (tot.row_slots - tot.sum_n) * p.Hkv;
-                p.hdr->error_word = total > p.tasks_cap ? 1 : 0;
-                p.hdr->sum_seq_lens = tot.sum_seq;
-                p.hdr->build_launches = 0;
+    PlanArgs plan = p.plan;   // BALANCED: the planner resolves the batch-wide chunk
+    if (warp == kPlanWarp) {
+        // ================================================================ planner warp
+        // Fused build: one warp of every CTA derives split_offsets from
+        // seq_lens (one load round trip + warp scans), hands the plan to producer 0 through shared
+        // memory, and then -- off everybody's critical path -- writes this CTA's share of the
+        // queue (RowSlots, task list, split_offsets, header) that the merge kernel and
+        // pkv_read_workqueue read, and the outputs of rows without a task.
+        if (p.fused_build) {
+            const int32_t row_slots = plan_warp_prefix(plan, p.seq_lens, tail.so_s, tail.len_s, lane,
+                                                       (int)blockIdx.x / HGn, &tail.first_slot);
+            if (lane == 0) {
+                tail.plan_row_slots = row_slots;
+                tail.plan_chunk = plan.chunk_tiles;
+                trace_stamp(p, 8);
+            }
+            named_bar_sync(kPlanBar, 64);   // plan ready -> producer 0
+            const PlanTotals tot = plan_warp_totals(plan, tail.len_s, row_slots, lane);
+            for (int rs = blockIdx.x * 32 + lane; rs < tot.row_slots; rs += gridDim.x * 32) {
+                int32_t tb, te;
+                const RowSlot d = make_rowslot(plan, tail.so_s, tail.len_s, rs, &tb, &te);
+                write_pair(plan, d, tb, te, rs, p.rowslots, p.tasks, p.tasks_cap);
+            }
+            if (blockIdx.x == 0) {
+                for (int i = lane; i <= p.B; i += 32) p.split_offsets[i] = tail.so_s[i];
+                if (lane == 0) {
+                    const int64_t total = (int64_t)tot.row_slots * p.Hkv;
+                    p.hdr->num_tasks = (int32_t)(total < p.tasks_cap ? total : p.tasks_cap);
+                    p.hdr->max_row_splits = tot.max_n;
+                    p.hdr->total_row_slots = tot.row_slots;
+                    p.hdr->resolved_splits = plan.S;
+                    p.hdr->chunk_tiles = plan.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : plan.chunk_tiles;
+                    p.hdr->empty_tasks = (tot.row_slots - tot.sum_n) * p.Hkv;
+                    p.hdr->error_word = total > p.tasks_cap ? 1 : 0;
+                    p.hdr->sum_seq_lens = tot.sum_seq;
+                    p.hdr->build_launches = 0;
+                }
             }
         }
         for (int i = blockIdx.x; i < p.B; i += gridDim.x) {   // rows without a task (A9)
-            if (tail.len_s[i] > 0) continue;
-            for (int e = tid; e < p.Hq * kD; e += blockDim.x) {
+            if ((p.fused_build ? tail.len_s[i] : __ldcg(p.seq_lens + i)) > 0) continue;
+            for (int e = lane; e < p.Hq * kD; e += 32) {
                 p.out[(int64_t)i * p.Hq * kD + e] = __float2half_rn(0.f);
                 if (p.lse && e < p.Hq) p.lse[(int64_t)i * p.Hq + e] = -INFINITY;
             }
         }
-    } else {
-        zero_empty_rows(p);
+        return;
+    }
+    if (p.fused_build && warp == 0) {
+        named_bar_sync(kPlanBar, 64);
+        num_units = tail.plan_row_slots * HGn;
+        if (plan.split_mode == PKV_SPLIT_BALANCED) {
+            plan.split_mode = PKV_SPLIT_FIXED_CHUNK;
+            plan.chunk_tiles = tail.plan_chunk;
+        }
     }
 
     // ---- unit hand-out (producer 0) / pick-up (everybody else) -------------------------------
@@ -173,7 +197,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 if (t >= num_units) t = -1;
                 RowSlot d = {};
                 int32_t tb, te;
-                if (t >= 0) d = make_rowslot(plan, tail.so_s, tail.len_s, t / HGn, &tb, &te);
+                if (t >= 0 && k == 0) d = tail.first_slot;   // computed by the planner warp
+                else if (t >= 0) d = make_rowslot(plan, tail.so_s, tail.len_s, t / HGn, &tb, &te);
                 u.row = d.row; u.so = d.so; u.n = d.n; u.split = d.split; u.tok0 = d.tok0; u.tok1 = d.tok1;
             } else {
                 const int4* rsp = reinterpret_cast<const int4*>(p.rowslots + (k == 0 ? t / HGn : min(t, max(num_units - 1, 0)) / HGn));
@@ -194,7 +219,13 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
             mbar_wait(rfull0 + 8 * r, (k / kRing) & 1);
             u = tail.ring[r];
             __syncwarp();
-            if (lane == 0) mbar_arrive(rempty0 + 8 * r);
+            if (lane == 0) {
+                // The slot is released only after its loads have RETURNED: the store below needs
+                // every field (an mbarrier arrive may otherwise overtake loads still in flight).
+                sts_b32(smem_u32(&tail.sink_i[warp]),
+                        (uint32_t)(u.unit + u.row + u.so + u.n + u.split + u.tok0 + u.tok1 + u.pad_));
+                mbar_arrive(rempty0 + 8 * r);
+            }
         }
         return u;
     };
@@ -374,15 +405,28 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
 
                 // ---- O^T += V^T . P^T
                 mbar_wait(fullv0 + 8 * s, par);
+                uint32_t vdep = 0;   // a word of every V fragment (see the stage release below)
 #pragma unroll
                 for (int mt = 0; mt < 8; ++mt) {
                     uint32_t a0, a1, a2, a3;
                     const uint32_t chunk = ((mt & 3) << 1) | v_sel;
                     ldmatrix_x4_trans(vb + (mt >> 2) * 2048 + v_tok * 128 + ((chunk ^ xr) << 4), a0, a1, a2, a3);
                     mma_16816(o[mt], a0, a1, a2, a3, pb0, pb1);
+                    vdep ^= a3;
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(empty0 + 8 * s);   // this head's part of the stage is consumed
+                if (lane == 0) {
+                    // This head's part of the stage is consumed -- but only once the LAST ldmatrix
+                    // has returned its data.  ptxas schedules the arrive right behind the issue of
+                    // that ldmatrix, ahead of the HMMAs that wait for it, and the arrive can
+                    // overtake the load when the SM's memory pipe is backed up: the producer then
+                    // refills the stage under the load (seen as stale V rows in channels 112..127,
+                    // DESIGN.md "stage release").  The store needs a word of every V fragment, so
+                    // it cannot issue before all eight ldmatrix have completed, and a
+                    // release-arrive cannot move above a store of its own thread.
+                    sts_b32(smem_u32(&tail.sink_f[cw]), vdep);
+                    mbar_arrive(empty0 + 8 * s);
+                }
                 if (s + WPH < (uint32_t)kStages) { s += WPH; j += WPH; }
                 else { j += (int)((uint32_t)kStages - s) + sub; s = (uint32_t)sub; par ^= 1; }
             }
@@ -394,21 +438,64 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps) * 32, 1)
                 lA += __shfl_xor_sync(0xffffffffu, lA, off);
                 lB += __shfl_xor_sync(0xffffffffu, lB, off);
             }
-            if (hA < G) {
+            if constexpr (WPH == 1) {
+                // The warp owns the whole task: its state goes from the MMA accumulators straight
+                // to the task's slot (or to `out`), no shared-memory round trip.  Per store
+                // instruction the 8 lanes of a column write 32 contiguous bytes.
+                if (hA < G) {
+                    const int64_t hrow = (int64_t)row * p.Hq + kvh * G + hA;
+                    if (n_i <= 1) {
+                        const float iA = 1.0f / lA, iB = 1.0f / lB;
+                        __half* oA = p.out + hrow * kD + g4;
+                        __half* oB = oA + kD;
 #pragma unroll
-                for (int mt = 0; mt < 8; ++mt) {
-                    tail.cb.acc[cw][hA][mt * 16 + g4] = o[mt][0];
-                    tail.cb.acc[cw][hB][mt * 16 + g4] = o[mt][1];
-                    tail.cb.acc[cw][hA][mt * 16 + g4 + 8] = o[mt][2];
-                    tail.cb.acc[cw][hB][mt * 16 + g4 + 8] = o[mt][3];
+                        for (int mt = 0; mt < 8; ++mt) {
+                            oA[mt * 16] = __float2half_rn(o[mt][0] * iA);
+                            oB[mt * 16] = __float2half_rn(o[mt][1] * iB);
+                            oA[mt * 16 + 8] = __float2half_rn(o[mt][2] * iA);
+                            oB[mt * 16 + 8] = __float2half_rn(o[mt][3] * iB);
+                        }
+                        if (p.lse && g4 == 0) {
+                            p.lse[hrow] = mA * p.scale + logf(lA);
+                            p.lse[hrow + 1] = mB * p.scale + logf(lB);
+                        }
+                    } else {
+                        float* aA = p.part_acc + (slot * G + hA) * kD + g4;
+                        float* aB = aA + kD;
+#pragma unroll
+                        for (int mt = 0; mt < 8; ++mt) {
+                            aA[mt * 16] = o[mt][0];
+                            aB[mt * 16] = o[mt][1];
+                            aA[mt * 16 + 8] = o[mt][2];
+                            aB[mt * 16 + 8] = o[mt][3];
+                        }
+                        if (g4 == 0) {
+                            p.part_m[slot * G + hA] = mA * p.scale;
+                            p.part_m[slot * G + hB] = mB * p.scale;
+                            p.part_l[slot * G + hA] = lA;
+                            p.part_l[slot * G + hB] = lB;
+                        }
+                    }
                 }
-                if (g4 == 0) {
-                    tail.cb.m[cw][hA] = mA; tail.cb.m[cw][hB] = mB;
-                    tail.cb.l[cw][hA] = lA; tail.cb.l[cw][hB] = lB;
+                if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED)
+                    fused_complete<G, 1>(p, &tail.cb.flag[cw], row, kvh, split, n_i, slot, lane, 1 + hl);
+            } else {
+                if (hA < G) {
+#pragma unroll
+                    for (int mt = 0; mt < 8; ++mt) {
+                        tail.cb.acc[cw][hA][mt * 16 + g4] = o[mt][0];
+                        tail.cb.acc[cw][hB][mt * 16 + g4] = o[mt][1];
+                        tail.cb.acc[cw][hA][mt * 16 + g4 + 8] = o[mt][2];
+                        tail.cb.acc[cw][hB][mt * 16 + g4 + 8] = o[mt][3];
+                    }
+                    if (g4 == 0) {
+                        tail.cb.m[cw][hA] = mA; tail.cb.m[cw][hB] = mB;
+                        tail.cb.l[cw][hA] = lA; tail.cb.l[cw][hB] = lB;
+                    }
                 }
+                group_sync<WPH>(1 + hl);
+                finalize_task<G, WPH, kComputeWarps>(p, tail.cb, hl, HG, row, kvh, split, n_i, slot, gtid, 1 + hl);
             }
-            group_sync<WPH>(1 + hl);
-            finalize_task<G, WPH, kComputeWarps>(p, tail.cb, hl, HG, row, kvh, split, n_i, slot, gtid, 1 + hl);
             if (k == 0 && cw == 0 && lane == 0) trace_stamp(p, 6);
         }
     }
@@ -418,7 +505,7 @@ template <int G, int HG>
 cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, const CUtensorMap& mv,
                        cudaStream_t stream) {
     constexpr int smem = stages_for<G, HG>() * HG * 8192 + (int)sizeof(SmemTail<G>) + 1024;
-    constexpr int threads = (producers_for(HG) + kComputeWarps) * 32;
+    constexpr int threads = (producers_for(HG) + kComputeWarps + 1) * 32;
     static bool attr_set = false;
     if (!attr_set) {
         const cudaError_t e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);

@@ -57,6 +57,9 @@ __device__ __forceinline__ float ex2_approx(float x) {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
+__device__ __forceinline__ void sts_b32(uint32_t addr, uint32_t v) {
+    asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -170,27 +173,67 @@ struct PlanTotals {
 
 // BALANCED (include/pkv.h): the batch-wide chunk, computed by one warp (every lane returns it).
 // lens[i] is row i's length (global or shared memory; values <= 0 count as empty rows).
+// Same result as the host's balanced_chunk (pkv_common.h): `fits` is monotone in c, so the
+// smallest fitting c of [lo, hi] is found either by the host's bisection (large batches: lanes
+// over rows) or by testing 32 candidates at once (small batches: lanes over candidates, no
+// shuffles on the critical path of a short decode step).  32-bit arithmetic while W < 2^31.
 __device__ __forceinline__ int32_t balanced_chunk_warp(const PlanArgs& a, const int32_t* lens, int lane) {
-    long long W = 0;
+    long long W64 = 0;
     for (int i = lane; i < a.B; i += 32) {
         const int N = lens[i];
-        if (N > 0) W += (N + a.tile_tokens - 1) / a.tile_tokens;
+        if (N > 0) W64 += (unsigned)(N + a.tile_tokens - 1) / (unsigned)a.tile_tokens;
     }
+    if (__any_sync(0xffffffffu, W64 >= (1 << 26))) {   // 32 lanes x 2^26 < 2^31: else one redux.sync
 #pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) W += __shfl_xor_sync(0xffffffffu, W, off);
-    return balanced_chunk((int64_t)W, a.num_sms, a.tile_tokens, [&](int32_t c) {
+        for (int off = 16; off >= 1; off >>= 1) W64 += __shfl_xor_sync(0xffffffffu, W64, off);
+    } else {
+        W64 = (long long)__reduce_add_sync(0xffffffffu, (unsigned)W64);
+    }
+    auto units_of = [&](unsigned c, int first, int step) {   // sum over rows first, first+step, ... of ceil(T_i / c)
         // ceil(T_i / c) = ceil(N_i / (tile_tokens * c)); 32-bit unsigned division
-        const long long span64 = (long long)a.tile_tokens * c;
-        const unsigned span = span64 >= 0x7fffffffLL ? 0x7fffffffu : (unsigned)span64;
-        int units = 0;
-        for (int i = lane; i < a.B; i += 32) {
+        const unsigned long long span64 = (unsigned long long)(unsigned)a.tile_tokens * c;
+        const unsigned span = span64 >= 0x7fffffffull ? 0x7fffffffu : (unsigned)span64;
+        unsigned units = 0;
+        for (int i = first; i < a.B; i += step) {
             const int N = lens[i];
-            if (N > 0) units += (int)(((unsigned)N + span - 1u) / span);
+            if (N > 0) units += ((unsigned)N + span - 1u) / span;
         }
+        return units;
+    };
+    if (W64 <= 0 || a.num_sms <= 0) return 1;
+    if (W64 >= 0x7fffffffLL) {
+        return balanced_chunk((int64_t)W64, a.num_sms, a.tile_tokens, [&](int32_t c) {
+            unsigned units = units_of((unsigned)c, lane, 32);
+#pragma unroll
+            for (int off = 16; off >= 1; off >>= 1) units += __shfl_xor_sync(0xffffffffu, units, off);
+            return units <= (unsigned)a.num_sms;
+        });
+    }
+    const unsigned W = (unsigned)W64, U = (unsigned)a.num_sms;
+    const unsigned m = ((unsigned)kBalMinTokens + a.tile_tokens - 1) / (unsigned)a.tile_tokens;
+    const unsigned w = (W + kBalWaves * U - 1) / (kBalWaves * U);
+    const unsigned c2 = w > m ? w : m;
+    unsigned lo = (W + U - 1) / U, hi = lo + c2;
+    if (a.B <= 16) {
+        for (unsigned base = lo; base <= hi; base += 32) {
+            const unsigned c = base + lane;
+            const unsigned ok = __ballot_sync(0xffffffffu, c <= hi && units_of(c, 0, 1) <= U);
+            if (ok) return (int32_t)(base + __ffs(ok) - 1);
+        }
+        return (int32_t)c2;
+    }
+    auto fits = [&](unsigned c) {
+        unsigned units = units_of(c, lane, 32);
 #pragma unroll
         for (int off = 16; off >= 1; off >>= 1) units += __shfl_xor_sync(0xffffffffu, units, off);
-        return units <= a.num_sms;
-    });
+        return units <= U;
+    };
+    if (!fits(hi)) return (int32_t)c2;
+    while (lo < hi) {
+        const unsigned mid = (lo + hi) >> 1;
+        if (fits(mid)) hi = mid; else lo = mid + 1;
+    }
+    return (int32_t)lo;
 }
 
 // Block-wide (every thread of the CTA calls it; blockDim.x a multiple of 32, <= 1024):
@@ -262,6 +305,87 @@ __device__ __forceinline__ PlanTotals plan_scan(PlanArgs& a, const int32_t* seq_
     t.max_n = sc.max_n;
     t.sum_n = sc.sum_n;
     t.sum_seq = (long long)sc.sum_seq;
+    return t;
+}
+
+// The same plan by ONE warp (the decode kernel's planner warp; B <= a few hundred rows), in two
+// parts.  plan_warp_prefix is the critical path of a decode launch: lens staged in len_out,
+// BALANCED chunk resolved into `a`, so_out[0..B] by warp scans with a carry, and -- by the lane
+// that owns the row -- the RowSlot of pair rs0 (the calling CTA's first work unit) into *first.
+// Returns the number of (row, split) pairs.  plan_warp_totals (off the critical path) redoes the
+// per-row bounds for the header counters.  so_out / len_out / first: shared memory of the CTA.
+__device__ __forceinline__ int32_t plan_warp_prefix(PlanArgs& a, const int32_t* seq_lens, int32_t* so_out,
+                                                    int32_t* len_out, int lane, int rs0, RowSlot* first) {
+#pragma unroll 4
+    for (int i = lane; i < a.B; i += 32) len_out[i] = max(__ldcg(seq_lens + i), 0);
+    if (lane == 0) so_out[0] = 0;
+    __syncwarp();
+    if (a.split_mode == PKV_SPLIT_BALANCED) {
+        a.chunk_tiles = balanced_chunk_warp(a, len_out, lane);
+        a.split_mode = PKV_SPLIT_FIXED_CHUNK;
+    }
+    int32_t carry = 0;
+    for (int base = 0; base < a.B; base += 32) {
+        const int i = base + lane;
+        int32_t slots = 0, N = 0;
+        RowSplits r = {0, 0, 0};
+        if (i < a.B) {
+            N = len_out[i];
+            r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
+            slots = a.route == PKV_ROUTE_WORKQUEUE ? r.n : a.S;
+        }
+        int32_t v = slots;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const int32_t u = __shfl_up_sync(0xffffffffu, v, off);
+            if (lane >= off) v += u;
+        }
+        const int32_t incl = carry + v, excl = incl - slots;
+        if (i < a.B) {
+            so_out[i + 1] = incl;
+            if (rs0 >= excl && rs0 < incl) {   // this lane's row owns pair rs0
+                RowSlot d;
+                d.row = i; d.so = excl; d.n = slots; d.split = rs0 - excl;
+                int32_t tb = 0, te = 0;
+                if (r.T > 0) {
+                    const long long b = (long long)d.split * r.c, e = b + r.c;
+                    tb = (int32_t)(b < r.T ? b : r.T);
+                    te = (int32_t)(e < r.T ? e : r.T);
+                }
+                d.tok0 = tb * a.tile_tokens;
+                d.tok1 = min(te * a.tile_tokens, N);
+                d.pad_[0] = d.pad_[1] = 0;
+                *first = d;
+            }
+        }
+        carry += __shfl_sync(0xffffffffu, v, 31);
+    }
+    __syncwarp();
+    return carry;
+}
+
+__device__ __forceinline__ PlanTotals plan_warp_totals(const PlanArgs& a, const int32_t* len_s, int32_t row_slots,
+                                                       int lane) {
+    int32_t max_n = 0, sum_n = 0;
+    long long sum_seq = 0;
+    for (int i = lane; i < a.B; i += 32) {
+        const int32_t N = len_s[i];
+        const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
+        sum_n += r.n;
+        sum_seq += N;
+        max_n = max(max_n, a.route == PKV_ROUTE_WORKQUEUE ? r.n : a.S);
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        max_n = max(max_n, __shfl_xor_sync(0xffffffffu, max_n, off));
+        sum_n += __shfl_xor_sync(0xffffffffu, sum_n, off);
+        sum_seq += __shfl_xor_sync(0xffffffffu, sum_seq, off);
+    }
+    PlanTotals t;
+    t.row_slots = row_slots;
+    t.max_n = max_n;
+    t.sum_n = sum_n;
+    t.sum_seq = sum_seq;
     return t;
 }
 

@@ -468,3 +468,36 @@ def test_balanced_policy_parity_single_wave_and_many_waves(kernel, Hkv):
         assert np.array_equal(tasks, np.array(want.tasks, dtype=np.int32).reshape(-1, 5)), pol
         assert np.array_equal(offs, np.array(want.split_offsets, dtype=np.int32))
         assert pkv.pkv_get_counters(dp.shape, pol, ws)["chunk_tiles"] == want.chunk_tiles
+
+
+def test_stage_release_waits_for_the_last_ldmatrix():
+    """Regression: a compute warp's mbarrier arrive on a stage's
+    `empty` barrier was scheduled right behind the ISSUE of its last ldmatrix and could overtake
+    it while the planner warp's queue stores backed up the SM's memory pipe; the producer then
+    refilled the stage under the load.  K = 0 makes every token's weight exactly 1, V rows are
+    one-hot tags of the token index mod 128, so out * N counts the tokens seen per tag: any
+    token read from another page shows up as a count that is off by one (it was 1..4 tags in
+    about 2 % of the launches, always in channels 112..127 -- the last ldmatrix)."""
+    rng = np.random.Generator(np.random.PCG64(10002))
+    B = 200
+    lens = rng.integers(1, 3000, size=B).astype(np.int32)
+    p = make_problem(list(lens), seed=502)
+    p.k_cache[:] = 0
+    p.v_cache[:] = 0
+    exp = np.zeros((B, 128))
+    for i in range(B):
+        j = np.arange(lens[i])
+        p.v_cache[p.block_table[i, j // 16], j % 16, :, j % 128] = 1.0
+        exp[i] = np.bincount(j % 128, minlength=128)
+    dp = DevProblem(p)
+    pkv.pkv_debug_force_heads_per_cta(2)
+    try:
+        pol = pkv.Policy(tile_tokens=32, num_splits=1)
+        ws = pkv.alloc_workspace(dp.shape, pol)
+        for rep in range(120):
+            out, lse, _ = dp.decode(pol, ws=ws)
+            cnt = out * lens[:, None, None].astype(np.float64)
+            assert np.abs(cnt - exp[:, None, :]).max() < 0.3, "launch %d: a token was read from another page" % rep
+            assert np.abs(lse - np.log(lens)[:, None]).max() < 1e-5
+    finally:
+        pkv.pkv_debug_force_heads_per_cta(0)
