@@ -506,6 +506,16 @@ def run_ours(args):
         # paper's auto rule (A12) and the BALANCED policy (A21); the timed run uses the fastest
         cands = [(str(S), pkv.Policy(tile_tokens=32, num_splits=S, route=pol.route, merge_mode=pol.merge_mode,
                                      kernel=pol.kernel)) for S in (1, 4, 16, 64, 0)] + [("balanced", pol)]
+        # FIXED_COUNT with one single-head unit per SM: S = floor(SMs / (B * Hkv))
+        s_fit = torch.cuda.get_device_properties(device).multi_processor_count // max(1, w.B * w.Hkv)
+        if s_fit > 1 and s_fit not in (4, 16, 64):
+            cands.append((str(s_fit), pkv.Policy(tile_tokens=32, num_splits=s_fit, route=pol.route,
+                                                 merge_mode=pol.merge_mode, kernel=pol.kernel)))
+        # BALANCED aimed at one unit per SM with 4 / 2 KV heads per CTA: U = SMs * HG / Hkv pairs
+        sms = torch.cuda.get_device_properties(device).multi_processor_count
+        for hg in (4, 2):
+            if w.Hkv % hg == 0 and w.Hkv > hg:
+                cands.append(("balanced_hg%d" % hg, pkv.Policy(**{**pol.__dict__, "num_sms": sms * hg // w.Hkv})))
         pols = {}
         for key, p2 in cands:
             r = time_workload(pkv, torch, w, p2, args, device, min(K, 4 * args.graph_steps), W, want_decode_only=False)

@@ -225,7 +225,12 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     }
     if (known_tasks != 0 && (stages & PKV_STAGE_DECODE)) {
         if (rp.kernel == PKV_KERNEL_TMA_MMA) {
-            const int64_t row_slots = known_slots >= 0 ? known_slots : (int64_t)s.B * rp.S;
+            // (row, split) pairs the queue will hold: known when planned on the host, else a bound.
+            // BALANCED aims at a single wave of at most U = policy.num_sms pairs, so a caller that
+            // passes U = SMs * HG / Hkv gets HG heads per CTA and one unit per SM.
+            int64_t row_slots = known_slots >= 0 ? known_slots : (int64_t)s.B * rp.S;
+            if (known_slots < 0 && rp.split_mode == PKV_SPLIT_BALANCED && rp.num_sms > 0 && rp.num_sms < row_slots)
+                row_slots = rp.num_sms;
             const int HG = choose_heads_per_cta(s.Hkv, row_slots, num_sms);
             // by value: inserting the V map may evict the cache entry the K pointer refers to
             const CUtensorMap* pk = get_map(k_cache, s, HG);

@@ -239,6 +239,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         // adjacent phases apart: a warp that skipped a phase of a stage could pass the wait for
         // the next one while the skipped fill is still in flight.)
         uint32_t ps = 0, pphase = 0;
+        const unsigned long long kv_policy = l2_policy_evict_first();
         for (int k = 0;; ++k) {
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
@@ -266,9 +267,9 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                         const uint32_t dst = stage_base + s * kStageBytes;
                         // box dims: (64 ch, 16 tok, 2 ch-halves, HG heads, 1 page)
                         mbar_arrive_expect_tx(fullk0 + 8 * s, HG * 4096);
-                        tma_load_5d(dst, &tmap_k, fullk0 + 8 * s, 0, 0, 0, head0, page);
+                        tma_load_5d(dst, &tmap_k, fullk0 + 8 * s, 0, 0, 0, head0, page, kv_policy);
                         mbar_arrive_expect_tx(fullv0 + 8 * s, HG * 4096);
-                        tma_load_5d(dst + HG * 4096, &tmap_v, fullv0 + 8 * s, 0, 0, 0, head0, page);
+                        tma_load_5d(dst + HG * 4096, &tmap_v, fullv0 + 8 * s, 0, 0, 0, head0, page, kv_policy);
                     }
                 }
                 mine = nxt;
