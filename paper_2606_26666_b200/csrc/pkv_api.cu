@@ -244,6 +244,12 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             }
             const CUtensorMap *mk = &mk_copy, *mv = &mv_copy;
             p.heads_per_cta = HG;
+            // Units are handed out by an atomic counter only when every head has ONE compute warp
+            // (HG = 8): with several warps per head the page-to-warp assignment follows the CTA's
+            // stream position, so a dynamic hand-out would make the FP32 combine order -- and the
+            // last bits of the result -- depend on which units a CTA drew before.  Round-robin
+            // keeps every launch bitwise reproducible.
+            p.dynamic_sched = HG == 8 ? 1 : 0;
             const int64_t units = row_slots * (s.Hkv / HG);
             const int grid = (int)(units < num_sms ? units : num_sms);
             e = launch_decode_tma(p, rp.G, HG, grid, mk, mv, stream);
