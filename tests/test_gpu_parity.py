@@ -501,3 +501,65 @@ def test_stage_release_waits_for_the_last_ldmatrix():
             assert np.abs(lse - np.log(lens)[:, None]).max() < 1e-5
     finally:
         pkv.pkv_debug_force_heads_per_cta(0)
+
+
+def _compact_rows(w, k_dev, v_dev, rows, lens):
+    """Host copy of the pages of `rows` only (compact pool + identity tables), for the oracle."""
+    P = w.page_size
+    tables, ks, vs, base = [], [], [], 0
+    width = max(-(-int(lens[i]) // P) for i in rows)
+    for i in rows:
+        npg = -(-int(lens[i]) // P)
+        pages = torch.from_numpy(w.block_table[i, :npg].astype(np.int64)).cuda()
+        ks.append(k_dev[pages].cpu().numpy())
+        vs.append(v_dev[pages].cpu().numpy())
+        t = np.full(width, pkv_inputs.PAD_PAGE, dtype=np.int32)
+        t[:npg] = np.arange(base, base + npg, dtype=np.int32)
+        tables.append(t)
+        base += npg
+    return np.concatenate(ks), np.concatenate(vs), np.stack(tables)
+
+
+@pytest.mark.parametrize("name", ["config2", "config3", "config4_b4", "config5"])
+def test_full_size_configs_in_the_bench_configuration(name):
+    """BASELINE.json's full sizes with the policies bench.py times (config 2: the sweep's
+    FIXED_COUNT S=16 and BALANCED; others: BALANCED, page-granular tiles), seeded device pools as in
+    bench.py.  Rows are checked one by one against the oracle on a host copy of their pages (all
+    rows up to B = 8; config 5: the shortest, the longest and two more of the 128); the task list of
+    the whole batch is bit-exact; token coverage at full size is pinned by lse = log-sum-exp."""
+    import pkv_inputs as pi
+    from oracle import pkv_oracle
+    w = {"config2": pi.config2, "config3": pi.config3, "config4_b4": pi.config4_b4, "config5": pi.config5}[name](pi.REPORT_SEEDS[0])
+    dev = torch.device("cuda", 0)
+    q = pi.fill_pool_torch((w.B, w.Hq, w.d), 11, dev)
+    k = pi.fill_pool_torch(w.pool_shape(), 12, dev)
+    v = pi.fill_pool_torch(w.pool_shape(), 13, dev)
+    bt = torch.from_numpy(w.block_table).to(dev)
+    lens = w.seq_lens_at(min(w.steps, 7)).astype(np.int32)
+    sl = torch.from_numpy(lens).to(dev)
+    shape = pkv.Shape(B=w.B, Hq=w.Hq, Hkv=w.Hkv, max_pages=w.max_pages, num_pages=w.num_pages)
+    pols = [pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0)]
+    if name == "config2":
+        pols.append(pkv.Policy(tile_tokens=32, num_splits=16))
+    if w.B <= 8:
+        rows = list(range(w.B))
+    else:
+        rows = sorted({int(np.argmin(lens)), int(np.argmax(lens)), 5, 77})
+    kc, vc, tc = _compact_rows(w, k, v, rows, lens)
+    scale = default_scale(w.d)
+    ref, ref_lse = pkv_oracle.attention(np.ascontiguousarray(q.cpu().numpy()[rows]), kc, vc, tc,
+                                        np.ascontiguousarray(lens[rows]), Hkv=w.Hkv, page_size=w.page_size, scale=scale)
+    for pol in pols:
+        out = torch.full((w.B, w.Hq, w.d), float("nan"), dtype=torch.float16, device=dev)
+        lse = torch.full((w.B, w.Hq), float("nan"), dtype=torch.float32, device=dev)
+        ws = pkv.alloc_workspace(shape, pol)
+        pkv.pkv_decode(shape, pol, q, k, v, bt, sl, out, lse, scale=scale, workspace=ws)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy().astype(np.float64)
+        assert not np.isnan(got).any()
+        assert_within_tolerance(got[rows], ref, "%s %s" % (name, pol))
+        assert np.abs(lse.cpu().numpy().astype(np.float64)[rows] - ref_lse).max() <= 2e-3
+        want = wq.build_workqueue([int(x) for x in lens], w.Hkv, oracle_policy(pol))
+        tasks, offs = pkv.pkv_read_workqueue(shape, pol, ws)
+        assert np.array_equal(tasks, np.array(want.tasks, dtype=np.int32).reshape(-1, 5))
+        assert np.array_equal(offs, np.array(want.split_offsets, dtype=np.int32))
