@@ -168,6 +168,10 @@ PKV_API pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_p
  * derives the queue from seq_lens itself ("fused build": no builder launch; the queue is still
  * written to the workspace, bit-identical to pkv_build_workqueue's).  The merge launch is skipped
  * when the policy cannot produce more than one split per row, or merge_mode is FUSED.
+ * Results are bitwise reproducible from launch to launch for the same inputs, policy and device.
+ * Heads per CTA: the TMA kernel streams HG = 8, 4, 2 or 1 KV heads per CTA, the largest value
+ * that still leaves one work unit per SM given the bound B*S on the (row, split) pairs; with
+ * BALANCED the bound is policy.num_sms, so num_sms = SMs*HG/Hkv asks for HG heads per CTA.
  */
 PKV_API pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
                               const void* k_cache, const void* v_cache, const int32_t* block_table,
