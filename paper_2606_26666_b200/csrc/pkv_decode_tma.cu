@@ -7,7 +7,8 @@
 // is ONE contiguous 32 KiB TMA box in the default [page, token, head, d] layout.
 //
 //   producer warps (NP)  producer 0 takes units (first by block index, then from an atomic
-//                        counter), resolves (row, split) and publishes the unit on a small
+//                        counter when every head has one compute warp, else round-robin: see
+//                        pkv_api.cu), resolves (row, split) and publishes the unit on a small
 //                        ring.  Every producer walks its share of the unit's slice of the
 //                        block table (PAPER.md:50 page accessor), 32 entries per load, and per
 //                        page issues one TMA box for K and one for V -- 16 tokens x HG heads x
@@ -23,9 +24,16 @@
 //                         on the N = 8 axis, so G = 8 fills the tile and G = 4
 //                        half of it; K is read with ldmatrix, V with ldmatrix.trans, P^T is
 //                        made from the S^T accumulator layout with movmatrix.
-//   unit end             the warps of a head combine their states through shared memory and
-//                        store the task's partial state, or the FP16 output directly when the
-//                        row has a single split (pkv_device.cuh finalize_task).
+//   unit end             with one warp per head the state goes from the MMA accumulators straight
+//                        to the task's partial-state slot (or, for a row with a single split, to
+//                        `out`); several warps per head combine through shared memory first
+//                        (pkv_device.cuh finalize_task).
+//   planner warp (1)     derives the queue from seq_lens inside the kernel (split-bound policy,
+//                        PAPER.md:63-75): one load round trip + warp scans, hands the plan and
+//                        this CTA's first unit to producer 0, then writes the CTA's share of the
+//                        bit-exact queue off everybody's critical path.
+// K/V loads carry an L2 evict_first policy: the stream is read once per step, the step's small
+// re-read data (seq_lens, block table, q, partial states) stays in L2.
 #include <cuda.h>
 
 #include "pkv_device.cuh"
