@@ -28,10 +28,11 @@
 //                        to the task's partial-state slot (or, for a row with a single split, to
 //                        `out`); several warps per head combine through shared memory first
 //                        (pkv_device.cuh finalize_task).
-//   planner warp (1)     derives the queue from seq_lens inside the kernel (split-bound policy,
-//                        PAPER.md:63-75): one load round trip + warp scans, hands the plan and
-//                        this CTA's first unit to producer 0, then writes the CTA's share of the
-//                        bit-exact queue off everybody's critical path.
+//   fused build          producer 0 derives the plan from seq_lens inside the kernel (split-bound
+//                        policy: one load round trip + warp scans) together with
+//                        this CTA's first unit; the planner warp (1) takes the plan from shared
+//                        memory and writes the CTA's share of the bit-exact queue off everybody's
+//                        critical path.
 // K/V loads carry an L2 evict_first policy: the stream is read once per step, the step's small
 // re-read data (seq_lens, block table, q, partial states) stays in L2.
 #include <cuda.h>
@@ -132,20 +133,18 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     PlanArgs plan = p.plan;   // BALANCED: the planner resolves the batch-wide chunk
     if (warp == kPlanWarp) {
         // ================================================================ planner warp
-        // Fused build: one warp of every CTA derives split_offsets from
-        // seq_lens (one load round trip + warp scans), hands the plan to producer 0 through shared
-        // memory, and then -- off everybody's critical path -- writes this CTA's share of the
-        // queue (RowSlots, task list, split_offsets, header) that the merge kernel and
-        // pkv_read_workqueue read, and the outputs of rows without a task.
+        // Fused build: producer 0 derives split_offsets from seq_lens
+        // (one load round trip + warp scans) and leaves the plan in shared memory; this warp --
+        // off everybody's critical path -- writes this CTA's share of the queue (RowSlots, task
+        // list, split_offsets, header) that the merge kernel and pkv_read_workqueue read, and
+        // the outputs of rows without a task.
         if (p.fused_build) {
-            const int32_t row_slots = plan_warp_prefix(plan, p.seq_lens, tail.so_s, tail.len_s, lane,
-                                                       (int)blockIdx.x / HGn, &tail.first_slot);
-            if (lane == 0) {
-                tail.plan_row_slots = row_slots;
-                tail.plan_chunk = plan.chunk_tiles;
-                trace_stamp(p, 8);
+            named_bar_sync(kPlanBar, 64);   // producer 0 has planned (it arrives without waiting)
+            const int32_t row_slots = tail.plan_row_slots;
+            if (plan.split_mode == PKV_SPLIT_BALANCED) {
+                plan.split_mode = PKV_SPLIT_FIXED_CHUNK;
+                plan.chunk_tiles = tail.plan_chunk;
             }
-            named_bar_sync(kPlanBar, 64);   // plan ready -> producer 0
             const PlanTotals tot = plan_warp_totals(plan, tail.len_s, row_slots, lane);
             for (int rs = blockIdx.x * 32 + lane; rs < tot.row_slots; rs += gridDim.x * 32) {
                 int32_t tb, te;
@@ -178,12 +177,18 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         return;
     }
     if (p.fused_build && warp == 0) {
-        named_bar_sync(kPlanBar, 64);
-        num_units = tail.plan_row_slots * HGn;
-        if (plan.split_mode == PKV_SPLIT_BALANCED) {
-            plan.split_mode = PKV_SPLIT_FIXED_CHUNK;
-            plan.chunk_tiles = tail.plan_chunk;
+        // Producer 0 plans for itself -- the plan is on the critical path of the first TMA load --
+        // and leaves it in shared memory for the planner warp, which writes the queue.
+        const int32_t row_slots = plan_warp_prefix(plan, p.seq_lens, tail.so_s, tail.len_s, lane,
+                                                   (int)blockIdx.x / HGn, &tail.first_slot);
+        if (lane == 0) {
+            tail.plan_row_slots = row_slots;
+            tail.plan_chunk = plan.chunk_tiles;
+            trace_stamp(p, 8);
         }
+        __syncwarp();
+        named_bar_arrive(kPlanBar, 64);
+        num_units = row_slots * HGn;
     }
 
     // ---- unit hand-out (producer 0) / pick-up (everybody else) -------------------------------
