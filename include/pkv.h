@@ -228,7 +228,8 @@ PKV_API pkv_status pkv_workspace_partials(const pkv_shape* shape, const pkv_spli
  *      `host_staging` and copies that image to `dev_scratch` with ONE cudaMemcpyAsync,
  *   3. launches decode (+ merge) -- skipping launches the plan shows to be empty, so
  *      decode/merge launch counts equal the oracle's (A13) -- and
- *   4. copies out to out_host and SYNCHRONISES the stream.
+ *   4. gets out to out_host -- the kernels write it there directly when out_host is pinned,
+ *      device-mapped memory (zero copy), else one cudaMemcpyAsync -- and SYNCHRONISES the stream.
  * host_staging: host memory of pkv_host_scratch_bytes() bytes (pinned recommended);
  * dev_scratch: device memory of the same size, 256-byte aligned.  counters_out may be NULL.
  */

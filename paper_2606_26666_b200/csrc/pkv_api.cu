@@ -556,13 +556,28 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     qp.rowslots = reinterpret_cast<RowSlot*>(ds + im.rowslots);
     qp.tasks = reinterpret_cast<pkv_task*>(ds + im.tasks);
     int dl = 0, ml = 0;
+    // Pinned (page-locked, device-mapped) out_host: the kernels write the FP16 result straight
+    // into it -- 8 KiB of posted writes per row -- and the D2H copy disappears from the step.
+    // Pageable out_host: result in dev_scratch, then one cudaMemcpyAsync.
+    void* out_dev = ds + im.out;
+    bool zero_copy_out = false;
+    {
+        cudaPointerAttributes attr;
+        if (cudaPointerGetAttributes(&attr, out_host) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
+            attr.devicePointer != nullptr && reinterpret_cast<uintptr_t>(attr.devicePointer) % 16 == 0) {
+            out_dev = attr.devicePointer;
+            zero_copy_out = true;
+        } else {
+            (void)cudaGetLastError();   // an unregistered host pointer is not an error here
+        }
+    }
     st = run_decode(s, rp, ds + im.q, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
-                    reinterpret_cast<const int32_t*>(ds + im.seq_lens), ds + im.out, nullptr, scale, qp, ws,
+                    reinterpret_cast<const int32_t*>(ds + im.seq_lens), out_dev, nullptr, scale, qp, ws,
                     hdr->num_tasks, hdr->max_row_splits, hdr->total_row_slots, sms, PKV_STAGE_ALL, false, L.slots_cap, cs, &dl,
                     &ml);
     if (st != PKV_OK) return st;
     const size_t out_bytes = 2 * (size_t)s.B * s.Hq * s.d;
-    e = cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);
+    e = zero_copy_out ? cudaSuccess : cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);
     if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     if (e != cudaSuccess) return cuda_fail(e, "D2H out / sync");
     if (counters_out) {

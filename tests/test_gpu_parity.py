@@ -303,6 +303,11 @@ def test_decode_host_entry_point():
         assert c["tasks"] == q.num_tasks
         assert c["decode_launches"] == q.decode_launches and c["merge_launches"] == q.merge_launches
         assert c["d2h_bytes"] == out.nbytes and c["h2d_bytes"] > p.q.nbytes
+        # pinned out_host: the kernels write the result straight into host memory (zero copy)
+        out_pin = torch.full((p.B, p.Hq, p.d), float("nan"), dtype=torch.float16).pin_memory()
+        pkv.pkv_decode_host(dp.shape, pol, p.q, dp.k, dp.v, p.block_table, p.seq_lens, out_pin.data_ptr(), p.scale,
+                            staging, scratch, ws)
+        assert np.array_equal(out_pin.numpy(), out)
     # every row empty: no launch at all, out = 0
     p0 = make_problem([0, 0], seed=92)
     dp0 = DevProblem(p0)
