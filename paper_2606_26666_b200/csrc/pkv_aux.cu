@@ -57,14 +57,15 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
     }
 }
 
-// One CTA of kMergeWarps warps per (row, query head).  Warp w owns the states w, w + NW, ...
+// One CTA of NW warps per (row, query head).  Warp w owns the states w, w + NW, ...
 // of the (row, kvh) slot range; it issues the loads of kMergeBatch of them (m, l and one 16-byte
 // piece of acc per lane) before any arithmetic, so a row of up to NW * kMergeBatch = 128 splits
 // is ONE round trip to L2/HBM, and folds them into an online state (M_w, L_w, A_w) -- the merge
 // of PAPER.md:60-61 is associative, so the per-warp states combine exactly the same way.  Warp 0
 // combines the NW warp states in fixed order (deterministic).  Rows with at most one slot were
-// written directly by the decode kernel.
-constexpr int kMergeWarps = 16;
+// written directly by the decode kernel.  NW = 16 for small batches (few CTAs, long rows: 128
+// splits per round trip), NW = 4 for large ones (thousands of (row, head) pairs of a few dozen
+// splits each: 16-warp CTAs are mostly idle there and only one of them fits on an SM).
 // debug trace (pkv_debug_set_trace): merge CTAs stamp behind the decode kernel's [148][16] block
 __device__ __forceinline__ void merge_trace_stamp(const DecodeParams& p, int slot) {
     if (p.trace && blockIdx.x < 4096) {
@@ -73,9 +74,9 @@ __device__ __forceinline__ void merge_trace_stamp(const DecodeParams& p, int slo
         p.trace[148 * 16 + (size_t)blockIdx.x * 4 + slot] = t;
     }
 }
-template <int G>
-__global__ void __launch_bounds__(kMergeWarps * 32) pkv_merge_kernel(const DecodeParams p) {
-    constexpr int NW = kMergeWarps, NB = kMergeBatch;
+template <int G, int NW>
+__global__ void __launch_bounds__(NW * 32) pkv_merge_kernel(const DecodeParams p) {
+    constexpr int NB = kMergeBatch;
     __shared__ float4 sA[NW][32];
     __shared__ float sM[NW], sL[NW];
     const int row = blockIdx.x / p.Hq, h = blockIdx.x % p.Hq;
@@ -170,8 +171,11 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     const int grid = p.B * p.Hq;
     if (grid <= 0) return cudaSuccess;
-    if (G == 4) return launch_pdl(pkv_merge_kernel<4>, dim3(grid), dim3(kMergeWarps * 32), 0, stream, p);
-    return launch_pdl(pkv_merge_kernel<8>, dim3(grid), dim3(kMergeWarps * 32), 0, stream, p);
+    const bool big = grid > 1024;
+    if (G == 4) return big ? launch_pdl(pkv_merge_kernel<4, 4>, dim3(grid), dim3(128), 0, stream, p)
+                           : launch_pdl(pkv_merge_kernel<4, 16>, dim3(grid), dim3(512), 0, stream, p);
+    return big ? launch_pdl(pkv_merge_kernel<8, 4>, dim3(grid), dim3(128), 0, stream, p)
+               : launch_pdl(pkv_merge_kernel<8, 16>, dim3(grid), dim3(512), 0, stream, p);
 }
 
 }  // namespace pkv
