@@ -64,8 +64,9 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
 // of PAPER.md:60-61 is associative, so the per-warp states combine exactly the same way.  Warp 0
 // combines the NW warp states in fixed order (deterministic).  Rows with at most one slot were
 // written directly by the decode kernel.  NW = 16 for small batches (few CTAs, long rows: 128
-// splits per round trip), NW = 4 for large ones (thousands of (row, head) pairs of a few dozen
-// splits each: 16-warp CTAs are mostly idle there and only one of them fits on an SM).
+// splits per round trip; with more (row, head) pairs than SMs the registers are capped so that
+// two CTAs share an SM), NW = 4 for large ones (thousands of pairs of a few dozen splits each:
+// 16-warp CTAs are mostly idle there and only one or two of them fit on an SM).
 // debug trace (pkv_debug_set_trace): merge CTAs stamp behind the decode kernel's [148][16] block
 __device__ __forceinline__ void merge_trace_stamp(const DecodeParams& p, int slot) {
     if (p.trace && blockIdx.x < 4096) {
@@ -74,8 +75,8 @@ __device__ __forceinline__ void merge_trace_stamp(const DecodeParams& p, int slo
         p.trace[148 * 16 + (size_t)blockIdx.x * 4 + slot] = t;
     }
 }
-template <int G, int NW>
-__global__ void __launch_bounds__(NW * 32) pkv_merge_kernel(const DecodeParams p) {
+template <int G, int NW, int MINB>
+__global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodeParams p) {
     constexpr int NB = kMergeBatch;
     __shared__ float4 sA[NW][32];
     __shared__ float sM[NW], sL[NW];
@@ -171,11 +172,15 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     const int grid = p.B * p.Hq;
     if (grid <= 0) return cudaSuccess;
-    const bool big = grid > 1024;
-    if (G == 4) return big ? launch_pdl(pkv_merge_kernel<4, 4>, dim3(grid), dim3(128), 0, stream, p)
-                           : launch_pdl(pkv_merge_kernel<4, 16>, dim3(grid), dim3(512), 0, stream, p);
-    return big ? launch_pdl(pkv_merge_kernel<8, 4>, dim3(grid), dim3(128), 0, stream, p)
-               : launch_pdl(pkv_merge_kernel<8, 16>, dim3(grid), dim3(512), 0, stream, p);
+    // up to one CTA per SM: 16 warps, all the registers they like; up to 1024 (row, head) pairs:
+    // 16 warps, two CTAs per SM (one wave at B = 8); beyond: 4 warps, six CTAs per SM
+    const int v = grid <= 148 ? 0 : (grid <= 1024 ? 1 : 2);
+#define PKV_MERGE_CASE(GG, VV, NWW, MB) \
+    if (G == GG && v == VV) return launch_pdl(pkv_merge_kernel<GG, NWW, MB>, dim3(grid), dim3(NWW * 32), 0, stream, p);
+    PKV_MERGE_CASE(4, 0, 16, 1) PKV_MERGE_CASE(4, 1, 16, 2) PKV_MERGE_CASE(4, 2, 4, 6)
+    PKV_MERGE_CASE(8, 0, 16, 1) PKV_MERGE_CASE(8, 1, 16, 2) PKV_MERGE_CASE(8, 2, 4, 6)
+#undef PKV_MERGE_CASE
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace pkv
