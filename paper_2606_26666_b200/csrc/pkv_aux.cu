@@ -63,10 +63,7 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
 // is ONE round trip to L2/HBM, and folds them into an online state (M_w, L_w, A_w) -- the merge
 // of PAPER.md:60-61 is associative, so the per-warp states combine exactly the same way.  Warp 0
 // combines the NW warp states in fixed order (deterministic).  Rows with at most one slot were
-// written directly by the decode kernel.  NW = 16 for small batches (few CTAs, long rows: 128
-// splits per round trip; with more (row, head) pairs than SMs the registers are capped so that
-// two CTAs share an SM), NW = 4 for large ones (thousands of pairs of a few dozen splits each:
-// 16-warp CTAs are mostly idle there and only one or two of them fit on an SM).
+// written directly by the decode kernel.  NW = 2 .. 16 is chosen at launch (launch_merge).
 // debug trace (pkv_debug_set_trace): merge CTAs stamp behind the decode kernel's [148][16] block
 __device__ __forceinline__ void merge_trace_stamp(const DecodeParams& p, int slot) {
     if (p.trace && blockIdx.x < 4096) {
@@ -172,13 +169,21 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     const int grid = p.B * p.Hq;
     if (grid <= 0) return cudaSuccess;
-    // up to one CTA per SM: 16 warps, all the registers they like; up to 1024 (row, head) pairs:
-    // 16 warps, two CTAs per SM (one wave at B = 8); beyond: 4 warps, six CTAs per SM
-    const int v = grid <= 148 ? 0 : (grid <= 1024 ? 1 : 2);
-#define PKV_MERGE_CASE(GG, VV, NWW, MB) \
-    if (G == GG && v == VV) return launch_pdl(pkv_merge_kernel<GG, NWW, MB>, dim3(grid), dim3(NWW * 32), 0, stream, p);
-    PKV_MERGE_CASE(4, 0, 16, 1) PKV_MERGE_CASE(4, 1, 16, 2) PKV_MERGE_CASE(4, 2, 4, 6)
-    PKV_MERGE_CASE(8, 0, 16, 1) PKV_MERGE_CASE(8, 1, 16, 2) PKV_MERGE_CASE(8, 2, 4, 6)
+    // Warps per CTA.  A warp covers 8 splits per round trip, and small CTAs start (and finish)
+    // sooner, so: as few warps as cover the row's splits in one round when the split count is
+    // known on the host (FIXED_COUNT: at most S; measured on config 2, S = 16: 2 warps 25.9 us per
+    // step, 4 warps 26.0, 16 warps 26.9); else by batch size -- 16 warps while there is at most
+    // one (row, head) pair per SM (a single long row can hold ~148 splits), 8 warps up to 1024
+    // pairs (49.6 vs 50.7 us on config 3), 4 warps, six CTAs per SM, beyond (config 5).
+    int nw;
+    if (p.plan.split_mode == PKV_SPLIT_FIXED_COUNT && p.plan.S > 0)
+        nw = p.plan.S <= 16 ? 2 : (p.plan.S <= 32 ? 4 : (p.plan.S <= 64 ? 8 : 16));
+    else
+        nw = grid <= 148 ? 16 : (grid <= 1024 ? 8 : 4);
+#define PKV_MERGE_CASE(GG, NWW, MB) \
+    if (G == GG && nw == NWW) return launch_pdl(pkv_merge_kernel<GG, NWW, MB>, dim3(grid), dim3(NWW * 32), 0, stream, p);
+    PKV_MERGE_CASE(4, 2, 1) PKV_MERGE_CASE(4, 4, 6) PKV_MERGE_CASE(4, 8, 1) PKV_MERGE_CASE(4, 16, 1)
+    PKV_MERGE_CASE(8, 2, 1) PKV_MERGE_CASE(8, 4, 6) PKV_MERGE_CASE(8, 8, 1) PKV_MERGE_CASE(8, 16, 1)
 #undef PKV_MERGE_CASE
     return cudaErrorInvalidValue;
 }
