@@ -51,6 +51,7 @@ def parse_args():
     ap.add_argument("--workload", default="config2",
                     choices=["config1", "config2", "config3", "config4", "config4_b4", "config5", "config5_hkv4"])
     ap.add_argument("--seed", type=int, default=pkv_inputs.REPORT_SEEDS[0])
+    ap.add_argument("--hkv", type=int, default=0, help="config3 only: KV heads (GQA sweep, G = 32 / hkv in {1, 2, 4, 8})")
     ap.add_argument("--rotate", type=int, default=0, help="rotating KV pools (0 = enough to exceed L2 4x)")
     ap.add_argument("--tile-tokens", type=int, default=0)
     ap.add_argument("--split-mode", type=int, default=-1)
@@ -70,13 +71,13 @@ def parse_args():
 
 # ------------------------------------------------------------------ workload
 
-def make_workload(name: str, seed: int):
+def make_workload(name: str, seed: int, hkv: int = 0):
     if name == "config1":
         return pkv_inputs.config1(seed)
     if name == "config2":
         return pkv_inputs.config2(seed)
     if name == "config3":
-        return pkv_inputs.config3(seed)
+        return pkv_inputs.config3(seed, Hkv=hkv) if hkv else pkv_inputs.config3(seed)
     if name == "config4":
         return pkv_inputs.config4(seed)
     if name == "config4_b4":
@@ -328,7 +329,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    w = make_workload(args.workload, args.seed)
+    w = make_workload(args.workload, args.seed, args.hkv)
     scale = float(np.float32(1.0 / math.sqrt(w.d)))
     lens = w.seq_lens_at(0)
     # budget: the whole run (K + W steps) within about two minutes
@@ -497,7 +498,7 @@ def run_ours(args):
 
     # every rank is a replica with its own seeded trace (data-parallel by row; DESIGN.md multi-GPU)
     seed = multirank.rank_seed(args.seed, rank)
-    w = make_workload(args.workload, seed)
+    w = make_workload(args.workload, seed, args.hkv)
     pol = default_policy(pkv, args.workload, args)
     peak, peak_src = measured_hbm_peak()
 

@@ -23,7 +23,7 @@
  *     (seq_lens[i] > max_pages*page_size, a page id >= num_pages) cannot be checked without a
  *     synchronisation: they are undefined behaviour.  seq_lens[i] == 0 is legal: the row
  *     emits no task, out[i] = 0 and lse[i] = -inf (reading A9).
- *   - compiled-in shapes: d = 128, page_size = 16, FP16, G = Hq/Hkv in {4, 8}.  Anything else
+ *   - compiled-in shapes: d = 128, page_size = 16, FP16, G = Hq/Hkv in {1, 2, 4, 8}.  Anything else
  *     returns PKV_ERR_UNSUPPORTED.
  */
 #ifndef PKV_H_

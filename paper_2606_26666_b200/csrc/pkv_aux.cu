@@ -184,6 +184,8 @@ cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     if (G == GG && nw == NWW) return launch_pdl(pkv_merge_kernel<GG, NWW, MB>, dim3(grid), dim3(NWW * 32), 0, stream, p);
     PKV_MERGE_CASE(4, 2, 1) PKV_MERGE_CASE(4, 4, 6) PKV_MERGE_CASE(4, 8, 1) PKV_MERGE_CASE(4, 16, 1)
     PKV_MERGE_CASE(8, 2, 1) PKV_MERGE_CASE(8, 4, 6) PKV_MERGE_CASE(8, 8, 1) PKV_MERGE_CASE(8, 16, 1)
+    PKV_MERGE_CASE(2, 2, 1) PKV_MERGE_CASE(2, 4, 6) PKV_MERGE_CASE(2, 8, 1) PKV_MERGE_CASE(2, 16, 1)
+    PKV_MERGE_CASE(1, 2, 1) PKV_MERGE_CASE(1, 4, 6) PKV_MERGE_CASE(1, 8, 1) PKV_MERGE_CASE(1, 16, 1)
 #undef PKV_MERGE_CASE
     return cudaErrorInvalidValue;
 }

@@ -457,21 +457,24 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 // to the task's slot (or to `out`), no shared-memory round trip.  Per store
                 // instruction the 8 lanes of a column write 32 contiguous bytes.
                 if (hA < G) {
+                    const bool hasB = hB < G;   // G = 1: column B is padding
                     const int64_t hrow = (int64_t)row * p.Hq + kvh * G + hA;
                     if (n_i <= 1) {
-                        const float iA = 1.0f / lA, iB = 1.0f / lB;
+                        const float iA = 1.0f / lA, iB = hasB ? 1.0f / lB : 0.f;
                         __half* oA = p.out + hrow * kD + g4;
                         __half* oB = oA + kD;
 #pragma unroll
                         for (int mt = 0; mt < 8; ++mt) {
                             oA[mt * 16] = __float2half_rn(o[mt][0] * iA);
-                            oB[mt * 16] = __float2half_rn(o[mt][1] * iB);
                             oA[mt * 16 + 8] = __float2half_rn(o[mt][2] * iA);
-                            oB[mt * 16 + 8] = __float2half_rn(o[mt][3] * iB);
+                            if (hasB) {
+                                oB[mt * 16] = __float2half_rn(o[mt][1] * iB);
+                                oB[mt * 16 + 8] = __float2half_rn(o[mt][3] * iB);
+                            }
                         }
                         if (p.lse && g4 == 0) {
                             p.lse[hrow] = mA * p.scale + logf(lA);
-                            p.lse[hrow + 1] = mB * p.scale + logf(lB);
+                            if (hasB) p.lse[hrow + 1] = mB * p.scale + logf(lB);
                         }
                     } else {
                         float* aA = p.part_acc + (slot * G + hA) * kD + g4;
@@ -479,15 +482,19 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
 #pragma unroll
                         for (int mt = 0; mt < 8; ++mt) {
                             aA[mt * 16] = o[mt][0];
-                            aB[mt * 16] = o[mt][1];
                             aA[mt * 16 + 8] = o[mt][2];
-                            aB[mt * 16 + 8] = o[mt][3];
+                            if (hasB) {
+                                aB[mt * 16] = o[mt][1];
+                                aB[mt * 16 + 8] = o[mt][3];
+                            }
                         }
                         if (g4 == 0) {
                             p.part_m[slot * G + hA] = mA * p.scale;
-                            p.part_m[slot * G + hB] = mB * p.scale;
                             p.part_l[slot * G + hA] = lA;
-                            p.part_l[slot * G + hB] = lB;
+                            if (hasB) {
+                                p.part_m[slot * G + hB] = mB * p.scale;
+                                p.part_l[slot * G + hB] = lB;
+                            }
                         }
                     }
                 }
@@ -495,16 +502,19 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     fused_complete<G, 1>(p, &tail.cb.flag[cw], row, kvh, split, n_i, slot, lane, 1 + hl);
             } else {
                 if (hA < G) {
+                    const bool hasB = hB < G;   // G = 1: column B is padding
 #pragma unroll
                     for (int mt = 0; mt < 8; ++mt) {
                         tail.cb.acc[cw][hA][mt * 16 + g4] = o[mt][0];
-                        tail.cb.acc[cw][hB][mt * 16 + g4] = o[mt][1];
                         tail.cb.acc[cw][hA][mt * 16 + g4 + 8] = o[mt][2];
-                        tail.cb.acc[cw][hB][mt * 16 + g4 + 8] = o[mt][3];
+                        if (hasB) {
+                            tail.cb.acc[cw][hB][mt * 16 + g4] = o[mt][1];
+                            tail.cb.acc[cw][hB][mt * 16 + g4 + 8] = o[mt][3];
+                        }
                     }
                     if (g4 == 0) {
-                        tail.cb.m[cw][hA] = mA; tail.cb.m[cw][hB] = mB;
-                        tail.cb.l[cw][hA] = lA; tail.cb.l[cw][hB] = lB;
+                        tail.cb.m[cw][hA] = mA; tail.cb.l[cw][hA] = lA;
+                        if (hasB) { tail.cb.m[cw][hB] = mB; tail.cb.l[cw][hB] = lB; }
                     }
                 }
                 group_sync<WPH>(1 + hl);
@@ -532,7 +542,8 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
 }  // namespace
 
 int decode_tma_smem_bytes(int G, int HG) {
-    const int tail = G == 4 ? (int)sizeof(SmemTail<4>) : (int)sizeof(SmemTail<8>);
+    const int tail = G == 1 ? (int)sizeof(SmemTail<1>) : G == 2 ? (int)sizeof(SmemTail<2>)
+                   : G == 4 ? (int)sizeof(SmemTail<4>) : (int)sizeof(SmemTail<8>);
     int st = (232448 - 1024 - tail) / (HG * 8192);
     if (st > kMaxStages) st = kMaxStages;
     return st * HG * 8192 + tail + 1024;
@@ -547,6 +558,8 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int grid, co
     if (G == GG && HG == HH) return launch_one<GG, HH>(p, grid, mk, mv, stream);
     PKV_CASE(4, 8) PKV_CASE(4, 4) PKV_CASE(4, 2) PKV_CASE(4, 1)
     PKV_CASE(8, 8) PKV_CASE(8, 4) PKV_CASE(8, 2) PKV_CASE(8, 1)
+    PKV_CASE(2, 8) PKV_CASE(2, 4) PKV_CASE(2, 2) PKV_CASE(2, 1)
+    PKV_CASE(1, 8) PKV_CASE(1, 4) PKV_CASE(1, 2) PKV_CASE(1, 1)
 #undef PKV_CASE
     return cudaErrorInvalidValue;
 }

@@ -135,12 +135,13 @@ def config2(seed: int = TUNE_SEED, seq_len: int = 32768) -> Workload:
     return make_workload("config2_b1_n%d" % seq_len, [seq_len], steps=0, hole_frac=0.5, seed=seed)
 
 
-def config3(seed: int = TUNE_SEED, B: int = 8, steps: int = 50) -> Workload:
+def config3(seed: int = TUNE_SEED, B: int = 8, steps: int = 50, Hkv: int = 8) -> Workload:
     """B=8 bimodal ragged trace, 50 decode steps (+1 token per step), rho=0.5.
     Lengths are drawn once at step 0 and then grow (reading A17)."""
     rng = _rng(seed)
     lens = bimodal_lengths(rng, B)
-    return make_workload("config3_b%d_bimodal" % B, lens, steps=steps, hole_frac=0.5, seed=seed, rng=rng)
+    name = "config3_b%d_bimodal" % B + ("" if Hkv == 8 else "_hkv%d" % Hkv)
+    return make_workload(name, lens, steps=steps, hole_frac=0.5, seed=seed, rng=rng, Hkv=Hkv)
 
 
 def config4(seed: int = TUNE_SEED, B: int = 8, steps: int = 50) -> Workload:

@@ -48,11 +48,12 @@ def test_config1(kernel):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-@pytest.mark.parametrize("Hkv", [8, 4])
+@pytest.mark.parametrize("Hkv", [8, 4, 16, 32])
 @pytest.mark.parametrize("route", [pkv.ROUTE_WORKQUEUE, pkv.ROUTE_RECT])
 def test_ragged_split_sweep(kernel, Hkv, route):
     """Ragged rows spanning several tiles and a ragged tail, every split count incl. S > T
-    (neutral states), separate and fused merge."""
+    (neutral states), separate and fused merge; G = Hq/Hkv = 4, 8, 2, 1
+    (the paper's GQA sweep)."""
     p = make_problem(RAGGED, seed=100 + Hkv, Hkv=Hkv)
     dp = DevProblem(p)
     ref = oracle_attention(p)
@@ -66,7 +67,7 @@ def test_ragged_split_sweep(kernel, Hkv, route):
 
 
 @pytest.mark.parametrize("hg", [1, 2, 4, 8])
-@pytest.mark.parametrize("Hkv", [8, 4])
+@pytest.mark.parametrize("Hkv", [8, 4, 16, 32])
 def test_tma_heads_per_cta_variants(hg, Hkv):
     if hg > Hkv:
         pytest.skip("hg > Hkv")
