@@ -9,6 +9,7 @@ namespace pkv {
 namespace {
 
 constexpr int kBuildThreadsMax = 1024;
+constexpr int kBuildWarpPlanRows = 512;   // up to this many rows the builder uses the decode kernel's warp planner
 
 struct BuildArgs {
     const int32_t* seq_lens;
@@ -25,18 +26,45 @@ struct BuildArgs {
 // per (row, split) pair writes the pair's RowSlot and its Hkv task entries (pkv_device.cuh).
 __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(const BuildArgs a) {
     __shared__ PlanScratch sc;
+    __shared__ int32_t so_s[kBuildWarpPlanRows + 1], len_s[kBuildWarpPlanRows];
+    __shared__ RowSlot unused_first;
+    __shared__ PlanTotals tot_s;
+    __shared__ int32_t chunk_s;
     const int tid = threadIdx.x, nthreads = blockDim.x;
     pdl_launch_dependents();
     pdl_wait();   // the queue may still be read by the previous step's kernels
-    PlanArgs plan = a.plan;   // BALANCED: plan_scan resolves the batch-wide chunk into this copy
-    const PlanTotals tot = plan_scan(plan, a.seq_lens, a.split_offsets, nullptr, sc);
+    PlanArgs plan = a.plan;   // BALANCED: the planner resolves the batch-wide chunk into this copy
+    PlanTotals tot;
+    const int32_t* so = a.split_offsets;
+    const int32_t* lens = a.seq_lens;
+    if (plan.B <= kBuildWarpPlanRows) {
+        // the decode kernel's own planner (plan_warp_prefix / plan_warp_totals): one warp plans
+        // into shared memory, everybody writes the queue -- so that this entry point and the
+        // fused build run (and the tests of either exercise) the same code
+        if (tid < 32) {
+            const int32_t rs = plan_warp_prefix(plan, a.seq_lens, so_s, len_s, tid, -1, &unused_first);
+            const PlanTotals t = plan_warp_totals(plan, len_s, rs, tid);
+            if (tid == 0) { tot_s = t; chunk_s = plan.chunk_tiles; }
+        }
+        __syncthreads();
+        tot = tot_s;
+        if (plan.split_mode == PKV_SPLIT_BALANCED) {
+            plan.split_mode = PKV_SPLIT_FIXED_CHUNK;
+            plan.chunk_tiles = chunk_s;
+        }
+        for (int i = tid; i <= plan.B; i += nthreads) a.split_offsets[i] = so_s[i];
+        so = so_s;
+        lens = len_s;
+    } else {
+        tot = plan_scan(plan, a.seq_lens, a.split_offsets, nullptr, sc);
+    }
     for (int i = tid; i < a.plan.B * a.plan.Hkv; i += nthreads) a.fuse_counters[i] = 0;
     __threadfence_block();
     __syncthreads();
     const int64_t total = (int64_t)tot.row_slots * a.plan.Hkv;
     for (int32_t rs = tid; rs < tot.row_slots; rs += nthreads) {
         int32_t tb, te;
-        const RowSlot d = make_rowslot(plan, a.split_offsets, a.seq_lens, rs, &tb, &te);
+        const RowSlot d = make_rowslot(plan, so, lens, rs, &tb, &te);
         write_pair(plan, d, tb, te, rs, a.rowslots, a.tasks, a.tasks_cap);
     }
     if (tid == 0) {

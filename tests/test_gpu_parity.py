@@ -88,7 +88,12 @@ def test_device_builder_bit_exact(route):
     launches and Table-4 counters."""
     rng = np.random.Generator(np.random.PCG64(77))
     cases = [[0], [1], [0, 0], RAGGED, list(rng.integers(0, 70000, size=8)), list(rng.integers(0, 9000, size=128)),
-             list(rng.integers(1, 400, size=1500))]
+             list(rng.integers(1, 400, size=1500)),
+             # very long rows and more shapes for the warp planner (B <= 512)
+             [2 ** 24 - 1, 5], [2 ** 24, 7, 100], [2 ** 24 + 17, 2 ** 20, 3], [2 ** 24 - 1] * 3 + [1],
+             list(rng.integers(0, 2 ** 22, size=16)), list(rng.integers(0, 300000, size=40)),
+             list(rng.integers(0, 5000, size=16)), list(rng.integers(1, 100, size=12)), [65536] * 8,
+             list(rng.integers(0, 2 ** 24, size=5))]
     pols = [pkv.Policy(tile_tokens=32, num_splits=20), pkv.Policy(tile_tokens=64, num_splits=0),
             pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=16),
             pkv.Policy(tile_tokens=16, num_splits=256),
