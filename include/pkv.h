@@ -250,6 +250,10 @@ PKV_API void pkv_debug_set_pdl(int on);
 /* Test hook: 0 makes pkv_decode run the builder as its own kernel even where the TMA decode kernel
  * could derive the queue itself.  Process-wide. */
 PKV_API void pkv_debug_set_fused_build(int on);
+/* Test hook: non-zero makes the TMA decode kernel discard the plan it made speculatively before its
+ * dependency wait and plan again afterwards -- the path taken when the kernel right before
+ * pkv_decode wrote seq_lens.  Process-wide. */
+PKV_API void pkv_debug_force_replan(int on);
 /* Debug hook: device buffer of grid*16 uint64 that the TMA decode kernel fills with %globaltimer
  * stamps of its phases, or NULL to switch tracing off.  Process-wide. */
 PKV_API void pkv_debug_set_trace(void* dev_u64);

@@ -54,7 +54,7 @@ class pkv_counters(ctypes.Structure):
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspace_init_bytes", "pkv_build_workqueue_host",
            "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
-           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_heads_per_cta", "pkv_debug_set_pdl", "pkv_debug_set_fused_build", "pkv_debug_set_trace")
+           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_heads_per_cta", "pkv_debug_set_pdl", "pkv_debug_set_fused_build", "pkv_debug_set_trace", "pkv_debug_force_replan")
 
 
 class PkvError(RuntimeError):
@@ -106,6 +106,8 @@ def _load() -> ctypes.CDLL:
     lib.pkv_debug_set_pdl.argtypes = [ctypes.c_int]
     lib.pkv_debug_set_fused_build.restype = None
     lib.pkv_debug_set_fused_build.argtypes = [ctypes.c_int]
+    lib.pkv_debug_force_replan.restype = None
+    lib.pkv_debug_force_replan.argtypes = [ctypes.c_int]
     lib.pkv_debug_set_trace.restype = None
     lib.pkv_debug_set_trace.argtypes = [_vp]
     return lib
@@ -298,6 +300,10 @@ def pkv_debug_force_heads_per_cta(heads: int) -> None:
 
 def pkv_debug_set_pdl(on: bool) -> None:
     _lib.pkv_debug_set_pdl(1 if on else 0)
+
+
+def pkv_debug_force_replan(on: bool) -> None:
+    _lib.pkv_debug_force_replan(1 if on else 0)
 
 
 def pkv_debug_set_trace(dev_u64) -> None:

@@ -20,6 +20,7 @@ unsigned long long* g_trace = nullptr;  // debug hook
 bool g_fused_build = true;              // test hook (pkv_debug_set_fused_build)
 constexpr int kMaxFusedRows = 512;      // = pkv_decode_tma.cu
 int g_force_hg = 0;  // test hook: 0 = automatic heads-per-CTA, else 1/2/4/8
+bool g_force_replan = false;  // test hook (pkv_debug_force_replan)
 
 int device_sm_count() {
     thread_local int cache[64];
@@ -197,6 +198,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.B = s.B; p.Hq = s.Hq; p.Hkv = s.Hkv; p.max_pages = s.max_pages;
     p.tile_tokens = rp.tile_tokens; p.merge_mode = rp.merge_mode;
     p.dynamic_sched = 1;
+    p.force_replan = g_force_replan ? 1 : 0;
     p.plan = make_plan_args(s, rp);
     p.tasks_cap = tasks_cap;
     p.fused_build = fused_build ? 1 : 0;
@@ -291,6 +293,7 @@ extern "C" {
 
 void pkv_debug_force_heads_per_cta(int hg) { g_force_hg = hg; }
 void pkv_debug_set_pdl(int on) { g_use_pdl = on != 0; }
+void pkv_debug_force_replan(int on) { g_force_replan = on != 0; }
 void pkv_debug_set_fused_build(int on) { g_fused_build = on != 0; }
 void pkv_debug_set_trace(void* dev) { g_trace = static_cast<unsigned long long*>(dev); }
 

@@ -125,12 +125,28 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         tma_prefetch_desc(&tmap_v);
     }
     __syncthreads();
-    pdl_wait();   // queue (builder), q / seq_lens (upstream), out / partials (previous step's readers)
-    if (tid == 0) trace_stamp(p, 1);
-
     const int HGn = p.Hkv / HG;                               // head groups per (row, split)
     int num_units = 0;
     PlanArgs plan = p.plan;   // BALANCED: the planner resolves the batch-wide chunk
+    // Speculative plan.  A decode CTA is usually resident a few microseconds before its dependency
+    // wait returns (programmatic launch), and the plan -- ~1 us with a fixed split count, ~2.5 us
+    // BALANCED; straight-line integer code that runs once per launch -- would otherwise sit on
+    // the critical path of the first TMA load.  Producer 0 makes it now from a race-tolerant read
+    // of seq_lens and, after the wait, only checks that the lengths are still the same (they
+    // are, unless the kernel right before this one wrote them; then it plans again).
+    PlanArgs spec_plan = plan;
+    int32_t spec_row_slots = 0;
+    if (p.fused_build && warp == 0)
+        spec_row_slots = plan_warp_prefix<true>(spec_plan, p.seq_lens, tail.so_s, tail.len_s, lane,
+                                                (int)blockIdx.x / HGn, &tail.first_slot);
+    if (p.force_replan && p.fused_build && warp == 0) {   // test hook: leave a wrong plan behind
+        for (int i = lane; i <= p.B; i += 32) tail.so_s[i] = 0x3fffffff;
+        for (int i = lane; i < p.B; i += 32) tail.len_s[i] = 1;
+        if (lane == 0) tail.first_slot.tok1 = 0;
+        __syncwarp();
+    }
+    pdl_wait();   // queue (builder), q / seq_lens (upstream), out / partials (previous step's readers)
+    if (tid == 0) trace_stamp(p, 1);
     if (warp == kPlanWarp) {
         // ================================================================ planner warp
         // Fused build: producer 0 derives split_offsets from seq_lens
@@ -179,8 +195,14 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     if (p.fused_build && warp == 0) {
         // Producer 0 plans for itself -- the plan is on the critical path of the first TMA load --
         // and leaves it in shared memory for the planner warp, which writes the queue.
-        const int32_t row_slots = plan_warp_prefix(plan, p.seq_lens, tail.so_s, tail.len_s, lane,
-                                                   (int)blockIdx.x / HGn, &tail.first_slot);
+        int32_t row_slots = spec_row_slots;
+        if (!p.force_replan && plan_lens_unchanged(plan, p.seq_lens, tail.len_s, lane)) {
+            plan = spec_plan;
+        } else {
+            __syncwarp();
+            row_slots = plan_warp_prefix(plan, p.seq_lens, tail.so_s, tail.len_s, lane, (int)blockIdx.x / HGn,
+                                         &tail.first_slot);
+        }
         if (lane == 0) {
             tail.plan_row_slots = row_slots;
             tail.plan_chunk = plan.chunk_tiles;

@@ -42,6 +42,7 @@ struct DecodeParams {
     int32_t fused_build;         // TMA kernel: 1 = every CTA derives the queue from seq_lens itself
     int32_t heads_per_cta;       // TMA kernel: KV heads one CTA streams together (1, 2, 4 or 8)
     int32_t dynamic_sched;      // 1: tasks handed out by an atomic counter
+    int32_t force_replan;       // test hook: treat the speculative plan as invalidated
     float scale;                // x = scale * <q, k>
     float scale_log2;           // scale * log2(e)
     unsigned long long* trace;  // debug: [grid][16] %globaltimer stamps, or nullptr (pkv_debug_set_trace)
@@ -325,10 +326,19 @@ __device__ __forceinline__ PlanTotals plan_scan(PlanArgs& a, const int32_t* seq_
 // that owns the row -- the RowSlot of pair rs0 (the calling CTA's first work unit) into *first.
 // Returns the number of (row, split) pairs.  plan_warp_totals (off the critical path) redoes the
 // per-row bounds for the header counters.  so_out / len_out / first: shared memory of the CTA.
+// SPEC: the lengths are read with relaxed (race-tolerant) loads before the kernel's dependency
+// wait; the caller validates them after the wait (plan_lens_unchanged) and re-plans on a mismatch.
+__device__ __forceinline__ int32_t ld_relaxed_s32(const int32_t* ptr) {
+    int32_t v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(ptr) : "memory");
+    return v;
+}
+template <bool SPEC = false>
 __device__ __forceinline__ int32_t plan_warp_prefix(PlanArgs& a, const int32_t* seq_lens, int32_t* so_out,
                                                     int32_t* len_out, int lane, int rs0, RowSlot* first) {
 #pragma unroll 4
-    for (int i = lane; i < a.B; i += 32) len_out[i] = max(__ldcg(seq_lens + i), 0);
+    for (int i = lane; i < a.B; i += 32)
+        len_out[i] = max(SPEC ? ld_relaxed_s32(seq_lens + i) : __ldcg(seq_lens + i), 0);
     if (lane == 0) so_out[0] = 0;
     __syncwarp();
     if (a.split_mode == PKV_SPLIT_BALANCED) {
@@ -373,6 +383,15 @@ __device__ __forceinline__ int32_t plan_warp_prefix(PlanArgs& a, const int32_t* 
     }
     __syncwarp();
     return carry;
+}
+
+// After the dependency wait: are the lengths a speculative plan was made from (len_s) still the
+// ones in memory?  Every lane returns the answer.
+__device__ __forceinline__ bool plan_lens_unchanged(const PlanArgs& a, const int32_t* seq_lens, const int32_t* len_s,
+                                                    int lane) {
+    bool same = true;
+    for (int i = lane; i < a.B; i += 32) same &= max(__ldcg(seq_lens + i), 0) == len_s[i];
+    return __all_sync(0xffffffffu, same);
 }
 
 __device__ __forceinline__ PlanTotals plan_warp_totals(const PlanArgs& a, const int32_t* len_s, int32_t row_slots,

@@ -574,3 +574,31 @@ def test_full_size_configs_in_the_bench_configuration(name):
         tasks, offs = pkv.pkv_read_workqueue(shape, pol, ws)
         assert np.array_equal(tasks, np.array(want.tasks, dtype=np.int32).reshape(-1, 5))
         assert np.array_equal(offs, np.array(want.split_offsets, dtype=np.int32))
+
+
+@pytest.mark.parametrize("mode", [pkv.SPLIT_FIXED_COUNT, pkv.SPLIT_BALANCED])
+def test_speculative_plan_is_discarded_when_lengths_changed(mode):
+    """The TMA kernel plans from seq_lens before its dependency wait and validates the lengths
+    afterwards.  With the test hook every launch behaves as if the
+    kernel right before it had rewritten seq_lens: a deliberately wrong speculative plan is left
+    behind and the kernel must plan again.  Same queue, bitwise the same output as without it."""
+    lens = [9000, 40, 1300, 0, 517, 4097, 16, 2222]
+    p = make_problem(lens, seed=43)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    pol = pkv.Policy(tile_tokens=16, split_mode=mode, num_splits=0 if mode == pkv.SPLIT_BALANCED else 6)
+    o1, l1, ws1, _ = check(dp, pol, ref)
+    pkv.pkv_debug_force_replan(True)
+    try:
+        o2, l2, ws2, _ = check(dp, pol, ref)
+    finally:
+        pkv.pkv_debug_force_replan(False)
+    assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
+    t1, f1 = pkv.pkv_read_workqueue(dp.shape, pol, ws1)
+    t2, f2 = pkv.pkv_read_workqueue(dp.shape, pol, ws2)
+    assert np.array_equal(t1, t2) and np.array_equal(f1, f2)
+    # seq_lens rewritten on the device right before the call (stream order): the new lengths count
+    new = np.array([100, 40, 1300, 0, 517, 33, 16, 2000], dtype=np.int32)     # within the reserved pages
+    dp.sl.copy_(to_dev(new))
+    p.seq_lens = new
+    check(dp, pol, oracle_attention(p))
