@@ -169,6 +169,10 @@ PKV_API pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_p
  * written to the workspace, bit-identical to pkv_build_workqueue's).  The merge launch is skipped
  * when the policy cannot produce more than one split per row, or merge_mode is FUSED.
  * Results are bitwise reproducible from launch to launch for the same inputs, policy and device.
+ * Programmatic launch: the decode kernel may start while the kernel before it in the stream is
+ * still running.  It then reads nothing but seq_lens (race-tolerant loads, for a speculative
+ * plan) before that kernel has finished, and re-validates those lengths afterwards -- a
+ * predecessor that writes seq_lens, q, the block table or the caches is handled correctly.
  * Heads per CTA: the TMA kernel streams HG = 8, 4, 2 or 1 KV heads per CTA, the largest value
  * that still leaves one work unit per SM given the bound B*S on the (row, split) pairs; with
  * BALANCED the bound is policy.num_sms, so num_sms = SMs*HG/Hkv asks for HG heads per CTA.
