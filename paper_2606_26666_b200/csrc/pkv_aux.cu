@@ -110,27 +110,41 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) merge_trace_stamp(p, 0);
     pdl_launch_dependents();
+    // A guess at the row's slot range, read (race-tolerant) before the decode grid has finished:
+    // merge CTAs are resident long before their wait returns, and from one decode step to the
+    // next the ranges rarely move.  After the wait the first batch of states is requested from
+    // the guessed range TOGETHER with the real split_offsets -- one round trip instead of two --
+    // and thrown away if the guess was wrong.  The guess is only used if it lies inside the
+    // partial-state buffers.
+    const int so_g = ld_relaxed_s32(p.split_offsets + row);
+    const int n_g = ld_relaxed_s32(p.split_offsets + row + 1) - so_g;
+    const bool guess = p.tasks_cap > 0 && so_g >= 0 && n_g > 1 && ((int64_t)so_g + (int64_t)n_g) * p.Hkv <= p.tasks_cap;
     pdl_wait();
     if (threadIdx.x == 0) merge_trace_stamp(p, 1);
     const int so = __ldcg(p.split_offsets + row);
     const int n = __ldcg(p.split_offsets + row + 1) - so;
-    if (n <= 1 && p.hdr != nullptr) return;   // library path: decode already produced out/lse
-    const int64_t base = (int64_t)so * p.Hkv + (int64_t)kvh * n;
-    float M = -INFINITY, L = 0.f;
-    float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int s0 = warp; s0 < n; s0 += NW * NB) {
-        float mv[NB], lv[NB];
-        float4 av[NB];
+    auto load_batch = [&](int64_t base_, int n_, int s0, float (&mv)[NB], float (&lv)[NB], float4 (&av)[NB]) {
 #pragma unroll
         for (int j = 0; j < NB; ++j) {
             const int s = s0 + j * NW;
-            const bool ok = s < n;
-            const int64_t r = (base + (ok ? s : 0)) * G + hh;
+            const bool ok = s < n_;
+            const int64_t r = (base_ + (ok ? s : 0)) * G + hh;
             mv[j] = ok ? __ldcg(p.part_m + r) : -INFINITY;
             lv[j] = ok ? __ldcg(p.part_l + r) : 0.f;
             av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * kD + lane * 4))
                        : make_float4(0.f, 0.f, 0.f, 0.f);
         }
+    };
+    float mv[NB], lv[NB];
+    float4 av[NB];
+    if (guess) load_batch((int64_t)so_g * p.Hkv + (int64_t)kvh * n_g, n_g, warp, mv, lv, av);
+    if (n <= 1 && p.hdr != nullptr) return;   // library path: decode already produced out/lse
+    const bool hit = guess && so == so_g && n == n_g;
+    const int64_t base = (int64_t)so * p.Hkv + (int64_t)kvh * n;
+    float M = -INFINITY, L = 0.f;
+    float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int s0 = warp; s0 < n; s0 += NW * NB) {
+        if (!(hit && s0 == warp)) load_batch(base, n, s0, mv, lv, av);
         float mb = mv[0];
 #pragma unroll
         for (int j = 1; j < NB; ++j) mb = fmaxf(mb, mv[j]);
