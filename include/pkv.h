@@ -21,8 +21,11 @@
  *     thread-local description of the last non-OK status.
  *   - host-checkable arguments are rejected before any launch.  Device-resident values
  *     (seq_lens[i] > max_pages*page_size, a page id >= num_pages) cannot be checked without a
- *     synchronisation: they are undefined behaviour.  seq_lens[i] == 0 is legal: the row
- *     emits no task, out[i] = 0 and lse[i] = -inf (reading A9).
+ *     synchronisation: they are undefined behaviour -- unless policy.flags has PKV_FLAG_VALIDATE,
+ *     which adds device-side checks that record the fault in the workspace's error word
+ *     (pkv_counters.error_word) and keep the kernels inside the caller's buffers (PAPER.md:67:
+ *     every bound is derived from N_i).  seq_lens[i] == 0 is legal: the row emits no task,
+ *     out[i] = 0 and lse[i] = -inf (reading A9).
  *   - compiled-in shapes: d = 128, page_size = 16, FP16, G = Hq/Hkv in {1, 2, 4, 8}.  Anything else
  *     returns PKV_ERR_UNSUPPORTED.
  */
@@ -90,7 +93,20 @@ typedef struct {
     int32_t num_sms;     /* SM count for the auto rule and for BALANCED; 0 = the current device's
                             (device calls only; the host builder needs it > 0 then)             */
     int32_t kernel;      /* pkv_kernel                                                           */
+    int32_t flags;       /* bit set of pkv_flag                                                  */
 } pkv_split_policy;
+
+/* policy.flags */
+typedef enum {
+    /* Device-side validation of device-resident inputs (SURVEY.md sec. 8(b) debug check): a row
+     * with seq_lens[i] > max_pages*page_size is decoded as if its length were max_pages*page_size
+     * and sets PKV_DEVERR_SEQ_LEN; a block-table entry outside [0, num_pages) that a task would
+     * dereference is replaced by page 0 and sets PKV_DEVERR_PAGE_ID.  The kernels then never read
+     * outside the block table or the page pool; the result of a faulted row is unspecified. */
+    PKV_FLAG_VALIDATE = 1
+} pkv_flag;
+/* bits of pkv_counters.error_word (sticky in the workspace until its init bytes are zeroed again) */
+typedef enum { PKV_DEVERR_QUEUE_OVERFLOW = 1, PKV_DEVERR_SEQ_LEN = 2, PKV_DEVERR_PAGE_ID = 4 } pkv_device_error;
 
 /* One workqueue entry: tile interval [t_begin, t_end) of row `row`, KV head `kvh`;
  * token range = [t_begin*tile_tokens, min(t_end*tile_tokens, N_row)). */
@@ -125,6 +141,12 @@ typedef struct {
     int64_t chunk_tiles;     /* FIXED_CHUNK / BALANCED: resolved tiles per task; else 0          */
     int64_t h2d_bytes;       /* pkv_decode_host only: bytes copied host->device this step        */
     int64_t d2h_bytes;       /* pkv_decode_host only: bytes copied device->host this step        */
+    /* What the last build / decode on this workspace REALLY launched (each kernel leaves its mark
+     * in the queue header).  On the device path the host cannot see the lengths, so a merge kernel
+     * is launched whenever the policy allows more than one split per row, and a decode kernel
+     * even when every row is empty: these can exceed the scheduler-derived counts above. */
+    int64_t launched_build, launched_decode, launched_merge;
+    int64_t error_word;      /* bit set of pkv_device_error                                      */
 } pkv_counters;
 
 /* Library/ABI version: (major << 16) | minor. */
@@ -245,6 +267,28 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
                                    size_t scratch_bytes, void* workspace, size_t workspace_bytes,
                                    void* stream, pkv_counters* counters_out);
 
+/*
+ * Calibration of the paper's cost-model constants on the current device ("beta is
+ * measured streaming read bandwidth ... lambda is a calibrated launch-overhead constant ... a
+ * different GPU should re-fit them").  dev_buffer: device memory, 256-byte aligned, at least 64 MiB
+ * (use several times the L2 size: it is read end to end, its first word may be written).  Runs
+ * probe kernels on a stream of its own after synchronising `stream`; allocates two events, a
+ * stream and a graph; NOT capture-safe; takes tens of milliseconds.
+ */
+typedef struct {
+    double read_gbps;           /* beta: the best of the three read probes below, GB/s                 */
+    double read_ldg_gbps;       /* 16-byte ld.global.nc loads, persistent grid of 4 CTAs per SM        */
+    double read_bulk8k_gbps;    /* cp.async.bulk 8 KiB chunks into a 12-stage shared-memory ring, 1 CTA/SM */
+    double read_bulk16k_gbps;   /* the same with 16 KiB chunks                                         */
+    double launch_us;           /* lambda: per kernel of a chain of empty kernels launched into a stream */
+    double launch_pdl_us;       /* the same with programmatic dependent launch                         */
+    double graph_launch_us;     /* the same chain replayed from a CUDA graph                           */
+    double graph_launch_pdl_us; /* graph + programmatic dependent launch (what a decode step pays)     */
+    int64_t buffer_bytes;
+    int32_t num_sms, l2_bytes;
+} pkv_calibration;
+PKV_API pkv_status pkv_calibrate(void* dev_buffer, size_t bytes, void* stream, pkv_calibration* out);
+
 /* Test hook: KV heads one CTA of the TMA kernel streams together.
  * 0 = automatic (largest of 8/4/2/1 dividing Hkv that leaves >= one work unit per SM), else
  * 1, 2, 4 or 8 (ignored when it does not divide Hkv).  Process-wide. */
@@ -258,9 +302,6 @@ PKV_API void pkv_debug_set_fused_build(int on);
  * dependency wait and plan again afterwards -- the path taken when the kernel right before
  * pkv_decode wrote seq_lens.  Process-wide. */
 PKV_API void pkv_debug_force_replan(int on);
-/* Debug hook: device buffer of grid*16 uint64 that the TMA decode kernel fills with %globaltimer
- * stamps of its phases, or NULL to switch tracing off.  Process-wide. */
-PKV_API void pkv_debug_set_trace(void* dev_u64);
 
 #ifdef __cplusplus
 }

@@ -22,6 +22,8 @@ ROUTE_RECT, ROUTE_WORKQUEUE = 0, 1
 MERGE_SEPARATE, MERGE_FUSED = 0, 1
 SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK, SPLIT_BALANCED = 0, 1, 2
 KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
+FLAG_VALIDATE = 1
+DEVERR_QUEUE_OVERFLOW, DEVERR_SEQ_LEN, DEVERR_PAGE_ID = 1, 2, 4
 STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL = 1, 2, 4, 7
 
 _i32, _i64 = ctypes.c_int32, ctypes.c_int64
@@ -30,7 +32,7 @@ _vp = ctypes.c_void_p
 
 class pkv_split_policy(ctypes.Structure):
     _fields_ = [("tile_tokens", _i32), ("split_mode", _i32), ("num_splits", _i32), ("chunk_tiles", _i32),
-                ("route", _i32), ("merge_mode", _i32), ("num_sms", _i32), ("kernel", _i32)]
+                ("route", _i32), ("merge_mode", _i32), ("num_sms", _i32), ("kernel", _i32), ("flags", _i32)]
 
 
 class pkv_task(ctypes.Structure):
@@ -45,16 +47,25 @@ class pkv_shape(ctypes.Structure):
 class pkv_counters(ctypes.Structure):
     _fields_ = [(n, _i64) for n in ("tasks", "empty_tasks", "decode_launches", "merge_launches", "build_launches",
                                     "useful_kv_bytes", "merge_bytes", "num_splits", "max_row_splits", "chunk_tiles", "h2d_bytes",
-                                    "d2h_bytes")]
+                                    "d2h_bytes", "launched_build", "launched_decode", "launched_merge", "error_word")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
 
 
+class pkv_calibration(ctypes.Structure):
+    _fields_ = ([(n, ctypes.c_double) for n in ("read_gbps", "read_ldg_gbps", "read_bulk8k_gbps", "read_bulk16k_gbps",
+                                                 "launch_us", "launch_pdl_us", "graph_launch_us", "graph_launch_pdl_us")]
+                + [("buffer_bytes", _i64), ("num_sms", _i32), ("l2_bytes", _i32)])
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspace_init_bytes", "pkv_build_workqueue_host",
            "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
-           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_debug_force_heads_per_cta", "pkv_debug_set_pdl", "pkv_debug_set_fused_build", "pkv_debug_set_trace", "pkv_debug_force_replan")
+           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate", "pkv_debug_force_heads_per_cta", "pkv_debug_set_pdl", "pkv_debug_set_fused_build", "pkv_debug_force_replan")
 
 
 class PkvError(RuntimeError):
@@ -100,6 +111,8 @@ def _load() -> ctypes.CDLL:
     lib.pkv_decode_host.restype = _i32
     lib.pkv_decode_host.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float,
                                     _vp, _vp, ctypes.c_size_t, _vp, ctypes.c_size_t, _vp, P(pkv_counters)]
+    lib.pkv_calibrate.restype = _i32
+    lib.pkv_calibrate.argtypes = [_vp, ctypes.c_size_t, _vp, P(pkv_calibration)]
     lib.pkv_debug_force_heads_per_cta.restype = None
     lib.pkv_debug_force_heads_per_cta.argtypes = [ctypes.c_int]
     lib.pkv_debug_set_pdl.restype = None
@@ -108,8 +121,6 @@ def _load() -> ctypes.CDLL:
     lib.pkv_debug_set_fused_build.argtypes = [ctypes.c_int]
     lib.pkv_debug_force_replan.restype = None
     lib.pkv_debug_force_replan.argtypes = [ctypes.c_int]
-    lib.pkv_debug_set_trace.restype = None
-    lib.pkv_debug_set_trace.argtypes = [_vp]
     return lib
 
 
@@ -149,10 +160,11 @@ class Policy:
     merge_mode: int = MERGE_SEPARATE
     num_sms: int = 0
     kernel: int = KERNEL_AUTO
+    flags: int = 0
 
     def c(self) -> pkv_split_policy:
         return pkv_split_policy(self.tile_tokens, self.split_mode, self.num_splits, self.chunk_tiles, self.route,
-                                self.merge_mode, self.num_sms, self.kernel)
+                                self.merge_mode, self.num_sms, self.kernel, self.flags)
 
 
 def _ptr(x) -> Optional[int]:
@@ -294,6 +306,13 @@ def pkv_decode_host(shape: Shape, policy: Policy, q_host, k_cache_dev, v_cache_d
     return c.as_dict()
 
 
+def pkv_calibrate(dev_buffer, stream=None) -> dict:
+    """Measures beta (read bandwidth) and lambda (launch overhead) on the current device."""
+    c = pkv_calibration()
+    _check(_lib.pkv_calibrate(_ptr(dev_buffer), _nbytes(dev_buffer), _stream_ptr(stream), ctypes.byref(c)))
+    return c.as_dict()
+
+
 def pkv_debug_force_heads_per_cta(heads: int) -> None:
     _lib.pkv_debug_force_heads_per_cta(int(heads))
 
@@ -304,10 +323,6 @@ def pkv_debug_set_pdl(on: bool) -> None:
 
 def pkv_debug_force_replan(on: bool) -> None:
     _lib.pkv_debug_force_replan(1 if on else 0)
-
-
-def pkv_debug_set_trace(dev_u64) -> None:
-    _lib.pkv_debug_set_trace(_ptr(dev_u64))
 
 
 def pkv_debug_set_fused_build(on: bool) -> None:

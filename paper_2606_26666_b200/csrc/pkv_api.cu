@@ -16,9 +16,10 @@ bool g_use_pdl = true;  // test hook (pkv_debug_set_pdl)
 
 namespace {
 
-unsigned long long* g_trace = nullptr;  // debug hook
+#ifdef PKV_TRACE
+unsigned long long* g_trace = nullptr;  // trace build only (pkv_debug_set_trace)
+#endif
 bool g_fused_build = true;              // test hook (pkv_debug_set_fused_build)
-constexpr int kMaxFusedRows = 512;      // = pkv_decode_tma.cu
 int g_force_hg = 0;  // test hook: 0 = automatic heads-per-CTA, else 1/2/4/8
 bool g_force_replan = false;  // test hook (pkv_debug_force_replan)
 
@@ -202,7 +203,10 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.plan = make_plan_args(s, rp);
     p.tasks_cap = tasks_cap;
     p.fused_build = fused_build ? 1 : 0;
+    p.num_pages = s.num_pages;
+#ifdef PKV_TRACE
     p.trace = g_trace;
+#endif
     const float sc = scale > 0.f ? scale : 1.0f / std::sqrt((float)s.d);
     p.scale = sc;
     p.scale_log2 = sc * kLog2e;
@@ -295,7 +299,11 @@ void pkv_debug_force_heads_per_cta(int hg) { g_force_hg = hg; }
 void pkv_debug_set_pdl(int on) { g_use_pdl = on != 0; }
 void pkv_debug_force_replan(int on) { g_force_replan = on != 0; }
 void pkv_debug_set_fused_build(int on) { g_fused_build = on != 0; }
-void pkv_debug_set_trace(void* dev) { g_trace = static_cast<unsigned long long*>(dev); }
+#ifdef PKV_TRACE
+// Trace build only (python -m paper_2606_26666_b200.build --trace): device buffer of grid*16
+// uint64 that the TMA decode kernel fills with %globaltimer stamps of its phases; NULL = off.
+__attribute__((visibility("default"))) void pkv_debug_set_trace(void* dev) { g_trace = static_cast<unsigned long long*>(dev); }
+#endif
 
 pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_policy* policy, const int32_t* seq_lens_dev,
                                void* workspace, size_t workspace_bytes, void* stream) {
@@ -410,6 +418,10 @@ pkv_status pkv_get_counters(const pkv_shape* shape, const pkv_split_policy* poli
     host_out->num_splits = h.resolved_splits;
     host_out->max_row_splits = h.max_row_splits;
     host_out->chunk_tiles = h.chunk_tiles;
+    host_out->launched_build = h.launched_build;
+    host_out->launched_decode = h.launched_decode;
+    host_out->launched_merge = h.launched_merge;
+    host_out->error_word = h.error_word;
     return PKV_OK;
 }
 
@@ -532,6 +544,24 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     st = check_workspace(workspace, workspace_bytes, L);
     if (st != PKV_OK) return st;
     cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    // here the lengths ARE host-checkable; the page ids are checked when the caller asks for it
+    for (int32_t i = 0; i < s.B; ++i) {
+        const int64_t N = seq_lens_host[i];
+        if (N > (int64_t)s.max_pages * s.page_size) {
+            set_error("seq_lens[%d]=%lld exceeds max_pages*page_size=%lld", i, (long long)N, (long long)s.max_pages * s.page_size);
+            return PKV_ERR_INVALID_ARG;
+        }
+        if (rp.flags & PKV_FLAG_VALIDATE) {
+            const int64_t np = N > 0 ? (N + s.page_size - 1) / s.page_size : 0;
+            for (int64_t j = 0; j < np; ++j) {
+                const int32_t pg = block_table_host[(int64_t)i * s.max_pages + j];
+                if (pg < 0 || pg >= s.num_pages) {
+                    set_error("block_table[%d][%lld]=%d outside [0, %lld)", i, (long long)j, pg, (long long)s.num_pages);
+                    return PKV_ERR_INVALID_ARG;
+                }
+            }
+        }
+    }
 
     // host planning ("Python planning" is part of the serving-facing time)
     unsigned char* hs = static_cast<unsigned char*>(host_staging);
@@ -597,6 +627,8 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         counters_out->chunk_tiles = hdr->chunk_tiles;
         counters_out->h2d_bytes = (int64_t)h2d;
         counters_out->d2h_bytes = (int64_t)out_bytes;
+        counters_out->launched_decode = dl;
+        counters_out->launched_merge = ml;
     }
     return PKV_OK;
 }

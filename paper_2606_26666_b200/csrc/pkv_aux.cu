@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
         // into shared memory, everybody writes the queue -- so that this entry point and the
         // fused build run (and the tests of either exercise) the same code
         if (tid < 32) {
-            const int32_t rs = plan_warp_prefix(plan, a.seq_lens, so_s, len_s, tid, -1, &unused_first);
+            const int32_t rs = plan_warp_prefix(plan, a.seq_lens, so_s, len_s, tid, -1, &unused_first, &a.hdr->error_word);
             const PlanTotals t = plan_warp_totals(plan, len_s, rs, tid);
             if (tid == 0) { tot_s = t; chunk_s = plan.chunk_tiles; }
         }
@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
         so = so_s;
         lens = len_s;
     } else {
-        tot = plan_scan(plan, a.seq_lens, a.split_offsets, nullptr, sc);
+        tot = plan_scan(plan, a.seq_lens, a.split_offsets, nullptr, sc, &a.hdr->error_word);
     }
     for (int i = tid; i < a.plan.B * a.plan.Hkv; i += nthreads) a.fuse_counters[i] = 0;
     __threadfence_block();
@@ -67,21 +67,22 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
         const RowSlot d = make_rowslot(plan, so, lens, rs, &tb, &te);
         write_pair(plan, d, tb, te, rs, a.rowslots, a.tasks, a.tasks_cap);
     }
-    if (tid == 0) {
-        QueueHeader h;
-        h.num_tasks = (int32_t)(total < a.tasks_cap ? total : a.tasks_cap);
-        h.max_row_splits = tot.max_n;
-        h.total_row_slots = tot.row_slots;
-        h.resolved_splits = a.plan.S;
-        h.empty_tasks = (tot.row_slots - tot.sum_n) * a.plan.Hkv;   // rect route; 0 on the workqueue route
-        h.work_counter = 0;
-        h.done_counter = 0;
-        h.error_word = total > a.tasks_cap ? 1 : 0;
-        h.sum_seq_lens = tot.sum_seq;
-        h.build_launches = 1;
-        h.chunk_tiles = plan.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : plan.chunk_tiles;
-        h.pad_[0] = h.pad_[1] = 0;
-        *a.hdr = h;
+    if (tid == 0) {   // field by field: error_word is sticky and only ever OR-ed into
+        QueueHeader* h = a.hdr;
+        h->num_tasks = (int32_t)(total < a.tasks_cap ? total : a.tasks_cap);
+        h->max_row_splits = tot.max_n;
+        h->total_row_slots = tot.row_slots;
+        h->resolved_splits = a.plan.S;
+        h->empty_tasks = (tot.row_slots - tot.sum_n) * a.plan.Hkv;   // rect route; 0 on the workqueue route
+        h->work_counter = 0;
+        h->done_counter = 0;
+        if (total > a.tasks_cap) atomicOr(&h->error_word, (int32_t)PKV_DEVERR_QUEUE_OVERFLOW);
+        h->sum_seq_lens = tot.sum_seq;
+        h->build_launches = 1;
+        h->chunk_tiles = plan.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : plan.chunk_tiles;
+        h->launched_build = 1;
+        h->launched_decode = 0;
+        h->launched_merge = 0;
     }
 }
 
@@ -92,14 +93,6 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
 // of PAPER.md:60-61 is associative, so the per-warp states combine exactly the same way.  Warp 0
 // combines the NW warp states in fixed order (deterministic).  Rows with at most one slot were
 // written directly by the decode kernel.  NW = 2 .. 16 is chosen at launch (launch_merge).
-// debug trace (pkv_debug_set_trace): merge CTAs stamp behind the decode kernel's [148][16] block
-__device__ __forceinline__ void merge_trace_stamp(const DecodeParams& p, int slot) {
-    if (p.trace && blockIdx.x < 4096) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        p.trace[148 * 16 + (size_t)blockIdx.x * 4 + slot] = t;
-    }
-}
 template <int G, int NW, int MINB>
 __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodeParams p) {
     constexpr int NB = kMergeBatch;
@@ -108,7 +101,6 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
     const int row = blockIdx.x / p.Hq, h = blockIdx.x % p.Hq;
     const int kvh = h / G, hh = h % G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) merge_trace_stamp(p, 0);
     pdl_launch_dependents();
     // A guess at the row's slot range, read (race-tolerant) before the decode grid has finished:
     // merge CTAs are resident long before their wait returns, and from one decode step to the
@@ -120,7 +112,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
     const int n_g = ld_relaxed_s32(p.split_offsets + row + 1) - so_g;
     const bool guess = p.tasks_cap > 0 && so_g >= 0 && n_g > 1 && ((int64_t)so_g + (int64_t)n_g) * p.Hkv <= p.tasks_cap;
     pdl_wait();
-    if (threadIdx.x == 0) merge_trace_stamp(p, 1);
+    if (blockIdx.x == 0 && threadIdx.x == 0 && p.hdr != nullptr) p.hdr->launched_merge = 1;   // this launch's mark
     const int so = __ldcg(p.split_offsets + row);
     const int n = __ldcg(p.split_offsets + row + 1) - so;
     auto load_batch = [&](int64_t base_, int n_, int s0, float (&mv)[NB], float (&lv)[NB], float4 (&av)[NB]) {
@@ -165,7 +157,6 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
     sA[warp][lane] = A;
     if (lane == 0) { sM[warp] = M; sL[warp] = L; }
     __syncthreads();
-    if (threadIdx.x == 0) merge_trace_stamp(p, 2);
     if (warp == 0) {
         float Mf = sM[0];
 #pragma unroll
@@ -183,7 +174,6 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
             }
         }
         merge_store(p, (int64_t)row * p.Hq + h, lane, Mf, Ls, As);
-        if (lane == 0) merge_trace_stamp(p, 3);
     }
 }
 

@@ -1,0 +1,233 @@
+// pkv_calibrate.cu -- measures the constants of the paper's cost model on THIS device
+// (sec. 3.5: "beta is measured streaming read bandwidth ... lambda is a calibrated
+// launch-overhead constant ... a different GPU should re-fit them before using the route policy").
+//
+//   beta     read-only streaming rate of a buffer larger than L2, two ways: 16-byte ld.global.nc
+//            loads from a persistent grid, and 1-D bulk copies (cp.async.bulk, the TMA engine) into a
+//            shared-memory ring -- the path the decode kernel's K/V stream takes.  The better of the
+//            two is the read ceiling a decode step is held against (the driver's copy figure counts
+//            read + write bytes and is not a ceiling for a read-only kernel).
+//   lambda   device time added by one more dependent kernel launch in a stream: a chain of empty
+//            kernels, plain and with programmatic dependent launch.
+// Not on the hot path; allocates nothing but two events; SYNCHRONISES the stream.
+#include <cstring>
+
+#include "pkv_device.cuh"
+
+namespace pkv {
+namespace {
+
+constexpr int kReadThreads = 512;
+constexpr int kReadUnroll = 8;
+
+__global__ void __launch_bounds__(kReadThreads) pkv_probe_read_kernel(const uint4* __restrict__ src, size_t n16,
+                                                                      unsigned* sink) {
+    const size_t stride = (size_t)gridDim.x * kReadThreads;
+    size_t i = (size_t)blockIdx.x * kReadThreads + threadIdx.x;
+    unsigned acc = 0;
+    for (; i + (kReadUnroll - 1) * stride < n16; i += kReadUnroll * stride) {
+        uint4 v[kReadUnroll];
+#pragma unroll
+        for (int u = 0; u < kReadUnroll; ++u) {
+            const uint4* ptr = src + i + u * stride;
+            asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(v[u].x), "=r"(v[u].y), "=r"(v[u].z), "=r"(v[u].w)
+                         : "l"(ptr));
+        }
+#pragma unroll
+        for (int u = 0; u < kReadUnroll; ++u) acc ^= v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
+    }
+    for (; i < n16; i += stride) {
+        const uint4 v = src[i];
+        acc ^= v.x ^ v.y ^ v.z ^ v.w;
+    }
+    if (acc == 0x9e3779b9u) *sink = acc;   // keeps the loads alive; practically never taken
+}
+
+// One CTA per SM, one thread: a ring of kStages bulk copies of `chunk` bytes each in flight; when a
+// stage lands it is re-issued for the CTA's next chunk (nothing reads the shared memory).
+constexpr int kBulkStages = 12;
+__global__ void __launch_bounds__(32) pkv_probe_bulk_kernel(const unsigned char* __restrict__ src, size_t bytes,
+                                                            int chunk) {
+    extern __shared__ __align__(128) unsigned char ring[];
+    __shared__ unsigned long long bars[kBulkStages];
+    if (threadIdx.x != 0) return;
+    const uint32_t bar0 = smem_u32(&bars[0]);
+    for (int s = 0; s < kBulkStages; ++s) mbar_init(bar0 + 8 * s, 1);
+    mbar_fence_init();
+    const unsigned long long pol = l2_policy_evict_first();
+    const size_t nchunks = bytes / (size_t)chunk;
+    size_t c = blockIdx.x;
+    uint32_t phase = 0;
+    int inflight = 0;
+    // fill, then steady state: wait for stage s, re-issue
+    for (int s = 0; s < kBulkStages && c < nchunks; ++s, c += gridDim.x, ++inflight) {
+        mbar_arrive_expect_tx(bar0 + 8 * s, (uint32_t)chunk);
+        asm volatile(
+            "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                smem_u32(ring + (size_t)s * chunk)),
+            "l"(src + c * (size_t)chunk), "r"(chunk), "r"(bar0 + 8 * s), "l"(pol)
+            : "memory");
+    }
+    while (inflight > 0) {
+        for (int s = 0; s < kBulkStages && inflight > 0; ++s) {
+            mbar_wait(bar0 + 8 * s, phase);
+            --inflight;
+            if (c < nchunks) {
+                mbar_arrive_expect_tx(bar0 + 8 * s, (uint32_t)chunk);
+                asm volatile(
+                    "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                        smem_u32(ring + (size_t)s * chunk)),
+                    "l"(src + c * (size_t)chunk), "r"(chunk), "r"(bar0 + 8 * s), "l"(pol)
+                    : "memory");
+                c += gridDim.x;
+                ++inflight;
+            }
+        }
+        phase ^= 1;
+    }
+}
+
+__global__ void pkv_probe_empty_kernel(int* p) {
+    pdl_launch_dependents();
+    pdl_wait();
+    if (p && threadIdx.x == 1025) *p = 0;
+}
+
+struct Timer {
+    cudaEvent_t a = nullptr, b = nullptr;
+    cudaStream_t s;
+    explicit Timer(cudaStream_t st) : s(st) {
+        cudaEventCreate(&a);
+        cudaEventCreate(&b);
+    }
+    ~Timer() {
+        if (a) cudaEventDestroy(a);
+        if (b) cudaEventDestroy(b);
+    }
+    void start() { cudaEventRecord(a, s); }
+    double stop_ms() {
+        cudaEventRecord(b, s);
+        cudaEventSynchronize(b);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        return (double)ms;
+    }
+};
+
+}  // namespace
+}  // namespace pkv
+
+using namespace pkv;
+
+extern "C" pkv_status pkv_calibrate(void* dev_buffer, size_t bytes, void* stream, pkv_calibration* out) {
+    clear_error();
+    if (!dev_buffer || !out || bytes < ((size_t)64 << 20) || reinterpret_cast<uintptr_t>(dev_buffer) % 256) {
+        set_error("pkv_calibrate needs a 256-byte aligned device buffer of at least 64 MiB and an output struct");
+        return PKV_ERR_INVALID_ARG;
+    }
+    std::memset(out, 0, sizeof(*out));
+    int dev = 0, sms = 0, l2 = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
+    if (e != cudaSuccess || sms <= 0) { set_error("no CUDA device: %s", cudaGetErrorString(e)); return PKV_ERR_CUDA; }
+    // measured on a stream of its own (graph capture is not allowed on the legacy default stream)
+    e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
+    cudaStream_t cs = nullptr;
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { set_error("pkv_calibrate stream: %s", cudaGetErrorString(e)); return PKV_ERR_CUDA; }
+    struct StreamGuard { cudaStream_t s; ~StreamGuard() { cudaStreamDestroy(s); } } guard{cs};
+    out->num_sms = sms;
+    out->l2_bytes = l2;
+    out->buffer_bytes = (int64_t)bytes;
+    Timer t(cs);
+    const int reps = 5;
+    // ---- beta: vector loads
+    {
+        const size_t n16 = bytes / 16;
+        double best = 0.0;
+        for (int r = 0; r < reps + 1; ++r) {
+            t.start();
+            pkv_probe_read_kernel<<<sms * 4, kReadThreads, 0, cs>>>(static_cast<const uint4*>(dev_buffer), n16,
+                                                                    static_cast<unsigned*>(dev_buffer));
+            const double ms = t.stop_ms();
+            if (r > 0 && ms > 0.0) best = best > (double)(n16 * 16) / ms / 1e6 ? best : (double)(n16 * 16) / ms / 1e6;
+        }
+        out->read_ldg_gbps = best;
+    }
+    // ---- beta: bulk copies into shared memory, 8 KiB and 16 KiB chunks
+    {
+        const int chunks[2] = {8192, 16384};
+        for (int ci = 0; ci < 2; ++ci) {
+            const int chunk = chunks[ci];
+            const int smem = chunk * kBulkStages;
+            e = cudaFuncSetAttribute(pkv_probe_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * kBulkStages);
+            if (e != cudaSuccess) { set_error("bulk probe attribute: %s", cudaGetErrorString(e)); return PKV_ERR_CUDA; }
+            const size_t used = bytes / chunk * chunk;
+            double best = 0.0;
+            for (int r = 0; r < reps + 1; ++r) {
+                t.start();
+                pkv_probe_bulk_kernel<<<sms, 32, smem, cs>>>(static_cast<const unsigned char*>(dev_buffer), used, chunk);
+                const double ms = t.stop_ms();
+                if (r > 0 && ms > 0.0) best = best > (double)used / ms / 1e6 ? best : (double)used / ms / 1e6;
+            }
+            (ci == 0 ? out->read_bulk8k_gbps : out->read_bulk16k_gbps) = best;
+        }
+    }
+    out->read_gbps = out->read_ldg_gbps;
+    if (out->read_bulk8k_gbps > out->read_gbps) out->read_gbps = out->read_bulk8k_gbps;
+    if (out->read_bulk16k_gbps > out->read_gbps) out->read_gbps = out->read_bulk16k_gbps;
+    // ---- lambda: a chain of empty kernels
+    {
+        const int n = 400;
+        for (int pdl = 0; pdl < 2; ++pdl) {
+            double best = 1e30;
+            const bool saved = g_use_pdl;
+            g_use_pdl = pdl != 0;
+            for (int r = 0; r < 4; ++r) {
+                t.start();
+                for (int i = 0; i < n; ++i) {
+                    e = launch_pdl(pkv_probe_empty_kernel, dim3(1), dim3(32), 0, cs, (int*)nullptr);
+                    if (e != cudaSuccess) break;
+                }
+                const double ms = t.stop_ms();
+                if (r > 0 && ms < best) best = ms;
+            }
+            g_use_pdl = saved;
+            if (e != cudaSuccess) { set_error("empty-kernel chain: %s", cudaGetErrorString(e)); return PKV_ERR_CUDA; }
+            (pdl ? out->launch_pdl_us : out->launch_us) = best * 1e3 / n;
+        }
+    }
+    // ---- lambda inside a CUDA graph (what a replayed decode step pays per extra kernel)
+    {
+        const int n = 400;
+        for (int pdl = 0; pdl < 2; ++pdl) {
+            const bool saved = g_use_pdl;
+            g_use_pdl = pdl != 0;
+            cudaGraph_t graph = nullptr;
+            cudaGraphExec_t exec = nullptr;
+            e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+            for (int i = 0; i < n && e == cudaSuccess; ++i)
+                e = launch_pdl(pkv_probe_empty_kernel, dim3(1), dim3(32), 0, cs, (int*)nullptr);
+            cudaError_t e2 = cudaStreamEndCapture(cs, &graph);
+            g_use_pdl = saved;
+            if (e == cudaSuccess) e = e2;
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&exec, graph, 0);
+            double best = 1e30;
+            for (int r = 0; r < 4 && e == cudaSuccess; ++r) {
+                t.start();
+                e = cudaGraphLaunch(exec, cs);
+                const double ms = t.stop_ms();
+                if (r > 0 && ms < best) best = ms;
+            }
+            if (exec) cudaGraphExecDestroy(exec);
+            if (graph) cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { set_error("empty-kernel graph: %s", cudaGetErrorString(e)); return PKV_ERR_CUDA; }
+            (pdl ? out->graph_launch_pdl_us : out->graph_launch_us) = best * 1e3 / n;
+        }
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { set_error("pkv_calibrate: %s", cudaGetErrorString(e)); return PKV_ERR_CUDA; }
+    return PKV_OK;
+}

@@ -13,6 +13,7 @@ constexpr int kD = 128;         // head dimension compiled in
 constexpr int kPage = 16;       // page size compiled in
 constexpr int kAutoCMin = 4;    // PAPER.md:85 "C_min = 4 CTAs/SM" (auto split rule, A12)
 constexpr int kMaxSplits = 256; // cap on S (and on n_i in FIXED_CHUNK mode)
+constexpr int kMaxFusedRows = 512;  // fused build (TMA kernel): the batch's offsets and lengths sit in shared memory
 
 void set_error(const char* fmt, ...);
 void clear_error();
@@ -30,11 +31,14 @@ struct QueueHeader {
     int32_t empty_tasks;     // rect route: entries with t_begin >= t_end
     int32_t work_counter;    // dynamic task scheduler; self-resetting
     int32_t done_counter;    // CTAs that finished; self-resetting
-    int32_t error_word;      // reserved
+    int32_t error_word;      // pkv_device_error bits; sticky (kernels only ever OR into it)
     int64_t sum_seq_lens;    // sum_i N_i
     int32_t build_launches;  // 1: written by the builder kernel, 0: by the decode kernel's fused build / the host
     int32_t chunk_tiles;     // FIXED_CHUNK / BALANCED: resolved tiles per task, else 0
-    int64_t pad_[2];
+    int32_t launched_build;  // what the last build / decode on this workspace really launched:
+    int32_t launched_decode; //   every kernel leaves its mark (pkv_counters.launched_*)
+    int32_t launched_merge;
+    int32_t pad_;
 };
 static_assert(sizeof(QueueHeader) == 64, "QueueHeader layout");
 
@@ -62,6 +66,7 @@ struct Resolved {
     int32_t kernel;
     int32_t G;
     int32_t num_sms;    // BALANCED: U (policy.num_sms, else the device's)
+    int32_t flags;      // pkv_flag bits
 };
 
 // Byte offsets inside the caller's workspace.  Pure function of (shape, S bound).

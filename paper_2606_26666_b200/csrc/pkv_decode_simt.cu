@@ -46,11 +46,15 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
     pdl_launch_dependents();
     pdl_wait();
     zero_empty_rows(p);
+    if (blockIdx.x == 0 && tid == 0) {   // this launch's mark (pkv_counters.launched_*)
+        p.hdr->launched_decode = 1;
+        p.hdr->launched_merge = 0;
+    }
     const int num_tasks = p.hdr->num_tasks;
     for (int t = blockIdx.x; t < num_tasks; t += gridDim.x) {
         const pkv_task task = p.tasks[t];
         const int row = task.row, kvh = task.kvh;
-        const int N = p.seq_lens[row];
+        const int N = plan_len(p.plan, p.seq_lens[row]);
         const int so = p.split_offsets[row];
         const int n_i = p.split_offsets[row + 1] - so;
         const int64_t slot = (int64_t)so * p.Hkv + (int64_t)kvh * n_i + task.split;
@@ -85,7 +89,7 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
             for (int u = 0; u < kUnroll; ++u) {
                 const int j = base + hw + 8 * u;
                 if (j < tok1) {
-                    const int64_t page = bt[j >> 4];
+                    const int64_t page = checked_page(bt[j >> 4], p.plan.flags, p.num_pages, &p.hdr->error_word);
                     const int64_t off = page * p.stride_page + (int64_t)(j & 15) * p.stride_token + head_off;
                     ku[u] = ldg_nc_16(p.k_cache + off);
                     vu[u] = ldg_nc_16(p.v_cache + off);

@@ -47,7 +47,6 @@ constexpr int kComputeWarps = 8;
 constexpr int kPlanBar = 9;         // named barrier: planner warp -> producer 0 (1..8 belong to the head groups)
 constexpr int kRing = 4;            // unit ring between producer 0 and everybody else
 constexpr int kMaxStages = 24;
-constexpr int kMaxFusedRows = 512;  // fused build: the batch's offsets and lengths sit in shared memory
 
 __host__ __device__ constexpr int producers_for(int HG) { return HG >= 4 ? 1 : (HG == 2 ? 2 : 4); }
 
@@ -108,7 +107,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     const uint32_t rfull0 = smem_u32(&tail.ring_full[0]);
     const uint32_t rempty0 = smem_u32(&tail.ring_empty[0]);
 
-    if (tid == 0) trace_stamp(p, 0);
+    if (tid == 0) PKV_TRACE_STAMP(p, 0);
     pdl_launch_dependents();
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) {
@@ -146,7 +145,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         __syncwarp();
     }
     pdl_wait();   // queue (builder), q / seq_lens (upstream), out / partials (previous step's readers)
-    if (tid == 0) trace_stamp(p, 1);
+    if (tid == 0) PKV_TRACE_STAMP(p, 1);
     if (warp == kPlanWarp) {
         // ================================================================ planner warp
         // Fused build: producer 0 derives split_offsets from seq_lens
@@ -177,11 +176,16 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     p.hdr->resolved_splits = plan.S;
                     p.hdr->chunk_tiles = plan.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : plan.chunk_tiles;
                     p.hdr->empty_tasks = (tot.row_slots - tot.sum_n) * p.Hkv;
-                    p.hdr->error_word = total > p.tasks_cap ? 1 : 0;
+                    if (total > p.tasks_cap) atomicOr(&p.hdr->error_word, (int32_t)PKV_DEVERR_QUEUE_OVERFLOW);
                     p.hdr->sum_seq_lens = tot.sum_seq;
                     p.hdr->build_launches = 0;
+                    p.hdr->launched_build = 0;
                 }
             }
+        }
+        if (blockIdx.x == 0 && lane == 0) {   // this launch's mark (pkv_counters.launched_*)
+            p.hdr->launched_decode = 1;
+            p.hdr->launched_merge = 0;
         }
         for (int i = blockIdx.x; i < p.B; i += gridDim.x) {   // rows without a task (A9)
             if ((p.fused_build ? tail.len_s[i] : __ldcg(p.seq_lens + i)) > 0) continue;
@@ -196,17 +200,18 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         // Producer 0 plans for itself -- the plan is on the critical path of the first TMA load --
         // and leaves it in shared memory for the planner warp, which writes the queue.
         int32_t row_slots = spec_row_slots;
-        if (!p.force_replan && plan_lens_unchanged(plan, p.seq_lens, tail.len_s, lane)) {
+        int32_t* const err = blockIdx.x == 0 ? &p.hdr->error_word : nullptr;   // one CTA reports bad lengths
+        if (!p.force_replan && plan_lens_unchanged(plan, p.seq_lens, tail.len_s, lane, err)) {
             plan = spec_plan;
         } else {
             __syncwarp();
             row_slots = plan_warp_prefix(plan, p.seq_lens, tail.so_s, tail.len_s, lane, (int)blockIdx.x / HGn,
-                                         &tail.first_slot);
+                                         &tail.first_slot, err);
         }
         if (lane == 0) {
             tail.plan_row_slots = row_slots;
             tail.plan_chunk = plan.chunk_tiles;
-            trace_stamp(p, 8);
+            PKV_TRACE_STAMP(p, 8);
         }
         __syncwarp();
         named_bar_arrive(kPlanBar, 64);
@@ -278,7 +283,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         for (int k = 0;; ++k) {
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
-            if (k == 0 && tid == 0) trace_stamp(p, 2);
+            if (k == 0 && tid == 0) PKV_TRACE_STAMP(p, 2);
             const int row = u.row, hg = u.unit % HGn;
             const int tok0 = u.tok0, tok1 = u.tok1;
             if (tok0 >= tok1) continue;  // empty split: nothing is staged
@@ -287,9 +292,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             const int head0 = hg * HG;
             const int32_t* bt = p.block_table + (int64_t)row * p.max_pages + p0;
             // table entries 32 at a time (lane i holds page c + i of the unit)
-            int mine = lane < np ? bt[lane] : 0;
+            int mine = lane < np ? checked_page(bt[lane], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
             for (int c = 0; c < np; c += 32) {
-                const int nxt = (c + 32 + lane < np) ? bt[c + 32 + lane] : 0;
+                const int nxt = (c + 32 + lane < np)
+                                    ? checked_page(bt[c + 32 + lane], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
                 const int cnt = min(32, np - c);
                 for (int i = 0; i < cnt; ++i) {
                     const int page = __shfl_sync(0xffffffffu, mine, i);
@@ -297,7 +303,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     if (++ps == (uint32_t)kStages) { ps = 0; pphase ^= 1; }
                     if ((s % NP) != (uint32_t)warp) continue;
                     if (lane == 0) {
-                        if (k == 0 && c == 0 && i == 0 && warp == 0) trace_stamp(p, 3 + (page & 0));
+                        if (k == 0 && c == 0 && i == 0 && warp == 0) PKV_TRACE_STAMP(p, 3);
                         mbar_wait(empty0 + 8 * s, par ^ 1);
                         const uint32_t dst = stage_base + s * kStageBytes;
                         // box dims: (64 ch, 16 tok, 2 ch-halves, HG heads, 1 page)
@@ -312,7 +318,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         }
         // the last CTA to run out of units re-arms the counters for the next launch / replay
         if (warp == 0 && lane == 0) {
-            trace_stamp(p, 7);
+            PKV_TRACE_STAMP(p, 7);
             const int old = atomicAdd(&p.hdr->done_counter, 1);
             if (old == (int)gridDim.x - 1) {
                 p.hdr->work_counter = 0;
@@ -389,7 +395,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
 
                 // ---- S^T = K . Q^T, two accumulation chains (channel halves)
                 mbar_wait(fullk0 + 8 * s, par);
-                if (k == 0 && first_page && cw == 0 && lane == 0) trace_stamp(p, 4);
+                if (k == 0 && first_page && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 4);
                 first_page = false;
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -466,7 +472,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 if (s + WPH < (uint32_t)kStages) { s += WPH; j += WPH; }
                 else { j += (int)((uint32_t)kStages - s) + sub; s = (uint32_t)sub; par ^= 1; }
             }
-            if (k == 0 && cw == 0 && lane == 0) trace_stamp(p, 5);
+            if (k == 0 && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 5);
 
             // ---- warp state -> combine buffer row cw
 #pragma unroll
@@ -542,7 +548,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 group_sync<WPH>(1 + hl);
                 finalize_task<G, WPH, kComputeWarps>(p, tail.cb, hl, HG, row, kvh, split, n_i, slot, gtid, 1 + hl);
             }
-            if (k == 0 && cw == 0 && lane == 0) trace_stamp(p, 6);
+            if (k == 0 && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 6);
         }
     }
 }
@@ -552,11 +558,16 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
                        cudaStream_t stream) {
     constexpr int smem = stages_for<G, HG>() * HG * 8192 + (int)sizeof(SmemTail<G>) + 1024;
     constexpr int threads = (producers_for(HG) + kComputeWarps + 1) * 32;
-    static bool attr_set = false;
-    if (!attr_set) {
-        const cudaError_t e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    // The dynamic shared-memory opt-in is a per-device (per-context) attribute of the kernel: one
+    // flag per device ordinal, set on the first launch there (races only repeat the call).
+    static bool attr_set[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !attr_set[dev]) {
+        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
     return launch_pdl(pkv_decode_tma_kernel<G, HG>, dim3(grid), dim3(threads), (size_t)smem, stream, p, mk, mv);
 }

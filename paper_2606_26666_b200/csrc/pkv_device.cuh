@@ -17,6 +17,8 @@ constexpr float kLn2 = 0.6931471805599453f;
 
 struct PlanArgs {   // split policy as the device-side planner needs it
     int32_t B, Hkv, S, tile_tokens, split_mode, chunk_tiles, route, num_sms;
+    int32_t flags;        // pkv_flag bits
+    int32_t max_tokens;   // max_pages * page_size: the longest row the block table can describe
 };
 
 struct DecodeParams {
@@ -45,7 +47,10 @@ struct DecodeParams {
     int32_t force_replan;       // test hook: treat the speculative plan as invalidated
     float scale;                // x = scale * <q, k>
     float scale_log2;           // scale * log2(e)
-    unsigned long long* trace;  // debug: [grid][16] %globaltimer stamps, or nullptr (pkv_debug_set_trace)
+    int64_t num_pages;          // PKV_FLAG_VALIDATE: block-table entries must lie in [0, num_pages)
+#ifdef PKV_TRACE
+    unsigned long long* trace;  // trace build only: [grid][16] %globaltimer stamps, or nullptr
+#endif
 };
 
 // ------------------------------------------------------------------ small PTX wrappers
@@ -73,6 +78,9 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// Phase stamps (%globaltimer) for the step timeline: compiled in only with -DPKV_TRACE (a separate
+// trace build of the library); the release build carries no stamp, no pointer and no hook.
+#ifdef PKV_TRACE
 __device__ __forceinline__ void trace_stamp(const DecodeParams& p, int slot) {
     if (p.trace) {
         unsigned long long t;
@@ -80,6 +88,10 @@ __device__ __forceinline__ void trace_stamp(const DecodeParams& p, int slot) {
         p.trace[(size_t)blockIdx.x * 16 + slot] = t;
     }
 }
+#define PKV_TRACE_STAMP(p, slot) trace_stamp(p, slot)
+#else
+#define PKV_TRACE_STAMP(p, slot) ((void)0)
+#endif
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
@@ -173,6 +185,26 @@ __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
 // (PAPER.md:63-75).  Shared by the builder kernel (pkv_aux.cu) and by the decode kernel's fused
 // build (pkv_decode_tma.cu): same integer formulas as the host planner (pkv_common.h row_splits).
 
+// A row's length as the planner uses it: negative counts as empty; with PKV_FLAG_VALIDATE a length
+// the block table cannot describe is clamped to max_tokens (and reported, plan_len_fault).
+__device__ __forceinline__ int32_t plan_len(const PlanArgs& a, int32_t N) {
+    N = max(N, 0);
+    if ((a.flags & PKV_FLAG_VALIDATE) && N > a.max_tokens) N = a.max_tokens;
+    return N;
+}
+__device__ __forceinline__ void plan_len_fault(const PlanArgs& a, int32_t N, int32_t* error_word) {
+    if (error_word && (a.flags & PKV_FLAG_VALIDATE) && N > a.max_tokens) atomicOr(error_word, (int32_t)PKV_DEVERR_SEQ_LEN);
+}
+// A block-table entry as the kernels use it: with PKV_FLAG_VALIDATE an id outside [0, num_pages)
+// is reported and replaced by page 0 (the pool is never read out of bounds).
+__device__ __forceinline__ int32_t checked_page(int32_t page, int32_t flags, int64_t num_pages, int32_t* error_word) {
+    if ((flags & PKV_FLAG_VALIDATE) && (page < 0 || (int64_t)page >= num_pages)) {
+        atomicOr(error_word, (int32_t)PKV_DEVERR_PAGE_ID);
+        return 0;
+    }
+    return page;
+}
+
 struct PlanScratch {   // shared memory of the calling CTA
     int32_t warp_sums[32];
     int32_t carry, max_n, sum_n;
@@ -192,7 +224,7 @@ struct PlanTotals {
 __device__ __forceinline__ int32_t balanced_chunk_warp(const PlanArgs& a, const int32_t* lens, int lane) {
     long long W64 = 0;
     for (int i = lane; i < a.B; i += 32) {
-        const int N = lens[i];
+        const int N = plan_len(a, lens[i]);
         if (N > 0) W64 += (unsigned)(N + a.tile_tokens - 1) / (unsigned)a.tile_tokens;
     }
     if (__any_sync(0xffffffffu, W64 >= (1 << 26))) {   // 32 lanes x 2^26 < 2^31: else one redux.sync
@@ -207,7 +239,7 @@ __device__ __forceinline__ int32_t balanced_chunk_warp(const PlanArgs& a, const 
         const unsigned span = span64 >= 0x7fffffffull ? 0x7fffffffu : (unsigned)span64;
         unsigned units = 0;
         for (int i = first; i < a.B; i += step) {
-            const int N = lens[i];
+            const int N = plan_len(a, lens[i]);
             if (N > 0) units += ((unsigned)N + span - 1u) / span;
         }
         return units;
@@ -254,12 +286,12 @@ __device__ __forceinline__ int32_t balanced_chunk_warp(const PlanArgs& a, const 
 // BALANCED: resolves the batch-wide chunk first and rewrites `a` to the FIXED_CHUNK policy it
 // stands for (a.chunk_tiles = the chunk), which make_rowslot then uses.
 __device__ __forceinline__ PlanTotals plan_scan(PlanArgs& a, const int32_t* seq_lens, int32_t* so_out,
-                                                int32_t* len_out, PlanScratch& sc) {
+                                                int32_t* len_out, PlanScratch& sc, int32_t* error_word) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nthreads = blockDim.x, nwarps = nthreads >> 5;
     const int32_t* lens = seq_lens;
     if (len_out) {   // one global round trip: stage the lengths, plan from the staged copy
-        for (int i = tid; i < a.B; i += nthreads) len_out[i] = max(__ldcg(seq_lens + i), 0);
+        for (int i = tid; i < a.B; i += nthreads) len_out[i] = plan_len(a, __ldcg(seq_lens + i));
         lens = len_out;
     }
     if (tid == 0) {
@@ -278,7 +310,8 @@ __device__ __forceinline__ PlanTotals plan_scan(PlanArgs& a, const int32_t* seq_
         const int i = base + tid;
         int32_t slots = 0, N = 0, nonempty = 0;
         if (i < a.B) {
-            N = max(lens[i], 0);
+            plan_len_fault(a, seq_lens[i], error_word);
+            N = plan_len(a, lens[i]);
             const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
             nonempty = r.n;
             slots = a.route == PKV_ROUTE_WORKQUEUE ? r.n : a.S;
@@ -335,10 +368,14 @@ __device__ __forceinline__ int32_t ld_relaxed_s32(const int32_t* ptr) {
 }
 template <bool SPEC = false>
 __device__ __forceinline__ int32_t plan_warp_prefix(PlanArgs& a, const int32_t* seq_lens, int32_t* so_out,
-                                                    int32_t* len_out, int lane, int rs0, RowSlot* first) {
+                                                    int32_t* len_out, int lane, int rs0, RowSlot* first,
+                                                    int32_t* error_word = nullptr) {
 #pragma unroll 4
-    for (int i = lane; i < a.B; i += 32)
-        len_out[i] = max(SPEC ? ld_relaxed_s32(seq_lens + i) : __ldcg(seq_lens + i), 0);
+    for (int i = lane; i < a.B; i += 32) {
+        const int32_t N = SPEC ? ld_relaxed_s32(seq_lens + i) : __ldcg(seq_lens + i);
+        if (!SPEC) plan_len_fault(a, N, error_word);
+        len_out[i] = plan_len(a, N);
+    }
     if (lane == 0) so_out[0] = 0;
     __syncwarp();
     if (a.split_mode == PKV_SPLIT_BALANCED) {
@@ -388,9 +425,13 @@ __device__ __forceinline__ int32_t plan_warp_prefix(PlanArgs& a, const int32_t* 
 // After the dependency wait: are the lengths a speculative plan was made from (len_s) still the
 // ones in memory?  Every lane returns the answer.
 __device__ __forceinline__ bool plan_lens_unchanged(const PlanArgs& a, const int32_t* seq_lens, const int32_t* len_s,
-                                                    int lane) {
+                                                    int lane, int32_t* error_word = nullptr) {
     bool same = true;
-    for (int i = lane; i < a.B; i += 32) same &= max(__ldcg(seq_lens + i), 0) == len_s[i];
+    for (int i = lane; i < a.B; i += 32) {
+        const int32_t N = __ldcg(seq_lens + i);
+        plan_len_fault(a, N, error_word);
+        same &= plan_len(a, N) == len_s[i];
+    }
     return __all_sync(0xffffffffu, same);
 }
 
@@ -433,7 +474,7 @@ __device__ __forceinline__ RowSlot make_rowslot(const PlanArgs& a, const int32_t
     d.so = so[lo];
     d.n = so[lo + 1] - d.so;
     d.split = rs - d.so;
-    const int32_t N = max(lens[lo], 0);
+    const int32_t N = plan_len(a, lens[lo]);
     const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
     int32_t tb = 0, te = 0;
     if (r.T > 0) {
@@ -689,6 +730,9 @@ inline PlanArgs make_plan_args(const pkv_shape& shape, const Resolved& rp) {
     PlanArgs a;
     a.B = shape.B; a.Hkv = shape.Hkv; a.S = rp.S; a.tile_tokens = rp.tile_tokens;
     a.split_mode = rp.split_mode; a.chunk_tiles = rp.chunk_tiles; a.route = rp.route; a.num_sms = rp.num_sms;
+    a.flags = rp.flags;
+    const int64_t mt = (int64_t)shape.max_pages * shape.page_size;
+    a.max_tokens = (int32_t)(mt < 0x7fffffff ? mt : 0x7fffffff);
     return a;
 }
 

@@ -65,6 +65,7 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     if (p.merge_mode != PKV_MERGE_SEPARATE && p.merge_mode != PKV_MERGE_FUSED) { set_error("bad merge_mode %d", p.merge_mode); return PKV_ERR_INVALID_ARG; }
     if (p.kernel < PKV_KERNEL_AUTO || p.kernel > PKV_KERNEL_SIMT) { set_error("bad kernel %d", p.kernel); return PKV_ERR_INVALID_ARG; }
     if (p.num_sms < 0) { set_error("num_sms < 0"); return PKV_ERR_INVALID_ARG; }
+    if (p.flags & ~(int32_t)PKV_FLAG_VALIDATE) { set_error("unknown policy flag bits 0x%x", p.flags); return PKV_ERR_INVALID_ARG; }
 
     int32_t S = p.num_splits;
     out->num_sms = p.num_sms > 0 ? p.num_sms : num_sms_or_0;
@@ -97,6 +98,7 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     out->merge_mode = p.merge_mode;
     out->kernel = p.kernel == PKV_KERNEL_AUTO ? PKV_KERNEL_TMA_MMA : p.kernel;
     out->G = G;
+    out->flags = p.flags;
     return PKV_OK;
 }
 
@@ -197,7 +199,7 @@ using namespace pkv;
 
 extern "C" {
 
-int32_t pkv_version(void) { return (1 << 16) | 0; }
+int32_t pkv_version(void) { return (2 << 16) | 0; }
 const char* pkv_last_error(void) { return g_error; }
 
 size_t pkv_workspace_bytes(const pkv_shape* shape, const pkv_split_policy* policy) {

@@ -31,11 +31,11 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_version_and_struct_sizes():
-    assert pkv.pkv_version() == (1 << 16)
+    assert pkv.pkv_version() >> 16 == 2
     assert ctypes.sizeof(binding.pkv_task) == 20            # 5 x int32
-    assert ctypes.sizeof(binding.pkv_split_policy) == 32
+    assert ctypes.sizeof(binding.pkv_split_policy) == 36
     assert ctypes.sizeof(binding.pkv_shape) == 56
-    assert ctypes.sizeof(binding.pkv_counters) == 96
+    assert ctypes.sizeof(binding.pkv_counters) == 128
 
 
 def shape(B, Hkv=8, Hq=32, max_pages=4096):
@@ -60,7 +60,7 @@ def test_shape_validation(bad, status):
 
 @pytest.mark.parametrize("bad", [dict(tile_tokens=24), dict(tile_tokens=0), dict(num_splits=257),
                                  dict(split_mode=3), dict(split_mode=2, num_sms=0), dict(route=3), dict(merge_mode=2), dict(kernel=9),
-                                 dict(split_mode=1, chunk_tiles=0), dict(num_splits=0, num_sms=0)])
+                                 dict(split_mode=1, chunk_tiles=0), dict(num_splits=0, num_sms=0), dict(flags=1 << 20)])
 def test_policy_validation(bad):
     with pytest.raises(pkv.PkvError) as e:
         pkv.pkv_build_workqueue_host(shape(1), pkv.Policy(**bad), np.array([100], np.int32))

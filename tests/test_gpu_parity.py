@@ -531,7 +531,11 @@ def _compact_rows(w, k_dev, v_dev, rows, lens):
     return np.concatenate(ks), np.concatenate(vs), np.stack(tables)
 
 
-@pytest.mark.parametrize("name", ["config2", "config3", "config4_b4", "config5"])
+FULL_SIZE_CASES = ["config2", "config3", "config3_rect", "config3_fused", "config4", "config4_b4", "config5",
+                   "config5_hkv4"]
+
+
+@pytest.mark.parametrize("name", FULL_SIZE_CASES)
 def test_full_size_configs_in_the_bench_configuration(name):
     """BASELINE.json's full sizes with the policies bench.py times (config 2: the sweep's
     FIXED_COUNT S=16 and BALANCED; others: BALANCED, page-granular tiles), seeded device pools as in
@@ -540,7 +544,10 @@ def test_full_size_configs_in_the_bench_configuration(name):
     the whole batch is bit-exact; token coverage at full size is pinned by lse = log-sum-exp."""
     import pkv_inputs as pi
     from oracle import pkv_oracle
-    w = {"config2": pi.config2, "config3": pi.config3, "config4_b4": pi.config4_b4, "config5": pi.config5}[name](pi.REPORT_SEEDS[0])
+    seed = pi.REPORT_SEEDS[0]
+    w = {"config2": pi.config2, "config3": pi.config3, "config3_rect": pi.config3, "config3_fused": pi.config3,
+         "config4": pi.config4, "config4_b4": pi.config4_b4, "config5": pi.config5,
+         "config5_hkv4": lambda s_: pi.config5(s_, Hkv=4)}[name](seed)
     dev = torch.device("cuda", 0)
     q = pi.fill_pool_torch((w.B, w.Hq, w.d), 11, dev)
     k = pi.fill_pool_torch(w.pool_shape(), 12, dev)
@@ -552,10 +559,18 @@ def test_full_size_configs_in_the_bench_configuration(name):
     pols = [pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0)]
     if name == "config2":
         pols.append(pkv.Policy(tile_tokens=32, num_splits=16))
+        pols.append(pkv.Policy(tile_tokens=32, num_splits=16, merge_mode=pkv.MERGE_FUSED))
+    if name == "config3_rect":      # BASELINE.json configs[2]: the rectangular (B, Hkv, S) grid
+        pols = [pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_RECT),
+                pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_WORKQUEUE)]
+    if name == "config3_fused":     # fused last-CTA merge at full size
+        pols = [pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, merge_mode=pkv.MERGE_FUSED),
+                pkv.Policy(tile_tokens=32, num_splits=20, merge_mode=pkv.MERGE_FUSED)]
     if w.B <= 8:
         rows = list(range(w.B))
-    else:
-        rows = sorted({int(np.argmin(lens)), int(np.argmax(lens)), 5, 77})
+    else:           # config 5: shortest, longest and 16 seeded rows of the 128
+        pick = np.random.Generator(np.random.PCG64(seed)).choice(w.B, size=16, replace=False)
+        rows = sorted({int(np.argmin(lens)), int(np.argmax(lens))} | {int(x) for x in pick})
     kc, vc, tc = _compact_rows(w, k, v, rows, lens)
     scale = default_scale(w.d)
     ref, ref_lse = pkv_oracle.attention(np.ascontiguousarray(q.cpu().numpy()[rows]), kc, vc, tc,
