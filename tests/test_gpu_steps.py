@@ -95,6 +95,15 @@ def test_validate_flag_reports_bad_lengths_and_page_ids():
                 bad[1] = max_tokens + 1234
                 dp.sl.copy_(to_dev(bad))
                 out, _, ws = dp.decode(pol)
+                # the row is decoded as if it had max_tokens tokens, so its padding entries are
+                # dereferenced too (and replaced by page 0): both bits
+                assert pkv.pkv_get_counters(dp.shape, pol, ws)["error_word"] == pkv.DEVERR_SEQ_LEN | pkv.DEVERR_PAGE_ID
+                assert_within_tolerance(out[[0, 2]], ref[[0, 2]])
+                # the same with a table row that is valid end to end: the length fault alone
+                bt = p.block_table.copy()
+                bt[1, :] = bt[1, 0]
+                dp.bt.copy_(to_dev(bt))
+                out, _, ws = dp.decode(pol)
                 assert pkv.pkv_get_counters(dp.shape, pol, ws)["error_word"] == pkv.DEVERR_SEQ_LEN
                 assert_within_tolerance(out[[0, 2]], ref[[0, 2]])
                 # row 2 points at a page outside the pool (row 1 keeps its padding entries unread)
