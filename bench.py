@@ -34,6 +34,7 @@ step finds its K/V in L2 ("inputs larger than L2").
 from __future__ import annotations
 
 import argparse
+import dataclasses
 import json
 import math
 import os
@@ -73,7 +74,8 @@ def parse_args(argv=None):
     ap.add_argument("--route", type=int, default=-1)
     ap.add_argument("--merge", type=int, default=-1)
     ap.add_argument("--kernel", type=int, default=-1)
-    ap.add_argument("--hg", type=int, default=0, help="force KV heads per CTA (test hook)")
+    ap.add_argument("--hg", type=int, default=0, help="policy.heads_per_cta (0 = automatic)")
+    ap.add_argument("--prefetch-kb", type=int, default=0, help="policy.prefetch_kb (0 = library default, < 0 = off)")
     ap.add_argument("--graph-steps", type=int, default=100, help="decode steps per CUDA graph (configs[1]: 100)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the split-count sweep on the tune seed")
     ap.add_argument("--no-others", action="store_true", help="skip config.other_workloads")
@@ -143,6 +145,10 @@ def default_policy(pkv, name: str, args):
         pol.merge_mode = args.merge
     if args.kernel >= 0:
         pol.kernel = args.kernel
+    if args.hg:
+        pol.heads_per_cta = args.hg
+    if args.prefetch_kb != 0:
+        pol.prefetch_kb = args.prefetch_kb
     return pol
 
 
@@ -592,10 +598,12 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
     PAPER.md:71, 204-206): us/step (median of >= 50 ms of K-step regions), roofline fraction of the
     decode kernel, launches per step, parity against the oracle on seeded rows."""
     out = {}
-    bal = pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0)
+    bal = pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, prefetch_kb=args.prefetch_kb)
     cases = [("config3", "config3", bal),
-             ("config3_workqueue_S20", "config3", pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_WORKQUEUE)),
-             ("config3_rect_S20", "config3", pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_RECT)),
+             ("config3_workqueue_S20", "config3", pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_WORKQUEUE,
+                                                             prefetch_kb=args.prefetch_kb)),
+             ("config3_rect_S20", "config3", pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_RECT,
+                                                        prefetch_kb=args.prefetch_kb)),
              ("config4", "config4", bal), ("config4_b4", "config4_b4", bal),
              ("config5", "config5", bal), ("config5_hkv4", "config5_hkv4", bal)]
     runner, cur = None, None
@@ -613,9 +621,9 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
             r = time_policy(pkv, runner, pol, K, chunk, 5)
             st, dc = summarize(r["step_ms"], K), summarize(r["decode_ms"], K)
             alg = mean_alg_bytes(w, K, runner.nlens)
-            c = runner.counters()
             rows = pick_rows(runner.lens_at(0), 70000, w.seed)
             par, _ = parity_of(torch, runner, rows)
+            c = runner.counters()      # after a whole eager step
             out[key] = {"workload": w.name, "policy": {k: int(v) for k, v in pol.__dict__.items()},
                         "steps": K, "us_per_step": round(st["us_per_step_median"], 3),
                         "us_per_step_min": round(st["us_per_step_min"], 3), "regions": st["regions"],
@@ -689,12 +697,11 @@ def sweep_on_tune_seed(pkv, torch, args, device, base_pol, K, W):
     w = make_workload(args.workload, pkv_inputs.TUNE_SEED, args.hkv)
     runner = Runner(pkv, torch, w, base_pol, rotation(torch, w, args, device), pkv_inputs.TUNE_SEED, device)
     sms = torch.cuda.get_device_properties(device).multi_processor_count
-    cands = [(str(S), pkv.Policy(tile_tokens=32, num_splits=S, route=base_pol.route, merge_mode=base_pol.merge_mode,
-                                 kernel=base_pol.kernel)) for S in (1, 4, 16, 64, 0)] + [("balanced", base_pol)]
+    fixed = lambda S: dataclasses.replace(base_pol, tile_tokens=32, split_mode=pkv.SPLIT_FIXED_COUNT, num_splits=S)
+    cands = [(str(S), fixed(S)) for S in (1, 4, 16, 64, 0)] + [("balanced", base_pol)]
     s_fit = sms // max(1, w.B * w.Hkv)
     if s_fit > 1 and s_fit not in (4, 16, 64):
-        cands.append((str(s_fit), pkv.Policy(tile_tokens=32, num_splits=s_fit, route=base_pol.route,
-                                             merge_mode=base_pol.merge_mode, kernel=base_pol.kernel)))
+        cands.append((str(s_fit), fixed(s_fit)))
     Ks = min(K, 2 * args.graph_steps)
     chunk = max(1, min(args.graph_steps, Ks))
     table, pols = {}, {}
@@ -729,8 +736,6 @@ def run_ours(args):
     device = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
-    if args.hg:
-        pkv.pkv_debug_force_heads_per_cta(args.hg)
     K, W = args.steps, max(args.warmup, 3)
     peak, peak_src = measured_hbm_peak()
 

@@ -94,6 +94,12 @@ typedef struct {
                             (device calls only; the host builder needs it > 0 then)             */
     int32_t kernel;      /* pkv_kernel                                                           */
     int32_t flags;       /* bit set of pkv_flag                                                  */
+    int32_t heads_per_cta; /* TMA kernel: KV heads one CTA streams together:
+                            0 = automatic (the largest of 8/4/2/1 dividing Hkv that leaves one work
+                            unit per SM), else 1, 2, 4 or 8 and a divisor of Hkv                  */
+    int32_t prefetch_kb; /* TMA kernel: KiB of its first work unit's K/V that every CTA requests into
+                            L2 BEFORE its dependency wait (programmatic launch; DESIGN.md "L2
+                            prefetch"): 0 = library default, < 0 = off                            */
 } pkv_split_policy;
 
 /* policy.flags */
@@ -103,7 +109,17 @@ typedef enum {
      * and sets PKV_DEVERR_SEQ_LEN; a block-table entry outside [0, num_pages) that a task would
      * dereference is replaced by page 0 and sets PKV_DEVERR_PAGE_ID.  The kernels then never read
      * outside the block table or the page pool; the result of a faulted row is unspecified. */
-    PKV_FLAG_VALIDATE = 1
+    PKV_FLAG_VALIDATE = 1,
+    /* Launch the kernels of this call without programmatic dependent launch: every
+     * kernel then starts after its predecessor in the stream has finished. */
+    PKV_FLAG_NO_PDL = 2,
+    /* Run the workqueue builder as its own kernel even where the TMA decode kernel could derive the
+     * queue itself. */
+    PKV_FLAG_SEPARATE_BUILD = 4,
+    /* Test only: the TMA decode kernel discards the plan it made speculatively before its dependency
+     * wait and plans again afterwards -- the path taken when the kernel right before pkv_decode wrote
+     * seq_lens. */
+    PKV_FLAG_TEST_REPLAN = 8
 } pkv_flag;
 /* bits of pkv_counters.error_word (sticky in the workspace until its init bytes are zeroed again) */
 typedef enum { PKV_DEVERR_QUEUE_OVERFLOW = 1, PKV_DEVERR_SEQ_LEN = 2, PKV_DEVERR_PAGE_ID = 4 } pkv_device_error;
@@ -197,7 +213,13 @@ PKV_API pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_p
  * predecessor that writes seq_lens, q, the block table or the caches is handled correctly.
  * Heads per CTA: the TMA kernel streams HG = 8, 4, 2 or 1 KV heads per CTA, the largest value
  * that still leaves one work unit per SM given the bound B*S on the (row, split) pairs; with
- * BALANCED the bound is policy.num_sms, so num_sms = SMs*HG/Hkv asks for HG heads per CTA.
+ * BALANCED the bound is policy.num_sms, so num_sms = SMs*HG/Hkv asks for HG heads per CTA
+ * (policy.heads_per_cta overrides the choice).
+ * L2 prefetch: before its dependency wait a CTA of the TMA kernel also asks the memory system to
+ * bring the first policy.prefetch_kb KiB of its first work unit's K/V (found through the speculative
+ * plan and a race-tolerant look at the block table) into L2.  A prefetch moves no data into the
+ * program: L2 is the point of coherence, so whatever the predecessor kernel still writes is seen by
+ * the loads after the wait; a wrong guess only costs bandwidth.
  */
 PKV_API pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
                               const void* k_cache, const void* v_cache, const int32_t* block_table,
@@ -288,20 +310,6 @@ typedef struct {
     int32_t num_sms, l2_bytes;
 } pkv_calibration;
 PKV_API pkv_status pkv_calibrate(void* dev_buffer, size_t bytes, void* stream, pkv_calibration* out);
-
-/* Test hook: KV heads one CTA of the TMA kernel streams together.
- * 0 = automatic (largest of 8/4/2/1 dividing Hkv that leaves >= one work unit per SM), else
- * 1, 2, 4 or 8 (ignored when it does not divide Hkv).  Process-wide. */
-PKV_API void pkv_debug_force_heads_per_cta(int heads);
-/* Test hook: 0 launches the kernels without programmatic dependent launch. Process-wide. */
-PKV_API void pkv_debug_set_pdl(int on);
-/* Test hook: 0 makes pkv_decode run the builder as its own kernel even where the TMA decode kernel
- * could derive the queue itself.  Process-wide. */
-PKV_API void pkv_debug_set_fused_build(int on);
-/* Test hook: non-zero makes the TMA decode kernel discard the plan it made speculatively before its
- * dependency wait and plan again afterwards -- the path taken when the kernel right before
- * pkv_decode wrote seq_lens.  Process-wide. */
-PKV_API void pkv_debug_force_replan(int on);
 
 #ifdef __cplusplus
 }

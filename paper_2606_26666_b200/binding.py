@@ -22,7 +22,7 @@ ROUTE_RECT, ROUTE_WORKQUEUE = 0, 1
 MERGE_SEPARATE, MERGE_FUSED = 0, 1
 SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK, SPLIT_BALANCED = 0, 1, 2
 KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
-FLAG_VALIDATE = 1
+FLAG_VALIDATE, FLAG_NO_PDL, FLAG_SEPARATE_BUILD, FLAG_TEST_REPLAN = 1, 2, 4, 8
 DEVERR_QUEUE_OVERFLOW, DEVERR_SEQ_LEN, DEVERR_PAGE_ID = 1, 2, 4
 STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL = 1, 2, 4, 7
 
@@ -32,7 +32,8 @@ _vp = ctypes.c_void_p
 
 class pkv_split_policy(ctypes.Structure):
     _fields_ = [("tile_tokens", _i32), ("split_mode", _i32), ("num_splits", _i32), ("chunk_tiles", _i32),
-                ("route", _i32), ("merge_mode", _i32), ("num_sms", _i32), ("kernel", _i32), ("flags", _i32)]
+                ("route", _i32), ("merge_mode", _i32), ("num_sms", _i32), ("kernel", _i32), ("flags", _i32),
+                ("heads_per_cta", _i32), ("prefetch_kb", _i32)]
 
 
 class pkv_task(ctypes.Structure):
@@ -65,7 +66,7 @@ class pkv_calibration(ctypes.Structure):
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspace_init_bytes", "pkv_build_workqueue_host",
            "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
-           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate", "pkv_debug_force_heads_per_cta", "pkv_debug_set_pdl", "pkv_debug_set_fused_build", "pkv_debug_force_replan")
+           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate")
 
 
 class PkvError(RuntimeError):
@@ -113,14 +114,6 @@ def _load() -> ctypes.CDLL:
                                     _vp, _vp, ctypes.c_size_t, _vp, ctypes.c_size_t, _vp, P(pkv_counters)]
     lib.pkv_calibrate.restype = _i32
     lib.pkv_calibrate.argtypes = [_vp, ctypes.c_size_t, _vp, P(pkv_calibration)]
-    lib.pkv_debug_force_heads_per_cta.restype = None
-    lib.pkv_debug_force_heads_per_cta.argtypes = [ctypes.c_int]
-    lib.pkv_debug_set_pdl.restype = None
-    lib.pkv_debug_set_pdl.argtypes = [ctypes.c_int]
-    lib.pkv_debug_set_fused_build.restype = None
-    lib.pkv_debug_set_fused_build.argtypes = [ctypes.c_int]
-    lib.pkv_debug_force_replan.restype = None
-    lib.pkv_debug_force_replan.argtypes = [ctypes.c_int]
     return lib
 
 
@@ -161,10 +154,13 @@ class Policy:
     num_sms: int = 0
     kernel: int = KERNEL_AUTO
     flags: int = 0
+    heads_per_cta: int = 0
+    prefetch_kb: int = 0
 
     def c(self) -> pkv_split_policy:
         return pkv_split_policy(self.tile_tokens, self.split_mode, self.num_splits, self.chunk_tiles, self.route,
-                                self.merge_mode, self.num_sms, self.kernel, self.flags)
+                                self.merge_mode, self.num_sms, self.kernel, self.flags, self.heads_per_cta,
+                                self.prefetch_kb)
 
 
 def _ptr(x) -> Optional[int]:
@@ -311,19 +307,3 @@ def pkv_calibrate(dev_buffer, stream=None) -> dict:
     c = pkv_calibration()
     _check(_lib.pkv_calibrate(_ptr(dev_buffer), _nbytes(dev_buffer), _stream_ptr(stream), ctypes.byref(c)))
     return c.as_dict()
-
-
-def pkv_debug_force_heads_per_cta(heads: int) -> None:
-    _lib.pkv_debug_force_heads_per_cta(int(heads))
-
-
-def pkv_debug_set_pdl(on: bool) -> None:
-    _lib.pkv_debug_set_pdl(1 if on else 0)
-
-
-def pkv_debug_force_replan(on: bool) -> None:
-    _lib.pkv_debug_force_replan(1 if on else 0)
-
-
-def pkv_debug_set_fused_build(on: bool) -> None:
-    _lib.pkv_debug_set_fused_build(1 if on else 0)

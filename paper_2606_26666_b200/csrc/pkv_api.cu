@@ -12,16 +12,11 @@
 
 namespace pkv {
 
-bool g_use_pdl = true;  // test hook (pkv_debug_set_pdl)
-
 namespace {
 
 #ifdef PKV_TRACE
 unsigned long long* g_trace = nullptr;  // trace build only (pkv_debug_set_trace)
 #endif
-bool g_fused_build = true;              // test hook (pkv_debug_set_fused_build)
-int g_force_hg = 0;  // test hook: 0 = automatic heads-per-CTA, else 1/2/4/8
-bool g_force_replan = false;  // test hook (pkv_debug_force_replan)
 
 int device_sm_count() {
     thread_local int cache[64];
@@ -122,8 +117,8 @@ const CUtensorMap* get_map(const void* base, const pkv_shape& s, int HG) {
 
 // KV heads one CTA streams together: the largest divisor of Hkv in {8, 4, 2, 1} that still
 // leaves at least one work unit per SM (units = row slots x Hkv / HG).
-int choose_heads_per_cta(int Hkv, int64_t row_slots, int num_sms) {
-    if (g_force_hg > 0 && Hkv % g_force_hg == 0) return g_force_hg;
+int choose_heads_per_cta(int forced, int Hkv, int64_t row_slots, int num_sms) {
+    if (forced > 0 && Hkv % forced == 0) return forced;
     int best = 1;
     for (int hg = 8; hg >= 1; hg >>= 1) {
         if (hg > Hkv || Hkv % hg) continue;
@@ -199,7 +194,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.B = s.B; p.Hq = s.Hq; p.Hkv = s.Hkv; p.max_pages = s.max_pages;
     p.tile_tokens = rp.tile_tokens; p.merge_mode = rp.merge_mode;
     p.dynamic_sched = 1;
-    p.force_replan = g_force_replan ? 1 : 0;
+    p.force_replan = (rp.flags & PKV_FLAG_TEST_REPLAN) ? 1 : 0;
     p.plan = make_plan_args(s, rp);
     p.tasks_cap = tasks_cap;
     p.fused_build = fused_build ? 1 : 0;
@@ -237,7 +232,8 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             int64_t row_slots = known_slots >= 0 ? known_slots : (int64_t)s.B * rp.S;
             if (known_slots < 0 && rp.split_mode == PKV_SPLIT_BALANCED && rp.num_sms > 0 && rp.num_sms < row_slots)
                 row_slots = rp.num_sms;
-            const int HG = choose_heads_per_cta(s.Hkv, row_slots, num_sms);
+            const int HG = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, row_slots, num_sms);
+            p.prefetch_pages = rp.prefetch_kb * 1024 / (HG * 8192);
             // by value: inserting the V map may evict the cache entry the K pointer refers to
             const CUtensorMap* pk = get_map(k_cache, s, HG);
             CUtensorMap mk_copy, mv_copy;
@@ -295,10 +291,6 @@ using namespace pkv;
 
 extern "C" {
 
-void pkv_debug_force_heads_per_cta(int hg) { g_force_hg = hg; }
-void pkv_debug_set_pdl(int on) { g_use_pdl = on != 0; }
-void pkv_debug_force_replan(int on) { g_force_replan = on != 0; }
-void pkv_debug_set_fused_build(int on) { g_fused_build = on != 0; }
 #ifdef PKV_TRACE
 // Trace build only (python -m paper_2606_26666_b200.build --trace): device buffer of grid*16
 // uint64 that the TMA decode kernel fills with %globaltimer stamps of its phases; NULL = off.
@@ -342,7 +334,7 @@ pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_policy* pol
     cudaStream_t cs = static_cast<cudaStream_t>(stream);
     // The TMA kernel derives the queue itself (fused build) when it runs in the same call;
     // otherwise (builder alone, SIMT kernel, very large batches) the builder kernel runs first.
-    const bool fused = (stages & PKV_STAGE_BUILD) && (stages & PKV_STAGE_DECODE) && g_fused_build &&
+    const bool fused = (stages & PKV_STAGE_BUILD) && (stages & PKV_STAGE_DECODE) && !(rp.flags & PKV_FLAG_SEPARATE_BUILD) &&
                        rp.kernel == PKV_KERNEL_TMA_MMA && shape->B <= kMaxFusedRows;
     if ((stages & PKV_STAGE_BUILD) && !fused) {
         const cudaError_t e = launch_builder(*shape, rp, seq_lens, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,

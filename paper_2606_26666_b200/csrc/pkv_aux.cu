@@ -86,21 +86,45 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
     }
 }
 
-// One CTA of NW warps per (row, query head).  Warp w owns the states w, w + NW, ...
-// of the (row, kvh) slot range; it issues the loads of kMergeBatch of them (m, l and one 16-byte
-// piece of acc per lane) before any arithmetic, so a row of up to NW * kMergeBatch = 128 splits
-// is ONE round trip to L2/HBM, and folds them into an online state (M_w, L_w, A_w) -- the merge
-// of PAPER.md:60-61 is associative, so the per-warp states combine exactly the same way.  Warp 0
-// combines the NW warp states in fixed order (deterministic).  Rows with at most one slot were
-// written directly by the decode kernel.  NW = 2 .. 16 is chosen at launch (launch_merge).
-template <int G, int NW, int MINB>
+// One CTA of NW warps per (row, query head, channel slice); CS = 1, 2 or 4 slices of 128 / CS
+// channels.  A state's slice is read by 32 / CS lanes (16 bytes each), so one load instruction of
+// a warp covers CS states; every lane issues the loads of kMergeBatch states (m, l and its piece
+// of acc) before any arithmetic, so a row of up to NW * kMergeBatch * CS splits is ONE round trip
+// to L2, and folds them into an online state (M, L, A) -- the merge of PAPER.md:60-61 is
+// associative, so the lane states of a warp (shuffles) and the NW warp states (shared memory)
+// combine exactly the same way, in a fixed order (deterministic).  Rows with at most one slot were
+// written directly by the decode kernel.  Slices spread a single long row (B = 1: 32 (row, head)
+// pairs of 128 .. 148 splits) over 128 small CTAs instead of 32 large ones: four times the SMs
+// pull the states out of L2, and 4-warp CTAs fit beside a resident decode CTA, so they are in
+// place -- guess made, waiting -- when the decode grid finishes.  NW and CS are chosen at launch.
+struct MergeState {
+    float M, L;
+    float4 A;
+};
+__device__ __forceinline__ void merge_combine(MergeState& a, float M2, float L2, const float4& A2) {
+    const float nM = fmaxf(a.M, M2);
+    if (nM == -INFINITY) return;                              // both neutral
+    const float w1 = ex2_approx((a.M - nM) * kLog2e);         // exp2(-inf) = 0
+    const float w2 = ex2_approx((M2 - nM) * kLog2e);
+    a.L = fmaf(w2, L2, w1 * a.L);
+    a.A.x = fmaf(w2, A2.x, w1 * a.A.x); a.A.y = fmaf(w2, A2.y, w1 * a.A.y);
+    a.A.z = fmaf(w2, A2.z, w1 * a.A.z); a.A.w = fmaf(w2, A2.w, w1 * a.A.w);
+    a.M = nM;
+}
+
+template <int G, int NW, int CS, int MINB>
 __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodeParams p) {
     constexpr int NB = kMergeBatch;
-    __shared__ float4 sA[NW][32];
+    constexpr int LPS = 32 / CS;          // lanes per state
+    __shared__ float4 sA[NW][LPS];
     __shared__ float sM[NW], sL[NW];
-    const int row = blockIdx.x / p.Hq, h = blockIdx.x % p.Hq;
+    const int slice = blockIdx.x % CS, rh = blockIdx.x / CS;
+    const int row = rh / p.Hq, h = rh % p.Hq;
     const int kvh = h / G, hh = h % G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int sub = lane / LPS, cl = lane % LPS;
+    const int ch = slice * (kD / CS) + cl * 4;   // this lane's four channels
+    if (blockIdx.x == 0 && threadIdx.x == 0) PKV_TRACE_STAMP_MERGE(p, 0);
     pdl_launch_dependents();
     // A guess at the row's slot range, read (race-tolerant) before the decode grid has finished:
     // merge CTAs are resident long before their wait returns, and from one decode step to the
@@ -112,52 +136,70 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
     const int n_g = ld_relaxed_s32(p.split_offsets + row + 1) - so_g;
     const bool guess = p.tasks_cap > 0 && so_g >= 0 && n_g > 1 && ((int64_t)so_g + (int64_t)n_g) * p.Hkv <= p.tasks_cap;
     pdl_wait();
+    if (blockIdx.x == 0 && threadIdx.x == 0) PKV_TRACE_STAMP_MERGE(p, 1);
     if (blockIdx.x == 0 && threadIdx.x == 0 && p.hdr != nullptr) p.hdr->launched_merge = 1;   // this launch's mark
     const int so = __ldcg(p.split_offsets + row);
     const int n = __ldcg(p.split_offsets + row + 1) - so;
-    auto load_batch = [&](int64_t base_, int n_, int s0, float (&mv)[NB], float (&lv)[NB], float4 (&av)[NB]) {
+    // batch b of this warp: states (b * NB * NW + j * NW + warp) * CS + sub, j = 0 .. NB-1
+    auto load_batch = [&](int64_t base_, int n_, int b, float (&mv)[NB], float (&lv)[NB], float4 (&av)[NB]) {
 #pragma unroll
         for (int j = 0; j < NB; ++j) {
-            const int s = s0 + j * NW;
-            const bool ok = s < n_;
-            const int64_t r = (base_ + (ok ? s : 0)) * G + hh;
+            const int s_ = ((b * NB + j) * NW + warp) * CS + sub;
+            const bool ok = s_ < n_;
+            const int64_t r = (base_ + (ok ? s_ : 0)) * G + hh;
             mv[j] = ok ? __ldcg(p.part_m + r) : -INFINITY;
             lv[j] = ok ? __ldcg(p.part_l + r) : 0.f;
-            av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * kD + lane * 4))
+            av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * kD + ch))
                        : make_float4(0.f, 0.f, 0.f, 0.f);
         }
     };
     float mv[NB], lv[NB];
     float4 av[NB];
-    if (guess) load_batch((int64_t)so_g * p.Hkv + (int64_t)kvh * n_g, n_g, warp, mv, lv, av);
+    if (guess) load_batch((int64_t)so_g * p.Hkv + (int64_t)kvh * n_g, n_g, 0, mv, lv, av);
     if (n <= 1 && p.hdr != nullptr) return;   // library path: decode already produced out/lse
     const bool hit = guess && so == so_g && n == n_g;
     const int64_t base = (int64_t)so * p.Hkv + (int64_t)kvh * n;
-    float M = -INFINITY, L = 0.f;
-    float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int s0 = warp; s0 < n; s0 += NW * NB) {
-        if (!(hit && s0 == warp)) load_batch(base, n, s0, mv, lv, av);
+    MergeState st;
+    st.M = -INFINITY; st.L = 0.f; st.A = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int b = 0; b * NB * NW * CS < n; ++b) {
+        if (!(hit && b == 0)) load_batch(base, n, b, mv, lv, av);
         float mb = mv[0];
 #pragma unroll
         for (int j = 1; j < NB; ++j) mb = fmaxf(mb, mv[j]);
-        const float nM = fmaxf(M, mb);
-        if (nM == -INFINITY) continue;        // only neutral states so far (warp-uniform)
-        const float al = ex2_approx((M - nM) * kLog2e);   // M = -inf -> 0
-        L *= al;
-        A.x *= al; A.y *= al; A.z *= al; A.w *= al;
+        const float nM = fmaxf(st.M, mb);
+        if (nM == -INFINITY) continue;        // only neutral states so far
+        const float al = ex2_approx((st.M - nM) * kLog2e);   // M = -inf -> 0
+        st.L *= al;
+        st.A.x *= al; st.A.y *= al; st.A.z *= al; st.A.w *= al;
 #pragma unroll
         for (int j = 0; j < NB; ++j) {
             const float w = ex2_approx((mv[j] - nM) * kLog2e);   // exp2(-inf) = 0
-            L = fmaf(w, lv[j], L);
-            A.x = fmaf(w, av[j].x, A.x); A.y = fmaf(w, av[j].y, A.y);
-            A.z = fmaf(w, av[j].z, A.z); A.w = fmaf(w, av[j].w, A.w);
+            st.L = fmaf(w, lv[j], st.L);
+            st.A.x = fmaf(w, av[j].x, st.A.x); st.A.y = fmaf(w, av[j].y, st.A.y);
+            st.A.z = fmaf(w, av[j].z, st.A.z); st.A.w = fmaf(w, av[j].w, st.A.w);
         }
-        M = nM;
+        st.M = nM;
     }
-    sA[warp][lane] = A;
-    if (lane == 0) { sM[warp] = M; sL[warp] = L; }
+    // the CS lane groups of the warp hold different states of the same channels
+#pragma unroll
+    for (int off = LPS; off < 32; off <<= 1) {
+        const float M2 = __shfl_xor_sync(0xffffffffu, st.M, off), L2 = __shfl_xor_sync(0xffffffffu, st.L, off);
+        float4 A2;
+        A2.x = __shfl_xor_sync(0xffffffffu, st.A.x, off); A2.y = __shfl_xor_sync(0xffffffffu, st.A.y, off);
+        A2.z = __shfl_xor_sync(0xffffffffu, st.A.z, off); A2.w = __shfl_xor_sync(0xffffffffu, st.A.w, off);
+        // the lower lane group's state goes first on both sides: identical results in all groups
+        if (lane & off) {
+            MergeState t; t.M = M2; t.L = L2; t.A = A2;
+            merge_combine(t, st.M, st.L, st.A);
+            st = t;
+        } else {
+            merge_combine(st, M2, L2, A2);
+        }
+    }
+    if (sub == 0) sA[warp][cl] = st.A;
+    if (lane == 0) { sM[warp] = st.M; sL[warp] = st.L; }
     __syncthreads();
-    if (warp == 0) {
+    if (warp == 0 && sub == 0) {
         float Mf = sM[0];
 #pragma unroll
         for (int w = 1; w < NW; ++w) Mf = fmaxf(Mf, sM[w]);
@@ -167,13 +209,14 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
 #pragma unroll
             for (int w = 0; w < NW; ++w) {
                 const float wt = ex2_approx((sM[w] - Mf) * kLog2e);
-                const float4 a = sA[w][lane];
+                const float4 a = sA[w][cl];
                 Ls = fmaf(wt, sL[w], Ls);
                 As.x = fmaf(wt, a.x, As.x); As.y = fmaf(wt, a.y, As.y);
                 As.z = fmaf(wt, a.z, As.z); As.w = fmaf(wt, a.w, As.w);
             }
         }
-        merge_store(p, (int64_t)row * p.Hq + h, lane, Mf, Ls, As);
+        merge_store(p, (int64_t)row * p.Hq + h, ch, slice == 0 && cl == 0, Mf, Ls, As);
+        if (blockIdx.x == 0 && lane == 0) PKV_TRACE_STAMP_MERGE(p, 2);
     }
 }
 
@@ -195,29 +238,44 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
     const int64_t want = (int64_t)shape.B * rp.S;
     int threads = 128;
     while (threads < kBuildThreadsMax && threads < want) threads <<= 1;
-    return launch_pdl(pkv_build_workqueue_kernel, dim3(1), dim3(threads), 0, stream, a);
+    return launch_pdl(!(rp.flags & PKV_FLAG_NO_PDL), pkv_build_workqueue_kernel, dim3(1), dim3(threads), 0, stream, a);
 }
 
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
-    const int grid = p.B * p.Hq;
-    if (grid <= 0) return cudaSuccess;
-    // Warps per CTA.  A warp covers 8 splits per round trip, and small CTAs start (and finish)
-    // sooner, so: as few warps as cover the row's splits in one round when the split count is
-    // known on the host (FIXED_COUNT: at most S; measured on config 2, S = 16: 2 warps 25.9 us per
-    // step, 4 warps 26.0, 16 warps 26.9); else by batch size -- 16 warps while there is at most
-    // one (row, head) pair per SM (a single long row can hold ~148 splits), 8 warps up to 1024
-    // pairs (49.6 vs 50.7 us on config 3), 4 warps, six CTAs per SM, beyond (config 5).
-    int nw;
-    if (p.plan.split_mode == PKV_SPLIT_FIXED_COUNT && p.plan.S > 0)
-        nw = p.plan.S <= 16 ? 2 : (p.plan.S <= 32 ? 4 : (p.plan.S <= 64 ? 8 : 16));
-    else
-        nw = grid <= 148 ? 16 : (grid <= 1024 ? 8 : 4);
-#define PKV_MERGE_CASE(GG, NWW, MB) \
-    if (G == GG && nw == NWW) return launch_pdl(pkv_merge_kernel<GG, NWW, MB>, dim3(grid), dim3(NWW * 32), 0, stream, p);
-    PKV_MERGE_CASE(4, 2, 1) PKV_MERGE_CASE(4, 4, 6) PKV_MERGE_CASE(4, 8, 1) PKV_MERGE_CASE(4, 16, 1)
-    PKV_MERGE_CASE(8, 2, 1) PKV_MERGE_CASE(8, 4, 6) PKV_MERGE_CASE(8, 8, 1) PKV_MERGE_CASE(8, 16, 1)
-    PKV_MERGE_CASE(2, 2, 1) PKV_MERGE_CASE(2, 4, 6) PKV_MERGE_CASE(2, 8, 1) PKV_MERGE_CASE(2, 16, 1)
-    PKV_MERGE_CASE(1, 2, 1) PKV_MERGE_CASE(1, 4, 6) PKV_MERGE_CASE(1, 8, 1) PKV_MERGE_CASE(1, 16, 1)
+    const int pairs = p.B * p.Hq;
+    if (pairs <= 0) return cudaSuccess;
+    const bool pdl = !(p.plan.flags & PKV_FLAG_NO_PDL);
+    // Warps per CTA (NW) and channel slices (CS).  A warp covers 8 * CS splits per round trip, and
+    // small CTAs start (and finish) sooner, so: as few warps as cover the row's splits in one round
+    // when the split count is known on the host (FIXED_COUNT: at most S; measured on config 2,
+    // S = 16: 2 warps 25.9 us per step, 4 warps 26.0, 16 warps 26.9); else by batch size -- 16 warps
+    // while there is at most one (row, head) pair per SM, 8 warps up to 1024 pairs (49.6 vs 50.7 us
+    // on config 3), 4 warps, six CTAs per SM, beyond (config 5).
+    // Slices when rows can hold more than 32 splits and the CTAs still fit the machine in one wave
+    // (B * Hq * 4 <= 160, i.e. a single long row): 128 CTAs of 8 warps pull one row's 128 .. 148
+    // states per head out of L2 instead of 32 CTAs of 16 warps (config 2, whole step, S = 147:
+    // 23.4 vs 24.5 us; S = 128: 23.4 vs 23.6; 4-warp CTAs and 2 slices are slower, r02 sweep).
+    int nw, cs = 1;
+    const bool known = p.plan.split_mode == PKV_SPLIT_FIXED_COUNT && p.plan.S > 0;
+    const int n_max = known ? p.plan.S : kMaxSplits;
+    if (n_max > 32 && pairs * 4 <= 160) {
+        cs = 4;
+        nw = 8;
+    } else if (known) {
+        nw = n_max <= 16 ? 2 : (n_max <= 32 ? 4 : (n_max <= 64 ? 8 : 16));
+    } else {
+        nw = pairs <= 148 ? 16 : (pairs <= 1024 ? 8 : 4);
+    }
+    const int grid = pairs * cs;
+#define PKV_MERGE_CASE(GG, NWW, CSS, MB) \
+    if (G == GG && nw == NWW && cs == CSS)  \
+        return launch_pdl(pdl, pkv_merge_kernel<GG, NWW, CSS, MB>, dim3(grid), dim3(NWW * 32), 0, stream, p);
+#define PKV_MERGE_G(GG) \
+    PKV_MERGE_CASE(GG, 2, 1, 1) PKV_MERGE_CASE(GG, 4, 1, 6) PKV_MERGE_CASE(GG, 8, 1, 1) PKV_MERGE_CASE(GG, 16, 1, 1) \
+    PKV_MERGE_CASE(GG, 2, 2, 1) PKV_MERGE_CASE(GG, 4, 2, 1) PKV_MERGE_CASE(GG, 8, 2, 1) PKV_MERGE_CASE(GG, 16, 2, 1) \
+    PKV_MERGE_CASE(GG, 2, 4, 1) PKV_MERGE_CASE(GG, 4, 4, 1) PKV_MERGE_CASE(GG, 8, 4, 1) PKV_MERGE_CASE(GG, 16, 4, 1)
+    PKV_MERGE_G(4) PKV_MERGE_G(8) PKV_MERGE_G(2) PKV_MERGE_G(1)
+#undef PKV_MERGE_G
 #undef PKV_MERGE_CASE
     return cudaErrorInvalidValue;
 }

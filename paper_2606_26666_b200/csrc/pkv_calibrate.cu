@@ -183,18 +183,15 @@ extern "C" pkv_status pkv_calibrate(void* dev_buffer, size_t bytes, void* stream
         const int n = 400;
         for (int pdl = 0; pdl < 2; ++pdl) {
             double best = 1e30;
-            const bool saved = g_use_pdl;
-            g_use_pdl = pdl != 0;
             for (int r = 0; r < 4; ++r) {
                 t.start();
                 for (int i = 0; i < n; ++i) {
-                    e = launch_pdl(pkv_probe_empty_kernel, dim3(1), dim3(32), 0, cs, (int*)nullptr);
+                    e = launch_pdl(pdl != 0, pkv_probe_empty_kernel, dim3(1), dim3(32), 0, cs, (int*)nullptr);
                     if (e != cudaSuccess) break;
                 }
                 const double ms = t.stop_ms();
                 if (r > 0 && ms < best) best = ms;
             }
-            g_use_pdl = saved;
             if (e != cudaSuccess) { set_error("empty-kernel chain: %s", cudaGetErrorString(e)); return PKV_ERR_CUDA; }
             (pdl ? out->launch_pdl_us : out->launch_us) = best * 1e3 / n;
         }
@@ -203,15 +200,12 @@ extern "C" pkv_status pkv_calibrate(void* dev_buffer, size_t bytes, void* stream
     {
         const int n = 400;
         for (int pdl = 0; pdl < 2; ++pdl) {
-            const bool saved = g_use_pdl;
-            g_use_pdl = pdl != 0;
             cudaGraph_t graph = nullptr;
             cudaGraphExec_t exec = nullptr;
             e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
             for (int i = 0; i < n && e == cudaSuccess; ++i)
-                e = launch_pdl(pkv_probe_empty_kernel, dim3(1), dim3(32), 0, cs, (int*)nullptr);
+                e = launch_pdl(pdl != 0, pkv_probe_empty_kernel, dim3(1), dim3(32), 0, cs, (int*)nullptr);
             cudaError_t e2 = cudaStreamEndCapture(cs, &graph);
-            g_use_pdl = saved;
             if (e == cudaSuccess) e = e2;
             if (e == cudaSuccess) e = cudaGraphInstantiate(&exec, graph, 0);
             double best = 1e30;

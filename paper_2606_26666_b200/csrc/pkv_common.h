@@ -13,6 +13,8 @@ constexpr int kD = 128;         // head dimension compiled in
 constexpr int kPage = 16;       // page size compiled in
 constexpr int kAutoCMin = 4;    // PAPER.md:85 "C_min = 4 CTAs/SM" (auto split rule, A12)
 constexpr int kMaxSplits = 256; // cap on S (and on n_i in FIXED_CHUNK mode)
+constexpr int kAllFlags = PKV_FLAG_VALIDATE | PKV_FLAG_NO_PDL | PKV_FLAG_SEPARATE_BUILD | PKV_FLAG_TEST_REPLAN;
+constexpr int kDefaultPrefetchKb = 256;   // policy.prefetch_kb == 0
 constexpr int kMaxFusedRows = 512;  // fused build (TMA kernel): the batch's offsets and lengths sit in shared memory
 
 void set_error(const char* fmt, ...);
@@ -67,6 +69,8 @@ struct Resolved {
     int32_t G;
     int32_t num_sms;    // BALANCED: U (policy.num_sms, else the device's)
     int32_t flags;      // pkv_flag bits
+    int32_t heads_per_cta;  // 0 = automatic
+    int32_t prefetch_kb;    // resolved: 0 = off
 };
 
 // Byte offsets inside the caller's workspace.  Pure function of (shape, S bound).

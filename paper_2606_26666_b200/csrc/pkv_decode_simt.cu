@@ -169,10 +169,11 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
 
 cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
-    if (G == 1) return launch_pdl(pkv_decode_simt_kernel<1>, dim3(grid), dim3(kThreads), 0, stream, p);
-    if (G == 2) return launch_pdl(pkv_decode_simt_kernel<2>, dim3(grid), dim3(kThreads), 0, stream, p);
-    if (G == 4) return launch_pdl(pkv_decode_simt_kernel<4>, dim3(grid), dim3(kThreads), 0, stream, p);
-    return launch_pdl(pkv_decode_simt_kernel<8>, dim3(grid), dim3(kThreads), 0, stream, p);
+    const bool pdl = !(p.plan.flags & PKV_FLAG_NO_PDL);
+    if (G == 1) return launch_pdl(pdl, pkv_decode_simt_kernel<1>, dim3(grid), dim3(kThreads), 0, stream, p);
+    if (G == 2) return launch_pdl(pdl, pkv_decode_simt_kernel<2>, dim3(grid), dim3(kThreads), 0, stream, p);
+    if (G == 4) return launch_pdl(pdl, pkv_decode_simt_kernel<4>, dim3(grid), dim3(kThreads), 0, stream, p);
+    return launch_pdl(pdl, pkv_decode_simt_kernel<8>, dim3(grid), dim3(kThreads), 0, stream, p);
 }
 
 }  // namespace pkv

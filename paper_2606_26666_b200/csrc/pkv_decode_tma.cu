@@ -126,6 +126,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     __syncthreads();
     const int HGn = p.Hkv / HG;                               // head groups per (row, split)
     int num_units = 0;
+    int early_row = -1, early_tok0 = 0, early_tok1 = 0, early_mine = 0;   // producer 0: first unit's table entries
     PlanArgs plan = p.plan;   // BALANCED: the planner resolves the batch-wide chunk
     // Speculative plan.  A decode CTA is usually resident a few microseconds before its dependency
     // wait returns (programmatic launch), and the plan -- ~1 us with a fixed split count, ~2.5 us
@@ -143,6 +144,33 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         for (int i = lane; i < p.B; i += 32) tail.len_s[i] = 1;
         if (lane == 0) tail.first_slot.tok1 = 0;
         __syncwarp();
+    }
+    // L2 prefetch.  Until the wait below returns the memory system is
+    // underused -- the predecessor's last CTAs are draining, the merge of the previous decode step
+    // is a handful of dependent round trips -- while this CTA already knows, from the speculative
+    // plan, which pages it will stream first.  Producer 0 looks at those block-table entries
+    // (race-tolerant loads) and asks for the pages' K/V boxes, and the unit's q rows, to be brought
+    // into L2.  Nothing enters the program: L2 is the point of coherence, every value is loaded after
+    // the wait; a stale guess only costs bandwidth.
+    if (p.fused_build && warp == 0 && p.prefetch_pages > 0 && (int)blockIdx.x < spec_row_slots * HGn) {
+        const RowSlot d = tail.first_slot;
+        const int p0 = d.tok0 >> 4;
+        int np = d.tok0 < d.tok1 ? ((d.tok1 + 15) >> 4) - p0 : 0;
+        np = min(min(np, p.prefetch_pages), p.max_pages - p0);
+        if (d.row >= 0 && d.row < p.B && p0 >= 0) {
+            const int32_t* bt = p.block_table + (int64_t)d.row * p.max_pages + p0;
+            const int head0 = ((int)blockIdx.x % HGn) * HG;
+            for (int j = lane; j < np; j += 32) {
+                const int page = ld_relaxed_s32(bt + j);
+                if (page >= 0 && (int64_t)page < p.num_pages) {
+                    tma_prefetch_5d(&tmap_k, 0, 0, 0, head0, page);
+                    tma_prefetch_5d(&tmap_v, 0, 0, 0, head0, page);
+                }
+            }
+            // q rows of the unit's HG*G query heads: HG*G*256 bytes, one 128-byte line per lane
+            const char* qrow = reinterpret_cast<const char*>(p.q + ((int64_t)d.row * p.Hq + head0 * G) * kD);
+            for (int b = lane * 128; b < HG * G * kD * 2; b += 32 * 128) prefetch_l2(qrow + b);
+        }
     }
     pdl_wait();   // queue (builder), q / seq_lens (upstream), out / partials (previous step's readers)
     if (tid == 0) PKV_TRACE_STAMP(p, 1);
@@ -201,6 +229,17 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         // and leaves it in shared memory for the planner warp, which writes the queue.
         int32_t row_slots = spec_row_slots;
         int32_t* const err = blockIdx.x == 0 ? &p.hdr->error_word : nullptr;   // one CTA reports bad lengths
+        // The first unit's block-table entries are requested together with the lengths the plan is
+        // validated against: one round trip instead of two on the way to the first TMA load.
+        if (!p.force_replan && (int)blockIdx.x < spec_row_slots * HGn) {
+            const RowSlot d = tail.first_slot;
+            const int p0 = d.tok0 >> 4;
+            const int np = d.tok0 < d.tok1 ? min(((d.tok1 + 15) >> 4) - p0, p.max_pages - p0) : 0;
+            if (d.row >= 0 && d.row < p.B && p0 >= 0) {
+                early_row = d.row; early_tok0 = d.tok0; early_tok1 = d.tok1;
+                if (lane < np) early_mine = __ldcg(p.block_table + (int64_t)d.row * p.max_pages + p0 + lane);
+            }
+        }
         if (!p.force_replan && plan_lens_unchanged(plan, p.seq_lens, tail.len_s, lane, err)) {
             plan = spec_plan;
         } else {
@@ -292,7 +331,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             const int head0 = hg * HG;
             const int32_t* bt = p.block_table + (int64_t)row * p.max_pages + p0;
             // table entries 32 at a time (lane i holds page c + i of the unit)
-            int mine = lane < np ? checked_page(bt[lane], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
+            const bool early = k == 0 && warp == 0 && row == early_row && tok0 == early_tok0 && tok1 == early_tok1;
+            int mine = lane < np ? checked_page(early ? early_mine : bt[lane], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
             for (int c = 0; c < np; c += 32) {
                 const int nxt = (c + 32 + lane < np)
                                     ? checked_page(bt[c + 32 + lane], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
@@ -569,7 +609,7 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
-    return launch_pdl(pkv_decode_tma_kernel<G, HG>, dim3(grid), dim3(threads), (size_t)smem, stream, p, mk, mv);
+    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG>, dim3(grid), dim3(threads), (size_t)smem, stream, p, mk, mv);
 }
 
 }  // namespace

@@ -45,6 +45,7 @@ struct DecodeParams {
     int32_t heads_per_cta;       // TMA kernel: KV heads one CTA streams together (1, 2, 4 or 8)
     int32_t dynamic_sched;      // 1: tasks handed out by an atomic counter
     int32_t force_replan;       // test hook: treat the speculative plan as invalidated
+    int32_t prefetch_pages;     // TMA kernel: pages of its first unit a CTA prefetches into L2 before the wait
     float scale;                // x = scale * <q, k>
     float scale_log2;           // scale * log2(e)
     int64_t num_pages;          // PKV_FLAG_VALIDATE: block-table entries must lie in [0, num_pages)
@@ -88,9 +89,20 @@ __device__ __forceinline__ void trace_stamp(const DecodeParams& p, int slot) {
         p.trace[(size_t)blockIdx.x * 16 + slot] = t;
     }
 }
+// the merge kernel's CTA 0 stamps row kTraceMergeRow of the same buffer
+constexpr int kTraceMergeRow = 148;
+__device__ __forceinline__ void trace_stamp_row(const DecodeParams& p, int row, int slot) {
+    if (p.trace) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        p.trace[(size_t)row * 16 + slot] = t;
+    }
+}
 #define PKV_TRACE_STAMP(p, slot) trace_stamp(p, slot)
+#define PKV_TRACE_STAMP_MERGE(p, slot) trace_stamp_row(p, kTraceMergeRow, slot)
 #else
 #define PKV_TRACE_STAMP(p, slot) ((void)0)
+#define PKV_TRACE_STAMP_MERGE(p, slot) ((void)0)
 #endif
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -137,6 +149,17 @@ __device__ __forceinline__ unsigned long long l2_policy_evict_first() {
     unsigned long long pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
+}
+// L2 prefetch of one tensor-map box (no shared-memory destination, no completion): used BEFORE the
+// kernel's dependency wait for the first pages of a CTA's first unit.  L2 is the point of
+// coherence, so a prefetched line can never hide a later write of the predecessor kernel.
+__device__ __forceinline__ void tma_prefetch_5d(const void* tmap, int c0, int c1, int c2, int c3, int c4) {
+    asm volatile("cp.async.bulk.prefetch.tensor.5d.L2.global.tile [%0, {%1, %2, %3, %4, %5}];" ::"l"(tmap), "r"(c0),
+                 "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+                 : "memory");
+}
+__device__ __forceinline__ void prefetch_l2(const void* ptr) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
 }
 __device__ __forceinline__ void tma_load_4d(uint32_t dst, const void* tmap, uint32_t bar, int c0, int c1,
                                             int c2, int c3) {
@@ -560,18 +583,20 @@ __device__ __forceinline__ void merge_accumulate(const DecodeParams& p, int64_t 
     }
 }
 
-__device__ __forceinline__ void merge_store(const DecodeParams& p, int64_t o, int lane, float M, float L, float4 A) {
-    __half2* dst = reinterpret_cast<__half2*>(p.out + o * kD + lane * 4);
+// Stores four channels ch .. ch+3 of output row o (FP16) and, by the lane with store_lse, its LSE.
+__device__ __forceinline__ void merge_store(const DecodeParams& p, int64_t o, int ch, bool store_lse, float M, float L,
+                                            float4 A) {
+    __half2* dst = reinterpret_cast<__half2*>(p.out + o * kD + ch);
     if (M == -INFINITY) {  // no state or only neutral states (A9)
         dst[0] = __floats2half2_rn(0.f, 0.f);
         dst[1] = __floats2half2_rn(0.f, 0.f);
-        if (p.lse && lane == 0) p.lse[o] = -INFINITY;
+        if (p.lse && store_lse) p.lse[o] = -INFINITY;
         return;
     }
     const float inv = 1.0f / L;
     dst[0] = __floats2half2_rn(A.x * inv, A.y * inv);
     dst[1] = __floats2half2_rn(A.z * inv, A.w * inv);
-    if (p.lse && lane == 0) p.lse[o] = M + logf(L);
+    if (p.lse && store_lse) p.lse[o] = M + logf(L);
 }
 
 // One warp merges head hh completely (fused path; also any caller without helpers).
@@ -588,7 +613,7 @@ __device__ __forceinline__ void merge_head_warp(const DecodeParams& p, int64_t s
     As.y = ((A[0].y + A[1].y) + A[2].y) + A[3].y;
     As.z = ((A[0].z + A[1].z) + A[2].z) + A[3].z;
     As.w = ((A[0].w + A[1].w) + A[2].w) + A[3].w;
-    merge_store(p, (int64_t)row * p.Hq + kvh * G + hh, lane, M, Ls, As);
+    merge_store(p, (int64_t)row * p.Hq + kvh * G + hh, lane * 4, lane == 0, M, Ls, As);
 }
 
 // ------------------------------------------------------------------ task epilogue
@@ -708,10 +733,9 @@ __device__ __forceinline__ void zero_empty_rows(const DecodeParams& p) {
 
 // Launch with the programmatic-stream-serialization attribute: in a stream (and in a captured
 // graph) the kernel may start while its predecessor is still running; it orders itself with
-// pdl_wait().  g_use_pdl = false falls back to plain launches (test hook).
-extern bool g_use_pdl;
+// pdl_wait().  pdl = false (PKV_FLAG_NO_PDL) is a plain launch.
 template <typename... KArgs, typename... Args>
-cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+cudaError_t launch_pdl(bool pdl, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
                        Args&&... args) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
@@ -722,7 +746,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = g_use_pdl ? 1 : 0;
+    cfg.numAttrs = pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
 

@@ -65,7 +65,12 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     if (p.merge_mode != PKV_MERGE_SEPARATE && p.merge_mode != PKV_MERGE_FUSED) { set_error("bad merge_mode %d", p.merge_mode); return PKV_ERR_INVALID_ARG; }
     if (p.kernel < PKV_KERNEL_AUTO || p.kernel > PKV_KERNEL_SIMT) { set_error("bad kernel %d", p.kernel); return PKV_ERR_INVALID_ARG; }
     if (p.num_sms < 0) { set_error("num_sms < 0"); return PKV_ERR_INVALID_ARG; }
-    if (p.flags & ~(int32_t)PKV_FLAG_VALIDATE) { set_error("unknown policy flag bits 0x%x", p.flags); return PKV_ERR_INVALID_ARG; }
+    if (p.flags & ~(int32_t)kAllFlags) { set_error("unknown policy flag bits 0x%x", p.flags); return PKV_ERR_INVALID_ARG; }
+    if (p.heads_per_cta != 0 && ((p.heads_per_cta != 1 && p.heads_per_cta != 2 && p.heads_per_cta != 4 && p.heads_per_cta != 8) ||
+                                 s.Hkv % p.heads_per_cta != 0)) {
+        set_error("heads_per_cta=%d must be 0 (auto), 1, 2, 4 or 8 and divide Hkv=%d", p.heads_per_cta, s.Hkv);
+        return PKV_ERR_INVALID_ARG;
+    }
 
     int32_t S = p.num_splits;
     out->num_sms = p.num_sms > 0 ? p.num_sms : num_sms_or_0;
@@ -99,6 +104,8 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     out->kernel = p.kernel == PKV_KERNEL_AUTO ? PKV_KERNEL_TMA_MMA : p.kernel;
     out->G = G;
     out->flags = p.flags;
+    out->heads_per_cta = p.heads_per_cta;
+    out->prefetch_kb = p.prefetch_kb == 0 ? kDefaultPrefetchKb : (p.prefetch_kb < 0 ? 0 : p.prefetch_kb);
     return PKV_OK;
 }
 

@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol():
 def test_version_and_struct_sizes():
     assert pkv.pkv_version() >> 16 == 2
     assert ctypes.sizeof(binding.pkv_task) == 20            # 5 x int32
-    assert ctypes.sizeof(binding.pkv_split_policy) == 36
+    assert ctypes.sizeof(binding.pkv_split_policy) == 44
     assert ctypes.sizeof(binding.pkv_shape) == 56
     assert ctypes.sizeof(binding.pkv_counters) == 128
 

@@ -2,6 +2,8 @@
 on the same seeded inputs.  Tolerance = BASELINE.json north_star with DESIGN.md reading A15:
 max abs <= 2e-3, floored max rel <= 1e-2, mean abs <= 3e-4.  Integer work
 (tasks, split_offsets, counters, token counts) is compared bit-exactly."""
+import dataclasses
+
 import numpy as np
 import pytest
 import torch
@@ -40,11 +42,8 @@ def test_config1(kernel):
                 seq_lens=w.seq_lens, Hkv=8, page_size=16, scale=default_scale(128))
     dp = DevProblem(p)
     for hg in (0, 1, 2, 4, 8):
-        pkv.pkv_debug_force_heads_per_cta(hg)
-        try:
-            check(dp, pkv.Policy(tile_tokens=32, num_splits=1, route=pkv.ROUTE_RECT, kernel=kernel), what="hg%d" % hg)
-        finally:
-            pkv.pkv_debug_force_heads_per_cta(0)
+        check(dp, pkv.Policy(tile_tokens=32, num_splits=1, route=pkv.ROUTE_RECT, kernel=kernel, heads_per_cta=hg),
+              what="hg%d" % hg)
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -74,12 +73,8 @@ def test_tma_heads_per_cta_variants(hg, Hkv):
     p = make_problem(RAGGED, seed=300 + Hkv, Hkv=Hkv)
     dp = DevProblem(p)
     ref = oracle_attention(p)
-    pkv.pkv_debug_force_heads_per_cta(hg)
-    try:
-        for S, mm in ((1, 0), (5, 0), (5, 1)):
-            check(dp, pkv.Policy(tile_tokens=32, num_splits=S, merge_mode=mm), ref, what="hg%d S%d" % (hg, S))
-    finally:
-        pkv.pkv_debug_force_heads_per_cta(0)
+    for S, mm in ((1, 0), (5, 0), (5, 1)):
+        check(dp, pkv.Policy(tile_tokens=32, num_splits=S, merge_mode=mm, heads_per_cta=hg), ref, what="hg%d S%d" % (hg, S))
 
 
 @pytest.mark.parametrize("route", [pkv.ROUTE_WORKQUEUE, pkv.ROUTE_RECT])
@@ -371,15 +366,12 @@ def test_many_units_per_cta_odd_page_counts(hg, Hkv):
     p = make_problem(list(lens), seed=400 + hg, Hkv=Hkv)
     dp = DevProblem(p)
     ref = oracle_attention(p)
-    pkv.pkv_debug_force_heads_per_cta(hg)
-    try:
-        for pol in (pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=16, num_splits=3),
-                    pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=5,
-                               merge_mode=pkv.MERGE_FUSED)):
-            for _ in range(2):          # twice: the dynamic unit counter must have re-armed itself
-                check(dp, pol, ref, what="hg%d %s" % (hg, pol))
-    finally:
-        pkv.pkv_debug_force_heads_per_cta(0)
+    for pol in (pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=16, num_splits=3),
+                pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=5,
+                           merge_mode=pkv.MERGE_FUSED)):
+        pol.heads_per_cta = hg
+        for _ in range(2):          # twice: the dynamic unit counter must have re-armed itself
+            check(dp, pol, ref, what="hg%d %s" % (hg, pol))
 
 
 @pytest.mark.parametrize("Hkv", [8, 4])
@@ -396,14 +388,11 @@ def test_long_units_ring_wraps_many_times(hg, Hkv):
     p = make_problem(list(lens), seed=500 + hg, Hkv=Hkv)
     dp = DevProblem(p)
     ref = oracle_attention(p)
-    pkv.pkv_debug_force_heads_per_cta(hg)
-    try:
-        for pol in (pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=8),
-                    pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=32, num_splits=4)):
-            for _ in range(3):
-                check(dp, pol, ref, what="hg%d %s" % (hg, pol))
-    finally:
-        pkv.pkv_debug_force_heads_per_cta(0)
+    for pol in (pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=8),
+                pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=32, num_splits=4)):
+        pol.heads_per_cta = hg
+        for _ in range(3):
+            check(dp, pol, ref, what="hg%d %s" % (hg, pol))
 
 
 def test_pdl_off_matches_pdl_on_bitwise():
@@ -412,11 +401,7 @@ def test_pdl_off_matches_pdl_on_bitwise():
     pol = pkv.Policy(tile_tokens=32, num_splits=5)
     dp = DevProblem(p)
     o1, l1, _ = dp.decode(pol)
-    pkv.pkv_debug_set_pdl(False)
-    try:
-        o2, l2, _ = dp.decode(pol)
-    finally:
-        pkv.pkv_debug_set_pdl(True)
+    o2, l2, _ = dp.decode(dataclasses.replace(pol, flags=pkv.FLAG_NO_PDL))
     assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
     assert_within_tolerance(o1, oracle_attention(p)[0])
 
@@ -443,11 +428,8 @@ def test_fused_build_queue_bit_exact_and_same_output(route):
         want = wq.build_workqueue(lens, 8, opol)
         outs = []
         for fused in (True, False):
-            pkv.pkv_debug_set_fused_build(fused)
-            try:
-                out, lse, ws, _ = check(dp, pol, ref, what="fused=%s %s" % (fused, pol))
-            finally:
-                pkv.pkv_debug_set_fused_build(True)
+            pol = dataclasses.replace(pol, flags=0 if fused else pkv.FLAG_SEPARATE_BUILD)
+            out, lse, ws, _ = check(dp, pol, ref, what="fused=%s %s" % (fused, pol))
             outs.append((out, lse))
             tasks, offs = pkv.pkv_read_workqueue(dp.shape, pol, ws)
             assert np.array_equal(tasks, np.array(want.tasks, dtype=np.int32).reshape(-1, 5)), (fused, pol)
@@ -501,17 +483,13 @@ def test_stage_release_waits_for_the_last_ldmatrix():
         p.v_cache[p.block_table[i, j // 16], j % 16, :, j % 128] = 1.0
         exp[i] = np.bincount(j % 128, minlength=128)
     dp = DevProblem(p)
-    pkv.pkv_debug_force_heads_per_cta(2)
-    try:
-        pol = pkv.Policy(tile_tokens=32, num_splits=1)
-        ws = pkv.alloc_workspace(dp.shape, pol)
-        for rep in range(120):
-            out, lse, _ = dp.decode(pol, ws=ws)
-            cnt = out * lens[:, None, None].astype(np.float64)
-            assert np.abs(cnt - exp[:, None, :]).max() < 0.3, "launch %d: a token was read from another page" % rep
-            assert np.abs(lse - np.log(lens)[:, None]).max() < 1e-5
-    finally:
-        pkv.pkv_debug_force_heads_per_cta(0)
+    pol = pkv.Policy(tile_tokens=32, num_splits=1, heads_per_cta=2)
+    ws = pkv.alloc_workspace(dp.shape, pol)
+    for rep in range(120):
+        out, lse, _ = dp.decode(pol, ws=ws)
+        cnt = out * lens[:, None, None].astype(np.float64)
+        assert np.abs(cnt - exp[:, None, :]).max() < 0.3, "launch %d: a token was read from another page" % rep
+        assert np.abs(lse - np.log(lens)[:, None]).max() < 1e-5
 
 
 def _compact_rows(w, k_dev, v_dev, rows, lens):
@@ -603,11 +581,7 @@ def test_speculative_plan_is_discarded_when_lengths_changed(mode):
     ref = oracle_attention(p)
     pol = pkv.Policy(tile_tokens=16, split_mode=mode, num_splits=0 if mode == pkv.SPLIT_BALANCED else 6)
     o1, l1, ws1, _ = check(dp, pol, ref)
-    pkv.pkv_debug_force_replan(True)
-    try:
-        o2, l2, ws2, _ = check(dp, pol, ref)
-    finally:
-        pkv.pkv_debug_force_replan(False)
+    o2, l2, ws2, _ = check(dp, dataclasses.replace(pol, flags=pkv.FLAG_TEST_REPLAN), ref)
     assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
     t1, f1 = pkv.pkv_read_workqueue(dp.shape, pol, ws1)
     t2, f2 = pkv.pkv_read_workqueue(dp.shape, pol, ws2)

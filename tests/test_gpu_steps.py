@@ -3,6 +3,8 @@ CUDA graph with programmatic dependent launch on and no host synchronisation in 
 (the overlapped replay bench.py times), the device-side validation of
 device-resident inputs (every bound derives from N_i), the launch marks behind
 pkv_counters.launched_*, and a second device in the same process."""
+import dataclasses
+
 import numpy as np
 import pytest
 import torch
@@ -25,25 +27,22 @@ def _multi_step_graph(dp, p, pol, lens0, steps, pdl):
     sl_all = to_dev(lens_all)
     out = torch.full((steps, B, p.Hq, p.d), float("nan"), dtype=torch.float16, device="cuda")
     lse = torch.full((steps, B, p.Hq), float("nan"), dtype=torch.float32, device="cuda")
+    pol = dataclasses.replace(pol, flags=pol.flags | (0 if pdl else pkv.FLAG_NO_PDL))
     ws = pkv.alloc_workspace(dp.shape, pol)
-    pkv.pkv_debug_set_pdl(pdl)
-    try:
-        s = torch.cuda.Stream()
-        with torch.cuda.stream(s):
-            pkv.pkv_decode(dp.shape, pol, dp.q, dp.k, dp.v, dp.bt, sl_all[0], out[0], lse[0], scale=p.scale,
-                           workspace=ws, stream=s)      # warm-up outside capture (function attributes)
-            s.synchronize()
-            out.fill_(float("nan"))
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=s):
-                for t in range(steps):
-                    pkv.pkv_decode(dp.shape, pol, dp.q, dp.k, dp.v, dp.bt, sl_all[t], out[t], lse[t],
-                                   scale=p.scale, workspace=ws, stream=torch.cuda.current_stream())
-            g.replay()
-            g.replay()      # twice: self-resetting counters, workspace reused across replays
-        torch.cuda.synchronize()
-    finally:
-        pkv.pkv_debug_set_pdl(True)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        pkv.pkv_decode(dp.shape, pol, dp.q, dp.k, dp.v, dp.bt, sl_all[0], out[0], lse[0], scale=p.scale,
+                       workspace=ws, stream=s)      # warm-up outside capture (function attributes)
+        s.synchronize()
+        out.fill_(float("nan"))
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            for t in range(steps):
+                pkv.pkv_decode(dp.shape, pol, dp.q, dp.k, dp.v, dp.bt, sl_all[t], out[t], lse[t],
+                               scale=p.scale, workspace=ws, stream=torch.cuda.current_stream())
+        g.replay()
+        g.replay()      # twice: self-resetting counters, workspace reused across replays
+    torch.cuda.synchronize()
     return out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
 
 
@@ -82,9 +81,9 @@ def test_validate_flag_reports_bad_lengths_and_page_ids():
             p = make_problem(lens, seed=61)
             ref = oracle_attention(p)[0]
             max_tokens = p.block_table.shape[1] * 16
-            pol = pkv.Policy(tile_tokens=32, num_splits=3, kernel=kernel, flags=pkv.FLAG_VALIDATE)
-            pkv.pkv_debug_set_fused_build(fused_build)
-            try:
+            pol = pkv.Policy(tile_tokens=32, num_splits=3, kernel=kernel,
+                             flags=pkv.FLAG_VALIDATE | (0 if fused_build else pkv.FLAG_SEPARATE_BUILD))
+            if True:
                 # clean inputs: no error bit
                 dp = DevProblem(p)
                 out, _, ws = dp.decode(pol)
@@ -120,8 +119,6 @@ def test_validate_flag_reports_bad_lengths_and_page_ids():
                 out, _, _ = dp.decode(pol, ws=ws)
                 assert pkv.pkv_get_counters(dp.shape, pol, ws)["error_word"] == pkv.DEVERR_PAGE_ID
                 assert_within_tolerance(out, ref)
-            finally:
-                pkv.pkv_debug_set_fused_build(True)
 
 
 def test_launch_marks_count_what_was_really_launched():
@@ -136,12 +133,9 @@ def test_launch_marks_count_what_was_really_launched():
     c = pkv.pkv_get_counters(dp.shape, pol, ws)
     assert (c["decode_launches"], c["merge_launches"]) == (1, 0)
     assert (c["launched_build"], c["launched_decode"], c["launched_merge"]) == (0, 1, 1)
-    pkv.pkv_debug_set_fused_build(False)
-    try:
-        _, _, ws = dp.decode(pol)
-    finally:
-        pkv.pkv_debug_set_fused_build(True)
-    c = pkv.pkv_get_counters(dp.shape, pol, ws)
+    pol_sb = dataclasses.replace(pol, flags=pkv.FLAG_SEPARATE_BUILD)
+    _, _, ws = dp.decode(pol_sb)
+    c = pkv.pkv_get_counters(dp.shape, pol_sb, ws)
     assert (c["launched_build"], c["launched_decode"], c["launched_merge"]) == (1, 1, 1)
     pol1 = pkv.Policy(tile_tokens=32, num_splits=1)
     _, _, ws = dp.decode(pol1)
@@ -176,3 +170,51 @@ def test_second_device_in_the_same_process():
             pkv.pkv_decode(shape, pol, q, k, v, bt, sl, out, None, scale=p.scale, workspace=ws)
             torch.cuda.synchronize()
             assert_within_tolerance(out.cpu().numpy().astype(np.float64), ref, "device %d" % dev)
+
+
+@pytest.mark.parametrize("mode", [pkv.SPLIT_FIXED_COUNT, pkv.SPLIT_BALANCED])
+def test_block_table_and_lengths_rewritten_right_before_every_step(mode):
+    """The kernel right before pkv_decode rewrites the block table AND the lengths in every step of
+    one graph (PDL on).  Before its dependency wait the decode kernel looks at both with
+    race-tolerant loads -- for the speculative plan and for the L2 prefetch of its first pages
+     -- so what it sees there is the PREVIOUS step's table; every value the
+    result depends on must be loaded after the wait.  Two page assignments of the same logical
+    content alternate (pool = [pages | pages rolled by one]); every step is checked against the
+    oracle and bitwise against the same graph without programmatic launch and without prefetch."""
+    steps = 10
+    lens0 = np.array([3000, 40, 1111, 0, 257, 4090], dtype=np.int32)
+    p = make_problem(list(lens0 + steps), seed=71)
+    n = p.k_cache.shape[0]
+    p.k_cache = np.concatenate([p.k_cache, np.roll(p.k_cache, 1, axis=0)])
+    p.v_cache = np.concatenate([p.v_cache, np.roll(p.v_cache, 1, axis=0)])
+    tab_a = p.block_table.copy()
+    tab_b = np.where(tab_a == PAD_PAGE, PAD_PAGE, n + (tab_a.astype(np.int64) + 1) % n).astype(np.int32)
+    dp = DevProblem(p)
+    tabs = to_dev(np.stack([tab_a, tab_b]))
+    lens_all = to_dev(np.stack([lens0 + t for t in range(steps)]).astype(np.int32))
+    base = pkv.Policy(tile_tokens=16 if mode == pkv.SPLIT_BALANCED else 32, split_mode=mode,
+                      num_splits=0 if mode == pkv.SPLIT_BALANCED else 6, num_sms=40 if mode == pkv.SPLIT_BALANCED else 0)
+    results = []
+    for pol in (base, dataclasses.replace(base, flags=pkv.FLAG_NO_PDL, prefetch_kb=-1)):
+        out = torch.full((steps, p.B, p.Hq, p.d), float("nan"), dtype=torch.float16, device="cuda")
+        ws = pkv.alloc_workspace(dp.shape, pol)
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            pkv.pkv_decode(dp.shape, pol, dp.q, dp.k, dp.v, dp.bt, dp.sl, out[0], None, scale=p.scale, workspace=ws, stream=s)
+            s.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=s):
+                for t in range(steps):
+                    dp.bt.copy_(tabs[t % 2])          # the predecessor kernels of step t
+                    dp.sl.copy_(lens_all[t])
+                    pkv.pkv_decode(dp.shape, pol, dp.q, dp.k, dp.v, dp.bt, dp.sl, out[t], None, scale=p.scale,
+                                   workspace=ws, stream=torch.cuda.current_stream())
+            g.replay()
+            g.replay()
+        torch.cuda.synchronize()
+        results.append(out.cpu().numpy().astype(np.float64))
+    assert np.array_equal(results[0], results[1])
+    p.block_table = tab_a
+    for t in range(steps):
+        p.seq_lens = (lens0 + t).astype(np.int32)
+        assert_within_tolerance(results[0][t], oracle_attention(p)[0], "step %d" % t)
