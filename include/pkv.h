@@ -242,6 +242,49 @@ PKV_API pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_pol
                                      uint32_t stages, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * Indexed rows ("Indexed Q/O. The extension can read Q rows and write output rows by
+ * index, avoiding per-bucket index_select and index_copy_"): one decode step over a SUBSET of the
+ * batch's rows, in place.  shape->B = number of launch rows; launch row i works on request row
+ * row_index[i] (dev int32 [B], values in [0, rows of the caller's arrays)) of q, out, lse,
+ * block_table AND seq_lens -- nothing is gathered or scattered by the caller.  The queue in the
+ * workspace is in launch rows (pkv_task.row = i).  At most 512 rows per call.  Otherwise as
+ * pkv_decode with build_queue = 1.
+ */
+PKV_API pkv_status pkv_decode_indexed(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                                      const void* k_cache, const void* v_cache, const int32_t* block_table,
+                                      const int32_t* seq_lens, const int32_t* row_index, void* out, float* lse,
+                                      float scale, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * Length-bucket route ("one per route length"; DESIGN.md readings
+ * A22, A23) -- the route the compact workqueue replaces, kept as its comparator (Table 4: 16.00 vs
+ * 2.00 launches per step).
+ * pkv_plan_buckets_host (pure CPU): a row's route length is its true length rounded up to
+ * bucket_tokens (1 = exact length buckets); rows of equal route length form a bucket; buckets in
+ * ascending route length, rows ascending inside; rows with N_i <= 0 belong to no bucket and are
+ * listed after the last one.  Writes row_index_out [B] (a permutation of 0..B-1),
+ * bucket_offsets_out [B+1] (first num_buckets+1 entries used), bucket_lengths_out [B] or NULL.
+ * pkv_decode_buckets: one pkv_decode_indexed per bucket over row_index[offsets[b] .. offsets[b+1])
+ * (dev copy of the plan's row_index; bucket_offsets on the HOST), i.e. one decode (+ merge) launch
+ * per bucket with the policy's route and split count, all on one workspace sized for the whole
+ * batch; then one more launch for the rows of no bucket (out = 0, lse = -inf).
+ * pkv_bucket_counters_host (pure CPU): Table 4's counters for that step, summed over the buckets
+ * (policy.num_splits == 0 needs policy.num_sms > 0).
+ */
+PKV_API pkv_status pkv_plan_buckets_host(const int32_t* seq_lens_host, int32_t B, int32_t bucket_tokens,
+                                         int32_t* row_index_out, int32_t* bucket_offsets_out,
+                                         int32_t* bucket_lengths_out, int32_t* num_buckets_out);
+PKV_API pkv_status pkv_decode_buckets(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                                      const void* k_cache, const void* v_cache, const int32_t* block_table,
+                                      const int32_t* seq_lens, const int32_t* row_index,
+                                      const int32_t* bucket_offsets_host, int32_t num_buckets, void* out,
+                                      float* lse, float scale, void* workspace, size_t workspace_bytes,
+                                      void* stream);
+PKV_API pkv_status pkv_bucket_counters_host(const pkv_shape* shape, const pkv_split_policy* policy,
+                                            const int32_t* seq_lens_host, int32_t bucket_tokens,
+                                            pkv_counters* out);
+
+/*
  * Exact merge of split states (segmented over each row's compact slot range,
  * PAPER.md:75).  Public partial-state format, all FP32, natural-log domain:
  *   part_m [slots, G], part_l [slots, G], part_acc [slots, G, d],

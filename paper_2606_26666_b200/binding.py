@@ -66,7 +66,8 @@ class pkv_calibration(ctypes.Structure):
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspace_init_bytes", "pkv_build_workqueue_host",
            "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
-           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate")
+           "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate", "pkv_decode_indexed",
+           "pkv_plan_buckets_host", "pkv_decode_buckets", "pkv_bucket_counters_host")
 
 
 class PkvError(RuntimeError):
@@ -99,6 +100,16 @@ def _load() -> ctypes.CDLL:
     lib.pkv_decode_stages.restype = _i32
     lib.pkv_decode_stages.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp,
                                       ctypes.c_float, ctypes.c_uint32, _vp, ctypes.c_size_t, _vp]
+    lib.pkv_decode_indexed.restype = _i32
+    lib.pkv_decode_indexed.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp,
+                                       ctypes.c_float, _vp, ctypes.c_size_t, _vp]
+    lib.pkv_plan_buckets_host.restype = _i32
+    lib.pkv_plan_buckets_host.argtypes = [_vp, _i32, _i32, _vp, _vp, _vp, P(_i32)]
+    lib.pkv_decode_buckets.restype = _i32
+    lib.pkv_decode_buckets.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp,
+                                       ctypes.c_float, _vp, ctypes.c_size_t, _vp]
+    lib.pkv_bucket_counters_host.restype = _i32
+    lib.pkv_bucket_counters_host.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _i32, P(pkv_counters)]
     lib.pkv_merge.restype = _i32
     lib.pkv_merge.argtypes = [P(pkv_shape), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.pkv_get_counters.restype = _i32
@@ -255,6 +266,42 @@ def pkv_decode_stages(shape: Shape, policy: Policy, q, k_cache, v_cache, block_t
                                   _ptr(v_cache), _ptr(block_table), _ptr(seq_lens), _ptr(out), _ptr(lse),
                                   ctypes.c_float(scale), int(stages), _ptr(workspace), _nbytes(workspace),
                                   _stream_ptr(stream)))
+
+
+def pkv_decode_indexed(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, seq_lens, row_index, out, lse=None,
+                       scale: float = 0.0, workspace=None, stream=None) -> None:
+    _check(_lib.pkv_decode_indexed(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(q), _ptr(k_cache),
+                                   _ptr(v_cache), _ptr(block_table), _ptr(seq_lens), _ptr(row_index), _ptr(out), _ptr(lse),
+                                   ctypes.c_float(scale), _ptr(workspace), _nbytes(workspace), _stream_ptr(stream)))
+
+
+def pkv_plan_buckets_host(seq_lens_host: np.ndarray, bucket_tokens: int):
+    """Returns (row_index int32 [B], bucket_offsets int32 [num_buckets+1], bucket_lengths int32 [num_buckets])."""
+    seq = np.ascontiguousarray(seq_lens_host, dtype=np.int32)
+    B = len(seq)
+    index = np.zeros(max(B, 1), dtype=np.int32)
+    offs = np.zeros(B + 1, dtype=np.int32)
+    lens = np.zeros(max(B, 1), dtype=np.int32)
+    nb = _i32(0)
+    _check(_lib.pkv_plan_buckets_host(_ptr(seq), B, int(bucket_tokens), _ptr(index), _ptr(offs), _ptr(lens), ctypes.byref(nb)))
+    return index[:B], offs[:nb.value + 1], lens[:nb.value]
+
+
+def pkv_decode_buckets(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, seq_lens, row_index,
+                       bucket_offsets_host: np.ndarray, out, lse=None, scale: float = 0.0, workspace=None, stream=None) -> None:
+    offs = np.ascontiguousarray(bucket_offsets_host, dtype=np.int32)
+    _check(_lib.pkv_decode_buckets(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(q), _ptr(k_cache),
+                                   _ptr(v_cache), _ptr(block_table), _ptr(seq_lens), _ptr(row_index), _ptr(offs),
+                                   len(offs) - 1, _ptr(out), _ptr(lse), ctypes.c_float(scale), _ptr(workspace),
+                                   _nbytes(workspace), _stream_ptr(stream)))
+
+
+def pkv_bucket_counters_host(shape: Shape, policy: Policy, seq_lens_host: np.ndarray, bucket_tokens: int) -> dict:
+    seq = np.ascontiguousarray(seq_lens_host, dtype=np.int32)
+    c = pkv_counters()
+    _check(_lib.pkv_bucket_counters_host(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(seq), int(bucket_tokens),
+                                         ctypes.byref(c)))
+    return c.as_dict()
 
 
 def pkv_merge(shape: Shape, part_m, part_l, part_acc, split_offsets, out, lse=None, stream=None) -> None:

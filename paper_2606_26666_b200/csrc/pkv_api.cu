@@ -170,7 +170,7 @@ pkv_status check_workspace(const void* workspace, size_t bytes, const WorkspaceL
 // Launches decode (+ merge).  known_tasks / known_max_n >= 0: the queue was planned on the host,
 // so launches that have nothing to do are skipped (A13).
 pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, const void* k_cache, const void* v_cache,
-                      const int32_t* block_table, const int32_t* seq_lens, void* out, float* lse, float scale,
+                      const int32_t* block_table, const int32_t* seq_lens, const int32_t* row_index, void* out, float* lse, float scale,
                       const QueuePtrs& qp, const WsPtrs& ws, int64_t known_tasks, int known_max_n, int64_t known_slots,
                       int num_sms, uint32_t stages, bool fused_build, int64_t tasks_cap,
                       cudaStream_t stream, int* decode_launches, int* merge_launches) {
@@ -182,6 +182,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.v_cache = static_cast<const __half*>(v_cache);
     p.block_table = block_table;
     p.seq_lens = seq_lens;
+    p.row_index = row_index;
     p.tasks = qp.tasks;
     p.rowslots = qp.rowslots;
     p.split_offsets = qp.split_offsets;
@@ -196,6 +197,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.dynamic_sched = 1;
     p.force_replan = (rp.flags & PKV_FLAG_TEST_REPLAN) ? 1 : 0;
     p.plan = make_plan_args(s, rp);
+    p.plan.row_index = row_index;
     p.tasks_cap = tasks_cap;
     p.fused_build = fused_build ? 1 : 0;
     p.num_pages = s.num_pages;
@@ -308,16 +310,23 @@ pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_policy* p
     st = check_workspace(workspace, workspace_bytes, L);
     if (st != PKV_OK) return st;
     const WsPtrs ws = carve(workspace, L);
-    const cudaError_t e = launch_builder(*shape, rp, seq_lens_dev, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
+    const cudaError_t e = launch_builder(*shape, rp, seq_lens_dev, nullptr, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
                                          ws.q.rowslots, ws.q.tasks, L.slots_cap, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     return PKV_OK;
 }
 
-pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+}  // extern "C"
+
+namespace {
+
+pkv_status decode_stages(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
                              const void* k_cache, const void* v_cache, const int32_t* block_table,
-                             const int32_t* seq_lens, void* out, float* lse, float scale, uint32_t stages,
-                             void* workspace, size_t workspace_bytes, void* stream) {
+                             const int32_t* seq_lens, const int32_t* row_index, void* out, float* lse, float scale,
+                             uint32_t stages, void* workspace, size_t workspace_bytes, void* stream,
+                             const pkv_shape* layout_shape = nullptr) {
+    // layout_shape: the shape the workspace is carved for (pkv_decode_buckets: the whole batch, so
+    // that the header and the completion counters sit at the same place for every bucket)
     clear_error();
     Resolved rp;
     const int sms = device_sm_count();
@@ -327,7 +336,7 @@ pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_policy* pol
     if (stages & ~(uint32_t)PKV_STAGE_ALL) { set_error("unknown stage bits 0x%x", stages); return PKV_ERR_INVALID_ARG; }
     st = check_decode_ptrs(*shape, q, k_cache, v_cache, block_table, seq_lens, out);
     if (st != PKV_OK) return st;
-    const WorkspaceLayout L = workspace_layout(*shape, rp.S);
+    const WorkspaceLayout L = workspace_layout(layout_shape ? *layout_shape : *shape, rp.S);
     st = check_workspace(workspace, workspace_bytes, L);
     if (st != PKV_OK) return st;
     const WsPtrs ws = carve(workspace, L);
@@ -337,12 +346,74 @@ pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_policy* pol
     const bool fused = (stages & PKV_STAGE_BUILD) && (stages & PKV_STAGE_DECODE) && !(rp.flags & PKV_FLAG_SEPARATE_BUILD) &&
                        rp.kernel == PKV_KERNEL_TMA_MMA && shape->B <= kMaxFusedRows;
     if ((stages & PKV_STAGE_BUILD) && !fused) {
-        const cudaError_t e = launch_builder(*shape, rp, seq_lens, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
+        const cudaError_t e = launch_builder(*shape, rp, seq_lens, row_index, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters,
                                              ws.q.rowslots, ws.q.tasks, L.slots_cap, cs);
         if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     }
-    return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, out, lse, scale, ws.q, ws, -1, -1, -1, sms,
+    return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, row_index, out, lse, scale, ws.q, ws, -1, -1, -1, sms,
                       stages, fused, L.slots_cap, cs, nullptr, nullptr);
+}
+
+}  // namespace
+
+extern "C" {
+
+pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                             const void* k_cache, const void* v_cache, const int32_t* block_table,
+                             const int32_t* seq_lens, void* out, float* lse, float scale, uint32_t stages,
+                             void* workspace, size_t workspace_bytes, void* stream) {
+    return decode_stages(shape, policy, q, k_cache, v_cache, block_table, seq_lens, nullptr, out, lse, scale, stages,
+                         workspace, workspace_bytes, stream);
+}
+
+pkv_status pkv_decode_indexed(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                              const void* k_cache, const void* v_cache, const int32_t* block_table,
+                              const int32_t* seq_lens, const int32_t* row_index, void* out, float* lse, float scale,
+                              void* workspace, size_t workspace_bytes, void* stream) {
+    if (shape && shape->B > kMaxFusedRows) {
+        clear_error();
+        set_error("pkv_decode_indexed: at most %d indexed rows per launch", kMaxFusedRows);
+        return PKV_ERR_UNSUPPORTED;
+    }
+    if (shape && shape->B > 0 && !row_index) {
+        clear_error();
+        set_error("null row_index");
+        return PKV_ERR_INVALID_ARG;
+    }
+    return decode_stages(shape, policy, q, k_cache, v_cache, block_table, seq_lens, row_index, out, lse, scale,
+                         PKV_STAGE_ALL, workspace, workspace_bytes, stream);
+}
+
+pkv_status pkv_decode_buckets(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                              const void* k_cache, const void* v_cache, const int32_t* block_table,
+                              const int32_t* seq_lens, const int32_t* row_index, const int32_t* bucket_offsets_host,
+                              int32_t num_buckets, void* out, float* lse, float scale, void* workspace,
+                              size_t workspace_bytes, void* stream) {
+    clear_error();
+    if (!shape || !policy || num_buckets < 0 || (num_buckets > 0 && (!bucket_offsets_host || !row_index))) {
+        set_error("pkv_decode_buckets: null argument");
+        return PKV_ERR_INVALID_ARG;
+    }
+    if (bucket_offsets_host && (bucket_offsets_host[0] != 0 || bucket_offsets_host[num_buckets] > shape->B)) {
+        set_error("pkv_decode_buckets: bucket_offsets must start at 0 and end at or below B");
+        return PKV_ERR_INVALID_ARG;
+    }
+    // every bucket is a launch pair of its own over the bucket's rows ("one per route
+    // length"); then one more indexed launch for the rows that belong to no bucket (N_i = 0: out = 0)
+    const int32_t nb_rows = num_buckets > 0 ? bucket_offsets_host[num_buckets] : 0;
+    for (int32_t b = 0; b <= num_buckets; ++b) {
+        const int32_t lo = b < num_buckets ? bucket_offsets_host[b] : nb_rows;
+        const int32_t hi = b < num_buckets ? bucket_offsets_host[b + 1] : shape->B;
+        if (hi < lo) { set_error("pkv_decode_buckets: bucket_offsets must be non-decreasing"); return PKV_ERR_INVALID_ARG; }
+        if (hi == lo) continue;
+        pkv_shape sub = *shape;
+        sub.B = hi - lo;
+        if (sub.B > kMaxFusedRows) { set_error("pkv_decode_buckets: at most %d rows per bucket", kMaxFusedRows); return PKV_ERR_UNSUPPORTED; }
+        const pkv_status st = decode_stages(&sub, policy, q, k_cache, v_cache, block_table, seq_lens, row_index + lo, out, lse,
+                                            scale, PKV_STAGE_ALL, workspace, workspace_bytes, stream, shape);
+        if (st != PKV_OK) return st;
+    }
+    return PKV_OK;
 }
 
 pkv_status pkv_decode(const pkv_shape* shape, const pkv_split_policy* policy, const void* q, const void* k_cache,
@@ -597,7 +668,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         }
     }
     st = run_decode(s, rp, ds + im.q, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
-                    reinterpret_cast<const int32_t*>(ds + im.seq_lens), out_dev, nullptr, scale, qp, ws,
+                    reinterpret_cast<const int32_t*>(ds + im.seq_lens), nullptr, out_dev, nullptr, scale, qp, ws,
                     hdr->num_tasks, hdr->max_row_splits, hdr->total_row_slots, sms, PKV_STAGE_ALL, false, L.slots_cap, cs, &dl,
                     &ml);
     if (st != PKV_OK) return st;

@@ -140,6 +140,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
     if (blockIdx.x == 0 && threadIdx.x == 0 && p.hdr != nullptr) p.hdr->launched_merge = 1;   // this launch's mark
     const int so = __ldcg(p.split_offsets + row);
     const int n = __ldcg(p.split_offsets + row + 1) - so;
+    const int orow = request_row(p.row_index, row);   // loaded with the offsets: no extra round trip
     // batch b of this warp: states (b * NB * NW + j * NW + warp) * CS + sub, j = 0 .. NB-1
     auto load_batch = [&](int64_t base_, int n_, int b, float (&mv)[NB], float (&lv)[NB], float4 (&av)[NB]) {
 #pragma unroll
@@ -215,7 +216,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
                 As.z = fmaf(wt, a.z, As.z); As.w = fmaf(wt, a.w, As.w);
             }
         }
-        merge_store(p, (int64_t)row * p.Hq + h, ch, slice == 0 && cl == 0, Mf, Ls, As);
+        merge_store(p, (int64_t)orow * p.Hq + h, ch, slice == 0 && cl == 0, Mf, Ls, As);
         if (blockIdx.x == 0 && lane == 0) PKV_TRACE_STAMP_MERGE(p, 2);
     }
 }
@@ -223,7 +224,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
 }  // namespace
 
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
-                           QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
+                           const int32_t* row_index, QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
                            pkv_task* tasks, int64_t tasks_cap, cudaStream_t stream) {
     BuildArgs a;
     a.seq_lens = seq_lens_dev;
@@ -234,6 +235,7 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
     a.tasks = tasks;
     a.tasks_cap = tasks_cap;
     a.plan = make_plan_args(shape, rp);
+    a.plan.row_index = row_index;
     // one thread per (row, split) pair if that fits in a CTA, 128..1024 threads
     const int64_t want = (int64_t)shape.B * rp.S;
     int threads = 128;

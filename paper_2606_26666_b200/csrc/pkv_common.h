@@ -53,7 +53,8 @@ struct RowSlot {
     int32_t split;
     int32_t tok0;   // token range [tok0, tok1) -- empty when tok0 >= tok1
     int32_t tok1;
-    int32_t pad_[2];
+    int32_t grow;   // request row (= row unless the launch is indexed, pkv_decode_indexed)
+    int32_t pad_;
 };
 static_assert(sizeof(RowSlot) == 32, "RowSlot layout");
 

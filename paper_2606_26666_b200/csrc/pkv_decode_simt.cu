@@ -54,21 +54,22 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
     for (int t = blockIdx.x; t < num_tasks; t += gridDim.x) {
         const pkv_task task = p.tasks[t];
         const int row = task.row, kvh = task.kvh;
-        const int N = plan_len(p.plan, p.seq_lens[row]);
+        const int orow = request_row(p.row_index, row);   // row of q, out, lse, block_table, seq_lens
+        const int N = plan_len(p.plan, p.seq_lens[orow]);
         const int so = p.split_offsets[row];
         const int n_i = p.split_offsets[row + 1] - so;
         const int64_t slot = (int64_t)so * p.Hkv + (int64_t)kvh * n_i + task.split;
         const int tok0 = task.t_begin * p.tile_tokens;
         const int tok1 = min(task.t_end * p.tile_tokens, N);
         if (tok0 >= tok1) {  // empty split: neutral state, before loading Q
-            store_empty_task<G, kWarps>(p, &cb.flag[0], row, kvh, task.split, n_i, slot, tid, 0);
+            store_empty_task<G, kWarps>(p, &cb.flag[0], row, orow, kvh, task.split, n_i, slot, tid, 0);
             continue;
         }
 
         float qf[G][8];
 #pragma unroll
         for (int g = 0; g < G; ++g) {
-            const uint4 u = *reinterpret_cast<const uint4*>(p.q + ((int64_t)row * p.Hq + kvh * G + g) * kD + ch * 8);
+            const uint4 u = *reinterpret_cast<const uint4*>(p.q + ((int64_t)orow * p.Hq + kvh * G + g) * kD + ch * 8);
             unpack8(u, qf[g]);
         }
         float m[G], l[G], acc[G][8];
@@ -80,7 +81,7 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
             for (int c = 0; c < 8; ++c) acc[g][c] = 0.f;
         }
 
-        const int32_t* bt = p.block_table + (int64_t)row * p.max_pages;
+        const int32_t* bt = p.block_table + (int64_t)orow * p.max_pages;
         const int64_t head_off = (int64_t)kvh * p.stride_head + ch * 8;
         // the CTA walks 8 tokens per step (4 warps x 2 half-warps); kUnroll steps are in flight
         for (int base = tok0 + warp * 2; base < tok1; base += 8 * kUnroll) {  // warp-uniform bound
@@ -161,7 +162,7 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
             }
         }
         __syncthreads();
-        finalize_task<G, kWarps, kWarps>(p, cb, 0, 1, row, kvh, task.split, n_i, slot, tid, 0);
+        finalize_task<G, kWarps, kWarps>(p, cb, 0, 1, row, orow, kvh, task.split, n_i, slot, tid, 0);
     }
 }
 

@@ -53,7 +53,7 @@ __host__ __device__ constexpr int producers_for(int HG) { return HG >= 4 ? 1 : (
 struct UnitInfo {
     int unit;   // -1: no more work
     int row, so, n, split, tok0, tok1;   // the unit's RowSlot
-    int pad_;
+    int grow;   // request row: the row of q, out, lse and block_table (= row unless the launch is indexed)
 };
 
 template <int G>
@@ -157,8 +157,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         const int p0 = d.tok0 >> 4;
         int np = d.tok0 < d.tok1 ? ((d.tok1 + 15) >> 4) - p0 : 0;
         np = min(min(np, p.prefetch_pages), p.max_pages - p0);
-        if (d.row >= 0 && d.row < p.B && p0 >= 0) {
-            const int32_t* bt = p.block_table + (int64_t)d.row * p.max_pages + p0;
+        if (d.row >= 0 && d.row < p.B && d.grow >= 0 && p0 >= 0) {
+            const int32_t* bt = p.block_table + (int64_t)d.grow * p.max_pages + p0;
             const int head0 = ((int)blockIdx.x % HGn) * HG;
             for (int j = lane; j < np; j += 32) {
                 const int page = ld_relaxed_s32(bt + j);
@@ -168,7 +168,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 }
             }
             // q rows of the unit's HG*G query heads: HG*G*256 bytes, one 128-byte line per lane
-            const char* qrow = reinterpret_cast<const char*>(p.q + ((int64_t)d.row * p.Hq + head0 * G) * kD);
+            const char* qrow = reinterpret_cast<const char*>(p.q + ((int64_t)d.grow * p.Hq + head0 * G) * kD);
             for (int b = lane * 128; b < HG * G * kD * 2; b += 32 * 128) prefetch_l2(qrow + b);
         }
     }
@@ -216,10 +216,11 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             p.hdr->launched_merge = 0;
         }
         for (int i = blockIdx.x; i < p.B; i += gridDim.x) {   // rows without a task (A9)
-            if ((p.fused_build ? tail.len_s[i] : __ldcg(p.seq_lens + i)) > 0) continue;
+            const int64_t gi = request_row(p.row_index, i);
+            if ((p.fused_build ? tail.len_s[i] : __ldcg(p.seq_lens + gi)) > 0) continue;
             for (int e = lane; e < p.Hq * kD; e += 32) {
-                p.out[(int64_t)i * p.Hq * kD + e] = __float2half_rn(0.f);
-                if (p.lse && e < p.Hq) p.lse[(int64_t)i * p.Hq + e] = -INFINITY;
+                p.out[gi * p.Hq * kD + e] = __float2half_rn(0.f);
+                if (p.lse && e < p.Hq) p.lse[gi * p.Hq + e] = -INFINITY;
             }
         }
         return;
@@ -235,9 +236,9 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             const RowSlot d = tail.first_slot;
             const int p0 = d.tok0 >> 4;
             const int np = d.tok0 < d.tok1 ? min(((d.tok1 + 15) >> 4) - p0, p.max_pages - p0) : 0;
-            if (d.row >= 0 && d.row < p.B && p0 >= 0) {
-                early_row = d.row; early_tok0 = d.tok0; early_tok1 = d.tok1;
-                if (lane < np) early_mine = __ldcg(p.block_table + (int64_t)d.row * p.max_pages + p0 + lane);
+            if (d.row >= 0 && d.row < p.B && d.grow >= 0 && p0 >= 0) {
+                early_row = d.grow; early_tok0 = d.tok0; early_tok1 = d.tok1;
+                if (lane < np) early_mine = __ldcg(p.block_table + (int64_t)d.grow * p.max_pages + p0 + lane);
             }
         }
         if (!p.force_replan && plan_lens_unchanged(plan, p.seq_lens, tail.len_s, lane, err)) {
@@ -279,16 +280,16 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 if (t >= 0 && k == 0) d = tail.first_slot;   // computed by the planner warp
                 else if (t >= 0) d = make_rowslot(plan, tail.so_s, tail.len_s, t / HGn, &tb, &te);
                 u.row = d.row; u.so = d.so; u.n = d.n; u.split = d.split; u.tok0 = d.tok0; u.tok1 = d.tok1;
+                u.grow = d.grow;
             } else {
                 const int4* rsp = reinterpret_cast<const int4*>(p.rowslots + (k == 0 ? t / HGn : min(t, max(num_units - 1, 0)) / HGn));
                 const int4 a = __ldcg(rsp);
                 const int4 b = __ldcg(rsp + 1);
                 if (k == 0) num_units = __ldcg(&p.hdr->total_row_slots) * HGn;
                 if (t >= num_units) t = -1;
-                u.row = a.x; u.so = a.y; u.n = a.z; u.split = a.w; u.tok0 = b.x; u.tok1 = b.y;
+                u.row = a.x; u.so = a.y; u.n = a.z; u.split = a.w; u.tok0 = b.x; u.tok1 = b.y; u.grow = b.z;
             }
             u.unit = t;
-            u.pad_ = 0;
             if (lane == 0) {
                 mbar_wait(rempty0 + 8 * r, ((k / kRing) & 1) ^ 1);
                 tail.ring[r] = u;
@@ -302,7 +303,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 // The slot is released only after its loads have RETURNED: the store below needs
                 // every field (an mbarrier arrive may otherwise overtake loads still in flight).
                 sts_b32(smem_u32(&tail.sink_i[warp]),
-                        (uint32_t)(u.unit + u.row + u.so + u.n + u.split + u.tok0 + u.tok1 + u.pad_));
+                        (uint32_t)(u.unit + u.row + u.so + u.n + u.split + u.tok0 + u.tok1 + u.grow));
                 mbar_arrive(rempty0 + 8 * r);
             }
         }
@@ -323,7 +324,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
             if (k == 0 && tid == 0) PKV_TRACE_STAMP(p, 2);
-            const int row = u.row, hg = u.unit % HGn;
+            const int row = u.grow, hg = u.unit % HGn;   // the producers only need the request row
             const int tok0 = u.tok0, tok1 = u.tok1;
             if (tok0 >= tok1) continue;  // empty split: nothing is staged
             const int p0 = tok0 >> 4;
@@ -385,13 +386,13 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         for (int k = 0;; ++k) {
             const UnitInfo u = next_unit(k);
             if (u.unit < 0) break;
-            const int row = u.row, hg = u.unit % HGn;
+            const int row = u.row, orow = u.grow, hg = u.unit % HGn;
             const int so = u.so, n_i = u.n, split = u.split;
             const int kvh = hg * HG + hl;
             const int64_t slot = (int64_t)so * p.Hkv + (int64_t)kvh * n_i + split;
             const int tok0 = u.tok0, tok1 = u.tok1;
             if (tok0 >= tok1) {
-                store_empty_task<G, WPH>(p, &tail.cb.flag[hl], row, kvh, split, n_i, slot, gtid, 1 + hl);
+                store_empty_task<G, WPH>(p, &tail.cb.flag[hl], row, orow, kvh, split, n_i, slot, gtid, 1 + hl);
                 continue;
             }
             const int p0 = tok0 >> 4;
@@ -400,7 +401,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             // Q^T as the MMA B operand: b0 = Q[head g4][kk*16 + 2*t4 .. +1], b1 = same + 8
             uint32_t qb[8][2];
             {
-                const __half* qrow = p.q + ((int64_t)row * p.Hq + kvh * G + (g4 < G ? g4 : 0)) * kD;
+                const __half* qrow = p.q + ((int64_t)orow * p.Hq + kvh * G + (g4 < G ? g4 : 0)) * kD;
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk) {
                     const uint32_t lo = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + 2 * t4);
@@ -526,7 +527,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 // instruction the 8 lanes of a column write 32 contiguous bytes.
                 if (hA < G) {
                     const bool hasB = hB < G;   // G = 1: column B is padding
-                    const int64_t hrow = (int64_t)row * p.Hq + kvh * G + hA;
+                    const int64_t hrow = (int64_t)orow * p.Hq + kvh * G + hA;
                     if (n_i <= 1) {
                         const float iA = 1.0f / lA, iB = hasB ? 1.0f / lB : 0.f;
                         __half* oA = p.out + hrow * kD + g4;
@@ -567,7 +568,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     }
                 }
                 if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED)
-                    fused_complete<G, 1>(p, &tail.cb.flag[cw], row, kvh, split, n_i, slot, lane, 1 + hl);
+                    fused_complete<G, 1>(p, &tail.cb.flag[cw], row, orow, kvh, split, n_i, slot, lane, 1 + hl);
             } else {
                 if (hA < G) {
                     const bool hasB = hB < G;   // G = 1: column B is padding
@@ -586,7 +587,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     }
                 }
                 group_sync<WPH>(1 + hl);
-                finalize_task<G, WPH, kComputeWarps>(p, tail.cb, hl, HG, row, kvh, split, n_i, slot, gtid, 1 + hl);
+                finalize_task<G, WPH, kComputeWarps>(p, tail.cb, hl, HG, row, orow, kvh, split, n_i, slot, gtid, 1 + hl);
             }
             if (k == 0 && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 6);
         }

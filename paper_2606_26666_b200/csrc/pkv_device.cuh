@@ -19,7 +19,13 @@ struct PlanArgs {   // split policy as the device-side planner needs it
     int32_t B, Hkv, S, tile_tokens, split_mode, chunk_tiles, route, num_sms;
     int32_t flags;        // pkv_flag bits
     int32_t max_tokens;   // max_pages * page_size: the longest row the block table can describe
+    const int32_t* row_index;   // indexed rows (pkv_decode_indexed): launch row i is request row_index[i]; or nullptr
 };
+
+// Request row of launch row i: the row of q, out, lse, block_table and seq_lens it works on.
+__device__ __forceinline__ int32_t request_row(const int32_t* row_index, int i) {
+    return row_index ? __ldcg(row_index + i) : i;
+}
 
 struct DecodeParams {
     const __half* q;            // [B, Hq, d]
@@ -27,6 +33,7 @@ struct DecodeParams {
     const __half* v_cache;
     const int32_t* block_table; // [B, max_pages]
     const int32_t* seq_lens;    // [B]
+    const int32_t* row_index;   // [B] or nullptr: launch row -> request row (q, out, lse, block_table, seq_lens)
     pkv_task* tasks;              // written by the builder / the fused build, read by the SIMT kernel
     RowSlot* rowslots;            // [split_offsets[B]] (row, split) pairs
     int32_t* split_offsets;       // [B+1]
@@ -314,7 +321,7 @@ __device__ __forceinline__ PlanTotals plan_scan(PlanArgs& a, const int32_t* seq_
     const int nthreads = blockDim.x, nwarps = nthreads >> 5;
     const int32_t* lens = seq_lens;
     if (len_out) {   // one global round trip: stage the lengths, plan from the staged copy
-        for (int i = tid; i < a.B; i += nthreads) len_out[i] = plan_len(a, __ldcg(seq_lens + i));
+        for (int i = tid; i < a.B; i += nthreads) len_out[i] = plan_len(a, __ldcg(seq_lens + request_row(a.row_index, i)));
         lens = len_out;
     }
     if (tid == 0) {
@@ -333,8 +340,9 @@ __device__ __forceinline__ PlanTotals plan_scan(PlanArgs& a, const int32_t* seq_
         const int i = base + tid;
         int32_t slots = 0, N = 0, nonempty = 0;
         if (i < a.B) {
-            plan_len_fault(a, seq_lens[i], error_word);
-            N = plan_len(a, lens[i]);
+            const int32_t raw = __ldcg(seq_lens + request_row(a.row_index, i));
+            plan_len_fault(a, raw, error_word);
+            N = len_out ? lens[i] : plan_len(a, raw);
             const RowSplits r = row_splits(N, a.tile_tokens, a.split_mode, a.S, a.chunk_tiles);
             nonempty = r.n;
             slots = a.route == PKV_ROUTE_WORKQUEUE ? r.n : a.S;
@@ -395,7 +403,8 @@ __device__ __forceinline__ int32_t plan_warp_prefix(PlanArgs& a, const int32_t* 
                                                     int32_t* error_word = nullptr) {
 #pragma unroll 4
     for (int i = lane; i < a.B; i += 32) {
-        const int32_t N = SPEC ? ld_relaxed_s32(seq_lens + i) : __ldcg(seq_lens + i);
+        const int32_t gi = !a.row_index ? i : (SPEC ? ld_relaxed_s32(a.row_index + i) : __ldcg(a.row_index + i));
+        const int32_t N = SPEC ? ld_relaxed_s32(seq_lens + gi) : __ldcg(seq_lens + gi);
         if (!SPEC) plan_len_fault(a, N, error_word);
         len_out[i] = plan_len(a, N);
     }
@@ -435,7 +444,8 @@ __device__ __forceinline__ int32_t plan_warp_prefix(PlanArgs& a, const int32_t* 
                 }
                 d.tok0 = tb * a.tile_tokens;
                 d.tok1 = min(te * a.tile_tokens, N);
-                d.pad_[0] = d.pad_[1] = 0;
+                d.grow = !a.row_index ? i : (SPEC ? ld_relaxed_s32(a.row_index + i) : __ldcg(a.row_index + i));
+                d.pad_ = 0;
                 *first = d;
             }
         }
@@ -451,7 +461,7 @@ __device__ __forceinline__ bool plan_lens_unchanged(const PlanArgs& a, const int
                                                     int lane, int32_t* error_word = nullptr) {
     bool same = true;
     for (int i = lane; i < a.B; i += 32) {
-        const int32_t N = __ldcg(seq_lens + i);
+        const int32_t N = __ldcg(seq_lens + request_row(a.row_index, i));
         plan_len_fault(a, N, error_word);
         same &= plan_len(a, N) == len_s[i];
     }
@@ -507,7 +517,8 @@ __device__ __forceinline__ RowSlot make_rowslot(const PlanArgs& a, const int32_t
     }
     d.tok0 = tb * a.tile_tokens;
     d.tok1 = min(te * a.tile_tokens, N);
-    d.pad_[0] = d.pad_[1] = 0;
+    d.grow = request_row(a.row_index, lo);
+    d.pad_ = 0;
     *t_begin = tb;
     *t_end = te;
     return d;
@@ -601,7 +612,7 @@ __device__ __forceinline__ void merge_store(const DecodeParams& p, int64_t o, in
 
 // One warp merges head hh completely (fused path; also any caller without helpers).
 template <int G>
-__device__ __forceinline__ void merge_head_warp(const DecodeParams& p, int64_t slot_base, int n, int row, int kvh,
+__device__ __forceinline__ void merge_head_warp(const DecodeParams& p, int64_t slot_base, int n, int orow, int kvh,
                                                 int hh, int lane) {
     const float M = merge_row_max<G>(p, slot_base, n, hh, lane);
     float L[4];
@@ -613,7 +624,7 @@ __device__ __forceinline__ void merge_head_warp(const DecodeParams& p, int64_t s
     As.y = ((A[0].y + A[1].y) + A[2].y) + A[3].y;
     As.z = ((A[0].z + A[1].z) + A[2].z) + A[3].z;
     As.w = ((A[0].w + A[1].w) + A[2].w) + A[3].w;
-    merge_store(p, (int64_t)row * p.Hq + kvh * G + hh, lane * 4, lane == 0, M, Ls, As);
+    merge_store(p, (int64_t)orow * p.Hq + kvh * G + hh, lane * 4, lane == 0, M, Ls, As);
 }
 
 // ------------------------------------------------------------------ task epilogue
@@ -638,8 +649,8 @@ __device__ __forceinline__ void group_sync(int bar_id) {
 // group that completes the last of the n_i splits (atomic completion counter, self-resetting for
 // graph replay) merges the row's slot range in place.  flag = a shared-memory word of the group.
 template <int G, int NW>
-__device__ __forceinline__ void fused_complete(const DecodeParams& p, int* flag, int row, int kvh, int split, int n_i,
-                                               int64_t slot, int gtid, int bar_id) {
+__device__ __forceinline__ void fused_complete(const DecodeParams& p, int* flag, int row, int orow, int kvh, int split,
+                                               int n_i, int64_t slot, int gtid, int bar_id) {
     __threadfence();  // partial state visible device-wide before the completion count
     group_sync<NW>(bar_id);
     if (gtid == 0) {
@@ -652,7 +663,7 @@ __device__ __forceinline__ void fused_complete(const DecodeParams& p, int* flag,
     if (*flag) {
         __threadfence();
         const int64_t base = slot - split;  // first slot of (row, kvh): DESIGN.md A8
-        for (int hh = gtid >> 5; hh < G; hh += NW) merge_head_warp<G>(p, base, n_i, row, kvh, hh, gtid & 31);
+        for (int hh = gtid >> 5; hh < G; hh += NW) merge_head_warp<G>(p, base, n_i, orow, kvh, hh, gtid & 31);
     }
     group_sync<NW>(bar_id);  // flag may be rewritten after this
 }
@@ -660,12 +671,12 @@ __device__ __forceinline__ void fused_complete(const DecodeParams& p, int* flag,
 // Writes an empty task's result (rect route): neutral partial state, or zeros when
 // the row has a single slot (direct output).  Called by the NW warps that own the task.
 template <int G, int NW>
-__device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* flag, int row, int kvh, int split,
+__device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* flag, int row, int orow, int kvh, int split,
                                                  int n_i, int64_t slot, int gtid, int bar_id) {
     for (int idx = gtid; idx < G * kD; idx += NW * 32) {
         const int hh = idx / kD, dd = idx % kD;
         if (n_i <= 1) {
-            const int64_t o = (int64_t)row * p.Hq + kvh * G + hh;
+            const int64_t o = (int64_t)orow * p.Hq + kvh * G + hh;
             p.out[o * kD + dd] = __float2half_rn(0.f);
             if (p.lse && dd == 0) p.lse[o] = -INFINITY;
         } else {
@@ -676,7 +687,7 @@ __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* fla
             }
         }
     }
-    if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED) fused_complete<G, NW>(p, flag, row, kvh, split, n_i, slot, gtid, bar_id);
+    if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED) fused_complete<G, NW>(p, flag, row, orow, kvh, split, n_i, slot, gtid, bar_id);
 }
 
 // A group of NW warps (rows w0, w0+wstride, ... of `cb`) has processed one task.  Combines the
@@ -687,7 +698,7 @@ __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* fla
 // caller has synchronised after filling `cb`.
 template <int G, int NW, int NWTOT>
 __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<G, NWTOT>& cb, int w0, int wstride,
-                                              int row, int kvh, int split, int n_i, int64_t slot, int gtid,
+                                              int row, int orow, int kvh, int split, int n_i, int64_t slot, int gtid,
                                               int bar_id) {
     for (int idx = gtid; idx < G * kD; idx += NW * 32) {
         const int hh = idx / kD, dd = idx % kD;
@@ -703,7 +714,7 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
             A += wgt * cb.acc[w][hh][dd];
         }
         if (n_i <= 1) {
-            const int64_t o = (int64_t)row * p.Hq + kvh * G + hh;
+            const int64_t o = (int64_t)orow * p.Hq + kvh * G + hh;
             p.out[o * kD + dd] = __float2half_rn(A / L);
             if (p.lse && dd == 0) p.lse[o] = M * p.scale + logf(L);
         } else {
@@ -715,7 +726,7 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
         }
     }
     if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED)
-        fused_complete<G, NW>(p, &cb.flag[w0], row, kvh, split, n_i, slot, gtid, bar_id);
+        fused_complete<G, NW>(p, &cb.flag[w0], row, orow, kvh, split, n_i, slot, gtid, bar_id);
     group_sync<NW>(bar_id);  // cb rows may be refilled after this
 }
 
@@ -723,10 +734,11 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
 __device__ __forceinline__ void zero_empty_rows(const DecodeParams& p) {
     const int per_row = p.Hq * kD;
     for (int i = blockIdx.x; i < p.B; i += gridDim.x) {
-        if (p.seq_lens[i] > 0) continue;
+        const int64_t gi = request_row(p.row_index, i);
+        if (p.seq_lens[gi] > 0) continue;
         for (int e = threadIdx.x; e < per_row; e += blockDim.x) {
-            p.out[(int64_t)i * per_row + e] = __float2half_rn(0.f);
-            if (p.lse && e < p.Hq) p.lse[(int64_t)i * p.Hq + e] = -INFINITY;
+            p.out[gi * per_row + e] = __float2half_rn(0.f);
+            if (p.lse && e < p.Hq) p.lse[gi * p.Hq + e] = -INFINITY;
         }
     }
 }
@@ -757,6 +769,7 @@ inline PlanArgs make_plan_args(const pkv_shape& shape, const Resolved& rp) {
     a.flags = rp.flags;
     const int64_t mt = (int64_t)shape.max_pages * shape.page_size;
     a.max_tokens = (int32_t)(mt < 0x7fffffff ? mt : 0x7fffffff);
+    a.row_index = nullptr;
     return a;
 }
 
@@ -765,7 +778,7 @@ cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStrea
 cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int grid, const void* tmap_k,
                               const void* tmap_v, cudaStream_t stream);
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
-                           QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
+                           const int32_t* row_index, QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
                            pkv_task* tasks, int64_t tasks_cap, cudaStream_t stream);
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream);
 int decode_tma_smem_bytes(int G, int HG);

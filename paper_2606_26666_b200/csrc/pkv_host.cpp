@@ -3,6 +3,9 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
+#include <utility>
+#include <vector>
 
 #include "pkv_common.h"
 
@@ -173,7 +176,7 @@ pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_
             for (int32_t sp = 0; sp < slots; ++sp) {
                 RowSlot rs;
                 std::memset(&rs, 0, sizeof(rs));
-                rs.row = i; rs.so = off; rs.n = slots; rs.split = sp;
+                rs.row = i; rs.so = off; rs.n = slots; rs.split = sp; rs.grow = i;
                 if (r.T > 0) {
                     const int64_t b = (int64_t)sp * r.c, e = (int64_t)(sp + 1) * r.c;
                     const int64_t t0 = (b < r.T ? b : r.T) * rp.tile_tokens, t1 = (e < r.T ? e : r.T) * rp.tile_tokens;
@@ -219,6 +222,73 @@ size_t pkv_workspace_init_bytes(const pkv_shape* shape, const pkv_split_policy* 
     Resolved rp;
     if (validate_and_resolve(shape, policy, 0, /*bound_ok=*/true, &rp) != PKV_OK) return 0;
     return workspace_layout(*shape, rp.S).init_bytes;
+}
+
+pkv_status pkv_plan_buckets_host(const int32_t* seq_lens_host, int32_t B, int32_t bucket_tokens, int32_t* row_index_out,
+                                 int32_t* bucket_offsets_out, int32_t* bucket_lengths_out, int32_t* num_buckets_out) {
+    clear_error();
+    if (B < 0 || bucket_tokens <= 0 || !num_buckets_out || (B > 0 && (!seq_lens_host || !row_index_out || !bucket_offsets_out))) {
+        set_error("pkv_plan_buckets_host: bad argument");
+        return PKV_ERR_INVALID_ARG;
+    }
+    // route length = true length rounded up to the granularity; stable sort of the non-empty rows
+    // by route length (ascending), empty rows last (reading A22)
+    std::vector<std::pair<int64_t, int32_t>> keyed;
+    keyed.reserve((size_t)B);
+    for (int32_t i = 0; i < B; ++i)
+        if (seq_lens_host[i] > 0)
+            keyed.emplace_back(((int64_t)seq_lens_host[i] + bucket_tokens - 1) / bucket_tokens * bucket_tokens, i);
+    std::stable_sort(keyed.begin(), keyed.end(),
+                     [](const std::pair<int64_t, int32_t>& a, const std::pair<int64_t, int32_t>& b) { return a.first < b.first; });
+    int32_t nb = 0, pos = 0;
+    if (bucket_offsets_out) bucket_offsets_out[0] = 0;
+    for (size_t k = 0; k < keyed.size(); ++k) {
+        if (k > 0 && keyed[k].first != keyed[k - 1].first) bucket_offsets_out[++nb] = pos;
+        if (bucket_lengths_out && (k == 0 || keyed[k].first != keyed[k - 1].first))
+            bucket_lengths_out[k == 0 ? 0 : nb] = (int32_t)(keyed[k].first < 0x7fffffff ? keyed[k].first : 0x7fffffff);
+        row_index_out[pos++] = keyed[k].second;
+    }
+    if (!keyed.empty()) bucket_offsets_out[++nb] = pos;
+    for (int32_t i = 0; i < B; ++i)
+        if (seq_lens_host[i] <= 0) row_index_out[pos++] = i;
+    *num_buckets_out = nb;
+    return PKV_OK;
+}
+
+pkv_status pkv_bucket_counters_host(const pkv_shape* shape, const pkv_split_policy* policy, const int32_t* seq_lens_host,
+                                    int32_t bucket_tokens, pkv_counters* out) {
+    clear_error();
+    Resolved rp0;
+    pkv_status st = validate_and_resolve(shape, policy, 0, /*bound_ok=*/false, &rp0);
+    if (st != PKV_OK) return st;
+    if (!out || (shape->B > 0 && !seq_lens_host) || bucket_tokens <= 0) { set_error("pkv_bucket_counters_host: bad argument"); return PKV_ERR_INVALID_ARG; }
+    const int32_t B = shape->B;
+    std::vector<int32_t> index((size_t)B), offs((size_t)B + 1), lens;
+    int32_t nb = 0;
+    st = pkv_plan_buckets_host(seq_lens_host, B, bucket_tokens, index.data(), offs.data(), nullptr, &nb);
+    if (st != PKV_OK) return st;
+    std::memset(out, 0, sizeof(*out));
+    for (int32_t b = 0; b < nb; ++b) {
+        pkv_shape sub = *shape;
+        sub.B = offs[b + 1] - offs[b];
+        Resolved rp;
+        st = validate_and_resolve(&sub, policy, 0, false, &rp);   // the auto split count follows the bucket's size
+        if (st != PKV_OK) return st;
+        lens.assign((size_t)sub.B, 0);
+        for (int32_t i = 0; i < sub.B; ++i) lens[i] = seq_lens_host[index[offs[b] + i]];
+        QueueHeader hdr;
+        plan_host(sub, rp, lens.data(), nullptr, 0, nullptr, nullptr, &hdr);
+        const bool merge = hdr.max_row_splits > 1;
+        out->tasks += hdr.num_tasks;
+        out->empty_tasks += hdr.empty_tasks;
+        out->decode_launches += hdr.num_tasks > 0 ? 1 : 0;
+        out->merge_launches += (merge && rp.merge_mode == PKV_MERGE_SEPARATE) ? 1 : 0;
+        out->useful_kv_bytes += hdr.sum_seq_lens * 2 * shape->Hkv * shape->d * 2;
+        out->merge_bytes += merge ? (int64_t)hdr.num_tasks * rp.G * (shape->d + 2) * 4 : 0;
+        out->num_splits = rp.S;
+        if (hdr.max_row_splits > out->max_row_splits) out->max_row_splits = hdr.max_row_splits;
+    }
+    return PKV_OK;
 }
 
 pkv_status pkv_build_workqueue_host(const pkv_shape* shape, const pkv_split_policy* policy,

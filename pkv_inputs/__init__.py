@@ -33,6 +33,9 @@ from .workloads import (  # noqa: F401
     bimodal_lengths,
     zipf_lengths,
     uniform_lengths,
+    trace_lengths,
+    trace,
+    PROMPT_CYCLE,
     fill_normal_f16,
     fill_pool_torch,
     TUNE_SEED,

@@ -167,6 +167,49 @@ def config5(seed: int = TUNE_SEED, B: int = 128, steps: int = 20, Hkv: int = 8) 
                          seed=seed, rng=rng, Hkv=Hkv)
 
 
+# ---------------------------------------------------------------- the paper's other trace families
+
+PROMPT_CYCLE = (8192, 16384, 32768, 65536)     # PAPER.md:116 "cycles prompt lengths through 8K, 16K, 32K, and 64K"
+
+
+def trace_lengths(family: str, rng: np.random.Generator, B: int, decoded_max: int = 256) -> np.ndarray:
+    """Step-0 context lengths of the trace families of PAPER.md:116 (sec. 3.8).  A request's current
+    length is its prompt length plus the tokens it has decoded so far; the paper prints
+    no decode-length distribution, so the tokens decoded before step 0 are drawn from
+    U[0, decoded_max) per row (decoded_max = 0: every row sits exactly at its prompt length, the
+    case where rows of one prompt class share an exact length bucket).
+      bucketed     prompts cycle through 8K, 16K, 32K, 64K
+      homogeneous  a common 32K prompt, independent decode lengths
+      bimodal      "one long request for every three shorter": rows 3, 7, ... long U[16384, 32768],
+                   the others U[256, 1024] (config 3 uses BASELINE.json's p = 0.5 draw instead)
+      uniform      U[1024, 65536]          zipf  min(65536, 512 k), k ~ Zipf(1.2)"""
+    if family == "bucketed":
+        prompt = np.array([PROMPT_CYCLE[i % 4] for i in range(B)], dtype=np.int64)
+    elif family == "homogeneous":
+        prompt = np.full(B, 32768, dtype=np.int64)
+    elif family == "bimodal":
+        short = rng.integers(256, 1024, size=B, endpoint=True)
+        long_ = rng.integers(16384, 32768, size=B, endpoint=True)
+        prompt = np.where(np.arange(B) % 4 == 3, long_, short).astype(np.int64)
+    elif family == "uniform":
+        return uniform_lengths(rng, B)
+    elif family == "zipf":
+        return zipf_lengths(rng, B)
+    else:
+        raise ValueError(family)
+    decoded = rng.integers(0, decoded_max, size=B) if decoded_max > 0 else np.zeros(B, dtype=np.int64)
+    return (prompt + decoded).astype(np.int32)
+
+
+def trace(family: str, seed: int = TUNE_SEED, B: int = 8, steps: int = 50, decoded_max: int = 256,
+          hole_frac: float = 0.0) -> Workload:
+    """One of the paper's serving traces (main serving traces use rho = 0)."""
+    rng = _rng(seed)
+    lens = trace_lengths(family, rng, B, decoded_max)
+    return make_workload("trace_%s_b%d" % (family, B), lens, steps=steps, hole_frac=hole_frac, seed=seed, rng=rng,
+                         extra={"family": family, "decoded_max": decoded_max})
+
+
 # ---------------------------------------------------------------- random tensors
 
 def fill_normal_f16(shape, seed: int) -> np.ndarray:

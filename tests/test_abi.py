@@ -142,3 +142,35 @@ def test_tasks_cap_too_small_reports_needed_count():
     st = binding._lib.pkv_build_workqueue_host(ctypes.byref(s.c()), ctypes.byref(pol.c()), lens.ctypes.data,
                                                tasks.ctypes.data, 3, off.ctypes.data, ctypes.byref(n))
     assert st == pkv.PKV_ERR_WORKSPACE and n.value == 32
+
+
+def test_bucket_plan_and_counters_match_the_route_oracle():
+    """pkv_plan_buckets_host / pkv_bucket_counters_host against oracle/route_oracle.py (PAPER.md:71,
+    93, 204-206; readings A22, A23): grouping, order, and Table 4's bucket row (16.00 launches,
+    8.00 merge launches, 2048 tasks, 4.06 MB)."""
+    from oracle import route_oracle as ro
+    rng = np.random.Generator(np.random.PCG64(5))
+    cases = [[5000, 0, 4999, 5000, 17, 4990, 32], [0, 0], [7], list(rng.integers(0, 70000, size=64)),
+             [8192, 16384, 32768, 65536] * 3, [32768] * 8]
+    for lens in cases:
+        for gran in (1, 16, 1024, 8192, 1 << 20):
+            index, offs, blen = pkv.pkv_plan_buckets_host(np.array(lens, np.int32), gran)
+            want = ro.group_buckets(lens, gran)
+            assert len(offs) == len(want) + 1 and list(blen) == [k for k, _ in want]
+            assert [list(index[offs[b]:offs[b + 1]]) for b in range(len(want))] == [rows for _, rows in want]
+            assert sorted(index) == list(range(len(lens)))
+            assert list(index[offs[-1]:]) == [i for i, n in enumerate(lens) if n <= 0]
+            for pol in (pkv.Policy(tile_tokens=32, num_splits=32, route=pkv.ROUTE_RECT),
+                        pkv.Policy(tile_tokens=32, num_splits=5, route=pkv.ROUTE_WORKQUEUE, merge_mode=pkv.MERGE_FUSED),
+                        pkv.Policy(tile_tokens=16, num_splits=1, route=pkv.ROUTE_RECT)):
+                c = pkv.pkv_bucket_counters_host(shape(len(lens)), pol, np.array(lens, np.int32), gran)
+                w, _ = ro.bucket_route(lens, 8, 4, 128, wq.Policy(tile_tokens=pol.tile_tokens, num_splits=pol.num_splits,
+                                                                   route=pol.route, merge_mode=pol.merge_mode), gran)
+                assert (c["decode_launches"] + c["merge_launches"], c["merge_launches"], c["tasks"], c["empty_tasks"],
+                        c["merge_bytes"], c["useful_kv_bytes"]) == (w.launches, w.merge_launches, w.tasks, w.empty_tasks,
+                                                                    w.merge_bytes, w.useful_kv_bytes), (lens, gran, pol)
+    seq = [16384 + 977 * i for i in range(8)]
+    c = pkv.pkv_bucket_counters_host(shape(8), pkv.Policy(tile_tokens=32, num_splits=32, route=pkv.ROUTE_RECT),
+                                     np.array(seq, np.int32), 1)
+    assert (c["decode_launches"] + c["merge_launches"], c["merge_launches"], c["tasks"]) == (16, 8, 2048)
+    assert "%.2f" % (c["merge_bytes"] / 2 ** 20) == "4.06"
