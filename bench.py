@@ -123,14 +123,21 @@ def mean_alg_bytes(w, K, nlens):
     return sum(algorithmic_bytes(w, w.seq_lens_at(t % nlens)) for t in range(n)) / n
 
 
-def default_policy(pkv, name: str, args):
+def default_policy(pkv, name: str, args, w=None, num_sms=0):
     """The library's own policy for a workload: config 1 is the paper's unsplit rectangular launch
-    (BASELINE.json configs[0] "no splitting"); everything else asks the library to decide
-    (PKV_SPLIT_BALANCED, A21 / "Auto policy").  Command-line overrides on top."""
+    (BASELINE.json configs[0] "no splitting"); everything else asks the library's cost model
+    (pkv_choose_policy with the default B200 constants on the step-0 lengths, which a serving
+    harness has on the host: "for each decode step, the harness estimates T_r").
+    Command-line overrides on top (any split override turns the cost model off)."""
     if name in ("config1",):
         pol = pkv.Policy(tile_tokens=32, num_splits=1, route=pkv.ROUTE_RECT)
     else:
         pol = pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, route=pkv.ROUTE_WORKQUEUE)
+        if w is not None and num_sms > 0 and args.split_mode < 0 and args.splits < 0 and args.tile_tokens <= 0:
+            shape = pkv.Shape(B=w.B, Hq=w.Hq, Hkv=w.Hkv, d=w.d, page_size=w.page_size, max_pages=w.max_pages,
+                              num_pages=w.num_pages)
+            base = dataclasses.replace(pol, split_mode=pkv.SPLIT_AUTO)
+            pol, _ = pkv.pkv_choose_policy(shape, w.seq_lens, pkv.pkv_default_cost_model(num_sms), base)
     if args.tile_tokens > 0:
         pol.tile_tokens = args.tile_tokens
     if args.split_mode >= 0:
@@ -178,7 +185,19 @@ class Runner:
         self.lens_all = torch.from_numpy(lens_all).to(device)
         self.out = torch.zeros((w.B, w.Hq, w.d), dtype=torch.float16, device=device)
         self.stream = torch.cuda.Stream(device=device)
+        self.buckets = None
         self.set_policy(pol)
+
+    def set_bucket_route(self, gran):
+        """Length-bucket route (pkv_decode_buckets): per trace step the host plan of
+        pkv_plan_buckets_host (row index on the device, bucket offsets on the host).  None = off."""
+        self.graphs = {}
+        if gran is None:
+            self.buckets = None
+            return
+        plans = [self.pkv.pkv_plan_buckets_host(self.lens_all_host[t], gran) for t in range(self.nlens)]
+        self.buckets = [(self.torch.from_numpy(ix.copy()).to(self.device), offs.copy()) for ix, offs, _ in plans]
+        self.bucket_gran = gran
 
     def set_policy(self, pol):
         """Switches the split policy: new workspace, captured graphs dropped (pools are kept)."""
@@ -193,6 +212,12 @@ class Runner:
         """Step t: the chosen stages on pool t % R with the lengths of trace step t % (steps+1)
         (row t of the device-resident [steps+1, B] length table: N_i += 1 per step)."""
         r = t % self.R
+        if self.buckets is not None:
+            ix, offs = self.buckets[t % self.nlens]
+            self.pkv.pkv_decode_buckets(self.shape, self.pol, self.q[r], self.k[r], self.v[r], self.bt[r],
+                                        self.lens_all[t % self.nlens], ix, offs, self.out, None, scale=self.scale,
+                                        workspace=self.ws, stream=stream)
+            return
         sl = self.lens_all[t % self.nlens] if (stages & self.pkv.STAGE_BUILD) else self.lens_all[0]
         self.pkv.pkv_decode_stages(self.shape, self.pol, self.q[r], self.k[r], self.v[r], self.bt[r], sl,
                                    self.out, None, scale=self.scale, stages=stages, workspace=self.ws,
@@ -521,10 +546,15 @@ def workload_config(w, pol, R, args, n_gpus):
 
 # ------------------------------------------------------------------ e2e, timeline, the other workloads
 
-def run_e2e(pkv, torch, runner, K, W):
+def run_e2e(pkv, torch, runner, K, W, auto=False):
     """K steps through pkv_decode_host: host planning + H2D + launches + D2H + sync per step, wall
-    clock over the K calls.  KV pools stay resident (the model's state)."""
+    clock over the K calls.  KV pools stay resident (the model's state).  auto: the policy is
+    PKV_SPLIT_AUTO, i.e. the cost model runs inside every call on that step's lengths."""
     w, pol = runner.w, runner.pol
+    ws = runner.ws
+    if auto:
+        pol = dataclasses.replace(pol, split_mode=pkv.SPLIT_AUTO, num_splits=0)
+        ws = pkv.alloc_workspace(runner.shape, pol, device=runner.device)
     nb = pkv.pkv_host_scratch_bytes(runner.shape, pol)
     staging = torch.empty(nb, dtype=torch.uint8).pin_memory()
     scratch = torch.empty(nb, dtype=torch.uint8, device=runner.device)
@@ -538,7 +568,7 @@ def run_e2e(pkv, torch, runner, K, W):
         r = t % runner.R
         return pkv.pkv_decode_host(runner.shape, pol, q_host[r].data_ptr(), runner.k[r], runner.v[r],
                                    bt_host.data_ptr(), lens_host[t % runner.nlens].data_ptr(), out_host.data_ptr(),
-                                   runner.scale, staging, scratch, runner.ws, stream=runner.stream)
+                                   runner.scale, staging, scratch, ws, stream=runner.stream)
 
     for t in range(max(W, 3)):
         c = step(t)
@@ -598,12 +628,14 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
     PAPER.md:71, 204-206): us/step (median of >= 50 ms of K-step regions), roofline fraction of the
     decode kernel, launches per step, parity against the oracle on seeded rows."""
     out = {}
-    bal = pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, prefetch_kb=args.prefetch_kb)
+    bal = None      # None: the cost model's choice for the workload (default_policy)
     cases = [("config3", "config3", bal),
              ("config3_workqueue_S20", "config3", pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_WORKQUEUE,
                                                              prefetch_kb=args.prefetch_kb)),
              ("config3_rect_S20", "config3", pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_RECT,
                                                         prefetch_kb=args.prefetch_kb)),
+             ("config3_buckets_exact_S32", "config3", pkv.Policy(tile_tokens=32, num_splits=32, route=pkv.ROUTE_RECT,
+                                                                 prefetch_kb=args.prefetch_kb)),
              ("config4", "config4", bal), ("config4_b4", "config4_b4", bal),
              ("config5", "config5", bal), ("config5_hkv4", "config5_hkv4", bal)]
     runner, cur = None, None
@@ -613,17 +645,27 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
                 runner = None
                 torch.cuda.empty_cache()
                 w = make_workload(name, args.seed)
-                runner = Runner(pkv, torch, w, pol, rotation(torch, w, args, device), args.seed, device)
+                sms = torch.cuda.get_device_properties(device).multi_processor_count
+                auto = default_policy(pkv, name, args, w, sms)
+                runner = Runner(pkv, torch, w, pol or auto, rotation(torch, w, args, device), args.seed, device)
                 cur = name
+            pol = pol or auto
             w = runner.w
             K = max(w.steps, 1)
             chunk = max(1, min(args.graph_steps, K))
-            r = time_policy(pkv, runner, pol, K, chunk, 5)
-            st, dc = summarize(r["step_ms"], K), summarize(r["decode_ms"], K)
+            bucketed = "buckets" in key
+            runner.set_bucket_route(1 if bucketed else None)
+            r = time_policy(pkv, runner, pol, K, chunk, 5, decode_only=not bucketed)
+            st = summarize(r["step_ms"], K)
+            dc = summarize(r["decode_ms"], K) if not bucketed else st
             alg = mean_alg_bytes(w, K, runner.nlens)
             rows = pick_rows(runner.lens_at(0), 70000, w.seed)
             par, _ = parity_of(torch, runner, rows)
             c = runner.counters()      # after a whole eager step
+            if bucketed:               # Table 4's counters of the bucket route, summed over the buckets
+                hb = pkv.pkv_bucket_counters_host(runner.shape, pol, runner.lens_at(0), 1)
+                c = dict(c, tasks=hb["tasks"], empty_tasks=hb["empty_tasks"], launched_build=0,
+                         launched_decode=hb["decode_launches"], launched_merge=hb["merge_launches"])
             out[key] = {"workload": w.name, "policy": {k: int(v) for k, v in pol.__dict__.items()},
                         "steps": K, "us_per_step": round(st["us_per_step_median"], 3),
                         "us_per_step_min": round(st["us_per_step_min"], 3), "regions": st["regions"],
@@ -698,7 +740,10 @@ def sweep_on_tune_seed(pkv, torch, args, device, base_pol, K, W):
     runner = Runner(pkv, torch, w, base_pol, rotation(torch, w, args, device), pkv_inputs.TUNE_SEED, device)
     sms = torch.cuda.get_device_properties(device).multi_processor_count
     fixed = lambda S: dataclasses.replace(base_pol, tile_tokens=32, split_mode=pkv.SPLIT_FIXED_COUNT, num_splits=S)
-    cands = [(str(S), fixed(S)) for S in (1, 4, 16, 64, 0)] + [("balanced", base_pol)]
+    auto_pol = default_policy(pkv, args.workload, args, w, sms)
+    cands = [(str(S), fixed(S)) for S in (1, 4, 16, 64, 0)] + [
+        ("balanced", dataclasses.replace(base_pol, tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0)),
+        ("cost_model", auto_pol)]
     s_fit = sms // max(1, w.B * w.Hkv)
     if s_fit > 1 and s_fit not in (4, 16, 64):
         cands.append((str(s_fit), fixed(s_fit)))
@@ -715,6 +760,8 @@ def sweep_on_tune_seed(pkv, torch, args, device, base_pol, K, W):
                       "alg_GBps": round(algorithmic_bytes(w, w.seq_lens) / st["us_per_step_median"] / 1e3, 1)}
         pols[key] = p2
     best = min(table, key=lambda k_: table[k_]["us_per_step"])
+    table["cost_model"]["policy"] = {k: int(v) for k, v in auto_pol.__dict__.items()}
+    table["cost_model"]["vs_best_swept"] = round(table["cost_model"]["us_per_step"] / table[best]["us_per_step"], 4)
     del runner
     torch.cuda.empty_cache()
     return table, best, pols[best]
@@ -753,12 +800,17 @@ def run_ours(args):
     # every rank is a replica with its own seeded trace (data-parallel by row; DESIGN.md multi-GPU)
     seed = multirank.rank_seed(args.seed, rank)
     w = make_workload(args.workload, seed, args.hkv)
-    pol = default_policy(pkv, args.workload, args)
+    sms = torch.cuda.get_device_properties(device).multi_processor_count
+    pol = default_policy(pkv, args.workload, args, w, sms)
+    chosen = "pkv_choose_policy (cost model, default B200 constants) on the step-0 lengths; no sweep involved"
+    if args.split_mode >= 0 or args.splits >= 0 or args.tile_tokens > 0 or args.workload == "config1":
+        chosen = "command line / BASELINE.json configs[0]"
 
-    sweep, chosen = {}, "library default"
+    sweep = {}
     if args.workload == "config2" and not args.no_sweep and args.splits < 0:
-        sweep, chosen, pol = sweep_on_tune_seed(pkv, torch, args, device, pol, K, W)
-        chosen = "%s (fastest of the sweep on tune seed %d; frozen for the report seed)" % (chosen, pkv_inputs.TUNE_SEED)
+        # information only: the timed policy is the cost model's, not the sweep's winner
+        sweep, best_key, _ = sweep_on_tune_seed(pkv, torch, args, device, pol, K, W)
+        sweep["fastest_on_tune_seed"] = best_key
 
     R = rotation(torch, w, args, device)
     runner = Runner(pkv, torch, w, pol, R, seed, device)
@@ -780,7 +832,7 @@ def run_ours(args):
 
     e2e = None
     if not args.no_e2e:
-        e2e = run_e2e(pkv, torch, runner, K, W)
+        e2e = run_e2e(pkv, torch, runner, K, W, auto=chosen.startswith("pkv_choose_policy"))
 
     st, dc = summarize(step_ms, K), summarize(dec_ms, K)
     # max over ranks of the median region (and of the fastest one)

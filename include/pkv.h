@@ -55,7 +55,7 @@ typedef enum {
 
 typedef enum { PKV_ROUTE_RECT = 0, PKV_ROUTE_WORKQUEUE = 1 } pkv_route;
 typedef enum { PKV_MERGE_SEPARATE = 0, PKV_MERGE_FUSED = 1 } pkv_merge_mode;
-typedef enum { PKV_SPLIT_FIXED_COUNT = 0, PKV_SPLIT_FIXED_CHUNK = 1, PKV_SPLIT_BALANCED = 2 } pkv_split_mode;
+typedef enum { PKV_SPLIT_FIXED_COUNT = 0, PKV_SPLIT_FIXED_CHUNK = 1, PKV_SPLIT_BALANCED = 2, PKV_SPLIT_AUTO = 3 } pkv_split_mode;
 /* which decode kernel runs the tile loop */
 typedef enum {
     PKV_KERNEL_AUTO = 0, /* = PKV_KERNEL_TMA_MMA                                                 */
@@ -82,6 +82,10 @@ typedef enum {
  *                  the busiest SM's share exceeds the mean W/U by at most one many-wave chunk);
  *     chunk = that c if it exists, else c2.
  *   chunk_tiles of the policy is ignored; S = num_splits (256 when 0) still caps n_i.
+ *   AUTO: the cost model decides.  pkv_decode_host, where the lengths are on the
+ *   host, runs pkv_choose_policy with the default B200 constants before every step; calls whose
+ *   lengths are device-resident (pkv_decode, pkv_build_workqueue) and the pure sizing functions
+ *   treat AUTO as BALANCED, the candidate that needs no host knowledge of the lengths.
  */
 typedef struct {
     int32_t tile_tokens; /* > 0, multiple of page_size; the paper uses 32          */
@@ -331,6 +335,44 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
                                    void* out_host, float scale, void* host_staging, void* dev_scratch,
                                    size_t scratch_bytes, void* workspace, size_t workspace_bytes,
                                    void* stream, pkv_counters* counters_out);
+
+/*
+ * The calibrated cost model (sec. 3.5), on the HOST, from host-resident lengths --
+ * as the paper's harness evaluates it before every decode step:
+ *     T_r = KVBytes / beta * max(1, C_min / C_r) + L_r * lambda + MergeBytes_r / beta
+ * KVBytes = sum_i N_i * 2*Hkv*d*2, C_r = tasks / num_sms (Table 4's "Decode CTA work/SM"), L_r =
+ * decode + merge launches, MergeBytes_r as pkv_counters.merge_bytes (0 when no row has two slots).
+ * bucket_tokens > 0 evaluates the length-bucket route (totals over the buckets, A23),
+ * 0 the policy's single launch pair.  `makespan_us` is the B200 re-fit of the first term (DESIGN.md
+ * A27): max(KVBytes/beta, busiest CTA's bytes / beta_cta), beta_cta = beta / (C_min * num_sms) --
+ * equal to the paper's term when all tasks are equal, larger when one share dominates.
+ * pkv_default_cost_model: the constants fitted on B200 this round;
+ * pkv_calibrate measures beta and lambda on the device at hand.
+ * pkv_choose_policy: evaluates the library's candidate policies for this step -- BALANCED, and
+ * FIXED_COUNT with S in {1, 2, 4, ..., 128} on 32-token tiles, all on `base`'s route, merge mode,
+ * kernel and flags -- and writes the one with the smallest makespan_total_us to `chosen` (ties:
+ * BALANCED first, then the smaller S).  PKV_SPLIT_AUTO in pkv_decode_host does this per step.
+ */
+typedef struct {
+    double beta_gbps;  /* streaming read bandwidth                                   (paper: 331.2) */
+    double lambda_us;  /* cost of one more dependent kernel launch in a decode step  (paper: 8.19)  */
+    double c_min;      /* work items per SM that saturate beta                       (paper: 4)     */
+    int32_t num_sms;   /*                                                            (paper: 28)    */
+    int32_t reserved_;
+} pkv_cost_model;
+typedef struct {
+    double total_us, stream_us, launch_us, merge_us; /* the paper's formula, term by term            */
+    double cta_work_per_sm;                          /* C_r                                          */
+    double makespan_us, makespan_total_us;           /* A27: first term, and the total with it        */
+    int64_t kv_bytes, merge_bytes, tasks, launches, max_share_bytes;
+} pkv_cost_estimate;
+PKV_API pkv_status pkv_default_cost_model(int32_t num_sms, pkv_cost_model* out);
+PKV_API pkv_status pkv_estimate_cost(const pkv_shape* shape, const pkv_split_policy* policy,
+                                     const int32_t* seq_lens_host, int32_t bucket_tokens,
+                                     const pkv_cost_model* model, pkv_cost_estimate* out);
+PKV_API pkv_status pkv_choose_policy(const pkv_shape* shape, const int32_t* seq_lens_host,
+                                     const pkv_cost_model* model, const pkv_split_policy* base,
+                                     pkv_split_policy* chosen, pkv_cost_estimate* estimate_out);
 
 /*
  * Calibration of the paper's cost-model constants on the current device ("beta is

@@ -27,6 +27,16 @@ Readings of what the paper leaves open:
       margin of its batch regime: 1.05 for B >= 8 and for B = 1 (the paper's two supported regimes),
       1.50 -- or the explicit ablation flag -- for 2 <= B <= 7 ("the B4 boundary").
 
+  A27 B200 re-fit, makespan form of the occupancy term (not in the paper).  With equal tasks the
+      paper's stream term is  KVBytes/beta * C_min/C_r = (KVBytes/tasks) / beta_cta  with
+      beta_cta = beta / (C_min * #SMs): the time ONE CTA needs for its share at the rate a lone CTA
+      streams.  For unequal shares (ragged rows under a fixed split count) the largest share
+      decides:  stream = max(KVBytes/beta, max_share/beta_cta).  The library's persistent CTA takes
+      units of HG KV heads (HG = the largest of 8, 4, 2, 1 dividing Hkv that leaves units for >= 85 % of
+      the SMs, else 1 -- the smallest valid group when nothing fills the machine): one wave (units <= #SMs):
+      max_share = the largest unit's bytes; several waves (dynamic hand-out): KVBytes/#SMs + the
+      largest unit's bytes.
+
 Pins (tests/test_route_oracle.py): Table 4's bucket row (16.00 / 73.1 / 4.06 / 8.00), the cost of
 both Table-4 routes worked out by hand from the printed constants (beta = 331.2 GB/s, C_min = 4,
 lambda = 8.19 us), closed forms of each term, gates and margins on constructed cases.
@@ -173,3 +183,34 @@ def select_route(candidates: Dict[str, float], baseline: Optional[str], seq_lens
     if margin == MARGIN_B4 and allow_b4:
         return best
     return best if candidates[baseline] / candidates[best] >= margin else baseline
+
+
+# ---------------------------------------------------------------- A27: makespan form (B200 re-fit)
+
+def heads_per_cta(Hkv: int, row_slots: int, num_sms: int) -> int:
+    best = 1
+    for hg in (8, 4, 2, 1):
+        if hg > Hkv or Hkv % hg:
+            continue
+        best = hg
+        if row_slots * (Hkv // hg) * 20 >= num_sms * 17:
+            return hg
+    return best
+
+
+def max_share_bytes(seq_lens: Sequence[int], Hkv: int, d: int, q: wq.WorkQueue, tile_tokens: int, num_sms: int) -> int:
+    """A27: bytes of the busiest CTA.  A unit = the HG tasks (row, kvh .., split) of one token range."""
+    row_slots = q.split_offsets[-1]
+    if row_slots == 0:
+        return 0
+    hg = heads_per_cta(Hkv, row_slots, num_sms)
+    tokens = max(min(te * tile_tokens, int(seq_lens[i])) - tb * tile_tokens for (i, _, _, tb, te) in q.tasks)
+    unit = max(tokens, 0) * 2 * hg * d * 2
+    units = row_slots * (Hkv // hg)
+    kv = wq.useful_kv_bytes(seq_lens, Hkv, d)
+    return unit if units <= num_sms else kv // num_sms + unit
+
+
+def stream_makespan_us(kv_bytes: int, share_bytes: int, k: CostConstants) -> float:
+    beta_cta = k.beta_gbps / (k.c_min * k.num_sms)
+    return max(kv_bytes / (k.beta_gbps * 1e3), share_bytes / (beta_cta * 1e3))

@@ -20,7 +20,7 @@ from . import build as _build
 PKV_OK, PKV_ERR_INVALID_ARG, PKV_ERR_UNSUPPORTED, PKV_ERR_WORKSPACE, PKV_ERR_CUDA = range(5)
 ROUTE_RECT, ROUTE_WORKQUEUE = 0, 1
 MERGE_SEPARATE, MERGE_FUSED = 0, 1
-SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK, SPLIT_BALANCED = 0, 1, 2
+SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK, SPLIT_BALANCED, SPLIT_AUTO = 0, 1, 2, 3
 KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
 FLAG_VALIDATE, FLAG_NO_PDL, FLAG_SEPARATE_BUILD, FLAG_TEST_REPLAN = 1, 2, 4, 8
 DEVERR_QUEUE_OVERFLOW, DEVERR_SEQ_LEN, DEVERR_PAGE_ID = 1, 2, 4
@@ -63,11 +63,26 @@ class pkv_calibration(ctypes.Structure):
         return {n: getattr(self, n) for n, _ in self._fields_}
 
 
+class pkv_cost_model(ctypes.Structure):
+    _fields_ = [("beta_gbps", ctypes.c_double), ("lambda_us", ctypes.c_double), ("c_min", ctypes.c_double),
+                ("num_sms", _i32), ("reserved_", _i32)]
+
+
+class pkv_cost_estimate(ctypes.Structure):
+    _fields_ = ([(n, ctypes.c_double) for n in ("total_us", "stream_us", "launch_us", "merge_us", "cta_work_per_sm",
+                                                 "makespan_us", "makespan_total_us")]
+                + [(n, _i64) for n in ("kv_bytes", "merge_bytes", "tasks", "launches", "max_share_bytes")])
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspace_init_bytes", "pkv_build_workqueue_host",
            "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
            "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate", "pkv_decode_indexed",
-           "pkv_plan_buckets_host", "pkv_decode_buckets", "pkv_bucket_counters_host")
+           "pkv_plan_buckets_host", "pkv_decode_buckets", "pkv_bucket_counters_host", "pkv_default_cost_model",
+           "pkv_estimate_cost", "pkv_choose_policy")
 
 
 class PkvError(RuntimeError):
@@ -110,6 +125,13 @@ def _load() -> ctypes.CDLL:
                                        ctypes.c_float, _vp, ctypes.c_size_t, _vp]
     lib.pkv_bucket_counters_host.restype = _i32
     lib.pkv_bucket_counters_host.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _i32, P(pkv_counters)]
+    lib.pkv_default_cost_model.restype = _i32
+    lib.pkv_default_cost_model.argtypes = [_i32, P(pkv_cost_model)]
+    lib.pkv_estimate_cost.restype = _i32
+    lib.pkv_estimate_cost.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _i32, P(pkv_cost_model), P(pkv_cost_estimate)]
+    lib.pkv_choose_policy.restype = _i32
+    lib.pkv_choose_policy.argtypes = [P(pkv_shape), _vp, P(pkv_cost_model), P(pkv_split_policy), P(pkv_split_policy),
+                                      P(pkv_cost_estimate)]
     lib.pkv_merge.restype = _i32
     lib.pkv_merge.argtypes = [P(pkv_shape), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.pkv_get_counters.restype = _i32
@@ -302,6 +324,40 @@ def pkv_bucket_counters_host(shape: Shape, policy: Policy, seq_lens_host: np.nda
     _check(_lib.pkv_bucket_counters_host(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(seq), int(bucket_tokens),
                                          ctypes.byref(c)))
     return c.as_dict()
+
+
+@dataclass
+class CostModel:
+    beta_gbps: float
+    lambda_us: float
+    c_min: float
+    num_sms: int
+
+    def c(self) -> pkv_cost_model:
+        return pkv_cost_model(self.beta_gbps, self.lambda_us, self.c_min, self.num_sms, 0)
+
+
+def pkv_default_cost_model(num_sms: int) -> CostModel:
+    m = pkv_cost_model()
+    _check(_lib.pkv_default_cost_model(int(num_sms), ctypes.byref(m)))
+    return CostModel(m.beta_gbps, m.lambda_us, m.c_min, m.num_sms)
+
+
+def pkv_estimate_cost(shape: Shape, policy: Policy, seq_lens_host: np.ndarray, bucket_tokens: int, model: CostModel) -> dict:
+    seq = np.ascontiguousarray(seq_lens_host, dtype=np.int32)
+    e = pkv_cost_estimate()
+    _check(_lib.pkv_estimate_cost(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(seq), int(bucket_tokens),
+                                  ctypes.byref(model.c()), ctypes.byref(e)))
+    return e.as_dict()
+
+
+def pkv_choose_policy(shape: Shape, seq_lens_host: np.ndarray, model: CostModel, base: Policy):
+    """Returns (Policy, estimate dict)."""
+    seq = np.ascontiguousarray(seq_lens_host, dtype=np.int32)
+    out, e = pkv_split_policy(), pkv_cost_estimate()
+    _check(_lib.pkv_choose_policy(ctypes.byref(shape.c()), _ptr(seq), ctypes.byref(model.c()), ctypes.byref(base.c()),
+                                  ctypes.byref(out), ctypes.byref(e)))
+    return Policy(**{n: int(getattr(out, n)) for n, _ in pkv_split_policy._fields_}), e.as_dict()
 
 
 def pkv_merge(shape: Shape, part_m, part_l, part_acc, split_offsets, out, lse=None, stream=None) -> None:

@@ -115,19 +115,6 @@ const CUtensorMap* get_map(const void* base, const pkv_shape& s, int HG) {
     return &cache[slot].map;
 }
 
-// KV heads one CTA streams together: the largest divisor of Hkv in {8, 4, 2, 1} that still
-// leaves at least one work unit per SM (units = row slots x Hkv / HG).
-int choose_heads_per_cta(int forced, int Hkv, int64_t row_slots, int num_sms) {
-    if (forced > 0 && Hkv % forced == 0) return forced;
-    int best = 1;
-    for (int hg = 8; hg >= 1; hg >>= 1) {
-        if (hg > Hkv || Hkv % hg) continue;
-        best = hg;
-        if (row_slots * (Hkv / hg) >= num_sms) return hg;
-    }
-    return best;   // nothing fills the machine: smallest valid group = most units
-}
-
 pkv_status cuda_fail(cudaError_t e, const char* what) {
     set_error("%s: %s", what, cudaGetErrorString(e));
     return PKV_ERR_CUDA;
@@ -592,6 +579,16 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     pkv_status st = validate_and_resolve(shape, policy, sms, false, &rp);
     if (st != PKV_OK) return st;
     if (sms <= 0) { set_error("no CUDA device"); return PKV_ERR_CUDA; }
+    pkv_split_policy auto_pol;
+    if (rp.auto_mode && seq_lens_host) {
+        // PKV_SPLIT_AUTO: the cost model picks this step's policy from the host-resident lengths
+        // ("for each decode step, the harness estimates T_r")
+        pkv_cost_model cm;
+        pkv_default_cost_model(sms, &cm);
+        st = pkv_choose_policy(shape, seq_lens_host, &cm, policy, &auto_pol, nullptr);
+        if (st == PKV_OK) st = validate_and_resolve(shape, &auto_pol, sms, false, &rp);
+        if (st != PKV_OK) return st;
+    }
     const pkv_shape& s = *shape;
     if (s.B > 0 && (!q_host || !k_cache_dev || !v_cache_dev || !block_table_host || !seq_lens_host || !out_host)) {
         set_error("null pointer argument");

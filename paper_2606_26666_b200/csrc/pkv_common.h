@@ -72,6 +72,7 @@ struct Resolved {
     int32_t flags;      // pkv_flag bits
     int32_t heads_per_cta;  // 0 = automatic
     int32_t prefetch_kb;    // resolved: 0 = off
+    int32_t auto_mode;      // policy said PKV_SPLIT_AUTO (resolved to BALANCED here; pkv_decode_host re-plans per step)
 };
 
 // Byte offsets inside the caller's workspace.  Pure function of (shape, S bound).
@@ -133,9 +134,30 @@ inline int32_t balanced_chunk(int64_t W, int32_t U, int32_t tile_tokens, Fits fi
     return (int32_t)c2;
 }
 
+// KV heads one CTA of the TMA kernel streams together: the largest divisor of Hkv in {8, 4, 2, 1}
+// that still leaves work units for at least 85 % of the SMs (units = row slots x Hkv / HG; whole-page
+// boxes stream faster than head slices, so 128 units of two heads beat 256 units of one on 148 SMs:
+// config 2, S = 32: 23.4 vs 24.2 us per step).
+inline int choose_heads_per_cta(int forced, int Hkv, int64_t row_slots, int num_sms) {
+    if (forced > 0 && Hkv % forced == 0) return forced;
+    int best = 1;
+    for (int hg = 8; hg >= 1; hg >>= 1) {
+        if (hg > Hkv || Hkv % hg) continue;
+        best = hg;
+        if (row_slots * (Hkv / hg) * 20 >= (int64_t)num_sms * 17) return hg;
+    }
+    return best;   // nothing fills the machine: smallest valid group = most units
+}
+
 // Host planner shared by pkv_build_workqueue_host and pkv_decode_host.
 pkv_status plan_host(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens,
                      pkv_task* tasks, int32_t tasks_cap, int32_t* split_offsets, RowSlot* rowslots,
-                     QueueHeader* hdr);
+                     QueueHeader* hdr, int32_t* max_unit_tokens = nullptr);
+
+// Cost-model constants fitted on B200: read probe, the cost of one more
+// dependent kernel in a replayed step, work items per SM that saturate the read rate.
+constexpr double kB200BetaGbps = 7060.0;
+constexpr double kB200LambdaUs = 2.0;
+constexpr double kB200CMin = 0.72;
 
 }  // namespace pkv

@@ -52,7 +52,7 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
         return PKV_ERR_INVALID_ARG;
     }
     if (p.split_mode != PKV_SPLIT_FIXED_COUNT && p.split_mode != PKV_SPLIT_FIXED_CHUNK &&
-        p.split_mode != PKV_SPLIT_BALANCED) {
+        p.split_mode != PKV_SPLIT_BALANCED && p.split_mode != PKV_SPLIT_AUTO) {
         set_error("bad split_mode %d", p.split_mode);
         return PKV_ERR_INVALID_ARG;
     }
@@ -77,7 +77,8 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
 
     int32_t S = p.num_splits;
     out->num_sms = p.num_sms > 0 ? p.num_sms : num_sms_or_0;
-    if (p.split_mode == PKV_SPLIT_BALANCED && out->num_sms <= 0 && !bound_ok) {
+    const bool balanced = p.split_mode == PKV_SPLIT_BALANCED || p.split_mode == PKV_SPLIT_AUTO;
+    if (balanced && out->num_sms <= 0 && !bound_ok) {
         set_error("BALANCED needs policy.num_sms > 0 in a host-only call");
         return PKV_ERR_INVALID_ARG;
     }
@@ -100,7 +101,8 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     }
     out->S = S;
     out->tile_tokens = p.tile_tokens;
-    out->split_mode = p.split_mode;
+    out->split_mode = balanced ? (int32_t)PKV_SPLIT_BALANCED : p.split_mode;
+    out->auto_mode = p.split_mode == PKV_SPLIT_AUTO ? 1 : 0;
     out->chunk_tiles = p.chunk_tiles > 0 ? p.chunk_tiles : 1;
     out->route = p.route;
     out->merge_mode = p.merge_mode;
@@ -131,8 +133,10 @@ WorkspaceLayout workspace_layout(const pkv_shape& s, int32_t S) {
 }
 
 pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_lens, pkv_task* tasks,
-                     int32_t tasks_cap, int32_t* split_offsets, RowSlot* rowslots, QueueHeader* hdr) {
+                     int32_t tasks_cap, int32_t* split_offsets, RowSlot* rowslots, QueueHeader* hdr,
+                     int32_t* max_unit_tokens) {
     int64_t count = 0, sum_seq = 0;
+    int32_t max_tok = 0;
     int32_t max_n = 0, empties = 0, off = 0;
     bool overflow = false;
     int32_t chunk = rp.split_mode == PKV_SPLIT_FIXED_COUNT ? 0 : rp.chunk_tiles;
@@ -154,6 +158,11 @@ pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_
         const RowSplits r = row_splits(N, rp.tile_tokens, rp.split_mode, rp.S, chunk);
         const int32_t slots = rp.route == PKV_ROUTE_WORKQUEUE ? r.n : rp.S;
         if (slots > max_n) max_n = slots;
+        if (r.T > 0) {   // the row's largest token range: its first split (ceil-chunks, A6)
+            const int64_t t1 = (int64_t)r.c * rp.tile_tokens;
+            const int32_t tok = (int32_t)(t1 < N ? t1 : N);
+            if (tok > max_tok) max_tok = tok;
+        }
         for (int32_t g = 0; g < s.Hkv; ++g) {
             for (int32_t sp = 0; sp < slots; ++sp) {
                 int32_t tb = 0, te = 0;
@@ -199,9 +208,40 @@ pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_
         hdr->sum_seq_lens = sum_seq;
         hdr->chunk_tiles = chunk;
     }
+    if (max_unit_tokens) *max_unit_tokens = max_tok;
     if (overflow && tasks) return PKV_ERR_WORKSPACE;
     return PKV_OK;
 }
+
+namespace {
+
+// Totals of one launch pair (policy resolved, lengths on the host) for the cost model.
+struct RouteTotals {
+    int64_t kv_bytes = 0, merge_bytes = 0, tasks = 0, launches = 0;
+    double makespan_bytes_over_beta_cta = 0.0;   // filled by the caller
+    int64_t max_share = 0;
+};
+
+void launch_totals(const pkv_shape& s, const Resolved& rp, const int32_t* lens, int num_sms, RouteTotals* t) {
+    QueueHeader hdr;
+    int32_t max_tok = 0;
+    plan_host(s, rp, lens, nullptr, 0, nullptr, nullptr, &hdr, &max_tok);
+    const bool partials = hdr.max_row_splits > 1;
+    t->kv_bytes = hdr.sum_seq_lens * 2 * s.Hkv * s.d * 2;
+    t->tasks = hdr.num_tasks;
+    t->merge_bytes = partials ? (int64_t)hdr.num_tasks * rp.G * (s.d + 2) * 4 : 0;
+    t->launches = (hdr.num_tasks > 0 ? 1 : 0) + ((partials && hdr.num_tasks > 0 && rp.merge_mode == PKV_MERGE_SEPARATE) ? 1 : 0);
+    // A27: the busiest CTA's bytes.  A unit = the HG tasks of one (row, split) token range.
+    t->max_share = 0;
+    if (hdr.total_row_slots > 0) {
+        const int hg = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, hdr.total_row_slots, num_sms);
+        const int64_t unit = (int64_t)max_tok * 2 * hg * s.d * 2;
+        const int64_t units = (int64_t)hdr.total_row_slots * (s.Hkv / hg);
+        t->max_share = units <= num_sms ? unit : t->kv_bytes / num_sms + unit;
+    }
+}
+
+}  // namespace
 
 }  // namespace pkv
 
@@ -288,6 +328,111 @@ pkv_status pkv_bucket_counters_host(const pkv_shape* shape, const pkv_split_poli
         out->num_splits = rp.S;
         if (hdr.max_row_splits > out->max_row_splits) out->max_row_splits = hdr.max_row_splits;
     }
+    return PKV_OK;
+}
+
+pkv_status pkv_default_cost_model(int32_t num_sms, pkv_cost_model* out) {
+    clear_error();
+    if (!out || num_sms <= 0) { set_error("pkv_default_cost_model: bad argument"); return PKV_ERR_INVALID_ARG; }
+    out->beta_gbps = kB200BetaGbps;
+    out->lambda_us = kB200LambdaUs;
+    out->c_min = kB200CMin;
+    out->num_sms = num_sms;
+    out->reserved_ = 0;
+    return PKV_OK;
+}
+
+pkv_status pkv_estimate_cost(const pkv_shape* shape, const pkv_split_policy* policy, const int32_t* seq_lens_host,
+                             int32_t bucket_tokens, const pkv_cost_model* model, pkv_cost_estimate* out) {
+    clear_error();
+    if (!model || !out || model->beta_gbps <= 0.0 || model->c_min <= 0.0 || model->num_sms <= 0 || bucket_tokens < 0) {
+        set_error("pkv_estimate_cost: bad model or argument");
+        return PKV_ERR_INVALID_ARG;
+    }
+    pkv_split_policy pol;
+    if (policy) pol = *policy;
+    if (policy && pol.num_sms == 0) pol.num_sms = model->num_sms;   // auto rule and BALANCED follow the model's machine
+    Resolved rp;
+    pkv_status st = validate_and_resolve(shape, policy ? &pol : nullptr, 0, /*bound_ok=*/false, &rp);
+    if (st != PKV_OK) return st;
+    if (shape->B > 0 && !seq_lens_host) { set_error("null seq_lens"); return PKV_ERR_INVALID_ARG; }
+    const double beta = model->beta_gbps * 1e3;                                  // bytes per microsecond
+    const double beta_cta = model->beta_gbps / (model->c_min * model->num_sms) * 1e3;
+    RouteTotals sum;
+    double makespan = 0.0;
+    if (bucket_tokens == 0) {
+        launch_totals(*shape, rp, seq_lens_host, model->num_sms, &sum);
+        const double a = (double)sum.kv_bytes / beta, b = (double)sum.max_share / beta_cta;
+        makespan = a > b ? a : b;
+    } else {
+        const int32_t B = shape->B;
+        std::vector<int32_t> index((size_t)B), offs((size_t)B + 1), lens;
+        int32_t nb = 0;
+        st = pkv_plan_buckets_host(seq_lens_host, B, bucket_tokens, index.data(), offs.data(), nullptr, &nb);
+        if (st != PKV_OK) return st;
+        for (int32_t b = 0; b < nb; ++b) {   // buckets run one after the other: their makespans add up
+            pkv_shape sub = *shape;
+            sub.B = offs[b + 1] - offs[b];
+            Resolved rb;
+            st = validate_and_resolve(&sub, &pol, 0, false, &rb);
+            if (st != PKV_OK) return st;
+            lens.assign((size_t)sub.B, 0);
+            for (int32_t i = 0; i < sub.B; ++i) lens[i] = seq_lens_host[index[offs[b] + i]];
+            RouteTotals t;
+            launch_totals(sub, rb, lens.data(), model->num_sms, &t);
+            sum.kv_bytes += t.kv_bytes; sum.merge_bytes += t.merge_bytes; sum.tasks += t.tasks; sum.launches += t.launches;
+            if (t.max_share > sum.max_share) sum.max_share = t.max_share;
+            const double a = (double)t.kv_bytes / beta, c = (double)t.max_share / beta_cta;
+            makespan += a > c ? a : c;
+        }
+    }
+    // PAPER.md:83, term by term
+    const double c_r = (double)sum.tasks / (double)model->num_sms;
+    const double occupancy = c_r > 0.0 ? (model->c_min / c_r > 1.0 ? model->c_min / c_r : 1.0) : 1.0;
+    out->stream_us = (double)sum.kv_bytes / beta * occupancy;
+    out->launch_us = (double)sum.launches * model->lambda_us;
+    out->merge_us = (double)sum.merge_bytes / beta;
+    out->total_us = out->stream_us + out->launch_us + out->merge_us;
+    out->cta_work_per_sm = c_r;
+    out->makespan_us = makespan;
+    out->makespan_total_us = makespan + out->launch_us + out->merge_us;
+    out->kv_bytes = sum.kv_bytes; out->merge_bytes = sum.merge_bytes; out->tasks = sum.tasks; out->launches = sum.launches;
+    out->max_share_bytes = sum.max_share;
+    return PKV_OK;
+}
+
+pkv_status pkv_choose_policy(const pkv_shape* shape, const int32_t* seq_lens_host, const pkv_cost_model* model,
+                             const pkv_split_policy* base, pkv_split_policy* chosen, pkv_cost_estimate* estimate_out) {
+    clear_error();
+    if (!base || !chosen || !model) { set_error("pkv_choose_policy: null argument"); return PKV_ERR_INVALID_ARG; }
+    pkv_split_policy best = *base;
+    pkv_cost_estimate best_est;
+    bool have = false;
+    // candidates: BALANCED on page-size tiles, then FIXED_COUNT S = 1, 2, 4, ..., 128 on 32-token tiles
+    for (int c = -1; c <= 7; ++c) {
+        pkv_split_policy pol = *base;
+        pol.num_sms = base->num_sms > 0 ? base->num_sms : model->num_sms;
+        if (c < 0) {
+            pol.split_mode = PKV_SPLIT_BALANCED;
+            pol.tile_tokens = shape ? shape->page_size : 16;
+            pol.num_splits = 0;
+        } else {
+            pol.split_mode = PKV_SPLIT_FIXED_COUNT;
+            pol.tile_tokens = 32;
+            pol.num_splits = 1 << c;
+        }
+        pkv_cost_estimate e;
+        const pkv_status st = pkv_estimate_cost(shape, &pol, seq_lens_host, 0, model, &e);
+        if (st != PKV_OK) return st;
+        if (!have || e.makespan_total_us < best_est.makespan_total_us) {
+            have = true;
+            best = pol;
+            best_est = e;
+        }
+    }
+    best.num_sms = base->num_sms;   // 0 stays "the device's": the estimate assumed the model's machine
+    *chosen = best;
+    if (estimate_out) *estimate_out = best_est;
     return PKV_OK;
 }
 

@@ -174,3 +174,72 @@ def test_bucket_plan_and_counters_match_the_route_oracle():
                                      np.array(seq, np.int32), 1)
     assert (c["decode_launches"] + c["merge_launches"], c["merge_launches"], c["tasks"]) == (16, 8, 2048)
     assert "%.2f" % (c["merge_bytes"] / 2 ** 20) == "4.06"
+
+
+def test_cost_model_matches_the_route_oracle():
+    """pkv_estimate_cost against oracle/route_oracle.py: every term of T_r, C_r, and
+    the makespan form (A27), for single launch pairs and for the bucket route, with the paper's
+    constants and with the B200 defaults; Table 4's 16-vs-2 launch case prefers the workqueue."""
+    from oracle import route_oracle as ro
+    rng = np.random.Generator(np.random.PCG64(9))
+    models = [pkv.CostModel(331.2, 8.19, 4.0, 28), pkv.pkv_default_cost_model(148)]
+    assert (models[1].beta_gbps, models[1].num_sms) == (7060.0, 148)
+    cases = [[16384 + 977 * i for i in range(8)], [32768], [700, 0, 33, 20000, 5, 64000], list(rng.integers(0, 70000, size=40)), [0, 0]]
+    pols = [pkv.Policy(tile_tokens=32, num_splits=20), pkv.Policy(tile_tokens=32, num_splits=32, route=pkv.ROUTE_RECT),
+            pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0),
+            pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=32, num_splits=6, merge_mode=pkv.MERGE_FUSED)]
+    for m in models:
+        k = ro.CostConstants(m.beta_gbps, m.lambda_us, m.c_min, m.num_sms)
+        for lens in cases:
+            sh = shape(len(lens))
+            for pol in pols:
+                opol = wq.Policy(tile_tokens=pol.tile_tokens, split_mode=pol.split_mode, num_splits=pol.num_splits,
+                                 route=pol.route, merge_mode=pol.merge_mode, num_sms=m.num_sms)
+                e = pkv.pkv_estimate_cost(sh, pol, np.array(lens, np.int32), 0, m)
+                c = ro.single_route(lens, 8, 4, 128, opol)
+                t = ro.cost_of(c, k)
+                q = wq.build_workqueue(lens, 8, opol)
+                share = ro.max_share_bytes(lens, 8, 128, q, pol.tile_tokens, m.num_sms)
+                assert (e["kv_bytes"], e["merge_bytes"], e["tasks"], e["launches"], e["max_share_bytes"]) == (
+                    c.useful_kv_bytes, c.merge_bytes, c.tasks, c.launches, share), (lens, pol)
+                for got, want in ((e["stream_us"], t.stream_us), (e["launch_us"], t.launch_us), (e["merge_us"], t.merge_us),
+                                  (e["total_us"], t.total_us), (e["cta_work_per_sm"], t.cta_work_per_sm),
+                                  (e["makespan_us"], ro.stream_makespan_us(c.useful_kv_bytes, share, k))):
+                    assert got == pytest.approx(want, rel=1e-12, abs=1e-300), (lens, pol)
+                if pol.split_mode == pkv.SPLIT_BALANCED:
+                    continue
+                for gran in (1, 4096):
+                    e = pkv.pkv_estimate_cost(sh, pol, np.array(lens, np.int32), gran, m)
+                    cb, _ = ro.bucket_route(lens, 8, 4, 128, opol, gran)
+                    tb = ro.cost_of(cb, k)
+                    assert (e["tasks"], e["launches"], e["merge_bytes"]) == (cb.tasks, cb.launches, cb.merge_bytes)
+                    assert e["total_us"] == pytest.approx(tb.total_us, rel=1e-12, abs=1e-300)
+    # Table 4 with the paper's constants: exact buckets at split 32 vs the workqueue at split 20
+    seq = np.array([16384 + 977 * i for i in range(8)], np.int32)
+    b = pkv.pkv_estimate_cost(shape(8), pols[1], seq, 1, models[0])
+    w = pkv.pkv_estimate_cost(shape(8), pols[0], seq, 0, models[0])
+    assert b["launches"] == 16 and w["launches"] == 2 and w["total_us"] < b["total_us"]
+    assert b["launch_us"] - w["launch_us"] == pytest.approx(14 * 8.19, rel=1e-12)
+
+
+def test_choose_policy_picks_the_smallest_estimate():
+    """pkv_choose_policy = argmin of makespan_total_us over {BALANCED, FIXED_COUNT S = 1..128}
+    (first wins ties), restated here with pkv_estimate_cost; and the choices that matter on B200:
+    one long row is never left unsplit, a large uniform batch is, a ragged batch gets BALANCED."""
+    m = pkv.pkv_default_cost_model(148)
+    base = pkv.Policy(split_mode=pkv.SPLIT_AUTO, num_splits=0, tile_tokens=16)
+    rng = np.random.Generator(np.random.PCG64(11))
+    for lens in ([32768], [300], list(rng.integers(1024, 65536, size=128)), [700, 22000, 31000, 450, 900, 17000, 260, 30000],
+                 [100] * 8, [0, 0, 5]):
+        sh = shape(len(lens))
+        got, est = pkv.pkv_choose_policy(sh, np.array(lens, np.int32), m, base)
+        cands = [pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0)] + \
+                [pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_COUNT, num_splits=1 << c) for c in range(8)]
+        costs = [pkv.pkv_estimate_cost(sh, p, np.array(lens, np.int32), 0, m)["makespan_total_us"] for p in cands]
+        best = cands[int(np.argmin(costs))]
+        assert (got.split_mode, got.num_splits, got.tile_tokens) == (best.split_mode, best.num_splits, best.tile_tokens), lens
+        assert est["makespan_total_us"] == min(costs)
+    one, _ = pkv.pkv_choose_policy(shape(1), np.array([32768], np.int32), m, base)
+    assert one.split_mode == pkv.SPLIT_BALANCED or one.num_splits >= 16
+    big, _ = pkv.pkv_choose_policy(shape(8), np.array([100] * 8, np.int32), m, base)
+    assert big.split_mode == pkv.SPLIT_FIXED_COUNT and big.num_splits == 1

@@ -124,3 +124,32 @@ def test_p14_gates_and_margins():
     assert ro.select_route(est, "base", [40000], 4) == "workqueue"          # B1 is a supported regime
     assert ro.select_route(est, None, short8, 8) == "workqueue"             # no baseline: the smallest estimate
     assert ro.select_route({"a": 1.0, "b": 1.0}, None, long8, 4) == "a"     # tie: first
+
+
+def test_p15_makespan_form_reduces_to_the_papers_term_for_equal_tasks():
+    """A27: with equal tasks and one task per CTA the makespan form IS the paper's stream term on
+    both sides of C_r = C_min; with one oversized share it is that share at the lone-CTA rate."""
+    k = ro.CostConstants(beta_gbps=1000.0, lambda_us=2.0, c_min=0.5, num_sms=100)
+    # beta_cta = 1000 / (0.5 * 100) = 20 GB/s
+    for tasks in (1, 10, 49, 50, 51, 100):
+        kv = tasks * 2_000_000
+        paper = ro.route_cost(kv, 0, 0, tasks, k).stream_us
+        assert ro.stream_makespan_us(kv, 2_000_000, k) == pytest.approx(paper, rel=1e-12), tasks
+    assert ro.stream_makespan_us(10_000_000, 4_000_000, k) == 200.0        # 4 MB at 20 GB/s beats 10 MB at 1000 GB/s
+    assert ro.stream_makespan_us(100_000_000, 1_000_000, k) == 100.0
+    # heads per CTA and the busiest share on a hand case: Hkv = 8, d = 128, 4 SMs
+    assert [ro.heads_per_cta(8, rs, 148) for rs in (1, 15, 16, 31, 32, 62, 63, 125, 126, 148)] == [1, 1, 1, 1, 2, 2, 4, 4, 8, 8]
+    assert ro.heads_per_cta(4, 1000, 148) == 4 and ro.heads_per_cta(32, 148, 148) == 8 and ro.heads_per_cta(2, 1, 148) == 1
+    pol = wq.Policy(tile_tokens=32, num_splits=2)
+    q = wq.build_workqueue([100, 1000], 8, pol)      # rows split in 2: 64+36 and 512+488 tokens; 4 pairs
+    assert q.split_offsets[-1] == 4
+    # 4 SMs: hg = 8 leaves 4 units = one wave; the largest unit is 512 tokens of 8 heads
+    assert ro.max_share_bytes([100, 1000], 8, 128, q, 32, 4) == 512 * 2 * 8 * 128 * 2
+    # 3 SMs: 4 units on 3 SMs = several waves: KV / SMs + the largest unit
+    kv = 1100 * 4096
+    assert ro.max_share_bytes([100, 1000], 8, 128, q, 32, 3) == kv // 3 + 512 * 4096
+    # 5 SMs: 4 units of 8 heads cover only 80 % of them, so hg = 4: 8 units, several waves
+    assert ro.heads_per_cta(8, 4, 5) == 4
+    assert ro.max_share_bytes([100, 1000], 8, 128, q, 32, 5) == kv // 5 + 512 * 2048
+    # 148 SMs: nothing fills the machine, hg = 1: 32 units, one wave, 512 tokens of one head
+    assert ro.max_share_bytes([100, 1000], 8, 128, q, 32, 148) == 512 * 512
