@@ -556,26 +556,30 @@ def run_e2e(pkv, torch, runner, K, W, auto=False):
         pol = dataclasses.replace(pol, split_mode=pkv.SPLIT_AUTO, num_splits=0)
         ws = pkv.alloc_workspace(runner.shape, pol, device=runner.device)
     nb = pkv.pkv_host_scratch_bytes(runner.shape, pol)
-    staging = torch.empty(nb, dtype=torch.uint8).pin_memory()
-    scratch = torch.empty(nb, dtype=torch.uint8, device=runner.device)
+    # one (staging, scratch) pair per rotating KV pool: the pair holds that pool's block table
+    staging = [torch.zeros(nb, dtype=torch.uint8).pin_memory() for _ in range(runner.R)]
+    scratch = [torch.empty(nb, dtype=torch.uint8, device=runner.device) for _ in range(runner.R)]
     q_host = [runner.q[r].cpu().pin_memory() for r in range(runner.R)]
     bt_host = torch.from_numpy(np.ascontiguousarray(w.block_table)).pin_memory()
     out_host = torch.empty((w.B, w.Hq, w.d), dtype=torch.float16).pin_memory()
     lens_host = [torch.from_numpy(runner.lens_all_host[t].copy()).pin_memory() for t in range(runner.nlens)]
-    c = None
+    # the public API a serving loop uses: pkv.HostDecoder (one ctypes call into pkv_decode_host per step)
+    dec = [pkv.HostDecoder(runner.shape, pol, runner.k[r], runner.v[r], staging[r], scratch[r], ws, runner.scale,
+                           stream=runner.stream) for r in range(runner.R)]
+    qp = [q_host[r].data_ptr() for r in range(runner.R)]
+    lp = [x.data_ptr() for x in lens_host]
+    btp, outp, R, nl = bt_host.data_ptr(), out_host.data_ptr(), runner.R, runner.nlens
 
     def step(t):
-        r = t % runner.R
-        return pkv.pkv_decode_host(runner.shape, pol, q_host[r].data_ptr(), runner.k[r], runner.v[r],
-                                   bt_host.data_ptr(), lens_host[t % runner.nlens].data_ptr(), out_host.data_ptr(),
-                                   runner.scale, staging, scratch, ws, stream=runner.stream)
+        dec[t % R](qp[t % R], btp, lp[t % nl], outp)
 
     for t in range(max(W, 3)):
-        c = step(t)
+        step(t)
     torch.cuda.synchronize(runner.device)
     t0 = time.perf_counter()
     for t in range(K):
-        c = step(t)
+        step(t)
+    c = dec[(K - 1) % R].counters
     torch.cuda.synchronize(runner.device)
     return time.perf_counter() - t0, c
 

@@ -318,15 +318,22 @@ PKV_API pkv_status pkv_workspace_partials(const pkv_shape* shape, const pkv_spli
  * metadata is planned on the host and uploaded; bench.py's e2e leg).  The K/V page pool is the
  * model's resident state and stays on the device; q, block_table and seq_lens come from the
  * host, out goes back to the host.  The call
- *   1. plans the workqueue on the host from seq_lens_host (as pkv_build_workqueue_host),
- *   2. packs header, split_offsets, seq_lens, q, block_table and the task list into
- *      `host_staging` and copies that image to `dev_scratch` with ONE cudaMemcpyAsync,
- *   3. launches decode (+ merge) -- skipping launches the plan shows to be empty, so
- *      decode/merge launch counts equal the oracle's (A13) -- and
+ *   1. plans on the host from seq_lens_host -- with PKV_SPLIT_AUTO the cost model first picks the
+ *      step's policy -- but only the COUNTS of the queue (tasks, max_i n_i, (row, split) pairs):
+ *      they decide which launches happen, so decode/merge launch counts equal the oracle's
+ *      (A13); the queue itself is derived from the uploaded lengths inside the decode
+ *      kernel (fused build) and is bit-identical to pkv_build_workqueue_host's,
+ *   2. copies seq_lens and q to `dev_scratch` with ONE cudaMemcpyAsync, and of the block table only
+ *      the rows whose used entries changed since the previous call on the same (host_staging,
+ *      dev_scratch) pair -- `host_staging` keeps the shadow; a growing row changes one entry every
+ *      page_size steps, so most steps upload no table bytes at all,
+ *   3. launches decode (+ merge), and
  *   4. gets out to out_host -- the kernels write it there directly when out_host is pinned,
  *      device-mapped memory (zero copy), else one cudaMemcpyAsync -- and SYNCHRONISES the stream.
- * host_staging: host memory of pkv_host_scratch_bytes() bytes (pinned recommended);
- * dev_scratch: device memory of the same size, 256-byte aligned.  counters_out may be NULL.
+ * host_staging: host memory of pkv_host_scratch_bytes() bytes (pinned recommended), zeroed (or
+ * never used with another dev_scratch) before its first use; dev_scratch: device memory of the same
+ * size, 256-byte aligned; the pair must be passed together from step to step.  counters_out may be
+ * NULL.
  */
 PKV_API size_t pkv_host_scratch_bytes(const pkv_shape* shape, const pkv_split_policy* policy);
 PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* policy,

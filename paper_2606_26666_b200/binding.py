@@ -405,6 +405,33 @@ def pkv_decode_host(shape: Shape, policy: Policy, q_host, k_cache_dev, v_cache_d
     return c.as_dict()
 
 
+class HostDecoder:
+    """pkv_decode_host with everything that does not change from step to step marshalled ONCE
+    (shape, policy, caches, staging / scratch / workspace, stream): a serving loop then pays one
+    ctypes call per decode step.  Still argument marshalling only.  Per step pass raw addresses
+    (``tensor.data_ptr()`` / ``array.ctypes.data``) of q, block_table, seq_lens and out."""
+
+    def __init__(self, shape: Shape, policy: Policy, k_cache_dev, v_cache_dev, host_staging, dev_scratch, workspace,
+                 scale: float, stream=None):
+        self._keep = (k_cache_dev, v_cache_dev, host_staging, dev_scratch, workspace, stream)
+        self._shape, self._policy, self._counters = shape.c(), policy.c(), pkv_counters()
+        self._head = (ctypes.byref(self._shape), ctypes.byref(self._policy))
+        self._k, self._v = _vp(_ptr(k_cache_dev)), _vp(_ptr(v_cache_dev))
+        self._tail = (ctypes.c_float(scale), _vp(_ptr(host_staging)), _vp(_ptr(dev_scratch)),
+                      ctypes.c_size_t(min(_nbytes(host_staging), _nbytes(dev_scratch))), _vp(_ptr(workspace)),
+                      ctypes.c_size_t(_nbytes(workspace)), _vp(_stream_ptr(stream)), ctypes.byref(self._counters))
+        self._fn = _lib.pkv_decode_host
+
+    def __call__(self, q_host: int, block_table_host: int, seq_lens_host: int, out_host: int) -> None:
+        st = self._fn(*self._head, q_host, self._k, self._v, block_table_host, seq_lens_host, out_host, *self._tail)
+        if st != PKV_OK:
+            _check(st)
+
+    @property
+    def counters(self) -> dict:
+        return self._counters.as_dict()
+
+
 def pkv_calibrate(dev_buffer, stream=None) -> dict:
     """Measures beta (read bandwidth) and lambda (launch overhead) on the current device."""
     c = pkv_calibration()

@@ -535,26 +535,79 @@ namespace pkv {
 namespace {
 
 // Image of one step's host inputs, identical in the pinned staging buffer and in dev_scratch:
-//   [QueueHeader][split_offsets B+1][seq_lens B][q B*Hq*d f16][block_table B*max_pages][rowslots B*S][tasks ...]
-// followed (device only) by the FP16 output.  Tasks are last so that one H2D copy of
-// (tasks_off + num_tasks * 20) bytes moves exactly what the step needs.
-struct HostImage {
-    size_t hdr, split_offsets, seq_lens, q, block_table, rowslots, tasks, tasks_end, out, total;
+//   [StageHeader][seq_lens B][q B*Hq*d f16][block_table B*max_pages]
+// followed (device only) by the FP16 output.  seq_lens and q are adjacent: one H2D copy moves
+// both.  The block table in `staging` is the SHADOW of what dev_scratch holds: a step uploads only
+// the rows whose used entries differ from it (a growing row changes one entry every page_size steps).
+struct StageHeader {
+    uint64_t magic;
+    const void* table_src;   // block_table_host the shadow was made from (informational)
+    const void* dev;         // the dev_scratch the shadow mirrors
+    int32_t B, max_pages;
+    int64_t pad_[3];
 };
-HostImage host_image(const pkv_shape& s, int32_t S) {
+constexpr uint64_t kStageMagic = 0x706b765f73746731ull;   // "pkv_stg1"
+
+struct HostImage {
+    size_t hdr, seq_lens, q, block_table, out, total;
+};
+HostImage host_image(const pkv_shape& s) {
     HostImage h;
     size_t off = 0;
-    h.hdr = off;           off = align_up(off + sizeof(QueueHeader), 256);
-    h.split_offsets = off; off = align_up(off + 4 * ((size_t)s.B + 1), 256);
+    h.hdr = off;           off = align_up(off + sizeof(StageHeader), 256);
     h.seq_lens = off;      off = align_up(off + 4 * (size_t)s.B, 256);
     h.q = off;             off = align_up(off + 2 * (size_t)s.B * s.Hq * s.d, 256);
     h.block_table = off;   off = align_up(off + 4 * (size_t)s.B * s.max_pages, 256);
-    h.rowslots = off;      off = align_up(off + sizeof(RowSlot) * (size_t)s.B * S, 256);
-    h.tasks = off;         off = align_up(off + sizeof(pkv_task) * (size_t)s.B * s.Hkv * S, 256);
-    h.tasks_end = off;
     h.out = off;           off = align_up(off + 2 * (size_t)s.B * s.Hq * s.d, 256);
     h.total = off;
     return h;
+}
+
+// Device pointer of a pinned, device-mapped host buffer (else nullptr).  The last answers are cached
+// per thread (serving loops pass the same few buffers every step; a cudaPointerGetAttributes call
+// costs more than a microsecond).  A buffer that is freed and re-registered at the same address
+// keeps its mapping, so a stale hit is still a valid answer for pinned memory; a pageable buffer is
+// never cached as mapped.
+void* mapped_device_pointer(const void* host, size_t align) {
+    struct Entry { const void* host; void* dev; };
+    thread_local Entry cache[8] = {};
+    thread_local int next = 0;
+    for (const Entry& e : cache)
+        if (e.host == host && host != nullptr) return reinterpret_cast<uintptr_t>(e.dev) % align == 0 ? e.dev : nullptr;
+    cudaPointerAttributes attr;
+    void* dev = nullptr;
+    if (cudaPointerGetAttributes(&attr, host) == cudaSuccess && attr.type == cudaMemoryTypeHost && attr.devicePointer != nullptr)
+        dev = attr.devicePointer;
+    else
+        (void)cudaGetLastError();   // an unregistered host pointer is not an error here
+    cache[next] = Entry{host, dev};
+    next = (next + 1) % 8;
+    return reinterpret_cast<uintptr_t>(dev) % align == 0 ? dev : nullptr;
+}
+
+// PKV_SPLIT_AUTO: the cost model's choice for these lengths.  The last choice is kept per thread and
+// reused while the batch looks the same at a 128-token grain (a decode step adds one token per row:
+// the estimate moves by parts in ten thousand, the argmin almost never).
+pkv_status auto_policy(const pkv_shape& s, const pkv_split_policy& base, const int32_t* lens, int sms, pkv_split_policy* out) {
+    struct Memo {
+        std::vector<int32_t> coarse;
+        pkv_split_policy base, chosen;
+        int32_t Hq = 0, Hkv = 0, sms = 0;
+        bool valid = false;
+    };
+    thread_local Memo memo;
+    bool same = memo.valid && memo.Hq == s.Hq && memo.Hkv == s.Hkv && memo.sms == sms && (int32_t)memo.coarse.size() == s.B &&
+                std::memcmp(&memo.base, &base, sizeof(base)) == 0;
+    for (int32_t i = 0; same && i < s.B; ++i) same = memo.coarse[i] == (lens[i] > 0 ? (lens[i] >> 7) + 1 : 0);
+    if (same) { *out = memo.chosen; return PKV_OK; }
+    pkv_cost_model cm;
+    pkv_default_cost_model(sms, &cm);
+    const pkv_status st = pkv_choose_policy(&s, lens, &cm, &base, out, nullptr);
+    if (st != PKV_OK) return st;
+    memo.coarse.resize((size_t)s.B);
+    for (int32_t i = 0; i < s.B; ++i) memo.coarse[i] = lens[i] > 0 ? (lens[i] >> 7) + 1 : 0;
+    memo.base = base; memo.chosen = *out; memo.Hq = s.Hq; memo.Hkv = s.Hkv; memo.sms = sms; memo.valid = true;
+    return PKV_OK;
 }
 
 }  // namespace
@@ -565,7 +618,7 @@ extern "C" {
 size_t pkv_host_scratch_bytes(const pkv_shape* shape, const pkv_split_policy* policy) {
     Resolved rp;
     if (validate_and_resolve(shape, policy, 0, /*bound_ok=*/true, &rp) != PKV_OK) return 0;
-    return host_image(*shape, rp.S).total;
+    return host_image(*shape).total;
 }
 
 pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* policy, const void* q_host,
@@ -583,9 +636,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     if (rp.auto_mode && seq_lens_host) {
         // PKV_SPLIT_AUTO: the cost model picks this step's policy from the host-resident lengths
         // ("for each decode step, the harness estimates T_r")
-        pkv_cost_model cm;
-        pkv_default_cost_model(sms, &cm);
-        st = pkv_choose_policy(shape, seq_lens_host, &cm, policy, &auto_pol, nullptr);
+        st = auto_policy(*shape, *policy, seq_lens_host, sms, &auto_pol);
         if (st == PKV_OK) st = validate_and_resolve(shape, &auto_pol, sms, false, &rp);
         if (st != PKV_OK) return st;
     }
@@ -598,7 +649,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         set_error("host_staging / dev_scratch null or dev_scratch not 256-byte aligned");
         return PKV_ERR_INVALID_ARG;
     }
-    const HostImage im = host_image(s, rp.S);
+    const HostImage im = host_image(s);
     if (scratch_bytes < im.total) { set_error("scratch has %zu bytes, %zu needed", scratch_bytes, im.total); return PKV_ERR_WORKSPACE; }
     const WorkspaceLayout L = workspace_layout(s, rp.S);
     st = check_workspace(workspace, workspace_bytes, L);
@@ -623,51 +674,75 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         }
     }
 
-    // host planning ("Python planning" is part of the serving-facing time)
+    // Host planning (planning is part of the serving-facing time): only the COUNTS of
+    // the queue -- tasks, max_i n_i, (row, split) pairs -- which decide the launches (A13)
+    // and the kernel's grid; the queue itself is derived inside the decode kernel from the uploaded
+    // lengths (fused build), bit-identical to the host planner's.
     unsigned char* hs = static_cast<unsigned char*>(host_staging);
     unsigned char* ds = static_cast<unsigned char*>(dev_scratch);
-    QueueHeader* hdr = reinterpret_cast<QueueHeader*>(hs + im.hdr);
-    st = plan_host(s, rp, seq_lens_host, reinterpret_cast<pkv_task*>(hs + im.tasks),
-                   (int32_t)((im.tasks_end - im.tasks) / sizeof(pkv_task)),
-                   reinterpret_cast<int32_t*>(hs + im.split_offsets), reinterpret_cast<RowSlot*>(hs + im.rowslots), hdr);
-    if (st != PKV_OK) { set_error("host plan overflow"); return st; }
+    QueueHeader hdr_v;
+    QueueHeader* hdr = &hdr_v;
+    plan_host(s, rp, seq_lens_host, nullptr, 0, nullptr, nullptr, hdr);
+    // seq_lens and q: through the staging image, one cudaMemcpyAsync.  (Letting the kernels read a
+    // pinned q in place was measured and dropped: every split CTA re-reads its q slice in 4-byte
+    // pieces over the host link -- config 2: 74.6 us per step against 43.4 staged.)
+    const size_t q_bytes = 2 * (size_t)s.B * s.Hq * s.d;
     std::memcpy(hs + im.seq_lens, seq_lens_host, 4 * (size_t)s.B);
-    std::memcpy(hs + im.q, q_host, 2 * (size_t)s.B * s.Hq * s.d);
-    std::memcpy(hs + im.block_table, block_table_host, 4 * (size_t)s.B * s.max_pages);
-    const size_t h2d = im.tasks + sizeof(pkv_task) * (size_t)hdr->num_tasks;
-    cudaError_t e = cudaMemcpyAsync(ds, hs, h2d, cudaMemcpyHostToDevice, cs);
-    if (e != cudaSuccess) return cuda_fail(e, "H2D step image");
+    std::memcpy(hs + im.q, q_host, q_bytes);
+    size_t h2d = (im.q - im.seq_lens) + q_bytes;
+    cudaError_t e = cudaMemcpyAsync(ds + im.seq_lens, hs + im.seq_lens, h2d, cudaMemcpyHostToDevice, cs);
+    if (e != cudaSuccess) return cuda_fail(e, "H2D lengths and q");
+    const void* q_dev = ds + im.q;
+    const int32_t* lens_dev = reinterpret_cast<const int32_t*>(ds + im.seq_lens);
+    // block table: rows whose used entries differ from the shadow (everything on first use)
+    {
+        StageHeader* sh = reinterpret_cast<StageHeader*>(hs + im.hdr);
+        const bool fresh = sh->magic != kStageMagic || sh->B != s.B || sh->max_pages != s.max_pages || sh->dev != dev_scratch;
+        int32_t* shadow = reinterpret_cast<int32_t*>(hs + im.block_table);
+        int32_t run_lo = -1;       // pending run of changed rows [run_lo, i)
+        auto flush = [&](int32_t hi) -> cudaError_t {
+            if (run_lo < 0) return cudaSuccess;
+            const size_t off = im.block_table + 4 * (size_t)run_lo * s.max_pages, n = 4 * (size_t)(hi - run_lo) * s.max_pages;
+            run_lo = -1;
+            h2d += n;
+            return cudaMemcpyAsync(ds + off, hs + off, n, cudaMemcpyHostToDevice, cs);
+        };
+        for (int32_t i = 0; i < s.B; ++i) {
+            const int64_t N = seq_lens_host[i];
+            const size_t used = N > 0 ? (size_t)((N + s.page_size - 1) / s.page_size) : 0;
+            const int32_t* src = block_table_host + (size_t)i * s.max_pages;
+            int32_t* dst = shadow + (size_t)i * s.max_pages;
+            const bool changed = used > 0 && (fresh || std::memcmp(src, dst, 4 * used) != 0);
+            if (changed) {
+                std::memcpy(dst, src, 4 * used);
+                if (run_lo < 0) run_lo = i;
+            } else if (run_lo >= 0) {
+                e = flush(i);
+                if (e != cudaSuccess) return cuda_fail(e, "H2D block table rows");
+            }
+        }
+        e = flush(s.B);
+        if (e != cudaSuccess) return cuda_fail(e, "H2D block table rows");
+        sh->magic = kStageMagic; sh->B = s.B; sh->max_pages = s.max_pages; sh->table_src = block_table_host; sh->dev = dev_scratch;
+    }
 
     WsPtrs ws = carve(workspace, L);
-    if (rp.merge_mode == PKV_MERGE_FUSED && hdr->max_row_splits > 1) {
-        e = cudaMemsetAsync(ws.fuse_counters, 0, 4 * (size_t)s.B * s.Hkv, cs);
-        if (e != cudaSuccess) return cuda_fail(e, "memset fuse counters");
-    }
-    QueuePtrs qp;
-    qp.hdr = reinterpret_cast<QueueHeader*>(ds + im.hdr);
-    qp.split_offsets = reinterpret_cast<int32_t*>(ds + im.split_offsets);
-    qp.rowslots = reinterpret_cast<RowSlot*>(ds + im.rowslots);
-    qp.tasks = reinterpret_cast<pkv_task*>(ds + im.tasks);
     int dl = 0, ml = 0;
     // Pinned (page-locked, device-mapped) out_host: the kernels write the FP16 result straight
     // into it -- 8 KiB of posted writes per row -- and the D2H copy disappears from the step.
     // Pageable out_host: result in dev_scratch, then one cudaMemcpyAsync.
-    void* out_dev = ds + im.out;
-    bool zero_copy_out = false;
-    {
-        cudaPointerAttributes attr;
-        if (cudaPointerGetAttributes(&attr, out_host) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
-            attr.devicePointer != nullptr && reinterpret_cast<uintptr_t>(attr.devicePointer) % 16 == 0) {
-            out_dev = attr.devicePointer;
-            zero_copy_out = true;
-        } else {
-            (void)cudaGetLastError();   // an unregistered host pointer is not an error here
-        }
+    void* out_dev = mapped_device_pointer(out_host, 16);
+    const bool zero_copy_out = out_dev != nullptr;
+    if (!zero_copy_out) out_dev = ds + im.out;
+    const bool fused = rp.kernel == PKV_KERNEL_TMA_MMA && !(rp.flags & PKV_FLAG_SEPARATE_BUILD) && s.B <= kMaxFusedRows;
+    if (!fused && hdr->num_tasks > 0) {
+        e = launch_builder(s, rp, lens_dev, nullptr, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters, ws.q.rowslots, ws.q.tasks,
+                           L.slots_cap, cs);
+        if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     }
-    st = run_decode(s, rp, ds + im.q, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
-                    reinterpret_cast<const int32_t*>(ds + im.seq_lens), nullptr, out_dev, nullptr, scale, qp, ws,
-                    hdr->num_tasks, hdr->max_row_splits, hdr->total_row_slots, sms, PKV_STAGE_ALL, false, L.slots_cap, cs, &dl,
-                    &ml);
+    st = run_decode(s, rp, q_dev, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
+                    lens_dev, nullptr, out_dev, nullptr, scale, ws.q, ws, hdr->num_tasks, hdr->max_row_splits,
+                    hdr->total_row_slots, sms, PKV_STAGE_ALL, fused, L.slots_cap, cs, &dl, &ml);
     if (st != PKV_OK) return st;
     const size_t out_bytes = 2 * (size_t)s.B * s.Hq * s.d;
     e = zero_copy_out ? cudaSuccess : cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);
@@ -679,7 +754,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         counters_out->empty_tasks = hdr->empty_tasks;
         counters_out->decode_launches = dl;
         counters_out->merge_launches = ml;
-        counters_out->build_launches = 0;
+        counters_out->build_launches = (!fused && hdr->num_tasks > 0) ? 1 : 0;
         counters_out->useful_kv_bytes = hdr->sum_seq_lens * 2 * s.Hkv * s.d * 2;
         counters_out->merge_bytes = (int64_t)hdr->num_tasks * rp.G * (s.d + 2) * 4;
         counters_out->num_splits = hdr->resolved_splits;

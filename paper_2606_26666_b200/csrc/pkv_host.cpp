@@ -163,7 +163,12 @@ pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_
             const int32_t tok = (int32_t)(t1 < N ? t1 : N);
             if (tok > max_tok) max_tok = tok;
         }
-        for (int32_t g = 0; g < s.Hkv; ++g) {
+        if (!tasks) {   // counts only: no need to walk the row's tasks
+            count += (int64_t)s.Hkv * slots;
+            empties += (slots - r.n) * s.Hkv;
+            if (tasks_cap == 0 && (int64_t)s.Hkv * slots > 0) overflow = true;
+        }
+        for (int32_t g = 0; tasks && g < s.Hkv; ++g) {
             for (int32_t sp = 0; sp < slots; ++sp) {
                 int32_t tb = 0, te = 0;
                 if (r.T > 0) {

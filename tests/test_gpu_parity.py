@@ -293,7 +293,7 @@ def test_decode_host_entry_point():
     for pol in (pkv.Policy(num_splits=6), pkv.Policy(num_splits=1), pkv.Policy(num_splits=6, merge_mode=pkv.MERGE_FUSED),
                 pkv.Policy(num_splits=6, route=pkv.ROUTE_RECT, kernel=pkv.KERNEL_SIMT)):
         nb = pkv.pkv_host_scratch_bytes(dp.shape, pol)
-        staging = torch.empty(nb, dtype=torch.uint8).pin_memory()
+        staging = torch.zeros(nb, dtype=torch.uint8).pin_memory()
         scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
         ws = pkv.alloc_workspace(dp.shape, pol)
         out = np.full((p.B, p.Hq, p.d), np.nan, dtype=np.float16)
@@ -316,9 +316,70 @@ def test_decode_host_entry_point():
     nb = pkv.pkv_host_scratch_bytes(dp0.shape, pol)
     out = np.full((2, 32, 128), np.nan, dtype=np.float16)
     c = pkv.pkv_decode_host(dp0.shape, pol, p0.q, dp0.k, dp0.v, p0.block_table, p0.seq_lens, out, p0.scale,
-                            torch.empty(nb, dtype=torch.uint8).pin_memory(),
+                            torch.zeros(nb, dtype=torch.uint8).pin_memory(),
                             torch.empty(nb, dtype=torch.uint8, device="cuda"), pkv.alloc_workspace(dp0.shape, pol))
     assert np.all(out == 0) and c["decode_launches"] == 0 and c["merge_launches"] == 0
+
+
+@pytest.mark.parametrize("mode", [pkv.SPLIT_FIXED_COUNT, pkv.SPLIT_AUTO])
+def test_decode_host_serving_loop_uploads_only_what_changed(mode):
+    """A serving loop through pkv_decode_host on one (staging, scratch) pair: lengths grow across
+    page boundaries, one request is replaced by another (its whole table row changes), one finishes
+    (N = 0).  Every step matches the oracle and leaves the oracle's queue in the workspace; of the
+    block table only changed rows are uploaded (h2d_bytes); PKV_SPLIT_AUTO re-plans per step."""
+    lens = np.array([1500, 62, 4000, 333], dtype=np.int32)
+    p = make_problem(list(lens + 40), seed=93)
+    p2 = make_problem(list(lens + 40), seed=94)              # other page assignment, same pool size
+    assert p2.k_cache.shape == p.k_cache.shape
+    dp = DevProblem(p)
+    pol = pkv.Policy(tile_tokens=32, split_mode=mode, num_splits=5 if mode == pkv.SPLIT_FIXED_COUNT else 0)
+    nb = pkv.pkv_host_scratch_bytes(dp.shape, pol)
+    staging = torch.zeros(nb, dtype=torch.uint8).pin_memory()
+    scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    ws = pkv.alloc_workspace(dp.shape, pol)
+    out = torch.full((p.B, p.Hq, p.d), float("nan"), dtype=torch.float16).pin_memory()
+    table = p.block_table.copy()
+    row_bytes = 4 * table.shape[1]
+    base = p.q.nbytes + 256                                  # seq_lens (padded to 256) + q in one copy
+    shadow, seen = np.zeros_like(table), []
+    for t in range(8):
+        cur = (lens + t).astype(np.int32)
+        if t >= 3:
+            table[1] = p2.block_table[1] % p.k_cache.shape[0]          # row 1 now holds another request
+        if t >= 5:
+            cur[3] = 0
+        p.seq_lens, p.block_table = cur, table
+        c = pkv.pkv_decode_host(dp.shape, pol, p.q, dp.k, dp.v, table, cur, out.data_ptr(), p.scale, staging, scratch, ws)
+        ref, _ = oracle_attention(p)
+        assert_within_tolerance(out.numpy().astype(np.float64), ref, "step %d" % t)
+        # rows whose used entries differ from what the device holds (all of them at step 0)
+        nchanged = 0
+        for i in range(p.B):
+            used = -(-int(cur[i]) // 16)
+            if used and (t == 0 or not np.array_equal(table[i, :used], shadow[i, :used])):
+                shadow[i, :used] = table[i, :used]
+                nchanged += 1
+        assert c["h2d_bytes"] == base + nchanged * row_bytes, (t, nchanged)
+        seen.append(nchanged)
+        assert c["h2d_bytes"] <= base + 4 * row_bytes and c["d2h_bytes"] == out.numel() * 2
+        if mode == pkv.SPLIT_FIXED_COUNT:
+            q = wq.build_workqueue(list(cur), 8, oracle_policy(pol))
+            assert c["tasks"] == q.num_tasks and c["decode_launches"] == q.decode_launches and c["merge_launches"] == q.merge_launches
+            tasks, offs = pkv.pkv_read_workqueue(dp.shape, pol, ws)
+            assert tasks.tolist() == [list(x) for x in q.tasks] and offs.tolist() == q.split_offsets
+    assert seen[0] == 4 and 0 in seen and max(seen[1:]) <= 2
+    # steady state: nothing but lengths and q goes up
+    c = pkv.pkv_decode_host(dp.shape, pol, p.q, dp.k, dp.v, table, cur, out.data_ptr(), p.scale, staging, scratch, ws)
+    assert c["h2d_bytes"] == base
+    # the prepared call (pkv.HostDecoder): same result bit for bit, same bytes
+    want = out.numpy().copy()
+    qpin, lpin = torch.from_numpy(p.q.copy()).pin_memory(), torch.from_numpy(cur.copy()).pin_memory()
+    out.fill_(float("nan"))
+    dec = pkv.HostDecoder(dp.shape, pol, dp.k, dp.v, staging, scratch, ws, p.scale)
+    for _ in range(2):
+        dec(qpin.data_ptr(), table.ctypes.data, lpin.data_ptr(), out.data_ptr())
+    assert np.array_equal(out.numpy(), want)
+    assert dec.counters["h2d_bytes"] == base
 
 
 @pytest.mark.parametrize("mm", [pkv.MERGE_SEPARATE, pkv.MERGE_FUSED])
