@@ -71,14 +71,15 @@ Strides effective_strides(const pkv_shape& s) {
     return {s.kv_stride_page, s.kv_stride_token, s.kv_stride_head};
 }
 
-// Rank-5 tensor map over one cache: dims (64 ch, 16 tok, 2 ch-halves, Hkv heads, pages), strides
-// from the caller's layout, box (64, 16, 2, HG, 1): the HG-head slice of one page, landing in
+// Rank-5 tensor map over one cache: dims (64 ch, P tok, 2 ch-halves, Hkv heads, pages), strides
+// from the caller's layout, box (64, 16, 2, HG, 1): the HG-head slice of one 16-token block of a
+// page (the whole page when P = 16), landing in
 // shared memory as [head][ch-half][tok][64 ch] with the 128-byte swizzle (conflict-free ldmatrix).
 bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int HG, CUtensorMap* out) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t pages = (cuuint64_t)(s.num_pages > 0 ? s.num_pages : 1);
-    cuuint64_t dims[5] = {64, 16, 2, (cuuint64_t)s.Hkv, pages};
+    cuuint64_t dims[5] = {64, (cuuint64_t)s.page_size, 2, (cuuint64_t)s.Hkv, pages};
     cuuint64_t strides[4] = {(cuuint64_t)st.token * 2, 128, (cuuint64_t)st.head * 2, (cuuint64_t)st.page * 2};
     cuuint32_t box[5] = {64, 16, 2, (cuuint32_t)HG, 1};
     cuuint32_t estr[5] = {1, 1, 1, 1, 1};
@@ -91,7 +92,7 @@ bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int HG,
 struct MapCacheEntry {
     const void* base;
     int64_t num_pages, sp, st, sh;
-    int32_t Hkv, HG;
+    int32_t Hkv, HG, P;
     CUtensorMap map;
 };
 
@@ -104,11 +105,11 @@ const CUtensorMap* get_map(const void* base, const pkv_shape& s, int HG) {
     for (int i = 0; i < count; ++i) {
         const MapCacheEntry& e = cache[i];
         if (e.base == base && e.num_pages == s.num_pages && e.sp == st.page && e.st == st.token && e.sh == st.head &&
-            e.Hkv == s.Hkv && e.HG == HG)
+            e.Hkv == s.Hkv && e.HG == HG && e.P == s.page_size)
             return &e.map;
     }
     MapCacheEntry e;
-    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv; e.HG = HG;
+    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv; e.HG = HG; e.P = s.page_size;
     if (!encode_map(base, s, st, HG, &e.map)) return nullptr;
     const int slot = count < kCap ? count++ : (next = (next + 1) % kCap);
     cache[slot] = e;
@@ -188,6 +189,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.tasks_cap = tasks_cap;
     p.fused_build = fused_build ? 1 : 0;
     p.num_pages = s.num_pages;
+    p.page_shift = s.page_size == 64 ? 2 : (s.page_size == 32 ? 1 : 0);
 #ifdef PKV_TRACE
     p.trace = g_trace;
 #endif

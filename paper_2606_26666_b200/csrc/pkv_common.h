@@ -10,7 +10,7 @@
 namespace pkv {
 
 constexpr int kD = 128;         // head dimension compiled in
-constexpr int kPage = 16;       // page size compiled in
+constexpr int kBlock = 16;      // tokens per K/V stage (one TMA box); pages hold 1, 2 or 4 blocks
 constexpr int kAutoCMin = 4;    // PAPER.md:85 "C_min = 4 CTAs/SM" (auto split rule, A12)
 constexpr int kMaxSplits = 256; // cap on S (and on n_i in FIXED_CHUNK mode)
 constexpr int kAllFlags = PKV_FLAG_VALIDATE | PKV_FLAG_NO_PDL | PKV_FLAG_SEPARATE_BUILD | PKV_FLAG_TEST_REPLAN;

@@ -90,8 +90,8 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
             for (int u = 0; u < kUnroll; ++u) {
                 const int j = base + hw + 8 * u;
                 if (j < tok1) {
-                    const int64_t page = checked_page(bt[j >> 4], p.plan.flags, p.num_pages, &p.hdr->error_word);
-                    const int64_t off = page * p.stride_page + (int64_t)(j & 15) * p.stride_token + head_off;
+                    const int64_t page = checked_page(bt[j >> (4 + p.page_shift)], p.plan.flags, p.num_pages, &p.hdr->error_word);
+                    const int64_t off = page * p.stride_page + (int64_t)(j & ((16 << p.page_shift) - 1)) * p.stride_token + head_off;
                     ku[u] = ldg_nc_16(p.k_cache + off);
                     vu[u] = ldg_nc_16(p.v_cache + off);
                 } else {

@@ -127,6 +127,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     const int HGn = p.Hkv / HG;                               // head groups per (row, split)
     int num_units = 0;
     int early_row = -1, early_tok0 = 0, early_tok1 = 0, early_mine = 0;   // producer 0: first unit's table entries
+    const int pgs = p.page_shift, pmask = (1 << pgs) - 1;   // page = 1 << ps blocks of 16 tokens
     PlanArgs plan = p.plan;   // BALANCED: the planner resolves the batch-wide chunk
     // Speculative plan.  A decode CTA is usually resident a few microseconds before its dependency
     // wait returns (programmatic launch), and the plan -- ~1 us with a fixed split count, ~2.5 us
@@ -154,17 +155,18 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     // the wait; a stale guess only costs bandwidth.
     if (p.fused_build && warp == 0 && p.prefetch_pages > 0 && (int)blockIdx.x < spec_row_slots * HGn) {
         const RowSlot d = tail.first_slot;
-        const int p0 = d.tok0 >> 4;
+        const int p0 = d.tok0 >> 4;   // in blocks of 16 tokens (a page holds 1 << page_shift of them)
         int np = d.tok0 < d.tok1 ? ((d.tok1 + 15) >> 4) - p0 : 0;
-        np = min(min(np, p.prefetch_pages), p.max_pages - p0);
+        np = min(min(np, p.prefetch_pages), (p.max_pages << pgs) - p0);
         if (d.row >= 0 && d.row < p.B && d.grow >= 0 && p0 >= 0) {
-            const int32_t* bt = p.block_table + (int64_t)d.grow * p.max_pages + p0;
+            const int32_t* bt = p.block_table + (int64_t)d.grow * p.max_pages;
             const int head0 = ((int)blockIdx.x % HGn) * HG;
             for (int j = lane; j < np; j += 32) {
-                const int page = ld_relaxed_s32(bt + j);
+                const int page = ld_relaxed_s32(bt + ((p0 + j) >> pgs));
+                const int tok = ((p0 + j) & pmask) << 4;
                 if (page >= 0 && (int64_t)page < p.num_pages) {
-                    tma_prefetch_5d(&tmap_k, 0, 0, 0, head0, page);
-                    tma_prefetch_5d(&tmap_v, 0, 0, 0, head0, page);
+                    tma_prefetch_5d(&tmap_k, 0, tok, 0, head0, page);
+                    tma_prefetch_5d(&tmap_v, 0, tok, 0, head0, page);
                 }
             }
             // q rows of the unit's HG*G query heads: HG*G*256 bytes, one 128-byte line per lane
@@ -235,10 +237,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         if (!p.force_replan && (int)blockIdx.x < spec_row_slots * HGn) {
             const RowSlot d = tail.first_slot;
             const int p0 = d.tok0 >> 4;
-            const int np = d.tok0 < d.tok1 ? min(((d.tok1 + 15) >> 4) - p0, p.max_pages - p0) : 0;
+            const int np = d.tok0 < d.tok1 ? min(((d.tok1 + 15) >> 4) - p0, (p.max_pages << pgs) - p0) : 0;
             if (d.row >= 0 && d.row < p.B && d.grow >= 0 && p0 >= 0) {
                 early_row = d.grow; early_tok0 = d.tok0; early_tok1 = d.tok1;
-                if (lane < np) early_mine = __ldcg(p.block_table + (int64_t)d.grow * p.max_pages + p0 + lane);
+                if (lane < np) early_mine = __ldcg(p.block_table + (int64_t)d.grow * p.max_pages + ((p0 + lane) >> pgs));
             }
         }
         if (!p.force_replan && plan_lens_unchanged(plan, p.seq_lens, tail.len_s, lane, err)) {
@@ -330,16 +332,17 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             const int p0 = tok0 >> 4;
             const int np = ((tok1 + 15) >> 4) - p0;
             const int head0 = hg * HG;
-            const int32_t* bt = p.block_table + (int64_t)row * p.max_pages + p0;
-            // table entries 32 at a time (lane i holds page c + i of the unit)
+            const int32_t* bt = p.block_table + (int64_t)row * p.max_pages;
+            // table entries 32 blocks at a time (lane i holds the page of block c + i of the unit)
             const bool early = k == 0 && warp == 0 && row == early_row && tok0 == early_tok0 && tok1 == early_tok1;
-            int mine = lane < np ? checked_page(early ? early_mine : bt[lane], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
+            int mine = lane < np ? checked_page(early ? early_mine : bt[(p0 + lane) >> pgs], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
             for (int c = 0; c < np; c += 32) {
                 const int nxt = (c + 32 + lane < np)
-                                    ? checked_page(bt[c + 32 + lane], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
+                                    ? checked_page(bt[(p0 + c + 32 + lane) >> pgs], p.plan.flags, p.num_pages, &p.hdr->error_word) : 0;
                 const int cnt = min(32, np - c);
                 for (int i = 0; i < cnt; ++i) {
                     const int page = __shfl_sync(0xffffffffu, mine, i);
+                    const int tok = ((p0 + c + i) & pmask) << 4;   // the block's first token inside its page
                     const uint32_t s = ps, par = pphase;
                     if (++ps == (uint32_t)kStages) { ps = 0; pphase ^= 1; }
                     if ((s % NP) != (uint32_t)warp) continue;
@@ -349,9 +352,9 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                         const uint32_t dst = stage_base + s * kStageBytes;
                         // box dims: (64 ch, 16 tok, 2 ch-halves, HG heads, 1 page)
                         mbar_arrive_expect_tx(fullk0 + 8 * s, HG * 4096);
-                        tma_load_5d(dst, &tmap_k, fullk0 + 8 * s, 0, 0, 0, head0, page, kv_policy);
+                        tma_load_5d(dst, &tmap_k, fullk0 + 8 * s, 0, tok, 0, head0, page, kv_policy);
                         mbar_arrive_expect_tx(fullv0 + 8 * s, HG * 4096);
-                        tma_load_5d(dst + HG * 4096, &tmap_v, fullv0 + 8 * s, 0, 0, 0, head0, page, kv_policy);
+                        tma_load_5d(dst + HG * 4096, &tmap_v, fullv0 + 8 * s, 0, tok, 0, head0, page, kv_policy);
                     }
                 }
                 mine = nxt;

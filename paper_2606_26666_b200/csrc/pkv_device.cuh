@@ -52,7 +52,8 @@ struct DecodeParams {
     int32_t heads_per_cta;       // TMA kernel: KV heads one CTA streams together (1, 2, 4 or 8)
     int32_t dynamic_sched;      // 1: tasks handed out by an atomic counter
     int32_t force_replan;       // test hook: treat the speculative plan as invalidated
-    int32_t prefetch_pages;     // TMA kernel: pages of its first unit a CTA prefetches into L2 before the wait
+    int32_t prefetch_pages;     // TMA kernel: 16-token blocks of its first unit a CTA prefetches into L2 before the wait
+    int32_t page_shift;         // log2(page_size / 16): a page holds 1, 2 or 4 blocks of 16 tokens
     float scale;                // x = scale * <q, k>
     float scale_log2;           // scale * log2(e)
     int64_t num_pages;          // PKV_FLAG_VALIDATE: block-table entries must lie in [0, num_pages)

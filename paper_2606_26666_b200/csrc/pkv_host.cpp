@@ -33,7 +33,7 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     }
     if (s.Hq % s.Hkv != 0) { set_error("Hq=%d is not a multiple of Hkv=%d", s.Hq, s.Hkv); return PKV_ERR_INVALID_ARG; }
     if (s.d != kD) { set_error("d=%d not compiled in (d=128 only)", s.d); return PKV_ERR_UNSUPPORTED; }
-    if (s.page_size != kPage) { set_error("page_size=%d not compiled in (16 only)", s.page_size); return PKV_ERR_UNSUPPORTED; }
+    if (s.page_size != 16 && s.page_size != 32 && s.page_size != 64) { set_error("page_size=%d not supported (16, 32 or 64)", s.page_size); return PKV_ERR_UNSUPPORTED; }
     const int G = s.Hq / s.Hkv;
     if (G != 1 && G != 2 && G != 4 && G != 8) { set_error("G=Hq/Hkv=%d not compiled in (1, 2, 4 and 8 only)", G); return PKV_ERR_UNSUPPORTED; }
     const bool default_strides = s.kv_stride_page == 0 && s.kv_stride_token == 0 && s.kv_stride_head == 0;

@@ -44,7 +44,7 @@ def shape(B, Hkv=8, Hq=32, max_pages=4096):
 
 @pytest.mark.parametrize("bad,status", [
     (dict(d=64), pkv.PKV_ERR_UNSUPPORTED),
-    (dict(page_size=32), pkv.PKV_ERR_UNSUPPORTED),
+    (dict(page_size=48), pkv.PKV_ERR_UNSUPPORTED),
     (dict(Hq=48, Hkv=16), pkv.PKV_ERR_UNSUPPORTED),        # G = 3 not compiled in
     (dict(Hq=30, Hkv=8), pkv.PKV_ERR_INVALID_ARG),
     (dict(kv_strides=(4096, 4, 128)), pkv.PKV_ERR_INVALID_ARG),   # token stride not 16-byte multiple
