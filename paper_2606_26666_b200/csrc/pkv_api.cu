@@ -223,7 +223,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             int64_t row_slots = known_slots >= 0 ? known_slots : (int64_t)s.B * rp.S;
             if (known_slots < 0 && rp.split_mode == PKV_SPLIT_BALANCED && rp.num_sms > 0 && rp.num_sms < row_slots)
                 row_slots = rp.num_sms;
-            const int HG = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, row_slots, num_sms);
+            const int HG = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, row_slots, num_sms, rp.G == 16 ? 4 : 8);
             p.prefetch_pages = rp.prefetch_kb * 1024 / (HG * 8192);
             // by value: inserting the V map may evict the cache entry the K pointer refers to
             const CUtensorMap* pk = get_map(k_cache, s, HG);
@@ -242,7 +242,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             // stream position, so a dynamic hand-out would make the FP32 combine order -- and the
             // last bits of the result -- depend on which units a CTA drew before.  Round-robin
             // keeps every launch bitwise reproducible.
-            p.dynamic_sched = HG == 8 ? 1 : 0;
+            p.dynamic_sched = HG * (rp.G == 16 ? 2 : 1) == 8 ? 1 : 0;
             const int64_t units = row_slots * (s.Hkv / HG);
             const int grid = (int)(units < num_sms ? units : num_sms);
             e = launch_decode_tma(p, rp.G, HG, grid, mk, mv, stream);

@@ -276,7 +276,7 @@ cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     PKV_MERGE_CASE(GG, 2, 1, 1) PKV_MERGE_CASE(GG, 4, 1, 6) PKV_MERGE_CASE(GG, 8, 1, 1) PKV_MERGE_CASE(GG, 16, 1, 1) \
     PKV_MERGE_CASE(GG, 2, 2, 1) PKV_MERGE_CASE(GG, 4, 2, 1) PKV_MERGE_CASE(GG, 8, 2, 1) PKV_MERGE_CASE(GG, 16, 2, 1) \
     PKV_MERGE_CASE(GG, 2, 4, 1) PKV_MERGE_CASE(GG, 4, 4, 1) PKV_MERGE_CASE(GG, 8, 4, 1) PKV_MERGE_CASE(GG, 16, 4, 1)
-    PKV_MERGE_G(4) PKV_MERGE_G(8) PKV_MERGE_G(2) PKV_MERGE_G(1)
+    PKV_MERGE_G(4) PKV_MERGE_G(8) PKV_MERGE_G(2) PKV_MERGE_G(1) PKV_MERGE_G(16)
 #undef PKV_MERGE_G
 #undef PKV_MERGE_CASE
     return cudaErrorInvalidValue;

@@ -174,6 +174,7 @@ cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStrea
     if (G == 1) return launch_pdl(pdl, pkv_decode_simt_kernel<1>, dim3(grid), dim3(kThreads), 0, stream, p);
     if (G == 2) return launch_pdl(pdl, pkv_decode_simt_kernel<2>, dim3(grid), dim3(kThreads), 0, stream, p);
     if (G == 4) return launch_pdl(pdl, pkv_decode_simt_kernel<4>, dim3(grid), dim3(kThreads), 0, stream, p);
+    if (G == 16) return launch_pdl(pdl, pkv_decode_simt_kernel<16>, dim3(grid), dim3(kThreads), 0, stream, p);
     return launch_pdl(pdl, pkv_decode_simt_kernel<8>, dim3(grid), dim3(kThreads), 0, stream, p);
 }
 

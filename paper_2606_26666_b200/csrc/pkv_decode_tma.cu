@@ -74,10 +74,14 @@ struct SmemTail {
     int32_t len_s[kMaxFusedRows];      //              max(N_i, 0)
 };
 
+// G = 16 is two blocks of 8 query heads (the MMA's N = 8 columns): NBK column blocks of GW heads,
+// each with warps of its own that share the streamed K/V stage.
+__host__ __device__ constexpr int blocks_for(int G) { return G > 8 ? G / 8 : 1; }
+
 template <int G, int HG>
 __host__ __device__ constexpr int stages_for() {
     // 227 KiB per CTA, minus the tail, minus 1 KiB alignment slack
-    constexpr int avail = 232448 - 1024 - (int)sizeof(SmemTail<G>);
+    constexpr int avail = 232448 - 1024 - (int)sizeof(SmemTail<G / blocks_for(G)>);
     constexpr int n = avail / (HG * 8192);
     // Stage s always belongs to producer s % NP and, per head, to compute warp s % WPH (see the
     // kernel): any stage count works, the shares differ by at most one stage.
@@ -91,13 +95,17 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     constexpr int kStages = stages_for<G, HG>();
     constexpr int kStageBytes = HG * 8192;   // K: HG x 4096 | V: HG x 4096
     constexpr int NP = producers_for(HG);
-    constexpr int WPH = kComputeWarps / HG;  // warps per head
+    constexpr int NBK = blocks_for(G);       // blocks of query heads per KV head (2 when G = 16)
+    constexpr int GW = G / NBK;              // query heads one warp tracks (the MMA's N columns)
+    constexpr int NGRP = HG * NBK;           // (head, block) groups per CTA
+    constexpr int WPH = kComputeWarps / NGRP;  // warps per group: they split the unit's pages
     constexpr int kPlanWarp = NP + kComputeWarps;   // the last warp plans and writes the queue
     static_assert(kStages >= 2, "ring too small");
+    static_assert(NGRP <= kComputeWarps, "G = 16 streams at most 4 KV heads per CTA");
     extern __shared__ unsigned char smem_raw[];
     // 128-byte swizzle: every 2 KiB half-box must start on a 1024-byte boundary
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    SmemTail<G>& tail = *reinterpret_cast<SmemTail<G>*>(smem + (size_t)kStages * kStageBytes);
+    SmemTail<GW>& tail = *reinterpret_cast<SmemTail<GW>*>(smem + (size_t)kStages * kStageBytes);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t stage_base = smem_u32(smem);
@@ -113,7 +121,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         for (int s = 0; s < kStages; ++s) {
             mbar_init(fullk0 + 8 * s, 1);
             mbar_init(fullv0 + 8 * s, 1);
-            mbar_init(empty0 + 8 * s, HG);    // one arrival per head of the page
+            mbar_init(empty0 + 8 * s, NGRP);  // one arrival per (head, block) group of the page
         }
         for (int r = 0; r < kRing; ++r) {
             mbar_init(rfull0 + 8 * r, 1);
@@ -372,8 +380,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     } else {
         // ================================================================ compute warps
         const int cw = warp - NP;            // 0..7
-        const int hl = cw % HG;              // head within the unit's head group
-        const int sub = cw / HG;             // which of the head's WPH warps
+        const int grp = cw % NGRP;           // (head, block) group
+        const int hl = grp % HG;             // head within the unit's head group
+        const int h0 = (grp / HG) * GW;      // first query head of the warp's block within the KV head
+        const int sub = cw / NGRP;           // which of the group's WPH warps
         const int gtid = sub * 32 + lane;    // thread index within the head's warp group
         const int g4 = lane >> 2;            // fragment "groupID"
         const int t4 = lane & 3;             // fragment "threadID_in_group"
@@ -395,7 +405,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             const int64_t slot = (int64_t)so * p.Hkv + (int64_t)kvh * n_i + split;
             const int tok0 = u.tok0, tok1 = u.tok1;
             if (tok0 >= tok1) {
-                store_empty_task<G, WPH>(p, &tail.cb.flag[hl], row, orow, kvh, split, n_i, slot, gtid, 1 + hl);
+                store_empty_task<G, WPH, GW>(p, &tail.cb.flag[grp], row, orow, kvh, split, n_i, slot, gtid, 1 + grp, h0);
                 continue;
             }
             const int p0 = tok0 >> 4;
@@ -404,13 +414,13 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             // Q^T as the MMA B operand: b0 = Q[head g4][kk*16 + 2*t4 .. +1], b1 = same + 8
             uint32_t qb[8][2];
             {
-                const __half* qrow = p.q + ((int64_t)orow * p.Hq + kvh * G + (g4 < G ? g4 : 0)) * kD;
+                const __half* qrow = p.q + ((int64_t)orow * p.Hq + kvh * G + h0 + (g4 < GW ? g4 : 0)) * kD;
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk) {
                     const uint32_t lo = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + 2 * t4);
                     const uint32_t hi = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + 8 + 2 * t4);
-                    qb[kk][0] = g4 < G ? lo : 0u;
-                    qb[kk][1] = g4 < G ? hi : 0u;
+                    qb[kk][0] = g4 < GW ? lo : 0u;
+                    qb[kk][1] = g4 < GW ? hi : 0u;
                 }
             }
             float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
@@ -528,9 +538,9 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 // The warp owns the whole task: its state goes from the MMA accumulators straight
                 // to the task's slot (or to `out`), no shared-memory round trip.  Per store
                 // instruction the 8 lanes of a column write 32 contiguous bytes.
-                if (hA < G) {
-                    const bool hasB = hB < G;   // G = 1: column B is padding
-                    const int64_t hrow = (int64_t)orow * p.Hq + kvh * G + hA;
+                if (hA < GW) {
+                    const bool hasB = hB < GW;   // G = 1: column B is padding
+                    const int64_t hrow = (int64_t)orow * p.Hq + kvh * G + h0 + hA;
                     if (n_i <= 1) {
                         const float iA = 1.0f / lA, iB = hasB ? 1.0f / lB : 0.f;
                         __half* oA = p.out + hrow * kD + g4;
@@ -549,7 +559,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                             if (hasB) p.lse[hrow + 1] = mB * p.scale + logf(lB);
                         }
                     } else {
-                        float* aA = p.part_acc + (slot * G + hA) * kD + g4;
+                        float* aA = p.part_acc + (slot * G + h0 + hA) * kD + g4;
                         float* aB = aA + kD;
 #pragma unroll
                         for (int mt = 0; mt < 8; ++mt) {
@@ -561,20 +571,20 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                             }
                         }
                         if (g4 == 0) {
-                            p.part_m[slot * G + hA] = mA * p.scale;
-                            p.part_l[slot * G + hA] = lA;
+                            p.part_m[slot * G + h0 + hA] = mA * p.scale;
+                            p.part_l[slot * G + h0 + hA] = lA;
                             if (hasB) {
-                                p.part_m[slot * G + hB] = mB * p.scale;
-                                p.part_l[slot * G + hB] = lB;
+                                p.part_m[slot * G + h0 + hB] = mB * p.scale;
+                                p.part_l[slot * G + h0 + hB] = lB;
                             }
                         }
                     }
                 }
                 if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED)
-                    fused_complete<G, 1>(p, &tail.cb.flag[cw], row, orow, kvh, split, n_i, slot, lane, 1 + hl);
+                    fused_complete<G, 1>(p, &tail.cb.flag[cw], row, orow, kvh, split, n_i, slot, lane, 1 + grp, NBK);
             } else {
-                if (hA < G) {
-                    const bool hasB = hB < G;   // G = 1: column B is padding
+                if (hA < GW) {
+                    const bool hasB = hB < GW;   // G = 1: column B is padding
 #pragma unroll
                     for (int mt = 0; mt < 8; ++mt) {
                         tail.cb.acc[cw][hA][mt * 16 + g4] = o[mt][0];
@@ -589,8 +599,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                         if (hasB) { tail.cb.m[cw][hB] = mB; tail.cb.l[cw][hB] = lB; }
                     }
                 }
-                group_sync<WPH>(1 + hl);
-                finalize_task<G, WPH, kComputeWarps>(p, tail.cb, hl, HG, row, orow, kvh, split, n_i, slot, gtid, 1 + hl);
+                group_sync<WPH>(1 + grp);
+                finalize_task<G, WPH, kComputeWarps, GW>(p, tail.cb, grp, NGRP, row, orow, kvh, split, n_i, slot, gtid, 1 + grp, h0);
             }
             if (k == 0 && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 6);
         }
@@ -600,7 +610,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
 template <int G, int HG>
 cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, const CUtensorMap& mv,
                        cudaStream_t stream) {
-    constexpr int smem = stages_for<G, HG>() * HG * 8192 + (int)sizeof(SmemTail<G>) + 1024;
+    constexpr int smem = stages_for<G, HG>() * HG * 8192 + (int)sizeof(SmemTail<G / blocks_for(G)>) + 1024;
     constexpr int threads = (producers_for(HG) + kComputeWarps + 1) * 32;
     // The dynamic shared-memory opt-in is a per-device (per-context) attribute of the kernel: one
     // flag per device ordinal, set on the first launch there (races only repeat the call).
@@ -620,7 +630,7 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
 
 int decode_tma_smem_bytes(int G, int HG) {
     const int tail = G == 1 ? (int)sizeof(SmemTail<1>) : G == 2 ? (int)sizeof(SmemTail<2>)
-                   : G == 4 ? (int)sizeof(SmemTail<4>) : (int)sizeof(SmemTail<8>);
+                   : G == 4 ? (int)sizeof(SmemTail<4>) : (int)sizeof(SmemTail<8>);   // G = 16: two blocks of 8
     int st = (232448 - 1024 - tail) / (HG * 8192);
     if (st > kMaxStages) st = kMaxStages;
     return st * HG * 8192 + tail + 1024;
@@ -637,6 +647,7 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int grid, co
     PKV_CASE(8, 8) PKV_CASE(8, 4) PKV_CASE(8, 2) PKV_CASE(8, 1)
     PKV_CASE(2, 8) PKV_CASE(2, 4) PKV_CASE(2, 2) PKV_CASE(2, 1)
     PKV_CASE(1, 8) PKV_CASE(1, 4) PKV_CASE(1, 2) PKV_CASE(1, 1)
+    PKV_CASE(16, 4) PKV_CASE(16, 2) PKV_CASE(16, 1)
 #undef PKV_CASE
     return cudaErrorInvalidValue;
 }

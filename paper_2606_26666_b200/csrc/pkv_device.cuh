@@ -636,8 +636,8 @@ constexpr int kAccStride = 132;  // floats per (warp, head) row of acc; 132 % 32
 template <int G, int NWTOT>
 struct CombineBuf {
     float acc[NWTOT][G][kAccStride];
-    float m[NWTOT][8];
-    float l[NWTOT][8];
+    float m[NWTOT][G < 8 ? 8 : G];
+    float l[NWTOT][G < 8 ? 8 : G];
     int flag[NWTOT];
 };
 
@@ -649,14 +649,16 @@ __device__ __forceinline__ void group_sync(int bar_id) {
 // FUSED merge tail: a group of NW warps has stored split `split` of (row, kvh); the
 // group that completes the last of the n_i splits (atomic completion counter, self-resetting for
 // graph replay) merges the row's slot range in place.  flag = a shared-memory word of the group.
+// `arrivals`: groups that complete one split of (row, kvh) between them (2 when G = 16: one group
+// per block of 8 query heads); the last of the n_i * arrivals merges all G heads.
 template <int G, int NW>
 __device__ __forceinline__ void fused_complete(const DecodeParams& p, int* flag, int row, int orow, int kvh, int split,
-                                               int n_i, int64_t slot, int gtid, int bar_id) {
+                                               int n_i, int64_t slot, int gtid, int bar_id, int arrivals = 1) {
     __threadfence();  // partial state visible device-wide before the completion count
     group_sync<NW>(bar_id);
     if (gtid == 0) {
         const int old = atomicAdd(&p.fuse_counters[row * p.Hkv + kvh], 1);
-        const int last = (old == n_i - 1);
+        const int last = (old == n_i * arrivals - 1);
         if (last) p.fuse_counters[row * p.Hkv + kvh] = 0;
         *flag = last;
     }
@@ -671,11 +673,12 @@ __device__ __forceinline__ void fused_complete(const DecodeParams& p, int* flag,
 
 // Writes an empty task's result (rect route): neutral partial state, or zeros when
 // the row has a single slot (direct output).  Called by the NW warps that own the task.
-template <int G, int NW>
+// The group owns query heads h0 .. h0+GW-1 of the KV head's G (GW = G, h0 = 0 unless G = 16).
+template <int G, int NW, int GW = G>
 __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* flag, int row, int orow, int kvh, int split,
-                                                 int n_i, int64_t slot, int gtid, int bar_id) {
-    for (int idx = gtid; idx < G * kD; idx += NW * 32) {
-        const int hh = idx / kD, dd = idx % kD;
+                                                 int n_i, int64_t slot, int gtid, int bar_id, int h0 = 0) {
+    for (int idx = gtid; idx < GW * kD; idx += NW * 32) {
+        const int hh = h0 + idx / kD, dd = idx % kD;
         if (n_i <= 1) {
             const int64_t o = (int64_t)orow * p.Hq + kvh * G + hh;
             p.out[o * kD + dd] = __float2half_rn(0.f);
@@ -688,7 +691,8 @@ __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* fla
             }
         }
     }
-    if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED) fused_complete<G, NW>(p, flag, row, orow, kvh, split, n_i, slot, gtid, bar_id);
+    if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED)
+        fused_complete<G, NW>(p, flag, row, orow, kvh, split, n_i, slot, gtid, bar_id, G / GW);
 }
 
 // A group of NW warps (rows w0, w0+wstride, ... of `cb`) has processed one task.  Combines the
@@ -697,12 +701,12 @@ __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* fla
 // the group that completes the last split of (row, kvh) merges in place.
 // gtid = 0..NW*32-1 within the group; the group synchronises with group_sync<NW>(bar_id); the
 // caller has synchronised after filling `cb`.
-template <int G, int NW, int NWTOT>
-__device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<G, NWTOT>& cb, int w0, int wstride,
+template <int G, int NW, int NWTOT, int GW = G>
+__device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<GW, NWTOT>& cb, int w0, int wstride,
                                               int row, int orow, int kvh, int split, int n_i, int64_t slot, int gtid,
-                                              int bar_id) {
-    for (int idx = gtid; idx < G * kD; idx += NW * 32) {
-        const int hh = idx / kD, dd = idx % kD;
+                                              int bar_id, int h0 = 0) {
+    for (int idx = gtid; idx < GW * kD; idx += NW * 32) {
+        const int hh = idx / kD, dd = idx % kD;   // head within the group's block; h0 + hh within the KV head
         float M = -INFINITY;
 #pragma unroll
         for (int i = 0; i < NW; ++i) M = fmaxf(M, cb.m[w0 + i * wstride][hh]);
@@ -715,19 +719,19 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
             A += wgt * cb.acc[w][hh][dd];
         }
         if (n_i <= 1) {
-            const int64_t o = (int64_t)orow * p.Hq + kvh * G + hh;
+            const int64_t o = (int64_t)orow * p.Hq + kvh * G + h0 + hh;
             p.out[o * kD + dd] = __float2half_rn(A / L);
             if (p.lse && dd == 0) p.lse[o] = M * p.scale + logf(L);
         } else {
-            p.part_acc[(slot * G + hh) * kD + dd] = A;
+            p.part_acc[(slot * G + h0 + hh) * kD + dd] = A;
             if (dd == 0) {
-                p.part_m[slot * G + hh] = M * p.scale;
-                p.part_l[slot * G + hh] = L;
+                p.part_m[slot * G + h0 + hh] = M * p.scale;
+                p.part_l[slot * G + h0 + hh] = L;
             }
         }
     }
     if (n_i > 1 && p.merge_mode == PKV_MERGE_FUSED)
-        fused_complete<G, NW>(p, &cb.flag[w0], row, orow, kvh, split, n_i, slot, gtid, bar_id);
+        fused_complete<G, NW>(p, &cb.flag[w0], row, orow, kvh, split, n_i, slot, gtid, bar_id, G / GW);
     group_sync<NW>(bar_id);  // cb rows may be refilled after this
 }
 

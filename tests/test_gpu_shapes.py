@@ -82,3 +82,46 @@ def test_page_sizes_token_counts_exact_and_dominant_key(kernel, P):
         out, _, _ = DevProblem(pj).decode(pkv.Policy(tile_tokens=P, num_splits=S, kernel=kernel))
         for g in range(8):
             assert np.abs(out[0, g * 4] - pj.v_cache[page, r, g].astype(np.float64)).max() <= 2e-3, (j, g)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("Hq,Hkv", [(32, 2), (64, 4), (128, 8)])
+def test_g16_ragged_sweep(kernel, Hq, Hkv):
+    """G = Hq / Hkv = 16 ("G=1 and G=8 ... until separate mappings are
+    implemented"): two blocks of 8 query heads per KV head share each streamed K/V stage.  Every
+    heads-per-CTA variant, both routes, separate and fused merge; queue bit-exact."""
+    p = make_problem(RAGGED, seed=700 + Hkv, Hq=Hq, Hkv=Hkv)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    hgs = [h for h in (0, 1, 2, 4) if h <= Hkv]
+    for hg in hgs:
+        for pol in (pkv.Policy(tile_tokens=32, num_splits=1, kernel=kernel, heads_per_cta=hg),
+                    pkv.Policy(tile_tokens=32, num_splits=5, kernel=kernel, heads_per_cta=hg),
+                    pkv.Policy(tile_tokens=16, num_splits=3, kernel=kernel, heads_per_cta=hg, merge_mode=pkv.MERGE_FUSED,
+                               route=pkv.ROUTE_RECT),
+                    pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=24, kernel=kernel,
+                               heads_per_cta=hg)):
+            _, _, ws = _check(dp, pol, ref, "G16 hg%d %s" % (hg, pol))
+            tasks, offs = pkv.pkv_read_workqueue(dp.shape, pol, ws)
+            want = wq.build_workqueue(RAGGED, Hkv, oracle_policy(pol))
+            assert tasks.tolist() == [list(t) for t in want.tasks] and offs.tolist() == want.split_offsets
+        if kernel == pkv.KERNEL_SIMT:
+            break       # heads_per_cta only concerns the TMA kernel
+
+
+def test_g16_many_units_and_partials():
+    """G = 16 with more units than SMs and long units (ring wraps, dynamic hand-out at HG = 4), and the
+    partial states of both head blocks against the oracle's split states through the merge."""
+    rng = np.random.Generator(np.random.PCG64(17))
+    lens = list(rng.integers(1, 3000, size=96))
+    p = make_problem(lens, seed=711, Hq=64, Hkv=4)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    for pol in (pkv.Policy(tile_tokens=32, num_splits=4), pkv.Policy(tile_tokens=32, num_splits=1),
+                pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_CHUNK, num_splits=0, chunk_tiles=8, merge_mode=pkv.MERGE_FUSED)):
+        for hg in (4, 2, 1):
+            pol.heads_per_cta = hg
+            for _ in range(2):
+                _check(dp, pol, ref, "hg%d %s" % (hg, pol))
+    with pytest.raises(pkv.PkvError):
+        dp.decode(pkv.Policy(tile_tokens=32, num_splits=1, heads_per_cta=8))
