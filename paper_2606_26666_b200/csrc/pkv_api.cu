@@ -79,9 +79,10 @@ bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int HG,
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t pages = (cuuint64_t)(s.num_pages > 0 ? s.num_pages : 1);
-    cuuint64_t dims[5] = {64, (cuuint64_t)s.page_size, 2, (cuuint64_t)s.Hkv, pages};
+    const cuuint32_t blocks = (cuuint32_t)(s.d / 64);   // 64-channel (128-byte) blocks of a head's row
+    cuuint64_t dims[5] = {64, (cuuint64_t)s.page_size, blocks, (cuuint64_t)s.Hkv, pages};
     cuuint64_t strides[4] = {(cuuint64_t)st.token * 2, 128, (cuuint64_t)st.head * 2, (cuuint64_t)st.page * 2};
-    cuuint32_t box[5] = {64, 16, 2, (cuuint32_t)HG, 1};
+    cuuint32_t box[5] = {64, 16, blocks, (cuuint32_t)HG, 1};
     cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     const CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 5, const_cast<void*>(base), dims, strides, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -92,7 +93,7 @@ bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int HG,
 struct MapCacheEntry {
     const void* base;
     int64_t num_pages, sp, st, sh;
-    int32_t Hkv, HG, P;
+    int32_t Hkv, HG, P, d;
     CUtensorMap map;
 };
 
@@ -105,11 +106,11 @@ const CUtensorMap* get_map(const void* base, const pkv_shape& s, int HG) {
     for (int i = 0; i < count; ++i) {
         const MapCacheEntry& e = cache[i];
         if (e.base == base && e.num_pages == s.num_pages && e.sp == st.page && e.st == st.token && e.sh == st.head &&
-            e.Hkv == s.Hkv && e.HG == HG && e.P == s.page_size)
+            e.Hkv == s.Hkv && e.HG == HG && e.P == s.page_size && e.d == s.d)
             return &e.map;
     }
     MapCacheEntry e;
-    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv; e.HG = HG; e.P = s.page_size;
+    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv; e.HG = HG; e.P = s.page_size; e.d = s.d;
     if (!encode_map(base, s, st, HG, &e.map)) return nullptr;
     const int slot = count < kCap ? count++ : (next = (next + 1) % kCap);
     cache[slot] = e;
@@ -180,7 +181,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.part_m = ws.part_m; p.part_l = ws.part_l; p.part_acc = ws.part_acc;
     p.fuse_counters = ws.fuse_counters;
     p.stride_page = st.page; p.stride_token = st.token; p.stride_head = st.head;
-    p.B = s.B; p.Hq = s.Hq; p.Hkv = s.Hkv; p.max_pages = s.max_pages;
+    p.B = s.B; p.Hq = s.Hq; p.Hkv = s.Hkv; p.max_pages = s.max_pages; p.d = s.d;
     p.tile_tokens = rp.tile_tokens; p.merge_mode = rp.merge_mode;
     p.dynamic_sched = 1;
     p.force_replan = (rp.flags & PKV_FLAG_TEST_REPLAN) ? 1 : 0;
@@ -223,8 +224,8 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             int64_t row_slots = known_slots >= 0 ? known_slots : (int64_t)s.B * rp.S;
             if (known_slots < 0 && rp.split_mode == PKV_SPLIT_BALANCED && rp.num_sms > 0 && rp.num_sms < row_slots)
                 row_slots = rp.num_sms;
-            const int HG = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, row_slots, num_sms, rp.G == 16 ? 4 : 8);
-            p.prefetch_pages = rp.prefetch_kb * 1024 / (HG * 8192);
+            const int HG = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, row_slots, num_sms, max_heads_per_cta(rp.G, s.d));
+            p.prefetch_pages = rp.prefetch_kb * 1024 / decode_tma_stage_bytes(HG, s.d);
             // by value: inserting the V map may evict the cache entry the K pointer refers to
             const CUtensorMap* pk = get_map(k_cache, s, HG);
             CUtensorMap mk_copy, mv_copy;
@@ -245,7 +246,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             p.dynamic_sched = HG * (rp.G == 16 ? 2 : 1) == 8 ? 1 : 0;
             const int64_t units = row_slots * (s.Hkv / HG);
             const int grid = (int)(units < num_sms ? units : num_sms);
-            e = launch_decode_tma(p, rp.G, HG, grid, mk, mv, stream);
+            e = launch_decode_tma(p, rp.G, HG, s.d, grid, mk, mv, stream);
         } else {
             const int64_t cap = (int64_t)num_sms * 4;
             const int grid = (int)(bound < cap ? bound : cap);
@@ -436,7 +437,7 @@ pkv_status pkv_merge(const pkv_shape* shape, const float* part_m, const float* p
     p.hdr = nullptr;
     p.out = static_cast<__half*>(out);
     p.lse = lse;
-    p.B = shape->B; p.Hq = shape->Hq; p.Hkv = shape->Hkv;
+    p.B = shape->B; p.Hq = shape->Hq; p.Hkv = shape->Hkv; p.d = shape->d;
     const cudaError_t e = launch_merge(p, rp.G, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e, "merge launch");
     return PKV_OK;

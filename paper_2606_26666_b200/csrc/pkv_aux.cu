@@ -86,8 +86,8 @@ __global__ void __launch_bounds__(kBuildThreadsMax) pkv_build_workqueue_kernel(c
     }
 }
 
-// One CTA of NW warps per (row, query head, channel slice); CS = 1, 2 or 4 slices of 128 / CS
-// channels.  A state's slice is read by 32 / CS lanes (16 bytes each), so one load instruction of
+// One CTA of NW warps per (row, query head, channel slice); a slice is 128 / CS channels (CS = 1, 2
+// or 4), a row of d channels has d * CS / 128 of them.  A state's slice is read by 32 / CS lanes (16 bytes each), so one load instruction of
 // a warp covers CS states; every lane issues the loads of kMergeBatch states (m, l and its piece
 // of acc) before any arithmetic, so a row of up to NW * kMergeBatch * CS splits is ONE round trip
 // to L2, and folds them into an online state (M, L, A) -- the merge of PAPER.md:60-61 is
@@ -118,12 +118,13 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
     constexpr int LPS = 32 / CS;          // lanes per state
     __shared__ float4 sA[NW][LPS];
     __shared__ float sM[NW], sL[NW];
-    const int slice = blockIdx.x % CS, rh = blockIdx.x / CS;
+    const int nsl = p.d / (LPS * 4);      // slices of LPS * 4 channels per (row, head): d * CS / 128
+    const int slice = blockIdx.x % nsl, rh = blockIdx.x / nsl;
     const int row = rh / p.Hq, h = rh % p.Hq;
     const int kvh = h / G, hh = h % G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int sub = lane / LPS, cl = lane % LPS;
-    const int ch = slice * (kD / CS) + cl * 4;   // this lane's four channels
+    const int ch = slice * (LPS * 4) + cl * 4;   // this lane's four channels
     if (blockIdx.x == 0 && threadIdx.x == 0) PKV_TRACE_STAMP_MERGE(p, 0);
     pdl_launch_dependents();
     // A guess at the row's slot range, read (race-tolerant) before the decode grid has finished:
@@ -150,7 +151,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
             const int64_t r = (base_ + (ok ? s_ : 0)) * G + hh;
             mv[j] = ok ? __ldcg(p.part_m + r) : -INFINITY;
             lv[j] = ok ? __ldcg(p.part_l + r) : 0.f;
-            av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * kD + ch))
+            av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * p.d + ch))
                        : make_float4(0.f, 0.f, 0.f, 0.f);
         }
     };
@@ -260,7 +261,7 @@ cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     int nw, cs = 1;
     const bool known = p.plan.split_mode == PKV_SPLIT_FIXED_COUNT && p.plan.S > 0;
     const int n_max = known ? p.plan.S : kMaxSplits;
-    if (n_max > 32 && pairs * 4 <= 160) {
+    if (n_max > 32 && pairs * (p.d * 4 / 128) <= 160) {
         cs = 4;
         nw = 8;
     } else if (known) {
@@ -268,7 +269,8 @@ cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream) {
     } else {
         nw = pairs <= 148 ? 16 : (pairs <= 1024 ? 8 : 4);
     }
-    const int grid = pairs * cs;
+    if (p.d == 64 && cs == 1) cs = 2;     // a 64-channel row is half a warp: two states per load instruction
+    const int grid = pairs * (p.d * cs / 128);
 #define PKV_MERGE_CASE(GG, NWW, CSS, MB) \
     if (G == GG && nw == NWW && cs == CSS)  \
         return launch_pdl(pdl, pkv_merge_kernel<GG, NWW, CSS, MB>, dim3(grid), dim3(NWW * 32), 0, stream, p);

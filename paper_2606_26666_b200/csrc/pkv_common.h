@@ -138,7 +138,9 @@ inline int32_t balanced_chunk(int64_t W, int32_t U, int32_t tile_tokens, Fits fi
 // that still leaves work units for at least 85 % of the SMs (units = row slots x Hkv / HG; whole-page
 // boxes stream faster than head slices, so 128 units of two heads beat 256 units of one on 148 SMs:
 // config 2, S = 32: 23.4 vs 24.2 us per step).
-// max_hg: 4 when G = 16 (two warps per KV head, one per block of 8 query heads), else 8.
+// max_hg: 4 when G = 16 (two warps per KV head, one per block of 8 query heads) or d = 256 (a stage
+// of 8 heads would be 128 KiB), else 8.
+inline int max_heads_per_cta(int G, int d) { return (G == 16 || d == 256) ? 4 : 8; }
 inline int choose_heads_per_cta(int forced, int Hkv, int64_t row_slots, int num_sms, int max_hg = 8) {
     if (forced > 0 && Hkv % forced == 0 && forced <= max_hg) return forced;
     int best = 1;

@@ -56,9 +56,9 @@ struct UnitInfo {
     int grow;   // request row: the row of q, out, lse and block_table (= row unless the launch is indexed)
 };
 
-template <int G>
+template <int G, int D>
 struct SmemTail {
-    CombineBuf<G, kComputeWarps> cb;
+    CombineBuf<G, kComputeWarps, D> cb;
     unsigned long long full_k[kMaxStages];
     unsigned long long full_v[kMaxStages];
     unsigned long long empty_bar[kMaxStages];
@@ -78,22 +78,27 @@ struct SmemTail {
 // each with warps of its own that share the streamed K/V stage.
 __host__ __device__ constexpr int blocks_for(int G) { return G > 8 ? G / 8 : 1; }
 
-template <int G, int HG>
+// One stage = one block of 16 tokens of HG heads: K (16 x D halves) then V, per head D * 32 bytes each.
+__host__ __device__ constexpr int stage_bytes_for(int HG, int D) { return HG * D * 64; }
+
+template <int G, int HG, int D>
 __host__ __device__ constexpr int stages_for() {
     // 227 KiB per CTA, minus the tail, minus 1 KiB alignment slack
-    constexpr int avail = 232448 - 1024 - (int)sizeof(SmemTail<G / blocks_for(G)>);
-    constexpr int n = avail / (HG * 8192);
+    constexpr int avail = 232448 - 1024 - (int)sizeof(SmemTail<G / blocks_for(G), D>);
+    constexpr int n = avail / stage_bytes_for(HG, D);
     // Stage s always belongs to producer s % NP and, per head, to compute warp s % WPH (see the
     // kernel): any stage count works, the shares differ by at most one stage.
     return n > kMaxStages ? kMaxStages : n;
 }
 
-template <int G, int HG>
+template <int G, int HG, int D>
 __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 1)
     pkv_decode_tma_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap_k,
                           const __grid_constant__ CUtensorMap tmap_v) {
-    constexpr int kStages = stages_for<G, HG>();
-    constexpr int kStageBytes = HG * 8192;   // K: HG x 4096 | V: HG x 4096
+    constexpr int kStages = stages_for<G, HG, D>();
+    constexpr int kHeadBytes = D * 32;       // one head's 16 tokens x D channels of K (or V): D / 64 blocks of 2 KiB
+    constexpr int kStageBytes = stage_bytes_for(HG, D);   // K: HG x kHeadBytes | V: HG x kHeadBytes
+    constexpr int KK = D / 16;               // k-steps of S = K.Q^T and m-tiles of O^T = V^T.P^T
     constexpr int NP = producers_for(HG);
     constexpr int NBK = blocks_for(G);       // blocks of query heads per KV head (2 when G = 16)
     constexpr int GW = G / NBK;              // query heads one warp tracks (the MMA's N columns)
@@ -105,7 +110,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     extern __shared__ unsigned char smem_raw[];
     // 128-byte swizzle: every 2 KiB half-box must start on a 1024-byte boundary
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    SmemTail<GW>& tail = *reinterpret_cast<SmemTail<GW>*>(smem + (size_t)kStages * kStageBytes);
+    SmemTail<GW, D>& tail = *reinterpret_cast<SmemTail<GW, D>*>(smem + (size_t)kStages * kStageBytes);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t stage_base = smem_u32(smem);
@@ -178,8 +183,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 }
             }
             // q rows of the unit's HG*G query heads: HG*G*256 bytes, one 128-byte line per lane
-            const char* qrow = reinterpret_cast<const char*>(p.q + ((int64_t)d.grow * p.Hq + head0 * G) * kD);
-            for (int b = lane * 128; b < HG * G * kD * 2; b += 32 * 128) prefetch_l2(qrow + b);
+            const char* qrow = reinterpret_cast<const char*>(p.q + ((int64_t)d.grow * p.Hq + head0 * G) * D);
+            for (int b = lane * 128; b < HG * G * D * 2; b += 32 * 128) prefetch_l2(qrow + b);
         }
     }
     pdl_wait();   // queue (builder), q / seq_lens (upstream), out / partials (previous step's readers)
@@ -228,8 +233,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
         for (int i = blockIdx.x; i < p.B; i += gridDim.x) {   // rows without a task (A9)
             const int64_t gi = request_row(p.row_index, i);
             if ((p.fused_build ? tail.len_s[i] : __ldcg(p.seq_lens + gi)) > 0) continue;
-            for (int e = lane; e < p.Hq * kD; e += 32) {
-                p.out[gi * p.Hq * kD + e] = __float2half_rn(0.f);
+            for (int e = lane; e < p.Hq * D; e += 32) {
+                p.out[gi * p.Hq * D + e] = __float2half_rn(0.f);
                 if (p.lse && e < p.Hq) p.lse[gi * p.Hq + e] = -INFINITY;
             }
         }
@@ -358,11 +363,11 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                         if (k == 0 && c == 0 && i == 0 && warp == 0) PKV_TRACE_STAMP(p, 3);
                         mbar_wait(empty0 + 8 * s, par ^ 1);
                         const uint32_t dst = stage_base + s * kStageBytes;
-                        // box dims: (64 ch, 16 tok, 2 ch-halves, HG heads, 1 page)
-                        mbar_arrive_expect_tx(fullk0 + 8 * s, HG * 4096);
+                        // box dims: (64 ch, 16 tok, D / 64 channel blocks, HG heads, 1 page)
+                        mbar_arrive_expect_tx(fullk0 + 8 * s, HG * kHeadBytes);
                         tma_load_5d(dst, &tmap_k, fullk0 + 8 * s, 0, tok, 0, head0, page, kv_policy);
-                        mbar_arrive_expect_tx(fullv0 + 8 * s, HG * 4096);
-                        tma_load_5d(dst + HG * 4096, &tmap_v, fullv0 + 8 * s, 0, tok, 0, head0, page, kv_policy);
+                        mbar_arrive_expect_tx(fullv0 + 8 * s, HG * kHeadBytes);
+                        tma_load_5d(dst + HG * kHeadBytes, &tmap_v, fullv0 + 8 * s, 0, tok, 0, head0, page, kv_policy);
                     }
                 }
                 mine = nxt;
@@ -412,11 +417,11 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             const int np = ((tok1 + 15) >> 4) - p0;
 
             // Q^T as the MMA B operand: b0 = Q[head g4][kk*16 + 2*t4 .. +1], b1 = same + 8
-            uint32_t qb[8][2];
+            uint32_t qb[KK][2];
             {
-                const __half* qrow = p.q + ((int64_t)orow * p.Hq + kvh * G + h0 + (g4 < GW ? g4 : 0)) * kD;
+                const __half* qrow = p.q + ((int64_t)orow * p.Hq + kvh * G + h0 + (g4 < GW ? g4 : 0)) * D;
 #pragma unroll
-                for (int kk = 0; kk < 8; ++kk) {
+                for (int kk = 0; kk < KK; ++kk) {
                     const uint32_t lo = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + 2 * t4);
                     const uint32_t hi = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + 8 + 2 * t4);
                     qb[kk][0] = g4 < GW ? lo : 0u;
@@ -424,9 +429,9 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 }
             }
             float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
-            float o[8][4];
+            float o[KK][4];
 #pragma unroll
-            for (int mt = 0; mt < 8; ++mt) o[mt][0] = o[mt][1] = o[mt][2] = o[mt][3] = 0.f;
+            for (int mt = 0; mt < KK; ++mt) o[mt][0] = o[mt][1] = o[mt][2] = o[mt][3] = 0.f;
 
             bool first_page = true;
             // This warp's pages of the unit: those landing in the stages it owns (s % WPH == sub).
@@ -443,8 +448,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 cphase ^= (adv / kStages) & 1;
             }
             while (j < np) {
-                const uint32_t kb = stage_base + s * kStageBytes + hl * 4096;
-                const uint32_t vb = kb + HG * 4096;
+                const uint32_t kb = stage_base + s * kStageBytes + hl * kHeadBytes;
+                const uint32_t vb = kb + HG * kHeadBytes;
                 const int nvalid = tok1 - ((p0 + j) << 4);  // >= 1; >= 16 for all but the last page
 
                 // ---- S^T = K . Q^T, two accumulation chains (channel halves)
@@ -453,11 +458,11 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 first_page = false;
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-                for (int kk = 0; kk < 8; ++kk) {
+                for (int kk = 0; kk < KK; ++kk) {
                     uint32_t a0, a1, a2, a3;
                     const uint32_t chunk = ((kk & 3) << 1) | k_sel;
                     ldmatrix_x4(kb + (kk >> 2) * 2048 + k_tok * 128 + ((chunk ^ xr) << 4), a0, a1, a2, a3);
-                    if (kk < 4)
+                    if (((kk >> 2) & 1) == 0)   // alternate 64-channel blocks between the two chains
                         mma_16816(c0, a0, a1, a2, a3, qb[kk][0], qb[kk][1]);
                     else
                         mma_16816(c1, a0, a1, a2, a3, qb[kk][0], qb[kk][1]);
@@ -481,7 +486,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     lA *= alA;
                     lB *= alB;
 #pragma unroll
-                    for (int mt = 0; mt < 8; ++mt) {
+                    for (int mt = 0; mt < KK; ++mt) {
                         o[mt][0] *= alA; o[mt][2] *= alA;
                         o[mt][1] *= alB; o[mt][3] *= alB;
                     }
@@ -503,7 +508,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 mbar_wait(fullv0 + 8 * s, par);
                 uint32_t vdep = 0;   // a word of every V fragment (see the stage release below)
 #pragma unroll
-                for (int mt = 0; mt < 8; ++mt) {
+                for (int mt = 0; mt < KK; ++mt) {
                     uint32_t a0, a1, a2, a3;
                     const uint32_t chunk = ((mt & 3) << 1) | v_sel;
                     ldmatrix_x4_trans(vb + (mt >> 2) * 2048 + v_tok * 128 + ((chunk ^ xr) << 4), a0, a1, a2, a3);
@@ -543,10 +548,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     const int64_t hrow = (int64_t)orow * p.Hq + kvh * G + h0 + hA;
                     if (n_i <= 1) {
                         const float iA = 1.0f / lA, iB = hasB ? 1.0f / lB : 0.f;
-                        __half* oA = p.out + hrow * kD + g4;
-                        __half* oB = oA + kD;
+                        __half* oA = p.out + hrow * D + g4;
+                        __half* oB = oA + D;
 #pragma unroll
-                        for (int mt = 0; mt < 8; ++mt) {
+                        for (int mt = 0; mt < KK; ++mt) {
                             oA[mt * 16] = __float2half_rn(o[mt][0] * iA);
                             oA[mt * 16 + 8] = __float2half_rn(o[mt][2] * iA);
                             if (hasB) {
@@ -559,10 +564,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                             if (hasB) p.lse[hrow + 1] = mB * p.scale + logf(lB);
                         }
                     } else {
-                        float* aA = p.part_acc + (slot * G + h0 + hA) * kD + g4;
-                        float* aB = aA + kD;
+                        float* aA = p.part_acc + (slot * G + h0 + hA) * D + g4;
+                        float* aB = aA + D;
 #pragma unroll
-                        for (int mt = 0; mt < 8; ++mt) {
+                        for (int mt = 0; mt < KK; ++mt) {
                             aA[mt * 16] = o[mt][0];
                             aA[mt * 16 + 8] = o[mt][2];
                             if (hasB) {
@@ -586,7 +591,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 if (hA < GW) {
                     const bool hasB = hB < GW;   // G = 1: column B is padding
 #pragma unroll
-                    for (int mt = 0; mt < 8; ++mt) {
+                    for (int mt = 0; mt < KK; ++mt) {
                         tail.cb.acc[cw][hA][mt * 16 + g4] = o[mt][0];
                         tail.cb.acc[cw][hA][mt * 16 + g4 + 8] = o[mt][2];
                         if (hasB) {
@@ -600,17 +605,17 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     }
                 }
                 group_sync<WPH>(1 + grp);
-                finalize_task<G, WPH, kComputeWarps, GW>(p, tail.cb, grp, NGRP, row, orow, kvh, split, n_i, slot, gtid, 1 + grp, h0);
+                finalize_task<G, WPH, kComputeWarps, GW, D>(p, tail.cb, grp, NGRP, row, orow, kvh, split, n_i, slot, gtid, 1 + grp, h0);
             }
             if (k == 0 && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 6);
         }
     }
 }
 
-template <int G, int HG>
+template <int G, int HG, int D>
 cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, const CUtensorMap& mv,
                        cudaStream_t stream) {
-    constexpr int smem = stages_for<G, HG>() * HG * 8192 + (int)sizeof(SmemTail<G / blocks_for(G)>) + 1024;
+    constexpr int smem = stages_for<G, HG, D>() * stage_bytes_for(HG, D) + (int)sizeof(SmemTail<G / blocks_for(G), D>) + 1024;
     constexpr int threads = (producers_for(HG) + kComputeWarps + 1) * 32;
     // The dynamic shared-memory opt-in is a per-device (per-context) attribute of the kernel: one
     // flag per device ordinal, set on the first launch there (races only repeat the call).
@@ -619,35 +624,35 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64 || !attr_set[dev]) {
-        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
-    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG>, dim3(grid), dim3(threads), (size_t)smem, stream, p, mk, mv);
+    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG, D>, dim3(grid), dim3(threads),
+                      (size_t)smem, stream, p, mk, mv);
 }
 
 }  // namespace
 
-int decode_tma_smem_bytes(int G, int HG) {
-    const int tail = G == 1 ? (int)sizeof(SmemTail<1>) : G == 2 ? (int)sizeof(SmemTail<2>)
-                   : G == 4 ? (int)sizeof(SmemTail<4>) : (int)sizeof(SmemTail<8>);   // G = 16: two blocks of 8
-    int st = (232448 - 1024 - tail) / (HG * 8192);
-    if (st > kMaxStages) st = kMaxStages;
-    return st * HG * 8192 + tail + 1024;
-}
+int decode_tma_stage_bytes(int HG, int D) { return stage_bytes_for(HG, D); }
 
-cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int grid, const void* tmap_k,
+cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int grid, const void* tmap_k,
                               const void* tmap_v, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
     const CUtensorMap& mk = *reinterpret_cast<const CUtensorMap*>(tmap_k);
     const CUtensorMap& mv = *reinterpret_cast<const CUtensorMap*>(tmap_v);
-#define PKV_CASE(GG, HH) \
-    if (G == GG && HG == HH) return launch_one<GG, HH>(p, grid, mk, mv, stream);
-    PKV_CASE(4, 8) PKV_CASE(4, 4) PKV_CASE(4, 2) PKV_CASE(4, 1)
-    PKV_CASE(8, 8) PKV_CASE(8, 4) PKV_CASE(8, 2) PKV_CASE(8, 1)
-    PKV_CASE(2, 8) PKV_CASE(2, 4) PKV_CASE(2, 2) PKV_CASE(2, 1)
-    PKV_CASE(1, 8) PKV_CASE(1, 4) PKV_CASE(1, 2) PKV_CASE(1, 1)
-    PKV_CASE(16, 4) PKV_CASE(16, 2) PKV_CASE(16, 1)
+#define PKV_CASE(GG, HH, DD) \
+    if (G == GG && HG == HH && D == DD) return launch_one<GG, HH, DD>(p, grid, mk, mv, stream);
+    PKV_CASE(4, 8, 128) PKV_CASE(4, 4, 128) PKV_CASE(4, 2, 128) PKV_CASE(4, 1, 128)
+    PKV_CASE(8, 8, 128) PKV_CASE(8, 4, 128) PKV_CASE(8, 2, 128) PKV_CASE(8, 1, 128)
+    PKV_CASE(2, 8, 128) PKV_CASE(2, 4, 128) PKV_CASE(2, 2, 128) PKV_CASE(2, 1, 128)
+    PKV_CASE(1, 8, 128) PKV_CASE(1, 4, 128) PKV_CASE(1, 2, 128) PKV_CASE(1, 1, 128)
+    PKV_CASE(16, 4, 128) PKV_CASE(16, 2, 128) PKV_CASE(16, 1, 128)
+    // head dimensions 64 and 256: the paper's GQA shapes G = 4 and G = 8
+    PKV_CASE(4, 8, 64) PKV_CASE(4, 4, 64) PKV_CASE(4, 2, 64) PKV_CASE(4, 1, 64)
+    PKV_CASE(8, 8, 64) PKV_CASE(8, 4, 64) PKV_CASE(8, 2, 64) PKV_CASE(8, 1, 64)
+    PKV_CASE(4, 4, 256) PKV_CASE(4, 2, 256) PKV_CASE(4, 1, 256)   // d = 256: at most 4 heads per CTA
+    PKV_CASE(8, 4, 256) PKV_CASE(8, 2, 256) PKV_CASE(8, 1, 256)   // (a stage of 8 would be 128 KiB)
 #undef PKV_CASE
     return cudaErrorInvalidValue;
 }

@@ -46,6 +46,7 @@ struct DecodeParams {
     int32_t* fuse_counters;     // [B*Hkv]
     int64_t stride_page, stride_token, stride_head; // elements
     int32_t B, Hq, Hkv, max_pages, tile_tokens, merge_mode;
+    int32_t d;                   // head dimension: 64, 128 or 256
     PlanArgs plan;               // split policy (fused build)
     int64_t tasks_cap;
     int32_t fused_build;         // TMA kernel: 1 = every CTA derives the queue from seq_lens itself
@@ -565,7 +566,7 @@ __device__ __forceinline__ float merge_row_max(const DecodeParams& p, int64_t sl
 constexpr int kMergeBatch = 8;
 template <int G, int NK>
 __device__ __forceinline__ void merge_accumulate(const DecodeParams& p, int64_t slot_base, int n, int hh, float M,
-                                                 int first, int stride, int lane, float (&L)[NK], float4 (&A)[NK]) {
+                                                 int first, int stride, int ch, float (&L)[NK], float4 (&A)[NK]) {
 #pragma unroll
     for (int k = 0; k < NK; ++k) {
         L[k] = 0.f;
@@ -581,7 +582,7 @@ __device__ __forceinline__ void merge_accumulate(const DecodeParams& p, int64_t 
             const int64_t r = (slot_base + first + (int64_t)(ok ? i0 + j : 0) * stride) * G + hh;
             mv[j] = ok ? __ldcg(p.part_m + r) : -INFINITY;
             lv[j] = ok ? __ldcg(p.part_l + r) : 0.f;
-            av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * kD + lane * 4))
+            av[j] = ok ? __ldcg(reinterpret_cast<const float4*>(p.part_acc + r * p.d + ch))
                        : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
@@ -598,7 +599,7 @@ __device__ __forceinline__ void merge_accumulate(const DecodeParams& p, int64_t 
 // Stores four channels ch .. ch+3 of output row o (FP16) and, by the lane with store_lse, its LSE.
 __device__ __forceinline__ void merge_store(const DecodeParams& p, int64_t o, int ch, bool store_lse, float M, float L,
                                             float4 A) {
-    __half2* dst = reinterpret_cast<__half2*>(p.out + o * kD + ch);
+    __half2* dst = reinterpret_cast<__half2*>(p.out + o * p.d + ch);
     if (M == -INFINITY) {  // no state or only neutral states (A9)
         dst[0] = __floats2half2_rn(0.f, 0.f);
         dst[1] = __floats2half2_rn(0.f, 0.f);
@@ -616,26 +617,29 @@ template <int G>
 __device__ __forceinline__ void merge_head_warp(const DecodeParams& p, int64_t slot_base, int n, int orow, int kvh,
                                                 int hh, int lane) {
     const float M = merge_row_max<G>(p, slot_base, n, hh, lane);
-    float L[4];
-    float4 A[4];
-    merge_accumulate<G, 4>(p, slot_base, n, hh, M, 0, 1, lane, L, A);
-    const float Ls = ((L[0] + L[1]) + L[2]) + L[3];
-    float4 As;
-    As.x = ((A[0].x + A[1].x) + A[2].x) + A[3].x;
-    As.y = ((A[0].y + A[1].y) + A[2].y) + A[3].y;
-    As.z = ((A[0].z + A[1].z) + A[2].z) + A[3].z;
-    As.w = ((A[0].w + A[1].w) + A[2].w) + A[3].w;
-    merge_store(p, (int64_t)orow * p.Hq + kvh * G + hh, lane * 4, lane == 0, M, Ls, As);
+    // slabs of 128 channels: one for d = 64 (half the lanes) and 128, two for d = 256
+    for (int ch = lane * 4; ch < p.d; ch += 128) {
+        float L[4];
+        float4 A[4];
+        merge_accumulate<G, 4>(p, slot_base, n, hh, M, 0, 1, ch, L, A);
+        const float Ls = ((L[0] + L[1]) + L[2]) + L[3];
+        float4 As;
+        As.x = ((A[0].x + A[1].x) + A[2].x) + A[3].x;
+        As.y = ((A[0].y + A[1].y) + A[2].y) + A[3].y;
+        As.z = ((A[0].z + A[1].z) + A[2].z) + A[3].z;
+        As.w = ((A[0].w + A[1].w) + A[2].w) + A[3].w;
+        merge_store(p, (int64_t)orow * p.Hq + kvh * G + hh, ch, ch == 0, M, Ls, As);
+    }
 }
 
 // ------------------------------------------------------------------ task epilogue
 
 // Shared-memory combine buffer of one CTA: every compute warp leaves the state of its share of
 // a task's tokens in its own row; m in raw-dot units (x = scale * raw).
-constexpr int kAccStride = 132;  // floats per (warp, head) row of acc; 132 % 32 = 4 spreads banks
-template <int G, int NWTOT>
+// acc rows hold D + 4 floats: (D + 4) % 32 = 4 spreads the banks
+template <int G, int NWTOT, int D = kD>
 struct CombineBuf {
-    float acc[NWTOT][G][kAccStride];
+    float acc[NWTOT][G][D + 4];
     float m[NWTOT][G < 8 ? 8 : G];
     float l[NWTOT][G < 8 ? 8 : G];
     int flag[NWTOT];
@@ -677,14 +681,15 @@ __device__ __forceinline__ void fused_complete(const DecodeParams& p, int* flag,
 template <int G, int NW, int GW = G>
 __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* flag, int row, int orow, int kvh, int split,
                                                  int n_i, int64_t slot, int gtid, int bar_id, int h0 = 0) {
-    for (int idx = gtid; idx < GW * kD; idx += NW * 32) {
-        const int hh = h0 + idx / kD, dd = idx % kD;
+    const int dsh = __ffs(p.d) - 1;   // d is a power of two
+    for (int idx = gtid; idx < (GW << dsh); idx += NW * 32) {
+        const int hh = h0 + (idx >> dsh), dd = idx & (p.d - 1);
         if (n_i <= 1) {
             const int64_t o = (int64_t)orow * p.Hq + kvh * G + hh;
-            p.out[o * kD + dd] = __float2half_rn(0.f);
+            p.out[o * p.d + dd] = __float2half_rn(0.f);
             if (p.lse && dd == 0) p.lse[o] = -INFINITY;
         } else {
-            p.part_acc[(slot * G + hh) * kD + dd] = 0.f;
+            p.part_acc[(slot * G + hh) * p.d + dd] = 0.f;
             if (dd == 0) {
                 p.part_m[slot * G + hh] = -INFINITY;
                 p.part_l[slot * G + hh] = 0.f;
@@ -701,12 +706,12 @@ __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* fla
 // the group that completes the last split of (row, kvh) merges in place.
 // gtid = 0..NW*32-1 within the group; the group synchronises with group_sync<NW>(bar_id); the
 // caller has synchronised after filling `cb`.
-template <int G, int NW, int NWTOT, int GW = G>
-__device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<GW, NWTOT>& cb, int w0, int wstride,
+template <int G, int NW, int NWTOT, int GW = G, int D = kD>
+__device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<GW, NWTOT, D>& cb, int w0, int wstride,
                                               int row, int orow, int kvh, int split, int n_i, int64_t slot, int gtid,
                                               int bar_id, int h0 = 0) {
-    for (int idx = gtid; idx < GW * kD; idx += NW * 32) {
-        const int hh = idx / kD, dd = idx % kD;   // head within the group's block; h0 + hh within the KV head
+    for (int idx = gtid; idx < GW * D; idx += NW * 32) {
+        const int hh = idx / D, dd = idx % D;   // head within the group's block; h0 + hh within the KV head
         float M = -INFINITY;
 #pragma unroll
         for (int i = 0; i < NW; ++i) M = fmaxf(M, cb.m[w0 + i * wstride][hh]);
@@ -720,10 +725,10 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
         }
         if (n_i <= 1) {
             const int64_t o = (int64_t)orow * p.Hq + kvh * G + h0 + hh;
-            p.out[o * kD + dd] = __float2half_rn(A / L);
+            p.out[o * D + dd] = __float2half_rn(A / L);
             if (p.lse && dd == 0) p.lse[o] = M * p.scale + logf(L);
         } else {
-            p.part_acc[(slot * G + h0 + hh) * kD + dd] = A;
+            p.part_acc[(slot * G + h0 + hh) * D + dd] = A;
             if (dd == 0) {
                 p.part_m[slot * G + h0 + hh] = M * p.scale;
                 p.part_l[slot * G + h0 + hh] = L;
@@ -737,7 +742,7 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
 
 // Rows with N_i = 0 emit no task in the workqueue route: out = 0, lse = -inf (A9).
 __device__ __forceinline__ void zero_empty_rows(const DecodeParams& p) {
-    const int per_row = p.Hq * kD;
+    const int per_row = p.Hq * p.d;
     for (int i = blockIdx.x; i < p.B; i += gridDim.x) {
         const int64_t gi = request_row(p.row_index, i);
         if (p.seq_lens[gi] > 0) continue;
@@ -780,12 +785,12 @@ inline PlanArgs make_plan_args(const pkv_shape& shape, const Resolved& rp) {
 
 // launchers implemented in the .cu files
 cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStream_t stream);
-cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int grid, const void* tmap_k,
+cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int grid, const void* tmap_k,
                               const void* tmap_v, cudaStream_t stream);
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
                            const int32_t* row_index, QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
                            pkv_task* tasks, int64_t tasks_cap, cudaStream_t stream);
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream);
-int decode_tma_smem_bytes(int G, int HG);
+int decode_tma_stage_bytes(int HG, int D);
 
 }  // namespace pkv

@@ -32,7 +32,7 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
         return PKV_ERR_INVALID_ARG;
     }
     if (s.Hq % s.Hkv != 0) { set_error("Hq=%d is not a multiple of Hkv=%d", s.Hq, s.Hkv); return PKV_ERR_INVALID_ARG; }
-    if (s.d != kD) { set_error("d=%d not compiled in (d=128 only)", s.d); return PKV_ERR_UNSUPPORTED; }
+    if (s.d != 64 && s.d != 128 && s.d != 256) { set_error("d=%d not compiled in (64, 128 or 256)", s.d); return PKV_ERR_UNSUPPORTED; }
     if (s.page_size != 16 && s.page_size != 32 && s.page_size != 64) { set_error("page_size=%d not supported (16, 32 or 64)", s.page_size); return PKV_ERR_UNSUPPORTED; }
     const int G = s.Hq / s.Hkv;
     if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16) { set_error("G=Hq/Hkv=%d not compiled in (1, 2, 4, 8 and 16 only)", G); return PKV_ERR_UNSUPPORTED; }
@@ -74,7 +74,9 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
         set_error("heads_per_cta=%d must be 0 (auto), 1, 2, 4 or 8 and divide Hkv=%d", p.heads_per_cta, s.Hkv);
         return PKV_ERR_INVALID_ARG;
     }
-    if (G == 16 && p.heads_per_cta == 8) { set_error("heads_per_cta=8 is not available with G=16 (at most 4)"); return PKV_ERR_INVALID_ARG; }
+    if (p.heads_per_cta > max_heads_per_cta(G, s.d)) { set_error("heads_per_cta=8 is not available with G=16 or d=256 (at most 4)"); return PKV_ERR_INVALID_ARG; }
+    if (s.d != kD && G != 4 && G != 8) { set_error("d=%d is compiled in for G=4 and G=8 only (G=%d)", s.d, G); return PKV_ERR_UNSUPPORTED; }
+    if (s.d != kD && p.kernel == PKV_KERNEL_SIMT) { set_error("PKV_KERNEL_SIMT is compiled in for d=128 only"); return PKV_ERR_UNSUPPORTED; }
 
     int32_t S = p.num_splits;
     out->num_sms = p.num_sms > 0 ? p.num_sms : num_sms_or_0;
@@ -240,7 +242,7 @@ void launch_totals(const pkv_shape& s, const Resolved& rp, const int32_t* lens, 
     // A27: the busiest CTA's bytes.  A unit = the HG tasks of one (row, split) token range.
     t->max_share = 0;
     if (hdr.total_row_slots > 0) {
-        const int hg = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, hdr.total_row_slots, num_sms, rp.G == 16 ? 4 : 8);
+        const int hg = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, hdr.total_row_slots, num_sms, max_heads_per_cta(rp.G, s.d));
         const int64_t unit = (int64_t)max_tok * 2 * hg * s.d * 2;
         const int64_t units = (int64_t)hdr.total_row_slots * (s.Hkv / hg);
         t->max_share = units <= num_sms ? unit : t->kv_bytes / num_sms + unit;

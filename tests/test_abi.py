@@ -43,7 +43,7 @@ def shape(B, Hkv=8, Hq=32, max_pages=4096):
 
 
 @pytest.mark.parametrize("bad,status", [
-    (dict(d=64), pkv.PKV_ERR_UNSUPPORTED),
+    (dict(d=96), pkv.PKV_ERR_UNSUPPORTED),
     (dict(page_size=48), pkv.PKV_ERR_UNSUPPORTED),
     (dict(Hq=48, Hkv=16), pkv.PKV_ERR_UNSUPPORTED),        # G = 3 not compiled in
     (dict(Hq=30, Hkv=8), pkv.PKV_ERR_INVALID_ARG),

@@ -125,3 +125,58 @@ def test_g16_many_units_and_partials():
                 _check(dp, pol, ref, "hg%d %s" % (hg, pol))
     with pytest.raises(pkv.PkvError):
         dp.decode(pkv.Policy(tile_tokens=32, num_splits=1, heads_per_cta=8))
+
+
+@pytest.mark.parametrize("d", [64, 256])
+@pytest.mark.parametrize("Hkv", [8, 4])
+def test_head_dimensions_ragged_sweep(d, Hkv):
+    """d = 64 and d = 256 on the TMA kernel, G = 4 and G = 8: every heads-per-CTA
+    variant, both routes, separate / fused / channel-sliced merge, page size 32 as well."""
+    for P in (16, 32):
+        p = make_problem(RAGGED, seed=800 + d + Hkv + P, Hkv=Hkv, d=d, page_size=P)
+        dp = DevProblem(p)
+        ref = oracle_attention(p)
+        for hg in (0, 1, 2, 4, 8):
+            if hg > Hkv or (hg == 8 and d == 256):
+                continue
+            for pol in (pkv.Policy(tile_tokens=32, num_splits=1, heads_per_cta=hg),
+                        pkv.Policy(tile_tokens=32, num_splits=5, heads_per_cta=hg),
+                        pkv.Policy(tile_tokens=32, num_splits=40, heads_per_cta=hg),          # sliced merge when B*Hq is small
+                        pkv.Policy(tile_tokens=32, num_splits=3, heads_per_cta=hg, merge_mode=pkv.MERGE_FUSED, route=pkv.ROUTE_RECT),
+                        pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=24, heads_per_cta=hg)):
+                _, _, ws = _check(dp, pol, ref, "d%d P%d hg%d %s" % (d, P, hg, pol))
+        tasks, offs = pkv.pkv_read_workqueue(dp.shape, pol, ws)
+        want = wq.build_workqueue(RAGGED, Hkv, oracle_policy(pol))
+        assert tasks.tolist() == [list(t) for t in want.tasks]
+
+
+@pytest.mark.parametrize("d", [64, 256])
+def test_head_dimensions_single_long_row_and_token_counts(d):
+    """One long row (B = 1: the channel-sliced merge over 4 or 8 CTAs per head) and the K = 0
+    counting pin at d = 64 / 256; d with the SIMT kernel or another G is refused, not mis-computed."""
+    p = make_problem([9000], seed=900 + d, d=d)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    for pol in (pkv.Policy(tile_tokens=32, num_splits=64), pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0),
+                pkv.Policy(tile_tokens=32, num_splits=16)):
+        _check(dp, pol, ref, "d%d %s" % (d, pol))
+    lens = [4097, 33, 1, 1000]
+    p = make_problem(lens, seed=41 + d, d=d)
+    p.k_cache[...] = 0
+    p.v_cache[...] = np.random.Generator(np.random.PCG64(7)).integers(-8, 9, size=p.v_cache.shape).astype(np.float16)
+    dp = DevProblem(p)
+    pol = pkv.Policy(tile_tokens=32, num_splits=7)
+    out, lse, ws = dp.decode(pol)
+    assert_within_tolerance(out, oracle_attention(p)[0])
+    q = wq.build_workqueue(lens, 8, oracle_policy(pol))
+    m, l, a = read_partials(dp, pol, ws, q.num_tasks)
+    for (row, kvh, split, tb, te) in q.tasks:
+        n_i = q.split_offsets[row + 1] - q.split_offsets[row]
+        if n_i > 1:
+            slot = q.split_offsets[row] * 8 + kvh * n_i + split
+            assert np.all(l[slot] == min(te * 32, lens[row]) - tb * 32) and np.all(m[slot] == 0.0)
+    with pytest.raises(pkv.PkvError):
+        dp.decode(pkv.Policy(tile_tokens=32, num_splits=2, kernel=pkv.KERNEL_SIMT))
+    p2 = make_problem([100], seed=5, d=d, Hkv=16)
+    with pytest.raises(pkv.PkvError):
+        DevProblem(p2).decode(pkv.Policy(tile_tokens=32, num_splits=2))
