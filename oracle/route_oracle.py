@@ -35,7 +35,8 @@ Readings of what the paper leaves open:
       units of HG KV heads (HG = the largest of 8, 4, 2, 1 dividing Hkv that leaves units for >= 85 % of
       the SMs, else 1 -- the smallest valid group when nothing fills the machine): one wave (units <= #SMs):
       max_share = the largest unit's bytes; several waves (dynamic hand-out): KVBytes/#SMs + the
-      largest unit's bytes.
+      largest unit's bytes.  A CTA that reads HG heads' slices of every page instead of whole pages
+      streams at beta * eta(HG), eta = 1 / 0.96 / 0.94 / 0.87 for HG = 8 / 4 / 2 / 1 (measured).
 
 Pins (tests/test_route_oracle.py): Table 4's bucket row (16.00 / 73.1 / 4.06 / 8.00), the cost of
 both Table-4 routes worked out by hand from the printed constants (beta = 331.2 GB/s, C_min = 4,
@@ -211,6 +212,9 @@ def max_share_bytes(seq_lens: Sequence[int], Hkv: int, d: int, q: wq.WorkQueue, 
     return unit if units <= num_sms else kv // num_sms + unit
 
 
-def stream_makespan_us(kv_bytes: int, share_bytes: int, k: CostConstants) -> float:
+HEAD_SLICE_EFFICIENCY = {8: 1.0, 4: 0.96, 2: 0.94, 1: 0.87}    # A27, measured on B200 (config 2, decode kernel alone)
+
+
+def stream_makespan_us(kv_bytes: int, share_bytes: int, k: CostConstants, hg: int = 8) -> float:
     beta_cta = k.beta_gbps / (k.c_min * k.num_sms)
-    return max(kv_bytes / (k.beta_gbps * 1e3), share_bytes / (beta_cta * 1e3))
+    return max(kv_bytes / (k.beta_gbps * HEAD_SLICE_EFFICIENCY[hg] * 1e3), share_bytes / (beta_cta * 1e3))

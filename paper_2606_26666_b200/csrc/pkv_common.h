@@ -162,5 +162,9 @@ pkv_status plan_host(const pkv_shape& shape, const Resolved& rp, const int32_t* 
 constexpr double kB200BetaGbps = 7060.0;
 constexpr double kB200LambdaUs = 2.0;
 constexpr double kB200CMin = 0.72;
+// A27: streaming efficiency of a CTA that reads HG heads' slices of every page (HG * d * 2 bytes
+// per token row out of Hkv * d * 2): whole pages stream at beta, single-head slices at 0.87 beta
+// (config 2, decode kernel alone: 20.5 / 21.4 / 21.8 / 23.5 us at HG = 8 / 4 / 2 / 1).
+inline double head_slice_efficiency(int hg) { return hg >= 8 ? 1.0 : (hg >= 4 ? 0.96 : (hg >= 2 ? 0.94 : 0.87)); }
 
 }  // namespace pkv

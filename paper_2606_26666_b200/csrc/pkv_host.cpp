@@ -226,8 +226,8 @@ namespace {
 // Totals of one launch pair (policy resolved, lengths on the host) for the cost model.
 struct RouteTotals {
     int64_t kv_bytes = 0, merge_bytes = 0, tasks = 0, launches = 0;
-    double makespan_bytes_over_beta_cta = 0.0;   // filled by the caller
     int64_t max_share = 0;
+    double slice_eff = 1.0;   // A27: head_slice_efficiency of the launch's heads per CTA
 };
 
 void launch_totals(const pkv_shape& s, const Resolved& rp, const int32_t* lens, int num_sms, RouteTotals* t) {
@@ -246,6 +246,7 @@ void launch_totals(const pkv_shape& s, const Resolved& rp, const int32_t* lens, 
         const int64_t unit = (int64_t)max_tok * 2 * hg * s.d * 2;
         const int64_t units = (int64_t)hdr.total_row_slots * (s.Hkv / hg);
         t->max_share = units <= num_sms ? unit : t->kv_bytes / num_sms + unit;
+        t->slice_eff = head_slice_efficiency(hg);
     }
 }
 
@@ -370,7 +371,7 @@ pkv_status pkv_estimate_cost(const pkv_shape* shape, const pkv_split_policy* pol
     double makespan = 0.0;
     if (bucket_tokens == 0) {
         launch_totals(*shape, rp, seq_lens_host, model->num_sms, &sum);
-        const double a = (double)sum.kv_bytes / beta, b = (double)sum.max_share / beta_cta;
+        const double a = (double)sum.kv_bytes / (beta * sum.slice_eff), b = (double)sum.max_share / beta_cta;
         makespan = a > b ? a : b;
     } else {
         const int32_t B = shape->B;
@@ -390,7 +391,7 @@ pkv_status pkv_estimate_cost(const pkv_shape* shape, const pkv_split_policy* pol
             launch_totals(sub, rb, lens.data(), model->num_sms, &t);
             sum.kv_bytes += t.kv_bytes; sum.merge_bytes += t.merge_bytes; sum.tasks += t.tasks; sum.launches += t.launches;
             if (t.max_share > sum.max_share) sum.max_share = t.max_share;
-            const double a = (double)t.kv_bytes / beta, c = (double)t.max_share / beta_cta;
+            const double a = (double)t.kv_bytes / (beta * t.slice_eff), c = (double)t.max_share / beta_cta;
             makespan += a > c ? a : c;
         }
     }
@@ -416,8 +417,19 @@ pkv_status pkv_choose_policy(const pkv_shape* shape, const int32_t* seq_lens_hos
     pkv_split_policy best = *base;
     pkv_cost_estimate best_est;
     bool have = false;
-    // candidates: BALANCED on page-size tiles, then FIXED_COUNT S = 1, 2, 4, ..., 128 on 32-token tiles
-    for (int c = -1; c <= 7; ++c) {
+    // candidates: BALANCED on page-size tiles, then FIXED_COUNT S = 1, 2, 4, ..., 128 and the
+    // single-wave fit S = floor(SMs / (B * head groups)) on 32-token tiles
+    const int sms = base->num_sms > 0 ? base->num_sms : model->num_sms;
+    int s_fit = 0;
+    if (shape && shape->B > 0 && shape->Hkv > 0 && shape->Hq % shape->Hkv == 0) {
+        const int mh = max_heads_per_cta(shape->Hq / shape->Hkv, shape->d);
+        int hg = mh;
+        while (hg > 1 && (hg > shape->Hkv || shape->Hkv % hg)) hg >>= 1;
+        s_fit = sms / (shape->B * (shape->Hkv / hg));
+        if (s_fit > kMaxSplits) s_fit = kMaxSplits;
+    }
+    for (int c = -1; c <= 8; ++c) {
+        if (c == 8 && (s_fit < 2 || (s_fit & (s_fit - 1)) == 0)) continue;   // nothing new to try
         pkv_split_policy pol = *base;
         pol.num_sms = base->num_sms > 0 ? base->num_sms : model->num_sms;
         if (c < 0) {
@@ -427,7 +439,7 @@ pkv_status pkv_choose_policy(const pkv_shape* shape, const int32_t* seq_lens_hos
         } else {
             pol.split_mode = PKV_SPLIT_FIXED_COUNT;
             pol.tile_tokens = 32;
-            pol.num_splits = 1 << c;
+            pol.num_splits = c == 8 ? s_fit : 1 << c;
         }
         pkv_cost_estimate e;
         const pkv_status st = pkv_estimate_cost(shape, &pol, seq_lens_host, 0, model, &e);

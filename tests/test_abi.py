@@ -204,7 +204,8 @@ def test_cost_model_matches_the_route_oracle():
                     c.useful_kv_bytes, c.merge_bytes, c.tasks, c.launches, share), (lens, pol)
                 for got, want in ((e["stream_us"], t.stream_us), (e["launch_us"], t.launch_us), (e["merge_us"], t.merge_us),
                                   (e["total_us"], t.total_us), (e["cta_work_per_sm"], t.cta_work_per_sm),
-                                  (e["makespan_us"], ro.stream_makespan_us(c.useful_kv_bytes, share, k))):
+                                  (e["makespan_us"], ro.stream_makespan_us(c.useful_kv_bytes, share, k,
+                                                                            ro.heads_per_cta(8, q.split_offsets[-1], m.num_sms) if q.split_offsets[-1] else 8))):
                     assert got == pytest.approx(want, rel=1e-12, abs=1e-300), (lens, pol)
                 if pol.split_mode == pkv.SPLIT_BALANCED:
                     continue
@@ -235,6 +236,9 @@ def test_choose_policy_picks_the_smallest_estimate():
         got, est = pkv.pkv_choose_policy(sh, np.array(lens, np.int32), m, base)
         cands = [pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0)] + \
                 [pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_COUNT, num_splits=1 << c) for c in range(8)]
+        s_fit = min(256, 148 // len(lens))          # Hkv = 8 in one head group
+        if s_fit >= 2 and s_fit & (s_fit - 1):
+            cands.append(pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_FIXED_COUNT, num_splits=s_fit))
         costs = [pkv.pkv_estimate_cost(sh, p, np.array(lens, np.int32), 0, m)["makespan_total_us"] for p in cands]
         best = cands[int(np.argmin(costs))]
         assert (got.split_mode, got.num_splits, got.tile_tokens) == (best.split_mode, best.num_splits, best.tile_tokens), lens
