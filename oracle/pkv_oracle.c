@@ -30,6 +30,12 @@
  * dominant key => V of that token, N = 1 and N = 2 closed forms.
  *
  * FP16 is decoded by the bit decoder below (no cuda_fp16.h, no compiler half type).
+ *
+ * FP8 KV ("dequantization-aware paged decode", PAPER.md:271 future work; DESIGN.md
+ * reading A28): pkv_oracle_attention_fp8 is Eq. (1) on k_j = k_scale[g] * e4m3(K bytes),
+ * v_j = v_scale[g] * e4m3(V bytes) -- OCP FP8 E4M3 ("fn": no infinities, S.1111.111 = NaN, largest
+ * finite 448), one FP32 scale per KV head.  The byte decoder is pinned on all 256 patterns against
+ * torch.float8_e4m3fn and against closed forms (tests/test_oracle_pins.py).
  */
 #include <math.h>
 #include <stdint.h>
@@ -56,13 +62,45 @@ static double half_bits_to_double(uint16_t h)
     return sign ? -v : v;
 }
 
+/* OCP FP8 E4M3 (fn) -> double, exact: 1 sign, 4 exponent (bias 7), 3 mantissa bits. */
+static double e4m3_bits_to_double(uint8_t b)
+{
+    int sign = (b >> 7) & 1;
+    int expo = (b >> 3) & 0xf;
+    int mant = b & 0x7;
+    double v;
+    if (expo == 0) {
+        v = ldexp((double)mant, -9);                 /* subnormal or zero: mant/8 * 2^-6 */
+    } else if (expo == 15 && mant == 7) {
+        v = NAN;                                     /* the only non-finite code */
+    } else {
+        v = ldexp((double)(mant + 8), expo - 10);    /* (1 + mant/8) * 2^(expo-7) */
+    }
+    return sign ? -v : v;
+}
+
 typedef struct {
     int B, Hq, Hkv, d, page_size, max_pages;
     int64_t stride_page, stride_token, stride_head;
     const uint16_t *q, *k_cache, *v_cache;
     const int32_t *block_table, *seq_lens;
     double scale;
+    /* FP8 caches (NULL: FP16 caches above are used) and their per-KV-head scales */
+    const uint8_t *k8, *v8;
+    const double *k_scale, *v_scale;
 } oracle_problem;
+
+/* channel c of the K (V) row at element offset off, KV head g, as a real number */
+static double k_elem(const oracle_problem *p, int64_t off, int c, int g)
+{
+    if (p->k8) return p->k_scale[g] * e4m3_bits_to_double(p->k8[off + c]);
+    return half_bits_to_double(p->k_cache[off + c]);
+}
+static double v_elem(const oracle_problem *p, int64_t off, int c, int g)
+{
+    if (p->v8) return p->v_scale[g] * e4m3_bits_to_double(p->v8[off + c]);
+    return half_bits_to_double(p->v_cache[off + c]);
+}
 
 /* address (in elements) of token j of row i, KV head g: the page accessor of PAPER.md:50 */
 static int64_t token_offset(const oracle_problem *p, int i, int64_t j, int g)
@@ -80,10 +118,10 @@ static void scores_range(const oracle_problem *p, int i, int h, int64_t j0, int6
     int g = h / G;
     const uint16_t *qv = p->q + ((int64_t)i * p->Hq + h) * p->d;
     for (int64_t j = j0; j < j1; ++j) {
-        const uint16_t *kv = p->k_cache + token_offset(p, i, j, g);
+        int64_t off = token_offset(p, i, j, g);
         double dot = 0.0;
         for (int c = 0; c < p->d; ++c)
-            dot += half_bits_to_double(qv[c]) * half_bits_to_double(kv[c]);
+            dot += half_bits_to_double(qv[c]) * k_elem(p, off, c, g);
         x[j - j0] = p->scale * dot;
     }
 }
@@ -104,11 +142,13 @@ static void range_state(const oracle_problem *p, int i, int h, int64_t j0, int64
     for (int64_t j = j0; j < j1; ++j) {
         double w = exp(x_scratch[j - j0] - m);
         l += w;
-        const uint16_t *vv = p->v_cache + token_offset(p, i, j, g);
-        for (int c = 0; c < d; ++c) a_out[c] += w * half_bits_to_double(vv[c]);
+        int64_t off = token_offset(p, i, j, g);
+        for (int c = 0; c < d; ++c) a_out[c] += w * v_elem(p, off, c, g);
     }
     *m_out = m; *l_out = l;
 }
+
+static int attention_impl(const oracle_problem *pp, double *out, double *lse, int num_threads);
 
 /* Eq. (1).  out [B,Hq,d] f64, lse [B,Hq] f64 (may be NULL).  Returns 0, or -1 on bad arguments. */
 int pkv_oracle_attention(int B, int Hq, int Hkv, int d, int page_size, int max_pages,
@@ -119,7 +159,29 @@ int pkv_oracle_attention(int B, int Hq, int Hkv, int d, int page_size, int max_p
 {
     if (B < 0 || Hkv <= 0 || Hq % Hkv || d <= 0 || page_size <= 0) return -1;
     oracle_problem p = { B, Hq, Hkv, d, page_size, max_pages, stride_page, stride_token, stride_head,
-                         q, k_cache, v_cache, block_table, seq_lens, scale };
+                         q, k_cache, v_cache, block_table, seq_lens, scale, NULL, NULL, NULL, NULL };
+    return attention_impl(&p, out, lse, num_threads);
+}
+
+/* The same on FP8 (E4M3) caches with one scale per KV head (reading A28); strides in elements = bytes. */
+int pkv_oracle_attention_fp8(int B, int Hq, int Hkv, int d, int page_size, int max_pages,
+                             int64_t stride_page, int64_t stride_token, int64_t stride_head,
+                             const uint16_t *q, const uint8_t *k8, const uint8_t *v8,
+                             const double *k_scale, const double *v_scale,
+                             const int32_t *block_table, const int32_t *seq_lens, double scale,
+                             double *out, double *lse, int num_threads)
+{
+    if (B < 0 || Hkv <= 0 || Hq % Hkv || d <= 0 || page_size <= 0 || !k8 || !v8 || !k_scale || !v_scale) return -1;
+    oracle_problem p = { B, Hq, Hkv, d, page_size, max_pages, stride_page, stride_token, stride_head,
+                         q, NULL, NULL, block_table, seq_lens, scale, k8, v8, k_scale, v_scale };
+    return attention_impl(&p, out, lse, num_threads);
+}
+
+static int attention_impl(const oracle_problem *pp, double *out, double *lse, int num_threads)
+{
+    oracle_problem p = *pp;
+    int B = p.B, Hq = p.Hq, Hkv = p.Hkv, d = p.d;
+    const int32_t *seq_lens = p.seq_lens;
     int G = Hq / Hkv;
     int units = B * Hkv;
     int failed = 0;
@@ -164,7 +226,7 @@ int pkv_oracle_split_states(int B, int Hq, int Hkv, int d, int page_size, int ma
 {
     if (B < 0 || Hkv <= 0 || Hq % Hkv || d <= 0 || page_size <= 0 || tile_tokens <= 0) return -1;
     oracle_problem p = { B, Hq, Hkv, d, page_size, max_pages, stride_page, stride_token, stride_head,
-                         q, k_cache, v_cache, block_table, seq_lens, scale };
+                         q, k_cache, v_cache, block_table, seq_lens, scale, NULL, NULL, NULL, NULL };
     int G = Hq / Hkv;
     int failed = 0;
 #ifdef _OPENMP
@@ -225,3 +287,5 @@ int pkv_oracle_max_threads(void)
 
 /* exposed so a test can pin the FP16 decoder against numpy's float16 on all 65536 patterns */
 double pkv_oracle_half_to_double(uint16_t h) { return half_bits_to_double(h); }
+/* ... and the E4M3 decoder against torch.float8_e4m3fn on all 256 */
+double pkv_oracle_e4m3_to_double(uint8_t b) { return e4m3_bits_to_double(b); }

@@ -253,3 +253,57 @@ def test_scale_is_applied_to_scores():
                                         page_size=p.page_size, scale=p.scale)
     assert np.abs(out_a - out_b).max() <= 1e-13 and np.abs(lse_a - lse_b).max() <= 1e-12
     assert default_scale(128) == float(np.float32(1 / math.sqrt(128)))
+
+
+# ---------------------------------------------------------------- FP8 (E4M3) KV, reading A28
+
+def test_e4m3_decoder_all_bit_patterns_and_closed_forms():
+    """The oracle's own E4M3 decoder on all 256 codes against torch.float8_e4m3fn (a library
+    routine), and against what the format fixes: 1.0 = 0x38, largest finite 448 = 0x7E, smallest
+    subnormal 2^-9, smallest normal 2^-6, one NaN code per sign, no infinity, monotone codes."""
+    import torch
+    want = torch.arange(256, dtype=torch.uint8).view(torch.float8_e4m3fn).to(torch.float64).numpy()
+    got = np.array([pkv_oracle.e4m3_to_double(b) for b in range(256)])
+    assert np.array_equal(np.isnan(got), np.isnan(want))
+    ok = ~np.isnan(want)
+    assert np.array_equal(got[ok], want[ok]) and np.array_equal(np.signbit(got[ok]), np.signbit(want[ok]))
+    assert got[0x38] == 1.0 and got[0x7E] == 448.0 and got[0x01] == 2.0 ** -9 and got[0x08] == 2.0 ** -6
+    assert np.isnan(got[0x7F]) and np.isnan(got[0xFF]) and not np.isinf(got).any()
+    assert np.all(np.diff(got[:0x7F]) > 0) and np.array_equal(got[0x80:0xFF], -got[:0x7F])
+
+
+def _quantize_e4m3(x: np.ndarray, scale: np.ndarray):
+    """x [pages, P, Hkv, d] / scale[g] rounded to E4M3 by torch (bytes), per KV head."""
+    import torch
+    t = torch.from_numpy((x.astype(np.float32) / scale[None, None, :, None].astype(np.float32)))
+    return t.to(torch.float8_e4m3fn).view(torch.uint8).numpy().copy()
+
+
+def test_fp8_attention_reduces_to_the_fp16_oracle_and_to_brute_force():
+    """With power-of-two scales every dequantised value scale * e4m3 is exactly an FP16 number, so
+    the FP8 entry point must agree with the (pinned) FP16 entry point on the dequantised caches to
+    rounding order; with arbitrary scales it must agree with dense numpy on the real values.  A
+    swapped K/V scale, a scale indexed by the wrong head or a mis-decoded byte fails one of them."""
+    p = make_problem([1, 17, 100, 0, 33], seed=61)
+    ks = np.array([0.5, 1.0, 2.0, 0.25, 4.0, 0.125, 1.0, 8.0])
+    vs = np.array([2.0, 0.5, 1.0, 4.0, 0.25, 1.0, 0.125, 0.5])
+    k8, v8 = _quantize_e4m3(p.k_cache, ks), _quantize_e4m3(p.v_cache, vs)
+    dec = np.vectorize(pkv_oracle.e4m3_to_double)
+    kd = (dec(k8) * ks[None, None, :, None]).astype(np.float16)
+    vd = (dec(v8) * vs[None, None, :, None]).astype(np.float16)
+    assert np.array_equal(kd.astype(np.float64), dec(k8) * ks[None, None, :, None])      # exact in FP16
+    got, got_lse = pkv_oracle.attention_fp8(p.q, k8, v8, ks, vs, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    ref, ref_lse = pkv_oracle.attention(p.q, kd, vd, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    assert np.abs(got - ref).max() <= 1e-12
+    fin = np.isfinite(ref_lse)
+    assert np.array_equal(np.isneginf(got_lse), np.isneginf(ref_lse)) and np.abs(got_lse[fin] - ref_lse[fin]).max() <= 1e-12
+    # arbitrary scales: dense numpy on the real values
+    ks2, vs2 = np.linspace(0.03, 0.11, 8), np.linspace(0.9, 0.05, 8)
+    got, got_lse = pkv_oracle.attention_fp8(p.q, k8, v8, ks2, vs2, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    pr = Problem(q=p.q, k_cache=dec(k8) * ks2[None, None, :, None], v_cache=dec(v8) * vs2[None, None, :, None],
+                 block_table=p.block_table, seq_lens=p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    ref, ref_lse = dense_attention_bruteforce(pr)
+    assert np.abs(got - ref).max() <= 1e-12 and np.abs(got_lse[fin] - ref_lse[fin]).max() <= 1e-12
+    # swapping the scales changes the result (the test can see them)
+    bad, _ = pkv_oracle.attention_fp8(p.q, k8, v8, vs2, ks2, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    assert np.abs(bad - ref).max() > 1e-3
