@@ -54,7 +54,8 @@ import pkv_inputs  # noqa: E402  (seeded input generators; no attention arithmet
 L2_BYTES = 126 * 1000 * 1000
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
 MIN_TIMED_MS = 50.0                # the K-step region is repeated until this much has been timed
-WORKLOADS = ["config1", "config2", "config3", "config4", "config4_b4", "config5", "config5_hkv4"]
+WORKLOADS = ["config1", "config2", "config3", "config4", "config4_b4", "config5", "config5_hkv4", "config2_fp8", "config3_fp8"]
+FP8_SCALE = 1.0 / 32.0      # per-KV-head scale of the FP8 workloads: N(0,1) / scale stays far inside +-448
 
 
 def parse_args(argv=None):
@@ -91,6 +92,11 @@ def parse_args(argv=None):
 # ------------------------------------------------------------------ workload
 
 def make_workload(name: str, seed: int, hkv: int = 0):
+    if name.endswith("_fp8"):           # the same trace on FP8 (E4M3) caches
+        w = make_workload(name[:-4], seed, hkv)
+        w.name += "_fp8"
+        w.extra["kv_elem_bytes"] = 1
+        return w
     if name == "config1":
         return pkv_inputs.config1(seed)
     if name == "config2":
@@ -135,7 +141,7 @@ def default_policy(pkv, name: str, args, w=None, num_sms=0):
         pol = pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, route=pkv.ROUTE_WORKQUEUE)
         if w is not None and num_sms > 0 and args.split_mode < 0 and args.splits < 0 and args.tile_tokens <= 0:
             shape = pkv.Shape(B=w.B, Hq=w.Hq, Hkv=w.Hkv, d=w.d, page_size=w.page_size, max_pages=w.max_pages,
-                              num_pages=w.num_pages)
+                              num_pages=w.num_pages, kv_dtype=pkv.KV_E4M3 if int(w.extra.get("kv_elem_bytes", 2)) == 1 else pkv.KV_F16)
             base = dataclasses.replace(pol, split_mode=pkv.SPLIT_AUTO)
             pol, _ = pkv.pkv_choose_policy(shape, w.seq_lens, pkv.pkv_default_cost_model(num_sms), base)
     if args.tile_tokens > 0:
@@ -171,13 +177,24 @@ class Runner:
         self.pkv, self.torch, self.w, self.pol, self.R = pkv, torch, w, pol, R
         self.device = device
         self.scale = float(np.float32(1.0 / math.sqrt(w.d)))
+        self.fp8 = int(w.extra.get("kv_elem_bytes", 2)) == 1
+        self.kv_scale = torch.full((w.Hkv,), FP8_SCALE, dtype=torch.float32, device=device) if self.fp8 else None
         self.shape = pkv.Shape(B=w.B, Hq=w.Hq, Hkv=w.Hkv, d=w.d, page_size=w.page_size,
-                               max_pages=w.max_pages, num_pages=w.num_pages)
+                               max_pages=w.max_pages, num_pages=w.num_pages, kv_dtype=pkv.KV_E4M3 if self.fp8 else pkv.KV_F16,
+                               k_scale=self.kv_scale, v_scale=self.kv_scale)
         self.q, self.k, self.v, self.bt = [], [], [], []
+
+        def pool(sd):
+            t = pkv_inputs.fill_pool_torch(w.pool_shape(), sd, device)
+            if not self.fp8:
+                return t
+            # the same N(0,1) draw, quantised to E4M3 bytes (inputs, not outputs: the oracle gets these bytes)
+            return (t.float() / FP8_SCALE).to(torch.float8_e4m3fn).view(torch.uint8)
+
         for r in range(R):
             self.q.append(pkv_inputs.fill_pool_torch((w.B, w.Hq, w.d), seed * 100 + 3 * r + 1, device))
-            self.k.append(pkv_inputs.fill_pool_torch(w.pool_shape(), seed * 100 + 3 * r + 2, device))
-            self.v.append(pkv_inputs.fill_pool_torch(w.pool_shape(), seed * 100 + 3 * r + 3, device))
+            self.k.append(pool(seed * 100 + 3 * r + 2))
+            self.v.append(pool(seed * 100 + 3 * r + 3))
             self.bt.append(torch.from_numpy(w.block_table).to(device))
         self.nlens = w.steps + 1
         lens_all = np.stack([w.seq_lens_at(t) for t in range(self.nlens)]).astype(np.int32)
@@ -407,8 +424,13 @@ def oracle_rows(torch, runner, rows, lens, r=0):
     q = np.ascontiguousarray(runner.q[r].cpu().numpy()[rows])
     sl = np.ascontiguousarray(np.asarray(lens, dtype=np.int32)[rows])
     t0 = time.perf_counter()
-    out, _ = pkv_oracle.attention(q, kc, vc, tc, sl, Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale,
-                                  num_threads=host_threads())
+    if runner.fp8:
+        sc = np.full(w.Hkv, FP8_SCALE, dtype=np.float64)
+        out, _ = pkv_oracle.attention_fp8(q, kc, vc, sc, sc, tc, sl, Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale,
+                                          num_threads=host_threads())
+    else:
+        out, _ = pkv_oracle.attention(q, kc, vc, tc, sl, Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale,
+                                      num_threads=host_threads())
     return out, time.perf_counter() - t0
 
 
@@ -641,7 +663,8 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
              ("config3_buckets_exact_S32", "config3", pkv.Policy(tile_tokens=32, num_splits=32, route=pkv.ROUTE_RECT,
                                                                  prefetch_kb=args.prefetch_kb)),
              ("config4", "config4", bal), ("config4_b4", "config4_b4", bal),
-             ("config5", "config5", bal), ("config5_hkv4", "config5_hkv4", bal)]
+             ("config5", "config5", bal), ("config5_hkv4", "config5_hkv4", bal),
+             ("config2_fp8", "config2_fp8", bal), ("config3_fp8", "config3_fp8", bal)]
     runner, cur = None, None
     for key, name, pol in cases:
         try:

@@ -25,6 +25,7 @@ KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
 FLAG_VALIDATE, FLAG_NO_PDL, FLAG_SEPARATE_BUILD, FLAG_TEST_REPLAN = 1, 2, 4, 8
 DEVERR_QUEUE_OVERFLOW, DEVERR_SEQ_LEN, DEVERR_PAGE_ID = 1, 2, 4
 STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL = 1, 2, 4, 7
+KV_F16, KV_E4M3 = 0, 1
 
 _i32, _i64 = ctypes.c_int32, ctypes.c_int64
 _vp = ctypes.c_void_p
@@ -42,7 +43,8 @@ class pkv_task(ctypes.Structure):
 
 class pkv_shape(ctypes.Structure):
     _fields_ = [("B", _i32), ("Hq", _i32), ("Hkv", _i32), ("d", _i32), ("page_size", _i32), ("max_pages", _i32),
-                ("num_pages", _i64), ("kv_stride_page", _i64), ("kv_stride_token", _i64), ("kv_stride_head", _i64)]
+                ("num_pages", _i64), ("kv_stride_page", _i64), ("kv_stride_token", _i64), ("kv_stride_head", _i64),
+                ("kv_dtype", _i32), ("reserved_", _i32), ("k_scale", _vp), ("v_scale", _vp)]
 
 
 class pkv_counters(ctypes.Structure):
@@ -170,10 +172,13 @@ class Shape:
     max_pages: int = 0
     num_pages: int = 0
     kv_strides: Tuple[int, int, int] = (0, 0, 0)   # (page, token, head) in elements; zeros = default layout
+    kv_dtype: int = 0                              # KV_F16 / KV_E4M3
+    k_scale: object = None                         # device float32 [Hkv] tensors (or raw addresses) for KV_E4M3
+    v_scale: object = None
 
     def c(self) -> pkv_shape:
         return pkv_shape(self.B, self.Hq, self.Hkv, self.d, self.page_size, self.max_pages, self.num_pages,
-                         *self.kv_strides)
+                         *self.kv_strides, self.kv_dtype, 0, _ptr(self.k_scale), _ptr(self.v_scale))
 
 
 @dataclass

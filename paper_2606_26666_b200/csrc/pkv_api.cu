@@ -79,12 +79,15 @@ bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int HG,
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t pages = (cuuint64_t)(s.num_pages > 0 ? s.num_pages : 1);
-    const cuuint32_t blocks = (cuuint32_t)(s.d / 64);   // 64-channel (128-byte) blocks of a head's row
-    cuuint64_t dims[5] = {64, (cuuint64_t)s.page_size, blocks, (cuuint64_t)s.Hkv, pages};
-    cuuint64_t strides[4] = {(cuuint64_t)st.token * 2, 128, (cuuint64_t)st.head * 2, (cuuint64_t)st.page * 2};
-    cuuint32_t box[5] = {64, 16, blocks, (cuuint32_t)HG, 1};
+    const bool fp8 = s.kv_dtype == PKV_KV_E4M3;
+    const cuuint64_t eb = fp8 ? 1 : 2;                   // bytes per element
+    const cuuint32_t inner = (cuuint32_t)(128 / eb);     // elements of one 128-byte swizzled row
+    const cuuint32_t blocks = (cuuint32_t)(s.d / inner); // 128-byte blocks of a head's row
+    cuuint64_t dims[5] = {inner, (cuuint64_t)s.page_size, blocks, (cuuint64_t)s.Hkv, pages};
+    cuuint64_t strides[4] = {(cuuint64_t)st.token * eb, 128, (cuuint64_t)st.head * eb, (cuuint64_t)st.page * eb};
+    cuuint32_t box[5] = {inner, 16, blocks, (cuuint32_t)HG, 1};
     cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-    const CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 5, const_cast<void*>(base), dims, strides, box, estr,
+    const CUresult r = fn(out, fp8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 5, const_cast<void*>(base), dims, strides, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
@@ -93,7 +96,7 @@ bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int HG,
 struct MapCacheEntry {
     const void* base;
     int64_t num_pages, sp, st, sh;
-    int32_t Hkv, HG, P, d;
+    int32_t Hkv, HG, P, d, dt;
     CUtensorMap map;
 };
 
@@ -106,11 +109,11 @@ const CUtensorMap* get_map(const void* base, const pkv_shape& s, int HG) {
     for (int i = 0; i < count; ++i) {
         const MapCacheEntry& e = cache[i];
         if (e.base == base && e.num_pages == s.num_pages && e.sp == st.page && e.st == st.token && e.sh == st.head &&
-            e.Hkv == s.Hkv && e.HG == HG && e.P == s.page_size && e.d == s.d)
+            e.Hkv == s.Hkv && e.HG == HG && e.P == s.page_size && e.d == s.d && e.dt == s.kv_dtype)
             return &e.map;
     }
     MapCacheEntry e;
-    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv; e.HG = HG; e.P = s.page_size; e.d = s.d;
+    e.base = base; e.num_pages = s.num_pages; e.sp = st.page; e.st = st.token; e.sh = st.head; e.Hkv = s.Hkv; e.HG = HG; e.P = s.page_size; e.d = s.d; e.dt = s.kv_dtype;
     if (!encode_map(base, s, st, HG, &e.map)) return nullptr;
     const int slot = count < kCap ? count++ : (next = (next + 1) % kCap);
     cache[slot] = e;
@@ -182,6 +185,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.fuse_counters = ws.fuse_counters;
     p.stride_page = st.page; p.stride_token = st.token; p.stride_head = st.head;
     p.B = s.B; p.Hq = s.Hq; p.Hkv = s.Hkv; p.max_pages = s.max_pages; p.d = s.d;
+    p.k_scale = s.k_scale; p.v_scale = s.v_scale;
     p.tile_tokens = rp.tile_tokens; p.merge_mode = rp.merge_mode;
     p.dynamic_sched = 1;
     p.force_replan = (rp.flags & PKV_FLAG_TEST_REPLAN) ? 1 : 0;
@@ -225,7 +229,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             if (known_slots < 0 && rp.split_mode == PKV_SPLIT_BALANCED && rp.num_sms > 0 && rp.num_sms < row_slots)
                 row_slots = rp.num_sms;
             const int HG = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, row_slots, num_sms, max_heads_per_cta(rp.G, s.d));
-            p.prefetch_pages = rp.prefetch_kb * 1024 / decode_tma_stage_bytes(HG, s.d);
+            p.prefetch_pages = rp.prefetch_kb * 1024 / decode_tma_stage_bytes(HG, s.d, s.kv_dtype == PKV_KV_E4M3);
             // by value: inserting the V map may evict the cache entry the K pointer refers to
             const CUtensorMap* pk = get_map(k_cache, s, HG);
             CUtensorMap mk_copy, mv_copy;
@@ -246,7 +250,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             p.dynamic_sched = HG * (rp.G == 16 ? 2 : 1) == 8 ? 1 : 0;
             const int64_t units = row_slots * (s.Hkv / HG);
             const int grid = (int)(units < num_sms ? units : num_sms);
-            e = launch_decode_tma(p, rp.G, HG, s.d, grid, mk, mv, stream);
+            e = launch_decode_tma(p, rp.G, HG, s.d, s.kv_dtype == PKV_KV_E4M3, grid, mk, mv, stream);
         } else {
             const int64_t cap = (int64_t)num_sms * 4;
             const int grid = (int)(bound < cap ? bound : cap);
@@ -466,7 +470,7 @@ pkv_status pkv_get_counters(const pkv_shape* shape, const pkv_split_policy* poli
     host_out->merge_launches =
         (h.num_tasks > 0 && h.max_row_splits > 1 && rp.merge_mode == PKV_MERGE_SEPARATE) ? 1 : 0;
     host_out->build_launches = h.build_launches;
-    host_out->useful_kv_bytes = h.sum_seq_lens * 2 * shape->Hkv * shape->d * 2;
+    host_out->useful_kv_bytes = h.sum_seq_lens * 2 * shape->Hkv * shape->d * (shape->kv_dtype == PKV_KV_E4M3 ? 1 : 2);
     host_out->merge_bytes = (int64_t)h.num_tasks * rp.G * (shape->d + 2) * 4;
     host_out->num_splits = h.resolved_splits;
     host_out->max_row_splits = h.max_row_splits;
@@ -758,7 +762,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         counters_out->decode_launches = dl;
         counters_out->merge_launches = ml;
         counters_out->build_launches = (!fused && hdr->num_tasks > 0) ? 1 : 0;
-        counters_out->useful_kv_bytes = hdr->sum_seq_lens * 2 * s.Hkv * s.d * 2;
+        counters_out->useful_kv_bytes = hdr->sum_seq_lens * 2 * s.Hkv * s.d * (s.kv_dtype == PKV_KV_E4M3 ? 1 : 2);
         counters_out->merge_bytes = (int64_t)hdr->num_tasks * rp.G * (s.d + 2) * 4;
         counters_out->num_splits = hdr->resolved_splits;
         counters_out->max_row_splits = hdr->max_row_splits;

@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(kThreads) pkv_decode_simt_kernel(const DecodeP
             }
         }
         __syncthreads();
-        finalize_task<G, kWarps, kWarps>(p, cb, 0, 1, row, orow, kvh, task.split, n_i, slot, tid, 0);
+        finalize_task<G, kWarps, kWarps>(p, cb, 0, 1, row, orow, kvh, task.split, n_i, slot, tid, 0, 0, p.scale, p.scale_log2);
     }
 }
 

@@ -79,25 +79,27 @@ struct SmemTail {
 __host__ __device__ constexpr int blocks_for(int G) { return G > 8 ? G / 8 : 1; }
 
 // One stage = one block of 16 tokens of HG heads: K (16 x D halves) then V, per head D * 32 bytes each.
-__host__ __device__ constexpr int stage_bytes_for(int HG, int D) { return HG * D * 64; }
+// FP8 caches: one byte per channel, half the bytes.
+__host__ __device__ constexpr int stage_bytes_for(int HG, int D, bool fp8 = false) { return HG * D * (fp8 ? 32 : 64); }
 
-template <int G, int HG, int D>
+template <int G, int HG, int D, bool FP8 = false>
 __host__ __device__ constexpr int stages_for() {
     // 227 KiB per CTA, minus the tail, minus 1 KiB alignment slack
     constexpr int avail = 232448 - 1024 - (int)sizeof(SmemTail<G / blocks_for(G), D>);
-    constexpr int n = avail / stage_bytes_for(HG, D);
+    constexpr int n = avail / stage_bytes_for(HG, D, FP8);
     // Stage s always belongs to producer s % NP and, per head, to compute warp s % WPH (see the
     // kernel): any stage count works, the shares differ by at most one stage.
     return n > kMaxStages ? kMaxStages : n;
 }
 
-template <int G, int HG, int D>
+template <int G, int HG, int D, bool FP8>
 __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 1)
     pkv_decode_tma_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap_k,
                           const __grid_constant__ CUtensorMap tmap_v) {
-    constexpr int kStages = stages_for<G, HG, D>();
-    constexpr int kHeadBytes = D * 32;       // one head's 16 tokens x D channels of K (or V): D / 64 blocks of 2 KiB
-    constexpr int kStageBytes = stage_bytes_for(HG, D);   // K: HG x kHeadBytes | V: HG x kHeadBytes
+    static_assert(!FP8 || D == 128, "FP8 caches: one 128-byte swizzled row per token and head");
+    constexpr int kStages = stages_for<G, HG, D, FP8>();
+    constexpr int kHeadBytes = D * (FP8 ? 16 : 32);   // one head's 16 tokens x D channels of K (or V): blocks of 2 KiB
+    constexpr int kStageBytes = stage_bytes_for(HG, D, FP8);   // K: HG x kHeadBytes | V: HG x kHeadBytes
     constexpr int KK = D / 16;               // k-steps of S = K.Q^T and m-tiles of O^T = V^T.P^T
     constexpr int NP = producers_for(HG);
     constexpr int NBK = blocks_for(G);       // blocks of query heads per KV head (2 when G = 16)
@@ -416,14 +418,25 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             const int p0 = tok0 >> 4;
             const int np = ((tok1 + 15) >> 4) - p0;
 
-            // Q^T as the MMA B operand: b0 = Q[head g4][kk*16 + 2*t4 .. +1], b1 = same + 8
+            // FP8 caches (reading A28): x = (scale * k_scale[kvh]) * <q, e4m3(K)>, O = v_scale[kvh] * ...
+            float sc = p.scale, sc2 = p.scale_log2, vsc = 1.f;
+            if constexpr (FP8) {
+                const float ksc = p.k_scale ? __ldg(p.k_scale + kvh) : 1.f;
+                sc *= ksc;
+                sc2 *= ksc;
+                vsc = p.v_scale ? __ldg(p.v_scale + kvh) : 1.f;
+            }
+            // Q^T as the MMA B operand: b0 = Q[head g4][kk*16 + 2*t4 .. +1], b1 = same + 8.
+            // FP8: a lane's ldmatrix word holds FOUR consecutive channels 4*t4 .. 4*t4+3 of the
+            // 16-channel chunk; they stand for k = 2*t4, 2*t4+1 (a0/a1) and k = 2*t4+8, 2*t4+9
+            // (a2/a3), so Q is read with the same permutation of the contraction index.
             uint32_t qb[KK][2];
             {
                 const __half* qrow = p.q + ((int64_t)orow * p.Hq + kvh * G + h0 + (g4 < GW ? g4 : 0)) * D;
 #pragma unroll
                 for (int kk = 0; kk < KK; ++kk) {
-                    const uint32_t lo = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + 2 * t4);
-                    const uint32_t hi = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + 8 + 2 * t4);
+                    const uint32_t lo = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + (FP8 ? 4 * t4 : 2 * t4));
+                    const uint32_t hi = *reinterpret_cast<const uint32_t*>(qrow + kk * 16 + (FP8 ? 4 * t4 + 2 : 8 + 2 * t4));
                     qb[kk][0] = g4 < GW ? lo : 0u;
                     qb[kk][1] = g4 < GW ? hi : 0u;
                 }
@@ -457,15 +470,29 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 if (k == 0 && first_page && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 4);
                 first_page = false;
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
+                if constexpr (FP8) {
+                    // one ldmatrix.x4 = 16 tokens x 32 channels of bytes: (tok 0-7 | 8-15) x (chunk 2j | 2j+1)
 #pragma unroll
-                for (int kk = 0; kk < KK; ++kk) {
-                    uint32_t a0, a1, a2, a3;
-                    const uint32_t chunk = ((kk & 3) << 1) | k_sel;
-                    ldmatrix_x4(kb + (kk >> 2) * 2048 + k_tok * 128 + ((chunk ^ xr) << 4), a0, a1, a2, a3);
-                    if (((kk >> 2) & 1) == 0)   // alternate 64-channel blocks between the two chains
-                        mma_16816(c0, a0, a1, a2, a3, qb[kk][0], qb[kk][1]);
-                    else
-                        mma_16816(c1, a0, a1, a2, a3, qb[kk][0], qb[kk][1]);
+                    for (int j = 0; j < KK / 2; ++j) {
+                        uint32_t r0, r1, r2, r3;
+                        const uint32_t chunk = (j << 1) | k_sel;
+                        ldmatrix_x4(kb + k_tok * 128 + ((chunk ^ xr) << 4), r0, r1, r2, r3);
+                        mma_16816(c0, cvt_e4m3x2_to_half2(r0), cvt_e4m3x2_to_half2(r1), cvt_e4m3x2_to_half2(r0 >> 16),
+                                  cvt_e4m3x2_to_half2(r1 >> 16), qb[2 * j][0], qb[2 * j][1]);
+                        mma_16816(c1, cvt_e4m3x2_to_half2(r2), cvt_e4m3x2_to_half2(r3), cvt_e4m3x2_to_half2(r2 >> 16),
+                                  cvt_e4m3x2_to_half2(r3 >> 16), qb[2 * j + 1][0], qb[2 * j + 1][1]);
+                    }
+                } else {
+#pragma unroll
+                    for (int kk = 0; kk < KK; ++kk) {
+                        uint32_t a0, a1, a2, a3;
+                        const uint32_t chunk = ((kk & 3) << 1) | k_sel;
+                        ldmatrix_x4(kb + (kk >> 2) * 2048 + k_tok * 128 + ((chunk ^ xr) << 4), a0, a1, a2, a3);
+                        if (((kk >> 2) & 1) == 0)   // alternate 64-channel blocks between the two chains
+                            mma_16816(c0, a0, a1, a2, a3, qb[kk][0], qb[kk][1]);
+                        else
+                            mma_16816(c1, a0, a1, a2, a3, qb[kk][0], qb[kk][1]);
+                    }
                 }
                 // lane holds S^T[tok g4][hA], [g4][hB], [g4+8][hA], [g4+8][hB]
                 float s0 = c0[0] + c1[0], s1 = c0[1] + c1[1], s2 = c0[2] + c1[2], s3 = c0[3] + c1[3];
@@ -481,8 +508,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 }
                 const float nmA = fmaxf(mA, mxA), nmB = fmaxf(mB, mxB);   // finite: the page has a valid token
                 if (__any_sync(0xffffffffu, (nmA != mA) | (nmB != mB))) {
-                    const float alA = ex2_approx((mA - nmA) * p.scale_log2);  // m = -inf -> 0
-                    const float alB = ex2_approx((mB - nmB) * p.scale_log2);
+                    const float alA = ex2_approx((mA - nmA) * sc2);  // m = -inf -> 0
+                    const float alB = ex2_approx((mB - nmB) * sc2);
                     lA *= alA;
                     lB *= alB;
 #pragma unroll
@@ -493,11 +520,11 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     mA = nmA;
                     mB = nmB;
                 }
-                const float offA = mA * p.scale_log2, offB = mB * p.scale_log2;
-                const float p0f = ex2_approx(fmaf(s0, p.scale_log2, -offA));
-                const float p1f = ex2_approx(fmaf(s1, p.scale_log2, -offB));
-                const float p2f = ex2_approx(fmaf(s2, p.scale_log2, -offA));
-                const float p3f = ex2_approx(fmaf(s3, p.scale_log2, -offB));
+                const float offA = mA * sc2, offB = mB * sc2;
+                const float p0f = ex2_approx(fmaf(s0, sc2, -offA));
+                const float p1f = ex2_approx(fmaf(s1, sc2, -offB));
+                const float p2f = ex2_approx(fmaf(s2, sc2, -offA));
+                const float p3f = ex2_approx(fmaf(s3, sc2, -offB));
                 lA += p0f + p2f;   // lane-partial sums; reduced across lanes at unit end
                 lB += p1f + p3f;
                 // P^T as the MMA B operand: transpose the two 8x8 (token x head) blocks
@@ -507,13 +534,31 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 // ---- O^T += V^T . P^T
                 mbar_wait(fullv0 + 8 * s, par);
                 uint32_t vdep = 0;   // a word of every V fragment (see the stage release below)
+                if constexpr (FP8) {
+                    // ldmatrix.trans moves 16-bit units, i.e. PAIRS of channels: a lane gets tokens
+                    // 2*t4, 2*t4+1 of the channel pair (2*g4, 2*g4+1) of a 16-channel chunk.  Byte
+                    // permutes split the pair: MMA row g4 is channel 16*mt + 2*g4, row g4+8 is channel
+                    // 16*mt + 2*g4 + 1 (the epilogue stores with the same map).
 #pragma unroll
-                for (int mt = 0; mt < KK; ++mt) {
-                    uint32_t a0, a1, a2, a3;
-                    const uint32_t chunk = ((mt & 3) << 1) | v_sel;
-                    ldmatrix_x4_trans(vb + (mt >> 2) * 2048 + v_tok * 128 + ((chunk ^ xr) << 4), a0, a1, a2, a3);
-                    mma_16816(o[mt], a0, a1, a2, a3, pb0, pb1);
-                    vdep ^= a3;
+                    for (int j = 0; j < KK / 2; ++j) {
+                        uint32_t r0, r1, r2, r3;
+                        const uint32_t chunk = (j << 1) | k_sel;
+                        ldmatrix_x4_trans(vb + k_tok * 128 + ((chunk ^ xr) << 4), r0, r1, r2, r3);
+                        mma_16816(o[2 * j], cvt_e4m3x2_to_half2(__byte_perm(r0, 0, 0x0020)), cvt_e4m3x2_to_half2(__byte_perm(r0, 0, 0x0031)),
+                                  cvt_e4m3x2_to_half2(__byte_perm(r1, 0, 0x0020)), cvt_e4m3x2_to_half2(__byte_perm(r1, 0, 0x0031)), pb0, pb1);
+                        mma_16816(o[2 * j + 1], cvt_e4m3x2_to_half2(__byte_perm(r2, 0, 0x0020)), cvt_e4m3x2_to_half2(__byte_perm(r2, 0, 0x0031)),
+                                  cvt_e4m3x2_to_half2(__byte_perm(r3, 0, 0x0020)), cvt_e4m3x2_to_half2(__byte_perm(r3, 0, 0x0031)), pb0, pb1);
+                        vdep ^= r0 ^ r1 ^ r2 ^ r3;
+                    }
+                } else {
+#pragma unroll
+                    for (int mt = 0; mt < KK; ++mt) {
+                        uint32_t a0, a1, a2, a3;
+                        const uint32_t chunk = ((mt & 3) << 1) | v_sel;
+                        ldmatrix_x4_trans(vb + (mt >> 2) * 2048 + v_tok * 128 + ((chunk ^ xr) << 4), a0, a1, a2, a3);
+                        mma_16816(o[mt], a0, a1, a2, a3, pb0, pb1);
+                        vdep ^= a3;
+                    }
                 }
                 __syncwarp();
                 if (lane == 0) {
@@ -539,6 +584,8 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 lA += __shfl_xor_sync(0xffffffffu, lA, off);
                 lB += __shfl_xor_sync(0xffffffffu, lB, off);
             }
+            // channels of accumulator rows g4 and g4 + 8 inside an m-tile of 16 (FP8: see the V loop)
+            const int cA = FP8 ? 2 * g4 : g4, cB = FP8 ? 2 * g4 + 1 : g4 + 8;
             if constexpr (WPH == 1) {
                 // The warp owns the whole task: its state goes from the MMA accumulators straight
                 // to the task's slot (or to `out`), no shared-memory round trip.  Per store
@@ -547,39 +594,39 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     const bool hasB = hB < GW;   // G = 1: column B is padding
                     const int64_t hrow = (int64_t)orow * p.Hq + kvh * G + h0 + hA;
                     if (n_i <= 1) {
-                        const float iA = 1.0f / lA, iB = hasB ? 1.0f / lB : 0.f;
-                        __half* oA = p.out + hrow * D + g4;
+                        const float iA = vsc / lA, iB = hasB ? vsc / lB : 0.f;
+                        __half* oA = p.out + hrow * D;
                         __half* oB = oA + D;
 #pragma unroll
                         for (int mt = 0; mt < KK; ++mt) {
-                            oA[mt * 16] = __float2half_rn(o[mt][0] * iA);
-                            oA[mt * 16 + 8] = __float2half_rn(o[mt][2] * iA);
+                            oA[mt * 16 + cA] = __float2half_rn(o[mt][0] * iA);
+                            oA[mt * 16 + cB] = __float2half_rn(o[mt][2] * iA);
                             if (hasB) {
-                                oB[mt * 16] = __float2half_rn(o[mt][1] * iB);
-                                oB[mt * 16 + 8] = __float2half_rn(o[mt][3] * iB);
+                                oB[mt * 16 + cA] = __float2half_rn(o[mt][1] * iB);
+                                oB[mt * 16 + cB] = __float2half_rn(o[mt][3] * iB);
                             }
                         }
                         if (p.lse && g4 == 0) {
-                            p.lse[hrow] = mA * p.scale + logf(lA);
-                            if (hasB) p.lse[hrow + 1] = mB * p.scale + logf(lB);
+                            p.lse[hrow] = mA * sc + logf(lA);
+                            if (hasB) p.lse[hrow + 1] = mB * sc + logf(lB);
                         }
                     } else {
-                        float* aA = p.part_acc + (slot * G + h0 + hA) * D + g4;
+                        float* aA = p.part_acc + (slot * G + h0 + hA) * D;
                         float* aB = aA + D;
 #pragma unroll
                         for (int mt = 0; mt < KK; ++mt) {
-                            aA[mt * 16] = o[mt][0];
-                            aA[mt * 16 + 8] = o[mt][2];
+                            aA[mt * 16 + cA] = o[mt][0] * vsc;
+                            aA[mt * 16 + cB] = o[mt][2] * vsc;
                             if (hasB) {
-                                aB[mt * 16] = o[mt][1];
-                                aB[mt * 16 + 8] = o[mt][3];
+                                aB[mt * 16 + cA] = o[mt][1] * vsc;
+                                aB[mt * 16 + cB] = o[mt][3] * vsc;
                             }
                         }
                         if (g4 == 0) {
-                            p.part_m[slot * G + h0 + hA] = mA * p.scale;
+                            p.part_m[slot * G + h0 + hA] = mA * sc;
                             p.part_l[slot * G + h0 + hA] = lA;
                             if (hasB) {
-                                p.part_m[slot * G + h0 + hB] = mB * p.scale;
+                                p.part_m[slot * G + h0 + hB] = mB * sc;
                                 p.part_l[slot * G + h0 + hB] = lB;
                             }
                         }
@@ -592,11 +639,11 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     const bool hasB = hB < GW;   // G = 1: column B is padding
 #pragma unroll
                     for (int mt = 0; mt < KK; ++mt) {
-                        tail.cb.acc[cw][hA][mt * 16 + g4] = o[mt][0];
-                        tail.cb.acc[cw][hA][mt * 16 + g4 + 8] = o[mt][2];
+                        tail.cb.acc[cw][hA][mt * 16 + cA] = o[mt][0] * vsc;
+                        tail.cb.acc[cw][hA][mt * 16 + cB] = o[mt][2] * vsc;
                         if (hasB) {
-                            tail.cb.acc[cw][hB][mt * 16 + g4] = o[mt][1];
-                            tail.cb.acc[cw][hB][mt * 16 + g4 + 8] = o[mt][3];
+                            tail.cb.acc[cw][hB][mt * 16 + cA] = o[mt][1] * vsc;
+                            tail.cb.acc[cw][hB][mt * 16 + cB] = o[mt][3] * vsc;
                         }
                     }
                     if (g4 == 0) {
@@ -605,17 +652,17 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     }
                 }
                 group_sync<WPH>(1 + grp);
-                finalize_task<G, WPH, kComputeWarps, GW, D>(p, tail.cb, grp, NGRP, row, orow, kvh, split, n_i, slot, gtid, 1 + grp, h0);
+                finalize_task<G, WPH, kComputeWarps, GW, D>(p, tail.cb, grp, NGRP, row, orow, kvh, split, n_i, slot, gtid, 1 + grp, h0, sc, sc2);
             }
             if (k == 0 && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 6);
         }
     }
 }
 
-template <int G, int HG, int D>
+template <int G, int HG, int D, bool FP8>
 cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, const CUtensorMap& mv,
                        cudaStream_t stream) {
-    constexpr int smem = stages_for<G, HG, D>() * stage_bytes_for(HG, D) + (int)sizeof(SmemTail<G / blocks_for(G), D>) + 1024;
+    constexpr int smem = stages_for<G, HG, D, FP8>() * stage_bytes_for(HG, D, FP8) + (int)sizeof(SmemTail<G / blocks_for(G), D>) + 1024;
     constexpr int threads = (producers_for(HG) + kComputeWarps + 1) * 32;
     // The dynamic shared-memory opt-in is a per-device (per-context) attribute of the kernel: one
     // flag per device ordinal, set on the first launch there (races only repeat the call).
@@ -624,25 +671,25 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64 || !attr_set[dev]) {
-        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG, D, FP8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
-    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG, D>, dim3(grid), dim3(threads),
+    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG, D, FP8>, dim3(grid), dim3(threads),
                       (size_t)smem, stream, p, mk, mv);
 }
 
 }  // namespace
 
-int decode_tma_stage_bytes(int HG, int D) { return stage_bytes_for(HG, D); }
+int decode_tma_stage_bytes(int HG, int D, bool fp8) { return stage_bytes_for(HG, D, fp8); }
 
-cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int grid, const void* tmap_k,
+cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, bool fp8, int grid, const void* tmap_k,
                               const void* tmap_v, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
     const CUtensorMap& mk = *reinterpret_cast<const CUtensorMap*>(tmap_k);
     const CUtensorMap& mv = *reinterpret_cast<const CUtensorMap*>(tmap_v);
 #define PKV_CASE(GG, HH, DD) \
-    if (G == GG && HG == HH && D == DD) return launch_one<GG, HH, DD>(p, grid, mk, mv, stream);
+    if (G == GG && HG == HH && D == DD && !fp8) return launch_one<GG, HH, DD, false>(p, grid, mk, mv, stream);
     PKV_CASE(4, 8, 128) PKV_CASE(4, 4, 128) PKV_CASE(4, 2, 128) PKV_CASE(4, 1, 128)
     PKV_CASE(8, 8, 128) PKV_CASE(8, 4, 128) PKV_CASE(8, 2, 128) PKV_CASE(8, 1, 128)
     PKV_CASE(2, 8, 128) PKV_CASE(2, 4, 128) PKV_CASE(2, 2, 128) PKV_CASE(2, 1, 128)
@@ -654,6 +701,12 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int g
     PKV_CASE(4, 4, 256) PKV_CASE(4, 2, 256) PKV_CASE(4, 1, 256)   // d = 256: at most 4 heads per CTA
     PKV_CASE(8, 4, 256) PKV_CASE(8, 2, 256) PKV_CASE(8, 1, 256)   // (a stage of 8 would be 128 KiB)
 #undef PKV_CASE
+#define PKV_CASE8(GG, HH) \
+    if (G == GG && HG == HH && D == 128 && fp8) return launch_one<GG, HH, 128, true>(p, grid, mk, mv, stream);
+    // FP8 (E4M3) caches: d = 128, G = 4 and 8
+    PKV_CASE8(4, 8) PKV_CASE8(4, 4) PKV_CASE8(4, 2) PKV_CASE8(4, 1)
+    PKV_CASE8(8, 8) PKV_CASE8(8, 4) PKV_CASE8(8, 2) PKV_CASE8(8, 1)
+#undef PKV_CASE8
     return cudaErrorInvalidValue;
 }
 

@@ -47,6 +47,8 @@ struct DecodeParams {
     int64_t stride_page, stride_token, stride_head; // elements
     int32_t B, Hq, Hkv, max_pages, tile_tokens, merge_mode;
     int32_t d;                   // head dimension: 64, 128 or 256
+    const float* k_scale;        // FP8 caches: per-KV-head scales [Hkv] or nullptr (= 1)
+    const float* v_scale;
     PlanArgs plan;               // split policy (fused build)
     int64_t tasks_cap;
     int32_t fused_build;         // TMA kernel: 1 = every CTA derives the queue from seq_lens itself
@@ -207,6 +209,12 @@ __device__ __forceinline__ void mma_16816(float (&c)[4], uint32_t a0, uint32_t a
         "{%0, %1, %2, %3};"
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
         : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+// two E4M3 bytes (low 16 bits of x) -> half2, exact
+__device__ __forceinline__ uint32_t cvt_e4m3x2_to_half2(uint32_t x) {
+    uint32_t d;
+    asm("{\n\t.reg .b16 t;\n\tcvt.u16.u32 t, %1;\n\tcvt.rn.f16x2.e4m3x2 %0, t;\n\t}" : "=r"(d) : "r"(x));
+    return d;
 }
 __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
     __half2 h = __floats2half2_rn(lo, hi);
@@ -709,7 +717,8 @@ __device__ __forceinline__ void store_empty_task(const DecodeParams& p, int* fla
 template <int G, int NW, int NWTOT, int GW = G, int D = kD>
 __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<GW, NWTOT, D>& cb, int w0, int wstride,
                                               int row, int orow, int kvh, int split, int n_i, int64_t slot, int gtid,
-                                              int bar_id, int h0 = 0) {
+                                              int bar_id, int h0, float sc, float sc2) {
+    // sc = scale of the raw dot products in cb.m (x = sc * raw), sc2 = sc * log2(e)
     for (int idx = gtid; idx < GW * D; idx += NW * 32) {
         const int hh = idx / D, dd = idx % D;   // head within the group's block; h0 + hh within the KV head
         float M = -INFINITY;
@@ -719,18 +728,18 @@ __device__ __forceinline__ void finalize_task(const DecodeParams& p, CombineBuf<
 #pragma unroll
         for (int i = 0; i < NW; ++i) {
             const int w = w0 + i * wstride;
-            const float wgt = ex2_approx((cb.m[w][hh] - M) * p.scale_log2);  // m = -inf -> 0
+            const float wgt = ex2_approx((cb.m[w][hh] - M) * sc2);  // m = -inf -> 0
             L += wgt * cb.l[w][hh];
             A += wgt * cb.acc[w][hh][dd];
         }
         if (n_i <= 1) {
             const int64_t o = (int64_t)orow * p.Hq + kvh * G + h0 + hh;
             p.out[o * D + dd] = __float2half_rn(A / L);
-            if (p.lse && dd == 0) p.lse[o] = M * p.scale + logf(L);
+            if (p.lse && dd == 0) p.lse[o] = M * sc + logf(L);
         } else {
             p.part_acc[(slot * G + h0 + hh) * D + dd] = A;
             if (dd == 0) {
-                p.part_m[slot * G + h0 + hh] = M * p.scale;
+                p.part_m[slot * G + h0 + hh] = M * sc;
                 p.part_l[slot * G + h0 + hh] = L;
             }
         }
@@ -785,12 +794,12 @@ inline PlanArgs make_plan_args(const pkv_shape& shape, const Resolved& rp) {
 
 // launchers implemented in the .cu files
 cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStream_t stream);
-cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int grid, const void* tmap_k,
+cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, bool fp8, int grid, const void* tmap_k,
                               const void* tmap_v, cudaStream_t stream);
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
                            const int32_t* row_index, QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
                            pkv_task* tasks, int64_t tasks_cap, cudaStream_t stream);
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream);
-int decode_tma_stage_bytes(int HG, int D);
+int decode_tma_stage_bytes(int HG, int D, bool fp8);
 
 }  // namespace pkv

@@ -53,7 +53,9 @@ class Workload:
         return (self.num_pages, self.page_size, self.Hkv, self.d)
 
     def kv_bytes_per_token(self) -> int:
-        return 2 * self.Hkv * self.d * 2
+        """K + V bytes of one token: FP16 caches, or one byte per element with extra["kv_elem_bytes"] = 1
+        (FP8 caches, reading A28)."""
+        return 2 * self.Hkv * self.d * int(self.extra.get("kv_elem_bytes", 2))
 
 
 def _rng(seed: int) -> np.random.Generator:

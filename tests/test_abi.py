@@ -34,7 +34,7 @@ def test_version_and_struct_sizes():
     assert pkv.pkv_version() >> 16 == 2
     assert ctypes.sizeof(binding.pkv_task) == 20            # 5 x int32
     assert ctypes.sizeof(binding.pkv_split_policy) == 44
-    assert ctypes.sizeof(binding.pkv_shape) == 56
+    assert ctypes.sizeof(binding.pkv_shape) == 80
     assert ctypes.sizeof(binding.pkv_counters) == 128
 
 
