@@ -81,6 +81,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-sweep", action="store_true", help="skip the split-count sweep on the tune seed")
     ap.add_argument("--no-others", action="store_true", help="skip config.other_workloads")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-calibrate", action="store_true", help="skip pkv_calibrate (its probe kernels crowd an ncu launch list)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="target CPU time of the oracle sample")
     ap.add_argument("--timeline", default="", help="write a CUPTI kernel timeline of a few replayed steps to this file")
@@ -816,6 +817,8 @@ def run_ours(args):
     # beta / lambda of this device: the read-only streaming probe next to the copy peak
     cal = None
     try:
+        if args.no_calibrate:
+            raise RuntimeError("skipped (--no-calibrate)")
         buf = torch.empty(1 << 30, dtype=torch.uint8, device=device)
         cal = pkv.pkv_calibrate(buf)
         del buf

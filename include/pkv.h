@@ -368,8 +368,12 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
  * pkv_calibrate measures beta and lambda on the device at hand.
  * pkv_choose_policy: evaluates the library's candidate policies for this step -- BALANCED, and
  * FIXED_COUNT with S in {1, 2, 4, ..., 128} on 32-token tiles, all on `base`'s route, merge mode,
- * kernel and flags -- and writes the one with the smallest makespan_total_us to `chosen` (ties:
- * BALANCED first, then the smaller S).  PKV_SPLIT_AUTO in pkv_decode_host does this per step.
+ * kernel and flags -- and writes the winner to `chosen`: among the candidates whose makespan_total_us
+ * is within 1 % of the smallest, the one whose units cover the most SMs (min(units, num_sms); the
+ * model cannot tell such candidates apart, and measured steps favour the fuller machine: config 2,
+ * 147 vs 128 units: 23.4 vs 23.8 us), then the smaller estimate, then FIXED_COUNT before BALANCED (the
+ * same decomposition with the shorter in-kernel plan) and the smaller S.
+ * PKV_SPLIT_AUTO in pkv_decode_host does this per step.
  */
 typedef struct {
     double beta_gbps;  /* streaming read bandwidth                                   (paper: 331.2) */
@@ -383,6 +387,7 @@ typedef struct {
     double cta_work_per_sm;                          /* C_r                                          */
     double makespan_us, makespan_total_us;           /* A27: first term, and the total with it        */
     int64_t kv_bytes, merge_bytes, tasks, launches, max_share_bytes;
+    int64_t units;                                   /* CTA work units of the launch(es): (row, split) pairs x head groups */
 } pkv_cost_estimate;
 PKV_API pkv_status pkv_default_cost_model(int32_t num_sms, pkv_cost_model* out);
 PKV_API pkv_status pkv_estimate_cost(const pkv_shape* shape, const pkv_split_policy* policy,

@@ -73,7 +73,7 @@ class pkv_cost_model(ctypes.Structure):
 class pkv_cost_estimate(ctypes.Structure):
     _fields_ = ([(n, ctypes.c_double) for n in ("total_us", "stream_us", "launch_us", "merge_us", "cta_work_per_sm",
                                                  "makespan_us", "makespan_total_us")]
-                + [(n, _i64) for n in ("kv_bytes", "merge_bytes", "tasks", "launches", "max_share_bytes")])
+                + [(n, _i64) for n in ("kv_bytes", "merge_bytes", "tasks", "launches", "max_share_bytes", "units")])
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

@@ -119,7 +119,9 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     out->G = G;
     out->flags = p.flags;
     out->heads_per_cta = p.heads_per_cta;
-    out->prefetch_kb = p.prefetch_kb == 0 ? kDefaultPrefetchKb : (p.prefetch_kb < 0 ? 0 : p.prefetch_kb);
+    // default: 256 KiB of FP16 K/V per CTA (FP8: 128 KiB -- the same tokens); measured sweeps in DESIGN.md
+    out->prefetch_kb = p.prefetch_kb == 0 ? (s.kv_dtype == PKV_KV_E4M3 ? kDefaultPrefetchKb / 2 : kDefaultPrefetchKb)
+                                          : (p.prefetch_kb < 0 ? 0 : p.prefetch_kb);
     return PKV_OK;
 }
 
@@ -232,7 +234,7 @@ namespace {
 // Totals of one launch pair (policy resolved, lengths on the host) for the cost model.
 struct RouteTotals {
     int64_t kv_bytes = 0, merge_bytes = 0, tasks = 0, launches = 0;
-    int64_t max_share = 0;
+    int64_t max_share = 0, units = 0;
     double slice_eff = 1.0;   // A27: head_slice_efficiency of the launch's heads per CTA
 };
 
@@ -252,6 +254,7 @@ void launch_totals(const pkv_shape& s, const Resolved& rp, const int32_t* lens, 
         const int64_t unit = (int64_t)max_tok * 2 * hg * s.d * (s.kv_dtype == PKV_KV_E4M3 ? 1 : 2);
         const int64_t units = (int64_t)hdr.total_row_slots * (s.Hkv / hg);
         t->max_share = units <= num_sms ? unit : t->kv_bytes / num_sms + unit;
+        t->units = units;
         t->slice_eff = head_slice_efficiency(hg);
     }
 }
@@ -396,6 +399,7 @@ pkv_status pkv_estimate_cost(const pkv_shape* shape, const pkv_split_policy* pol
             RouteTotals t;
             launch_totals(sub, rb, lens.data(), model->num_sms, &t);
             sum.kv_bytes += t.kv_bytes; sum.merge_bytes += t.merge_bytes; sum.tasks += t.tasks; sum.launches += t.launches;
+            sum.units += t.units;
             if (t.max_share > sum.max_share) sum.max_share = t.max_share;
             const double a = (double)t.kv_bytes / (beta * t.slice_eff), c = (double)t.max_share / beta_cta;
             makespan += a > c ? a : c;
@@ -413,6 +417,7 @@ pkv_status pkv_estimate_cost(const pkv_shape* shape, const pkv_split_policy* pol
     out->makespan_total_us = makespan + out->launch_us + out->merge_us;
     out->kv_bytes = sum.kv_bytes; out->merge_bytes = sum.merge_bytes; out->tasks = sum.tasks; out->launches = sum.launches;
     out->max_share_bytes = sum.max_share;
+    out->units = sum.units;
     return PKV_OK;
 }
 
@@ -420,9 +425,9 @@ pkv_status pkv_choose_policy(const pkv_shape* shape, const int32_t* seq_lens_hos
                              const pkv_split_policy* base, pkv_split_policy* chosen, pkv_cost_estimate* estimate_out) {
     clear_error();
     if (!base || !chosen || !model) { set_error("pkv_choose_policy: null argument"); return PKV_ERR_INVALID_ARG; }
-    pkv_split_policy best = *base;
-    pkv_cost_estimate best_est;
-    bool have = false;
+    pkv_split_policy cand[10];
+    pkv_cost_estimate est[10];
+    int n = 0;
     // candidates: BALANCED on page-size tiles, then FIXED_COUNT S = 1, 2, 4, ..., 128 and the
     // single-wave fit S = floor(SMs / (B * head groups)) on 32-token tiles
     const int sms = base->num_sms > 0 ? base->num_sms : model->num_sms;
@@ -447,15 +452,27 @@ pkv_status pkv_choose_policy(const pkv_shape* shape, const int32_t* seq_lens_hos
             pol.tile_tokens = 32;
             pol.num_splits = c == 8 ? s_fit : 1 << c;
         }
-        pkv_cost_estimate e;
-        const pkv_status st = pkv_estimate_cost(shape, &pol, seq_lens_host, 0, model, &e);
+        const pkv_status st = pkv_estimate_cost(shape, &pol, seq_lens_host, 0, model, &est[n]);
         if (st != PKV_OK) return st;
-        if (!have || e.makespan_total_us < best_est.makespan_total_us) {
-            have = true;
-            best = pol;
-            best_est = e;
-        }
+        cand[n++] = pol;
     }
+    int lo = 0;
+    for (int i = 1; i < n; ++i)
+        if (est[i].makespan_total_us < est[lo].makespan_total_us) lo = i;
+    auto coverage = [&](int i) { return est[i].units < sms ? est[i].units : (int64_t)sms; };
+    int pick = lo;
+    for (int i = 0; i < n; ++i) {
+        if (est[i].makespan_total_us > 1.01 * est[lo].makespan_total_us) continue;
+        // equal coverage and estimate (the same decomposition): FIXED_COUNT, whose in-kernel plan is
+        // shorter than BALANCED's (config 2: 23.4 vs 23.8 us per step)
+        const bool better_tie = coverage(i) == coverage(pick) && est[i].makespan_total_us == est[pick].makespan_total_us &&
+                                cand[pick].split_mode == PKV_SPLIT_BALANCED && cand[i].split_mode == PKV_SPLIT_FIXED_COUNT;
+        if (coverage(i) > coverage(pick) || (coverage(i) == coverage(pick) && est[i].makespan_total_us < est[pick].makespan_total_us) ||
+            better_tie)
+            pick = i;
+    }
+    pkv_split_policy best = cand[pick];
+    const pkv_cost_estimate best_est = est[pick];
     best.num_sms = base->num_sms;   // 0 stays "the device's": the estimate assumed the model's machine
     *chosen = best;
     if (estimate_out) *estimate_out = best_est;
