@@ -307,3 +307,69 @@ def test_fp8_attention_reduces_to_the_fp16_oracle_and_to_brute_force():
     # swapping the scales changes the result (the test can see them)
     bad, _ = pkv_oracle.attention_fp8(p.q, k8, v8, vs2, ks2, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
     assert np.abs(bad - ref).max() > 1e-3
+
+
+# ---------------------------------------------------------------- fused KV-append + RoPE, reading A29
+
+def _rope_tables(positions, d, base=10000.0):
+    inv = base ** (-np.arange(0, d // 2, dtype=np.float64) * 2.0 / d)
+    ang = np.arange(positions, dtype=np.float64)[:, None] * inv[None, :]
+    return np.cos(ang).astype(np.float32), np.sin(ang).astype(np.float32)
+
+
+def test_rope_rotation_against_complex_multiplication_and_invariants():
+    """The rotate-half formula restated as a complex product (x[c] + i x[c+d/2]) * e^{i theta}; pair
+    norms are preserved; position 0 is the identity; scores depend on the position difference only."""
+    from oracle import append_oracle as ao
+    rng = np.random.Generator(np.random.PCG64(3))
+    d = 128
+    cos, sin = _rope_tables(5000, d)
+    x = rng.standard_normal((7, d)).astype(np.float16)
+    for pos in (0, 1, 17, 4999):
+        y = ao.rope_rotate_f16(x, cos[pos], sin[pos]).astype(np.float64)
+        z = (x[:, :64].astype(np.float64) + 1j * x[:, 64:].astype(np.float64)) * (cos[pos].astype(np.float64) + 1j * sin[pos].astype(np.float64))
+        want = np.concatenate([z.real, z.imag], axis=-1)
+        assert np.abs(y - want).max() <= 4e-3          # FP16 rounding of values up to ~4
+        n_in = x[:, :64].astype(np.float64) ** 2 + x[:, 64:].astype(np.float64) ** 2
+        assert np.abs((y[:, :64] ** 2 + y[:, 64:] ** 2) - n_in).max() <= 3e-2
+    assert np.array_equal(ao.rope_rotate_f16(x, cos[0], sin[0]), x)
+    # relative position: <R(q, m), R(k, n)> = <R(q, m + s), R(k, n + s)>
+    q, k = x[0:1], x[1:2]
+    a = (ao.rope_rotate_f16(q, cos[40], sin[40]).astype(np.float64) * ao.rope_rotate_f16(k, cos[25], sin[25]).astype(np.float64)).sum()
+    b = (ao.rope_rotate_f16(q, cos[1040], sin[1040]).astype(np.float64) * ao.rope_rotate_f16(k, cos[1025], sin[1025]).astype(np.float64)).sum()
+    assert abs(a - b) <= 5e-2
+
+
+def test_append_step_against_dense_brute_force():
+    """The fused step against numpy on a dense gathered copy: old tokens from the cache, the new
+    token from (RoPE'd) k_new / v_new, q RoPE'd -- no cache-update code involved.  Also: only the slots
+    of the new tokens change, rows with N = 0 change nothing, no tables = plain append."""
+    from oracle import append_oracle as ao
+    lens = np.array([1, 17, 100, 0, 33, 64], dtype=np.int32)
+    p = make_problem(list(lens), seed=71)
+    rng = np.random.Generator(np.random.PCG64(5))
+    k_new = rng.standard_normal((p.B, 8, 128)).astype(np.float16)
+    v_new = rng.standard_normal((p.B, 8, 128)).astype(np.float16)
+    cos, sin = _rope_tables(256, 128)
+    for tables in ((cos, sin), (None, None)):
+        out, lse, k2, v2 = ao.append_and_attend(p.q, p.k_cache, p.v_cache, k_new, v_new, p.block_table, lens, tables[0], tables[1],
+                                                 Hkv=8, page_size=16, scale=p.scale)
+        changed = np.zeros(p.k_cache.shape[:2], dtype=bool)
+        for i in range(p.B):
+            N = int(lens[i])
+            if N == 0:
+                assert np.all(out[i] == 0) and np.all(np.isneginf(lse[i]))
+                continue
+            pos = N - 1
+            kn = ao.rope_rotate_f16(k_new[i], cos[pos], sin[pos]) if tables[0] is not None else k_new[i]
+            qn = ao.rope_rotate_f16(p.q[i], cos[pos], sin[pos]) if tables[0] is not None else p.q[i]
+            Kd = np.stack([p.k_cache[p.block_table[i, j // 16], j % 16] for j in range(N - 1)] + [kn]).astype(np.float64)
+            Vd = np.stack([p.v_cache[p.block_table[i, j // 16], j % 16] for j in range(N - 1)] + [v_new[i]]).astype(np.float64)
+            for h in range(32):
+                x = (Kd[:, h // 4, :] @ qn[h].astype(np.float64)) * p.scale
+                w = np.exp(x - x.max())
+                assert np.abs(out[i, h] - (w[:, None] * Vd[:, h // 4, :]).sum(0) / w.sum()).max() <= 1e-12
+            changed[p.block_table[i, pos // 16], pos % 16] = True
+            assert np.array_equal(k2[p.block_table[i, pos // 16], pos % 16], kn)
+            assert np.array_equal(v2[p.block_table[i, pos // 16], pos % 16], v_new[i])
+        assert np.array_equal(k2[~changed], p.k_cache[~changed]) and np.array_equal(v2[~changed], p.v_cache[~changed])
