@@ -38,6 +38,7 @@ import dataclasses
 import json
 import math
 import os
+import re
 import subprocess
 import sys
 import threading
@@ -634,7 +635,8 @@ def write_timeline(torch, pkv, runner, path, steps=6):
         for i, e in enumerate(evs):
             s, d = e.time_range.start - t0, e.time_range.end - e.time_range.start
             gap = "" if prev_end is None else "%10.2f" % (e.time_range.start - prev_end)
-            lines.append("%-4d %-34s %10.2f %10.2f %10s" % (i, e.name.split("<")[0].split("(")[0][-34:], s, d, gap))
+            m = re.search(r"pkv_\w+", e.name)
+            lines.append("%-4d %-34s %10.2f %10.2f %10s" % (i, m.group(0) if m else e.name[:34], s, d, gap))
             prev_end = e.time_range.end
         n = len(evs) // 2
         span = evs[-1].time_range.end - evs[n].time_range.start
@@ -679,7 +681,7 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
                 cur = name
             pol = pol or auto
             w = runner.w
-            K = max(w.steps, 1)
+            K = w.steps if w.steps > 0 else 2 * args.graph_steps      # config 2 has no trace: 200 replayed steps
             chunk = max(1, min(args.graph_steps, K))
             bucketed = "buckets" in key
             runner.set_bucket_route(1 if bucketed else None)

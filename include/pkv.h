@@ -271,6 +271,36 @@ PKV_API pkv_status pkv_decode_indexed(const pkv_shape* shape, const pkv_split_po
                                       float scale, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * Fused KV-append (+RoPE) before decode ("fused RoPE/KV-cache writes", future work there;
+ * DESIGN.md reading A29).  seq_lens[i] = N_i already counts the new token; its position is N_i - 1.
+ * In ONE decode launch: q is rotated to that position in registers (q itself is not modified); the
+ * task that owns token N_i - 1 takes that token's K (rotated) and V from k_new / v_new instead of the
+ * pool -- patched into its shared-memory stage, so there is no write -> read dependency through the
+ * cache -- and writes both to the pool slot of token N_i - 1 (page block_table[i][(N_i-1)/P]) for
+ * later steps.  k_cache / v_cache are therefore WRITTEN by this call.  Rows with N_i = 0 append nothing.
+ *   k_new, v_new   dev [rows, Hkv, d] f16, indexed like q (by request row)
+ *   rope_cos/_sin  dev float [rope_positions, d/2]: cos / sin of position * theta_c, rotate-half
+ *                  pairing (channel c < d/2 with c + d/2); both NULL = no rotation.  The rotation is
+ *                  evaluated in FP32 product by product (no FMA) and rounded to FP16, so the bytes in
+ *                  the pool are reproducible by a plain CPU restatement.
+ * TMA kernel, FP16 caches, G <= 8 only (else PKV_ERR_UNSUPPORTED).  Otherwise as pkv_decode with
+ * build_queue = 1; row_index may be NULL.
+ */
+typedef struct {
+    const void* k_new;
+    const void* v_new;
+    const float* rope_cos;
+    const float* rope_sin;
+    int32_t rope_positions; /* rows of the tables; positions >= this are not rotated */
+    int32_t reserved_;
+} pkv_append;
+PKV_API pkv_status pkv_decode_append(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                                     void* k_cache, void* v_cache, const int32_t* block_table,
+                                     const int32_t* seq_lens, const int32_t* row_index, const pkv_append* append,
+                                     void* out, float* lse, float scale, void* workspace,
+                                     size_t workspace_bytes, void* stream);
+
+/*
  * Length-bucket route ("one per route length"; DESIGN.md readings
  * A22, A23) -- the route the compact workqueue replaces, kept as its comparator (Table 4: 16.00 vs
  * 2.00 launches per step).

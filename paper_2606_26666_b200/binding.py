@@ -79,12 +79,16 @@ class pkv_cost_estimate(ctypes.Structure):
         return {n: getattr(self, n) for n, _ in self._fields_}
 
 
+class pkv_append(ctypes.Structure):
+    _fields_ = [("k_new", _vp), ("v_new", _vp), ("rope_cos", _vp), ("rope_sin", _vp), ("rope_positions", _i32), ("reserved_", _i32)]
+
+
 # every symbol include/pkv.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspace_init_bytes", "pkv_build_workqueue_host",
            "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
            "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate", "pkv_decode_indexed",
            "pkv_plan_buckets_host", "pkv_decode_buckets", "pkv_bucket_counters_host", "pkv_default_cost_model",
-           "pkv_estimate_cost", "pkv_choose_policy")
+           "pkv_estimate_cost", "pkv_choose_policy", "pkv_decode_append")
 
 
 class PkvError(RuntimeError):
@@ -134,6 +138,9 @@ def _load() -> ctypes.CDLL:
     lib.pkv_choose_policy.restype = _i32
     lib.pkv_choose_policy.argtypes = [P(pkv_shape), _vp, P(pkv_cost_model), P(pkv_split_policy), P(pkv_split_policy),
                                       P(pkv_cost_estimate)]
+    lib.pkv_decode_append.restype = _i32
+    lib.pkv_decode_append.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, P(pkv_append), _vp, _vp,
+                                      ctypes.c_float, _vp, ctypes.c_size_t, _vp]
     lib.pkv_merge.restype = _i32
     lib.pkv_merge.argtypes = [P(pkv_shape), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.pkv_get_counters.restype = _i32
@@ -363,6 +370,26 @@ def pkv_choose_policy(shape: Shape, seq_lens_host: np.ndarray, model: CostModel,
     _check(_lib.pkv_choose_policy(ctypes.byref(shape.c()), _ptr(seq), ctypes.byref(model.c()), ctypes.byref(base.c()),
                                   ctypes.byref(out), ctypes.byref(e)))
     return Policy(**{n: int(getattr(out, n)) for n, _ in pkv_split_policy._fields_}), e.as_dict()
+
+
+@dataclass
+class Append:
+    """The new token of every row for pkv_decode_append: device tensors (or raw addresses)."""
+    k_new: object
+    v_new: object
+    rope_cos: object = None
+    rope_sin: object = None
+    rope_positions: int = 0
+
+    def c(self) -> pkv_append:
+        return pkv_append(_ptr(self.k_new), _ptr(self.v_new), _ptr(self.rope_cos), _ptr(self.rope_sin), int(self.rope_positions), 0)
+
+
+def pkv_decode_append(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, seq_lens, row_index, append: Append, out,
+                      lse=None, scale: float = 0.0, workspace=None, stream=None) -> None:
+    _check(_lib.pkv_decode_append(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(q), _ptr(k_cache), _ptr(v_cache),
+                                  _ptr(block_table), _ptr(seq_lens), _ptr(row_index), ctypes.byref(append.c()), _ptr(out),
+                                  _ptr(lse), ctypes.c_float(scale), _ptr(workspace), _nbytes(workspace), _stream_ptr(stream)))
 
 
 def pkv_merge(shape: Shape, part_m, part_l, part_acc, split_offsets, out, lse=None, stream=None) -> None:

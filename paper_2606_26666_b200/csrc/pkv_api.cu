@@ -163,6 +163,7 @@ pkv_status check_workspace(const void* workspace, size_t bytes, const WorkspaceL
 // so launches that have nothing to do are skipped (A13).
 pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, const void* k_cache, const void* v_cache,
                       const int32_t* block_table, const int32_t* seq_lens, const int32_t* row_index, void* out, float* lse, float scale,
+                      const pkv_append* append,
                       const QueuePtrs& qp, const WsPtrs& ws, int64_t known_tasks, int known_max_n, int64_t known_slots,
                       int num_sms, uint32_t stages, bool fused_build, int64_t tasks_cap,
                       cudaStream_t stream, int* decode_launches, int* merge_launches) {
@@ -186,6 +187,13 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
     p.stride_page = st.page; p.stride_token = st.token; p.stride_head = st.head;
     p.B = s.B; p.Hq = s.Hq; p.Hkv = s.Hkv; p.max_pages = s.max_pages; p.d = s.d;
     p.k_scale = s.k_scale; p.v_scale = s.v_scale;
+    if (append) {
+        p.k_new = static_cast<const __half*>(append->k_new);
+        p.v_new = static_cast<const __half*>(append->v_new);
+        p.rope_cos = append->rope_cos;
+        p.rope_sin = append->rope_sin;
+        p.rope_positions = append->rope_positions;
+    }
     p.tile_tokens = rp.tile_tokens; p.merge_mode = rp.merge_mode;
     p.dynamic_sched = 1;
     p.force_replan = (rp.flags & PKV_FLAG_TEST_REPLAN) ? 1 : 0;
@@ -318,7 +326,7 @@ pkv_status decode_stages(const pkv_shape* shape, const pkv_split_policy* policy,
                              const void* k_cache, const void* v_cache, const int32_t* block_table,
                              const int32_t* seq_lens, const int32_t* row_index, void* out, float* lse, float scale,
                              uint32_t stages, void* workspace, size_t workspace_bytes, void* stream,
-                             const pkv_shape* layout_shape = nullptr) {
+                             const pkv_shape* layout_shape = nullptr, const pkv_append* append = nullptr) {
     // layout_shape: the shape the workspace is carved for (pkv_decode_buckets: the whole batch, so
     // that the header and the completion counters sit at the same place for every bucket)
     clear_error();
@@ -344,8 +352,19 @@ pkv_status decode_stages(const pkv_shape* shape, const pkv_split_policy* policy,
                                              ws.q.rowslots, ws.q.tasks, L.slots_cap, cs);
         if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     }
-    return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, row_index, out, lse, scale, ws.q, ws, -1, -1, -1, sms,
-                      stages, fused, L.slots_cap, cs, nullptr, nullptr);
+    if (append) {
+        if (!append->k_new || !append->v_new || (append->rope_cos == nullptr) != (append->rope_sin == nullptr) ||
+            (append->rope_cos && append->rope_positions <= 0)) {
+            set_error("pkv_decode_append: k_new / v_new null, or only one RoPE table, or rope_positions <= 0");
+            return PKV_ERR_INVALID_ARG;
+        }
+        if (rp.kernel != PKV_KERNEL_TMA_MMA || shape->kv_dtype != PKV_KV_F16 || rp.G > 8) {
+            set_error("pkv_decode_append needs the TMA kernel, FP16 caches and G <= 8");
+            return PKV_ERR_UNSUPPORTED;
+        }
+    }
+    return run_decode(*shape, rp, q, k_cache, v_cache, block_table, seq_lens, row_index, out, lse, scale, append, ws.q, ws, -1, -1,
+                      -1, sms, stages, fused, L.slots_cap, cs, nullptr, nullptr);
 }
 
 }  // namespace
@@ -376,6 +395,24 @@ pkv_status pkv_decode_indexed(const pkv_shape* shape, const pkv_split_policy* po
     }
     return decode_stages(shape, policy, q, k_cache, v_cache, block_table, seq_lens, row_index, out, lse, scale,
                          PKV_STAGE_ALL, workspace, workspace_bytes, stream);
+}
+
+pkv_status pkv_decode_append(const pkv_shape* shape, const pkv_split_policy* policy, const void* q, void* k_cache,
+                             void* v_cache, const int32_t* block_table, const int32_t* seq_lens, const int32_t* row_index,
+                             const pkv_append* append, void* out, float* lse, float scale, void* workspace,
+                             size_t workspace_bytes, void* stream) {
+    if (!append) {
+        clear_error();
+        set_error("pkv_decode_append: null append");
+        return PKV_ERR_INVALID_ARG;
+    }
+    if (row_index && shape && shape->B > kMaxFusedRows) {
+        clear_error();
+        set_error("pkv_decode_append: at most %d indexed rows per launch", kMaxFusedRows);
+        return PKV_ERR_UNSUPPORTED;
+    }
+    return decode_stages(shape, policy, q, k_cache, v_cache, block_table, seq_lens, row_index, out, lse, scale, PKV_STAGE_ALL,
+                         workspace, workspace_bytes, stream, nullptr, append);
 }
 
 pkv_status pkv_decode_buckets(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
@@ -748,7 +785,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         if (e != cudaSuccess) return cuda_fail(e, "builder launch");
     }
     st = run_decode(s, rp, q_dev, k_cache_dev, v_cache_dev, reinterpret_cast<const int32_t*>(ds + im.block_table),
-                    lens_dev, nullptr, out_dev, nullptr, scale, ws.q, ws, hdr->num_tasks, hdr->max_row_splits,
+                    lens_dev, nullptr, out_dev, nullptr, scale, nullptr, ws.q, ws, hdr->num_tasks, hdr->max_row_splits,
                     hdr->total_row_slots, sms, PKV_STAGE_ALL, fused, L.slots_cap, cs, &dl, &ml);
     if (st != PKV_OK) return st;
     const size_t out_bytes = 2 * (size_t)s.B * s.Hq * s.d;

@@ -54,7 +54,7 @@ struct RowSlot {
     int32_t tok0;   // token range [tok0, tok1) -- empty when tok0 >= tok1
     int32_t tok1;
     int32_t grow;   // request row (= row unless the launch is indexed, pkv_decode_indexed)
-    int32_t pad_;
+    int32_t nlen;   // the row's length N_i (the fused KV-append needs the position of its last token)
 };
 static_assert(sizeof(RowSlot) == 32, "RowSlot layout");
 

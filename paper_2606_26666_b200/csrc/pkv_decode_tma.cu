@@ -54,6 +54,7 @@ struct UnitInfo {
     int unit;   // -1: no more work
     int row, so, n, split, tok0, tok1;   // the unit's RowSlot
     int grow;   // request row: the row of q, out, lse and block_table (= row unless the launch is indexed)
+    int nlen;   // the row's length N_i
 };
 
 template <int G, int D>
@@ -90,6 +91,46 @@ __host__ __device__ constexpr int stages_for() {
     // Stage s always belongs to producer s % NP and, per head, to compute warp s % WPH (see the
     // kernel): any stage count works, the shares differ by at most one stage.
     return n > kMaxStages ? kMaxStages : n;
+}
+
+// Fused KV-append (reading A29): row `orow`'s new token (position pos, row `r` = pos % 16 of
+// its 16-token block) for KV head kvh.  One warp: lane pairs channels (c, c+1) with (c + D/2, c + D/2 + 1),
+// rotates K in FP32 (product by product, as the oracle), and stores the FP16 result both into the
+// head's block of the shared-memory stage `sb` (128-byte swizzled rows of 64 channels) and into the
+// pool at the token's slot.  V is copied unrotated.
+template <int D, bool IS_K>
+__device__ __forceinline__ void append_patch(const DecodeParams& p, uint32_t sb, int orow, int kvh, int pos, int r, int lane,
+                                             int page_shift) {
+    const __half* src = (IS_K ? p.k_new : p.v_new) + ((int64_t)orow * p.Hkv + kvh) * D;
+    __half* pool = const_cast<__half*>(IS_K ? p.k_cache : p.v_cache);
+    const int psz = 16 << page_shift;
+    const int64_t page = __ldg(p.block_table + (int64_t)orow * p.max_pages + (pos >> (4 + page_shift)));
+    __half* dst = pool + page * p.stride_page + (int64_t)(pos & (psz - 1)) * p.stride_token + (int64_t)kvh * p.stride_head;
+    const bool rot = IS_K && p.rope_cos != nullptr && pos < p.rope_positions;
+    for (int c = lane * 2; c < D / 2; c += 64) {
+        __half2 lo = *reinterpret_cast<const __half2*>(src + c);
+        __half2 hi = *reinterpret_cast<const __half2*>(src + c + D / 2);
+        if (rot) {
+            const float2 cs2 = __ldg(reinterpret_cast<const float2*>(p.rope_cos + (int64_t)pos * (D / 2) + c));
+            const float2 sn2 = __ldg(reinterpret_cast<const float2*>(p.rope_sin + (int64_t)pos * (D / 2) + c));
+            const float2 x1 = __half22float2(lo), x2 = __half22float2(hi);
+            lo = __floats2half2_rn(__fsub_rn(__fmul_rn(x1.x, cs2.x), __fmul_rn(x2.x, sn2.x)),
+                                   __fsub_rn(__fmul_rn(x1.y, cs2.y), __fmul_rn(x2.y, sn2.y)));
+            hi = __floats2half2_rn(__fadd_rn(__fmul_rn(x2.x, cs2.x), __fmul_rn(x1.x, sn2.x)),
+                                   __fadd_rn(__fmul_rn(x2.y, cs2.y), __fmul_rn(x1.y, sn2.y)));
+        }
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+            const int ch = c + hf * (D / 2);
+            const __half2 val = hf ? hi : lo;
+            // stage: 64-channel block ch / 64, row r, 16-byte chunk ((ch % 64) / 8) ^ (r % 8), byte (ch % 8) * 2
+            const uint32_t a = sb + (ch >> 6) * 2048 + r * 128 + (((((ch & 63) >> 3) ^ (r & 7))) << 4) + (ch & 7) * 2;
+            sts_b32(a, *reinterpret_cast<const uint32_t*>(&val));
+            *reinterpret_cast<__half2*>(dst + ch) = val;
+        }
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the stage is refilled by the async proxy later
+    __syncwarp();
 }
 
 template <int G, int HG, int D, bool FP8>
@@ -297,14 +338,14 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 if (t >= 0 && k == 0) d = tail.first_slot;   // computed by the planner warp
                 else if (t >= 0) d = make_rowslot(plan, tail.so_s, tail.len_s, t / HGn, &tb, &te);
                 u.row = d.row; u.so = d.so; u.n = d.n; u.split = d.split; u.tok0 = d.tok0; u.tok1 = d.tok1;
-                u.grow = d.grow;
+                u.grow = d.grow; u.nlen = d.nlen;
             } else {
                 const int4* rsp = reinterpret_cast<const int4*>(p.rowslots + (k == 0 ? t / HGn : min(t, max(num_units - 1, 0)) / HGn));
                 const int4 a = __ldcg(rsp);
                 const int4 b = __ldcg(rsp + 1);
                 if (k == 0) num_units = __ldcg(&p.hdr->total_row_slots) * HGn;
                 if (t >= num_units) t = -1;
-                u.row = a.x; u.so = a.y; u.n = a.z; u.split = a.w; u.tok0 = b.x; u.tok1 = b.y; u.grow = b.z;
+                u.row = a.x; u.so = a.y; u.n = a.z; u.split = a.w; u.tok0 = b.x; u.tok1 = b.y; u.grow = b.z; u.nlen = b.w;
             }
             u.unit = t;
             if (lane == 0) {
@@ -320,7 +361,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 // The slot is released only after its loads have RETURNED: the store below needs
                 // every field (an mbarrier arrive may otherwise overtake loads still in flight).
                 sts_b32(smem_u32(&tail.sink_i[warp]),
-                        (uint32_t)(u.unit + u.row + u.so + u.n + u.split + u.tok0 + u.tok1 + u.grow));
+                        (uint32_t)(u.unit + u.row + u.so + u.n + u.split + u.tok0 + u.tok1 + u.grow + u.nlen));
                 mbar_arrive(rempty0 + 8 * r);
             }
         }
@@ -441,6 +482,40 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     qb[kk][1] = g4 < GW ? hi : 0u;
                 }
             }
+            // Fused KV-append (+RoPE) (reading A29): q is rotated to the new token's position
+            // N - 1 in registers -- the rotate-half partner of channel c < d/2 is channel c + d/2, i.e.
+            // the same fragment slot of k-step kk + KK/2 -- in FP32, product by product, as the oracle.
+            bool patch = false;
+            int last_blk = -1, last_row = 0;
+            if constexpr (!FP8 && NBK == 1) {
+                if (p.k_new != nullptr) {
+                    const int pos = u.nlen - 1;
+                    patch = tok1 == u.nlen;            // this unit's range ends with the row's new token
+                    last_blk = pos >> 4;
+                    last_row = pos & 15;
+                    if (p.rope_cos != nullptr && pos < p.rope_positions) {
+                        const float* cr = p.rope_cos + (int64_t)pos * (D / 2);
+                        const float* sr = p.rope_sin + (int64_t)pos * (D / 2);
+#pragma unroll
+                        for (int kk = 0; kk < KK / 2; ++kk) {
+#pragma unroll
+                            for (int hf = 0; hf < 2; ++hf) {
+                                const int c = kk * 16 + 2 * t4 + 8 * hf;     // channels c, c+1 (< d/2)
+                                const float2 cs2 = __ldg(reinterpret_cast<const float2*>(cr + c));
+                                const float2 sn2 = __ldg(reinterpret_cast<const float2*>(sr + c));
+                                const float2 x1 = __half22float2(*reinterpret_cast<const __half2*>(&qb[kk][hf]));
+                                const float2 x2 = __half22float2(*reinterpret_cast<const __half2*>(&qb[kk + KK / 2][hf]));
+                                const float y1x = __fsub_rn(__fmul_rn(x1.x, cs2.x), __fmul_rn(x2.x, sn2.x));
+                                const float y1y = __fsub_rn(__fmul_rn(x1.y, cs2.y), __fmul_rn(x2.y, sn2.y));
+                                const float y2x = __fadd_rn(__fmul_rn(x2.x, cs2.x), __fmul_rn(x1.x, sn2.x));
+                                const float y2y = __fadd_rn(__fmul_rn(x2.y, cs2.y), __fmul_rn(x1.y, sn2.y));
+                                qb[kk][hf] = pack_half2(y1x, y1y);
+                                qb[kk + KK / 2][hf] = pack_half2(y2x, y2y);
+                            }
+                        }
+                    }
+                }
+            }
             float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
             float o[KK][4];
 #pragma unroll
@@ -469,6 +544,12 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 mbar_wait(fullk0 + 8 * s, par);
                 if (k == 0 && first_page && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 4);
                 first_page = false;
+                if constexpr (!FP8 && NBK == 1) {
+                    // the block that holds the row's new token: its K row comes from k_new (rotated), not
+                    // from the pool -- patched into the stage here and written to the pool for later steps
+                    if (patch && p0 + j == last_blk)
+                        append_patch<D, true>(p, kb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                }
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
                 if constexpr (FP8) {
                     // one ldmatrix.x4 = 16 tokens x 32 channels of bytes: (tok 0-7 | 8-15) x (chunk 2j | 2j+1)
@@ -533,6 +614,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
 
                 // ---- O^T += V^T . P^T
                 mbar_wait(fullv0 + 8 * s, par);
+                if constexpr (!FP8 && NBK == 1) {
+                    if (patch && p0 + j == last_blk)
+                        append_patch<D, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                }
                 uint32_t vdep = 0;   // a word of every V fragment (see the stage release below)
                 if constexpr (FP8) {
                     // ldmatrix.trans moves 16-bit units, i.e. PAIRS of channels: a lane gets tokens

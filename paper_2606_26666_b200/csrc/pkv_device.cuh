@@ -49,6 +49,12 @@ struct DecodeParams {
     int32_t d;                   // head dimension: 64, 128 or 256
     const float* k_scale;        // FP8 caches: per-KV-head scales [Hkv] or nullptr (= 1)
     const float* v_scale;
+    // fused KV-append (+RoPE) before decode (pkv_decode_append; reading A29), or nullptr
+    const __half* k_new;         // [rows, Hkv, d]: the new token's K (before RoPE), by request row
+    const __half* v_new;         // [rows, Hkv, d]
+    const float* rope_cos;       // [rope_positions, d/2] or nullptr (no rotation)
+    const float* rope_sin;
+    int32_t rope_positions;
     PlanArgs plan;               // split policy (fused build)
     int64_t tasks_cap;
     int32_t fused_build;         // TMA kernel: 1 = every CTA derives the queue from seq_lens itself
@@ -455,7 +461,7 @@ __device__ __forceinline__ int32_t plan_warp_prefix(PlanArgs& a, const int32_t* 
                 d.tok0 = tb * a.tile_tokens;
                 d.tok1 = min(te * a.tile_tokens, N);
                 d.grow = !a.row_index ? i : (SPEC ? ld_relaxed_s32(a.row_index + i) : __ldcg(a.row_index + i));
-                d.pad_ = 0;
+                d.nlen = N;
                 *first = d;
             }
         }
@@ -528,7 +534,7 @@ __device__ __forceinline__ RowSlot make_rowslot(const PlanArgs& a, const int32_t
     d.tok0 = tb * a.tile_tokens;
     d.tok1 = min(te * a.tile_tokens, N);
     d.grow = request_row(a.row_index, lo);
-    d.pad_ = 0;
+    d.nlen = N;
     *t_begin = tb;
     *t_end = te;
     return d;

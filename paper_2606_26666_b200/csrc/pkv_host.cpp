@@ -201,7 +201,7 @@ pkv_status plan_host(const pkv_shape& s, const Resolved& rp, const int32_t* seq_
             for (int32_t sp = 0; sp < slots; ++sp) {
                 RowSlot rs;
                 std::memset(&rs, 0, sizeof(rs));
-                rs.row = i; rs.so = off; rs.n = slots; rs.split = sp; rs.grow = i;
+                rs.row = i; rs.so = off; rs.n = slots; rs.split = sp; rs.grow = i; rs.nlen = N;
                 if (r.T > 0) {
                     const int64_t b = (int64_t)sp * r.c, e = (int64_t)(sp + 1) * r.c;
                     const int64_t t0 = (b < r.T ? b : r.T) * rp.tile_tokens, t1 = (e < r.T ? e : r.T) * rp.tile_tokens;
