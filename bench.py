@@ -55,7 +55,8 @@ import pkv_inputs  # noqa: E402  (seeded input generators; no attention arithmet
 L2_BYTES = 126 * 1000 * 1000
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
 MIN_TIMED_MS = 50.0                # the K-step region is repeated until this much has been timed
-WORKLOADS = ["config1", "config2", "config3", "config4", "config4_b4", "config5", "config5_hkv4", "config2_fp8", "config3_fp8"]
+WORKLOADS = ["config1", "config2", "config3", "config4", "config4_b4", "config5", "config5_hkv4", "config2_fp8", "config3_fp8",
+             "config2_append", "config3_append"]
 FP8_SCALE = 1.0 / 32.0      # per-KV-head scale of the FP8 workloads: N(0,1) / scale stays far inside +-448
 
 
@@ -98,6 +99,11 @@ def make_workload(name: str, seed: int, hkv: int = 0):
         w = make_workload(name[:-4], seed, hkv)
         w.name += "_fp8"
         w.extra["kv_elem_bytes"] = 1
+        return w
+    if name.endswith("_append"):        # the same trace with the fused KV-append + RoPE step
+        w = make_workload(name[:-7], seed, hkv)
+        w.name += "_append"
+        w.extra["append"] = True
         return w
     if name == "config1":
         return pkv_inputs.config1(seed)
@@ -205,6 +211,17 @@ class Runner:
         self.out = torch.zeros((w.B, w.Hq, w.d), dtype=torch.float16, device=device)
         self.stream = torch.cuda.Stream(device=device)
         self.buckets = None
+        self.append = None
+        if w.extra.get("append"):
+            # the new token of every row (the same draw every step) and the RoPE tables of a serving engine
+            npos = int(lens_all.max()) + 1
+            inv = 10000.0 ** (-np.arange(0, w.d // 2, dtype=np.float64) * 2.0 / w.d)
+            ang = np.arange(npos, dtype=np.float64)[:, None] * inv[None, :]
+            self.rope_host = (np.cos(ang).astype(np.float32), np.sin(ang).astype(np.float32))
+            self.knew = pkv_inputs.fill_pool_torch((w.B, w.Hkv, w.d), seed * 100 + 91, device)
+            self.vnew = pkv_inputs.fill_pool_torch((w.B, w.Hkv, w.d), seed * 100 + 92, device)
+            self.append = pkv.Append(k_new=self.knew, v_new=self.vnew, rope_cos=torch.from_numpy(self.rope_host[0]).to(device),
+                                     rope_sin=torch.from_numpy(self.rope_host[1]).to(device), rope_positions=npos)
         self.set_policy(pol)
 
     def set_bucket_route(self, gran):
@@ -236,6 +253,11 @@ class Runner:
             self.pkv.pkv_decode_buckets(self.shape, self.pol, self.q[r], self.k[r], self.v[r], self.bt[r],
                                         self.lens_all[t % self.nlens], ix, offs, self.out, None, scale=self.scale,
                                         workspace=self.ws, stream=stream)
+            return
+        if self.append is not None:
+            self.pkv.pkv_decode_append(self.shape, self.pol, self.q[r], self.k[r], self.v[r], self.bt[r],
+                                       self.lens_all[t % self.nlens], None, self.append, self.out, None, scale=self.scale,
+                                       workspace=self.ws, stream=stream)
             return
         sl = self.lens_all[t % self.nlens] if (stages & self.pkv.STAGE_BUILD) else self.lens_all[0]
         self.pkv.pkv_decode_stages(self.shape, self.pol, self.q[r], self.k[r], self.v[r], self.bt[r], sl,
@@ -426,7 +448,13 @@ def oracle_rows(torch, runner, rows, lens, r=0):
     q = np.ascontiguousarray(runner.q[r].cpu().numpy()[rows])
     sl = np.ascontiguousarray(np.asarray(lens, dtype=np.int32)[rows])
     t0 = time.perf_counter()
-    if runner.fp8:
+    if runner.append is not None:
+        from oracle import append_oracle
+        kn = np.ascontiguousarray(runner.knew.cpu().numpy()[rows])
+        vn = np.ascontiguousarray(runner.vnew.cpu().numpy()[rows])
+        out, _, _, _ = append_oracle.append_and_attend(q, kc, vc, kn, vn, tc, sl, runner.rope_host[0], runner.rope_host[1],
+                                                        Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale)
+    elif runner.fp8:
         sc = np.full(w.Hkv, FP8_SCALE, dtype=np.float64)
         out, _ = pkv_oracle.attention_fp8(q, kc, vc, sc, sc, tc, sl, Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale,
                                           num_threads=host_threads())
@@ -667,7 +695,8 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
                                                                  prefetch_kb=args.prefetch_kb)),
              ("config4", "config4", bal), ("config4_b4", "config4_b4", bal),
              ("config5", "config5", bal), ("config5_hkv4", "config5_hkv4", bal),
-             ("config2_fp8", "config2_fp8", bal), ("config3_fp8", "config3_fp8", bal)]
+             ("config2_fp8", "config2_fp8", bal), ("config3_fp8", "config3_fp8", bal),
+             ("config2_append", "config2_append", bal), ("config3_append", "config3_append", bal)]
     runner, cur = None, None
     for key, name, pol in cases:
         try:
@@ -684,10 +713,11 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
             K = w.steps if w.steps > 0 else 2 * args.graph_steps      # config 2 has no trace: 200 replayed steps
             chunk = max(1, min(args.graph_steps, K))
             bucketed = "buckets" in key
+            whole_only = bucketed or runner.append is not None       # no decode-alone variant of these steps
             runner.set_bucket_route(1 if bucketed else None)
-            r = time_policy(pkv, runner, pol, K, chunk, 5, decode_only=not bucketed)
+            r = time_policy(pkv, runner, pol, K, chunk, 5, decode_only=not whole_only)
             st = summarize(r["step_ms"], K)
-            dc = summarize(r["decode_ms"], K) if not bucketed else st
+            dc = summarize(r["decode_ms"], K) if not whole_only else st
             alg = mean_alg_bytes(w, K, runner.nlens)
             rows = pick_rows(runner.lens_at(0), 70000, w.seed)
             par, _ = parity_of(torch, runner, rows)
