@@ -596,9 +596,14 @@ def test_full_size_configs_in_the_bench_configuration(name):
     sl = torch.from_numpy(lens).to(dev)
     shape = pkv.Shape(B=w.B, Hq=w.Hq, Hkv=w.Hkv, max_pages=w.max_pages, num_pages=w.num_pages)
     pols = [pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0)]
+    # what bench.py times: the cost model's choice for these lengths (pkv_choose_policy, default constants)
+    auto, _ = pkv.pkv_choose_policy(shape, lens, pkv.pkv_default_cost_model(sm_count()),
+                                    pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_AUTO, num_splits=0))
+    pols.append(auto)
     if name == "config2":
         pols.append(pkv.Policy(tile_tokens=32, num_splits=16))
         pols.append(pkv.Policy(tile_tokens=32, num_splits=16, merge_mode=pkv.MERGE_FUSED))
+        pols.append(pkv.Policy(tile_tokens=32, num_splits=128))          # channel-sliced merge, 128 whole-page units
     if name == "config3_rect":      # BASELINE.json configs[2]: the rectangular (B, Hkv, S) grid
         pols = [pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_RECT),
                 pkv.Policy(tile_tokens=32, num_splits=20, route=pkv.ROUTE_WORKQUEUE)]
@@ -652,3 +657,72 @@ def test_speculative_plan_is_discarded_when_lengths_changed(mode):
     dp.sl.copy_(to_dev(new))
     p.seq_lens = new
     check(dp, pol, oracle_attention(p))
+
+
+@pytest.mark.parametrize("variant", ["fp8", "append", "buckets"])
+@pytest.mark.parametrize("name", ["config2", "config3"])
+def test_full_size_round2_routes(name, variant):
+    """BASELINE.json's config 2 and 3 at full size through the round-2 paths as bench.py times them
+    (cost-model policy): FP8 caches against the FP8 oracle, the fused KV-append + RoPE step against the
+    append oracle (outputs and the pool bytes of the new tokens), exact length buckets against the
+    FP16 oracle.  Every row of the batch is checked."""
+    import pkv_inputs as pi
+    from oracle import append_oracle, pkv_oracle
+    seed = pi.REPORT_SEEDS[0]
+    w = {"config2": pi.config2, "config3": pi.config3}[name](seed)
+    dev = torch.device("cuda", 0)
+    q = pi.fill_pool_torch((w.B, w.Hq, w.d), 21, dev)
+    k = pi.fill_pool_torch(w.pool_shape(), 22, dev)
+    v = pi.fill_pool_torch(w.pool_shape(), 23, dev)
+    bt = torch.from_numpy(w.block_table).to(dev)
+    lens = w.seq_lens_at(min(w.steps, 5)).astype(np.int32)
+    sl = torch.from_numpy(lens).to(dev)
+    rows = list(range(w.B))
+    scale = default_scale(w.d)
+    qh = np.ascontiguousarray(q.cpu().numpy())
+    out = torch.full((w.B, w.Hq, w.d), float("nan"), dtype=torch.float16, device=dev)
+    lse = torch.full((w.B, w.Hq), float("nan"), dtype=torch.float32, device=dev)
+    base = pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_AUTO, num_splits=0)
+    if variant == "fp8":
+        sc = torch.full((w.Hkv,), 1.0 / 32.0, dtype=torch.float32, device=dev)
+        k = (k.float() * 32.0).to(torch.float8_e4m3fn).view(torch.uint8)
+        v = (v.float() * 32.0).to(torch.float8_e4m3fn).view(torch.uint8)
+        shape = pkv.Shape(B=w.B, Hq=w.Hq, Hkv=w.Hkv, max_pages=w.max_pages, num_pages=w.num_pages, kv_dtype=pkv.KV_E4M3,
+                          k_scale=sc, v_scale=sc)
+        pol, _ = pkv.pkv_choose_policy(shape, lens, pkv.pkv_default_cost_model(sm_count()), base)
+        kc, vc, tc = _compact_rows(w, k, v, rows, lens)
+        s64 = np.full(w.Hkv, 1.0 / 32.0)
+        ref, ref_lse = pkv_oracle.attention_fp8(qh, kc, vc, s64, s64, tc, lens, Hkv=w.Hkv, page_size=w.page_size, scale=scale)
+        pkv.pkv_decode(shape, pol, q, k, v, bt, sl, out, lse, scale=scale, workspace=pkv.alloc_workspace(shape, pol))
+    else:
+        shape = pkv.Shape(B=w.B, Hq=w.Hq, Hkv=w.Hkv, max_pages=w.max_pages, num_pages=w.num_pages)
+        pol, _ = pkv.pkv_choose_policy(shape, lens, pkv.pkv_default_cost_model(sm_count()), base)
+        kc, vc, tc = _compact_rows(w, k, v, rows, lens)
+        if variant == "append":
+            kn = pi.fill_pool_torch((w.B, w.Hkv, w.d), 24, dev)
+            vn = pi.fill_pool_torch((w.B, w.Hkv, w.d), 25, dev)
+            npos = int(lens.max()) + 1
+            inv = 10000.0 ** (-np.arange(0, w.d // 2, dtype=np.float64) * 2.0 / w.d)
+            ang = np.arange(npos, dtype=np.float64)[:, None] * inv[None, :]
+            cos, sin = np.cos(ang).astype(np.float32), np.sin(ang).astype(np.float32)
+            ref, ref_lse, k2, v2 = append_oracle.append_and_attend(qh, kc, vc, kn.cpu().numpy(), vn.cpu().numpy(), tc, lens, cos, sin,
+                                                                   Hkv=w.Hkv, page_size=w.page_size, scale=scale)
+            app = pkv.Append(k_new=kn, v_new=vn, rope_cos=torch.from_numpy(cos).to(dev), rope_sin=torch.from_numpy(sin).to(dev),
+                             rope_positions=npos)
+            pkv.pkv_decode_append(shape, pol, q, k, v, bt, sl, None, app, out, lse, scale=scale,
+                                  workspace=pkv.alloc_workspace(shape, pol))
+            torch.cuda.synchronize()
+            kc_after, vc_after, _ = _compact_rows(w, k, v, rows, lens)
+            assert np.array_equal(kc_after.view(np.uint16), k2.view(np.uint16))
+            assert np.array_equal(vc_after.view(np.uint16), v2.view(np.uint16))
+        else:
+            ref, ref_lse = pkv_oracle.attention(qh, kc, vc, tc, lens, Hkv=w.Hkv, page_size=w.page_size, scale=scale)
+            pol = pkv.Policy(tile_tokens=32, num_splits=32, route=pkv.ROUTE_RECT)
+            index, offs, _ = pkv.pkv_plan_buckets_host(lens, 1)
+            pkv.pkv_decode_buckets(shape, pol, q, k, v, bt, sl, torch.from_numpy(index).to(dev), offs, out, lse, scale=scale,
+                                   workspace=pkv.alloc_workspace(shape, pol))
+    torch.cuda.synchronize()
+    got = out.cpu().numpy().astype(np.float64)
+    assert not np.isnan(got).any()
+    assert_within_tolerance(got, ref, "%s %s %s" % (name, variant, pol))
+    assert np.abs(lse.cpu().numpy().astype(np.float64) - ref_lse).max() <= 2e-3
