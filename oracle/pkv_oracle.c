@@ -31,10 +31,10 @@
  *
  * FP16 is decoded by the bit decoder below (no cuda_fp16.h, no compiler half type).
  *
- * FP8 KV ("dequantization-aware paged decode", PAPER.md:271 future work; DESIGN.md
- * reading A28): pkv_oracle_attention_fp8 is Eq. (1) on k_j = k_scale[g] * e4m3(K bytes),
- * v_j = v_scale[g] * e4m3(V bytes) -- OCP FP8 E4M3 ("fn": no infinities, S.1111.111 = NaN, largest
- * finite 448), one FP32 scale per KV head.  The byte decoder is pinned on all 256 patterns against
+ * One-byte KV ("dequantization-aware paged decode", PAPER.md:271 future work; DESIGN.md
+ * reading A28): pkv_oracle_attention_q8 is Eq. (1) on k_j = k_scale[g] * dec(K bytes),
+ * v_j = v_scale[g] * dec(V bytes), one scale per KV head; dec = OCP FP8 E4M3 ("fn": no infinities,
+ * S.1111.111 = NaN, largest finite 448) or two's-complement INT8.  The byte decoder is pinned on all 256 patterns against
  * torch.float8_e4m3fn and against closed forms (tests/test_oracle_pins.py).
  */
 #include <math.h>
@@ -85,20 +85,26 @@ typedef struct {
     const uint16_t *q, *k_cache, *v_cache;
     const int32_t *block_table, *seq_lens;
     double scale;
-    /* FP8 caches (NULL: FP16 caches above are used) and their per-KV-head scales */
+    /* one-byte caches (NULL: FP16 caches above are used) and their per-KV-head scales */
     const uint8_t *k8, *v8;
     const double *k_scale, *v_scale;
+    int kv_kind;   /* 1: OCP FP8 E4M3 bytes, 2: two's-complement INT8 bytes */
 } oracle_problem;
+
+static double byte_to_double(int kv_kind, uint8_t b)
+{
+    return kv_kind == 2 ? (double)(int8_t)b : e4m3_bits_to_double(b);
+}
 
 /* channel c of the K (V) row at element offset off, KV head g, as a real number */
 static double k_elem(const oracle_problem *p, int64_t off, int c, int g)
 {
-    if (p->k8) return p->k_scale[g] * e4m3_bits_to_double(p->k8[off + c]);
+    if (p->k8) return p->k_scale[g] * byte_to_double(p->kv_kind, p->k8[off + c]);
     return half_bits_to_double(p->k_cache[off + c]);
 }
 static double v_elem(const oracle_problem *p, int64_t off, int c, int g)
 {
-    if (p->v8) return p->v_scale[g] * e4m3_bits_to_double(p->v8[off + c]);
+    if (p->v8) return p->v_scale[g] * byte_to_double(p->kv_kind, p->v8[off + c]);
     return half_bits_to_double(p->v_cache[off + c]);
 }
 
@@ -159,21 +165,23 @@ int pkv_oracle_attention(int B, int Hq, int Hkv, int d, int page_size, int max_p
 {
     if (B < 0 || Hkv <= 0 || Hq % Hkv || d <= 0 || page_size <= 0) return -1;
     oracle_problem p = { B, Hq, Hkv, d, page_size, max_pages, stride_page, stride_token, stride_head,
-                         q, k_cache, v_cache, block_table, seq_lens, scale, NULL, NULL, NULL, NULL };
+                         q, k_cache, v_cache, block_table, seq_lens, scale, NULL, NULL, NULL, NULL, 0 };
     return attention_impl(&p, out, lse, num_threads);
 }
 
-/* The same on FP8 (E4M3) caches with one scale per KV head (reading A28); strides in elements = bytes. */
-int pkv_oracle_attention_fp8(int B, int Hq, int Hkv, int d, int page_size, int max_pages,
-                             int64_t stride_page, int64_t stride_token, int64_t stride_head,
-                             const uint16_t *q, const uint8_t *k8, const uint8_t *v8,
-                             const double *k_scale, const double *v_scale,
-                             const int32_t *block_table, const int32_t *seq_lens, double scale,
-                             double *out, double *lse, int num_threads)
+/* The same on one-byte caches with one scale per KV head (reading A28): kv_kind 1 = FP8 E4M3,
+ * 2 = INT8; strides in elements = bytes. */
+int pkv_oracle_attention_q8(int B, int Hq, int Hkv, int d, int page_size, int max_pages,
+                            int64_t stride_page, int64_t stride_token, int64_t stride_head,
+                            const uint16_t *q, const uint8_t *k8, const uint8_t *v8,
+                            const double *k_scale, const double *v_scale, int kv_kind,
+                            const int32_t *block_table, const int32_t *seq_lens, double scale,
+                            double *out, double *lse, int num_threads)
 {
     if (B < 0 || Hkv <= 0 || Hq % Hkv || d <= 0 || page_size <= 0 || !k8 || !v8 || !k_scale || !v_scale) return -1;
+    if (kv_kind != 1 && kv_kind != 2) return -1;
     oracle_problem p = { B, Hq, Hkv, d, page_size, max_pages, stride_page, stride_token, stride_head,
-                         q, NULL, NULL, block_table, seq_lens, scale, k8, v8, k_scale, v_scale };
+                         q, NULL, NULL, block_table, seq_lens, scale, k8, v8, k_scale, v_scale, kv_kind };
     return attention_impl(&p, out, lse, num_threads);
 }
 
@@ -226,7 +234,7 @@ int pkv_oracle_split_states(int B, int Hq, int Hkv, int d, int page_size, int ma
 {
     if (B < 0 || Hkv <= 0 || Hq % Hkv || d <= 0 || page_size <= 0 || tile_tokens <= 0) return -1;
     oracle_problem p = { B, Hq, Hkv, d, page_size, max_pages, stride_page, stride_token, stride_head,
-                         q, k_cache, v_cache, block_table, seq_lens, scale, NULL, NULL, NULL, NULL };
+                         q, k_cache, v_cache, block_table, seq_lens, scale, NULL, NULL, NULL, NULL, 0 };
     int G = Hq / Hkv;
     int failed = 0;
 #ifdef _OPENMP

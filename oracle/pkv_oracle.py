@@ -48,8 +48,8 @@ def _load():
         lib.pkv_oracle_half_to_double.restype = f64
         lib.pkv_oracle_e4m3_to_double.argtypes = [ctypes.c_uint8]
         lib.pkv_oracle_e4m3_to_double.restype = f64
-        lib.pkv_oracle_attention_fp8.argtypes = [i32] * 6 + [i64] * 3 + [vp] * 7 + [f64, vp, vp, i32]
-        lib.pkv_oracle_attention_fp8.restype = i32
+        lib.pkv_oracle_attention_q8.argtypes = [i32] * 6 + [i64] * 3 + [vp] * 5 + [i32, vp, vp, f64, vp, vp, i32]
+        lib.pkv_oracle_attention_q8.restype = i32
         _lib = lib
     return _lib
 
@@ -101,11 +101,16 @@ def e4m3_to_double(bits: int) -> float:
     return float(_load().pkv_oracle_e4m3_to_double(int(bits) & 0xFF))
 
 
+def attention_int8(q, k8, v8, k_scale, v_scale, block_table, seq_lens, **kw):
+    """Eq. (1) on INT8 caches (reading A28): k8, v8 uint8 views of two's-complement bytes."""
+    return attention_fp8(q, k8, v8, k_scale, v_scale, block_table, seq_lens, kv_kind=2, **kw)
+
+
 def attention_fp8(q: np.ndarray, k8: np.ndarray, v8: np.ndarray, k_scale: np.ndarray, v_scale: np.ndarray,
                   block_table: np.ndarray, seq_lens: np.ndarray, *, Hkv: int, page_size: int, scale: float,
-                  strides: Optional[Tuple[int, int, int]] = None, num_threads: int = 0):
-    """Eq. (1) on FP8 caches (reading A28): k8, v8 uint8 E4M3 bytes, k_scale, v_scale [Hkv] (any float
-    dtype; used as FP64).  Returns (out [B,Hq,d] f64, lse [B,Hq] f64)."""
+                  strides: Optional[Tuple[int, int, int]] = None, num_threads: int = 0, kv_kind: int = 1):
+    """Eq. (1) on one-byte caches (reading A28): k8, v8 uint8 bytes (E4M3, or INT8 with kv_kind=2),
+    k_scale, v_scale [Hkv] (any float dtype; used as FP64).  Returns (out [B,Hq,d] f64, lse [B,Hq] f64)."""
     assert q.dtype == np.float16 and k8.dtype == np.uint8 and v8.dtype == np.uint8
     assert block_table.dtype == np.int32 and seq_lens.dtype == np.int32
     ks = np.ascontiguousarray(k_scale, dtype=np.float64)
@@ -117,11 +122,11 @@ def attention_fp8(q: np.ndarray, k8: np.ndarray, v8: np.ndarray, k_scale: np.nda
     sp, st, sh = strides or _default_strides(page_size, Hkv, d)
     out = np.empty((B, Hq, d), dtype=np.float64)
     lse = np.empty((B, Hq), dtype=np.float64)
-    rc = _load().pkv_oracle_attention_fp8(B, Hq, Hkv, d, page_size, block_table.shape[1], sp, st, sh,
-                                          _ptr(q), _ptr(k8), _ptr(v8), _ptr(ks), _ptr(vs), _ptr(block_table),
-                                          _ptr(seq_lens), float(scale), _ptr(out), _ptr(lse), num_threads)
+    rc = _load().pkv_oracle_attention_q8(B, Hq, Hkv, d, page_size, block_table.shape[1], sp, st, sh,
+                                         _ptr(q), _ptr(k8), _ptr(v8), _ptr(ks), _ptr(vs), int(kv_kind), _ptr(block_table),
+                                         _ptr(seq_lens), float(scale), _ptr(out), _ptr(lse), num_threads)
     if rc != 0:
-        raise RuntimeError("pkv_oracle_attention_fp8 failed: %d" % rc)
+        raise RuntimeError("pkv_oracle_attention_q8 failed: %d" % rc)
     return out, lse
 
 

@@ -373,3 +373,32 @@ def test_append_step_against_dense_brute_force():
             assert np.array_equal(k2[p.block_table[i, pos // 16], pos % 16], kn)
             assert np.array_equal(v2[p.block_table[i, pos // 16], pos % 16], v_new[i])
         assert np.array_equal(k2[~changed], p.k_cache[~changed]) and np.array_equal(v2[~changed], p.v_cache[~changed])
+
+
+def test_int8_attention_reduces_to_the_fp16_oracle_and_to_brute_force():
+    """INT8 caches (reading A28): with power-of-two scales every dequantised value is an FP16 number,
+    so the INT8 entry point must agree with the FP16 oracle on the dequantised caches; with arbitrary
+    scales with dense numpy on the real values (the byte decode here is numpy's own int8 view)."""
+    p = make_problem([1, 17, 100, 0, 33], seed=63)
+    rng = np.random.Generator(np.random.PCG64(9))
+    k8 = rng.integers(-128, 128, size=p.k_cache.shape).astype(np.int8).view(np.uint8)
+    v8 = rng.integers(-128, 128, size=p.v_cache.shape).astype(np.int8).view(np.uint8)
+    ks = np.array([2.0 ** -5, 2.0 ** -6, 2.0 ** -4, 2.0 ** -7, 2.0 ** -5, 2.0 ** -6, 2.0 ** -5, 2.0 ** -8])
+    vs = np.array([2.0 ** -6, 2.0 ** -5, 2.0 ** -7, 2.0 ** -4, 2.0 ** -6, 2.0 ** -5, 2.0 ** -6, 2.0 ** -5])
+    kd = (k8.view(np.int8).astype(np.float64) * ks[None, None, :, None])
+    vd = (v8.view(np.int8).astype(np.float64) * vs[None, None, :, None])
+    assert np.array_equal(kd.astype(np.float16).astype(np.float64), kd)
+    got, got_lse = pkv_oracle.attention_int8(p.q, k8, v8, ks, vs, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    ref, ref_lse = pkv_oracle.attention(p.q, kd.astype(np.float16), vd.astype(np.float16), p.block_table, p.seq_lens, Hkv=8,
+                                        page_size=16, scale=p.scale)
+    fin = np.isfinite(ref_lse)
+    assert np.abs(got - ref).max() <= 1e-12 and np.abs(got_lse[fin] - ref_lse[fin]).max() <= 1e-12
+    ks2, vs2 = np.linspace(0.003, 0.011, 8), np.linspace(0.02, 0.005, 8)
+    got, got_lse = pkv_oracle.attention_int8(p.q, k8, v8, ks2, vs2, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    pr = Problem(q=p.q, k_cache=k8.view(np.int8).astype(np.float64) * ks2[None, None, :, None],
+                 v_cache=v8.view(np.int8).astype(np.float64) * vs2[None, None, :, None],
+                 block_table=p.block_table, seq_lens=p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    ref, ref_lse = dense_attention_bruteforce(pr)
+    assert np.abs(got - ref).max() <= 1e-12 and np.abs(got_lse[fin] - ref_lse[fin]).max() <= 1e-12
+    e4, _ = pkv_oracle.attention_fp8(p.q, k8, v8, ks2, vs2, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
+    assert not np.allclose(np.nan_to_num(e4), got)          # the byte kind matters
