@@ -145,9 +145,10 @@ typedef struct {
     int64_t num_pages;
     int64_t kv_stride_page, kv_stride_token, kv_stride_head;
     /* FP8 KV cache with in-loop dequantisation ("dequantization-aware paged decode";
-     * DESIGN.md reading A28): kv_dtype = PKV_KV_E4M3 makes k_cache / v_cache buffers of OCP FP8 E4M3
-     * bytes (same layout, strides in elements = bytes, multiples of 16) that stand for
-     *   k = k_scale[kv head] * e4m3(byte),  v = v_scale[kv head] * e4m3(byte)
+     * DESIGN.md reading A28): kv_dtype = PKV_KV_E4M3 / PKV_KV_INT8 makes k_cache / v_cache buffers of
+     * OCP FP8 E4M3 / two's-complement INT8 bytes (same layout, strides in elements = bytes, multiples
+     * of 16) that stand for
+     *   k = k_scale[kv head] * dec(byte),  v = v_scale[kv head] * dec(byte)
      * k_scale / v_scale: dev float [Hkv], or NULL for 1.0.  q and out stay FP16, arithmetic as for
      * FP16 caches (E4M3 values are FP16 numbers).  TMA kernel, d = 128, G in {4, 8} only. */
     int32_t kv_dtype;                            /* pkv_kv_dtype; 0 = FP16                       */
@@ -155,7 +156,7 @@ typedef struct {
     const float* k_scale;
     const float* v_scale;
 } pkv_shape;
-typedef enum { PKV_KV_F16 = 0, PKV_KV_E4M3 = 1 } pkv_kv_dtype;
+typedef enum { PKV_KV_F16 = 0, PKV_KV_E4M3 = 1, PKV_KV_INT8 = 2 } pkv_kv_dtype;
 
 /* Scheduler-derived counters with the definitions of Table 4 (A13,
  * A14).  Filled by pkv_get_counters from the workqueue state of the last build / decode. */

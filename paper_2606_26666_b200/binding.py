@@ -25,7 +25,7 @@ KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
 FLAG_VALIDATE, FLAG_NO_PDL, FLAG_SEPARATE_BUILD, FLAG_TEST_REPLAN = 1, 2, 4, 8
 DEVERR_QUEUE_OVERFLOW, DEVERR_SEQ_LEN, DEVERR_PAGE_ID = 1, 2, 4
 STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL = 1, 2, 4, 7
-KV_F16, KV_E4M3 = 0, 1
+KV_F16, KV_E4M3, KV_INT8 = 0, 1, 2
 
 _i32, _i64 = ctypes.c_int32, ctypes.c_int64
 _vp = ctypes.c_void_p

@@ -79,7 +79,7 @@ bool encode_map(const void* base, const pkv_shape& s, const Strides& st, int HG,
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t pages = (cuuint64_t)(s.num_pages > 0 ? s.num_pages : 1);
-    const bool fp8 = s.kv_dtype == PKV_KV_E4M3;
+    const bool fp8 = s.kv_dtype != PKV_KV_F16;           // one-byte caches (E4M3, INT8)
     const cuuint64_t eb = fp8 ? 1 : 2;                   // bytes per element
     const cuuint32_t inner = (cuuint32_t)(128 / eb);     // elements of one 128-byte swizzled row
     const cuuint32_t blocks = (cuuint32_t)(s.d / inner); // 128-byte blocks of a head's row
@@ -237,7 +237,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             if (known_slots < 0 && rp.split_mode == PKV_SPLIT_BALANCED && rp.num_sms > 0 && rp.num_sms < row_slots)
                 row_slots = rp.num_sms;
             const int HG = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, row_slots, num_sms, max_heads_per_cta(rp.G, s.d));
-            p.prefetch_pages = rp.prefetch_kb * 1024 / decode_tma_stage_bytes(HG, s.d, s.kv_dtype == PKV_KV_E4M3);
+            p.prefetch_pages = rp.prefetch_kb * 1024 / decode_tma_stage_bytes(HG, s.d, s.kv_dtype != PKV_KV_F16);
             // by value: inserting the V map may evict the cache entry the K pointer refers to
             const CUtensorMap* pk = get_map(k_cache, s, HG);
             CUtensorMap mk_copy, mv_copy;
@@ -258,7 +258,7 @@ pkv_status run_decode(const pkv_shape& s, const Resolved& rp, const void* q, con
             p.dynamic_sched = HG * (rp.G == 16 ? 2 : 1) == 8 ? 1 : 0;
             const int64_t units = row_slots * (s.Hkv / HG);
             const int grid = (int)(units < num_sms ? units : num_sms);
-            e = launch_decode_tma(p, rp.G, HG, s.d, s.kv_dtype == PKV_KV_E4M3, grid, mk, mv, stream);
+            e = launch_decode_tma(p, rp.G, HG, s.d, s.kv_dtype, grid, mk, mv, stream);
         } else {
             const int64_t cap = (int64_t)num_sms * 4;
             const int grid = (int)(bound < cap ? bound : cap);
@@ -507,7 +507,7 @@ pkv_status pkv_get_counters(const pkv_shape* shape, const pkv_split_policy* poli
     host_out->merge_launches =
         (h.num_tasks > 0 && h.max_row_splits > 1 && rp.merge_mode == PKV_MERGE_SEPARATE) ? 1 : 0;
     host_out->build_launches = h.build_launches;
-    host_out->useful_kv_bytes = h.sum_seq_lens * 2 * shape->Hkv * shape->d * (shape->kv_dtype == PKV_KV_E4M3 ? 1 : 2);
+    host_out->useful_kv_bytes = h.sum_seq_lens * 2 * shape->Hkv * shape->d * (shape->kv_dtype != PKV_KV_F16 ? 1 : 2);
     host_out->merge_bytes = (int64_t)h.num_tasks * rp.G * (shape->d + 2) * 4;
     host_out->num_splits = h.resolved_splits;
     host_out->max_row_splits = h.max_row_splits;
@@ -799,7 +799,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
         counters_out->decode_launches = dl;
         counters_out->merge_launches = ml;
         counters_out->build_launches = (!fused && hdr->num_tasks > 0) ? 1 : 0;
-        counters_out->useful_kv_bytes = hdr->sum_seq_lens * 2 * s.Hkv * s.d * (s.kv_dtype == PKV_KV_E4M3 ? 1 : 2);
+        counters_out->useful_kv_bytes = hdr->sum_seq_lens * 2 * s.Hkv * s.d * (s.kv_dtype != PKV_KV_F16 ? 1 : 2);
         counters_out->merge_bytes = (int64_t)hdr->num_tasks * rp.G * (s.d + 2) * 4;
         counters_out->num_splits = hdr->resolved_splits;
         counters_out->max_row_splits = hdr->max_row_splits;

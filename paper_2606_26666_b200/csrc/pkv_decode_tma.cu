@@ -83,7 +83,7 @@ __host__ __device__ constexpr int blocks_for(int G) { return G > 8 ? G / 8 : 1; 
 // FP8 caches: one byte per channel, half the bytes.
 __host__ __device__ constexpr int stage_bytes_for(int HG, int D, bool fp8 = false) { return HG * D * (fp8 ? 32 : 64); }
 
-template <int G, int HG, int D, bool FP8 = false>
+template <int G, int HG, int D, bool FP8 = false>   // FP8: one-byte caches (E4M3 or INT8)
 __host__ __device__ constexpr int stages_for() {
     // 227 KiB per CTA, minus the tail, minus 1 KiB alignment slack
     constexpr int avail = 232448 - 1024 - (int)sizeof(SmemTail<G / blocks_for(G), D>);
@@ -133,11 +133,13 @@ __device__ __forceinline__ void append_patch(const DecodeParams& p, uint32_t sb,
     __syncwarp();
 }
 
-template <int G, int HG, int D, bool FP8>
+// KVT: pkv_kv_dtype of the caches (0 FP16, 1 FP8 E4M3, 2 INT8); "FP8" below means any one-byte cache.
+template <int G, int HG, int D, int KVT>
 __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 1)
     pkv_decode_tma_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap_k,
                           const __grid_constant__ CUtensorMap tmap_v) {
-    static_assert(!FP8 || D == 128, "FP8 caches: one 128-byte swizzled row per token and head");
+    constexpr bool FP8 = KVT != 0;
+    static_assert(!FP8 || D == 128, "one-byte caches: one 128-byte swizzled row per token and head");
     constexpr int kStages = stages_for<G, HG, D, FP8>();
     constexpr int kHeadBytes = D * (FP8 ? 16 : 32);   // one head's 16 tokens x D channels of K (or V): blocks of 2 KiB
     constexpr int kStageBytes = stage_bytes_for(HG, D, FP8);   // K: HG x kHeadBytes | V: HG x kHeadBytes
@@ -558,10 +560,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                         uint32_t r0, r1, r2, r3;
                         const uint32_t chunk = (j << 1) | k_sel;
                         ldmatrix_x4(kb + k_tok * 128 + ((chunk ^ xr) << 4), r0, r1, r2, r3);
-                        mma_16816(c0, cvt_e4m3x2_to_half2(r0), cvt_e4m3x2_to_half2(r1), cvt_e4m3x2_to_half2(r0 >> 16),
-                                  cvt_e4m3x2_to_half2(r1 >> 16), qb[2 * j][0], qb[2 * j][1]);
-                        mma_16816(c1, cvt_e4m3x2_to_half2(r2), cvt_e4m3x2_to_half2(r3), cvt_e4m3x2_to_half2(r2 >> 16),
-                                  cvt_e4m3x2_to_half2(r3 >> 16), qb[2 * j + 1][0], qb[2 * j + 1][1]);
+                        mma_16816(c0, cvt_bytes2_to_half2<KVT>(r0), cvt_bytes2_to_half2<KVT>(r1), cvt_bytes2_to_half2<KVT>(r0 >> 16),
+                                  cvt_bytes2_to_half2<KVT>(r1 >> 16), qb[2 * j][0], qb[2 * j][1]);
+                        mma_16816(c1, cvt_bytes2_to_half2<KVT>(r2), cvt_bytes2_to_half2<KVT>(r3), cvt_bytes2_to_half2<KVT>(r2 >> 16),
+                                  cvt_bytes2_to_half2<KVT>(r3 >> 16), qb[2 * j + 1][0], qb[2 * j + 1][1]);
                     }
                 } else {
 #pragma unroll
@@ -629,10 +631,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                         uint32_t r0, r1, r2, r3;
                         const uint32_t chunk = (j << 1) | k_sel;
                         ldmatrix_x4_trans(vb + k_tok * 128 + ((chunk ^ xr) << 4), r0, r1, r2, r3);
-                        mma_16816(o[2 * j], cvt_e4m3x2_to_half2(__byte_perm(r0, 0, 0x0020)), cvt_e4m3x2_to_half2(__byte_perm(r0, 0, 0x0031)),
-                                  cvt_e4m3x2_to_half2(__byte_perm(r1, 0, 0x0020)), cvt_e4m3x2_to_half2(__byte_perm(r1, 0, 0x0031)), pb0, pb1);
-                        mma_16816(o[2 * j + 1], cvt_e4m3x2_to_half2(__byte_perm(r2, 0, 0x0020)), cvt_e4m3x2_to_half2(__byte_perm(r2, 0, 0x0031)),
-                                  cvt_e4m3x2_to_half2(__byte_perm(r3, 0, 0x0020)), cvt_e4m3x2_to_half2(__byte_perm(r3, 0, 0x0031)), pb0, pb1);
+                        mma_16816(o[2 * j], cvt_bytes2_to_half2<KVT>(__byte_perm(r0, 0, 0x0020)), cvt_bytes2_to_half2<KVT>(__byte_perm(r0, 0, 0x0031)),
+                                  cvt_bytes2_to_half2<KVT>(__byte_perm(r1, 0, 0x0020)), cvt_bytes2_to_half2<KVT>(__byte_perm(r1, 0, 0x0031)), pb0, pb1);
+                        mma_16816(o[2 * j + 1], cvt_bytes2_to_half2<KVT>(__byte_perm(r2, 0, 0x0020)), cvt_bytes2_to_half2<KVT>(__byte_perm(r2, 0, 0x0031)),
+                                  cvt_bytes2_to_half2<KVT>(__byte_perm(r3, 0, 0x0020)), cvt_bytes2_to_half2<KVT>(__byte_perm(r3, 0, 0x0031)), pb0, pb1);
                         vdep ^= r0 ^ r1 ^ r2 ^ r3;
                     }
                 } else {
@@ -744,10 +746,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     }
 }
 
-template <int G, int HG, int D, bool FP8>
+template <int G, int HG, int D, int KVT>
 cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, const CUtensorMap& mv,
                        cudaStream_t stream) {
-    constexpr int smem = stages_for<G, HG, D, FP8>() * stage_bytes_for(HG, D, FP8) + (int)sizeof(SmemTail<G / blocks_for(G), D>) + 1024;
+    constexpr int smem = stages_for<G, HG, D, KVT != 0>() * stage_bytes_for(HG, D, KVT != 0) + (int)sizeof(SmemTail<G / blocks_for(G), D>) + 1024;
     constexpr int threads = (producers_for(HG) + kComputeWarps + 1) * 32;
     // The dynamic shared-memory opt-in is a per-device (per-context) attribute of the kernel: one
     // flag per device ordinal, set on the first launch there (races only repeat the call).
@@ -756,11 +758,11 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64 || !attr_set[dev]) {
-        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG, D, FP8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG, D, KVT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
-    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG, D, FP8>, dim3(grid), dim3(threads),
+    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG, D, KVT>, dim3(grid), dim3(threads),
                       (size_t)smem, stream, p, mk, mv);
 }
 
@@ -768,13 +770,13 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
 
 int decode_tma_stage_bytes(int HG, int D, bool fp8) { return stage_bytes_for(HG, D, fp8); }
 
-cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, bool fp8, int grid, const void* tmap_k,
+cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int kvt, int grid, const void* tmap_k,
                               const void* tmap_v, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
     const CUtensorMap& mk = *reinterpret_cast<const CUtensorMap*>(tmap_k);
     const CUtensorMap& mv = *reinterpret_cast<const CUtensorMap*>(tmap_v);
 #define PKV_CASE(GG, HH, DD) \
-    if (G == GG && HG == HH && D == DD && !fp8) return launch_one<GG, HH, DD, false>(p, grid, mk, mv, stream);
+    if (G == GG && HG == HH && D == DD && kvt == 0) return launch_one<GG, HH, DD, 0>(p, grid, mk, mv, stream);
     PKV_CASE(4, 8, 128) PKV_CASE(4, 4, 128) PKV_CASE(4, 2, 128) PKV_CASE(4, 1, 128)
     PKV_CASE(8, 8, 128) PKV_CASE(8, 4, 128) PKV_CASE(8, 2, 128) PKV_CASE(8, 1, 128)
     PKV_CASE(2, 8, 128) PKV_CASE(2, 4, 128) PKV_CASE(2, 2, 128) PKV_CASE(2, 1, 128)
@@ -787,8 +789,9 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, bool 
     PKV_CASE(8, 4, 256) PKV_CASE(8, 2, 256) PKV_CASE(8, 1, 256)   // (a stage of 8 would be 128 KiB)
 #undef PKV_CASE
 #define PKV_CASE8(GG, HH) \
-    if (G == GG && HG == HH && D == 128 && fp8) return launch_one<GG, HH, 128, true>(p, grid, mk, mv, stream);
-    // FP8 (E4M3) caches: d = 128, G = 4 and 8
+    if (G == GG && HG == HH && D == 128 && kvt == 1) return launch_one<GG, HH, 128, 1>(p, grid, mk, mv, stream); \
+    if (G == GG && HG == HH && D == 128 && kvt == 2) return launch_one<GG, HH, 128, 2>(p, grid, mk, mv, stream);
+    // one-byte caches (FP8 E4M3, INT8): d = 128, G = 4 and 8
     PKV_CASE8(4, 8) PKV_CASE8(4, 4) PKV_CASE8(4, 2) PKV_CASE8(4, 1)
     PKV_CASE8(8, 8) PKV_CASE8(8, 4) PKV_CASE8(8, 2) PKV_CASE8(8, 1)
 #undef PKV_CASE8

@@ -222,6 +222,18 @@ __device__ __forceinline__ uint32_t cvt_e4m3x2_to_half2(uint32_t x) {
     asm("{\n\t.reg .b16 t;\n\tcvt.u16.u32 t, %1;\n\tcvt.rn.f16x2.e4m3x2 %0, t;\n\t}" : "=r"(d) : "r"(x));
     return d;
 }
+// two cache bytes (low 16 bits of x) -> half2, exact.  INT8: (b ^ 0x80) | 0x6400 is the FP16 number
+// 1024 + (b + 128); subtracting 1152 leaves b (integers below 2048 are exact in FP16).
+template <int KVT>
+__device__ __forceinline__ uint32_t cvt_bytes2_to_half2(uint32_t x) {
+    if constexpr (KVT == 2) {
+        const uint32_t biased = __byte_perm(x ^ 0x8080u, 0x64646464u, 0x4140);
+        const __half2 h = __hsub2(*reinterpret_cast<const __half2*>(&biased), __floats2half2_rn(1152.f, 1152.f));
+        return *reinterpret_cast<const uint32_t*>(&h);
+    } else {
+        return cvt_e4m3x2_to_half2(x);
+    }
+}
 __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
     __half2 h = __floats2half2_rn(lo, hi);
     return *reinterpret_cast<uint32_t*>(&h);
@@ -800,7 +812,7 @@ inline PlanArgs make_plan_args(const pkv_shape& shape, const Resolved& rp) {
 
 // launchers implemented in the .cu files
 cudaError_t launch_decode_simt(const DecodeParams& p, int G, int grid, cudaStream_t stream);
-cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, bool fp8, int grid, const void* tmap_k,
+cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int kvt, int grid, const void* tmap_k,
                               const void* tmap_v, cudaStream_t stream);
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
                            const int32_t* row_index, QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,

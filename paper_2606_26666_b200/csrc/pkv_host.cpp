@@ -36,8 +36,8 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     if (s.page_size != 16 && s.page_size != 32 && s.page_size != 64) { set_error("page_size=%d not supported (16, 32 or 64)", s.page_size); return PKV_ERR_UNSUPPORTED; }
     const int G = s.Hq / s.Hkv;
     if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16) { set_error("G=Hq/Hkv=%d not compiled in (1, 2, 4, 8 and 16 only)", G); return PKV_ERR_UNSUPPORTED; }
-    if (s.kv_dtype != PKV_KV_F16 && s.kv_dtype != PKV_KV_E4M3) { set_error("bad kv_dtype %d", s.kv_dtype); return PKV_ERR_INVALID_ARG; }
-    if (s.kv_dtype == PKV_KV_E4M3) {
+    if (s.kv_dtype != PKV_KV_F16 && s.kv_dtype != PKV_KV_E4M3 && s.kv_dtype != PKV_KV_INT8) { set_error("bad kv_dtype %d", s.kv_dtype); return PKV_ERR_INVALID_ARG; }
+    if (s.kv_dtype != PKV_KV_F16) {
         if (s.d != kD || (G != 4 && G != 8)) { set_error("FP8 KV is compiled in for d=128 and G=4 or 8 only (d=%d, G=%d)", s.d, G); return PKV_ERR_UNSUPPORTED; }
         if (p.kernel == PKV_KERNEL_SIMT) { set_error("FP8 KV needs the TMA kernel"); return PKV_ERR_UNSUPPORTED; }
         if (s.kv_stride_page % 16 || s.kv_stride_token % 16 || s.kv_stride_head % 16) { set_error("FP8 kv strides must be multiples of 16 bytes"); return PKV_ERR_INVALID_ARG; }
@@ -120,7 +120,7 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     out->flags = p.flags;
     out->heads_per_cta = p.heads_per_cta;
     // default: 256 KiB of FP16 K/V per CTA (FP8: 128 KiB -- the same tokens); measured sweeps in DESIGN.md
-    out->prefetch_kb = p.prefetch_kb == 0 ? (s.kv_dtype == PKV_KV_E4M3 ? kDefaultPrefetchKb / 2 : kDefaultPrefetchKb)
+    out->prefetch_kb = p.prefetch_kb == 0 ? (s.kv_dtype != PKV_KV_F16 ? kDefaultPrefetchKb / 2 : kDefaultPrefetchKb)
                                           : (p.prefetch_kb < 0 ? 0 : p.prefetch_kb);
     return PKV_OK;
 }
@@ -243,7 +243,7 @@ void launch_totals(const pkv_shape& s, const Resolved& rp, const int32_t* lens, 
     int32_t max_tok = 0;
     plan_host(s, rp, lens, nullptr, 0, nullptr, nullptr, &hdr, &max_tok);
     const bool partials = hdr.max_row_splits > 1;
-    t->kv_bytes = hdr.sum_seq_lens * 2 * s.Hkv * s.d * (s.kv_dtype == PKV_KV_E4M3 ? 1 : 2);
+    t->kv_bytes = hdr.sum_seq_lens * 2 * s.Hkv * s.d * (s.kv_dtype != PKV_KV_F16 ? 1 : 2);
     t->tasks = hdr.num_tasks;
     t->merge_bytes = partials ? (int64_t)hdr.num_tasks * rp.G * (s.d + 2) * 4 : 0;
     t->launches = (hdr.num_tasks > 0 ? 1 : 0) + ((partials && hdr.num_tasks > 0 && rp.merge_mode == PKV_MERGE_SEPARATE) ? 1 : 0);
@@ -251,7 +251,7 @@ void launch_totals(const pkv_shape& s, const Resolved& rp, const int32_t* lens, 
     t->max_share = 0;
     if (hdr.total_row_slots > 0) {
         const int hg = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, hdr.total_row_slots, num_sms, max_heads_per_cta(rp.G, s.d));
-        const int64_t unit = (int64_t)max_tok * 2 * hg * s.d * (s.kv_dtype == PKV_KV_E4M3 ? 1 : 2);
+        const int64_t unit = (int64_t)max_tok * 2 * hg * s.d * (s.kv_dtype != PKV_KV_F16 ? 1 : 2);
         const int64_t units = (int64_t)hdr.total_row_slots * (s.Hkv / hg);
         t->max_share = units <= num_sms ? unit : t->kv_bytes / num_sms + unit;
         t->units = units;
@@ -341,7 +341,7 @@ pkv_status pkv_bucket_counters_host(const pkv_shape* shape, const pkv_split_poli
         out->empty_tasks += hdr.empty_tasks;
         out->decode_launches += hdr.num_tasks > 0 ? 1 : 0;
         out->merge_launches += (merge && rp.merge_mode == PKV_MERGE_SEPARATE) ? 1 : 0;
-        out->useful_kv_bytes += hdr.sum_seq_lens * 2 * shape->Hkv * shape->d * (shape->kv_dtype == PKV_KV_E4M3 ? 1 : 2);
+        out->useful_kv_bytes += hdr.sum_seq_lens * 2 * shape->Hkv * shape->d * (shape->kv_dtype != PKV_KV_F16 ? 1 : 2);
         out->merge_bytes += merge ? (int64_t)hdr.num_tasks * rp.G * (shape->d + 2) * 4 : 0;
         out->num_splits = rp.S;
         if (hdr.max_row_splits > out->max_row_splits) out->max_row_splits = hdr.max_row_splits;

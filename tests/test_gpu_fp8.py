@@ -16,30 +16,35 @@ pytestmark = pytest.mark.gpu
 RAGGED = [1, 2, 15, 16, 17, 31, 32, 33, 100, 0, 257, 700, 4099]
 
 
-def quantize(x: np.ndarray, scale: np.ndarray) -> np.ndarray:
-    t = torch.from_numpy(np.clip(x.astype(np.float32) / scale[None, None, :, None].astype(np.float32), -448.0, 448.0))
+def quantize(x: np.ndarray, scale: np.ndarray, kind: int = 1) -> np.ndarray:
+    y = x.astype(np.float32) / scale[None, None, :, None].astype(np.float32)
+    if kind == pkv.KV_INT8:
+        return np.clip(np.rint(y), -127, 127).astype(np.int8).view(np.uint8).copy()
+    t = torch.from_numpy(np.clip(y, -448.0, 448.0))
     return t.to(torch.float8_e4m3fn).view(torch.uint8).numpy().copy()
 
 
 class Fp8Problem:
-    def __init__(self, lens, seed, Hkv=8, page_size=16, scales=True):
+    def __init__(self, lens, seed, Hkv=8, page_size=16, scales=True, kind=pkv.KV_E4M3):
         self.p = p = make_problem(lens, seed=seed, Hkv=Hkv, page_size=page_size)
+        self.kind = kind
         rng = np.random.Generator(np.random.PCG64(seed))
-        self.ks = (rng.uniform(0.02, 0.06, size=Hkv) if scales else np.ones(Hkv)).astype(np.float32)
-        self.vs = (rng.uniform(0.02, 0.08, size=Hkv) if scales else np.ones(Hkv)).astype(np.float32)
-        self.k8, self.v8 = quantize(p.k_cache, self.ks), quantize(p.v_cache, self.vs)
+        lo, hi = (0.02, 0.06) if kind == pkv.KV_E4M3 else (0.04, 0.08)      # INT8: N(0,1) / scale inside +-127
+        self.ks = (rng.uniform(lo, hi, size=Hkv) if scales else np.ones(Hkv)).astype(np.float32)
+        self.vs = (rng.uniform(lo, hi, size=Hkv) if scales else np.ones(Hkv)).astype(np.float32)
+        self.k8, self.v8 = quantize(p.k_cache, self.ks, kind), quantize(p.v_cache, self.vs, kind)
         self.q, self.k, self.v = to_dev(p.q), to_dev(self.k8), to_dev(self.v8)
         self.bt, self.sl = to_dev(p.block_table), to_dev(p.seq_lens)
         self.dks, self.dvs = (to_dev(self.ks), to_dev(self.vs)) if scales else (None, None)
         self.shape = pkv.Shape(B=p.B, Hq=p.Hq, Hkv=Hkv, page_size=page_size, max_pages=p.block_table.shape[1],
-                               num_pages=p.k_cache.shape[0], kv_dtype=pkv.KV_E4M3, k_scale=self.dks, v_scale=self.dvs)
+                               num_pages=p.k_cache.shape[0], kv_dtype=kind, k_scale=self.dks, v_scale=self.dvs)
         self.out = torch.full((p.B, p.Hq, p.d), float("nan"), dtype=torch.float16, device="cuda")
         self.lse = torch.full((p.B, p.Hq), float("nan"), dtype=torch.float32, device="cuda")
 
     def oracle(self):
         p = self.p
         return pkv_oracle.attention_fp8(p.q, self.k8, self.v8, self.ks, self.vs, p.block_table, p.seq_lens, Hkv=p.Hkv,
-                                        page_size=p.page_size, scale=p.scale)
+                                        page_size=p.page_size, scale=p.scale, kv_kind=2 if self.kind == pkv.KV_INT8 else 1)
 
     def decode(self, pol):
         ws = pkv.alloc_workspace(self.shape, pol)
@@ -61,10 +66,11 @@ def _check(fp, pol, ref, what):
     return ws
 
 
+@pytest.mark.parametrize("kind", [pkv.KV_E4M3, pkv.KV_INT8])
 @pytest.mark.parametrize("Hkv", [8, 4])
 @pytest.mark.parametrize("P", [16, 32])
-def test_fp8_ragged_sweep(Hkv, P):
-    fp = Fp8Problem(RAGGED, seed=1000 + Hkv + P, Hkv=Hkv, page_size=P)
+def test_fp8_ragged_sweep(Hkv, P, kind):
+    fp = Fp8Problem(RAGGED, seed=1000 + Hkv + P, Hkv=Hkv, page_size=P, kind=kind)
     ref = fp.oracle()
     for hg in (0, 1, 2, 4, 8):
         if hg > Hkv:
@@ -113,3 +119,24 @@ def test_fp8_unsupported_combinations_are_refused():
     f16 = Fp8Problem([100], seed=1201, Hkv=16)          # G = 2
     with pytest.raises(pkv.PkvError):
         f16.decode(pkv.Policy(tile_tokens=32, num_splits=2))
+
+
+def test_int8_all_byte_values_and_token_counts():
+    """INT8 caches: every byte value -128 .. 127 appears in K and V (the in-register int8 -> FP16
+    conversion is exact for all of them, so the result matches the oracle as closely as FP16 caches
+    do), unit scales through NULL pointers, and the K = 0 counting pin."""
+    fp = Fp8Problem([600, 33, 4097], seed=1500, scales=False, kind=pkv.KV_INT8)
+    rng = np.random.Generator(np.random.PCG64(4))
+    fp.k8 = (rng.integers(-3, 4, size=fp.k8.shape)).astype(np.int8).view(np.uint8)      # small keys: soft attention
+    fp.v8 = rng.integers(-128, 128, size=fp.v8.shape).astype(np.int8).view(np.uint8)     # every byte value
+    assert len(np.unique(fp.v8)) == 256
+    fp.k, fp.v = to_dev(fp.k8), to_dev(fp.v8)
+    ref = fp.oracle()
+    for pol in (pkv.Policy(tile_tokens=32, num_splits=4), pkv.Policy(tile_tokens=32, num_splits=1, heads_per_cta=2)):
+        out, lse, _ = fp.decode(pol)
+        assert np.abs(out - ref[0]).max() <= 0.05 and np.abs(out - ref[0]).max() / np.abs(ref[0]).max() <= 2e-3
+        assert np.abs(lse - ref[1]).max() <= 2e-3
+    fp.k8[...] = 0
+    fp.k = to_dev(fp.k8)
+    out, lse, _ = fp.decode(pkv.Policy(tile_tokens=32, num_splits=7))
+    assert np.allclose(lse, np.log(np.array([600, 33, 4097], dtype=np.float64))[:, None], atol=1e-5)
