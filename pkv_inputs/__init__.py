@@ -19,6 +19,7 @@ concrete lengths):
   that dereferences them faults instead of silently reading a valid page.
 * q, K, V ~ N(0,1) rounded to FP16; the whole pool is filled, holes included.
 """
+from .serving import ServingStep, ServingTrace  # noqa: F401
 from .workloads import (  # noqa: F401
     PAD_PAGE,
     Workload,

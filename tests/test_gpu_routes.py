@@ -102,3 +102,43 @@ def test_table4_launch_fan_out_on_a_bimodal_b8_step():
     cw = pkv.pkv_get_counters(dp.shape, pw, ws)
     assert (cw["decode_launches"] + cw["merge_launches"], cw["merge_launches"]) == (2, 1)
     assert (cw["launched_decode"], cw["launched_merge"]) == (1, 1)
+
+
+@pytest.mark.parametrize("family", ["bimodal", "bucketed"])
+def test_serving_loop_with_arrivals_and_finishes(family):
+    """A continuous-decode loop (PAPER.md:93): requests arrive, grow by one token per step and finish;
+    slots go empty and are re-used with other pages.  Every step runs through pkv.HostDecoder with
+    PKV_SPLIT_AUTO (the cost model re-plans per step) on one (staging, scratch) pair; every third step
+    is checked against the oracle, and all rows of empty slots must be zero."""
+    from gpu_helpers import oracle_attention
+    from helpers import Problem, default_scale
+    tr = pkv_inputs.ServingTrace(family, seed=21, requests=14, max_active=6, decode_lo=4, decode_hi=12, prompt_div=8)
+    k = pkv_inputs.fill_normal_f16((tr.num_pages, 16, 8, 128), 31)
+    v = pkv_inputs.fill_normal_f16((tr.num_pages, 16, 8, 128), 32)
+    q = pkv_inputs.fill_normal_f16((6, 32, 128), 33)
+    dk, dv = to_dev(k), to_dev(v)
+    shape = pkv.Shape(B=6, Hq=32, Hkv=8, max_pages=tr.max_pages, num_pages=tr.num_pages)
+    pol = pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_AUTO, num_splits=0)
+    nb = pkv.pkv_host_scratch_bytes(shape, pol)
+    staging = torch.zeros(nb, dtype=torch.uint8).pin_memory()
+    scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    ws = pkv.alloc_workspace(shape, pol)
+    out = torch.full((6, 32, 128), float("nan"), dtype=torch.float16).pin_memory()
+    dec = pkv.HostDecoder(shape, pol, dk, dv, staging, scratch, ws, default_scale(128))
+    steps = empties = checked = 0
+    for st in tr.steps():
+        lens = np.ascontiguousarray(st.seq_lens)
+        table = np.ascontiguousarray(st.block_table)
+        dec(q.ctypes.data, table.ctypes.data, lens.ctypes.data, out.data_ptr())
+        got = out.numpy().astype(np.float64)
+        assert not np.isnan(got).any()
+        for s in range(6):
+            if lens[s] == 0:
+                assert np.all(got[s] == 0)
+                empties += 1
+        if st.step % 3 == 0 or st.started or st.finished:
+            p = Problem(q=q, k_cache=k, v_cache=v, block_table=table, seq_lens=lens, Hkv=8, page_size=16, scale=default_scale(128))
+            assert_within_tolerance(got, oracle_attention(p)[0], "step %d" % st.step)
+            checked += 1
+        steps += 1
+    assert steps > 20 and empties > 0 and checked > 10
