@@ -284,7 +284,7 @@ PKV_API pkv_status pkv_decode_indexed(const pkv_shape* shape, const pkv_split_po
  *                  pairing (channel c < d/2 with c + d/2); both NULL = no rotation.  The rotation is
  *                  evaluated in FP32 product by product (no FMA) and rounded to FP16, so the bytes in
  *                  the pool are reproducible by a plain CPU restatement.
- * TMA kernel, FP16 caches, G <= 8 only (else PKV_ERR_UNSUPPORTED).  Otherwise as pkv_decode with
+ * TMA kernel, FP16 caches, d = 128, G <= 8 only (else PKV_ERR_UNSUPPORTED).  Otherwise as pkv_decode with
  * build_queue = 1; row_index may be NULL.
  */
 typedef struct {

@@ -134,11 +134,14 @@ __device__ __forceinline__ void append_patch(const DecodeParams& p, uint32_t sb,
 }
 
 // KVT: pkv_kv_dtype of the caches (0 FP16, 1 FP8 E4M3, 2 INT8); "FP8" below means any one-byte cache.
-template <int G, int HG, int D, int KVT>
+// APP: the fused KV-append (+RoPE) step (pkv_decode_append); compiled apart because its extra live
+// values cost the plain step 21 registers and 0.17 us (config 2: 23.83 vs 23.66 us).
+template <int G, int HG, int D, int KVT, bool APP>
 __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 1)
     pkv_decode_tma_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap_k,
                           const __grid_constant__ CUtensorMap tmap_v) {
     constexpr bool FP8 = KVT != 0;
+    static_assert(!APP || (KVT == 0 && G <= 8 && D == 128), "fused append: FP16 caches, G <= 8, d = 128");
     static_assert(!FP8 || D == 128, "one-byte caches: one 128-byte swizzled row per token and head");
     constexpr int kStages = stages_for<G, HG, D, FP8>();
     constexpr int kHeadBytes = D * (FP8 ? 16 : 32);   // one head's 16 tokens x D channels of K (or V): blocks of 2 KiB
@@ -489,7 +492,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
             // the same fragment slot of k-step kk + KK/2 -- in FP32, product by product, as the oracle.
             bool patch = false;
             int last_blk = -1, last_row = 0;
-            if constexpr (!FP8 && NBK == 1) {
+            if constexpr (APP) {
                 if (p.k_new != nullptr) {
                     const int pos = u.nlen - 1;
                     patch = tok1 == u.nlen;            // this unit's range ends with the row's new token
@@ -546,7 +549,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 mbar_wait(fullk0 + 8 * s, par);
                 if (k == 0 && first_page && cw == 0 && lane == 0) PKV_TRACE_STAMP(p, 4);
                 first_page = false;
-                if constexpr (!FP8 && NBK == 1) {
+                if constexpr (APP) {
                     // the block that holds the row's new token: its K row comes from k_new (rotated), not
                     // from the pool -- patched into the stage here and written to the pool for later steps
                     if (patch && p0 + j == last_blk)
@@ -616,7 +619,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
 
                 // ---- O^T += V^T . P^T
                 mbar_wait(fullv0 + 8 * s, par);
-                if constexpr (!FP8 && NBK == 1) {
+                if constexpr (APP) {
                     if (patch && p0 + j == last_blk)
                         append_patch<D, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
                 }
@@ -746,7 +749,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     }
 }
 
-template <int G, int HG, int D, int KVT>
+template <int G, int HG, int D, int KVT, bool APP = false>
 cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, const CUtensorMap& mv,
                        cudaStream_t stream) {
     constexpr int smem = stages_for<G, HG, D, KVT != 0>() * stage_bytes_for(HG, D, KVT != 0) + (int)sizeof(SmemTail<G / blocks_for(G), D>) + 1024;
@@ -758,11 +761,11 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64 || !attr_set[dev]) {
-        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG, D, KVT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        e = cudaFuncSetAttribute(pkv_decode_tma_kernel<G, HG, D, KVT, APP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
-    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG, D, KVT>, dim3(grid), dim3(threads),
+    return launch_pdl(!(p.plan.flags & PKV_FLAG_NO_PDL), pkv_decode_tma_kernel<G, HG, D, KVT, APP>, dim3(grid), dim3(threads),
                       (size_t)smem, stream, p, mk, mv);
 }
 
@@ -775,6 +778,15 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int k
     if (grid <= 0) return cudaSuccess;
     const CUtensorMap& mk = *reinterpret_cast<const CUtensorMap*>(tmap_k);
     const CUtensorMap& mv = *reinterpret_cast<const CUtensorMap*>(tmap_v);
+    const bool app = p.k_new != nullptr;
+#define PKV_CASE_APP(GG, HH) \
+    if (G == GG && HG == HH && D == 128 && kvt == 0 && app) return launch_one<GG, HH, 128, 0, true>(p, grid, mk, mv, stream);
+    PKV_CASE_APP(4, 8) PKV_CASE_APP(4, 4) PKV_CASE_APP(4, 2) PKV_CASE_APP(4, 1)
+    PKV_CASE_APP(8, 8) PKV_CASE_APP(8, 4) PKV_CASE_APP(8, 2) PKV_CASE_APP(8, 1)
+    PKV_CASE_APP(2, 8) PKV_CASE_APP(2, 4) PKV_CASE_APP(2, 2) PKV_CASE_APP(2, 1)
+    PKV_CASE_APP(1, 8) PKV_CASE_APP(1, 4) PKV_CASE_APP(1, 2) PKV_CASE_APP(1, 1)
+#undef PKV_CASE_APP
+    if (app) return cudaErrorInvalidValue;
 #define PKV_CASE(GG, HH, DD) \
     if (G == GG && HG == HH && D == DD && kvt == 0) return launch_one<GG, HH, DD, 0>(p, grid, mk, mv, stream);
     PKV_CASE(4, 8, 128) PKV_CASE(4, 4, 128) PKV_CASE(4, 2, 128) PKV_CASE(4, 1, 128)
