@@ -602,7 +602,8 @@ def run_e2e(pkv, torch, runner, K, W, auto=False):
     """K steps through pkv_decode_host: host planning + H2D + launches + D2H + sync per step, wall
     clock over the K calls.  KV pools stay resident (the model's state).  auto: the policy is
     PKV_SPLIT_AUTO, i.e. the cost model runs inside every call on that step's lengths."""
-    w, pol = runner.w, runner.pol
+    w = runner.w
+    pol = dataclasses.replace(runner.pol, flags=runner.pol.flags | pkv.FLAG_OUT_PINNED)    # out_host below is pinned for good
     ws = runner.ws
     if auto:
         pol = dataclasses.replace(pol, split_mode=pkv.SPLIT_AUTO, num_splits=0)

@@ -123,7 +123,13 @@ typedef enum {
     /* Test only: the TMA decode kernel discards the plan it made speculatively before its dependency
      * wait and plans again afterwards -- the path taken when the kernel right before pkv_decode wrote
      * seq_lens. */
-    PKV_FLAG_TEST_REPLAN = 8
+    PKV_FLAG_TEST_REPLAN = 8,
+    /* pkv_decode_host: the caller promises that out_host is pinned, device-mapped host memory that
+     * stays registered while it is passed to the library.  The device address is then looked up once
+     * per buffer (per thread) instead of in every call (a pointer query costs about a microsecond).
+     * Without the flag every call asks the driver, so a buffer that was freed and whose address was
+     * reused can never be mistaken for a mapped one. */
+    PKV_FLAG_OUT_PINNED = 16
 } pkv_flag;
 /* bits of pkv_counters.error_word (sticky in the workspace until its init bytes are zeroed again) */
 typedef enum { PKV_DEVERR_QUEUE_OVERFLOW = 1, PKV_DEVERR_SEQ_LEN = 2, PKV_DEVERR_PAGE_ID = 4 } pkv_device_error;

@@ -22,7 +22,7 @@ ROUTE_RECT, ROUTE_WORKQUEUE = 0, 1
 MERGE_SEPARATE, MERGE_FUSED = 0, 1
 SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK, SPLIT_BALANCED, SPLIT_AUTO = 0, 1, 2, 3
 KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT = 0, 1, 2
-FLAG_VALIDATE, FLAG_NO_PDL, FLAG_SEPARATE_BUILD, FLAG_TEST_REPLAN = 1, 2, 4, 8
+FLAG_VALIDATE, FLAG_NO_PDL, FLAG_SEPARATE_BUILD, FLAG_TEST_REPLAN, FLAG_OUT_PINNED = 1, 2, 4, 8, 16
 DEVERR_QUEUE_OVERFLOW, DEVERR_SEQ_LEN, DEVERR_PAGE_ID = 1, 2, 4
 STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL = 1, 2, 4, 7
 KV_F16, KV_E4M3, KV_INT8 = 0, 1, 2

@@ -20,7 +20,9 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 BUILD_DIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpkv.so")
 
-SOURCES = ["pkv_host.cpp", "pkv_aux.cu", "pkv_decode_simt.cu", "pkv_decode_tma.cu", "pkv_api.cu", "pkv_calibrate.cu"]
+TMA_PARTS = 7      # pkv_decode_tma.cu is compiled once per group of instantiations (-DPKV_TMA_PART=k), in parallel
+SOURCES = (["pkv_host.cpp", "pkv_aux.cu", "pkv_decode_simt.cu", "pkv_api.cu", "pkv_calibrate.cu"]
+           + [("pkv_decode_tma.cu", k) for k in range(TMA_PARTS)])
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", INCLUDE, "-I", CSRC]
 
@@ -49,10 +51,11 @@ def build(force: bool = False, verbose: bool = False, trace: bool = False) -> st
     os.makedirs(bdir, exist_ok=True)
     objs = []
 
-    def compile_one(src):
-        obj = os.path.join(bdir, os.path.splitext(src)[0] + ".o")
+    def compile_one(item):
+        src, part = item if isinstance(item, tuple) else (item, None)
+        obj = os.path.join(bdir, os.path.splitext(src)[0] + ("" if part is None else "_part%d" % part) + ".o")
         cmd = ([nvcc] + ARCH + COMMON + (["-DPKV_TRACE"] if trace else []) + (["-Xptxas", "-v"] if verbose else [])
-               + ["-c", os.path.join(CSRC, src), "-o", obj])
+               + ([] if part is None else ["-DPKV_TMA_PART=%d" % part]) + ["-c", os.path.join(CSRC, src), "-o", obj])
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (src, r.stdout, r.stderr))

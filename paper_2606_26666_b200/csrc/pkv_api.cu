@@ -607,25 +607,27 @@ HostImage host_image(const pkv_shape& s) {
     return h;
 }
 
-// Device pointer of a pinned, device-mapped host buffer (else nullptr).  The last answers are cached
-// per thread (serving loops pass the same few buffers every step; a cudaPointerGetAttributes call
-// costs more than a microsecond).  A buffer that is freed and re-registered at the same address
-// keeps its mapping, so a stale hit is still a valid answer for pinned memory; a pageable buffer is
-// never cached as mapped.
-void* mapped_device_pointer(const void* host, size_t align) {
+// Device pointer of a pinned, device-mapped host buffer (else nullptr).  use_cache (the caller set
+// PKV_FLAG_OUT_PINNED: the buffer stays registered while the library sees it): the last answers are
+// kept per thread, a serving loop passes the same few buffers every step and a pointer query costs
+// about a microsecond.  Without it the driver is asked every time.
+void* mapped_device_pointer(const void* host, size_t align, bool use_cache) {
     struct Entry { const void* host; void* dev; };
     thread_local Entry cache[8] = {};
     thread_local int next = 0;
     for (const Entry& e : cache)
-        if (e.host == host && host != nullptr) return reinterpret_cast<uintptr_t>(e.dev) % align == 0 ? e.dev : nullptr;
+        if (use_cache && e.host == host && host != nullptr && e.dev != nullptr)
+            return reinterpret_cast<uintptr_t>(e.dev) % align == 0 ? e.dev : nullptr;
     cudaPointerAttributes attr;
     void* dev = nullptr;
     if (cudaPointerGetAttributes(&attr, host) == cudaSuccess && attr.type == cudaMemoryTypeHost && attr.devicePointer != nullptr)
         dev = attr.devicePointer;
     else
         (void)cudaGetLastError();   // an unregistered host pointer is not an error here
-    cache[next] = Entry{host, dev};
-    next = (next + 1) % 8;
+    if (use_cache && dev != nullptr) {
+        cache[next] = Entry{host, dev};
+        next = (next + 1) % 8;
+    }
     return reinterpret_cast<uintptr_t>(dev) % align == 0 ? dev : nullptr;
 }
 
@@ -775,7 +777,7 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
     // Pinned (page-locked, device-mapped) out_host: the kernels write the FP16 result straight
     // into it -- 8 KiB of posted writes per row -- and the D2H copy disappears from the step.
     // Pageable out_host: result in dev_scratch, then one cudaMemcpyAsync.
-    void* out_dev = mapped_device_pointer(out_host, 16);
+    void* out_dev = mapped_device_pointer(out_host, 16, (rp.flags & PKV_FLAG_OUT_PINNED) != 0);
     const bool zero_copy_out = out_dev != nullptr;
     if (!zero_copy_out) out_dev = ds + im.out;
     const bool fused = rp.kernel == PKV_KERNEL_TMA_MMA && !(rp.flags & PKV_FLAG_SEPARATE_BUILD) && s.B <= kMaxFusedRows;

@@ -771,6 +771,48 @@ cudaError_t launch_one(const DecodeParams& p, int grid, const CUtensorMap& mk, c
 
 }  // namespace
 
+template <int PART>
+cudaError_t launch_decode_tma_part(const DecodeParams& p, int G, int HG, int D, int kvt, bool app, int grid, const CUtensorMap& mk,
+                                   const CUtensorMap& mv, cudaStream_t stream);
+
+// The 65 instantiations are compiled as kTmaParts translation units of this one source
+// (-DPKV_TMA_PART=k, see build.py): part k defines launch_decode_tma_part<k>, which launches the
+// kernel if the requested instantiation belongs to it and returns cudaErrorNotSupported otherwise;
+// part 0 also holds the dispatcher.
+#ifndef PKV_TMA_PART
+#define PKV_TMA_PART 0
+#endif
+
+#define PKV_CASE(GG, HH, DD, KK, AA) \
+    if (G == GG && HG == HH && D == DD && kvt == KK && app == AA) return launch_one<GG, HH, DD, KK, AA>(p, grid, mk, mv, stream);
+#define PKV_CASE_HG(GG, DD, KK, AA) PKV_CASE(GG, 8, DD, KK, AA) PKV_CASE(GG, 4, DD, KK, AA) PKV_CASE(GG, 2, DD, KK, AA) PKV_CASE(GG, 1, DD, KK, AA)
+#define PKV_CASE_HG4(GG, DD, KK, AA) PKV_CASE(GG, 4, DD, KK, AA) PKV_CASE(GG, 2, DD, KK, AA) PKV_CASE(GG, 1, DD, KK, AA)
+
+template <>
+cudaError_t launch_decode_tma_part<PKV_TMA_PART>(const DecodeParams& p, int G, int HG, int D, int kvt, bool app, int grid,
+                                                 const CUtensorMap& mk, const CUtensorMap& mv, cudaStream_t stream) {
+#if PKV_TMA_PART == 0      // the paper's shapes: FP16, d = 128, G = 4 and 8
+    PKV_CASE_HG(4, 128, 0, false) PKV_CASE_HG(8, 128, 0, false)
+#elif PKV_TMA_PART == 1    // G = 1, 2 and 16 (two blocks of 8 query heads: at most 4 heads per CTA)
+    PKV_CASE_HG(2, 128, 0, false) PKV_CASE_HG(1, 128, 0, false) PKV_CASE_HG4(16, 128, 0, false)
+#elif PKV_TMA_PART == 2    // head dimensions 64 and 256 (d = 256: at most 4 heads per CTA, a stage of 8 would be 128 KiB)
+    PKV_CASE_HG(4, 64, 0, false) PKV_CASE_HG(8, 64, 0, false) PKV_CASE_HG4(4, 256, 0, false) PKV_CASE_HG4(8, 256, 0, false)
+#elif PKV_TMA_PART == 3    // FP8 (E4M3) caches
+    PKV_CASE_HG(4, 128, 1, false) PKV_CASE_HG(8, 128, 1, false)
+#elif PKV_TMA_PART == 4    // INT8 caches
+    PKV_CASE_HG(4, 128, 2, false) PKV_CASE_HG(8, 128, 2, false)
+#elif PKV_TMA_PART == 5    // fused KV-append + RoPE, G = 4 and 8
+    PKV_CASE_HG(4, 128, 0, true) PKV_CASE_HG(8, 128, 0, true)
+#elif PKV_TMA_PART == 6    // fused KV-append + RoPE, G = 1 and 2
+    PKV_CASE_HG(2, 128, 0, true) PKV_CASE_HG(1, 128, 0, true)
+#endif
+    return cudaErrorNotSupported;
+}
+#undef PKV_CASE_HG4
+#undef PKV_CASE_HG
+#undef PKV_CASE
+
+#if PKV_TMA_PART == 0
 int decode_tma_stage_bytes(int HG, int D, bool fp8) { return stage_bytes_for(HG, D, fp8); }
 
 cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int kvt, int grid, const void* tmap_k,
@@ -779,35 +821,15 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int k
     const CUtensorMap& mk = *reinterpret_cast<const CUtensorMap*>(tmap_k);
     const CUtensorMap& mv = *reinterpret_cast<const CUtensorMap*>(tmap_v);
     const bool app = p.k_new != nullptr;
-#define PKV_CASE_APP(GG, HH) \
-    if (G == GG && HG == HH && D == 128 && kvt == 0 && app) return launch_one<GG, HH, 128, 0, true>(p, grid, mk, mv, stream);
-    PKV_CASE_APP(4, 8) PKV_CASE_APP(4, 4) PKV_CASE_APP(4, 2) PKV_CASE_APP(4, 1)
-    PKV_CASE_APP(8, 8) PKV_CASE_APP(8, 4) PKV_CASE_APP(8, 2) PKV_CASE_APP(8, 1)
-    PKV_CASE_APP(2, 8) PKV_CASE_APP(2, 4) PKV_CASE_APP(2, 2) PKV_CASE_APP(2, 1)
-    PKV_CASE_APP(1, 8) PKV_CASE_APP(1, 4) PKV_CASE_APP(1, 2) PKV_CASE_APP(1, 1)
-#undef PKV_CASE_APP
-    if (app) return cudaErrorInvalidValue;
-#define PKV_CASE(GG, HH, DD) \
-    if (G == GG && HG == HH && D == DD && kvt == 0) return launch_one<GG, HH, DD, 0>(p, grid, mk, mv, stream);
-    PKV_CASE(4, 8, 128) PKV_CASE(4, 4, 128) PKV_CASE(4, 2, 128) PKV_CASE(4, 1, 128)
-    PKV_CASE(8, 8, 128) PKV_CASE(8, 4, 128) PKV_CASE(8, 2, 128) PKV_CASE(8, 1, 128)
-    PKV_CASE(2, 8, 128) PKV_CASE(2, 4, 128) PKV_CASE(2, 2, 128) PKV_CASE(2, 1, 128)
-    PKV_CASE(1, 8, 128) PKV_CASE(1, 4, 128) PKV_CASE(1, 2, 128) PKV_CASE(1, 1, 128)
-    PKV_CASE(16, 4, 128) PKV_CASE(16, 2, 128) PKV_CASE(16, 1, 128)
-    // head dimensions 64 and 256: the paper's GQA shapes G = 4 and G = 8
-    PKV_CASE(4, 8, 64) PKV_CASE(4, 4, 64) PKV_CASE(4, 2, 64) PKV_CASE(4, 1, 64)
-    PKV_CASE(8, 8, 64) PKV_CASE(8, 4, 64) PKV_CASE(8, 2, 64) PKV_CASE(8, 1, 64)
-    PKV_CASE(4, 4, 256) PKV_CASE(4, 2, 256) PKV_CASE(4, 1, 256)   // d = 256: at most 4 heads per CTA
-    PKV_CASE(8, 4, 256) PKV_CASE(8, 2, 256) PKV_CASE(8, 1, 256)   // (a stage of 8 would be 128 KiB)
-#undef PKV_CASE
-#define PKV_CASE8(GG, HH) \
-    if (G == GG && HG == HH && D == 128 && kvt == 1) return launch_one<GG, HH, 128, 1>(p, grid, mk, mv, stream); \
-    if (G == GG && HG == HH && D == 128 && kvt == 2) return launch_one<GG, HH, 128, 2>(p, grid, mk, mv, stream);
-    // one-byte caches (FP8 E4M3, INT8): d = 128, G = 4 and 8
-    PKV_CASE8(4, 8) PKV_CASE8(4, 4) PKV_CASE8(4, 2) PKV_CASE8(4, 1)
-    PKV_CASE8(8, 8) PKV_CASE8(8, 4) PKV_CASE8(8, 2) PKV_CASE8(8, 1)
-#undef PKV_CASE8
-    return cudaErrorInvalidValue;
+    cudaError_t e = launch_decode_tma_part<0>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<1>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<2>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<3>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<4>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<5>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<6>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    return e == cudaErrorNotSupported ? cudaErrorInvalidValue : e;
 }
+#endif
 
 }  // namespace pkv
