@@ -26,8 +26,9 @@
  *     (pkv_counters.error_word) and keep the kernels inside the caller's buffers (PAPER.md:67:
  *     every bound is derived from N_i).  seq_lens[i] == 0 is legal: the row emits no task,
  *     out[i] = 0 and lse[i] = -inf (reading A9).
- *   - compiled-in shapes: d = 128, page_size = 16, FP16, G = Hq/Hkv in {1, 2, 4, 8}.  Anything else
- *     returns PKV_ERR_UNSUPPORTED.
+ *   - compiled-in shapes: G = Hq/Hkv in {1, 2, 4, 8, 16}, page_size in {16, 32, 64}, d = 128; d in
+ *     {64, 256} and one-byte caches (FP8 E4M3, INT8; d = 128) for G in {4, 8} on the TMA kernel; the
+ *     fused KV-append for FP16 caches, d = 128, G <= 8.  Anything else returns PKV_ERR_UNSUPPORTED.
  */
 #ifndef PKV_H_
 #define PKV_H_
@@ -233,8 +234,9 @@ PKV_API pkv_status pkv_build_workqueue(const pkv_shape* shape, const pkv_split_p
  * still running.  It then reads nothing but seq_lens (race-tolerant loads, for a speculative
  * plan) before that kernel has finished, and re-validates those lengths afterwards -- a
  * predecessor that writes seq_lens, q, the block table or the caches is handled correctly.
- * Heads per CTA: the TMA kernel streams HG = 8, 4, 2 or 1 KV heads per CTA, the largest value
- * that still leaves one work unit per SM given the bound B*S on the (row, split) pairs; with
+ * Heads per CTA: the TMA kernel streams HG = 8, 4, 2 or 1 KV heads per CTA (at most 4 with G = 16 or
+ * d = 256), the largest value that still leaves work units for 85 % of the SMs given the bound B*S on
+ * the (row, split) pairs; with
  * BALANCED the bound is policy.num_sms, so num_sms = SMs*HG/Hkv asks for HG heads per CTA
  * (policy.heads_per_cta overrides the choice).
  * L2 prefetch: before its dependency wait a CTA of the TMA kernel also asks the memory system to
