@@ -9,4 +9,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 * ``workqueue_oracle.py`` -- the split-bound policy and the compact workqueue as a pure-Python
   integer algorithm, plus the scheduler-derived counters of Table 4
   (PAPER.md:183-192).
+* ``route_oracle.py`` -- the length-bucket route and the calibrated cost model
+  with its gates and margins; the makespan form of its first term (A27).
+* ``append_oracle.py`` -- the fused KV-append + RoPE step (PAPER.md:271 future work; A29).
+* ``pkv_oracle.attention_fp8`` / ``attention_int8`` -- Eq. (1) on one-byte caches (A28).
 """
