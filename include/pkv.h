@@ -272,7 +272,9 @@ PKV_API pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_pol
  * row_index[i] (dev int32 [B], values in [0, rows of the caller's arrays)) of q, out, lse,
  * block_table AND seq_lens -- nothing is gathered or scattered by the caller.  The queue in the
  * workspace is in launch rows (pkv_task.row = i).  At most 512 rows per call.  Otherwise as
- * pkv_decode with build_queue = 1.
+ * pkv_decode with build_queue = 1.  The workspace layout depends on shape->B: keep one workspace per
+ * subset size (or zero its init bytes again when B changes); pkv_decode_buckets lays every bucket
+ * out for the whole batch and has no such restriction.
  */
 PKV_API pkv_status pkv_decode_indexed(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
                                       const void* k_cache, const void* v_cache, const int32_t* block_table,
