@@ -34,8 +34,9 @@ Readings of what the paper leaves open:
       decides:  stream = max(KVBytes/beta, max_share/beta_cta).  The library's persistent CTA takes
       units of HG KV heads (HG = the largest of 8, 4, 2, 1 dividing Hkv that leaves units for >= 85 % of
       the SMs, else 1 -- the smallest valid group when nothing fills the machine): one wave (units <= #SMs):
-      max_share = the largest unit's bytes; several waves (dynamic hand-out): KVBytes/#SMs + the
-      largest unit's bytes.  A CTA that reads HG heads' slices of every page instead of whole pages
+      max_share = the largest unit's bytes; several waves: KVBytes/#SMs + the largest unit's bytes
+      when units are handed out dynamically (HG = 8), waves x the largest unit's bytes when they are
+      dealt round-robin (HG < 8: several warps share a head).  A CTA that reads HG heads' slices of every page instead of whole pages
       streams at beta * eta(HG), eta = 1 / 0.96 / 0.94 / 0.87 for HG = 8 / 4 / 2 / 1 (measured).
 
 Pins (tests/test_route_oracle.py): Table 4's bucket row (16.00 / 73.1 / 4.06 / 8.00), the cost of
@@ -209,7 +210,11 @@ def max_share_bytes(seq_lens: Sequence[int], Hkv: int, d: int, q: wq.WorkQueue, 
     unit = max(tokens, 0) * 2 * hg * d * 2
     units = row_slots * (Hkv // hg)
     kv = wq.useful_kv_bytes(seq_lens, Hkv, d)
-    return unit if units <= num_sms else kv // num_sms + unit
+    if units <= num_sms:
+        return unit
+    if hg == 8:                      # dynamic hand-out (G <= 8: one warp per head at HG = 8)
+        return kv // num_sms + unit
+    return wq.ceil_div(units, num_sms) * unit      # round-robin: the busiest CTA may draw only largest units
 
 
 HEAD_SLICE_EFFICIENCY = {8: 1.0, 4: 0.96, 2: 0.94, 1: 0.87}    # A27, measured on B200 (config 2, decode kernel alone)

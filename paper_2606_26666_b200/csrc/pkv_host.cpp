@@ -253,7 +253,11 @@ void launch_totals(const pkv_shape& s, const Resolved& rp, const int32_t* lens, 
         const int hg = choose_heads_per_cta(rp.heads_per_cta, s.Hkv, hdr.total_row_slots, num_sms, max_heads_per_cta(rp.G, s.d));
         const int64_t unit = (int64_t)max_tok * 2 * hg * s.d * (s.kv_dtype != PKV_KV_F16 ? 1 : 2);
         const int64_t units = (int64_t)hdr.total_row_slots * (s.Hkv / hg);
-        t->max_share = units <= num_sms ? unit : t->kv_bytes / num_sms + unit;
+        // several waves: units are handed out dynamically when every (head, block) group of a CTA is one
+        // warp (HG x blocks = 8), else round-robin -- then the busiest CTA may draw only largest units
+        const bool dynamic = hg * (rp.G == 16 ? 2 : 1) == 8;
+        const int64_t waves = (units + num_sms - 1) / num_sms;
+        t->max_share = units <= num_sms ? unit : (dynamic ? t->kv_bytes / num_sms + unit : waves * unit);
         t->units = units;
         t->slice_eff = head_slice_efficiency(hg);
     }

@@ -148,8 +148,8 @@ def test_p15_makespan_form_reduces_to_the_papers_term_for_equal_tasks():
     # 3 SMs: 4 units on 3 SMs = several waves: KV / SMs + the largest unit
     kv = 1100 * 4096
     assert ro.max_share_bytes([100, 1000], 8, 128, q, 32, 3) == kv // 3 + 512 * 4096
-    # 5 SMs: 4 units of 8 heads cover only 80 % of them, so hg = 4: 8 units, several waves
+    # 5 SMs: 4 units of 8 heads cover only 80 % of them, so hg = 4: 8 units in 2 round-robin waves
     assert ro.heads_per_cta(8, 4, 5) == 4
-    assert ro.max_share_bytes([100, 1000], 8, 128, q, 32, 5) == kv // 5 + 512 * 2048
+    assert ro.max_share_bytes([100, 1000], 8, 128, q, 32, 5) == 2 * 512 * 2048
     # 148 SMs: nothing fills the machine, hg = 1: 32 units, one wave, 512 tokens of one head
     assert ro.max_share_bytes([100, 1000], 8, 128, q, 32, 148) == 512 * 512
