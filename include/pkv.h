@@ -266,6 +266,34 @@ PKV_API pkv_status pkv_decode_stages(const pkv_shape* shape, const pkv_split_pol
                                      uint32_t stages, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * Allocation-free entry point: pkv_decode(build_queue = 1) for callers that cannot provide device
+ * scratch memory (code under CUDA graph capture, serving loops and harnesses that forbid
+ * cudaMalloc).  The step's scratch -- queue header and counters, split_offsets, task list and the
+ * split-local partial states (m, l, acc) of PAPER.md:56 and 71-75 -- lives in ONE static array of
+ * PKV_STATIC_WORKSPACE_BYTES in the library's device image; every GPU that loads the library holds
+ * those bytes until the process exits.  The caller passes inputs and outputs only (device pointers,
+ * same meaning, layout and ownership as for pkv_decode).  The call makes no cudaMalloc / cudaFree and
+ * calls no allocating library routine; it launches one small clear kernel (the layout's
+ * pkv_workspace_init_bytes must start at zero and the array keeps the previous call's contents)
+ * and then the launches of pkv_decode.
+ *   - PKV_ERR_WORKSPACE, before any CUDA call, if pkv_workspace_bytes(shape, policy) exceeds
+ *     PKV_STATIC_WORKSPACE_BYTES (pkv_last_error() states both numbers).  8 MiB holds about 500
+ *     (row, split) pairs at Hkv = 8, G = 4, d = 128: B = 1 at any split count, B = 8 up to S = 32;
+ *     BALANCED / AUTO policies size for 256 splits per row and fit only B = 1.
+ *   - All calls on one device share the array: calls that OVERLAP on the GPU (two streams) race on
+ *     it and give undefined results -- serialise them or use pkv_decode with workspaces of your own.
+ *   - The array's address is looked up once per device (cudaGetSymbolAddress, with the calling
+ *     thread's current device) on the first call on that device; make that first call outside
+ *     stream capture.  pkv_get_counters / pkv_read_workqueue have no static variant.
+ * Other errors as pkv_decode.
+ */
+#define PKV_STATIC_WORKSPACE_BYTES (8u << 20)
+PKV_API size_t pkv_static_workspace_bytes(void);   /* = PKV_STATIC_WORKSPACE_BYTES of the loaded library */
+PKV_API pkv_status pkv_decode_static(const pkv_shape* shape, const pkv_split_policy* policy, const void* q,
+                                     const void* k_cache, const void* v_cache, const int32_t* block_table,
+                                     const int32_t* seq_lens, void* out, float* lse, float scale, void* stream);
+
+/*
  * Indexed rows ("Indexed Q/O. The extension can read Q rows and write output rows by
  * index, avoiding per-bucket index_select and index_copy_"): one decode step over a SUBSET of the
  * batch's rows, in place.  shape->B = number of launch rows; launch row i works on request row

@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     pkv_version, pkv_last_error, pkv_workspace_bytes, pkv_workspace_init_bytes, pkv_host_scratch_bytes, pkv_build_workqueue_host,
     pkv_build_workqueue, pkv_decode, pkv_decode_stages, pkv_merge, pkv_get_counters, pkv_read_workqueue, pkv_workspace_partials,
     pkv_decode_host, pkv_calibrate, pkv_decode_indexed, pkv_plan_buckets_host, pkv_decode_buckets, pkv_bucket_counters_host,
+    pkv_decode_static, pkv_static_workspace_bytes,
 )
 
 

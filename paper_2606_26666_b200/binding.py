@@ -88,7 +88,8 @@ EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspac
            "pkv_build_workqueue", "pkv_decode", "pkv_decode_stages", "pkv_merge", "pkv_get_counters", "pkv_read_workqueue",
            "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate", "pkv_decode_indexed",
            "pkv_plan_buckets_host", "pkv_decode_buckets", "pkv_bucket_counters_host", "pkv_default_cost_model",
-           "pkv_estimate_cost", "pkv_choose_policy", "pkv_decode_append")
+           "pkv_estimate_cost", "pkv_choose_policy", "pkv_decode_append", "pkv_decode_static",
+           "pkv_static_workspace_bytes")
 
 
 class PkvError(RuntimeError):
@@ -121,6 +122,10 @@ def _load() -> ctypes.CDLL:
     lib.pkv_decode_stages.restype = _i32
     lib.pkv_decode_stages.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp,
                                       ctypes.c_float, ctypes.c_uint32, _vp, ctypes.c_size_t, _vp]
+    lib.pkv_static_workspace_bytes.restype = ctypes.c_size_t
+    lib.pkv_static_workspace_bytes.argtypes = []
+    lib.pkv_decode_static.restype = _i32
+    lib.pkv_decode_static.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp]
     lib.pkv_decode_indexed.restype = _i32
     lib.pkv_decode_indexed.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp,
                                        ctypes.c_float, _vp, ctypes.c_size_t, _vp]
@@ -292,6 +297,18 @@ def pkv_decode(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, s
     _check(_lib.pkv_decode(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(q), _ptr(k_cache), _ptr(v_cache),
                            _ptr(block_table), _ptr(seq_lens), _ptr(out), _ptr(lse), ctypes.c_float(scale),
                            1 if build_queue else 0, _ptr(workspace), _nbytes(workspace), _stream_ptr(stream)))
+
+
+def pkv_static_workspace_bytes() -> int:
+    return int(_lib.pkv_static_workspace_bytes())
+
+
+def pkv_decode_static(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, seq_lens, out, lse=None,
+                      scale: float = 0.0, stream=None) -> None:
+    """pkv_decode without a caller workspace: the scratch is the library's static device array."""
+    _check(_lib.pkv_decode_static(ctypes.byref(shape.c()), ctypes.byref(policy.c()), _ptr(q), _ptr(k_cache), _ptr(v_cache),
+                                  _ptr(block_table), _ptr(seq_lens), _ptr(out), _ptr(lse), ctypes.c_float(scale),
+                                  _stream_ptr(stream)))
 
 
 def pkv_decode_stages(shape: Shape, policy: Policy, q, k_cache, v_cache, block_table, seq_lens, out, lse=None,

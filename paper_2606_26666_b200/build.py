@@ -21,7 +21,7 @@ BUILD_DIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpkv.so")
 
 TMA_PARTS = 7      # pkv_decode_tma.cu is compiled once per group of instantiations (-DPKV_TMA_PART=k), in parallel
-SOURCES = (["pkv_host.cpp", "pkv_aux.cu", "pkv_decode_simt.cu", "pkv_api.cu", "pkv_calibrate.cu"]
+SOURCES = (["pkv_host.cpp", "pkv_aux.cu", "pkv_decode_simt.cu", "pkv_api.cu", "pkv_calibrate.cu", "pkv_static.cu"]
            + [("pkv_decode_tma.cu", k) for k in range(TMA_PARTS)])
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", INCLUDE, "-I", CSRC]
