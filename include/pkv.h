@@ -27,7 +27,7 @@
  *     every bound is derived from N_i).  seq_lens[i] == 0 is legal: the row emits no task,
  *     out[i] = 0 and lse[i] = -inf (reading A9).
  *   - compiled-in shapes: G = Hq/Hkv in {1, 2, 4, 8, 16}, page_size in {16, 32, 64}, d = 128; d in
- *     {64, 256} and one-byte caches (FP8 E4M3, INT8; d = 128) for G in {4, 8} on the TMA kernel; the
+ *     {64, 256} (FP16 caches) and one-byte caches (FP8 E4M3, INT8; d = 128) on the TMA kernel; the
  *     fused KV-append for FP16 caches, d = 128, G <= 8.  Anything else returns PKV_ERR_UNSUPPORTED.
  */
 #ifndef PKV_H_
@@ -157,7 +157,7 @@ typedef struct {
      * of 16) that stand for
      *   k = k_scale[kv head] * dec(byte),  v = v_scale[kv head] * dec(byte)
      * k_scale / v_scale: dev float [Hkv], or NULL for 1.0.  q and out stay FP16, arithmetic as for
-     * FP16 caches (E4M3 values are FP16 numbers).  TMA kernel, d = 128, G in {4, 8} only. */
+     * FP16 caches (E4M3 values are FP16 numbers).  TMA kernel, d = 128 only. */
     int32_t kv_dtype;                            /* pkv_kv_dtype; 0 = FP16                       */
     int32_t reserved_;
     const float* k_scale;

@@ -775,7 +775,7 @@ template <int PART>
 cudaError_t launch_decode_tma_part(const DecodeParams& p, int G, int HG, int D, int kvt, bool app, int grid, const CUtensorMap& mk,
                                    const CUtensorMap& mv, cudaStream_t stream);
 
-// The 65 instantiations are compiled as kTmaParts translation units of this one source
+// The 106 instantiations are compiled as kTmaParts translation units of this one source
 // (-DPKV_TMA_PART=k, see build.py): part k defines launch_decode_tma_part<k>, which launches the
 // kernel if the requested instantiation belongs to it and returns cudaErrorNotSupported otherwise;
 // part 0 also holds the dispatcher.
@@ -805,6 +805,14 @@ cudaError_t launch_decode_tma_part<PKV_TMA_PART>(const DecodeParams& p, int G, i
     PKV_CASE_HG(4, 128, 0, true) PKV_CASE_HG(8, 128, 0, true)
 #elif PKV_TMA_PART == 6    // fused KV-append + RoPE, G = 1 and 2
     PKV_CASE_HG(2, 128, 0, true) PKV_CASE_HG(1, 128, 0, true)
+#elif PKV_TMA_PART == 7    // FP8 (E4M3) caches, G = 1, 2 and 16
+    PKV_CASE_HG(2, 128, 1, false) PKV_CASE_HG(1, 128, 1, false) PKV_CASE_HG4(16, 128, 1, false)
+#elif PKV_TMA_PART == 8    // INT8 caches, G = 1, 2 and 16
+    PKV_CASE_HG(2, 128, 2, false) PKV_CASE_HG(1, 128, 2, false) PKV_CASE_HG4(16, 128, 2, false)
+#elif PKV_TMA_PART == 9    // d = 64, G = 1, 2 and 16
+    PKV_CASE_HG(2, 64, 0, false) PKV_CASE_HG(1, 64, 0, false) PKV_CASE_HG4(16, 64, 0, false)
+#elif PKV_TMA_PART == 10   // d = 256, G = 1, 2 and 16
+    PKV_CASE_HG4(2, 256, 0, false) PKV_CASE_HG4(1, 256, 0, false) PKV_CASE_HG4(16, 256, 0, false)
 #endif
     return cudaErrorNotSupported;
 }
@@ -828,6 +836,10 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int k
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<4>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<5>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<6>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<7>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<8>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<9>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<10>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     return e == cudaErrorNotSupported ? cudaErrorInvalidValue : e;
 }
 #endif

@@ -38,7 +38,7 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
     if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16) { set_error("G=Hq/Hkv=%d not compiled in (1, 2, 4, 8 and 16 only)", G); return PKV_ERR_UNSUPPORTED; }
     if (s.kv_dtype != PKV_KV_F16 && s.kv_dtype != PKV_KV_E4M3 && s.kv_dtype != PKV_KV_INT8) { set_error("bad kv_dtype %d", s.kv_dtype); return PKV_ERR_INVALID_ARG; }
     if (s.kv_dtype != PKV_KV_F16) {
-        if (s.d != kD || (G != 4 && G != 8)) { set_error("FP8 KV is compiled in for d=128 and G=4 or 8 only (d=%d, G=%d)", s.d, G); return PKV_ERR_UNSUPPORTED; }
+        if (s.d != kD) { set_error("one-byte KV caches are compiled in for d=128 only (d=%d)", s.d); return PKV_ERR_UNSUPPORTED; }
         if (p.kernel == PKV_KERNEL_SIMT) { set_error("FP8 KV needs the TMA kernel"); return PKV_ERR_UNSUPPORTED; }
         if (s.kv_stride_page % 16 || s.kv_stride_token % 16 || s.kv_stride_head % 16) { set_error("FP8 kv strides must be multiples of 16 bytes"); return PKV_ERR_INVALID_ARG; }
     }
@@ -81,7 +81,6 @@ pkv_status validate_and_resolve(const pkv_shape* shape, const pkv_split_policy* 
         return PKV_ERR_INVALID_ARG;
     }
     if (p.heads_per_cta > max_heads_per_cta(G, s.d)) { set_error("heads_per_cta=8 is not available with G=16 or d=256 (at most 4)"); return PKV_ERR_INVALID_ARG; }
-    if (s.d != kD && G != 4 && G != 8) { set_error("d=%d is compiled in for G=4 and G=8 only (G=%d)", s.d, G); return PKV_ERR_UNSUPPORTED; }
     if (s.d != kD && p.kernel == PKV_KERNEL_SIMT) { set_error("PKV_KERNEL_SIMT is compiled in for d=128 only"); return PKV_ERR_UNSUPPORTED; }
 
     int32_t S = p.num_splits;

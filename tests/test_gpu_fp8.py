@@ -25,8 +25,8 @@ def quantize(x: np.ndarray, scale: np.ndarray, kind: int = 1) -> np.ndarray:
 
 
 class Fp8Problem:
-    def __init__(self, lens, seed, Hkv=8, page_size=16, scales=True, kind=pkv.KV_E4M3):
-        self.p = p = make_problem(lens, seed=seed, Hkv=Hkv, page_size=page_size)
+    def __init__(self, lens, seed, Hkv=8, page_size=16, scales=True, kind=pkv.KV_E4M3, Hq=32):
+        self.p = p = make_problem(lens, seed=seed, Hq=Hq, Hkv=Hkv, page_size=page_size)
         self.kind = kind
         rng = np.random.Generator(np.random.PCG64(seed))
         lo, hi = (0.02, 0.06) if kind == pkv.KV_E4M3 else (0.04, 0.08)      # INT8: N(0,1) / scale inside +-127
@@ -112,13 +112,35 @@ def test_fp8_unit_scales_dominant_key_and_token_counts():
     assert np.allclose(lse, np.log(np.array([4097, 33, 1, 1000], dtype=np.float64))[:, None], atol=1e-5)
 
 
+@pytest.mark.parametrize("kind", [pkv.KV_E4M3, pkv.KV_INT8])
+@pytest.mark.parametrize("Hq,Hkv", [(32, 32), (32, 16), (64, 4), (32, 2)])
+def test_fp8_other_group_sizes(Hq, Hkv, kind):
+    """One-byte caches with G = 1, 2 and 16 (the paper's GQA sweep, on the caches of
+    PAPER.md:271): every heads-per-CTA variant, both routes, separate and fused merge."""
+    G = Hq // Hkv
+    fp = Fp8Problem(RAGGED, seed=1300 + Hq + Hkv, Hkv=Hkv, Hq=Hq, kind=kind)
+    ref = fp.oracle()
+    for hg in (0, 1, 2, 4, 8):
+        if hg > Hkv or (G == 16 and hg == 8):
+            continue
+        for pol in (pkv.Policy(tile_tokens=32, num_splits=1, heads_per_cta=hg),
+                    pkv.Policy(tile_tokens=32, num_splits=5, heads_per_cta=hg),
+                    pkv.Policy(tile_tokens=32, num_splits=3, heads_per_cta=hg, merge_mode=pkv.MERGE_FUSED, route=pkv.ROUTE_RECT),
+                    pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=24, heads_per_cta=hg)):
+            ws = _check(fp, pol, ref, "one-byte G%d Hkv%d hg%d %s" % (G, Hkv, hg, pol))
+    tasks, offs = pkv.pkv_read_workqueue(fp.shape, pol, ws)
+    want = wq.build_workqueue(RAGGED, Hkv, oracle_policy(pol))
+    assert tasks.tolist() == [list(t) for t in want.tasks]
+
+
 def test_fp8_unsupported_combinations_are_refused():
     fp = Fp8Problem([100], seed=1200)
     with pytest.raises(pkv.PkvError):
         fp.decode(pkv.Policy(tile_tokens=32, num_splits=2, kernel=pkv.KERNEL_SIMT))
-    f16 = Fp8Problem([100], seed=1201, Hkv=16)          # G = 2
-    with pytest.raises(pkv.PkvError):
-        f16.decode(pkv.Policy(tile_tokens=32, num_splits=2))
+    with pytest.raises(pkv.PkvError) as ei:              # one-byte caches: d = 128 only
+        pkv.pkv_workspace_partials(pkv.Shape(B=1, Hq=32, Hkv=8, d=64, page_size=16, max_pages=8, num_pages=8, kv_dtype=pkv.KV_E4M3),
+                                   pkv.Policy(tile_tokens=32, num_splits=2), torch.zeros(1 << 20, dtype=torch.uint8, device="cuda"))
+    assert ei.value.status == pkv.PKV_ERR_UNSUPPORTED
 
 
 def test_int8_all_byte_values_and_token_counts():

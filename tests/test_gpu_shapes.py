@@ -151,9 +151,32 @@ def test_head_dimensions_ragged_sweep(d, Hkv):
 
 
 @pytest.mark.parametrize("d", [64, 256])
+@pytest.mark.parametrize("Hq,Hkv", [(32, 32), (32, 16), (64, 4), (32, 2)])
+def test_head_dimensions_other_group_sizes(d, Hq, Hkv):
+    """d = 64 and d = 256 with G = 1, 2 and 16: every heads-per-CTA variant (at most 4 with G = 16 or
+    d = 256), both routes, separate / fused / channel-sliced merge."""
+    G = Hq // Hkv
+    p = make_problem(RAGGED, seed=860 + d + Hq + Hkv, Hq=Hq, Hkv=Hkv, d=d)
+    dp = DevProblem(p)
+    ref = oracle_attention(p)
+    for hg in (0, 1, 2, 4, 8):
+        if hg > Hkv or (hg == 8 and (d == 256 or G == 16)):
+            continue
+        for pol in (pkv.Policy(tile_tokens=32, num_splits=1, heads_per_cta=hg),
+                    pkv.Policy(tile_tokens=32, num_splits=5, heads_per_cta=hg),
+                    pkv.Policy(tile_tokens=32, num_splits=40, heads_per_cta=hg),
+                    pkv.Policy(tile_tokens=32, num_splits=3, heads_per_cta=hg, merge_mode=pkv.MERGE_FUSED, route=pkv.ROUTE_RECT),
+                    pkv.Policy(tile_tokens=32, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=24, heads_per_cta=hg)):
+            _, _, ws = _check(dp, pol, ref, "d%d G%d Hkv%d hg%d %s" % (d, G, Hkv, hg, pol))
+    tasks, offs = pkv.pkv_read_workqueue(dp.shape, pol, ws)
+    want = wq.build_workqueue(RAGGED, Hkv, oracle_policy(pol))
+    assert tasks.tolist() == [list(t) for t in want.tasks]
+
+
+@pytest.mark.parametrize("d", [64, 256])
 def test_head_dimensions_single_long_row_and_token_counts(d):
     """One long row (B = 1: the channel-sliced merge over 4 or 8 CTAs per head) and the K = 0
-    counting pin at d = 64 / 256; d with the SIMT kernel or another G is refused, not mis-computed."""
+    counting pin at d = 64 / 256; d with the SIMT kernel is refused, not mis-computed."""
     p = make_problem([9000], seed=900 + d, d=d)
     dp = DevProblem(p)
     ref = oracle_attention(p)
@@ -177,6 +200,3 @@ def test_head_dimensions_single_long_row_and_token_counts(d):
             assert np.all(l[slot] == min(te * 32, lens[row]) - tb * 32) and np.all(m[slot] == 0.0)
     with pytest.raises(pkv.PkvError):
         dp.decode(pkv.Policy(tile_tokens=32, num_splits=2, kernel=pkv.KERNEL_SIMT))
-    p2 = make_problem([100], seed=5, d=d, Hkv=16)
-    with pytest.raises(pkv.PkvError):
-        DevProblem(p2).decode(pkv.Policy(tile_tokens=32, num_splits=2))
