@@ -402,3 +402,95 @@ def test_int8_attention_reduces_to_the_fp16_oracle_and_to_brute_force():
     assert np.abs(got - ref).max() <= 1e-12 and np.abs(got_lse[fin] - ref_lse[fin]).max() <= 1e-12
     e4, _ = pkv_oracle.attention_fp8(p.q, k8, v8, ks2, vs2, p.block_table, p.seq_lens, Hkv=8, page_size=16, scale=p.scale)
     assert not np.allclose(np.nan_to_num(e4), got)          # the byte kind matters
+
+
+def test_one_byte_quantisers_closed_forms_round_trip_and_torch():
+    """Reading A30: FP32 -> E4M3 (nearest, ties to the even code, saturating at 448) and FP32 -> INT8
+    (half to even, clamp to +-127).  Pinned by: every finite code survives decode -> encode (the decoder
+    is pinned on all 256 codes above); ties / saturation / subnormals worked out by hand; sign symmetry
+    and monotonicity; torch.float8_e4m3fn on the whole FP16 grid inside +-448."""
+    import torch
+    from oracle import append_oracle as ao
+    codes = np.arange(0x7F, dtype=np.uint8)
+    vals = np.array([pkv_oracle.e4m3_to_double(int(c)) for c in codes], dtype=np.float32)
+    assert np.array_equal(ao.quantize_e4m3(vals), codes)
+    assert np.array_equal(ao.quantize_e4m3(-vals[1:]), codes[1:] | 0x80)
+    hand = {1.0: 0x38, 1.0625: 0x38, 1.1875: 0x3A, 1.0626: 0x39, 448.0: 0x7E, 464.0: 0x7E, 1000.0: 0x7E, 3e38: 0x7E,
+            2.0 ** -9: 0x01, 2.0 ** -10: 0x00, 3 * 2.0 ** -11: 0x01, 3 * 2.0 ** -10: 0x02, 2.0 ** -6: 0x08, 0.0: 0x00,
+            240.0: 0x77, 232.0: 0x76, 248.0: 0x78}      # 232 = tie 224|240 -> even code 0x76; 248 = tie 240|256 -> 0x78
+    for x, c in hand.items():
+        assert int(ao.quantize_e4m3(np.float32(x))) == c, (x, hex(c))
+        if x > 0:
+            assert int(ao.quantize_e4m3(np.float32(-x))) == c | 0x80
+    assert int(ao.quantize_e4m3(np.float32("nan"))) == 0x7F and int(ao.quantize_e4m3(np.float32(-0.0))) == 0x80
+    xs = np.sort(np.random.Generator(np.random.PCG64(3)).uniform(-500, 500, 20000).astype(np.float32))
+    dec = np.array([pkv_oracle.e4m3_to_double(int(c)) for c in ao.quantize_e4m3(xs)])
+    assert np.all(np.diff(dec) >= 0)                                        # monotone
+    inside = np.abs(xs) <= 448
+    assert np.all(np.abs(dec[inside] - xs[inside]) <= np.maximum(np.abs(xs[inside]) * 2.0 ** -4, 2.0 ** -10))   # half an ulp
+    g = np.arange(65536, dtype=np.uint16).view(np.float16)
+    g = g[np.isfinite(g) & (np.abs(g.astype(np.float32)) <= 448)].astype(np.float32)
+    t = torch.from_numpy(g).to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+    assert np.array_equal(ao.quantize_e4m3(g), t)
+    i8 = ao.quantize_int8(np.array([0.5, 1.5, 2.5, -0.5, -1.5, -2.5, 126.5, 127.4, 127.5, 300.0, -127.5, -128.0, -1e9, 0.49999997],
+                                   dtype=np.float32)).view(np.int8)
+    assert i8.tolist() == [0, 2, 2, 0, -2, -2, 126, 127, 127, 127, -127, -127, -127, 0]
+    # the division is FP32: one correctly rounded quotient, then one rounding to the code
+    tok = np.array([[3.0, 1.0, -7.0, 0.1]], dtype=np.float16)
+    sc = np.array([0.3], dtype=np.float32)
+    y = np.float32(tok.astype(np.float32)) / sc[0]
+    assert np.array_equal(ao.quantize_token(tok, sc, 1), ao.quantize_e4m3(y)) and np.array_equal(ao.quantize_token(tok, sc, 2), ao.quantize_int8(y))
+
+
+@pytest.mark.parametrize("kind", [1, 2])
+def test_one_byte_append_step_against_dense_brute_force(kind):
+    """Reading A30 against numpy on a dense gathered copy: old tokens dequantised from the cache bytes,
+    the new token = scale * dec(code) with the code worked out here from numpy's own rounding of the
+    FP32 quotient (INT8) or the nearest-table-value search (E4M3, cross-checked with torch), q RoPE'd.
+    Only the new tokens' slots change; rows with N = 0 change nothing."""
+    import torch
+    from oracle import append_oracle as ao
+    lens = np.array([1, 17, 100, 0, 33, 64], dtype=np.int32)
+    p = make_problem(list(lens), seed=73)
+    rng = np.random.Generator(np.random.PCG64(6))
+    ks, vs = rng.uniform(0.03, 0.07, 8).astype(np.float32), rng.uniform(0.03, 0.07, 8).astype(np.float32)
+
+    def to_codes(x32):
+        if kind == 2:
+            return np.clip(np.rint(x32), -127, 127).astype(np.int8).view(np.uint8)
+        return torch.from_numpy(np.clip(x32, -448, 448).astype(np.float32)).to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+
+    def dec(codes):
+        if kind == 2:
+            return codes.view(np.int8).astype(np.float64)
+        return torch.from_numpy(codes.copy()).view(torch.float8_e4m3fn).to(torch.float64).numpy()
+
+    k8 = to_codes(p.k_cache.astype(np.float32) / ks[None, None, :, None])
+    v8 = to_codes(p.v_cache.astype(np.float32) / vs[None, None, :, None])
+    k_new = rng.standard_normal((p.B, 8, 128)).astype(np.float16)
+    v_new = rng.standard_normal((p.B, 8, 128)).astype(np.float16)
+    cos, sin = _rope_tables(256, 128)
+    for tables in ((cos, sin), (None, None)):
+        out, lse, k2, v2 = ao.append_and_attend_q8(p.q, k8, v8, ks, vs, k_new, v_new, p.block_table, lens, tables[0], tables[1],
+                                                    Hkv=8, page_size=16, scale=p.scale, kv_kind=kind)
+        changed = np.zeros(k8.shape[:2], dtype=bool)
+        for i in range(p.B):
+            N = int(lens[i])
+            if N == 0:
+                assert np.all(out[i] == 0) and np.all(np.isneginf(lse[i]))
+                continue
+            pos = N - 1
+            kn = ao.rope_rotate_f16(k_new[i], cos[pos], sin[pos]) if tables[0] is not None else k_new[i]
+            qn = ao.rope_rotate_f16(p.q[i], cos[pos], sin[pos]) if tables[0] is not None else p.q[i]
+            kc = to_codes((kn.astype(np.float32) / ks[:, None]).astype(np.float32))
+            vc = to_codes((v_new[i].astype(np.float32) / vs[:, None]).astype(np.float32))
+            page, slot = p.block_table[i, pos // 16], pos % 16
+            assert np.array_equal(k2[page, slot], kc) and np.array_equal(v2[page, slot], vc)
+            changed[page, slot] = True
+            Kd = np.stack([dec(k8[p.block_table[i, j // 16], j % 16]) for j in range(N - 1)] + [dec(kc)]) * ks.astype(np.float64)[None, :, None]
+            Vd = np.stack([dec(v8[p.block_table[i, j // 16], j % 16]) for j in range(N - 1)] + [dec(vc)]) * vs.astype(np.float64)[None, :, None]
+            for h in range(32):
+                x = (Kd[:, h // 4, :] @ qn[h].astype(np.float64)) * p.scale
+                w = np.exp(x - x.max())
+                assert np.abs(out[i, h] - (w[:, None] * Vd[:, h // 4, :]).sum(0) / w.sum()).max() <= 1e-12
+        assert np.array_equal(k2[~changed], k8[~changed]) and np.array_equal(v2[~changed], v8[~changed])
