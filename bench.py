@@ -57,7 +57,7 @@ L2_BYTES = 126 * 1000 * 1000
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
 MIN_TIMED_MS = 50.0                # the K-step region is repeated until this much has been timed
 WORKLOADS = ["config1", "config2", "config3", "config4", "config4_b4", "config5", "config5_hkv4", "config2_fp8", "config3_fp8",
-             "config2_append", "config3_append"]
+             "config2_append", "config3_append", "config2_fp8_append"]
 FP8_SCALE = 1.0 / 32.0      # per-KV-head scale of the FP8 workloads: N(0,1) / scale stays far inside +-448
 
 
@@ -464,8 +464,13 @@ def oracle_rows(torch, runner, rows, lens, r=0):
         from oracle import append_oracle
         kn = np.ascontiguousarray(runner.knew.cpu().numpy()[rows])
         vn = np.ascontiguousarray(runner.vnew.cpu().numpy()[rows])
-        out, _, _, _ = append_oracle.append_and_attend(q, kc, vc, kn, vn, tc, sl, runner.rope_host[0], runner.rope_host[1],
-                                                        Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale)
+        if runner.fp8:      # the new token is quantised inside the step (reading A30)
+            sc = np.full(w.Hkv, FP8_SCALE, dtype=np.float32)
+            out, _, _, _ = append_oracle.append_and_attend_q8(q, kc, vc, sc, sc, kn, vn, tc, sl, runner.rope_host[0], runner.rope_host[1],
+                                                               Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale, kv_kind=1)
+        else:
+            out, _, _, _ = append_oracle.append_and_attend(q, kc, vc, kn, vn, tc, sl, runner.rope_host[0], runner.rope_host[1],
+                                                            Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale)
     elif runner.fp8:
         sc = np.full(w.Hkv, FP8_SCALE, dtype=np.float64)
         out, _ = pkv_oracle.attention_fp8(q, kc, vc, sc, sc, tc, sl, Hkv=w.Hkv, page_size=w.page_size, scale=runner.scale,
@@ -709,7 +714,8 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
              ("config4", "config4", bal), ("config4_b4", "config4_b4", bal),
              ("config5", "config5", bal), ("config5_hkv4", "config5_hkv4", bal),
              ("config2_fp8", "config2_fp8", bal), ("config3_fp8", "config3_fp8", bal),
-             ("config2_append", "config2_append", bal), ("config3_append", "config3_append", bal)]
+             ("config2_append", "config2_append", bal), ("config3_append", "config3_append", bal),
+             ("config2_fp8_append", "config2_fp8_append", bal)]
     runner, cur = None, None
     for key, name, pol in cases:
         try:

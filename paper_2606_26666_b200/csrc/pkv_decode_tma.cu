@@ -133,6 +133,47 @@ __device__ __forceinline__ void append_patch(const DecodeParams& p, uint32_t sb,
     __syncwarp();
 }
 
+// The same for one-byte caches (d = 128; reading A30): the token is rotated as above (FP16
+// result), divided by its head's scale in FP32 and rounded once to the cache's code; the code bytes go
+// into the head's block of the stage (one 128-byte swizzled row of 128 channels per token) and into
+// the pool.  A lane owns channels (c, c+1) and (c + 64, c + 65), c = 2 * lane.
+template <int KVT, bool IS_K>
+__device__ __forceinline__ void append_patch_q8(const DecodeParams& p, uint32_t sb, int orow, int kvh, int pos, int r, int lane,
+                                                int page_shift) {
+    constexpr int D = 128;
+    const __half* src = (IS_K ? p.k_new : p.v_new) + ((int64_t)orow * p.Hkv + kvh) * D;
+    unsigned char* pool = reinterpret_cast<unsigned char*>(const_cast<__half*>(IS_K ? p.k_cache : p.v_cache));
+    const float* scales = IS_K ? p.k_scale : p.v_scale;
+    const float hs = scales ? __ldg(scales + kvh) : 1.f;
+    const int psz = 16 << page_shift;
+    const int64_t page = __ldg(p.block_table + (int64_t)orow * p.max_pages + (pos >> (4 + page_shift)));
+    unsigned char* dst = pool + page * p.stride_page + (int64_t)(pos & (psz - 1)) * p.stride_token + (int64_t)kvh * p.stride_head;
+    const bool rot = IS_K && p.rope_cos != nullptr && pos < p.rope_positions;
+    const int c = lane * 2;
+    __half2 lo = *reinterpret_cast<const __half2*>(src + c);
+    __half2 hi = *reinterpret_cast<const __half2*>(src + c + D / 2);
+    if (rot) {
+        const float2 cs2 = __ldg(reinterpret_cast<const float2*>(p.rope_cos + (int64_t)pos * (D / 2) + c));
+        const float2 sn2 = __ldg(reinterpret_cast<const float2*>(p.rope_sin + (int64_t)pos * (D / 2) + c));
+        const float2 x1 = __half22float2(lo), x2 = __half22float2(hi);
+        lo = __floats2half2_rn(__fsub_rn(__fmul_rn(x1.x, cs2.x), __fmul_rn(x2.x, sn2.x)),
+                               __fsub_rn(__fmul_rn(x1.y, cs2.y), __fmul_rn(x2.y, sn2.y)));
+        hi = __floats2half2_rn(__fadd_rn(__fmul_rn(x2.x, cs2.x), __fmul_rn(x1.x, sn2.x)),
+                               __fadd_rn(__fmul_rn(x2.y, cs2.y), __fmul_rn(x1.y, sn2.y)));
+    }
+#pragma unroll
+    for (int hf = 0; hf < 2; ++hf) {
+        const int ch = c + hf * (D / 2);
+        const float2 x = __half22float2(hf ? hi : lo);
+        const uint32_t code = cvt_float2_to_bytes2<KVT>(__fdiv_rn(x.x, hs), __fdiv_rn(x.y, hs));
+        // stage: row r, 16-byte chunk (ch / 16) ^ (r % 8), byte ch % 16
+        sts_b16(sb + r * 128 + ((((ch >> 4) ^ (r & 7))) << 4) + (ch & 15), code);
+        *reinterpret_cast<unsigned short*>(dst + ch) = (unsigned short)code;
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the stage is refilled by the async proxy later
+    __syncwarp();
+}
+
 // KVT: pkv_kv_dtype of the caches (0 FP16, 1 FP8 E4M3, 2 INT8); "FP8" below means any one-byte cache.
 // APP: the fused KV-append (+RoPE) step (pkv_decode_append); compiled apart because its extra live
 // values cost the plain step 21 registers and 0.17 us (config 2: 23.83 vs 23.66 us).
@@ -141,7 +182,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     pkv_decode_tma_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap_k,
                           const __grid_constant__ CUtensorMap tmap_v) {
     constexpr bool FP8 = KVT != 0;
-    static_assert(!APP || (KVT == 0 && G <= 8 && D == 128), "fused append: FP16 caches, G <= 8, d = 128");
+    static_assert(!APP || (G <= 8 && D == 128), "fused append: G <= 8, d = 128");
     static_assert(!FP8 || D == 128, "one-byte caches: one 128-byte swizzled row per token and head");
     constexpr int kStages = stages_for<G, HG, D, FP8>();
     constexpr int kHeadBytes = D * (FP8 ? 16 : 32);   // one head's 16 tokens x D channels of K (or V): blocks of 2 KiB
@@ -505,7 +546,9 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                         for (int kk = 0; kk < KK / 2; ++kk) {
 #pragma unroll
                             for (int hf = 0; hf < 2; ++hf) {
-                                const int c = kk * 16 + 2 * t4 + 8 * hf;     // channels c, c+1 (< d/2)
+                                // channels c, c+1 (< d/2) of fragment slot (kk, hf); one-byte caches read Q with
+                                // the permuted contraction index (see qb above)
+                                const int c = kk * 16 + (FP8 ? 4 * t4 + 2 * hf : 2 * t4 + 8 * hf);
                                 const float2 cs2 = __ldg(reinterpret_cast<const float2*>(cr + c));
                                 const float2 sn2 = __ldg(reinterpret_cast<const float2*>(sr + c));
                                 const float2 x1 = __half22float2(*reinterpret_cast<const __half2*>(&qb[kk][hf]));
@@ -552,8 +595,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 if constexpr (APP) {
                     // the block that holds the row's new token: its K row comes from k_new (rotated), not
                     // from the pool -- patched into the stage here and written to the pool for later steps
-                    if (patch && p0 + j == last_blk)
-                        append_patch<D, true>(p, kb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                    if (patch && p0 + j == last_blk) {
+                        if constexpr (FP8) append_patch_q8<KVT, true>(p, kb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                        else append_patch<D, true>(p, kb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                    }
                 }
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
                 if constexpr (FP8) {
@@ -620,8 +665,10 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 // ---- O^T += V^T . P^T
                 mbar_wait(fullv0 + 8 * s, par);
                 if constexpr (APP) {
-                    if (patch && p0 + j == last_blk)
-                        append_patch<D, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                    if (patch && p0 + j == last_blk) {
+                        if constexpr (FP8) append_patch_q8<KVT, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                        else append_patch<D, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                    }
                 }
                 uint32_t vdep = 0;   // a word of every V fragment (see the stage release below)
                 if constexpr (FP8) {
@@ -775,7 +822,7 @@ template <int PART>
 cudaError_t launch_decode_tma_part(const DecodeParams& p, int G, int HG, int D, int kvt, bool app, int grid, const CUtensorMap& mk,
                                    const CUtensorMap& mv, cudaStream_t stream);
 
-// The 106 instantiations are compiled as kTmaParts translation units of this one source
+// The 138 instantiations are compiled as kTmaParts translation units of this one source
 // (-DPKV_TMA_PART=k, see build.py): part k defines launch_decode_tma_part<k>, which launches the
 // kernel if the requested instantiation belongs to it and returns cudaErrorNotSupported otherwise;
 // part 0 also holds the dispatcher.
@@ -813,6 +860,14 @@ cudaError_t launch_decode_tma_part<PKV_TMA_PART>(const DecodeParams& p, int G, i
     PKV_CASE_HG(2, 64, 0, false) PKV_CASE_HG(1, 64, 0, false) PKV_CASE_HG4(16, 64, 0, false)
 #elif PKV_TMA_PART == 10   // d = 256, G = 1, 2 and 16
     PKV_CASE_HG4(2, 256, 0, false) PKV_CASE_HG4(1, 256, 0, false) PKV_CASE_HG4(16, 256, 0, false)
+#elif PKV_TMA_PART == 11   // fused KV-append on FP8 (E4M3) caches, G = 4 and 8
+    PKV_CASE_HG(4, 128, 1, true) PKV_CASE_HG(8, 128, 1, true)
+#elif PKV_TMA_PART == 12   // fused KV-append on INT8 caches, G = 4 and 8
+    PKV_CASE_HG(4, 128, 2, true) PKV_CASE_HG(8, 128, 2, true)
+#elif PKV_TMA_PART == 13   // fused KV-append on FP8 (E4M3) caches, G = 1 and 2
+    PKV_CASE_HG(2, 128, 1, true) PKV_CASE_HG(1, 128, 1, true)
+#elif PKV_TMA_PART == 14   // fused KV-append on INT8 caches, G = 1 and 2
+    PKV_CASE_HG(2, 128, 2, true) PKV_CASE_HG(1, 128, 2, true)
 #endif
     return cudaErrorNotSupported;
 }
@@ -840,6 +895,10 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int k
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<8>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<9>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<10>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<11>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<12>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<13>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<14>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     return e == cudaErrorNotSupported ? cudaErrorInvalidValue : e;
 }
 #endif

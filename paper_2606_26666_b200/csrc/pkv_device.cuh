@@ -234,6 +234,23 @@ __device__ __forceinline__ uint32_t cvt_bytes2_to_half2(uint32_t x) {
         return cvt_e4m3x2_to_half2(x);
     }
 }
+// two FP32 values -> two cache bytes (lo in bits 7..0, hi in bits 15..8), ONE rounding each (DESIGN.md
+// reading A30).  E4M3: round to nearest even, magnitudes beyond 448 saturate (satfinite); INT8: round
+// half to even, clamped to [-127, 127].
+template <int KVT>
+__device__ __forceinline__ uint32_t cvt_float2_to_bytes2(float lo, float hi) {
+    if constexpr (KVT == 2) {
+        const int a = max(-127, min(127, __float2int_rn(lo))), b = max(-127, min(127, __float2int_rn(hi)));
+        return (uint32_t)(a & 0xff) | ((uint32_t)(b & 0xff) << 8);
+    } else {
+        unsigned short r;
+        asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(r) : "f"(hi), "f"(lo));
+        return r;
+    }
+}
+__device__ __forceinline__ void sts_b16(uint32_t addr, uint32_t v) {
+    asm volatile("st.shared.b16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
 __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
     __half2 h = __floats2half2_rn(lo, hi);
     return *reinterpret_cast<uint32_t*>(&h);
