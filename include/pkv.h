@@ -28,7 +28,7 @@
  *     out[i] = 0 and lse[i] = -inf (reading A9).
  *   - compiled-in shapes: G = Hq/Hkv in {1, 2, 4, 8, 16}, page_size in {16, 32, 64}, d = 128; d in
  *     {64, 256} (FP16 caches) and one-byte caches (FP8 E4M3, INT8; d = 128) on the TMA kernel; the
- *     fused KV-append for d = 128, G <= 8.  Anything else returns PKV_ERR_UNSUPPORTED.
+ *     fused KV-append for d = 128.  Anything else returns PKV_ERR_UNSUPPORTED.
  */
 #ifndef PKV_H_
 #define PKV_H_
@@ -326,7 +326,7 @@ PKV_API pkv_status pkv_decode_indexed(const pkv_shape* shape, const pkv_split_po
  * (rotated) token is divided by its KV head's k_scale / v_scale in FP32 and rounded once to the cache's
  * code -- E4M3: to nearest even, magnitudes beyond 448 saturate; INT8: half to even, clamped to
  * [-127, 127] -- and that byte is what the pool receives and what this step attends over.
- * TMA kernel, d = 128, G <= 8 only (else PKV_ERR_UNSUPPORTED).  Otherwise as pkv_decode with
+ * TMA kernel and d = 128 only (else PKV_ERR_UNSUPPORTED).  Otherwise as pkv_decode with
  * build_queue = 1; row_index may be NULL.
  */
 typedef struct {

@@ -20,7 +20,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 BUILD_DIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpkv.so")
 
-TMA_PARTS = 15     # pkv_decode_tma.cu is compiled once per group of instantiations (-DPKV_TMA_PART=k), in parallel
+TMA_PARTS = 16     # pkv_decode_tma.cu is compiled once per group of instantiations (-DPKV_TMA_PART=k), in parallel
 SOURCES = (["pkv_host.cpp", "pkv_aux.cu", "pkv_decode_simt.cu", "pkv_api.cu", "pkv_calibrate.cu", "pkv_static.cu"]
            + [("pkv_decode_tma.cu", k) for k in range(TMA_PARTS)])
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]

@@ -358,8 +358,8 @@ pkv_status decode_stages(const pkv_shape* shape, const pkv_split_policy* policy,
             set_error("pkv_decode_append: k_new / v_new null, or only one RoPE table, or rope_positions <= 0");
             return PKV_ERR_INVALID_ARG;
         }
-        if (rp.kernel != PKV_KERNEL_TMA_MMA || rp.G > 8 || shape->d != kD) {
-            set_error("pkv_decode_append needs the TMA kernel, d = 128 and G <= 8");
+        if (rp.kernel != PKV_KERNEL_TMA_MMA || shape->d != kD) {
+            set_error("pkv_decode_append needs the TMA kernel and d = 128");
             return PKV_ERR_UNSUPPORTED;
         }
     }

@@ -45,6 +45,7 @@ namespace {
 
 constexpr int kComputeWarps = 8;
 constexpr int kPlanBar = 9;         // named barrier: planner warp -> producer 0 (1..8 belong to the head groups)
+constexpr int kPatchBar0 = 10;      // named barriers 10..13: fused append with G = 16, the two warps that share a stage
 constexpr int kRing = 4;            // unit ring between producer 0 and everybody else
 constexpr int kMaxStages = 24;
 
@@ -182,7 +183,7 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
     pkv_decode_tma_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap_k,
                           const __grid_constant__ CUtensorMap tmap_v) {
     constexpr bool FP8 = KVT != 0;
-    static_assert(!APP || (G <= 8 && D == 128), "fused append: G <= 8, d = 128");
+    static_assert(!APP || D == 128, "fused append: d = 128");
     static_assert(!FP8 || D == 128, "one-byte caches: one 128-byte swizzled row per token and head");
     constexpr int kStages = stages_for<G, HG, D, FP8>();
     constexpr int kHeadBytes = D * (FP8 ? 16 : 32);   // one head's 16 tokens x D channels of K (or V): blocks of 2 KiB
@@ -596,8 +597,13 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                     // the block that holds the row's new token: its K row comes from k_new (rotated), not
                     // from the pool -- patched into the stage here and written to the pool for later steps
                     if (patch && p0 + j == last_blk) {
-                        if constexpr (FP8) append_patch_q8<KVT, true>(p, kb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
-                        else append_patch<D, true>(p, kb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                        // G = 16: the two warps of a KV head (one per block of 8 query heads) read the same
+                        // stage; the first block's warp patches, its partner waits for the patch
+                        if (NBK == 1 || h0 == 0) {
+                            if constexpr (FP8) append_patch_q8<KVT, true>(p, kb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                            else append_patch<D, true>(p, kb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                        }
+                        if constexpr (NBK > 1) named_bar_sync(kPatchBar0 + sub * HG + hl, NBK * 32);
                     }
                 }
                 float c0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f};
@@ -666,8 +672,11 @@ __global__ void __launch_bounds__((producers_for(HG) + kComputeWarps + 1) * 32, 
                 mbar_wait(fullv0 + 8 * s, par);
                 if constexpr (APP) {
                     if (patch && p0 + j == last_blk) {
-                        if constexpr (FP8) append_patch_q8<KVT, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
-                        else append_patch<D, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                        if (NBK == 1 || h0 == 0) {
+                            if constexpr (FP8) append_patch_q8<KVT, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                            else append_patch<D, false>(p, vb, orow, kvh, u.nlen - 1, last_row, lane, pgs);
+                        }
+                        if constexpr (NBK > 1) named_bar_sync(kPatchBar0 + sub * HG + hl, NBK * 32);
                     }
                 }
                 uint32_t vdep = 0;   // a word of every V fragment (see the stage release below)
@@ -822,7 +831,7 @@ template <int PART>
 cudaError_t launch_decode_tma_part(const DecodeParams& p, int G, int HG, int D, int kvt, bool app, int grid, const CUtensorMap& mk,
                                    const CUtensorMap& mv, cudaStream_t stream);
 
-// The 138 instantiations are compiled as kTmaParts translation units of this one source
+// The 147 instantiations are compiled as kTmaParts translation units of this one source
 // (-DPKV_TMA_PART=k, see build.py): part k defines launch_decode_tma_part<k>, which launches the
 // kernel if the requested instantiation belongs to it and returns cudaErrorNotSupported otherwise;
 // part 0 also holds the dispatcher.
@@ -868,6 +877,8 @@ cudaError_t launch_decode_tma_part<PKV_TMA_PART>(const DecodeParams& p, int G, i
     PKV_CASE_HG(2, 128, 1, true) PKV_CASE_HG(1, 128, 1, true)
 #elif PKV_TMA_PART == 14   // fused KV-append on INT8 caches, G = 1 and 2
     PKV_CASE_HG(2, 128, 2, true) PKV_CASE_HG(1, 128, 2, true)
+#elif PKV_TMA_PART == 15   // fused KV-append, G = 16 (FP16, FP8 and INT8 caches)
+    PKV_CASE_HG4(16, 128, 0, true) PKV_CASE_HG4(16, 128, 1, true) PKV_CASE_HG4(16, 128, 2, true)
 #endif
     return cudaErrorNotSupported;
 }
@@ -899,6 +910,7 @@ cudaError_t launch_decode_tma(const DecodeParams& p, int G, int HG, int D, int k
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<12>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<13>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     if (e == cudaErrorNotSupported) e = launch_decode_tma_part<14>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
+    if (e == cudaErrorNotSupported) e = launch_decode_tma_part<15>(p, G, HG, D, kvt, app, grid, mk, mv, stream);
     return e == cudaErrorNotSupported ? cudaErrorInvalidValue : e;
 }
 #endif

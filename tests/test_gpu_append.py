@@ -31,7 +31,7 @@ def run_append(dp, p, pol, k_new, v_new, cos, sin, lens):
     return dp.out.cpu().numpy().astype(np.float64), dp.lse.cpu().numpy().astype(np.float64)
 
 
-@pytest.mark.parametrize("Hkv", [8, 4, 16])
+@pytest.mark.parametrize("Hkv", [8, 4, 16, 32, 2])          # G = 4, 8, 2, 1, 16
 @pytest.mark.parametrize("rope", [True, False])
 def test_append_step_matches_the_oracle_and_writes_the_pool_bit_exact(Hkv, rope):
     lens = np.array([1, 16, 17, 100, 0, 257, 700, 4099, 32, 33], dtype=np.int32)
@@ -46,7 +46,7 @@ def test_append_step_matches_the_oracle_and_writes_the_pool_bit_exact(Hkv, rope)
     for pol in (pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=32, num_splits=5),
                 pkv.Policy(tile_tokens=16, num_splits=3, merge_mode=pkv.MERGE_FUSED, route=pkv.ROUTE_RECT, heads_per_cta=1),
                 pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=24, heads_per_cta=2),
-                pkv.Policy(tile_tokens=32, num_splits=4, heads_per_cta=4)):
+                pkv.Policy(tile_tokens=32, num_splits=4, heads_per_cta=min(4, Hkv))):
         dp = DevProblem(p)          # fresh pool: the step writes it
         out, lse = run_append(dp, p, pol, k_new, v_new, cos, sin, lens)
         assert not np.isnan(out).any()
@@ -81,9 +81,9 @@ def test_append_loop_grows_rows_across_pages_and_page_sizes():
 
 
 def test_append_unsupported_combinations_are_refused():
-    p = make_problem([100], seed=5, Hkv=2)                  # G = 16
+    p = make_problem([100], seed=5, d=64)                   # the append is compiled for d = 128
     dp = DevProblem(p)
-    kn = np.zeros((1, 2, 128), np.float16)
+    kn = np.zeros((1, 8, 64), np.float16)
     with pytest.raises(pkv.PkvError):
         run_append(dp, p, pkv.Policy(tile_tokens=32, num_splits=2), kn, kn, None, None, np.array([100], np.int32))
     p = make_problem([100], seed=6)
@@ -109,10 +109,10 @@ def run_append_q8(fp, pol, k_new, v_new, cos, sin, lens):
 
 
 @pytest.mark.parametrize("kind", [pkv.KV_E4M3, pkv.KV_INT8])
-@pytest.mark.parametrize("Hkv", [8, 4, 16, 32])
+@pytest.mark.parametrize("Hkv", [8, 4, 16, 32, 2])          # G = 4, 8, 2, 1, 16
 @pytest.mark.parametrize("rope", [True, False])
 def test_one_byte_append_step_matches_the_oracle_and_writes_the_pool_bit_exact(Hkv, rope, kind):
-    """FP8 (E4M3) and INT8 caches, G = 4, 8, 2, 1: the new token is quantised inside the decode launch
+    """FP8 (E4M3) and INT8 caches, G = 4, 8, 2, 1, 16: the new token is quantised inside the decode launch
     (FP32 division by the head's scale, one rounding); outputs within tolerance, pool bytes bit-exact.
     Some elements of the new tokens saturate the code range."""
     from test_gpu_fp8 import Fp8Problem
@@ -126,7 +126,7 @@ def test_one_byte_append_step_matches_the_oracle_and_writes_the_pool_bit_exact(H
     for pol in (pkv.Policy(tile_tokens=32, num_splits=1), pkv.Policy(tile_tokens=32, num_splits=5),
                 pkv.Policy(tile_tokens=16, num_splits=3, merge_mode=pkv.MERGE_FUSED, route=pkv.ROUTE_RECT, heads_per_cta=1),
                 pkv.Policy(tile_tokens=16, split_mode=pkv.SPLIT_BALANCED, num_splits=0, num_sms=24, heads_per_cta=2),
-                pkv.Policy(tile_tokens=32, num_splits=4, heads_per_cta=4)):
+                pkv.Policy(tile_tokens=32, num_splits=4, heads_per_cta=min(4, Hkv))):
         fp = Fp8Problem(list(lens), seed=1500 + Hkv, Hkv=Hkv, kind=kind)          # fresh pools: the step writes them
         ref, ref_lse, k2, v2 = ao.append_and_attend_q8(fp.p.q, fp.k8, fp.v8, fp.ks, fp.vs, k_new, v_new, fp.p.block_table, lens, cos, sin,
                                                         Hkv=Hkv, page_size=16, scale=fp.p.scale, kv_kind=2 if kind == pkv.KV_INT8 else 1)
