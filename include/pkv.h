@@ -186,6 +186,8 @@ typedef struct {
      * even when every row is empty: these can exceed the scheduler-derived counts above. */
     int64_t launched_build, launched_decode, launched_merge;
     int64_t error_word;      /* bit set of pkv_device_error                                      */
+    int64_t armed_step;      /* pkv_decode_host_pipelined only: 1 = this step's launches had been
+                                enqueued by the previous call and were only released by this one */
 } pkv_counters;
 
 /* Library/ABI version: (major << 16) | minor. */
@@ -426,6 +428,55 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
                                    void* out_host, float scale, void* host_staging, void* dev_scratch,
                                    size_t scratch_bytes, void* workspace, size_t workspace_bytes,
                                    void* stream, pkv_counters* counters_out);
+
+/*
+ * The host-buffer step with its submission taken off the critical path (the serving-
+ * facing time includes planning and launching).  A synchronous step pays, before its first kernel
+ * runs, the driver calls that enqueue it and the start of a kernel on an idle GPU, and after its last
+ * the wake-up of the synchronising thread -- about 20 us of a 45 us config-2 step.  Here the caller
+ * tells the call what the NEXT step will be (`next`: its lengths and block table -- a decode loop knows
+ * them when it schedules: N + 1 for every continuing row -- and optionally other caches / another
+ * out_host).  While the GPU works on this step, the call plans the next one, writes its lengths and
+ * changed table rows into the staging image and enqueues its launches BEHIND A GATE:
+ *       gate / stage kernel -> decode -> merge -> signal kernel
+ * The gate is one CTA that polls a flag word of the pinned staging buffer over the host link; once the
+ * host has released the step it fetches lengths, q and table rows from the image into dev_scratch.
+ * Decode, merge and signal are chained behind it by programmatic launch: they are resident and
+ * planned when the gate opens.  The signal kernel writes the step's number into a done word of the
+ * image.  The next call then only copies q into the image, stores the flag and spins on the done word.
+ * Results are those of pkv_decode_host, bit for bit (the same kernels on the same inputs).
+ *   - Needs: host_staging and out_host pinned and device-mapped, host_staging 256-byte aligned, the TMA
+ *     kernel with the fused build (B <= 512), no PKV_FLAG_VALIDATE / SEPARATE_BUILD, at most 64 KiB of
+ *     inputs in at most four pieces per step.  Otherwise -- and whenever the armed step turns out not to
+ *     be the one the next call asks for (other lengths, table, buffers, policy) -- the call does what
+ *     pkv_decode_host does; a mispredicted armed step is first run on whatever the image holds and its
+ *     result discarded.  A step is only armed when the kernels it launches have run before in this
+ *     thread.
+ *   - WHILE A STEP IS ARMED THE STREAM IS BLOCKED by the polling gate: anything that waits for the stream
+ *     or for the whole device (cudaStreamSynchronize, cudaDeviceSynchronize, cudaFree, cudaMemcpy)
+ *     does not return until the step is released -- or until the gate gives up, 200 ms after it
+ *     started; such an expired step runs on stale inputs, is marked, and the next call redoes it.
+ *     pkv_decode_host_drain(host_staging, stream) releases an armed step at once (it runs on stale
+ *     inputs; its result is discarded) and waits for it.  pkv_decode_host drains its staging buffer
+ *     itself.  State is per (thread, host_staging): call from one thread.
+ *   - next == NULL (or next->seq_lens_host == NULL): nothing is armed; the call is a synchronous step
+ *     that waits on the done word instead of cudaStreamSynchronize.
+ * Arguments as pkv_decode_host.
+ */
+typedef struct {
+    const int32_t* seq_lens_host;    /* [B] the next step's lengths                                     */
+    const int32_t* block_table_host; /* [B, max_pages] the next step's table                            */
+    const void* k_cache_dev;         /* NULL = the same caches as this step                              */
+    const void* v_cache_dev;
+    void* out_host;                  /* NULL = the same out_host                                         */
+} pkv_next_step;
+PKV_API pkv_status pkv_decode_host_pipelined(const pkv_shape* shape, const pkv_split_policy* policy,
+                                             const void* q_host, const void* k_cache_dev, const void* v_cache_dev,
+                                             const int32_t* block_table_host, const int32_t* seq_lens_host,
+                                             void* out_host, float scale, void* host_staging, void* dev_scratch,
+                                             size_t scratch_bytes, void* workspace, size_t workspace_bytes,
+                                             void* stream, const pkv_next_step* next, pkv_counters* counters_out);
+PKV_API pkv_status pkv_decode_host_drain(void* host_staging, void* stream);
 
 /*
  * The calibrated cost model (sec. 3.5), on the HOST, from host-resident lengths --

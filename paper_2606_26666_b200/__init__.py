@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     ROUTE_RECT, ROUTE_WORKQUEUE, MERGE_SEPARATE, MERGE_FUSED, SPLIT_FIXED_COUNT, SPLIT_FIXED_CHUNK, SPLIT_BALANCED, SPLIT_AUTO,
     KERNEL_AUTO, KERNEL_TMA_MMA, KERNEL_SIMT, FLAG_VALIDATE, FLAG_NO_PDL, FLAG_SEPARATE_BUILD, FLAG_TEST_REPLAN, FLAG_OUT_PINNED,
     DEVERR_QUEUE_OVERFLOW, DEVERR_SEQ_LEN, DEVERR_PAGE_ID, STAGE_BUILD, STAGE_DECODE, STAGE_MERGE, STAGE_ALL, KV_F16, KV_E4M3, KV_INT8, EXPORTS,
-    PkvError, Shape, Policy, CostModel, HostDecoder, Append, pkv_decode_append, pkv_default_cost_model, pkv_estimate_cost, pkv_choose_policy,
+    PkvError, Shape, Policy, CostModel, HostDecoder, PipelinedHostDecoder, Append, pkv_decode_append, pkv_default_cost_model, pkv_estimate_cost, pkv_choose_policy,
     pkv_version, pkv_last_error, pkv_workspace_bytes, pkv_workspace_init_bytes, pkv_host_scratch_bytes, pkv_build_workqueue_host,
     pkv_build_workqueue, pkv_decode, pkv_decode_stages, pkv_merge, pkv_get_counters, pkv_read_workqueue, pkv_workspace_partials,
     pkv_decode_host, pkv_calibrate, pkv_decode_indexed, pkv_plan_buckets_host, pkv_decode_buckets, pkv_bucket_counters_host,

@@ -50,7 +50,7 @@ class pkv_shape(ctypes.Structure):
 class pkv_counters(ctypes.Structure):
     _fields_ = [(n, _i64) for n in ("tasks", "empty_tasks", "decode_launches", "merge_launches", "build_launches",
                                     "useful_kv_bytes", "merge_bytes", "num_splits", "max_row_splits", "chunk_tiles", "h2d_bytes",
-                                    "d2h_bytes", "launched_build", "launched_decode", "launched_merge", "error_word")]
+                                    "d2h_bytes", "launched_build", "launched_decode", "launched_merge", "error_word", "armed_step")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -89,7 +89,11 @@ EXPORTS = ("pkv_version", "pkv_last_error", "pkv_workspace_bytes", "pkv_workspac
            "pkv_workspace_partials", "pkv_host_scratch_bytes", "pkv_decode_host", "pkv_calibrate", "pkv_decode_indexed",
            "pkv_plan_buckets_host", "pkv_decode_buckets", "pkv_bucket_counters_host", "pkv_default_cost_model",
            "pkv_estimate_cost", "pkv_choose_policy", "pkv_decode_append", "pkv_decode_static",
-           "pkv_static_workspace_bytes")
+           "pkv_static_workspace_bytes", "pkv_decode_host_pipelined", "pkv_decode_host_drain")
+
+
+class pkv_next_step(ctypes.Structure):
+    _fields_ = [("seq_lens_host", _vp), ("block_table_host", _vp), ("k_cache_dev", _vp), ("v_cache_dev", _vp), ("out_host", _vp)]
 
 
 class PkvError(RuntimeError):
@@ -159,6 +163,11 @@ def _load() -> ctypes.CDLL:
     lib.pkv_decode_host.restype = _i32
     lib.pkv_decode_host.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float,
                                     _vp, _vp, ctypes.c_size_t, _vp, ctypes.c_size_t, _vp, P(pkv_counters)]
+    lib.pkv_decode_host_pipelined.restype = _i32
+    lib.pkv_decode_host_pipelined.argtypes = [P(pkv_shape), P(pkv_split_policy), _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float,
+                                              _vp, _vp, ctypes.c_size_t, _vp, ctypes.c_size_t, _vp, P(pkv_next_step), P(pkv_counters)]
+    lib.pkv_decode_host_drain.restype = _i32
+    lib.pkv_decode_host_drain.argtypes = [_vp, _vp]
     lib.pkv_calibrate.restype = _i32
     lib.pkv_calibrate.argtypes = [_vp, ctypes.c_size_t, _vp, P(pkv_calibration)]
     return lib
@@ -479,6 +488,37 @@ class HostDecoder:
     @property
     def counters(self) -> dict:
         return self._counters.as_dict()
+
+
+class PipelinedHostDecoder(HostDecoder):
+    """pkv_decode_host_pipelined, marshalled once like HostDecoder.  Per step pass raw addresses of this
+    step's q, block_table, seq_lens and out and -- to take the next step's submission off the critical
+    path -- of the NEXT step's seq_lens and block_table (0 = arm nothing), optionally its caches / out.
+    While a step is armed the stream is blocked: call drain() before anything that waits for the stream
+    or the device (torch.cuda.synchronize(), freeing memory, ...)."""
+
+    def __init__(self, shape: Shape, policy: Policy, k_cache_dev, v_cache_dev, host_staging, dev_scratch, workspace,
+                 scale: float, stream=None):
+        super().__init__(shape, policy, k_cache_dev, v_cache_dev, host_staging, dev_scratch, workspace, scale, stream)
+        self._fn = _lib.pkv_decode_host_pipelined
+        self._next = pkv_next_step()
+        self._next_ref = ctypes.byref(self._next)
+        self._tail_a, self._tail_b = self._tail[:-1], self._tail[-1]     # ... stream | counters
+        self._staging, self._stream = _vp(_ptr(host_staging)), _vp(_stream_ptr(stream))
+
+    def __call__(self, q_host: int, block_table_host: int, seq_lens_host: int, out_host: int, next_seq_lens_host: int = 0,
+                 next_block_table_host: int = 0, k_cache_dev: int = 0, v_cache_dev: int = 0, next_k_cache_dev: int = 0,
+                 next_v_cache_dev: int = 0, next_out_host: int = 0) -> None:
+        n = self._next
+        n.seq_lens_host, n.block_table_host = next_seq_lens_host or None, next_block_table_host or None
+        n.k_cache_dev, n.v_cache_dev, n.out_host = next_k_cache_dev or None, next_v_cache_dev or None, next_out_host or None
+        st = self._fn(*self._head, q_host, k_cache_dev or self._k, v_cache_dev or self._v, block_table_host, seq_lens_host, out_host,
+                      *self._tail_a, self._next_ref, self._tail_b)
+        if st != PKV_OK:
+            _check(st)
+
+    def drain(self) -> None:
+        _check(_lib.pkv_decode_host_drain(self._staging, self._stream))
 
 
 def pkv_calibrate(dev_buffer, stream=None) -> dict:

@@ -222,7 +222,80 @@ __global__ void __launch_bounds__(NW * 32, MINB) pkv_merge_kernel(const DecodePa
     }
 }
 
+// Pipelined host-buffer step (pkv_decode_host_pipelined).  The step's launches are enqueued BEFORE the
+// host has its inputs; this kernel is the first of them and the gate: one CTA that
+//   1. lets its dependents go at once (the decode CTAs become resident, plan speculatively on the
+//      previous step's lengths -- re-validated after their dependency wait -- and prefetch),
+//   2. gate = true: polls the flag word of the pinned, device-mapped staging image until the host has
+//      released step `seq` (one PCIe read per poll by one thread), or until `timeout_ns` have passed --
+//      then it records `expired = seq` and goes on, so a stream that nobody releases is blocked for a
+//      bounded time only (the step then runs on stale inputs and the host discards its result),
+//   3. fetches the step's small inputs -- lengths, q, changed block-table rows -- from the image over
+//      the host link into the device scratch (same layout: a segment is (offset, 16-byte chunks));
+//      system-scope volatile loads: the CPU wrote these bytes after the launch was enqueued,
+//   4. tells the host that it has finished reading the image (`staged = seq`).
+__global__ void __launch_bounds__(kStageThreads) pkv_stage_kernel(const unsigned char* __restrict__ src, unsigned char* __restrict__ dst,
+                                                                  const StageSegs segs, volatile uint32_t* words, uint32_t seq, bool gate,
+                                                                  unsigned long long timeout_ns) {
+    pdl_launch_dependents();
+    if (gate) {
+        if (threadIdx.x == 0) {
+            unsigned long long t0, t1;
+            asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t0));
+            while ((int32_t)(words[kPipeFlagWord] - seq) < 0) {
+                asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t1));
+                if (t1 - t0 > timeout_ns) {
+                    words[kPipeExpiredWord] = seq;
+                    break;
+                }
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int k = 0; k < kMaxStageSegs; ++k) {
+        if (k >= segs.n) break;
+        const size_t base = segs.off[k];
+        for (uint32_t i = threadIdx.x; i < segs.chunks[k]; i += kStageThreads) {
+            uint4 v;
+            asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                         : "l"(src + base + 16 * (size_t)i));
+            *reinterpret_cast<uint4*>(dst + base + 16 * (size_t)i) = v;
+        }
+    }
+    __syncthreads();     // every load of the image has returned
+    if (threadIdx.x == 0) {
+        __threadfence_system();
+        words[kPipeStagedWord] = seq;
+    }
+}
+
+// Last launch of a pipelined step: resident early (programmatic launch), it waits for everything before
+// it in the stream -- the merge's (or the decode's) stores to the pinned out_host included -- and
+// writes the step's number into the image's `done` word, which the host is spinning on.
+__global__ void pkv_signal_kernel(volatile uint32_t* words, uint32_t seq) {
+    pdl_launch_dependents();
+    pdl_wait();
+    if (threadIdx.x == 0) {
+        __threadfence_system();
+        words[kPipeDoneWord] = seq;
+    }
+}
+
 }  // namespace
+
+cudaError_t launch_stage(const void* src_mapped, void* dst, const StageSegs& segs, uint32_t* words_mapped, uint32_t seq, bool gate,
+                         unsigned long long timeout_ns, cudaStream_t stream) {
+    // a plain launch: whatever is ahead of it in the stream (the previous step) has finished when it starts
+    pkv_stage_kernel<<<1, kStageThreads, 0, stream>>>(static_cast<const unsigned char*>(src_mapped), static_cast<unsigned char*>(dst), segs,
+                                                      words_mapped, seq, gate, timeout_ns);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_signal(uint32_t* words_mapped, uint32_t seq, bool pdl, cudaStream_t stream) {
+    return launch_pdl(pdl, pkv_signal_kernel, dim3(1), dim3(32), 0, stream, (volatile uint32_t*)words_mapped, seq);
+}
 
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,
                            const int32_t* row_index, QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,

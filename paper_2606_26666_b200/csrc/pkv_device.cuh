@@ -835,6 +835,23 @@ cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int
                            const int32_t* row_index, QueueHeader* hdr, int32_t* split_offsets, int32_t* fuse_counters, RowSlot* rowslots,
                            pkv_task* tasks, int64_t tasks_cap, cudaStream_t stream);
 cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream);
+// pkv_decode_host_pipelined (pkv_aux.cu): the gate / stage kernel and the completion signal.
+constexpr int kMaxStageSegs = 4;
+constexpr int kStageThreads = 1024;           // 16 KiB of inputs in one round of 16-byte loads over the host link
+constexpr size_t kMaxStageBytes = 64 << 10;   // beyond this the copy engine is the faster way up
+struct StageSegs {
+    uint32_t off[kMaxStageSegs];      // byte offset in the image, multiple of 16
+    uint32_t chunks[kMaxStageSegs];   // 16-byte chunks
+    int32_t n;
+};
+// 32-bit words of the pipeline in the pinned, device-mapped image header (pkv_api.cu PipeWords)
+constexpr int kPipeFlagWord = 0;      // host -> GPU: number of the last released step
+constexpr int kPipeStagedWord = 16;   // GPU -> host: the stage kernel of step n has read the image
+constexpr int kPipeDoneWord = 17;     //              step n's result is in out_host
+constexpr int kPipeExpiredWord = 18;  //              step n was never released: it ran on stale inputs
+cudaError_t launch_stage(const void* src_mapped, void* dst, const StageSegs& segs, uint32_t* words_mapped, uint32_t seq, bool gate,
+                         unsigned long long timeout_ns, cudaStream_t stream);
+cudaError_t launch_signal(uint32_t* words_mapped, uint32_t seq, bool pdl, cudaStream_t stream);
 int decode_tma_stage_bytes(int HG, int D, bool fp8);
 
 }  // namespace pkv

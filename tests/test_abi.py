@@ -35,7 +35,7 @@ def test_version_and_struct_sizes():
     assert ctypes.sizeof(binding.pkv_task) == 20            # 5 x int32
     assert ctypes.sizeof(binding.pkv_split_policy) == 44
     assert ctypes.sizeof(binding.pkv_shape) == 80
-    assert ctypes.sizeof(binding.pkv_counters) == 128
+    assert ctypes.sizeof(binding.pkv_counters) == 136
 
 
 def shape(B, Hkv=8, Hq=32, max_pages=4096):
