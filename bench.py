@@ -88,6 +88,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="target CPU time of the oracle sample")
     ap.add_argument("--timeline", default="", help="write a CUPTI kernel timeline of a few replayed steps to this file")
+    ap.add_argument("--timeline-e2e", default="", help="write a CUPTI kernel timeline of a few pipelined host-buffer steps to this file")
     ap.add_argument("--launcher-check", action="store_true",
                     help="exercise only the multi-rank launcher and bookkeeping (gloo, no CUDA): CPU test hook")
     return ap.parse_args(argv)
@@ -740,6 +741,75 @@ def write_timeline(torch, pkv, runner, path, steps=6):
         f.write("\n".join(lines) + "\n")
 
 
+def write_timeline_e2e(torch, pkv, runner, path, steps=8, auto=False):
+    """CUPTI (torch.profiler) kernel records of `steps` consecutive steps through pkv.PipelinedHostDecoder, after
+    warm-up: per step the gate / stage kernel (its duration includes the time it waits for the host's flag:
+    the host's think time plus the flag's way over the host link), decode, merge and the signal kernel.
+    Evidence for the e2e wall-clock number; the pipeline is drained before the profiler stops."""
+    from torch.profiler import ProfilerActivity, profile
+    w = runner.w
+    pol = dataclasses.replace(runner.pol, flags=runner.pol.flags | pkv.FLAG_OUT_PINNED)
+    ws = runner.ws
+    if auto:
+        pol = dataclasses.replace(pol, split_mode=pkv.SPLIT_AUTO, num_splits=0)
+        ws = pkv.alloc_workspace(runner.shape, pol, device=runner.device)
+    nb = pkv.pkv_host_scratch_bytes(runner.shape, pol)
+    staging = torch.zeros(nb, dtype=torch.uint8).pin_memory()
+    scratch = torch.empty(nb, dtype=torch.uint8, device=runner.device)
+    q_host = [runner.q[r].cpu().pin_memory() for r in range(runner.R)]
+    bt_host = torch.from_numpy(np.ascontiguousarray(w.block_table)).pin_memory()
+    out_host = torch.empty((w.B, w.Hq, w.d), dtype=torch.float16).pin_memory()
+    lens_host = [torch.from_numpy(runner.lens_all_host[t].copy()).pin_memory() for t in range(runner.nlens)]
+    torch.cuda.synchronize(runner.device)
+    dec = pkv.PipelinedHostDecoder(runner.shape, pol, runner.k[0], runner.v[0], staging, scratch, ws, runner.scale, stream=runner.stream)
+    R, nl = runner.R, runner.nlens
+
+    def step(t):
+        r, rn = t % R, (t + 1) % R
+        dec(q_host[r].data_ptr(), bt_host.data_ptr(), lens_host[t % nl].data_ptr(), out_host.data_ptr(), lens_host[(t + 1) % nl].data_ptr(),
+            bt_host.data_ptr(), runner.k[r].data_ptr(), runner.v[r].data_ptr(), runner.k[rn].data_ptr(), runner.v[rn].data_ptr())
+
+    walls = []
+    try:
+        for t in range(20):
+            step(t)
+        dec.drain()
+        with profile(activities=[ProfilerActivity.CUDA]) as prof:
+            for t in range(20, 24):          # inside the profiler: first steps re-warm its hooks
+                step(t)
+            for t in range(24, 24 + steps):
+                t0 = time.perf_counter()
+                step(t)
+                walls.append(1e6 * (time.perf_counter() - t0))
+            dec.drain()
+            torch.cuda.synchronize(runner.device)
+    finally:
+        dec.drain()
+    evs = [e for e in prof.events() if "pkv_" in e.name]
+    evs.sort(key=lambda e: e.time_range.start)
+    per_step = 4 if any("pkv_merge" in e.name for e in evs) else 3
+    evs = evs[-(steps + 1) * per_step:-per_step]      # the timed steps (the last group is the drained, discarded step)
+    lines = ["# CUPTI kernel timeline of %d consecutive pipelined host-buffer steps: %s, policy %s" % (steps, w.name, pol),
+             "# command: python bench.py --workload %s --timeline-e2e <this file> (pkv.PipelinedHostDecoder; under the profiler)" % w.name.split("_")[0],
+             "# times in microseconds after the first listed kernel's start; gap = start - end of the previous kernel (negative: resident early)",
+             "# pkv_stage_kernel is the gate: it starts when the previous step has finished and its duration includes the wait for the host's flag",
+             "# wall clock of these calls under the profiler, us: " + " ".join("%.1f" % x for x in walls),
+             "%-4s %-34s %10s %10s %10s" % ("#", "kernel", "start", "duration", "gap")]
+    if evs:
+        t0, prev_end = evs[0].time_range.start, None
+        for i, e in enumerate(evs):
+            s_, d_ = e.time_range.start - t0, e.time_range.end - e.time_range.start
+            gap = "" if prev_end is None else "%10.2f" % (e.time_range.start - prev_end)
+            m = re.search(r"pkv_\w+", e.name)
+            lines.append("%-4d %-34s %10.2f %10.2f %10s" % (i, m.group(0) if m else e.name[:34], s_, d_, gap))
+            prev_end = e.time_range.end
+        span = evs[-1].time_range.end - evs[0].time_range.start
+        lines.append("# %d kernels in %.2f us = %.2f us per step from gate start to signal end (host think time between steps included)" % (
+            len(evs), span, span / steps))
+    with open(path, "w") as f:
+        f.write("\n".join(lines) + "\n")
+
+
 def summarize(regions_ms, K):
     us = [1e3 * m / K for m in regions_ms]
     return {"regions": len(us), "us_per_step_median": float(np.median(us)), "us_per_step_min": float(min(us)),
@@ -1046,6 +1116,8 @@ def run_ours(args):
         line["parity"], _ = parity_of(torch, runner, pick_rows(runner.lens_at(0), 70000, w.seed))
     if args.timeline:
         write_timeline(torch, pkv, runner, args.timeline)
+    if args.timeline_e2e:
+        write_timeline_e2e(torch, pkv, runner, args.timeline_e2e, auto=chosen.startswith("pkv_choose_policy"))
     # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel from the
     # committed `ncu --set full` capture of this workload (profiles/traffic.csv names the capture)
     traffic_path = os.path.join(ROOT, "profiles", "traffic.csv")
