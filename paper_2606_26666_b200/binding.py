@@ -517,6 +517,22 @@ class PipelinedHostDecoder(HostDecoder):
         if st != PKV_OK:
             _check(st)
 
+    def prepare(self, q_host: int, block_table_host: int, seq_lens_host: int, out_host: int, next_seq_lens_host: int = 0,
+                next_block_table_host: int = 0, k_cache_dev: int = 0, v_cache_dev: int = 0, next_k_cache_dev: int = 0,
+                next_v_cache_dev: int = 0, next_out_host: int = 0):
+        """The marshalled argument list of one step, for run(): a decode loop passes the same few buffers
+        again and again, so the per-step cost of building a struct and seventeen arguments can be paid once."""
+        n = pkv_next_step()
+        n.seq_lens_host, n.block_table_host = next_seq_lens_host or None, next_block_table_host or None
+        n.k_cache_dev, n.v_cache_dev, n.out_host = next_k_cache_dev or None, next_v_cache_dev or None, next_out_host or None
+        return (*self._head, _vp(q_host), _vp(k_cache_dev) if k_cache_dev else self._k, _vp(v_cache_dev) if v_cache_dev else self._v,
+                _vp(block_table_host), _vp(seq_lens_host), _vp(out_host), *self._tail_a, ctypes.byref(n), self._tail_b, n)
+
+    def run(self, prepared) -> None:
+        st = self._fn(*prepared[:-1])       # the last element keeps the pkv_next_step alive
+        if st != PKV_OK:
+            _check(st)
+
     def drain(self) -> None:
         _check(_lib.pkv_decode_host_drain(self._staging, self._stream))
 

@@ -165,3 +165,25 @@ def test_unreleased_step_expires_and_is_redone():
     assert dec.counters["armed_step"] == 1                    # the pipeline is back in step
     dec.drain()
     torch.cuda.synchronize()
+
+
+def test_prepared_calls_replay_the_same_step_arguments():
+    """PipelinedHostDecoder.prepare() / run(): the marshalled argument list of a step, built once."""
+    pol = pkv.Policy(tile_tokens=32, num_splits=4, flags=pkv.FLAG_OUT_PINNED)
+    lp = Loop(pol, seed=2400)
+    want, _ = lp.plain_pass()
+    staging, scratch, ws = lp.buffers()
+    dec = pkv.PipelinedHostDecoder(lp.dp.shape, pol, lp.dp.k, lp.dp.v, staging, scratch, ws, lp.p.scale, stream=lp.stream)
+    steps = [dec.prepare(lp.q[t % 3].data_ptr(), lp.tables[t].data_ptr(), lp.lens[t].data_ptr(), lp.out.data_ptr(),
+                         lp.lens[t + 1].data_ptr(), lp.tables[t + 1].data_ptr()) for t in range(8)]
+    armed = 0
+    try:
+        for t in range(8):
+            lp.out.fill_(float("nan"))
+            dec.run(steps[t])
+            assert np.array_equal(lp.out.numpy().view(np.uint16), want[t].view(np.uint16)), "step %d" % t
+            armed += dec.counters["armed_step"]
+    finally:
+        dec.drain()
+    assert armed >= 5
+    torch.cuda.synchronize()
