@@ -684,6 +684,13 @@ struct PipeCtx {
     uint32_t seq = 0;             // number of the last step issued on this staging buffer
     bool armed = false;           // step `seq` is enqueued behind a wait on flag
     uint64_t armed_sig = 0;       // everything the armed launches were made for (see step_sig)
+    // the armed step's call, argument by argument: a call that repeats them byte for byte is released
+    // before anything else is done (validation and planning then run while the GPU works)
+    pkv_shape id_shape;
+    pkv_split_policy id_policy;
+    const void *id_k = nullptr, *id_v = nullptr, *id_out = nullptr, *id_ws = nullptr, *id_ds = nullptr, *id_stream = nullptr;
+    float id_scale = 0.f;
+    size_t id_scratch_bytes = 0, id_ws_bytes = 0;
     pkv_counters armed_counters;  // what the armed step's call will report
     uint64_t seen[32];            // launch keys that have been launched WITHOUT a pending wait (kernels loaded)
     int nseen = 0;
@@ -1051,6 +1058,30 @@ pkv_status pkv_decode_host_pipelined(const pkv_shape* shape, const pkv_split_pol
                                      const pkv_next_step* next, pkv_counters* counters_out) {
     using namespace pkv;
     clear_error();
+    // Early release: the call repeats, byte for byte, the arguments the armed step was enqueued for.
+    bool early = false;
+    if (shape && policy && q_host && seq_lens_host && block_table_host) {
+        PipeCtx* c0 = pipe_ctx(host_staging, false);
+        if (c0 && c0->armed && std::memcmp(&c0->id_shape, shape, sizeof(*shape)) == 0 &&
+            std::memcmp(&c0->id_policy, policy, sizeof(*policy)) == 0 && c0->id_k == k_cache_dev && c0->id_v == v_cache_dev &&
+            c0->id_out == out_host && c0->id_ws == workspace && c0->id_ds == dev_scratch && c0->id_stream == stream &&
+            std::memcmp(&c0->id_scale, &scale, 4) == 0 && c0->id_scratch_bytes == scratch_bytes && c0->id_ws_bytes == workspace_bytes) {
+            const pkv_shape& s0 = *shape;
+            const HostImage im0 = host_image(s0);
+            unsigned char* hs0 = static_cast<unsigned char*>(host_staging);
+            PipeWords* w0 = reinterpret_cast<PipeWords*>(hs0 + im0.hdr + kPipeWordsOffset);
+            Piece tmp[1];
+            int nrun = 0;
+            size_t run_bytes = 0;
+            if (*reinterpret_cast<volatile uint32_t*>(&w0->expired) != c0->seq &&
+                std::memcmp(hs0 + im0.seq_lens, seq_lens_host, 4 * (size_t)s0.B) == 0 &&
+                table_runs(s0, im0, hs0, block_table_host, seq_lens_host, false, false, tmp, 0, &nrun, &run_bytes) && run_bytes == 0) {
+                std::memcpy(hs0 + im0.q, q_host, 2 * (size_t)s0.B * s0.Hq * s0.d);
+                release_step(w0, c0->seq);
+                early = true;
+            }
+        }
+    }
     auto plain = [&]() -> pkv_status {       // anything the pipeline cannot do: the synchronous call, after emptying the pipeline
         const pkv_status ds = pkv_decode_host_drain(host_staging, stream);
         if (ds != PKV_OK) return ds;
@@ -1109,11 +1140,13 @@ pkv_status pkv_decode_host_pipelined(const pkv_shape* shape, const pkv_split_pol
         const bool same = !fresh && c->armed_sig == sig && w->expired != c->seq &&
                           std::memcmp(hs + im.seq_lens, seq_lens_host, 4 * (size_t)s.B) == 0 &&
                           table_runs(s, im, hs, block_table_host, seq_lens_host, false, false, tmp, 0, &nrun, &run_bytes) && run_bytes == 0;
-        if (same) {
+        if (same || early) {     // (early: released at the top of the call; the same comparisons, on the raw arguments)
             my_seq = c->seq;
             was_armed = true;
-            std::memcpy(hs + im.q, q_host, q_bytes);
-            release_step(w, my_seq);
+            if (!early) {
+                std::memcpy(hs + im.q, q_host, q_bytes);
+                release_step(w, my_seq);
+            }
             counters = c->armed_counters;
             counters.armed_step = 1;
             c->armed = false;
@@ -1197,6 +1230,10 @@ pkv_status pkv_decode_host_pipelined(const pkv_shape* shape, const pkv_split_pol
             st = issue_step(s, nx, nseq, true, scale, im, hs_mapped, ds, workspace, sms, cs, &c->armed_counters);
             if (st != PKV_OK) return st;
             c->armed = true;
+            c->id_shape = s; c->id_policy = *policy; c->id_k = nx.k; c->id_v = nx.v;
+            c->id_out = next->out_host ? next->out_host : out_host;
+            c->id_ws = workspace; c->id_ds = dev_scratch; c->id_stream = stream; c->id_scale = scale;
+            c->id_scratch_bytes = scratch_bytes; c->id_ws_bytes = workspace_bytes;
             c->armed_sig = step_sig(nkey, s, nx.hdr, nx.k, nx.v, nx.out_dev, workspace, dev_scratch, scale, stream);
         }
     }

@@ -264,11 +264,9 @@ __global__ void __launch_bounds__(kStageThreads) pkv_stage_kernel(const unsigned
             *reinterpret_cast<uint4*>(dst + base + 16 * (size_t)i) = v;
         }
     }
-    __syncthreads();     // every load of the image has returned
-    if (threadIdx.x == 0) {
-        __threadfence_system();
-        words[kPipeStagedWord] = seq;
-    }
+    __syncthreads();     // every load of the image has returned: its value has gone into the store behind it
+    // no fence: `staged` publishes nothing, it only says that the image is no longer being read
+    if (threadIdx.x == 0) words[kPipeStagedWord] = seq;
 }
 
 // Last launch of a pipelined step: resident early (programmatic launch), it waits for everything before
