@@ -1017,12 +1017,14 @@ pkv_status issue_step(const pkv_shape& s, const PipeStep& st, uint32_t seq, bool
     const WorkspaceLayout L = workspace_layout(s, st.rp.S);
     const WsPtrs ws = carve(workspace, L);
     int dl = 0, ml = 0;
+    // the result goes to the device image; the signal kernel takes it to the pinned out_host with the done word
+    // (a kernel that writes host memory itself cannot complete before those writes have drained over the link)
     const pkv_status rs = run_decode(s, st.rp, ds + im.q, st.k, st.v, reinterpret_cast<const int32_t*>(ds + im.block_table),
-                                     reinterpret_cast<const int32_t*>(ds + im.seq_lens), nullptr, st.out_dev, nullptr, scale, nullptr, ws.q, ws,
+                                     reinterpret_cast<const int32_t*>(ds + im.seq_lens), nullptr, ds + im.out, nullptr, scale, nullptr, ws.q, ws,
                                      st.hdr.num_tasks, st.hdr.max_row_splits, st.hdr.total_row_slots, sms, PKV_STAGE_ALL, true,
                                      L.slots_cap, cs, &dl, &ml);
     if (rs != PKV_OK) return rs;
-    e = launch_signal(words, seq, !(st.rp.flags & PKV_FLAG_NO_PDL), cs);
+    e = launch_signal(words, seq, !(st.rp.flags & PKV_FLAG_NO_PDL), ds + im.out, st.out_dev, 2 * (size_t)s.B * s.Hq * s.d, cs);
     if (e != cudaSuccess) return cuda_fail(e, "signal kernel launch");
     fill_counters(s, st, dl, ml, counters);
     return PKV_OK;

@@ -272,9 +272,14 @@ __global__ void __launch_bounds__(kStageThreads) pkv_stage_kernel(const unsigned
 // Last launch of a pipelined step: resident early (programmatic launch), it waits for everything before
 // it in the stream -- the merge's (or the decode's) stores to the pinned out_host included -- and
 // writes the step's number into the image's `done` word, which the host is spinning on.
-__global__ void pkv_signal_kernel(volatile uint32_t* words, uint32_t seq) {
+__global__ void __launch_bounds__(kSignalThreads) pkv_signal_kernel(volatile uint32_t* words, uint32_t seq, const uint4* out_dev, uint4* out_host,
+                                                                    uint32_t out_chunks) {
     pdl_launch_dependents();
     pdl_wait();
+    // the step's result, from device memory to the pinned out_host (out_chunks 16-byte pieces; 0: the
+    // kernels wrote it there themselves)
+    for (uint32_t i = threadIdx.x; i < out_chunks; i += kSignalThreads) out_host[i] = out_dev[i];
+    __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence_system();
         words[kPipeDoneWord] = seq;
@@ -291,8 +296,10 @@ cudaError_t launch_stage(const void* src_mapped, void* dst, const StageSegs& seg
     return cudaGetLastError();
 }
 
-cudaError_t launch_signal(uint32_t* words_mapped, uint32_t seq, bool pdl, cudaStream_t stream) {
-    return launch_pdl(pdl, pkv_signal_kernel, dim3(1), dim3(32), 0, stream, (volatile uint32_t*)words_mapped, seq);
+cudaError_t launch_signal(uint32_t* words_mapped, uint32_t seq, bool pdl, const void* out_dev, void* out_host_mapped, size_t out_bytes,
+                          cudaStream_t stream) {
+    return launch_pdl(pdl, pkv_signal_kernel, dim3(1), dim3(kSignalThreads), 0, stream, (volatile uint32_t*)words_mapped, seq,
+                      static_cast<const uint4*>(out_dev), static_cast<uint4*>(out_host_mapped), (uint32_t)(out_bytes / 16));
 }
 
 cudaError_t launch_builder(const pkv_shape& shape, const Resolved& rp, const int32_t* seq_lens_dev,

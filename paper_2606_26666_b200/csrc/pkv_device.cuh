@@ -851,7 +851,9 @@ constexpr int kPipeDoneWord = 17;     //              step n's result is in out_
 constexpr int kPipeExpiredWord = 18;  //              step n was never released: it ran on stale inputs
 cudaError_t launch_stage(const void* src_mapped, void* dst, const StageSegs& segs, uint32_t* words_mapped, uint32_t seq, bool gate,
                          unsigned long long timeout_ns, cudaStream_t stream);
-cudaError_t launch_signal(uint32_t* words_mapped, uint32_t seq, bool pdl, cudaStream_t stream);
+constexpr int kSignalThreads = 512;
+cudaError_t launch_signal(uint32_t* words_mapped, uint32_t seq, bool pdl, const void* out_dev, void* out_host_mapped, size_t out_bytes,
+                          cudaStream_t stream);
 int decode_tma_stage_bytes(int HG, int D, bool fp8);
 
 }  // namespace pkv
