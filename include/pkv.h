@@ -414,8 +414,9 @@ PKV_API pkv_status pkv_workspace_partials(const pkv_shape* shape, const pkv_spli
  *      dev_scratch) pair -- `host_staging` keeps the shadow; a growing row changes one entry every
  *      page_size steps, so most steps upload no table bytes at all,
  *   3. launches decode (+ merge), and
- *   4. gets out to out_host -- the kernels write it there directly when out_host is pinned,
- *      device-mapped memory (zero copy), else one cudaMemcpyAsync -- and SYNCHRONISES the stream.
+ *   4. gets out to out_host -- when out_host is pinned, device-mapped memory a small kernel chained
+ *      behind the merge stores it there (no copy-engine hop), else one cudaMemcpyAsync -- and
+ *      SYNCHRONISES the stream.
  * host_staging: host memory of pkv_host_scratch_bytes() bytes (pinned recommended), zeroed (or
  * never used with another dev_scratch) before its first use; dev_scratch: device memory of the same
  * size, 256-byte aligned; the pair must be passed together from step to step.  counters_out may be

@@ -924,12 +924,15 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
 
     WsPtrs ws = carve(workspace, L);
     int dl = 0, ml = 0;
-    // Pinned (page-locked, device-mapped) out_host: the kernels write the FP16 result straight
-    // into it -- 8 KiB of posted writes per row -- and the D2H copy disappears from the step.
-    // Pageable out_host: result in dev_scratch, then one cudaMemcpyAsync.
-    void* out_dev = mapped_device_pointer(out_host, 16, (rp.flags & PKV_FLAG_OUT_PINNED) != 0);
-    const bool zero_copy_out = out_dev != nullptr;
-    if (!zero_copy_out) out_dev = ds + im.out;
+    // Pinned (page-locked, device-mapped) out_host: a small kernel behind the merge stores the FP16 result
+    // into it -- 8 KiB of posted writes per row -- and the copy-engine hop disappears from the step.
+    // Pageable out_host: one cudaMemcpyAsync from dev_scratch.
+    void* out_mapped = mapped_device_pointer(out_host, 16, (rp.flags & PKV_FLAG_OUT_PINNED) != 0);
+    const bool zero_copy_out = out_mapped != nullptr;
+    // the kernels write the result into the device image either way: a kernel that stores into host memory
+    // itself cannot complete before those stores have drained over the link (measured on the pipelined step,
+    // DESIGN.md 6.6); a small kernel chained behind them carries it to a pinned out_host
+    void* out_dev = ds + im.out;
     const bool fused = rp.kernel == PKV_KERNEL_TMA_MMA && !(rp.flags & PKV_FLAG_SEPARATE_BUILD) && s.B <= kMaxFusedRows;
     if (!fused && hdr->num_tasks > 0) {
         e = launch_builder(s, rp, lens_dev, nullptr, ws.q.hdr, ws.q.split_offsets, ws.fuse_counters, ws.q.rowslots, ws.q.tasks,
@@ -941,7 +944,8 @@ pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_policy* polic
                     hdr->total_row_slots, sms, PKV_STAGE_ALL, fused, L.slots_cap, cs, &dl, &ml);
     if (st != PKV_OK) return st;
     const size_t out_bytes = 2 * (size_t)s.B * s.Hq * s.d;
-    e = zero_copy_out ? cudaSuccess : cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);
+    e = zero_copy_out ? launch_signal(nullptr, 0, !(rp.flags & PKV_FLAG_NO_PDL), ds + im.out, out_mapped, out_bytes, cs)
+                      : cudaMemcpyAsync(out_host, ds + im.out, out_bytes, cudaMemcpyDeviceToHost, cs);
     if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     if (e != cudaSuccess) return cuda_fail(e, "D2H out / sync");
     if (counters_out) {

@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(kSignalThreads) pkv_signal_kernel(volatile uin
     // kernels wrote it there themselves)
     for (uint32_t i = threadIdx.x; i < out_chunks; i += kSignalThreads) out_host[i] = out_dev[i];
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0 && words != nullptr) {      // (no words: pkv_decode_host, which synchronises the stream instead)
         __threadfence_system();
         words[kPipeDoneWord] = seq;
     }
