@@ -443,8 +443,10 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
  * The gate is one CTA that polls a flag word of the pinned staging buffer over the host link; once the
  * host has released the step it fetches lengths, q and table rows from the image into dev_scratch.
  * Decode, merge and signal are chained behind it by programmatic launch: they are resident and
- * planned when the gate opens.  The signal kernel writes the step's number into a done word of the
- * image.  The next call then only copies q into the image, stores the flag and spins on the done word.
+ * planned when the gate opens.  Decode and merge write the result into dev_scratch; the signal kernel
+ * copies it into the pinned out_host and writes the step's number into a done word of the image.  The
+ * next call then only copies q into the image, stores the flag (before it validates or plans anything,
+ * when it repeats the armed step's arguments byte for byte) and spins on the done word.
  * Results are those of pkv_decode_host, bit for bit (the same kernels on the same inputs).
  *   - Needs: host_staging and out_host pinned and device-mapped, host_staging 256-byte aligned, the TMA
  *     kernel with the fused build (B <= 512), no PKV_FLAG_VALIDATE / SEPARATE_BUILD, at most 64 KiB of
