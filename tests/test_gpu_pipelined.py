@@ -187,3 +187,29 @@ def test_prepared_calls_replay_the_same_step_arguments():
         dec.drain()
     assert armed >= 5
     torch.cuda.synchronize()
+
+
+def test_pipelined_steps_on_fp8_caches():
+    """The pipeline is the host path around the same launches: one-byte caches (per-head scales in the
+    shape) go through it unchanged, bit-identical to the plain call."""
+    from test_gpu_fp8 import Fp8Problem
+    pol = pkv.Policy(tile_tokens=32, num_splits=5, flags=pkv.FLAG_OUT_PINNED)
+    lp = Loop(pol, seed=2500)
+    lp.dp = Fp8Problem(list(lp.lens0 + STEPS + 8), seed=2500)       # the same tables and pool size; E4M3 bytes, scales
+    assert np.array_equal(lp.dp.p.block_table, lp.p.block_table) and lp.dp.shape.kv_dtype == pkv.KV_E4M3
+    want, _ = lp.plain_pass()
+    assert not np.isnan(want[0]).any()
+    staging, scratch, ws = lp.buffers()
+    dec = pkv.PipelinedHostDecoder(lp.dp.shape, pol, lp.dp.k, lp.dp.v, staging, scratch, ws, lp.p.scale, stream=lp.stream)
+    armed = 0
+    try:
+        for t in range(STEPS):
+            lp.out.fill_(float("nan"))
+            dec(lp.q[t % 3].data_ptr(), lp.tables[t].data_ptr(), lp.lens[t].data_ptr(), lp.out.data_ptr(),
+                lp.lens[t + 1].data_ptr(), lp.tables[t + 1].data_ptr())
+            assert np.array_equal(lp.out.numpy().view(np.uint16), want[t].view(np.uint16)), "step %d" % t
+            armed += dec.counters["armed_step"]
+    finally:
+        dec.drain()
+    assert armed >= STEPS - 4
+    torch.cuda.synchronize()
