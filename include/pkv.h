@@ -449,7 +449,7 @@ PKV_API pkv_status pkv_decode_host(const pkv_shape* shape, const pkv_split_polic
  * when it repeats the armed step's arguments byte for byte) and spins on the done word.
  * Results are those of pkv_decode_host, bit for bit (the same kernels on the same inputs).
  *   - Needs: host_staging and out_host pinned and device-mapped, host_staging 256-byte aligned, the TMA
- *     kernel with the fused build (B <= 512), no PKV_FLAG_VALIDATE / SEPARATE_BUILD, at most 64 KiB of
+ *     kernel with the fused build (B <= 512), no PKV_FLAG_VALIDATE / SEPARATE_BUILD, at most 256 KiB of
  *     inputs in at most four pieces per step.  Otherwise -- and whenever the armed step turns out not to
  *     be the one the next call asks for (other lengths, table, buffers, policy) -- the call does what
  *     pkv_decode_host does; a mispredicted armed step is first run on whatever the image holds and its

@@ -256,12 +256,22 @@ __global__ void __launch_bounds__(kStageThreads) pkv_stage_kernel(const unsigned
     for (int k = 0; k < kMaxStageSegs; ++k) {
         if (k >= segs.n) break;
         const size_t base = segs.off[k];
-        for (uint32_t i = threadIdx.x; i < segs.chunks[k]; i += kStageThreads) {
-            uint4 v;
-            asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];"
-                         : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                         : "l"(src + base + 16 * (size_t)i));
-            *reinterpret_cast<uint4*>(dst + base + 16 * (size_t)i) = v;
+        // four loads in flight per thread: 64 KiB cross the host link in one round trip, not four
+        for (uint32_t i0 = threadIdx.x; i0 < segs.chunks[k]; i0 += 4 * kStageThreads) {
+            uint4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = i0 + u * kStageThreads;
+                if (i < segs.chunks[k])
+                    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                 : "=r"(v[u].x), "=r"(v[u].y), "=r"(v[u].z), "=r"(v[u].w)
+                                 : "l"(src + base + 16 * (size_t)i));
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = i0 + u * kStageThreads;
+                if (i < segs.chunks[k]) *reinterpret_cast<uint4*>(dst + base + 16 * (size_t)i) = v[u];
+            }
         }
     }
     __syncthreads();     // every load of the image has returned: its value has gone into the store behind it

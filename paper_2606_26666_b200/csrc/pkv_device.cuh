@@ -838,7 +838,7 @@ cudaError_t launch_merge(const DecodeParams& p, int G, cudaStream_t stream);
 // pkv_decode_host_pipelined (pkv_aux.cu): the gate / stage kernel and the completion signal.
 constexpr int kMaxStageSegs = 4;
 constexpr int kStageThreads = 1024;           // 16 KiB of inputs in one round of 16-byte loads over the host link
-constexpr size_t kMaxStageBytes = 64 << 10;   // beyond this the copy engine is the faster way up
+constexpr size_t kMaxStageBytes = 256 << 10;  // beyond this the copy engine is the faster way up
 struct StageSegs {
     uint32_t off[kMaxStageSegs];      // byte offset in the image, multiple of 16
     uint32_t chunks[kMaxStageSegs];   // 16-byte chunks
