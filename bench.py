@@ -886,6 +886,16 @@ def other_workloads(pkv, torch, args, device, peak, read_peak):
                         "tasks": c["tasks"], "empty_tasks": c["empty_tasks"],
                         "launches_per_step": c["launched_build"] + c["launched_decode"] + c["launched_merge"],
                         "parity": par}
+            if key in ("config3", "config2_fp8") and not args.no_e2e:
+                # the host-buffer step of these workloads too: pipelined and synchronous call, 200 steps each
+                try:
+                    es = run_e2e(pkv, torch, runner, 200, 5, auto=True)
+                    ep = run_e2e_pipelined(pkv, torch, runner, 200, 5, auto=True)
+                    out[key]["e2e"] = {"us_per_step": round(1e6 * ep[0] / 200, 2), "steps_enqueued_a_call_early": ep[2],
+                                       "synchronous_us_per_step": round(1e6 * es[0] / 200, 2),
+                                       "h2d_bytes_per_step": ep[1]["h2d_bytes"], "d2h_bytes_per_step": ep[1]["d2h_bytes"]}
+                except Exception as ex:
+                    out[key]["e2e"] = {"error": "%s: %s" % (type(ex).__name__, str(ex)[:200])}
         except Exception as e:      # an out-of-memory pool must not lose the headline line
             out[key] = {"error": "%s: %s" % (type(e).__name__, str(e)[:200])}
     runner = None
